@@ -1,0 +1,145 @@
+/* lqcd.h -- C ABI of the B200 staggered-fermion hot path (even/odd Dslash + multi-shift CG).
+ *
+ * Source of the operations: arxiv/paper_1801_01473, "Portable multi-node LQCD Monte Carlo simulations
+ * using OpenACC".  The library implements, for ONE GPU (sm_100a), in double precision:
+ *
+ *   D_oe, D_eo   the off-diagonal even/odd blocks of the staggered Dirac matrix (the
+ *                hopping term between x and x+mu is proportional to U_mu(x); D_oe^dagger = -D_eo), with
+ *                the U(1) factors that carry the staggered phases and the antiperiodic time boundary
+ *                 computed in registers:
+ *                  (D psi)(x) = 1/2 sum_mu [ s_mu(x) U_mu(x) psi(x+mu) - s_mu(x-mu) U_mu(x-mu)^+ psi(x-mu) ]
+ *                  s_mu(x) = eta_mu(x) bc_mu(x), eta = (1, (-1)^x, (-1)^(x+y), (-1)^(x+y+z)),
+ *                  bc_t(x) = -1 for x_t = Lt-1 when ANTIPERIODIC_T is on, +1 otherwise;
+ *   Eq. 2        (m^2 - D_eo D_oe + sigma_i) x_i = b, i = 1..r, solved for all shifts at once by the
+ *                shifted ("multimass") conjugate gradient;
+ *   link compression  only the first two rows of each SU(3) link are stored and read; the third is
+ *                recomputed as r2 = conj(r0 x r1)  [option LQCD_OPT_RECON = 12].
+ *
+ * Conventions
+ *   Sites: lex = x + Lx*(y + Ly*(z + Lz*t)); parity = (x+y+z+t)&1, even = 0.  All extents even, >= 2.
+ *   V = Lx*Ly*Lz*Lt, Vh = V/2.  A complex number is two consecutive doubles (re, im).
+ *
+ *   PARITY VECTOR ("vec3_soa") -- the layout of every in/out/b/x argument:
+ *       v[(c*Vh + k)*2 + {0,1}],  c = colour 0..2,  k = lex>>1 of a site of the stated parity.
+ *       3*Vh complex doubles = 48*Vh bytes (3 double complex per even site).
+ *   CANONICAL GAUGE FIELD -- the argument of lqcd_set_gauge:
+ *       links[(((mu*V + lex)*3 + row)*3 + col)*2 + {0,1}],  mu = 0..3 = x,y,z,t;
+ *       U_mu(lex) is the link that leaves site lex in direction +mu.  4*V*18 doubles.
+ *   SITE FIELD (lqcd_pack_vector / lqcd_unpack_vector only): f[((lex*3) + c)*2 + {0,1}], V*3 complex.
+ *
+ * Pointers
+ *   Unless a parameter is marked HOST, every data pointer is a DEVICE pointer, 16-byte aligned, owned by
+ *   the caller; the library reads/writes it on the context's stream and never frees it.  The *_host
+ *   entry points take HOST pointers (pinned memory makes the copies asynchronous and faster) and perform
+ *   the host<->device copies themselves on the context's stream.
+ *   in/out (and b/x[i], x[i]/x[j]) must not alias.
+ *
+ * Execution
+ *   All work is enqueued on the stream set with lqcd_set_stream (default: the legacy default stream).
+ *   lqcd_doe / lqcd_deo / lqcd_mdagm / lqcd_pack_vector / lqcd_unpack_vector return after enqueueing.
+ *   lqcd_set_gauge and lqcd_mshift_cg (and all *_host calls) return after their work has completed.
+ *   A context is not thread-safe; use one per host thread.
+ *
+ * Errors
+ *   Every int-returning call returns LQCD_OK (0) or a negative code; nothing is printed, thrown or
+ *   aborted.  lqcd_last_error(ctx) gives a short text for the last failure on that context
+ *   (lqcd_last_error(NULL): the last failed lqcd_create).
+ */
+#ifndef LQCD_H
+#define LQCD_H
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct lqcd_ctx lqcd_ctx;
+
+/* status codes */
+#define LQCD_OK           0
+#define LQCD_EINVAL      -1   /* NULL pointer, odd or < 2 extent, nshift < 1, shift < 0, tol <= 0, bad key/value */
+#define LQCD_ENOGAUGE    -2   /* operator or solver called before lqcd_set_gauge */
+#define LQCD_ENOMEM      -3   /* device allocation failed or caller workspace too small */
+#define LQCD_ECUDA       -4   /* a CUDA runtime call or kernel failed (text in lqcd_last_error) */
+#define LQCD_ENOCONV     -5   /* MAX_ITER reached; x[] holds the last iterate */
+#define LQCD_EBREAKDOWN  -6   /* <p,Ap> <= 0 or non-finite (cannot happen for SU(3) links) */
+#define LQCD_ENOTSU3     -7   /* RECON=12 and some link has max|r2 - conj(r0 x r1)| > 1e-12 */
+
+/* option keys for lqcd_set_option / lqcd_get_option */
+#define LQCD_OPT_MASS            0  /* m of Eq. 2; default 0                               */
+#define LQCD_OPT_ANTIPERIODIC_T  1  /* 1 (default): antiperiodic in t; 0: periodic         */
+#define LQCD_OPT_RECON           2  /* 18 (default): full links; 12: two-row compression.
+                                       Takes effect at the next lqcd_set_gauge.                           */
+#define LQCD_OPT_MAX_ITER        3  /* iteration cap of lqcd_mshift_cg; default 100000                    */
+#define LQCD_OPT_CHECK_EVERY     4  /* the host looks at the device-side stop flag every this many
+                                       iterations; default 0 = chosen from the lattice size                */
+#define LQCD_OPT_USE_GRAPH       5  /* 1 (default): replay the CG iteration as a CUDA graph; 0: plain launches */
+
+/* statistic keys for lqcd_get_stat (about the last lqcd_mshift_cg on this context) */
+#define LQCD_STAT_ITERS          0  /* number of iterations performed                                     */
+#define LQCD_STAT_REL_RES        1  /* sqrt(|r|^2/|b|^2) of the base recurrence residual at the stop       */
+#define LQCD_STAT_FREEZE_ITER    2  /* idx = shift index: iteration after which x[idx] was no longer updated */
+#define LQCD_STAT_BASE_SHIFT     3  /* index of the shift used as base system (the smallest)              */
+#define LQCD_STAT_GPU_LAUNCHES   4  /* kernels launched by this context since creation                    */
+#define LQCD_STAT_SOLVE_MS       5  /* device time of the last solve between CUDA events, milliseconds     */
+
+/* Create a context for an Lx*Ly*Lz*Lt lattice on the current CUDA device.  NULL on error
+ * (extent odd or < 2, volume too large, no device). */
+lqcd_ctx* lqcd_create(int Lx, int Ly, int Lz, int Lt);
+void      lqcd_destroy(lqcd_ctx* ctx);
+
+/* cuda_stream: a cudaStream_t (e.g. torch.cuda.current_stream().cuda_stream); NULL = default stream. */
+int lqcd_set_stream(lqcd_ctx* ctx, void* cuda_stream);
+int lqcd_set_option(lqcd_ctx* ctx, int key, double value);
+int lqcd_get_option(const lqcd_ctx* ctx, int key, double* value /*HOST*/);
+
+/* Device memory.  By default the library allocates what it needs with cudaMalloc.  Alternatively the
+ * caller provides one arena of at least lqcd_workspace_bytes(ctx, nshift) bytes (256-byte aligned) that
+ * then holds the stored links and all solver temporaries for up to nshift shifts; it must stay valid
+ * until lqcd_destroy or the next lqcd_set_workspace.  Must be called before lqcd_set_gauge. */
+size_t lqcd_workspace_bytes(const lqcd_ctx* ctx, int nshift);
+int    lqcd_set_workspace(lqcd_ctx* ctx, void* dev, size_t bytes);
+
+/* Store the gauge field (step A1): canonical layout above -> per-parity structure of arrays, 18 or 12
+ * reals per link according to LQCD_OPT_RECON.  The input is copied; it may be freed afterwards.
+ * With RECON=12 returns LQCD_ENOTSU3 if some third row differs from conj(r0 x r1) by more than 1e-12. */
+int lqcd_set_gauge(lqcd_ctx* ctx, const double* links);
+int lqcd_set_gauge_host(lqcd_ctx* ctx, const double* links /*HOST*/);
+
+/* out_odd = D_oe in_even;  out_even = D_eo in_odd.  Parity vectors. */
+int lqcd_doe(lqcd_ctx* ctx, double* out_odd, const double* in_even);
+int lqcd_deo(lqcd_ctx* ctx, double* out_even, const double* in_odd);
+int lqcd_doe_host(lqcd_ctx* ctx, double* out_odd /*HOST*/, const double* in_even /*HOST*/);
+int lqcd_deo_host(lqcd_ctx* ctx, double* out_even /*HOST*/, const double* in_odd /*HOST*/);
+
+/* out_even = (m^2 + sigma) in_even - D_eo D_oe in_even: the operator of Eq. 2, the
+ * paper's D_oe, D_eo, zaxpy sequence in two launches. */
+int lqcd_mdagm(lqcd_ctx* ctx, double* out_even, const double* in_even, double sigma);
+
+/* Multi-shift CG for (m^2 - D_eo D_oe + shifts[i]) x[i] = b, i = 0..nshift-1, zero
+ * initial guess, base system = smallest shift, stop when |r| <= tol*|b| for the base system, shift i is
+ * frozen once zeta_i*|r| <= tol*|b| (readings R5-R7).
+ *   b_even : parity vector (even sites);  shifts : HOST array of nshift values >= 0;
+ *   x      : HOST array of nshift DEVICE pointers to parity vectors (overwritten).
+ * Returns LQCD_OK, LQCD_ENOCONV or LQCD_EBREAKDOWN (or an argument / CUDA error). */
+int lqcd_mshift_cg(lqcd_ctx* ctx, const double* b_even, const double* shifts /*HOST*/, int nshift,
+                   double tol, double* const* x /*HOST array of DEVICE pointers*/);
+/* Same, b and every x[i] in HOST memory; copies are part of the call. */
+int lqcd_mshift_cg_host(lqcd_ctx* ctx, const double* b_even /*HOST*/, const double* shifts /*HOST*/,
+                        int nshift, double tol, double* const* x /*HOST array of HOST pointers*/);
+
+/* Statistics of the last solve; *out is HOST. idx is used by LQCD_STAT_FREEZE_ITER only. */
+int lqcd_get_stat(const lqcd_ctx* ctx, int key, int idx, double* out /*HOST*/);
+
+/* Convenience: site field (whole lattice, V*3 complex, array of structs) <-> parity vector.
+ * pack reads only the sites of `parity`; unpack writes only those sites. */
+int lqcd_pack_vector(lqcd_ctx* ctx, int parity, const double* site_field, double* parity_vector);
+int lqcd_unpack_vector(lqcd_ctx* ctx, int parity, const double* parity_vector, double* site_field);
+
+const char* lqcd_last_error(const lqcd_ctx* ctx);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* LQCD_H */

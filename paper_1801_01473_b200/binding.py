@@ -1,0 +1,323 @@
+"""ctypes binding of include/lqcd.h -- same names, argument marshalling only."""
+from __future__ import annotations
+
+import ctypes
+import os
+from typing import Optional, Sequence
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+
+# ---- constants of include/lqcd.h ---------------------------------------------------------------------
+LQCD_OK, LQCD_EINVAL, LQCD_ENOGAUGE, LQCD_ENOMEM, LQCD_ECUDA = 0, -1, -2, -3, -4
+LQCD_ENOCONV, LQCD_EBREAKDOWN, LQCD_ENOTSU3 = -5, -6, -7
+LQCD_OPT_MASS, LQCD_OPT_ANTIPERIODIC_T, LQCD_OPT_RECON, LQCD_OPT_MAX_ITER = 0, 1, 2, 3
+LQCD_OPT_CHECK_EVERY, LQCD_OPT_USE_GRAPH = 4, 5
+LQCD_STAT_ITERS, LQCD_STAT_REL_RES, LQCD_STAT_FREEZE_ITER, LQCD_STAT_BASE_SHIFT = 0, 1, 2, 3
+LQCD_STAT_GPU_LAUNCHES, LQCD_STAT_SOLVE_MS = 4, 5
+
+_ERRNAMES = {0: "LQCD_OK", -1: "LQCD_EINVAL", -2: "LQCD_ENOGAUGE", -3: "LQCD_ENOMEM", -4: "LQCD_ECUDA",
+             -5: "LQCD_ENOCONV", -6: "LQCD_EBREAKDOWN", -7: "LQCD_ENOTSU3"}
+
+_vp, _dp, _sz, _i, _d = ctypes.c_void_p, ctypes.c_void_p, ctypes.c_size_t, ctypes.c_int, ctypes.c_double
+_pd = ctypes.POINTER(ctypes.c_double)
+
+# every symbol include/lqcd.h declares: name -> (restype, argtypes)
+EXPORTS = {
+    "lqcd_create": (_vp, [_i, _i, _i, _i]),
+    "lqcd_destroy": (None, [_vp]),
+    "lqcd_set_stream": (_i, [_vp, _vp]),
+    "lqcd_set_option": (_i, [_vp, _i, _d]),
+    "lqcd_get_option": (_i, [_vp, _i, _pd]),
+    "lqcd_workspace_bytes": (_sz, [_vp, _i]),
+    "lqcd_set_workspace": (_i, [_vp, _vp, _sz]),
+    "lqcd_set_gauge": (_i, [_vp, _dp]),
+    "lqcd_set_gauge_host": (_i, [_vp, _dp]),
+    "lqcd_doe": (_i, [_vp, _dp, _dp]),
+    "lqcd_deo": (_i, [_vp, _dp, _dp]),
+    "lqcd_doe_host": (_i, [_vp, _dp, _dp]),
+    "lqcd_deo_host": (_i, [_vp, _dp, _dp]),
+    "lqcd_mdagm": (_i, [_vp, _dp, _dp, _d]),
+    "lqcd_mshift_cg": (_i, [_vp, _dp, _pd, _i, _d, ctypes.POINTER(ctypes.c_void_p)]),
+    "lqcd_mshift_cg_host": (_i, [_vp, _dp, _pd, _i, _d, ctypes.POINTER(ctypes.c_void_p)]),
+    "lqcd_get_stat": (_i, [_vp, _i, _i, _pd]),
+    "lqcd_pack_vector": (_i, [_vp, _i, _dp, _dp]),
+    "lqcd_unpack_vector": (_i, [_vp, _i, _dp, _dp]),
+    "lqcd_last_error": (ctypes.c_char_p, [_vp]),
+}
+
+_lib = None
+
+
+def library_path() -> str:
+    return os.path.join(HERE, "liblqcd_b200.so")
+
+
+def load_library():
+    """dlopen liblqcd_b200.so (building it with nvcc if it is not there).  Raises if that fails: there is
+    no other implementation to fall back to."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    path = library_path()
+    if not os.path.exists(path):
+        from .build import build
+        build()
+    lib = ctypes.CDLL(path)
+    for name, (res, args) in EXPORTS.items():
+        fn = getattr(lib, name)          # AttributeError if the symbol is missing
+        fn.restype = res
+        fn.argtypes = args
+    _lib = lib
+    return lib
+
+
+class LqcdError(RuntimeError):
+    def __init__(self, code: int, text: str):
+        super().__init__(f"{_ERRNAMES.get(code, code)}: {text}")
+        self.code = code
+
+
+# ---- the C functions under their own names (raw pointers as ints) ------------------------------------
+def lqcd_create(Lx, Ly, Lz, Lt):
+    return load_library().lqcd_create(int(Lx), int(Ly), int(Lz), int(Lt))
+
+
+def lqcd_destroy(ctx):
+    load_library().lqcd_destroy(ctx)
+
+
+def lqcd_set_stream(ctx, cuda_stream):
+    return load_library().lqcd_set_stream(ctx, cuda_stream)
+
+
+def lqcd_set_option(ctx, key, value):
+    return load_library().lqcd_set_option(ctx, int(key), float(value))
+
+
+def lqcd_get_option(ctx, key):
+    out = ctypes.c_double()
+    rc = load_library().lqcd_get_option(ctx, int(key), ctypes.byref(out))
+    return rc, out.value
+
+
+def lqcd_workspace_bytes(ctx, nshift):
+    return load_library().lqcd_workspace_bytes(ctx, int(nshift))
+
+
+def lqcd_set_workspace(ctx, dev, nbytes):
+    return load_library().lqcd_set_workspace(ctx, dev, int(nbytes))
+
+
+def lqcd_set_gauge(ctx, links):
+    return load_library().lqcd_set_gauge(ctx, links)
+
+
+def lqcd_set_gauge_host(ctx, links):
+    return load_library().lqcd_set_gauge_host(ctx, links)
+
+
+def lqcd_doe(ctx, out_odd, in_even):
+    return load_library().lqcd_doe(ctx, out_odd, in_even)
+
+
+def lqcd_deo(ctx, out_even, in_odd):
+    return load_library().lqcd_deo(ctx, out_even, in_odd)
+
+
+def lqcd_doe_host(ctx, out_odd, in_even):
+    return load_library().lqcd_doe_host(ctx, out_odd, in_even)
+
+
+def lqcd_deo_host(ctx, out_even, in_odd):
+    return load_library().lqcd_deo_host(ctx, out_even, in_odd)
+
+
+def lqcd_mdagm(ctx, out_even, in_even, sigma):
+    return load_library().lqcd_mdagm(ctx, out_even, in_even, float(sigma))
+
+
+def _cg_args(shifts, x_ptrs):
+    n = len(shifts)
+    sh = (ctypes.c_double * n)(*[float(s) for s in shifts])
+    xs = (ctypes.c_void_p * n)(*[int(p) for p in x_ptrs])
+    return n, sh, xs
+
+
+def lqcd_mshift_cg(ctx, b_even, shifts: Sequence[float], tol: float, x_ptrs: Sequence[int]):
+    n, sh, xs = _cg_args(shifts, x_ptrs)
+    return load_library().lqcd_mshift_cg(ctx, b_even, sh, n, float(tol), xs)
+
+
+def lqcd_mshift_cg_host(ctx, b_even, shifts: Sequence[float], tol: float, x_ptrs: Sequence[int]):
+    n, sh, xs = _cg_args(shifts, x_ptrs)
+    return load_library().lqcd_mshift_cg_host(ctx, b_even, sh, n, float(tol), xs)
+
+
+def lqcd_get_stat(ctx, key, idx=0):
+    out = ctypes.c_double()
+    rc = load_library().lqcd_get_stat(ctx, int(key), int(idx), ctypes.byref(out))
+    return rc, out.value
+
+
+def lqcd_pack_vector(ctx, parity, site_field, parity_vector):
+    return load_library().lqcd_pack_vector(ctx, int(parity), site_field, parity_vector)
+
+
+def lqcd_unpack_vector(ctx, parity, parity_vector, site_field):
+    return load_library().lqcd_unpack_vector(ctx, int(parity), parity_vector, site_field)
+
+
+def lqcd_last_error(ctx) -> str:
+    s = load_library().lqcd_last_error(ctx)
+    return s.decode() if s else ""
+
+
+# ---- torch-tensor convenience wrapper ------------------------------------------------------------------
+class Lattice:
+    """One lqcd_ctx.  Tensors are float64; device tensors go to the device entry points on torch's
+    current stream, CPU tensors go to the ``*_host`` entry points (the copies happen inside the call)."""
+
+    def __init__(self, L: Sequence[int], mass: float = 0.0, antiperiodic: bool = True, recon: int = 18):
+        import torch
+        if not torch.cuda.is_available():
+            raise RuntimeError("paper_1801_01473_b200 needs a CUDA device (there is no CPU fallback)")
+        self._torch = torch
+        self.L = tuple(int(v) for v in L)
+        self.V = self.L[0] * self.L[1] * self.L[2] * self.L[3]
+        self.Vh = self.V // 2
+        self.ctx = lqcd_create(*self.L)
+        if not self.ctx:
+            raise LqcdError(LQCD_EINVAL, lqcd_last_error(None))
+        self.set_option(LQCD_OPT_MASS, mass)
+        self.set_option(LQCD_OPT_ANTIPERIODIC_T, 1.0 if antiperiodic else 0.0)
+        self.set_option(LQCD_OPT_RECON, recon)
+
+    def close(self):
+        if getattr(self, "ctx", None):
+            lqcd_destroy(self.ctx)
+            self.ctx = None
+
+    def __del__(self):  # pragma: no cover
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    # -- helpers
+    def _check(self, rc: int, allow=()):
+        if rc != LQCD_OK and rc not in allow:
+            raise LqcdError(rc, lqcd_last_error(self.ctx))
+        return rc
+
+    def _sync_stream(self):
+        self._check(lqcd_set_stream(self.ctx, self._torch.cuda.current_stream().cuda_stream))
+
+    def _t(self, t, shape, device_type=None):
+        torch = self._torch
+        assert t.dtype == torch.float64 and t.is_contiguous(), "float64 contiguous tensor expected"
+        assert tuple(t.shape) == tuple(shape), f"shape {tuple(t.shape)} != {tuple(shape)}"
+        if device_type is not None:
+            assert t.device.type == device_type
+        return t.data_ptr()
+
+    def new_vector(self, n: Optional[int] = None):
+        shape = (3, self.Vh, 2) if n is None else (n, 3, self.Vh, 2)
+        return self._torch.empty(shape, dtype=self._torch.float64, device="cuda")
+
+    # -- options / stats
+    def set_option(self, key, value):
+        self._check(lqcd_set_option(self.ctx, key, value))
+
+    def get_option(self, key) -> float:
+        rc, v = lqcd_get_option(self.ctx, key)
+        self._check(rc)
+        return v
+
+    def stat(self, key, idx=0) -> float:
+        rc, v = lqcd_get_stat(self.ctx, key, idx)
+        self._check(rc)
+        return v
+
+    @property
+    def launches(self) -> int:
+        return int(self.stat(LQCD_STAT_GPU_LAUNCHES))
+
+    # -- the path
+    def set_gauge(self, links):
+        """links: (4, V, 3, 3, 2) float64, canonical layout; CUDA or CPU tensor."""
+        p = self._t(links, (4, self.V, 3, 3, 2))
+        self._sync_stream()
+        if links.device.type == "cuda":
+            self._check(lqcd_set_gauge(self.ctx, p))
+        else:
+            self._check(lqcd_set_gauge_host(self.ctx, p))
+
+    def _apply(self, fn_dev, fn_host, v, out):
+        torch = self._torch
+        pin = self._t(v, (3, self.Vh, 2))
+        if out is None:
+            out = torch.empty_like(v)
+        pout = self._t(out, (3, self.Vh, 2), v.device.type)
+        self._sync_stream()
+        self._check((fn_dev if v.device.type == "cuda" else fn_host)(self.ctx, pout, pin))
+        return out
+
+    def doe(self, v_even, out=None):
+        """D_oe: even -> odd parity vector."""
+        return self._apply(lqcd_doe, lqcd_doe_host, v_even, out)
+
+    def deo(self, v_odd, out=None):
+        """D_eo: odd -> even parity vector."""
+        return self._apply(lqcd_deo, lqcd_deo_host, v_odd, out)
+
+    def mdagm(self, v_even, sigma: float = 0.0, out=None):
+        """(m^2 + sigma) v - D_eo D_oe v."""
+        pin = self._t(v_even, (3, self.Vh, 2), "cuda")
+        if out is None:
+            out = self._torch.empty_like(v_even)
+        pout = self._t(out, (3, self.Vh, 2), "cuda")
+        self._sync_stream()
+        self._check(lqcd_mdagm(self.ctx, pout, pin, sigma))
+        return out
+
+    def mshift_cg(self, b_even, shifts: Sequence[float], tol: float, x=None, raise_on_noconv: bool = True):
+        """Solve (m^2 - D_eo D_oe + shifts[i]) x[i] = b.  Returns (x, info); x is (nshift, 3, Vh, 2)."""
+        torch = self._torch
+        n = len(shifts)
+        pb = self._t(b_even, (3, self.Vh, 2))
+        if x is None:
+            x = torch.empty((n, 3, self.Vh, 2), dtype=torch.float64, device=b_even.device,
+                            pin_memory=(b_even.device.type == "cpu"))
+        self._t(x, (n, 3, self.Vh, 2), b_even.device.type)
+        ptrs = [x[i].data_ptr() for i in range(n)]
+        self._sync_stream()
+        fn = lqcd_mshift_cg if b_even.device.type == "cuda" else lqcd_mshift_cg_host
+        rc = fn(self.ctx, pb, shifts, tol, ptrs)
+        self._check(rc, allow=() if raise_on_noconv else (LQCD_ENOCONV,))
+        info = dict(
+            status=rc,
+            iters=int(self.stat(LQCD_STAT_ITERS)),
+            rel_res=self.stat(LQCD_STAT_REL_RES),
+            freeze_iter=[int(self.stat(LQCD_STAT_FREEZE_ITER, i)) for i in range(n)],
+            base_shift=int(self.stat(LQCD_STAT_BASE_SHIFT)),
+            solve_ms=self.stat(LQCD_STAT_SOLVE_MS),
+        )
+        return x, info
+
+    def pack(self, site_field, parity: int, out=None):
+        """(V,3,2) site field -> (3,Vh,2) parity vector of the given parity."""
+        ps = self._t(site_field, (self.V, 3, 2), "cuda")
+        if out is None:
+            out = self.new_vector()
+        self._sync_stream()
+        self._check(lqcd_pack_vector(self.ctx, parity, ps, self._t(out, (3, self.Vh, 2), "cuda")))
+        return out
+
+    def unpack(self, v, parity: int, out=None):
+        """(3,Vh,2) parity vector -> (V,3,2) site field (other parity zero unless `out` is given)."""
+        pv = self._t(v, (3, self.Vh, 2), "cuda")
+        if out is None:
+            out = self._torch.zeros((self.V, 3, 2), dtype=self._torch.float64, device="cuda")
+        self._sync_stream()
+        self._check(lqcd_unpack_vector(self.ctx, parity, pv, self._t(out, (self.V, 3, 2), "cuda")))
+        return out

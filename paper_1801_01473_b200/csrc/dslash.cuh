@@ -1,0 +1,246 @@
+// dslash.cuh -- the even/odd staggered Dirac operator on sm_100a (steps A2-A5 of DESIGN.md).
+//
+//   out(x) = 1/2 sum_mu [ s_mu(x) U_mu(x) in(x+mu) - s_mu(x-mu) U_mu(x-mu)^+ in(x-mu) ]
+//
+// One thread per output site.  All traffic is 128-bit (double2) and unit-stride in the site index k:
+//   links   W[((mu*2 + parity_of_origin)*NE + e)*Vh + k],  e = 3*row+col, NE = 9 (18-real) or 6 (12-real)
+//   vectors v[c*Vh + k]
+// Neighbour indices, staggered phases eta_mu and the antiperiodic sign are computed in registers from
+// k (no tables: they would add 32 B/site); signs are applied by flipping the IEEE sign bit on the
+// integer pipe, so the FP64 pipe only sees the 8 x 9 complex multiply-adds.
+// Links are streamed once (L1 no-allocate, L2 evict-first policy); neighbour vectors are re-used 8 times
+// across sites and are kept in L1/L2 (evict-last policy).
+//
+// EPI = 0 : out = D in
+// EPI = 1 : out = coef*pv - D in, plus the block partial of Re<pv, out> and the CG scalar step
+//           (this is the paper's separate zaxpy kernel, fused into the D_eo epilogue)
+// EPI = 2 : out = coef*pv - D in only
+#ifndef LQCD_DSLASH_CUH
+#define LQCD_DSLASH_CUH
+
+#include "lqcd_internal.cuh"
+#include "reduce.cuh"
+
+#ifndef DS_BLOCK
+#define DS_BLOCK 128
+#endif
+#ifndef DS_MINB
+#define DS_MINB 4
+#endif
+
+__device__ __forceinline__ uint64_t l2_policy_evict_first() {
+    uint64_t p;
+    asm("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(p));
+    return p;
+}
+__device__ __forceinline__ uint64_t l2_policy_evict_last() {
+    uint64_t p;
+    asm("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(p));
+    return p;
+}
+
+// streamed once: bypass L1 allocation, first to leave L2
+__device__ __forceinline__ double2 ld_stream(const double2* p, uint64_t pol) {
+    double2 v;
+    asm("ld.global.nc.L1::no_allocate.L2::cache_hint.v2.f64 {%0, %1}, [%2], %3;"
+        : "=d"(v.x), "=d"(v.y)
+        : "l"(p), "l"(pol));
+    return v;
+}
+// re-used by neighbouring sites: allocate in L1, last to leave L2
+__device__ __forceinline__ double2 ld_reuse(const double2* p, uint64_t pol) {
+    double2 v;
+    asm("ld.global.nc.L1::evict_last.L2::cache_hint.v2.f64 {%0, %1}, [%2], %3;"
+        : "=d"(v.x), "=d"(v.y)
+        : "l"(p), "l"(pol));
+    return v;
+}
+
+// x -> +-x by flipping the sign bit (mask is 0 or 0x80000000); integer pipe, not FP64
+__device__ __forceinline__ double flip(double x, unsigned int mask) {
+    return __hiloint2double(__double2hiint(x) ^ (int)mask, __double2loint(x));
+}
+
+// acc += u * v
+__device__ __forceinline__ void cmad(double& ar, double& ai, const double2 u, const double vr, const double vi) {
+    ar = fma(u.x, vr, ar);
+    ar = fma(-u.y, vi, ar);
+    ai = fma(u.x, vi, ai);
+    ai = fma(u.y, vr, ai);
+}
+// acc += conj(u) * v
+__device__ __forceinline__ void cmad_conj(double& ar, double& ai, const double2 u, const double vr, const double vi) {
+    ar = fma(u.x, vr, ar);
+    ar = fma(u.y, vi, ar);
+    ai = fma(u.x, vi, ai);
+    ai = fma(-u.y, vr, ai);
+}
+
+__device__ __forceinline__ double2 cmul(const double2 a, const double2 b) {
+    return make_double2(a.x * b.x - a.y * b.y, a.x * b.y + a.y * b.x);
+}
+
+// Load one link (9 complex).  12-real storage: rows 0,1 are read, r2 = conj(r0 x r1).
+template <int RECON>
+__device__ __forceinline__ void load_link(const double2* __restrict__ w, const size_t vh, uint64_t pol, double2 (&u)[9]) {
+    constexpr int NE = (RECON == 12) ? 6 : 9;
+#pragma unroll
+    for (int e = 0; e < NE; ++e) u[e] = ld_stream(w + e * vh, pol);
+    if (RECON == 12) {
+        double2 c;
+        c = cmul(u[1], u[5]); { const double2 d = cmul(u[2], u[4]); u[6] = make_double2(c.x - d.x, -(c.y - d.y)); }
+        c = cmul(u[2], u[3]); { const double2 d = cmul(u[0], u[5]); u[7] = make_double2(c.x - d.x, -(c.y - d.y)); }
+        c = cmul(u[0], u[4]); { const double2 d = cmul(u[1], u[3]); u[8] = make_double2(c.x - d.x, -(c.y - d.y)); }
+    }
+}
+
+__device__ __forceinline__ void load_vec(const double2* __restrict__ v, const size_t vh, uint64_t pol, unsigned int mask,
+                                         double (&vr)[3], double (&vi)[3]) {
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+        const double2 t = ld_reuse(v + c * vh, pol);
+        vr[c] = flip(t.x, mask);
+        vi[c] = flip(t.y, mask);
+    }
+}
+
+// acc += sign * U v          (forward hop; the sign is already folded into v)
+template <int RECON>
+__device__ __forceinline__ void hop_fwd(double (&ar)[3], double (&ai)[3], const double2* __restrict__ w,
+                                        const double2* __restrict__ v, const size_t vh, unsigned int mask,
+                                        uint64_t pol_s, uint64_t pol_r) {
+    double2 u[9];
+    double vr[3], vi[3];
+    load_link<RECON>(w, vh, pol_s, u);
+    load_vec(v, vh, pol_r, mask, vr, vi);
+#pragma unroll
+    for (int a = 0; a < 3; ++a)
+#pragma unroll
+        for (int b = 0; b < 3; ++b) cmad(ar[a], ai[a], u[3 * a + b], vr[b], vi[b]);
+}
+
+// acc += sign * U^dagger v   (backward hop; caller passes the mask of -s)
+template <int RECON>
+__device__ __forceinline__ void hop_bwd(double (&ar)[3], double (&ai)[3], const double2* __restrict__ w,
+                                        const double2* __restrict__ v, const size_t vh, unsigned int mask,
+                                        uint64_t pol_s, uint64_t pol_r) {
+    double2 u[9];
+    double vr[3], vi[3];
+    load_link<RECON>(w, vh, pol_s, u);
+    load_vec(v, vh, pol_r, mask, vr, vi);
+#pragma unroll
+    for (int a = 0; a < 3; ++a)
+#pragma unroll
+        for (int b = 0; b < 3; ++b) cmad_conj(ar[a], ai[a], u[3 * b + a], vr[b], vi[b]);
+}
+
+struct DslashArgs {
+    Geom g;
+    const double2* W;        // stored links
+    const double2* in;       // parity 1-par
+    double2* out;            // parity par
+    int par;                 // parity of the output sites
+    const double2* pv;       // EPI >= 1: vector of parity par
+    double coef;             // EPI >= 1: m^2 + sigma
+    double* partials;        // EPI == 1
+    CgState* st;             // EPI == 1, or any EPI with check_stop
+    int check_stop;          // 1: return at once if st->stop (CG already converged)
+};
+
+template <int RECON, int EPI>
+__global__ void __launch_bounds__(DS_BLOCK, DS_MINB) dslash_kernel(const DslashArgs A) {
+    constexpr int NE = (RECON == 12) ? 6 : 9;
+    if (A.check_stop) {
+        if (A.st->stop) {
+            // tell the x/p update kernel of the *following* iterations to do nothing (see cg.cuh)
+            if (EPI == 0 && blockIdx.x == 0 && threadIdx.x == 0) A.st->stop4 = 1;
+            return;
+        }
+    }
+    const Geom& g = A.g;
+    const int kraw = blockIdx.x * DS_BLOCK + threadIdx.x;
+    const bool valid = kraw < g.Vh;
+    const int k = valid ? kraw : g.Vh - 1;
+    const size_t vh = (size_t)g.Vh;
+
+    // step A3: coordinates, neighbours, phases
+    const unsigned int r1 = fastdiv((unsigned)k, g.dxh);
+    const int xh = k - (int)r1 * g.Lxh;
+    const unsigned int r2 = fastdiv(r1, g.dy);
+    const int y = (int)r1 - (int)r2 * g.Ly;
+    const int t = (int)fastdiv(r2, g.dz);
+    const int z = (int)r2 - t * g.Lz;
+    const int q = (y + z + t + A.par) & 1;
+    const int x = 2 * xh + q;
+
+    const int kxf = k + (q ? ((xh == g.Lxh - 1) ? 1 - g.Lxh : 1) : 0);
+    const int kxb = k - (q ? 0 : ((xh == 0) ? 1 - g.Lxh : 1));
+    const int kyf = k + ((y == g.Ly - 1) ? -(g.Ly - 1) * g.sy : g.sy);
+    const int kyb = k + ((y == 0) ? (g.Ly - 1) * g.sy : -g.sy);
+    const int kzf = k + ((z == g.Lz - 1) ? -(g.Lz - 1) * g.sz : g.sz);
+    const int kzb = k + ((z == 0) ? (g.Lz - 1) * g.sz : -g.sz);
+    const int ktf = k + ((t == g.Lt - 1) ? -(g.Lt - 1) * g.st : g.st);
+    const int ktb = k + ((t == 0) ? (g.Lt - 1) * g.st : -g.st);
+
+    const unsigned int SB = 0x80000000u;
+    const unsigned int my = (unsigned)(x & 1) << 31;                    // eta_y = (-1)^x
+    const unsigned int mz = (unsigned)((x + y) & 1) << 31;              // eta_z = (-1)^(x+y)
+    const unsigned int mt = (unsigned)((x + y + z) & 1) << 31;          // eta_t = (-1)^(x+y+z)
+    const unsigned int mtf = mt ^ ((g.antiperiodic && t == g.Lt - 1) ? SB : 0u);   // link (x,t) leaves Lt-1
+    const unsigned int mtb = mt ^ ((g.antiperiodic && t == 0) ? SB : 0u);          // link (x-t,t) leaves Lt-1
+
+    const uint64_t pol_s = l2_policy_evict_first();
+    const uint64_t pol_r = l2_policy_evict_last();
+
+    const double2* __restrict__ Wf = A.W + (size_t)A.par * NE * vh + k;          // links of the output parity
+    const double2* __restrict__ Wb = A.W + (size_t)(1 - A.par) * NE * vh;        // links of the input parity
+    const size_t mu_stride = (size_t)2 * NE * vh;
+    const double2* __restrict__ in = A.in;
+
+    double ar[3] = {0.0, 0.0, 0.0}, ai[3] = {0.0, 0.0, 0.0};
+    hop_fwd<RECON>(ar, ai, Wf + 0 * mu_stride, in + kxf, vh, 0u, pol_s, pol_r);
+    hop_bwd<RECON>(ar, ai, Wb + 0 * mu_stride + kxb, in + kxb, vh, SB, pol_s, pol_r);
+    hop_fwd<RECON>(ar, ai, Wf + 1 * mu_stride, in + kyf, vh, my, pol_s, pol_r);
+    hop_bwd<RECON>(ar, ai, Wb + 1 * mu_stride + kyb, in + kyb, vh, my ^ SB, pol_s, pol_r);
+    hop_fwd<RECON>(ar, ai, Wf + 2 * mu_stride, in + kzf, vh, mz, pol_s, pol_r);
+    hop_bwd<RECON>(ar, ai, Wb + 2 * mu_stride + kzb, in + kzb, vh, mz ^ SB, pol_s, pol_r);
+    hop_fwd<RECON>(ar, ai, Wf + 3 * mu_stride, in + ktf, vh, mtf, pol_s, pol_r);
+    hop_bwd<RECON>(ar, ai, Wb + 3 * mu_stride + ktb, in + ktb, vh, mtb ^ SB, pol_s, pol_r);
+
+    if (EPI == 0) {
+        if (valid) {
+#pragma unroll
+            for (int c = 0; c < 3; ++c) A.out[c * vh + k] = make_double2(0.5 * ar[c], 0.5 * ai[c]);
+        }
+        return;
+    }
+
+    // epilogue: out = coef*pv - D in;  Re<pv, out>.  In the CG the coefficient m^2 + sigma0 comes from
+    // the device state, so that the captured graph does not depend on the shifts of a solve.
+    const double coef = (EPI == 1) ? A.st->c0 : A.coef;
+    double dot = 0.0;
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+        const double2 p = A.pv[c * vh + k];
+        const double2 o = make_double2(fma(-0.5, ar[c], coef * p.x), fma(-0.5, ai[c], coef * p.y));
+        if (valid) {
+            A.out[c * vh + k] = o;
+            dot = fma(p.x, o.x, dot);
+            dot = fma(p.y, o.y, dot);
+        }
+    }
+    if (EPI == 1) {
+        __shared__ double red[32];
+        __shared__ int last_flag;
+        const double bsum = block_sum<DS_BLOCK>(dot, red);
+        if (publish_partial<DS_BLOCK>(bsum, A.partials, &A.st->ticket[1], &last_flag)) {
+            const double pAp = final_sum<DS_BLOCK>(A.partials, gridDim.x, red);
+            if (threadIdx.x == 0) {
+                A.st->ticket[1] = 0;
+                cg_scalars_after_pAp(A.st, pAp);
+            }
+        }
+    }
+}
+
+#endif

@@ -1,0 +1,654 @@
+// lqcd_api.cu -- the C ABI of include/lqcd.h: context, memory, gauge storage, operators, solver driver.
+// Every step of the path runs in the kernels of dslash.cuh / cg.cuh; this file only validates
+// arguments, owns device memory and enqueues launches.  There is no CPU fallback: without a CUDA
+// device lqcd_create fails.
+#include "../../include/lqcd.h"
+
+#include <cuda_runtime.h>
+
+#include <cmath>
+#include <cstdarg>
+#include <cstdint>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <vector>
+
+#include "cg.cuh"
+#include "dslash.cuh"
+#include "lqcd_internal.cuh"
+
+namespace {
+
+thread_local char g_create_error[256] = "";
+
+constexpr size_t ALIGN = 256;
+inline size_t align_up(size_t b) { return (b + ALIGN - 1) / ALIGN * ALIGN; }
+
+}  // namespace
+
+struct lqcd_ctx {
+    int L[4];
+    Geom g;
+    size_t V, Vh;
+    int device, num_sms;
+    cudaStream_t stream;
+
+    // options
+    double mass;
+    int recon_opt, max_iter, check_every, use_graph;
+
+    // memory
+    char* arena;             // caller workspace (not owned) or NULL
+    size_t arena_bytes, arena_used;
+    std::vector<void*> owned;    // cudaMalloc'ed by us
+
+    // stored gauge field
+    double2* W;
+    size_t W_bytes;
+    int recon_stored;        // 0 = no gauge yet, else 18 or 12
+    double* dev_max;
+
+    // operator / solver buffers
+    double2 *r, *p, *s, *t;
+    double2* pextra[LQCD_MAX_SHIFTS];
+    int n_pextra;
+    double* partials;
+    size_t n_partials;
+    CgState* st_dev;
+    CgState* st_host;        // pinned
+    int* flag_host;          // pinned, 2 ints
+    double* max_host;        // pinned
+    cudaEvent_t ev[2], ev_t0, ev_t1;
+    bool basics;
+
+    // CUDA graph of `graph_iters` CG iterations
+    cudaGraphExec_t graph_exec;
+    int graph_iters;
+
+    // host-call staging (device copies of host arguments)
+    double2* stage_b;
+    double2* stage_x[LQCD_MAX_SHIFTS];
+    int n_stage_x;
+    double2* stage_links;
+
+    // statistics
+    int last_iters, last_i0, last_nshift;
+    double last_rel;
+    int last_freeze[LQCD_MAX_SHIFTS];
+    float last_ms;
+    long long launches;
+
+    char err[256];
+};
+
+namespace {
+
+int fail(lqcd_ctx* c, int code, const char* fmt, ...) {
+    if (c) {
+        va_list ap;
+        va_start(ap, fmt);
+        vsnprintf(c->err, sizeof(c->err), fmt, ap);
+        va_end(ap);
+    }
+    return code;
+}
+
+#define CU(expr)                                                                                     \
+    do {                                                                                             \
+        cudaError_t e_ = (expr);                                                                     \
+        if (e_ != cudaSuccess)                                                                       \
+            return fail(c, LQCD_ECUDA, "%s failed: %s (%s:%d)", #expr, cudaGetErrorString(e_), __FILE__, __LINE__); \
+    } while (0)
+
+int dev_alloc(lqcd_ctx* c, void** out, size_t bytes) {
+    bytes = align_up(bytes);
+    if (c->arena) {
+        if (c->arena_used + bytes > c->arena_bytes)
+            return fail(c, LQCD_ENOMEM, "workspace too small: need %zu more bytes", c->arena_used + bytes - c->arena_bytes);
+        *out = c->arena + c->arena_used;
+        c->arena_used += bytes;
+        return LQCD_OK;
+    }
+    void* p = nullptr;
+    cudaError_t e = cudaMalloc(&p, bytes);
+    if (e != cudaSuccess) {
+        cudaGetLastError();
+        return fail(c, LQCD_ENOMEM, "cudaMalloc(%zu) failed: %s", bytes, cudaGetErrorString(e));
+    }
+    c->owned.push_back(p);
+    *out = p;
+    return LQCD_OK;
+}
+
+void dev_free_owned(lqcd_ctx* c, void* p) {
+    for (size_t i = 0; i < c->owned.size(); ++i)
+        if (c->owned[i] == p) {
+            cudaFree(p);
+            c->owned.erase(c->owned.begin() + i);
+            return;
+        }
+}
+
+void drop_graph(lqcd_ctx* c) {
+    if (c->graph_exec) {
+        cudaGraphExecDestroy(c->graph_exec);
+        c->graph_exec = nullptr;
+    }
+    c->graph_iters = 0;
+}
+
+size_t vec_bytes(const lqcd_ctx* c) { return c->Vh * 3 * sizeof(double2); }
+size_t links_bytes(const lqcd_ctx* c, int recon) { return (size_t)8 * (recon == 12 ? 6 : 9) * c->Vh * sizeof(double2); }
+
+int ds_grid(const lqcd_ctx* c) { return (int)((c->Vh + DS_BLOCK - 1) / DS_BLOCK); }
+int cg_grid(const lqcd_ctx* c) {
+    const size_t n = c->Vh * 3;
+    size_t blocks = (n + CG_BLOCK - 1) / CG_BLOCK;
+    const size_t cap = (size_t)c->num_sms * 8;
+    return (int)(blocks < cap ? blocks : cap);
+}
+
+// buffers every operator call needs: the odd temporary, the CG state, pinned mirrors, events
+int ensure_basics(lqcd_ctx* c) {
+    if (c->basics) return LQCD_OK;
+    int rc;
+    if ((rc = dev_alloc(c, (void**)&c->t, vec_bytes(c)))) return rc;
+    if ((rc = dev_alloc(c, (void**)&c->st_dev, sizeof(CgState)))) return rc;
+    c->n_partials = (size_t)(ds_grid(c) > cg_grid(c) ? ds_grid(c) : cg_grid(c));
+    if ((rc = dev_alloc(c, (void**)&c->partials, c->n_partials * sizeof(double)))) return rc;
+    if ((rc = dev_alloc(c, (void**)&c->dev_max, sizeof(double)))) return rc;
+    CU(cudaMemsetAsync(c->st_dev, 0, sizeof(CgState), c->stream));
+    CU(cudaMallocHost((void**)&c->st_host, sizeof(CgState)));
+    CU(cudaMallocHost((void**)&c->flag_host, 2 * sizeof(int)));
+    CU(cudaMallocHost((void**)&c->max_host, sizeof(double)));
+    CU(cudaEventCreateWithFlags(&c->ev[0], cudaEventDisableTiming));
+    CU(cudaEventCreateWithFlags(&c->ev[1], cudaEventDisableTiming));
+    CU(cudaEventCreate(&c->ev_t0));
+    CU(cudaEventCreate(&c->ev_t1));
+    c->basics = true;
+    return LQCD_OK;
+}
+
+int ensure_solver(lqcd_ctx* c, int nshift) {
+    int rc;
+    if ((rc = ensure_basics(c))) return rc;
+    if (!c->r) {
+        if ((rc = dev_alloc(c, (void**)&c->r, vec_bytes(c)))) return rc;
+        if ((rc = dev_alloc(c, (void**)&c->p, vec_bytes(c)))) return rc;
+        if ((rc = dev_alloc(c, (void**)&c->s, vec_bytes(c)))) return rc;
+    }
+    while (c->n_pextra < nshift - 1) {
+        if ((rc = dev_alloc(c, (void**)&c->pextra[c->n_pextra], vec_bytes(c)))) return rc;
+        ++c->n_pextra;
+    }
+    return LQCD_OK;
+}
+
+template <int EPI>
+void launch_dslash_t(lqcd_ctx* c, const DslashArgs& a) {
+    if (c->recon_stored == 12)
+        dslash_kernel<12, EPI><<<ds_grid(c), DS_BLOCK, 0, c->stream>>>(a);
+    else
+        dslash_kernel<18, EPI><<<ds_grid(c), DS_BLOCK, 0, c->stream>>>(a);
+    ++c->launches;
+}
+
+// out(par) = D in, optionally with the epilogue
+void launch_dslash(lqcd_ctx* c, int epi, double2* out, const double2* in, int par, const double2* pv, double coef,
+                   int check_stop) {
+    DslashArgs a;
+    a.g = c->g;
+    a.W = c->W;
+    a.in = in;
+    a.out = out;
+    a.par = par;
+    a.pv = pv;
+    a.coef = coef;
+    a.partials = c->partials;
+    a.st = c->st_dev;
+    a.check_stop = check_stop;
+    if (epi == 0) launch_dslash_t<0>(c, a);
+    else if (epi == 1) launch_dslash_t<1>(c, a);
+    else launch_dslash_t<2>(c, a);
+}
+
+// one CG iteration = K1..K4 (cg.cuh)
+void launch_cg_iteration(lqcd_ctx* c) {
+    const size_t n = c->Vh * 3;
+    launch_dslash(c, 0, c->t, c->p, 1, nullptr, 0.0, 1);
+    launch_dslash(c, 1, c->s, c->t, 0, c->p, 0.0, 1);
+    cg_update_r_kernel<<<cg_grid(c), CG_BLOCK, 0, c->stream>>>(c->r, c->s, c->st_dev, c->partials, n);
+    cg_update_xp_kernel<<<cg_grid(c), CG_BLOCK, 0, c->stream>>>(c->r, c->st_dev, n);
+    c->launches += 2;
+}
+
+int default_check_every(const lqcd_ctx* c) {
+    long v = (long)(4000000 / (long)c->Vh);
+    if (v < 1) v = 1;
+    if (v > 64) v = 64;
+    return (int)v;
+}
+
+int build_graph(lqcd_ctx* c, int iters) {
+    drop_graph(c);
+    cudaGraph_t graph = nullptr;
+    const long long before = c->launches;
+    CU(cudaStreamBeginCapture(c->stream, cudaStreamCaptureModeThreadLocal));
+    for (int i = 0; i < iters; ++i) launch_cg_iteration(c);
+    cudaError_t e = cudaStreamEndCapture(c->stream, &graph);
+    c->launches = before;     // capturing is not launching
+    if (e != cudaSuccess) return fail(c, LQCD_ECUDA, "graph capture failed: %s", cudaGetErrorString(e));
+    e = cudaGraphInstantiate(&c->graph_exec, graph, 0);
+    cudaGraphDestroy(graph);
+    if (e != cudaSuccess) {
+        c->graph_exec = nullptr;
+        return fail(c, LQCD_ECUDA, "graph instantiate failed: %s", cudaGetErrorString(e));
+    }
+    c->graph_iters = iters;
+    return LQCD_OK;
+}
+
+int check_ctx_gauge(lqcd_ctx* c) {
+    if (!c->recon_stored) return fail(c, LQCD_ENOGAUGE, "no gauge field set (call lqcd_set_gauge first)");
+    return LQCD_OK;
+}
+
+int ensure_stage(lqcd_ctx* c, int nx) {
+    int rc;
+    if (!c->stage_b && (rc = dev_alloc(c, (void**)&c->stage_b, vec_bytes(c)))) return rc;
+    while (c->n_stage_x < nx) {
+        if ((rc = dev_alloc(c, (void**)&c->stage_x[c->n_stage_x], vec_bytes(c)))) return rc;
+        ++c->n_stage_x;
+    }
+    return LQCD_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+lqcd_ctx* lqcd_create(int Lx, int Ly, int Lz, int Lt) {
+    const int L[4] = {Lx, Ly, Lz, Lt};
+    for (int i = 0; i < 4; ++i)
+        if (L[i] < 2 || (L[i] & 1)) {
+            snprintf(g_create_error, sizeof(g_create_error), "extent %d = %d must be even and >= 2", i, L[i]);
+            return nullptr;
+        }
+    const double vol = (double)Lx * Ly * Lz * Lt;
+    if (vol / 2 >= 2147483648.0 / 4) {       // k, and k + stride, must stay below 2^31
+        snprintf(g_create_error, sizeof(g_create_error), "volume too large for 32-bit site indices");
+        return nullptr;
+    }
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    cudaDeviceProp prop;
+    if (e == cudaSuccess) e = cudaGetDeviceProperties(&prop, dev);
+    if (e != cudaSuccess) {
+        cudaGetLastError();
+        snprintf(g_create_error, sizeof(g_create_error), "no usable CUDA device: %s", cudaGetErrorString(e));
+        return nullptr;
+    }
+    lqcd_ctx* c = new (std::nothrow) lqcd_ctx();
+    if (!c) {
+        snprintf(g_create_error, sizeof(g_create_error), "out of host memory");
+        return nullptr;
+    }
+    for (int i = 0; i < 4; ++i) c->L[i] = L[i];
+    c->V = (size_t)Lx * Ly * Lz * Lt;
+    c->Vh = c->V / 2;
+    Geom& g = c->g;
+    g.Lxh = Lx / 2;
+    g.Ly = Ly;
+    g.Lz = Lz;
+    g.Lt = Lt;
+    g.Vh = (int)c->Vh;
+    g.sy = g.Lxh;
+    g.sz = g.Lxh * Ly;
+    g.st = g.Lxh * Ly * Lz;
+    g.dxh = make_fastdiv((uint32_t)g.Lxh);
+    g.dy = make_fastdiv((uint32_t)Ly);
+    g.dz = make_fastdiv((uint32_t)Lz);
+    g.antiperiodic = 1;
+    c->device = dev;
+    c->num_sms = prop.multiProcessorCount;
+    c->stream = nullptr;
+    c->mass = 0.0;
+    c->recon_opt = 18;
+    c->max_iter = 100000;
+    c->check_every = 0;
+    c->use_graph = 1;
+    c->err[0] = 0;
+    return c;
+}
+
+void lqcd_destroy(lqcd_ctx* c) {
+    if (!c) return;
+    cudaStreamSynchronize(c->stream);
+    drop_graph(c);
+    for (void* p : c->owned) cudaFree(p);
+    if (c->st_host) cudaFreeHost(c->st_host);
+    if (c->flag_host) cudaFreeHost(c->flag_host);
+    if (c->max_host) cudaFreeHost(c->max_host);
+    if (c->basics) {
+        cudaEventDestroy(c->ev[0]);
+        cudaEventDestroy(c->ev[1]);
+        cudaEventDestroy(c->ev_t0);
+        cudaEventDestroy(c->ev_t1);
+    }
+    cudaGetLastError();
+    delete c;
+}
+
+const char* lqcd_last_error(const lqcd_ctx* c) { return c ? c->err : g_create_error; }
+
+int lqcd_set_stream(lqcd_ctx* c, void* cuda_stream) {
+    if (!c) return LQCD_EINVAL;
+    c->stream = (cudaStream_t)cuda_stream;
+    return LQCD_OK;
+}
+
+int lqcd_set_option(lqcd_ctx* c, int key, double v) {
+    if (!c) return LQCD_EINVAL;
+    switch (key) {
+        case LQCD_OPT_MASS:
+            if (!std::isfinite(v)) return fail(c, LQCD_EINVAL, "mass must be finite");
+            c->mass = v;
+            break;
+        case LQCD_OPT_ANTIPERIODIC_T:
+            if (v != 0.0 && v != 1.0) return fail(c, LQCD_EINVAL, "ANTIPERIODIC_T must be 0 or 1");
+            c->g.antiperiodic = (int)v;
+            drop_graph(c);        // Geom is a kernel argument baked into the graph
+            break;
+        case LQCD_OPT_RECON:
+            if (v != 18.0 && v != 12.0) return fail(c, LQCD_EINVAL, "RECON must be 18 or 12");
+            c->recon_opt = (int)v;
+            break;
+        case LQCD_OPT_MAX_ITER:
+            if (!(v >= 1.0) || v > 2.0e9) return fail(c, LQCD_EINVAL, "MAX_ITER must be in [1, 2e9]");
+            c->max_iter = (int)v;
+            break;
+        case LQCD_OPT_CHECK_EVERY:
+            if (!(v >= 0.0) || v > 1.0e6) return fail(c, LQCD_EINVAL, "CHECK_EVERY must be in [0, 1e6]");
+            c->check_every = (int)v;
+            break;
+        case LQCD_OPT_USE_GRAPH:
+            if (v != 0.0 && v != 1.0) return fail(c, LQCD_EINVAL, "USE_GRAPH must be 0 or 1");
+            c->use_graph = (int)v;
+            break;
+        default:
+            return fail(c, LQCD_EINVAL, "unknown option key %d", key);
+    }
+    return LQCD_OK;
+}
+
+int lqcd_get_option(const lqcd_ctx* c, int key, double* v) {
+    if (!c || !v) return LQCD_EINVAL;
+    switch (key) {
+        case LQCD_OPT_MASS: *v = c->mass; break;
+        case LQCD_OPT_ANTIPERIODIC_T: *v = c->g.antiperiodic; break;
+        case LQCD_OPT_RECON: *v = c->recon_opt; break;
+        case LQCD_OPT_MAX_ITER: *v = c->max_iter; break;
+        case LQCD_OPT_CHECK_EVERY: *v = c->check_every ? c->check_every : default_check_every(c); break;
+        case LQCD_OPT_USE_GRAPH: *v = c->use_graph; break;
+        default: return LQCD_EINVAL;
+    }
+    return LQCD_OK;
+}
+
+size_t lqcd_workspace_bytes(const lqcd_ctx* c, int nshift) {
+    if (!c || nshift < 1 || nshift > LQCD_MAX_SHIFTS) return 0;
+    const size_t vb = align_up(vec_bytes(c));
+    size_t b = align_up(links_bytes(c, 18));
+    b += vb * (size_t)(4 + (nshift - 1));                       // t, r, p, s, extra directions
+    b += align_up(sizeof(CgState)) + align_up(sizeof(double));
+    const size_t np = (size_t)(ds_grid(c) > cg_grid(c) ? ds_grid(c) : cg_grid(c));
+    b += align_up(np * sizeof(double));
+    return b;
+}
+
+int lqcd_set_workspace(lqcd_ctx* c, void* dev, size_t bytes) {
+    if (!c) return LQCD_EINVAL;
+    if (c->recon_stored || c->basics || !c->owned.empty())
+        return fail(c, LQCD_EINVAL, "lqcd_set_workspace must be called before any other device work on the context");
+    if (!dev || ((uintptr_t)dev % ALIGN) != 0) return fail(c, LQCD_EINVAL, "workspace must be a 256-byte aligned device pointer");
+    c->arena = (char*)dev;
+    c->arena_bytes = bytes;
+    c->arena_used = 0;
+    return LQCD_OK;
+}
+
+int lqcd_set_gauge(lqcd_ctx* c, const double* links) {
+    if (!c) return LQCD_EINVAL;
+    if (!links) return fail(c, LQCD_EINVAL, "links is NULL");
+    int rc;
+    if ((rc = ensure_basics(c))) return rc;
+    const int recon = c->recon_opt;
+    const size_t need = links_bytes(c, recon);
+    if (!c->W || c->W_bytes < need) {
+        if (c->W && !c->arena) dev_free_owned(c, c->W);
+        c->W = nullptr;
+        c->recon_stored = 0;
+        const size_t want = c->arena ? links_bytes(c, 18) : need;   // an arena slot is sized for either format
+        if ((rc = dev_alloc(c, (void**)&c->W, want))) return rc;
+        c->W_bytes = align_up(want);
+    }
+    drop_graph(c);
+    c->recon_stored = 0;
+    CU(cudaMemsetAsync(c->dev_max, 0, sizeof(double), c->stream));
+    const size_t nthreads = 8 * c->Vh;
+    const int grid = (int)((nthreads + 255) / 256);
+    if (recon == 12)
+        repack_gauge_kernel<12><<<grid, 256, 0, c->stream>>>(c->g, (const double2*)links, c->W, c->dev_max);
+    else
+        repack_gauge_kernel<18><<<grid, 256, 0, c->stream>>>(c->g, (const double2*)links, c->W, c->dev_max);
+    ++c->launches;
+    CU(cudaGetLastError());
+    CU(cudaMemcpyAsync(c->max_host, c->dev_max, sizeof(double), cudaMemcpyDeviceToHost, c->stream));
+    CU(cudaStreamSynchronize(c->stream));
+    if (recon == 12 && !(*c->max_host <= 1e-12))
+        return fail(c, LQCD_ENOTSU3, "RECON=12 but max|r2 - conj(r0 x r1)| = %.3e > 1e-12", *c->max_host);
+    c->recon_stored = recon;
+    return LQCD_OK;
+}
+
+int lqcd_set_gauge_host(lqcd_ctx* c, const double* links) {
+    if (!c) return LQCD_EINVAL;
+    if (!links) return fail(c, LQCD_EINVAL, "links is NULL");
+    const size_t bytes = (size_t)4 * c->V * 9 * sizeof(double2);
+    void* tmp = nullptr;
+    cudaError_t e = cudaMalloc(&tmp, bytes);
+    if (e != cudaSuccess) {
+        cudaGetLastError();
+        return fail(c, LQCD_ENOMEM, "cudaMalloc(%zu) for the canonical links failed", bytes);
+    }
+    e = cudaMemcpyAsync(tmp, links, bytes, cudaMemcpyHostToDevice, c->stream);
+    int rc = LQCD_OK;
+    if (e != cudaSuccess) rc = fail(c, LQCD_ECUDA, "copy of the links failed: %s", cudaGetErrorString(e));
+    if (!rc) rc = lqcd_set_gauge(c, (const double*)tmp);
+    cudaStreamSynchronize(c->stream);
+    cudaFree(tmp);
+    return rc;
+}
+
+static int apply_d(lqcd_ctx* c, double* out, const double* in, int par) {
+    if (!c) return LQCD_EINVAL;
+    if (!out || !in) return fail(c, LQCD_EINVAL, "NULL vector");
+    if (out == in) return fail(c, LQCD_EINVAL, "in and out must not alias");
+    int rc;
+    if ((rc = check_ctx_gauge(c))) return rc;
+    launch_dslash(c, 0, (double2*)out, (const double2*)in, par, nullptr, 0.0, 0);
+    CU(cudaGetLastError());
+    return LQCD_OK;
+}
+
+int lqcd_doe(lqcd_ctx* c, double* out_odd, const double* in_even) { return apply_d(c, out_odd, in_even, 1); }
+int lqcd_deo(lqcd_ctx* c, double* out_even, const double* in_odd) { return apply_d(c, out_even, in_odd, 0); }
+
+static int apply_d_host(lqcd_ctx* c, double* out, const double* in, int par) {
+    if (!c) return LQCD_EINVAL;
+    if (!out || !in) return fail(c, LQCD_EINVAL, "NULL vector");
+    int rc;
+    if ((rc = check_ctx_gauge(c))) return rc;
+    if ((rc = ensure_stage(c, 1))) return rc;
+    CU(cudaMemcpyAsync(c->stage_b, in, vec_bytes(c), cudaMemcpyHostToDevice, c->stream));
+    if ((rc = apply_d(c, (double*)c->stage_x[0], (const double*)c->stage_b, par))) return rc;
+    CU(cudaMemcpyAsync(out, c->stage_x[0], vec_bytes(c), cudaMemcpyDeviceToHost, c->stream));
+    CU(cudaStreamSynchronize(c->stream));
+    return LQCD_OK;
+}
+
+int lqcd_doe_host(lqcd_ctx* c, double* out_odd, const double* in_even) { return apply_d_host(c, out_odd, in_even, 1); }
+int lqcd_deo_host(lqcd_ctx* c, double* out_even, const double* in_odd) { return apply_d_host(c, out_even, in_odd, 0); }
+
+int lqcd_mdagm(lqcd_ctx* c, double* out_even, const double* in_even, double sigma) {
+    if (!c) return LQCD_EINVAL;
+    if (!out_even || !in_even) return fail(c, LQCD_EINVAL, "NULL vector");
+    if (out_even == in_even) return fail(c, LQCD_EINVAL, "in and out must not alias");
+    int rc;
+    if ((rc = check_ctx_gauge(c))) return rc;
+    launch_dslash(c, 0, c->t, (const double2*)in_even, 1, nullptr, 0.0, 0);
+    launch_dslash(c, 2, (double2*)out_even, c->t, 0, (const double2*)in_even, c->mass * c->mass + sigma, 0);
+    CU(cudaGetLastError());
+    return LQCD_OK;
+}
+
+int lqcd_mshift_cg(lqcd_ctx* c, const double* b_even, const double* shifts, int nshift, double tol, double* const* x) {
+    if (!c) return LQCD_EINVAL;
+    if (!b_even || !shifts || !x) return fail(c, LQCD_EINVAL, "NULL argument");
+    if (nshift < 1 || nshift > LQCD_MAX_SHIFTS) return fail(c, LQCD_EINVAL, "nshift must be in [1, %d]", LQCD_MAX_SHIFTS);
+    if (!(tol > 0.0) || !std::isfinite(tol)) return fail(c, LQCD_EINVAL, "tol must be positive");
+    for (int i = 0; i < nshift; ++i) {
+        if (!(shifts[i] >= 0.0) || !std::isfinite(shifts[i])) return fail(c, LQCD_EINVAL, "shift %d must be >= 0", i);
+        if (!x[i] || (const double*)x[i] == b_even) return fail(c, LQCD_EINVAL, "x[%d] is NULL or aliases b", i);
+        for (int j = 0; j < i; ++j)
+            if (x[j] == x[i]) return fail(c, LQCD_EINVAL, "x[%d] aliases x[%d]", i, j);
+    }
+    int rc;
+    if ((rc = check_ctx_gauge(c))) return rc;
+    if ((rc = ensure_solver(c, nshift))) return rc;
+
+    // base system = smallest shift (R5); ties: the first
+    int i0 = 0;
+    for (int i = 1; i < nshift; ++i)
+        if (shifts[i] < shifts[i0]) i0 = i;
+
+    CgState* h = c->st_host;
+    memset(h, 0, sizeof(CgState));
+    h->nshift = nshift;
+    h->i0 = i0;
+    h->max_iter = c->max_iter;
+    h->c0 = c->mass * c->mass + shifts[i0];
+    int extra = 0;
+    for (int i = 0; i < nshift; ++i) {
+        h->delta[i] = shifts[i] - shifts[i0];
+        h->x[i] = (double2*)x[i];
+        h->p[i] = (i == i0) ? c->p : c->pextra[extra++];
+    }
+    const size_t n = c->Vh * 3;
+    CU(cudaMemcpyAsync(c->st_dev, h, sizeof(CgState), cudaMemcpyHostToDevice, c->stream));
+    CU(cudaEventRecord(c->ev_t0, c->stream));
+    cg_init_kernel<<<cg_grid(c), CG_BLOCK, 0, c->stream>>>((const double2*)b_even, c->r, c->st_dev, c->partials, n, tol);
+    ++c->launches;
+    CU(cudaGetLastError());
+
+    const int ce = c->check_every ? c->check_every : default_check_every(c);
+    // the legacy default stream cannot be captured: plain launches there
+    const bool use_graph = c->use_graph && c->stream != nullptr && c->stream != cudaStreamLegacy;
+    if (use_graph && c->graph_iters != ce) {
+        if ((rc = build_graph(c, ce))) return rc;
+    }
+    c->flag_host[0] = c->flag_host[1] = 0;
+    bool done = false;
+    const long max_batches = (long)c->max_iter / ce + 3;
+    for (long batch = 0; batch < max_batches && !done; ++batch) {
+        if (use_graph) {
+            CU(cudaGraphLaunch(c->graph_exec, c->stream));
+            c->launches += 4LL * ce;
+        } else {
+            for (int i = 0; i < ce; ++i) launch_cg_iteration(c);
+            CU(cudaGetLastError());
+        }
+        const int slot = (int)(batch & 1);
+        CU(cudaMemcpyAsync(&c->flag_host[slot], &c->st_dev->stop, sizeof(int), cudaMemcpyDeviceToHost, c->stream));
+        CU(cudaEventRecord(c->ev[slot], c->stream));
+        if (batch >= 1) {
+            CU(cudaEventSynchronize(c->ev[slot ^ 1]));
+            if (c->flag_host[slot ^ 1]) done = true;
+        }
+    }
+    CU(cudaEventRecord(c->ev_t1, c->stream));
+    CU(cudaMemcpyAsync(h, c->st_dev, sizeof(CgState), cudaMemcpyDeviceToHost, c->stream));
+    CU(cudaStreamSynchronize(c->stream));
+    CU(cudaEventElapsedTime(&c->last_ms, c->ev_t0, c->ev_t1));
+
+    c->last_iters = h->iter;
+    c->last_i0 = i0;
+    c->last_nshift = nshift;
+    c->last_rel = (h->bb > 0.0) ? std::sqrt(h->rr / h->bb) : 0.0;
+    for (int i = 0; i < nshift; ++i) c->last_freeze[i] = h->active[i] ? h->iter : h->freeze_iter[i];
+    if (!h->stop) return fail(c, LQCD_ECUDA, "solver loop ended without the device raising its stop flag");
+    if (h->status == LQCD_EBREAKDOWN) return fail(c, LQCD_EBREAKDOWN, "<p,Ap> = %g at iteration %d", h->pAp, h->iter);
+    if (h->status == LQCD_ENOCONV)
+        return fail(c, LQCD_ENOCONV, "no convergence in %d iterations, |r|/|b| = %.3e", h->iter, c->last_rel);
+    return LQCD_OK;
+}
+
+int lqcd_mshift_cg_host(lqcd_ctx* c, const double* b_even, const double* shifts, int nshift, double tol, double* const* x) {
+    if (!c) return LQCD_EINVAL;
+    if (!b_even || !shifts || !x) return fail(c, LQCD_EINVAL, "NULL argument");
+    if (nshift < 1 || nshift > LQCD_MAX_SHIFTS) return fail(c, LQCD_EINVAL, "nshift must be in [1, %d]", LQCD_MAX_SHIFTS);
+    for (int i = 0; i < nshift; ++i)
+        if (!x[i]) return fail(c, LQCD_EINVAL, "x[%d] is NULL", i);
+    int rc;
+    if ((rc = check_ctx_gauge(c))) return rc;
+    if ((rc = ensure_stage(c, nshift))) return rc;
+    CU(cudaMemcpyAsync(c->stage_b, b_even, vec_bytes(c), cudaMemcpyHostToDevice, c->stream));
+    double* xd[LQCD_MAX_SHIFTS];
+    for (int i = 0; i < nshift; ++i) xd[i] = (double*)c->stage_x[i];
+    const int status = lqcd_mshift_cg(c, (const double*)c->stage_b, shifts, nshift, tol, xd);
+    if (status != LQCD_OK && status != LQCD_ENOCONV) return status;
+    for (int i = 0; i < nshift; ++i)
+        CU(cudaMemcpyAsync(x[i], c->stage_x[i], vec_bytes(c), cudaMemcpyDeviceToHost, c->stream));
+    CU(cudaStreamSynchronize(c->stream));
+    return status;
+}
+
+int lqcd_get_stat(const lqcd_ctx* c, int key, int idx, double* out) {
+    if (!c || !out) return LQCD_EINVAL;
+    switch (key) {
+        case LQCD_STAT_ITERS: *out = c->last_iters; break;
+        case LQCD_STAT_REL_RES: *out = c->last_rel; break;
+        case LQCD_STAT_FREEZE_ITER:
+            if (idx < 0 || idx >= c->last_nshift) return LQCD_EINVAL;
+            *out = c->last_freeze[idx];
+            break;
+        case LQCD_STAT_BASE_SHIFT: *out = c->last_i0; break;
+        case LQCD_STAT_GPU_LAUNCHES: *out = (double)c->launches; break;
+        case LQCD_STAT_SOLVE_MS: *out = c->last_ms; break;
+        default: return LQCD_EINVAL;
+    }
+    return LQCD_OK;
+}
+
+int lqcd_pack_vector(lqcd_ctx* c, int parity, const double* site_field, double* parity_vector) {
+    if (!c) return LQCD_EINVAL;
+    if (!site_field || !parity_vector || (parity != 0 && parity != 1)) return fail(c, LQCD_EINVAL, "bad argument");
+    pack_vector_kernel<<<(int)((c->Vh + 255) / 256), 256, 0, c->stream>>>(c->g, parity, (const double2*)site_field,
+                                                                         (double2*)parity_vector);
+    ++c->launches;
+    CU(cudaGetLastError());
+    return LQCD_OK;
+}
+
+int lqcd_unpack_vector(lqcd_ctx* c, int parity, const double* parity_vector, double* site_field) {
+    if (!c) return LQCD_EINVAL;
+    if (!site_field || !parity_vector || (parity != 0 && parity != 1)) return fail(c, LQCD_EINVAL, "bad argument");
+    unpack_vector_kernel<<<(int)((c->Vh + 255) / 256), 256, 0, c->stream>>>(c->g, parity, (const double2*)parity_vector,
+                                                                           (double2*)site_field);
+    ++c->launches;
+    CU(cudaGetLastError());
+    return LQCD_OK;
+}
+
+}  // extern "C"

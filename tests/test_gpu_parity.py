@@ -1,0 +1,332 @@
+"""GPU parity: the CUDA library (through its C ABI) against the CPU oracle on the same seeded inputs.
+
+Tolerances (BASELINE.json north_star; derivation in DESIGN.md "Tolerances"):
+  * one Dslash application: relative L2 <= 1e-12 (expected ~1e-16: 8x9 complex FMAs per output);
+  * CG solutions: relative L2 <= 1e-8 per shift, iteration count within +-1 of the oracle's.
+"""
+import numpy as np
+import pytest
+import torch
+
+import lqcd_inputs as gen
+import oracle
+from helpers import make_inputs, oracle_parity_vector, rel_l2, soa_gpu_to_aos
+
+pytestmark = pytest.mark.gpu
+
+TOL_D = 1e-12
+TOL_CG = 1e-8
+
+
+@pytest.fixture(scope="module")
+def lq():
+    import paper_1801_01473_b200 as lq
+    lq.load_library()
+    return lq
+
+
+def cuda(a):
+    return torch.as_tensor(np.ascontiguousarray(a)).cuda()
+
+
+DSLASH_LATTICES = [(4, 4, 4, 4), (4, 6, 8, 10), (2, 2, 2, 2), (2, 4, 2, 6), (6, 2, 4, 2), (8, 8, 8, 6),
+                   (10, 6, 4, 14), (16, 16, 16, 16), (24, 12, 8, 6)]
+
+
+def test_pack_unpack_match_oracle_layout(lq):
+    L = (4, 6, 8, 10)
+    _, f = make_inputs(L)
+    lat = lq.Lattice(L)
+    fg = f.cuda()
+    for p in (0, 1):
+        soa, aos = oracle_parity_vector(L, f.numpy(), p)
+        v = lat.pack(fg, p)
+        assert np.array_equal(v.cpu().numpy(), soa)
+        back = lat.unpack(v, p).cpu().numpy()
+        assert np.array_equal(back, oracle.scatter(L, p, aos))
+    lat.close()
+
+
+@pytest.mark.parametrize("L", DSLASH_LATTICES)
+@pytest.mark.parametrize("recon", [18, 12])
+@pytest.mark.parametrize("antiperiodic", [True, False])
+def test_dslash_doe_then_deo(lq, L, recon, antiperiodic):
+    """BASELINE config 1 (4^4) and the asymmetric / ragged / L=2 cases: t = D_oe b, u = D_eo t."""
+    U, f = make_inputs(L)
+    b_soa, b_aos = oracle_parity_vector(L, f.numpy(), 0)
+    t_ref = oracle.doe(L, U.numpy(), b_aos, antiperiodic)
+    u_ref = oracle.deo(L, U.numpy(), t_ref, antiperiodic)
+
+    lat = lq.Lattice(L, antiperiodic=antiperiodic, recon=recon)
+    lat.set_gauge(U.cuda())
+    b = cuda(b_soa)
+    t = lat.doe(b)
+    u = lat.deo(t)
+    torch.cuda.synchronize()
+    assert rel_l2(soa_gpu_to_aos(t), t_ref) <= TOL_D
+    assert rel_l2(soa_gpu_to_aos(u), u_ref) <= TOL_D
+    # D_eo alone on an independent odd vector
+    o_soa, o_aos = oracle_parity_vector(L, f.numpy(), 1)
+    w = lat.deo(cuda(o_soa))
+    assert rel_l2(soa_gpu_to_aos(w), oracle.deo(L, U.numpy(), o_aos, antiperiodic)) <= TOL_D
+    # Eq. 2 operator in two launches
+    lat.set_option(lq.LQCD_OPT_MASS, 0.37)
+    a = lat.mdagm(b, 0.11)
+    assert rel_l2(soa_gpu_to_aos(a), oracle.mdagm(L, U.numpy(), 0.37, 0.11, b_aos, antiperiodic)) <= TOL_D
+    lat.close()
+
+
+def test_dslash_host_entry_points(lq):
+    L = (4, 6, 8, 10)
+    U, f = make_inputs(L)
+    b_soa, b_aos = oracle_parity_vector(L, f.numpy(), 0)
+    lat = lq.Lattice(L)
+    lat.set_gauge(U)                                   # CPU tensor -> lqcd_set_gauge_host
+    b = torch.as_tensor(b_soa).pin_memory()
+    t = lat.doe(b)                                     # CPU tensors -> lqcd_doe_host
+    assert t.device.type == "cpu"
+    t_ref = oracle.doe(L, U.numpy(), b_aos)
+    assert rel_l2(oracle.soa_to_aos(t.numpy()), t_ref) <= TOL_D
+    u = lat.deo(t)
+    assert rel_l2(oracle.soa_to_aos(u.numpy()), oracle.deo(L, U.numpy(), t_ref)) <= TOL_D
+    lat.close()
+
+
+def run_cg_both(lq, L, mass, shifts, tol, recon=18, use_graph=True, stream=None, max_iter=None, host=False,
+                check_every=None):
+    U, f = make_inputs(L)
+    b_soa, b_aos = oracle_parity_vector(L, f.numpy(), 0)
+    kw = {} if max_iter is None else dict(max_iter=max_iter)
+    x_ref, info_ref = oracle.mshift_cg(L, U.numpy(), mass, b_aos, shifts, tol, **kw)
+    lat = lq.Lattice(L, mass=mass, recon=recon)
+    lat.set_option(lq.LQCD_OPT_USE_GRAPH, 1 if use_graph else 0)
+    if max_iter is not None:
+        lat.set_option(lq.LQCD_OPT_MAX_ITER, max_iter)
+    if check_every is not None:
+        lat.set_option(lq.LQCD_OPT_CHECK_EVERY, check_every)
+
+    def go():
+        lat.set_gauge(U.cuda())
+        b = torch.as_tensor(b_soa).pin_memory() if host else cuda(b_soa)
+        return lat.mshift_cg(b, shifts, tol, raise_on_noconv=False)
+
+    if stream is not None:
+        with torch.cuda.stream(stream):
+            x, info = go()
+        stream.synchronize()
+    else:
+        x, info = go()
+    torch.cuda.synchronize()
+    launches = lat.launches
+    lat.close()
+    return x, info, x_ref, info_ref, launches
+
+
+def check_cg(x, info, x_ref, info_ref, shifts, exact_iters=False):
+    if exact_iters:
+        assert info["iters"] == info_ref["iters"]
+    else:
+        assert abs(info["iters"] - info_ref["iters"]) <= 1, (info["iters"], info_ref["iters"])
+    for i in range(len(shifts)):
+        err = rel_l2(soa_gpu_to_aos(x[i]), x_ref[i])
+        assert err <= TOL_CG, (i, shifts[i], err)
+        assert abs(info["freeze_iter"][i] - info_ref["freeze_iter"][i]) <= 2, (i, info["freeze_iter"], info_ref["freeze_iter"])
+
+
+@pytest.mark.parametrize("L,mass,shifts", [
+    ((4, 4, 4, 4), 0.01, [1e-4 * 10 ** (i / 2) for i in range(8)]),
+    ((2, 2, 2, 2), 0.05, [0.3, 0.0, 2.0, 1e-3]),
+    ((4, 6, 8, 10), 0.02, [1e-2, 1e-3, 1e-1, 1.0, 0.5]),
+    ((8, 8, 8, 8), 0.01, [1e-4 * 10 ** (i / 2) for i in range(8)]),
+])
+@pytest.mark.parametrize("mode", ["graph", "plain", "legacy_stream", "recon12", "host"])
+def test_mshift_cg_small(lq, L, mass, shifts, mode):
+    s = None if mode == "legacy_stream" else torch.cuda.Stream()
+    x, info, x_ref, info_ref, launches = run_cg_both(
+        lq, L, mass, shifts, 1e-10, recon=12 if mode == "recon12" else 18, use_graph=(mode != "plain"),
+        stream=s, host=(mode == "host"))
+    assert info["status"] == 0 and info_ref["status"] == 0
+    assert info["rel_res"] <= 1e-10
+    assert info["base_shift"] == int(np.argmin(shifts))
+    check_cg(x, info, x_ref, info_ref, shifts)
+    assert launches >= 4 * info["iters"] + 2
+
+
+def test_mshift_cg_config2_16x4(lq):
+    """BASELINE config 2: 16^4, m = 0.01, 8 shifts 1e-4*10^(i/2), tol 1e-10 -- full solve on both sides."""
+    cfg = gen.CONFIGS["config2_16^4"]
+    x, info, x_ref, info_ref, _ = run_cg_both(lq, cfg["L"], cfg["mass"], cfg["shifts"], cfg["tol"],
+                                              stream=torch.cuda.Stream())
+    assert info["status"] == 0 and info_ref["status"] == 0
+    check_cg(x, info, x_ref, info_ref, cfg["shifts"])
+    # true residual of every GPU solution, computed by the oracle operator (one application per shift)
+    L = cfg["L"]
+    U, f = make_inputs(L)
+    _, b_aos = oracle_parity_vector(L, f.numpy(), 0)
+    bn = np.linalg.norm(b_aos)
+    for i, sigma in enumerate(cfg["shifts"]):
+        xi = soa_gpu_to_aos(x[i])
+        res = b_aos - oracle.mdagm(L, U.numpy(), cfg["mass"], sigma, xi)
+        assert np.linalg.norm(res) / bn <= 3 * cfg["tol"], (i, np.linalg.norm(res) / bn)
+
+
+def test_mshift_cg_fixed_iteration_count(lq):
+    """The protocol used at the large configs (R9): both sides run exactly n iterations."""
+    L, mass = (8, 8, 8, 8), 0.0075
+    shifts = gen.shifts_geometric(1e-5, 1.0, 16)
+    x, info, x_ref, info_ref, _ = run_cg_both(lq, L, mass, shifts, 1e-30, max_iter=40, stream=torch.cuda.Stream())
+    assert info["status"] == lq.LQCD_ENOCONV and info_ref["status"] == 1
+    assert info["iters"] == 40 == info_ref["iters"]
+    for i in range(16):
+        assert rel_l2(soa_gpu_to_aos(x[i]), x_ref[i]) <= 1e-11
+    assert abs(info["rel_res"] - info_ref["rel_res"]) <= 1e-9 * info_ref["rel_res"]
+
+
+@pytest.mark.parametrize("check_every", [1, 3, 64])
+def test_mshift_cg_check_every_does_not_change_the_result(lq, check_every):
+    L, mass, shifts = (4, 4, 4, 4), 0.05, [1e-3, 1e-1]
+    x, info, x_ref, info_ref, _ = run_cg_both(lq, L, mass, shifts, 1e-10, stream=torch.cuda.Stream(),
+                                              check_every=check_every)
+    check_cg(x, info, x_ref, info_ref, shifts)
+
+
+def test_mshift_cg_is_bit_reproducible(lq):
+    L, mass, shifts = (8, 8, 8, 8), 0.02, [1e-3, 1e-2, 1e-1]
+    U, f = make_inputs(L)
+    b_soa, _ = oracle_parity_vector(L, f.numpy(), 0)
+    lat = lq.Lattice(L, mass=mass)
+    lat.set_gauge(U.cuda())
+    b = cuda(b_soa)
+    with torch.cuda.stream(torch.cuda.Stream()):
+        x1, i1 = lat.mshift_cg(b, shifts, 1e-10)
+        x2, i2 = lat.mshift_cg(b, shifts, 1e-10)
+    torch.cuda.synchronize()
+    assert i1["iters"] == i2["iters"] and i1["freeze_iter"] == i2["freeze_iter"]
+    assert torch.equal(x1, x2)
+    lat.close()
+
+
+def test_edge_cases_and_errors(lq):
+    L = (4, 4, 4, 4)
+    U, f = make_inputs(L)
+    b_soa, b_aos = oracle_parity_vector(L, f.numpy(), 0)
+    # bad extents
+    assert not lq.lqcd_create(3, 4, 4, 4) and "even" in lq.lqcd_last_error(None)
+    assert not lq.lqcd_create(4, 4, 0, 4)
+    lat = lq.Lattice(L, mass=0.1)
+    b = cuda(b_soa)
+    out = torch.empty_like(b)
+    # no gauge yet
+    assert lq.lqcd_doe(lat.ctx, out.data_ptr(), b.data_ptr()) == lq.LQCD_ENOGAUGE
+    assert lq.lqcd_mshift_cg(lat.ctx, b.data_ptr(), [0.1], 1e-8, [out.data_ptr()]) == lq.LQCD_ENOGAUGE
+    lat.set_gauge(U.cuda())
+    # argument errors
+    assert lq.lqcd_doe(lat.ctx, b.data_ptr(), b.data_ptr()) == lq.LQCD_EINVAL
+    assert lq.lqcd_doe(lat.ctx, None, b.data_ptr()) == lq.LQCD_EINVAL
+    assert lq.lqcd_mshift_cg(lat.ctx, b.data_ptr(), [-0.1], 1e-8, [out.data_ptr()]) == lq.LQCD_EINVAL
+    assert lq.lqcd_mshift_cg(lat.ctx, b.data_ptr(), [0.1], 0.0, [out.data_ptr()]) == lq.LQCD_EINVAL
+    assert lq.lqcd_mshift_cg(lat.ctx, b.data_ptr(), [0.1, 0.2], 1e-8, [out.data_ptr(), out.data_ptr()]) == lq.LQCD_EINVAL
+    assert lq.lqcd_set_option(lat.ctx, lq.LQCD_OPT_RECON, 10) == lq.LQCD_EINVAL
+    assert lq.lqcd_set_option(lat.ctx, 99, 1) == lq.LQCD_EINVAL
+    # zero source -> zero solutions, zero iterations
+    x, info = lat.mshift_cg(torch.zeros_like(b), [0.0, 1.0], 1e-10)
+    assert info["iters"] == 0 and info["status"] == 0 and not x.any()
+    # single shift, and the iteration cap
+    x, info = lat.mshift_cg(b, [0.25], 1e-12)
+    xr, ir = oracle.mshift_cg(L, U.numpy(), 0.1, b_aos, [0.25], 1e-12)
+    assert abs(info["iters"] - ir["iters"]) <= 1 and rel_l2(soa_gpu_to_aos(x[0]), xr[0]) <= TOL_CG
+    lat.set_option(lq.LQCD_OPT_MAX_ITER, 3)
+    x, info = lat.mshift_cg(b, [0.0], 1e-12, raise_on_noconv=False)
+    assert info["status"] == lq.LQCD_ENOCONV and info["iters"] == 3
+    xr, ir = oracle.mshift_cg(L, U.numpy(), 0.1, b_aos, [0.0], 1e-12, max_iter=3)
+    assert rel_l2(soa_gpu_to_aos(x[0]), xr[0]) <= 1e-12
+    # links that are not SU(3) are refused in 12-real mode, accepted in 18-real mode
+    bad = U.clone()
+    bad[2, 17, 2, 1, 0] += 1e-6
+    lat.set_option(lq.LQCD_OPT_RECON, 12)
+    assert lq.lqcd_set_gauge(lat.ctx, bad.cuda().data_ptr()) == lq.LQCD_ENOTSU3
+    assert lq.lqcd_doe(lat.ctx, out.data_ptr(), b.data_ptr()) == lq.LQCD_ENOGAUGE      # nothing stored after a refusal
+    lat.set_option(lq.LQCD_OPT_RECON, 18)
+    lat.set_gauge(bad.cuda())
+    t = lat.doe(b)
+    assert rel_l2(soa_gpu_to_aos(t), oracle.doe(L, bad.numpy(), b_aos)) <= TOL_D
+    lat.close()
+
+
+def test_caller_workspace(lq):
+    L, mass, shifts = (4, 6, 8, 10), 0.05, [1e-2, 1e-1, 1.0]
+    U, f = make_inputs(L)
+    b_soa, b_aos = oracle_parity_vector(L, f.numpy(), 0)
+    lat = lq.Lattice(L, mass=mass)
+    need = lq.lqcd_workspace_bytes(lat.ctx, len(shifts))
+    assert need > 4 * lat.V * 144
+    small = torch.empty(need // 2, dtype=torch.uint8, device="cuda")
+    assert lq.lqcd_set_workspace(lat.ctx, small.data_ptr(), small.numel()) == 0
+    assert lq.lqcd_set_gauge(lat.ctx, U.cuda().data_ptr()) == lq.LQCD_ENOMEM
+    lat.close()
+    lat = lq.Lattice(L, mass=mass)
+    ws = torch.empty(need, dtype=torch.uint8, device="cuda")
+    assert lq.lqcd_set_workspace(lat.ctx, ws.data_ptr(), ws.numel()) == 0
+    lat.set_gauge(U.cuda())
+    x, info = lat.mshift_cg(cuda(b_soa), shifts, 1e-10)
+    xr, ir = oracle.mshift_cg(L, U.numpy(), mass, b_aos, shifts, 1e-10)
+    check_cg(x, info, xr, ir, shifts)
+    lat.close()
+
+
+# ---- full BASELINE sizes, in the launch configuration bench.py times ---------------------------------
+@pytest.mark.parametrize("L", [(32, 32, 32, 32), (48, 48, 48, 48)])
+@pytest.mark.parametrize("recon", [18, 12])
+def test_dslash_full_size(lq, L, recon):
+    """Configs 3 and 4: the whole output field of D_oe then D_eo against the oracle (inputs drawn on the GPU,
+    the same bytes copied to the host for the oracle)."""
+    U, f = make_inputs(L, device="cuda")
+    lat = lq.Lattice(L, recon=recon)
+    lat.set_gauge(U)
+    b = lat.pack(f, 0)
+    t = lat.doe(b)
+    u = lat.deo(t)
+    torch.cuda.synchronize()
+    Uh = U.cpu().numpy()
+    del U
+    b_aos = soa_gpu_to_aos(b)
+    t_ref = oracle.doe(L, Uh, b_aos)
+    assert rel_l2(soa_gpu_to_aos(t), t_ref) <= TOL_D
+    u_ref = oracle.deo(L, Uh, t_ref)
+    assert rel_l2(soa_gpu_to_aos(u), u_ref) <= TOL_D
+    lat.close()
+
+
+def test_mshift_cg_config4_fixed_count(lq):
+    """Config 4 (48^4, 16 shifts, m = 0.0075): 12 iterations on both sides, every x_i compared; then the
+    GPU's own full solve is checked through oracle-computed true residuals of sampled shifts."""
+    cfg = gen.CONFIGS["config4_48^4"]
+    L, mass, shifts = cfg["L"], cfg["mass"], cfg["shifts"]
+    U, f = make_inputs(L, device="cuda")
+    lat = lq.Lattice(L, mass=mass)
+    lat.set_gauge(U)
+    b = lat.pack(f, 0)
+    Uh = U.cpu().numpy()
+    del U
+    b_aos = soa_gpu_to_aos(b)
+    n_it = 12
+    lat.set_option(lq.LQCD_OPT_MAX_ITER, n_it)
+    with torch.cuda.stream(torch.cuda.Stream()):
+        x, info = lat.mshift_cg(b, shifts, 1e-30, raise_on_noconv=False)
+    torch.cuda.synchronize()
+    x_ref, info_ref = oracle.mshift_cg(L, Uh, mass, b_aos, shifts, 1e-30, max_iter=n_it)
+    assert info["iters"] == n_it == info_ref["iters"]
+    for i in range(len(shifts)):
+        assert rel_l2(soa_gpu_to_aos(x[i]), x_ref[i]) <= 1e-11, i
+    del x_ref
+    # full solve on the GPU; true residual of three shifts via the oracle operator
+    lat.set_option(lq.LQCD_OPT_MAX_ITER, 100000)
+    with torch.cuda.stream(torch.cuda.Stream()):
+        x, info = lat.mshift_cg(b, shifts, cfg["tol"])
+    torch.cuda.synchronize()
+    assert info["status"] == 0
+    bn = np.linalg.norm(b_aos)
+    for i in (0, 7, 15):
+        res = b_aos - oracle.mdagm(L, Uh, mass, shifts[i], soa_gpu_to_aos(x[i]))
+        assert np.linalg.norm(res) / bn <= 3 * cfg["tol"], (i, np.linalg.norm(res) / bn)
+    lat.close()
