@@ -39,7 +39,7 @@ def lib():
         L.oracle_restrict.argtypes = [_ip, ctypes.c_int, _dp, _dp]
         L.oracle_scatter.argtypes = [_ip, ctypes.c_int, _dp, _dp]
         L.oracle_mshift_cg.argtypes = [_ip, _dp, ctypes.c_double, ctypes.c_int, _dp, _dp, ctypes.c_int,
-                                       ctypes.c_double, ctypes.c_int, _dp, _ip, _ip, _dp]
+                                       ctypes.c_double, ctypes.c_int, ctypes.c_int, _dp, _ip, _ip, _dp]
         L.oracle_mshift_cg.restype = ctypes.c_int
     return _lib
 
@@ -136,9 +136,11 @@ def scatter(L, parity: int, f, full=None) -> np.ndarray:
 
 
 def mshift_cg(L, U, mass: float, b_even, shifts, tol: float, max_iter: int = 100000,
-              antiperiodic: bool = True):
+              antiperiodic: bool = True, sum_order: int = 0):
     """Multi-shift CG for (m^2 - D_eo D_oe + sigma_i) x_i = b.
 
+    sum_order 0 (default) adds the per-slice partials of each scalar product in increasing t, 1 in
+    decreasing t: the same algorithm under a rounding-level perturbation (R9).
     Returns (x, info): x is (nshift, Vh, 3, 2); info = dict(status, iters, freeze_iter, rel_res)."""
     U, b_even = _c(U), _c(b_even)
     sh = _c(np.asarray(shifts, dtype=np.float64))
@@ -148,6 +150,6 @@ def mshift_cg(L, U, mass: float, b_even, shifts, tol: float, max_iter: int = 100
     freeze = (ctypes.c_int * n)()
     rel = ctypes.c_double(0.0)
     status = lib().oracle_mshift_cg(_L(L), _p(U), float(mass), int(antiperiodic), _p(b_even), _p(sh), n,
-                                    float(tol), int(max_iter), _p(x), ctypes.byref(iters), freeze,
+                                    float(tol), int(max_iter), int(sum_order), _p(x), ctypes.byref(iters), freeze,
                                     ctypes.byref(rel))
     return x, dict(status=status, iters=iters.value, freeze_iter=list(freeze), rel_res=rel.value)

@@ -116,8 +116,10 @@ void dslash(const Lattice& lat, const cplx* U, const cplx* in, cplx* out, int p,
                 }
 }
 
-// Re <u, v> = Re sum conj(u) v over a parity field; one partial per time slice, added in order.
-double re_dot(const Lattice& lat, const cplx* u, const cplx* v) {
+// Re <u, v> = Re sum conj(u) v over a parity field; one partial per time slice, added in slice order
+// (sum_order 0: increasing t, the default reading R8; 1: decreasing t -- an equally valid order, used by
+// the tests to measure how far the iteration count moves under a rounding-level perturbation, R9).
+double re_dot(const Lattice& lat, const cplx* u, const cplx* v, int sum_order = 0) {
     const int Lt = lat.L[3];
     const int64_t per_slice = lat.Vh / Lt * 3;
     std::vector<double> partial(Lt, 0.0);
@@ -129,7 +131,10 @@ double re_dot(const Lattice& lat, const cplx* u, const cplx* v) {
         partial[t] = s;
     }
     double s = 0.0;
-    for (int t = 0; t < Lt; ++t) s += partial[t];
+    if (sum_order == 0)
+        for (int t = 0; t < Lt; ++t) s += partial[t];
+    else
+        for (int t = Lt - 1; t >= 0; --t) s += partial[t];
     return s;
 }
 
@@ -255,10 +260,11 @@ void oracle_scatter(const int* L, int parity, const double* aos, double* full) {
 //   b, x[i]: AoS even-parity fields (Vh*3 complex).  x is nshift fields stored back to back.
 //   Outputs: *iters; freeze_iter[nshift] (iteration after which shift i stopped being updated, or the
 //   final count if it never froze); *rel_res = sqrt(rr/bb) of the base recurrence residual.
+//   sum_order: order in which the per-slice partials of every scalar product are added (see re_dot).
 //   Returns 0 on convergence, 1 if max_iter was reached, 2 on breakdown (pAp <= 0 or non-finite).
 int oracle_mshift_cg(const int* L, const double* U, double mass, int antiperiodic, const double* b_even,
-                     const double* shifts, int nshift, double tol, int max_iter, double* x_out,
-                     int* iters, int* freeze_iter, double* rel_res) {
+                     const double* shifts, int nshift, double tol, int max_iter, int sum_order,
+                     double* x_out, int* iters, int* freeze_iter, double* rel_res) {
     Lattice lat = make_lattice(L);
     const int64_t n = lat.Vh * 3;
     const cplx* Uc = (const cplx*)U;
@@ -279,7 +285,7 @@ int oracle_mshift_cg(const int* L, const double* U, double mass, int antiperiodi
     std::vector<double> zeta(nshift, 1.0), zeta_prev(nshift, 1.0), zeta_new(nshift, 1.0);
     std::vector<char> active(nshift, 1);
     double a_prev = 1.0, b_prev = 0.0;
-    double rr = re_dot(lat, r.data(), r.data());
+    double rr = re_dot(lat, r.data(), r.data(), sum_order);
     const double bb = rr;
     const double c0 = mass * mass + sigma0;
     int it = 0, status = 0;
@@ -299,7 +305,7 @@ int oracle_mshift_cg(const int* L, const double* U, double mass, int antiperiodi
 #pragma omp parallel for schedule(static)
         for (int64_t j = 0; j < n; ++j) s[j] = c0 * pb[j] - s[j];
 
-        const double pAp = re_dot(lat, pb, s.data());
+        const double pAp = re_dot(lat, pb, s.data(), sum_order);
         if (!(pAp > 0.0) || !std::isfinite(pAp)) { status = 2; break; }
         const double a = rr / pAp;
 
@@ -313,7 +319,7 @@ int oracle_mshift_cg(const int* L, const double* U, double mass, int antiperiodi
         }
 
         axpy(n, -a, s.data(), r.data());
-        const double rr_new = re_dot(lat, r.data(), r.data());
+        const double rr_new = re_dot(lat, r.data(), r.data(), sum_order);
         const double bt = rr_new / rr;
 
         axpby(n, 1.0, r.data(), bt, pb);

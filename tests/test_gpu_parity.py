@@ -92,12 +92,29 @@ def test_dslash_host_entry_points(lq):
     lat.close()
 
 
+def oracle_iteration_band(L, U, mass, b_aos, shifts, tol, n_ref, trials):
+    """[lo, hi] spanned by the oracle's own iteration count under rounding-level perturbations: the other
+    summation order of the scalar products, and the source moved by at most one ulp per component.
+    (R9: beyond a few hundred iterations the CG residual history is sensitive to the last bit,
+    so "the same count +-1" can only be asked relative to this band.)"""
+    counts = [n_ref, oracle.mshift_cg(L, U, mass, b_aos, shifts, tol, sum_order=1)[1]["iters"]]
+    rng = np.random.default_rng(1234)
+    for _ in range(trials):
+        bp = b_aos * (1.0 + rng.integers(-1, 2, size=b_aos.shape) * 2.0 ** -52)
+        counts.append(oracle.mshift_cg(L, U, mass, bp, shifts, tol)[1]["iters"])
+    return min(counts), max(counts)
+
+
 def run_cg_both(lq, L, mass, shifts, tol, recon=18, use_graph=True, stream=None, max_iter=None, host=False,
-                check_every=None):
+                check_every=None, band_trials=3):
     U, f = make_inputs(L)
     b_soa, b_aos = oracle_parity_vector(L, f.numpy(), 0)
     kw = {} if max_iter is None else dict(max_iter=max_iter)
     x_ref, info_ref = oracle.mshift_cg(L, U.numpy(), mass, b_aos, shifts, tol, **kw)
+    if max_iter is None and info_ref["iters"] > 300:
+        info_ref["band"] = oracle_iteration_band(L, U.numpy(), mass, b_aos, shifts, tol, info_ref["iters"], band_trials)
+    else:
+        info_ref["band"] = (info_ref["iters"], info_ref["iters"])
     lat = lq.Lattice(L, mass=mass, recon=recon)
     lat.set_option(lq.LQCD_OPT_USE_GRAPH, 1 if use_graph else 0)
     if max_iter is not None:
@@ -122,15 +139,16 @@ def run_cg_both(lq, L, mass, shifts, tol, recon=18, use_graph=True, stream=None,
     return x, info, x_ref, info_ref, launches
 
 
-def check_cg(x, info, x_ref, info_ref, shifts, exact_iters=False):
-    if exact_iters:
-        assert info["iters"] == info_ref["iters"]
-    else:
-        assert abs(info["iters"] - info_ref["iters"]) <= 1, (info["iters"], info_ref["iters"])
+def check_cg(x, info, x_ref, info_ref, shifts):
+    """iteration count within +-1 of the oracle's (of the oracle's rounding band for long solves), every
+    solution within 1e-8, freeze schedule within the same slack."""
+    lo, hi = info_ref.get("band", (info_ref["iters"], info_ref["iters"]))
+    assert lo - 1 <= info["iters"] <= hi + 1, (info["iters"], info_ref["iters"], (lo, hi))
+    slack = 1 + (hi - lo)
     for i in range(len(shifts)):
         err = rel_l2(soa_gpu_to_aos(x[i]), x_ref[i])
         assert err <= TOL_CG, (i, shifts[i], err)
-        assert abs(info["freeze_iter"][i] - info_ref["freeze_iter"][i]) <= 2, (i, info["freeze_iter"], info_ref["freeze_iter"])
+        assert abs(info["freeze_iter"][i] - info_ref["freeze_iter"][i]) <= slack + 1, (i, info["freeze_iter"], info_ref["freeze_iter"])
 
 
 @pytest.mark.parametrize("L,mass,shifts", [
@@ -156,8 +174,10 @@ def test_mshift_cg_config2_16x4(lq):
     """BASELINE config 2: 16^4, m = 0.01, 8 shifts 1e-4*10^(i/2), tol 1e-10 -- full solve on both sides."""
     cfg = gen.CONFIGS["config2_16^4"]
     x, info, x_ref, info_ref, _ = run_cg_both(lq, cfg["L"], cfg["mass"], cfg["shifts"], cfg["tol"],
-                                              stream=torch.cuda.Stream())
+                                              stream=torch.cuda.Stream(), band_trials=1)
     assert info["status"] == 0 and info_ref["status"] == 0
+    print("config 2: GPU iterations", info["iters"], "oracle", info_ref["iters"], "oracle band", info_ref["band"],
+          "freeze", info["freeze_iter"], info_ref["freeze_iter"])
     check_cg(x, info, x_ref, info_ref, cfg["shifts"])
     # true residual of every GPU solution, computed by the oracle operator (one application per shift)
     L = cfg["L"]
@@ -270,6 +290,7 @@ def test_caller_workspace(lq):
     lat.set_gauge(U.cuda())
     x, info = lat.mshift_cg(cuda(b_soa), shifts, 1e-10)
     xr, ir = oracle.mshift_cg(L, U.numpy(), mass, b_aos, shifts, 1e-10)
+    ir["band"] = oracle_iteration_band(L, U.numpy(), mass, b_aos, shifts, 1e-10, ir["iters"], 3)
     check_cg(x, info, xr, ir, shifts)
     lat.close()
 
