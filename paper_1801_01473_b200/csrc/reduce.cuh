@@ -46,11 +46,22 @@ __device__ __forceinline__ bool publish_partial(double block_value, double* part
     return *flag_smem != 0;
 }
 
-// Sum of n partials by one whole block, fixed order; result valid in thread 0.
+// Sum of n partials by one whole block, fixed order; result valid in thread 0.  Eight independent loads
+// per thread are in flight at a time: with ~20k partials (48^4) a one-load-at-a-time loop costs tens of
+// microseconds of exposed L2 latency at the tail of the kernel.
 template <int BLOCK>
 __device__ __forceinline__ double final_sum(const double* partials, int n, double* red) {
-    double v = 0.0;
-    for (int i = threadIdx.x; i < n; i += BLOCK) v += __ldcg(partials + i);
+    double a[8] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0, 0.0, 0.0};
+    int i = threadIdx.x;
+    for (; i + 7 * BLOCK < n; i += 8 * BLOCK) {
+        double v[8];
+#pragma unroll
+        for (int u = 0; u < 8; ++u) v[u] = __ldcg(partials + i + u * BLOCK);
+#pragma unroll
+        for (int u = 0; u < 8; ++u) a[u] += v[u];
+    }
+    for (; i < n; i += BLOCK) a[0] += __ldcg(partials + i);
+    const double v = ((a[0] + a[1]) + (a[2] + a[3])) + ((a[4] + a[5]) + (a[6] + a[7]));
     return block_sum<BLOCK>(v, red);
 }
 
