@@ -27,6 +27,9 @@
 #ifndef DS_MINB
 #define DS_MINB 4
 #endif
+#ifndef EPI_PLOAD
+#define EPI_PLOAD 1      // 0: load p in the epilogue, 1: load p into registers up front, 2: L2 prefetch up front
+#endif
 
 __device__ __forceinline__ uint64_t l2_policy_evict_first() {
     uint64_t p;
@@ -197,6 +200,20 @@ __global__ void __launch_bounds__(DS_BLOCK, DS_MINB) dslash_kernel(const DslashA
     const size_t mu_stride = (size_t)2 * NE * vh;
     const double2* __restrict__ in = A.in;
 
+    // epilogue operands are requested first, so that their latency hides behind the eight hops
+    double coef = 0.0;
+    double2 pv[3];
+    if (EPI != 0) {
+        coef = (EPI == 1) ? A.st->c0 : A.coef;     // CG: m^2 + sigma0 from the device state (graph-invariant)
+#if EPI_PLOAD == 1
+#pragma unroll
+        for (int c = 0; c < 3; ++c) pv[c] = A.pv[c * vh + k];
+#elif EPI_PLOAD == 2
+#pragma unroll
+        for (int c = 0; c < 3; ++c) asm volatile("prefetch.global.L2 [%0];" ::"l"(A.pv + c * vh + k));
+#endif
+    }
+
     double ar[3] = {0.0, 0.0, 0.0}, ai[3] = {0.0, 0.0, 0.0};
     hop_fwd<RECON>(ar, ai, Wf + 0 * mu_stride, in + kxf, vh, 0u, pol_s, pol_r);
     hop_bwd<RECON>(ar, ai, Wb + 0 * mu_stride + kxb, in + kxb, vh, SB, pol_s, pol_r);
@@ -215,13 +232,15 @@ __global__ void __launch_bounds__(DS_BLOCK, DS_MINB) dslash_kernel(const DslashA
         return;
     }
 
-    // epilogue: out = coef*pv - D in;  Re<pv, out>.  In the CG the coefficient m^2 + sigma0 comes from
-    // the device state, so that the captured graph does not depend on the shifts of a solve.
-    const double coef = (EPI == 1) ? A.st->c0 : A.coef;
+    // epilogue: out = coef*pv - D in;  Re<pv, out>
     double dot = 0.0;
 #pragma unroll
     for (int c = 0; c < 3; ++c) {
+#if EPI_PLOAD == 1
+        const double2 p = pv[c];
+#else
         const double2 p = A.pv[c * vh + k];
+#endif
         const double2 o = make_double2(fma(-0.5, ar[c], coef * p.x), fma(-0.5, ai[c], coef * p.y));
         if (valid) {
             A.out[c * vh + k] = o;

@@ -16,11 +16,11 @@ __device__ __forceinline__ double warp_sum(double v) {
 }
 
 // Sum over the block; result valid in thread 0.  `red` holds >= 32 doubles of shared memory.
+// One barrier; the caller must put a barrier between two calls that use the same `red`.
 template <int BLOCK>
 __device__ __forceinline__ double block_sum(double v, double* red) {
     v = warp_sum(v);
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
-    __syncthreads();                       // `red` may still be read from a previous call
     if (lane == 0) red[w] = v;
     __syncthreads();
     double s = 0.0;
@@ -33,6 +33,7 @@ __device__ __forceinline__ double block_sum(double v, double* red) {
 
 // Writes this block's partial, then tells whether this block is the last one of the grid to do so.
 // When it returns true (for every thread of that block) all partials of the grid are visible.
+// The barrier inside also separates the caller's block_sum from a following final_sum.
 template <int BLOCK>
 __device__ __forceinline__ bool publish_partial(double block_value, double* partials, unsigned int* ticket,
                                                 int* flag_smem) {
@@ -46,23 +47,29 @@ __device__ __forceinline__ bool publish_partial(double block_value, double* part
     return *flag_smem != 0;
 }
 
-// Sum of n partials by one whole block, fixed order; result valid in thread 0.  Eight independent loads
+// Sum of n partials by one whole block, fixed order; result valid in thread 0.  Sixteen independent loads
 // per thread are in flight at a time: with ~20k partials (48^4) a one-load-at-a-time loop costs tens of
 // microseconds of exposed L2 latency at the tail of the kernel.
 template <int BLOCK>
 __device__ __forceinline__ double final_sum(const double* partials, int n, double* red) {
-    double a[8] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0, 0.0, 0.0};
+    constexpr int U = 16;
+    double a[U];
+#pragma unroll
+    for (int u = 0; u < U; ++u) a[u] = 0.0;
     int i = threadIdx.x;
-    for (; i + 7 * BLOCK < n; i += 8 * BLOCK) {
-        double v[8];
+    for (; i + (U - 1) * BLOCK < n; i += U * BLOCK) {
+        double v[U];
 #pragma unroll
-        for (int u = 0; u < 8; ++u) v[u] = __ldcg(partials + i + u * BLOCK);
+        for (int u = 0; u < U; ++u) v[u] = __ldcg(partials + i + u * BLOCK);
 #pragma unroll
-        for (int u = 0; u < 8; ++u) a[u] += v[u];
+        for (int u = 0; u < U; ++u) a[u] += v[u];
     }
     for (; i < n; i += BLOCK) a[0] += __ldcg(partials + i);
-    const double v = ((a[0] + a[1]) + (a[2] + a[3])) + ((a[4] + a[5]) + (a[6] + a[7]));
-    return block_sum<BLOCK>(v, red);
+#pragma unroll
+    for (int w = U / 2; w > 0; w >>= 1)
+#pragma unroll
+        for (int u = 0; u < w; ++u) a[u] += a[u + w];
+    return block_sum<BLOCK>(a[0], red);
 }
 
 // ---- scalar recurrences (SURVEY.md §8(c2) / DESIGN.md R5), run by thread 0 of the last block ------
