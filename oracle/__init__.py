@@ -41,6 +41,9 @@ def lib():
         L.oracle_mshift_cg.argtypes = [_ip, _dp, ctypes.c_double, ctypes.c_int, _dp, _dp, ctypes.c_int,
                                        ctypes.c_double, ctypes.c_int, ctypes.c_int, _dp, _ip, _ip, _dp]
         L.oracle_mshift_cg.restype = ctypes.c_int
+        L.oracle_rational_apply.argtypes = [_ip, _dp, ctypes.c_double, ctypes.c_int, _dp, ctypes.c_double, _dp, _dp,
+                                            ctypes.c_int, ctypes.c_double, ctypes.c_int, _dp, _ip, _dp]
+        L.oracle_rational_apply.restype = ctypes.c_int
     return _lib
 
 
@@ -153,3 +156,20 @@ def mshift_cg(L, U, mass: float, b_even, shifts, tol: float, max_iter: int = 100
                                     float(tol), int(max_iter), int(sum_order), _p(x), ctypes.byref(iters), freeze,
                                     ctypes.byref(rel))
     return x, dict(status=status, iters=iters.value, freeze_iter=list(freeze), rel_res=rel.value)
+
+
+def rational_apply(L, U, mass: float, b_even, alpha0: float, alpha, shifts, tol: float, max_iter: int = 100000,
+                   antiperiodic: bool = True):
+    """y = alpha0 b + sum_i alpha_i (m^2 - D_eo D_oe + sigma_i)^-1 b: the partial-fraction form of the RHMC's
+    rational function of the Eq. 2 operator.  Returns (y, info)."""
+    U, b_even = _c(U), _c(b_even)
+    sh = _c(np.asarray(shifts, dtype=np.float64))
+    al = _c(np.asarray(alpha, dtype=np.float64))
+    assert sh.shape == al.shape and sh.ndim == 1
+    y = np.empty_like(b_even)
+    iters = ctypes.c_int(0)
+    rel = ctypes.c_double(0.0)
+    status = lib().oracle_rational_apply(_L(L), _p(U), float(mass), int(antiperiodic), _p(b_even), float(alpha0),
+                                         _p(al), _p(sh), sh.shape[0], float(tol), int(max_iter), _p(y),
+                                         ctypes.byref(iters), ctypes.byref(rel))
+    return y, dict(status=status, iters=iters.value, rel_res=rel.value)

@@ -357,4 +357,30 @@ int oracle_mshift_cg(const int* L, const double* U, double mass, int antiperiodi
     return status;
 }
 
+// Rational function of the operator of Eq. 2 applied to a vector,
+//     y = alpha0 b + sum_i alpha_i (m^2 - D_eo D_oe + sigma_i)^{-1} b ,
+// the partial-fraction form in which the RHMC uses the solutions of Eq. 2: "the fractional power of M(U)
+// is approximated ... by a rational function of M(U)" whose poles are the sigma_i.
+// Plain definition: solve Eq. 2 for every shift with oracle_mshift_cg, then add the terms in index order.
+// Returns the status of the solve.
+int oracle_rational_apply(const int* L, const double* U, double mass, int antiperiodic, const double* b_even,
+                          double alpha0, const double* alpha, const double* shifts, int nshift, double tol,
+                          int max_iter, double* y_out, int* iters, double* rel_res) {
+    Lattice lat = make_lattice(L);
+    const int64_t n = lat.Vh * 3;
+    std::vector<double> x((size_t)nshift * n * 2);
+    std::vector<int> freeze(nshift);
+    const int status = oracle_mshift_cg(L, U, mass, antiperiodic, b_even, shifts, nshift, tol, max_iter, 0, x.data(),
+                                        iters, freeze.data(), rel_res);
+    const cplx* b = (const cplx*)b_even;
+    const cplx* xs = (const cplx*)x.data();
+    cplx* y = (cplx*)y_out;
+    for (int64_t j = 0; j < n; ++j) {
+        cplx acc = alpha0 * b[j];
+        for (int i = 0; i < nshift; ++i) acc += alpha[i] * xs[(int64_t)i * n + j];
+        y[j] = acc;
+    }
+    return status;
+}
+
 }  // extern "C"

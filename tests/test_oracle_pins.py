@@ -347,3 +347,42 @@ def test_iteration_count_moves_under_one_ulp_perturbations():
         for i in range(len(shifts)):
             assert np.linalg.norm(xp[i] - x0[i]) <= 1e-9 * np.linalg.norm(x0[i])
     assert 0 <= max(counts) - min(counts) <= 6 and min(counts) > 700
+
+
+# ---------------------------------------------------------------------------------------------------
+# rational function of the Eq. 2 operator: y = alpha0 b + sum_i alpha_i (A+sigma_i)^-1 b
+# ---------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("L,mass", [((2, 2, 2, 2), 0.05), ((4, 2, 2, 4), 0.02)])
+def test_rational_apply_against_dense_function_of_the_matrix(L, mass):
+    """r(x) = (x+c1)(x+c2)(x+c3) / ((x+s1)(x+s2)(x+s3)) has the partial fractions 1 + sum_i alpha_i/(x+s_i)
+    with alpha_i = prod_j (c_j - s_i) / prod_{j != i} (s_j - s_i); r(A) b is computed independently from the
+    eigen-decomposition of the dense A.  Pins alpha0, the pairing alpha_i <-> sigma_i and the signs."""
+    U = links(L)
+    b = oracle.restrict(L, 0, gen.gaussian_field(L).numpy())
+    A = dense_A(L, U, mass)
+    ev, W = np.linalg.eigh(A)
+    cz = np.array([0.7, 0.03, 2.5])
+    sp = np.array([0.2, 1.3, 0.004])                                 # base shift is the last one
+    alpha = np.array([np.prod(cz - sp[i]) / np.prod(np.delete(sp, i) - sp[i]) for i in range(3)])
+    rl = np.prod(ev[:, None] + cz[None, :], axis=1) / np.prod(ev[:, None] + sp[None, :], axis=1)
+    ref = W @ (rl * (W.conj().T @ c(b).ravel()))
+    y, info = oracle.rational_apply(L, U, mass, b, 1.0, alpha, sp, 1e-12)
+    assert info["status"] == 0
+    assert np.linalg.norm(c(y).ravel() - ref) <= 1e-9 * np.linalg.norm(ref)
+    # alpha0 alone, and one pole alone against numpy.linalg.solve
+    y0, _ = oracle.rational_apply(L, U, mass, b, -2.5, [0.0, 0.0], [0.1, 0.2], 1e-12)
+    assert np.abs(c(y0) + 2.5 * c(b)).max() < 1e-14
+    y1, _ = oracle.rational_apply(L, U, mass, b, 0.0, [3.0], [0.3], 1e-12)
+    ref1 = 3.0 * np.linalg.solve(A + 0.3 * np.eye(A.shape[0]), c(b).ravel())
+    assert np.linalg.norm(c(y1).ravel() - ref1) <= 1e-10 * np.linalg.norm(ref1)
+
+
+def test_rational_apply_product_of_two_inverses():
+    """1/((x+s1)(x+s2)) = [1/(x+s1) - 1/(x+s2)]/(s2-s1): applying (A+s2)(A+s1) to y must give b back."""
+    L, mass, s1, s2 = (4, 4, 4, 4), 0.05, 0.01, 0.4
+    U = links(L)
+    b = oracle.restrict(L, 0, gen.gaussian_field(L).numpy())
+    y, info = oracle.rational_apply(L, U, mass, b, 0.0, [1 / (s2 - s1), -1 / (s2 - s1)], [s1, s2], 1e-12)
+    assert info["status"] == 0
+    back = oracle.mdagm(L, U, mass, s2, oracle.mdagm(L, U, mass, s1, y))
+    assert np.linalg.norm(back - b) <= 1e-10 * np.linalg.norm(b)
