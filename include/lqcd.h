@@ -129,6 +129,21 @@ int lqcd_mshift_cg(lqcd_ctx* ctx, const double* b_even, const double* shifts /*H
 int lqcd_mshift_cg_host(lqcd_ctx* ctx, const double* b_even /*HOST*/, const double* shifts /*HOST*/,
                         int nshift, double tol, double* const* x /*HOST array of HOST pointers*/);
 
+/* Rational function of the Eq. 2 operator applied to b,
+ *     y = alpha0 b + sum_i alpha[i] (m^2 - D_eo D_oe + shifts[i])^{-1} b ,
+ * the partial-fraction form in which the RHMC uses the solutions of Eq. 2 (the rational approximation of the
+ * fractional power of the Dirac matrix with poles sigma_i).  Same solver, stopping and
+ * freezing rules as lqcd_mshift_cg, but the sum is accumulated during the solve (y += alpha_i a_i p_i) and
+ * the x_i are never stored: 96 instead of 192 bytes per site and active shift in the update sweep, and no
+ * memory for nshift solution vectors.
+ *   alpha, shifts : HOST arrays of nshift values;  y_even : parity vector (overwritten), must not alias b.
+ * Statistics as for lqcd_mshift_cg.  Returns as lqcd_mshift_cg. */
+int lqcd_rational_apply(lqcd_ctx* ctx, const double* b_even, double alpha0, const double* alpha /*HOST*/,
+                        const double* shifts /*HOST*/, int nshift, double tol, double* y_even);
+/* Same, b and y in HOST memory; copies are part of the call. */
+int lqcd_rational_apply_host(lqcd_ctx* ctx, const double* b_even /*HOST*/, double alpha0, const double* alpha /*HOST*/,
+                             const double* shifts /*HOST*/, int nshift, double tol, double* y_even /*HOST*/);
+
 /* Statistics of the last solve; *out is HOST. idx is used by LQCD_STAT_FREEZE_ITER only. */
 int lqcd_get_stat(const lqcd_ctx* ctx, int key, int idx, double* out /*HOST*/);
 

@@ -39,6 +39,8 @@ EXPORTS = {
     "lqcd_mdagm": (_i, [_vp, _dp, _dp, _d]),
     "lqcd_mshift_cg": (_i, [_vp, _dp, _pd, _i, _d, ctypes.POINTER(ctypes.c_void_p)]),
     "lqcd_mshift_cg_host": (_i, [_vp, _dp, _pd, _i, _d, ctypes.POINTER(ctypes.c_void_p)]),
+    "lqcd_rational_apply": (_i, [_vp, _dp, _d, _pd, _pd, _i, _d, _dp]),
+    "lqcd_rational_apply_host": (_i, [_vp, _dp, _d, _pd, _pd, _i, _d, _dp]),
     "lqcd_get_stat": (_i, [_vp, _i, _i, _pd]),
     "lqcd_pack_vector": (_i, [_vp, _i, _dp, _dp]),
     "lqcd_unpack_vector": (_i, [_vp, _i, _dp, _dp]),
@@ -151,6 +153,20 @@ def lqcd_mshift_cg(ctx, b_even, shifts: Sequence[float], tol: float, x_ptrs: Seq
 def lqcd_mshift_cg_host(ctx, b_even, shifts: Sequence[float], tol: float, x_ptrs: Sequence[int]):
     n, sh, xs = _cg_args(shifts, x_ptrs)
     return load_library().lqcd_mshift_cg_host(ctx, b_even, sh, n, float(tol), xs)
+
+
+def lqcd_rational_apply(ctx, b_even, alpha0: float, alpha: Sequence[float], shifts: Sequence[float], tol: float,
+                        y_even, host: bool = False):
+    n = len(shifts)
+    assert len(alpha) == n
+    al = (ctypes.c_double * n)(*[float(a) for a in alpha])
+    sh = (ctypes.c_double * n)(*[float(s) for s in shifts])
+    fn = load_library().lqcd_rational_apply_host if host else load_library().lqcd_rational_apply
+    return fn(ctx, b_even, float(alpha0), al, sh, n, float(tol), y_even)
+
+
+def lqcd_rational_apply_host(ctx, b_even, alpha0, alpha, shifts, tol, y_even):
+    return lqcd_rational_apply(ctx, b_even, alpha0, alpha, shifts, tol, y_even, host=True)
 
 
 def lqcd_get_stat(ctx, key, idx=0):
@@ -294,7 +310,10 @@ class Lattice:
         fn = lqcd_mshift_cg if b_even.device.type == "cuda" else lqcd_mshift_cg_host
         rc = fn(self.ctx, pb, shifts, tol, ptrs)
         self._check(rc, allow=() if raise_on_noconv else (LQCD_ENOCONV,))
-        info = dict(
+        return x, self._solve_info(rc, n)
+
+    def _solve_info(self, rc, n):
+        return dict(
             status=rc,
             iters=int(self.stat(LQCD_STAT_ITERS)),
             rel_res=self.stat(LQCD_STAT_REL_RES),
@@ -302,7 +321,21 @@ class Lattice:
             base_shift=int(self.stat(LQCD_STAT_BASE_SHIFT)),
             solve_ms=self.stat(LQCD_STAT_SOLVE_MS),
         )
-        return x, info
+
+    def rational_apply(self, b_even, alpha0: float, alpha: Sequence[float], shifts: Sequence[float], tol: float,
+                       y=None, raise_on_noconv: bool = True):
+        """y = alpha0 b + sum_i alpha_i (m^2 - D_eo D_oe + shifts[i])^-1 b, accumulated
+        during the multi-shift solve.  Returns (y, info)."""
+        torch = self._torch
+        pb = self._t(b_even, (3, self.Vh, 2))
+        host = b_even.device.type == "cpu"
+        if y is None:
+            y = torch.empty((3, self.Vh, 2), dtype=torch.float64, device=b_even.device, pin_memory=host)
+        py = self._t(y, (3, self.Vh, 2), b_even.device.type)
+        self._sync_stream()
+        rc = lqcd_rational_apply(self.ctx, pb, alpha0, alpha, shifts, tol, py, host=host)
+        self._check(rc, allow=() if raise_on_noconv else (LQCD_ENOCONV,))
+        return y, self._solve_info(rc, len(shifts))
 
     def pack(self, site_field, parity: int, out=None):
         """(V,3,2) site field -> (3,Vh,2) parity vector of the given parity."""

@@ -21,14 +21,19 @@ __global__ void __launch_bounds__(CG_BLOCK) cg_init_kernel(const double2* __rest
     __shared__ double red[32];
     __shared__ int last_flag;
     const int ns = st->nshift;
+    const int rational = st->rational;
+    const double alpha0 = st->alpha0;
+    double2* __restrict__ y = st->y;
     double acc = 0.0;
     const double2 zero = make_double2(0.0, 0.0);
     for (size_t j = (size_t)blockIdx.x * CG_BLOCK + threadIdx.x; j < n; j += (size_t)gridDim.x * CG_BLOCK) {
         const double2 v = b[j];
         r[j] = v;
-        for (int i = 0; i < ns; ++i) {
-            st->p[i][j] = v;
-            st->x[i][j] = zero;
+        for (int i = 0; i < ns; ++i) st->p[i][j] = v;
+        if (rational) {
+            y[j] = make_double2(alpha0 * v.x, alpha0 * v.y);
+        } else {
+            for (int i = 0; i < ns; ++i) st->x[i][j] = zero;
         }
         acc = fma(v.x, v.x, acc);
         acc = fma(v.y, v.y, acc);
@@ -136,6 +141,53 @@ __global__ void __launch_bounds__(CG_BLOCK) cg_update_xp_kernel(const double2* _
             sx[e][j] = xv;
             sp[e][j] = pv;
         }
+    }
+}
+
+// K4 of lqcd_rational_apply: y += sum_i (alpha_i a_i) p_i ; p_i = zeta_new_i r + b_i p_i.  The x_i are never
+// stored: 96 B per site and active shift instead of 192 (the sum is taken in list order, per element).
+__global__ void __launch_bounds__(CG_BLOCK) cg_update_yp_kernel(const double2* __restrict__ r, const CgState* st, size_t n) {
+    if (st->stop4) return;
+    __shared__ double2* sp[LQCD_MAX_SHIFTS];
+    __shared__ double sa[LQCD_MAX_SHIFTS], sz[LQCD_MAX_SHIFTS], sb[LQCD_MAX_SHIFTS];
+    const int nl = st->nlist;
+    for (int e = threadIdx.x; e < nl; e += CG_BLOCK) {
+        sp[e] = st->p[st->list_idx[e]];
+        sa[e] = st->list_a[e];
+        sz[e] = st->list_zn[e];
+        sb[e] = st->list_b[e];
+    }
+    __syncthreads();
+    double2* __restrict__ y = st->y;
+    const size_t stride = (size_t)gridDim.x * CG_BLOCK;
+    for (size_t j = (size_t)blockIdx.x * CG_BLOCK + threadIdx.x; j < n; j += stride) {
+        const double2 rv = r[j];
+        double2 yv = y[j];
+        int e = 0;
+        for (; e + 4 <= nl; e += 4) {
+            double2 pv[4];
+#pragma unroll
+            for (int u = 0; u < 4; ++u) pv[u] = sp[e + u][j];
+#pragma unroll
+            for (int u = 0; u < 4; ++u) {
+                const double a = sa[e + u], zn = sz[e + u], bi = sb[e + u];
+                yv.x = fma(a, pv[u].x, yv.x);
+                yv.y = fma(a, pv[u].y, yv.y);
+                pv[u].x = fma(zn, rv.x, bi * pv[u].x);
+                pv[u].y = fma(zn, rv.y, bi * pv[u].y);
+                sp[e + u][j] = pv[u];
+            }
+        }
+        for (; e < nl; ++e) {
+            double2 pv = sp[e][j];
+            const double a = sa[e], zn = sz[e], bi = sb[e];
+            yv.x = fma(a, pv.x, yv.x);
+            yv.y = fma(a, pv.y, yv.y);
+            pv.x = fma(zn, rv.x, bi * pv.x);
+            pv.y = fma(zn, rv.y, bi * pv.y);
+            sp[e][j] = pv;
+        }
+        y[j] = yv;
     }
 }
 

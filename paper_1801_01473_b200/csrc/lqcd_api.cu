@@ -64,7 +64,7 @@ struct lqcd_ctx {
 
     // CUDA graph of `graph_iters` CG iterations
     cudaGraphExec_t graph_exec;
-    int graph_iters;
+    int graph_iters, graph_rational;
 
     // host-call staging (device copies of host arguments)
     double2* stage_b;
@@ -214,12 +214,15 @@ void launch_dslash(lqcd_ctx* c, int epi, double2* out, const double2* in, int pa
 }
 
 // one CG iteration = K1..K4 (cg.cuh)
-void launch_cg_iteration(lqcd_ctx* c) {
+void launch_cg_iteration(lqcd_ctx* c, int rational) {
     const size_t n = c->Vh * 3;
     launch_dslash(c, 0, c->t, c->p, 1, nullptr, 0.0, 1);
     launch_dslash(c, 1, c->s, c->t, 0, c->p, 0.0, 1);
     cg_update_r_kernel<<<cg_grid(c), CG_BLOCK, 0, c->stream>>>(c->r, c->s, c->st_dev, c->partials, n);
-    cg_update_xp_kernel<<<cg_grid(c), CG_BLOCK, 0, c->stream>>>(c->r, c->st_dev, n);
+    if (rational)
+        cg_update_yp_kernel<<<cg_grid(c), CG_BLOCK, 0, c->stream>>>(c->r, c->st_dev, n);
+    else
+        cg_update_xp_kernel<<<cg_grid(c), CG_BLOCK, 0, c->stream>>>(c->r, c->st_dev, n);
     c->launches += 2;
 }
 
@@ -230,12 +233,12 @@ int default_check_every(const lqcd_ctx* c) {
     return (int)v;
 }
 
-int build_graph(lqcd_ctx* c, int iters) {
+int build_graph(lqcd_ctx* c, int iters, int rational) {
     drop_graph(c);
     cudaGraph_t graph = nullptr;
     const long long before = c->launches;
     CU(cudaStreamBeginCapture(c->stream, cudaStreamCaptureModeThreadLocal));
-    for (int i = 0; i < iters; ++i) launch_cg_iteration(c);
+    for (int i = 0; i < iters; ++i) launch_cg_iteration(c, rational);
     cudaError_t e = cudaStreamEndCapture(c->stream, &graph);
     c->launches = before;     // capturing is not launching
     if (e != cudaSuccess) return fail(c, LQCD_ECUDA, "graph capture failed: %s", cudaGetErrorString(e));
@@ -246,6 +249,7 @@ int build_graph(lqcd_ctx* c, int iters) {
         return fail(c, LQCD_ECUDA, "graph instantiate failed: %s", cudaGetErrorString(e));
     }
     c->graph_iters = iters;
+    c->graph_rational = rational;
     return LQCD_OK;
 }
 
@@ -513,17 +517,26 @@ int lqcd_mdagm(lqcd_ctx* c, double* out_even, const double* in_even, double sigm
     return LQCD_OK;
 }
 
-int lqcd_mshift_cg(lqcd_ctx* c, const double* b_even, const double* shifts, int nshift, double tol, double* const* x) {
+// The solver behind lqcd_mshift_cg (x != NULL: every x[i] is stored) and lqcd_rational_apply (y != NULL:
+// only y = alpha0 b + sum_i alpha[i] x_i is accumulated).
+static int solve(lqcd_ctx* c, const double* b_even, const double* shifts, int nshift, double tol, double* const* x,
+                 double* y, double alpha0, const double* alpha) {
     if (!c) return LQCD_EINVAL;
-    if (!b_even || !shifts || !x) return fail(c, LQCD_EINVAL, "NULL argument");
+    if (!b_even || !shifts || (!x && !y) || (y && !alpha)) return fail(c, LQCD_EINVAL, "NULL argument");
     if (nshift < 1 || nshift > LQCD_MAX_SHIFTS) return fail(c, LQCD_EINVAL, "nshift must be in [1, %d]", LQCD_MAX_SHIFTS);
     if (!(tol > 0.0) || !std::isfinite(tol)) return fail(c, LQCD_EINVAL, "tol must be positive");
     for (int i = 0; i < nshift; ++i) {
         if (!(shifts[i] >= 0.0) || !std::isfinite(shifts[i])) return fail(c, LQCD_EINVAL, "shift %d must be >= 0", i);
+        if (y) {
+            if (!std::isfinite(alpha[i])) return fail(c, LQCD_EINVAL, "alpha[%d] must be finite", i);
+            continue;
+        }
         if (!x[i] || (const double*)x[i] == b_even) return fail(c, LQCD_EINVAL, "x[%d] is NULL or aliases b", i);
         for (int j = 0; j < i; ++j)
             if (x[j] == x[i]) return fail(c, LQCD_EINVAL, "x[%d] aliases x[%d]", i, j);
     }
+    if (y && (y == b_even || !std::isfinite(alpha0))) return fail(c, LQCD_EINVAL, "y aliases b, or alpha0 is not finite");
+    const int rational = y ? 1 : 0;
     int rc;
     if ((rc = check_ctx_gauge(c))) return rc;
     if ((rc = ensure_solver(c, nshift))) return rc;
@@ -542,9 +555,13 @@ int lqcd_mshift_cg(lqcd_ctx* c, const double* b_even, const double* shifts, int 
     int extra = 0;
     for (int i = 0; i < nshift; ++i) {
         h->delta[i] = shifts[i] - shifts[i0];
-        h->x[i] = (double2*)x[i];
+        h->x[i] = rational ? nullptr : (double2*)x[i];
+        h->alpha[i] = rational ? alpha[i] : 0.0;
         h->p[i] = (i == i0) ? c->p : c->pextra[extra++];
     }
+    h->rational = rational;
+    h->alpha0 = alpha0;
+    h->y = (double2*)y;
     const size_t n = c->Vh * 3;
     CU(cudaMemcpyAsync(c->st_dev, h, sizeof(CgState), cudaMemcpyHostToDevice, c->stream));
     CU(cudaEventRecord(c->ev_t0, c->stream));
@@ -555,8 +572,8 @@ int lqcd_mshift_cg(lqcd_ctx* c, const double* b_even, const double* shifts, int 
     const int ce = c->check_every ? c->check_every : default_check_every(c);
     // the legacy default stream cannot be captured: plain launches there
     const bool use_graph = c->use_graph && c->stream != nullptr && c->stream != cudaStreamLegacy;
-    if (use_graph && c->graph_iters != ce) {
-        if ((rc = build_graph(c, ce))) return rc;
+    if (use_graph && (c->graph_iters != ce || c->graph_rational != rational)) {
+        if ((rc = build_graph(c, ce, rational))) return rc;
     }
     c->flag_host[0] = c->flag_host[1] = 0;
     bool done = false;
@@ -566,7 +583,7 @@ int lqcd_mshift_cg(lqcd_ctx* c, const double* b_even, const double* shifts, int 
             CU(cudaGraphLaunch(c->graph_exec, c->stream));
             c->launches += 4LL * ce;
         } else {
-            for (int i = 0; i < ce; ++i) launch_cg_iteration(c);
+            for (int i = 0; i < ce; ++i) launch_cg_iteration(c, rational);
             CU(cudaGetLastError());
         }
         const int slot = (int)(batch & 1);
@@ -592,6 +609,33 @@ int lqcd_mshift_cg(lqcd_ctx* c, const double* b_even, const double* shifts, int 
     if (h->status == LQCD_ENOCONV)
         return fail(c, LQCD_ENOCONV, "no convergence in %d iterations, |r|/|b| = %.3e", h->iter, c->last_rel);
     return LQCD_OK;
+}
+
+int lqcd_mshift_cg(lqcd_ctx* c, const double* b_even, const double* shifts, int nshift, double tol, double* const* x) {
+    if (c && !x) return fail(c, LQCD_EINVAL, "NULL argument");
+    return solve(c, b_even, shifts, nshift, tol, x, nullptr, 0.0, nullptr);
+}
+
+int lqcd_rational_apply(lqcd_ctx* c, const double* b_even, double alpha0, const double* alpha, const double* shifts,
+                        int nshift, double tol, double* y_even) {
+    if (c && !y_even) return fail(c, LQCD_EINVAL, "NULL argument");
+    return solve(c, b_even, shifts, nshift, tol, nullptr, y_even, alpha0, alpha);
+}
+
+int lqcd_rational_apply_host(lqcd_ctx* c, const double* b_even, double alpha0, const double* alpha,
+                             const double* shifts, int nshift, double tol, double* y_even) {
+    if (!c) return LQCD_EINVAL;
+    if (!b_even || !y_even) return fail(c, LQCD_EINVAL, "NULL argument");
+    int rc;
+    if ((rc = check_ctx_gauge(c))) return rc;
+    if ((rc = ensure_stage(c, 1))) return rc;
+    CU(cudaMemcpyAsync(c->stage_b, b_even, vec_bytes(c), cudaMemcpyHostToDevice, c->stream));
+    const int status = lqcd_rational_apply(c, (const double*)c->stage_b, alpha0, alpha, shifts, nshift, tol,
+                                           (double*)c->stage_x[0]);
+    if (status != LQCD_OK && status != LQCD_ENOCONV) return status;
+    CU(cudaMemcpyAsync(y_even, c->stage_x[0], vec_bytes(c), cudaMemcpyDeviceToHost, c->stream));
+    CU(cudaStreamSynchronize(c->stream));
+    return status;
 }
 
 int lqcd_mshift_cg_host(lqcd_ctx* c, const double* b_even, const double* shifts, int nshift, double tol, double* const* x) {

@@ -33,6 +33,12 @@ struct CgState {
     double list_a[LQCD_MAX_SHIFTS], list_zn[LQCD_MAX_SHIFTS], list_b[LQCD_MAX_SHIFTS];
     double2* x[LQCD_MAX_SHIFTS];
     double2* p[LQCD_MAX_SHIFTS];
+    // rational-sum mode (lqcd_rational_apply): y = alpha0 b + sum_i alpha_i x_i is accumulated during the
+    // solve and the x_i are never stored; list_a then holds alpha_i * a_i
+    int rational;
+    double alpha0;
+    double alpha[LQCD_MAX_SHIFTS];
+    double2* y;
 };
 
 #endif

@@ -116,7 +116,7 @@ __device__ inline void cg_scalars_after_pAp(CgState* st, double pAp) {
         const double zn = z * zp * a_prev / (a_prev * zp * (1.0 + st->delta[i] * a) + a * b_prev * (zp - z));
         st->zeta_new[i] = zn;
         st->list_idx[n] = i;
-        st->list_a[n] = a * zn / z;
+        st->list_a[n] = st->rational ? st->alpha[i] * (a * zn / z) : a * zn / z;
         st->list_zn[n] = zn;
         ++n;
     }

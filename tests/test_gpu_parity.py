@@ -295,6 +295,76 @@ def test_caller_workspace(lq):
     lat.close()
 
 
+# ---- rational function of the Eq. 2 operator, accumulated during the solve ------
+RATIONAL_CASES = [
+    ((4, 4, 4, 4), 0.01, [1e-4 * 10 ** (i / 2) for i in range(8)]),
+    ((2, 2, 2, 2), 0.05, [0.3, 0.0, 2.0, 1e-3]),
+    ((4, 6, 8, 10), 0.02, [1e-2, 1e-3, 1e-1, 1.0, 0.5]),
+    ((8, 8, 8, 8), 0.01, [1e-4 * 10 ** (i / 2) for i in range(8)]),
+]
+
+
+def rational_coefficients(n):
+    """alpha_i of mixed sign and size (seeded; not a particular rational approximation)."""
+    rng = np.random.default_rng(7)
+    return 0.37, list(rng.uniform(0.05, 1.5, n) * rng.choice([-1.0, 1.0], n))
+
+
+@pytest.mark.parametrize("L,mass,shifts", RATIONAL_CASES)
+@pytest.mark.parametrize("mode", ["graph", "plain", "recon12", "host"])
+def test_rational_apply_small(lq, L, mass, shifts, mode):
+    U, f = make_inputs(L)
+    b_soa, b_aos = oracle_parity_vector(L, f.numpy(), 0)
+    a0, al = rational_coefficients(len(shifts))
+    y_ref, info_ref = oracle.rational_apply(L, U.numpy(), mass, b_aos, a0, al, shifts, 1e-10)
+    lat = lq.Lattice(L, mass=mass, recon=12 if mode == "recon12" else 18)
+    lat.set_option(lq.LQCD_OPT_USE_GRAPH, 0 if mode == "plain" else 1)
+    with torch.cuda.stream(torch.cuda.Stream()):
+        lat.set_gauge(U.cuda())
+        b = torch.as_tensor(b_soa).pin_memory() if mode == "host" else cuda(b_soa)
+        y, info = lat.rational_apply(b, a0, al, shifts, 1e-10)
+        # the same solve with the x_i stored: the fused sum must be the sum of those x_i
+        x, info_x = lat.mshift_cg(cuda(b_soa), shifts, 1e-10)
+    torch.cuda.synchronize()
+    assert info["status"] == 0 and info["rel_res"] <= 1e-10
+    assert info["iters"] == info_x["iters"] and info["freeze_iter"] == info_x["freeze_iter"]
+    lo, hi = (info_ref["iters"],) * 2
+    if info_ref["iters"] > 300:
+        lo, hi = oracle_iteration_band(L, U.numpy(), mass, b_aos, shifts, 1e-10, info_ref["iters"], 2)
+    assert lo - 1 <= info["iters"] <= hi + 1
+    assert rel_l2(soa_gpu_to_aos(y), y_ref) <= TOL_CG
+    y_sum = a0 * cuda(b_soa) + sum(al[i] * x[i] for i in range(len(shifts)))
+    assert rel_l2(y.cpu().numpy(), y_sum.cpu().numpy()) <= 1e-11
+    lat.close()
+
+
+def test_rational_apply_fixed_iteration_count_and_errors(lq):
+    L, mass = (8, 8, 8, 8), 0.0075
+    shifts = gen.shifts_geometric(1e-5, 1.0, 16)
+    a0, al = rational_coefficients(16)
+    U, f = make_inputs(L)
+    b_soa, b_aos = oracle_parity_vector(L, f.numpy(), 0)
+    y_ref, info_ref = oracle.rational_apply(L, U.numpy(), mass, b_aos, a0, al, shifts, 1e-30, max_iter=40)
+    lat = lq.Lattice(L, mass=mass)
+    lat.set_gauge(U.cuda())
+    lat.set_option(lq.LQCD_OPT_MAX_ITER, 40)
+    b = cuda(b_soa)
+    with torch.cuda.stream(torch.cuda.Stream()):
+        y, info = lat.rational_apply(b, a0, al, shifts, 1e-30, raise_on_noconv=False)
+    torch.cuda.synchronize()
+    assert info["status"] == lq.LQCD_ENOCONV and info["iters"] == 40 == info_ref["iters"]
+    assert rel_l2(soa_gpu_to_aos(y), y_ref) <= 1e-11
+    # zero source, argument errors
+    y0, info0 = lat.rational_apply(torch.zeros_like(b), a0, al, shifts, 1e-10)
+    assert info0["iters"] == 0 and not y0.any()
+    out = torch.empty_like(b)
+    assert lq.lqcd_rational_apply(lat.ctx, b.data_ptr(), 1.0, [1.0], [-1.0], 1e-8, out.data_ptr()) == lq.LQCD_EINVAL
+    assert lq.lqcd_rational_apply(lat.ctx, b.data_ptr(), 1.0, [float("nan")], [1.0], 1e-8, out.data_ptr()) == lq.LQCD_EINVAL
+    assert lq.lqcd_rational_apply(lat.ctx, b.data_ptr(), 1.0, [1.0], [1.0], 1e-8, b.data_ptr()) == lq.LQCD_EINVAL
+    assert lq.lqcd_rational_apply(lat.ctx, b.data_ptr(), 1.0, [1.0], [1.0], 1e-8, None) == lq.LQCD_EINVAL
+    lat.close()
+
+
 # ---- full BASELINE sizes, in the launch configuration bench.py times ---------------------------------
 @pytest.mark.parametrize("L", [(32, 32, 32, 32), (48, 48, 48, 48)])
 @pytest.mark.parametrize("recon", [18, 12])
