@@ -1,7 +1,9 @@
 /* lqcd.h -- C ABI of the B200 staggered-fermion hot path (even/odd Dslash + multi-shift CG).
  *
  * Source of the operations: arxiv/paper_1801_01473, "Portable multi-node LQCD Monte Carlo simulations
- * using OpenACC".  The library implements, for ONE GPU (sm_100a), in double precision:
+ * using OpenACC".  The library implements, for ONE GPU (sm_100a), in double precision (and, through
+ * the *_f32 entry points, in single precision: the paper keeps its fields as "double (or float) C99 complex
+ * numbers", and runs the MD evolution in single precision):
  *
  *   D_oe, D_eo   the off-diagonal even/odd blocks of the staggered Dirac matrix (the
  *                hopping term between x and x+mu is proportional to U_mu(x); D_oe^dagger = -D_eo), with
@@ -75,6 +77,11 @@ typedef struct lqcd_ctx lqcd_ctx;
 #define LQCD_OPT_CHECK_EVERY     4  /* the host looks at the device-side stop flag every this many
                                        iterations; default 0 = chosen from the lattice size                */
 #define LQCD_OPT_USE_GRAPH       5  /* 1 (default): replay the CG iteration as a CUDA graph; 0: plain launches */
+#define LQCD_OPT_LINK_PRECISIONS 6  /* which copies of the links the next lqcd_set_gauge stores: LQCD_PREC_F64
+                                       (default; serves the double entry points), LQCD_PREC_F32 (serves the
+                                       *_f32 entry points), or both OR-ed together                         */
+#define LQCD_PREC_F64 1
+#define LQCD_PREC_F32 2
 
 /* statistic keys for lqcd_get_stat (about the last lqcd_mshift_cg on this context) */
 #define LQCD_STAT_ITERS          0  /* number of iterations performed                                     */
@@ -117,6 +124,16 @@ int lqcd_deo_host(lqcd_ctx* ctx, double* out_even /*HOST*/, const double* in_odd
  * paper's D_oe, D_eo, zaxpy sequence in two launches. */
 int lqcd_mdagm(lqcd_ctx* ctx, double* out_even, const double* in_even, double sigma);
 
+/* Single precision: the same operators on float parity vectors (3*Vh complex floats,
+ * same index order) with the links stored as floats (LQCD_OPT_LINK_PRECISIONS must include LQCD_PREC_F32 at
+ * lqcd_set_gauge time, otherwise LQCD_ENOGAUGE).  Arithmetic is float; only the CG's scalar products and
+ * scalar recurrences are kept in double. */
+int lqcd_doe_f32(lqcd_ctx* ctx, float* out_odd, const float* in_even);
+int lqcd_deo_f32(lqcd_ctx* ctx, float* out_even, const float* in_odd);
+int lqcd_doe_f32_host(lqcd_ctx* ctx, float* out_odd /*HOST*/, const float* in_even /*HOST*/);
+int lqcd_deo_f32_host(lqcd_ctx* ctx, float* out_even /*HOST*/, const float* in_odd /*HOST*/);
+int lqcd_mdagm_f32(lqcd_ctx* ctx, float* out_even, const float* in_even, double sigma);
+
 /* Multi-shift CG for (m^2 - D_eo D_oe + shifts[i]) x[i] = b, i = 0..nshift-1, zero
  * initial guess, base system = smallest shift, stop when |r| <= tol*|b| for the base system, shift i is
  * frozen once zeta_i*|r| <= tol*|b| (readings R5-R7).
@@ -128,6 +145,14 @@ int lqcd_mshift_cg(lqcd_ctx* ctx, const double* b_even, const double* shifts /*H
 /* Same, b and every x[i] in HOST memory; copies are part of the call. */
 int lqcd_mshift_cg_host(lqcd_ctx* ctx, const double* b_even /*HOST*/, const double* shifts /*HOST*/,
                         int nshift, double tol, double* const* x /*HOST array of HOST pointers*/);
+
+/* Single-precision multi-shift CG: float vectors and links, float sweeps; the scalar products are summed and
+ * the recurrences run in double.  tol is limited by the arithmetic (the recurrence residual of a float CG
+ * stops following the true residual around 1e-6..1e-5 relative for these condition numbers). */
+int lqcd_mshift_cg_f32(lqcd_ctx* ctx, const float* b_even, const double* shifts /*HOST*/, int nshift,
+                       double tol, float* const* x /*HOST array of DEVICE pointers*/);
+int lqcd_mshift_cg_f32_host(lqcd_ctx* ctx, const float* b_even /*HOST*/, const double* shifts /*HOST*/,
+                            int nshift, double tol, float* const* x /*HOST array of HOST pointers*/);
 
 /* Rational function of the Eq. 2 operator applied to b,
  *     y = alpha0 b + sum_i alpha[i] (m^2 - D_eo D_oe + shifts[i])^{-1} b ,
@@ -144,6 +169,9 @@ int lqcd_rational_apply(lqcd_ctx* ctx, const double* b_even, double alpha0, cons
 int lqcd_rational_apply_host(lqcd_ctx* ctx, const double* b_even /*HOST*/, double alpha0, const double* alpha /*HOST*/,
                              const double* shifts /*HOST*/, int nshift, double tol, double* y_even /*HOST*/);
 
+int lqcd_rational_apply_f32(lqcd_ctx* ctx, const float* b_even, double alpha0, const double* alpha /*HOST*/,
+                            const double* shifts /*HOST*/, int nshift, double tol, float* y_even);
+
 /* Statistics of the last solve; *out is HOST. idx is used by LQCD_STAT_FREEZE_ITER only. */
 int lqcd_get_stat(const lqcd_ctx* ctx, int key, int idx, double* out /*HOST*/);
 
@@ -151,6 +179,8 @@ int lqcd_get_stat(const lqcd_ctx* ctx, int key, int idx, double* out /*HOST*/);
  * pack reads only the sites of `parity`; unpack writes only those sites. */
 int lqcd_pack_vector(lqcd_ctx* ctx, int parity, const double* site_field, double* parity_vector);
 int lqcd_unpack_vector(lqcd_ctx* ctx, int parity, const double* parity_vector, double* site_field);
+int lqcd_pack_vector_f32(lqcd_ctx* ctx, int parity, const float* site_field, float* parity_vector);
+int lqcd_unpack_vector_f32(lqcd_ctx* ctx, int parity, const float* parity_vector, float* site_field);
 
 const char* lqcd_last_error(const lqcd_ctx* ctx);
 

@@ -11,7 +11,7 @@ takes torch tensors (device memory and streams are torch's job, nothing else is)
 from .binding import (  # noqa: F401
     LQCD_OK, LQCD_EINVAL, LQCD_ENOGAUGE, LQCD_ENOMEM, LQCD_ECUDA, LQCD_ENOCONV, LQCD_EBREAKDOWN, LQCD_ENOTSU3,
     LQCD_OPT_MASS, LQCD_OPT_ANTIPERIODIC_T, LQCD_OPT_RECON, LQCD_OPT_MAX_ITER, LQCD_OPT_CHECK_EVERY,
-    LQCD_OPT_USE_GRAPH,
+    LQCD_OPT_USE_GRAPH, LQCD_OPT_LINK_PRECISIONS, LQCD_PREC_F64, LQCD_PREC_F32,
     LQCD_STAT_ITERS, LQCD_STAT_REL_RES, LQCD_STAT_FREEZE_ITER, LQCD_STAT_BASE_SHIFT, LQCD_STAT_GPU_LAUNCHES,
     LQCD_STAT_SOLVE_MS,
     LqcdError, Lattice, load_library, library_path, EXPORTS,
@@ -19,4 +19,6 @@ from .binding import (  # noqa: F401
     lqcd_set_workspace, lqcd_set_gauge, lqcd_set_gauge_host, lqcd_doe, lqcd_deo, lqcd_doe_host, lqcd_deo_host,
     lqcd_mdagm, lqcd_mshift_cg, lqcd_mshift_cg_host, lqcd_rational_apply, lqcd_rational_apply_host, lqcd_get_stat, lqcd_pack_vector, lqcd_unpack_vector,
     lqcd_last_error,
+    lqcd_doe_f32, lqcd_deo_f32, lqcd_doe_f32_host, lqcd_deo_f32_host, lqcd_mdagm_f32, lqcd_mshift_cg_f32,
+    lqcd_mshift_cg_f32_host, lqcd_rational_apply_f32, lqcd_pack_vector_f32, lqcd_unpack_vector_f32,
 )

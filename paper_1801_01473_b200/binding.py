@@ -11,7 +11,8 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 LQCD_OK, LQCD_EINVAL, LQCD_ENOGAUGE, LQCD_ENOMEM, LQCD_ECUDA = 0, -1, -2, -3, -4
 LQCD_ENOCONV, LQCD_EBREAKDOWN, LQCD_ENOTSU3 = -5, -6, -7
 LQCD_OPT_MASS, LQCD_OPT_ANTIPERIODIC_T, LQCD_OPT_RECON, LQCD_OPT_MAX_ITER = 0, 1, 2, 3
-LQCD_OPT_CHECK_EVERY, LQCD_OPT_USE_GRAPH = 4, 5
+LQCD_OPT_CHECK_EVERY, LQCD_OPT_USE_GRAPH, LQCD_OPT_LINK_PRECISIONS = 4, 5, 6
+LQCD_PREC_F64, LQCD_PREC_F32 = 1, 2
 LQCD_STAT_ITERS, LQCD_STAT_REL_RES, LQCD_STAT_FREEZE_ITER, LQCD_STAT_BASE_SHIFT = 0, 1, 2, 3
 LQCD_STAT_GPU_LAUNCHES, LQCD_STAT_SOLVE_MS = 4, 5
 
@@ -41,9 +42,19 @@ EXPORTS = {
     "lqcd_mshift_cg_host": (_i, [_vp, _dp, _pd, _i, _d, ctypes.POINTER(ctypes.c_void_p)]),
     "lqcd_rational_apply": (_i, [_vp, _dp, _d, _pd, _pd, _i, _d, _dp]),
     "lqcd_rational_apply_host": (_i, [_vp, _dp, _d, _pd, _pd, _i, _d, _dp]),
+    "lqcd_doe_f32": (_i, [_vp, _dp, _dp]),
+    "lqcd_deo_f32": (_i, [_vp, _dp, _dp]),
+    "lqcd_doe_f32_host": (_i, [_vp, _dp, _dp]),
+    "lqcd_deo_f32_host": (_i, [_vp, _dp, _dp]),
+    "lqcd_mdagm_f32": (_i, [_vp, _dp, _dp, _d]),
+    "lqcd_mshift_cg_f32": (_i, [_vp, _dp, _pd, _i, _d, ctypes.POINTER(ctypes.c_void_p)]),
+    "lqcd_mshift_cg_f32_host": (_i, [_vp, _dp, _pd, _i, _d, ctypes.POINTER(ctypes.c_void_p)]),
+    "lqcd_rational_apply_f32": (_i, [_vp, _dp, _d, _pd, _pd, _i, _d, _dp]),
     "lqcd_get_stat": (_i, [_vp, _i, _i, _pd]),
     "lqcd_pack_vector": (_i, [_vp, _i, _dp, _dp]),
     "lqcd_unpack_vector": (_i, [_vp, _i, _dp, _dp]),
+    "lqcd_pack_vector_f32": (_i, [_vp, _i, _dp, _dp]),
+    "lqcd_unpack_vector_f32": (_i, [_vp, _i, _dp, _dp]),
     "lqcd_last_error": (ctypes.c_char_p, [_vp]),
 }
 
@@ -138,6 +149,26 @@ def lqcd_mdagm(ctx, out_even, in_even, sigma):
     return load_library().lqcd_mdagm(ctx, out_even, in_even, float(sigma))
 
 
+def lqcd_doe_f32(ctx, out_odd, in_even):
+    return load_library().lqcd_doe_f32(ctx, out_odd, in_even)
+
+
+def lqcd_deo_f32(ctx, out_even, in_odd):
+    return load_library().lqcd_deo_f32(ctx, out_even, in_odd)
+
+
+def lqcd_doe_f32_host(ctx, out_odd, in_even):
+    return load_library().lqcd_doe_f32_host(ctx, out_odd, in_even)
+
+
+def lqcd_deo_f32_host(ctx, out_even, in_odd):
+    return load_library().lqcd_deo_f32_host(ctx, out_even, in_odd)
+
+
+def lqcd_mdagm_f32(ctx, out_even, in_even, sigma):
+    return load_library().lqcd_mdagm_f32(ctx, out_even, in_even, float(sigma))
+
+
 def _cg_args(shifts, x_ptrs):
     n = len(shifts)
     sh = (ctypes.c_double * n)(*[float(s) for s in shifts])
@@ -155,14 +186,32 @@ def lqcd_mshift_cg_host(ctx, b_even, shifts: Sequence[float], tol: float, x_ptrs
     return load_library().lqcd_mshift_cg_host(ctx, b_even, sh, n, float(tol), xs)
 
 
-def lqcd_rational_apply(ctx, b_even, alpha0: float, alpha: Sequence[float], shifts: Sequence[float], tol: float,
-                        y_even, host: bool = False):
+def lqcd_mshift_cg_f32(ctx, b_even, shifts: Sequence[float], tol: float, x_ptrs: Sequence[int]):
+    n, sh, xs = _cg_args(shifts, x_ptrs)
+    return load_library().lqcd_mshift_cg_f32(ctx, b_even, sh, n, float(tol), xs)
+
+
+def lqcd_mshift_cg_f32_host(ctx, b_even, shifts: Sequence[float], tol: float, x_ptrs: Sequence[int]):
+    n, sh, xs = _cg_args(shifts, x_ptrs)
+    return load_library().lqcd_mshift_cg_f32_host(ctx, b_even, sh, n, float(tol), xs)
+
+
+def _rational(name, ctx, b_even, alpha0, alpha, shifts, tol, y_even):
     n = len(shifts)
     assert len(alpha) == n
     al = (ctypes.c_double * n)(*[float(a) for a in alpha])
     sh = (ctypes.c_double * n)(*[float(s) for s in shifts])
-    fn = load_library().lqcd_rational_apply_host if host else load_library().lqcd_rational_apply
-    return fn(ctx, b_even, float(alpha0), al, sh, n, float(tol), y_even)
+    return getattr(load_library(), name)(ctx, b_even, float(alpha0), al, sh, n, float(tol), y_even)
+
+
+def lqcd_rational_apply(ctx, b_even, alpha0: float, alpha: Sequence[float], shifts: Sequence[float], tol: float,
+                        y_even, host: bool = False):
+    return _rational("lqcd_rational_apply_host" if host else "lqcd_rational_apply", ctx, b_even, alpha0, alpha,
+                     shifts, tol, y_even)
+
+
+def lqcd_rational_apply_f32(ctx, b_even, alpha0, alpha, shifts, tol, y_even):
+    return _rational("lqcd_rational_apply_f32", ctx, b_even, alpha0, alpha, shifts, tol, y_even)
 
 
 def lqcd_rational_apply_host(ctx, b_even, alpha0, alpha, shifts, tol, y_even):
@@ -183,6 +232,14 @@ def lqcd_unpack_vector(ctx, parity, parity_vector, site_field):
     return load_library().lqcd_unpack_vector(ctx, int(parity), parity_vector, site_field)
 
 
+def lqcd_pack_vector_f32(ctx, parity, site_field, parity_vector):
+    return load_library().lqcd_pack_vector_f32(ctx, int(parity), site_field, parity_vector)
+
+
+def lqcd_unpack_vector_f32(ctx, parity, parity_vector, site_field):
+    return load_library().lqcd_unpack_vector_f32(ctx, int(parity), parity_vector, site_field)
+
+
 def lqcd_last_error(ctx) -> str:
     s = load_library().lqcd_last_error(ctx)
     return s.decode() if s else ""
@@ -190,10 +247,13 @@ def lqcd_last_error(ctx) -> str:
 
 # ---- torch-tensor convenience wrapper ------------------------------------------------------------------
 class Lattice:
-    """One lqcd_ctx.  Tensors are float64; device tensors go to the device entry points on torch's
-    current stream, CPU tensors go to the ``*_host`` entry points (the copies happen inside the call)."""
+    """One lqcd_ctx.  float64 tensors go to the double entry points, float32 tensors to the ``*_f32`` ones
+    (``precisions`` says which copies of the links ``set_gauge`` stores); device tensors go to the device
+    entry points on torch's current stream, CPU tensors to the ``*_host`` entry points (the copies happen
+    inside the call)."""
 
-    def __init__(self, L: Sequence[int], mass: float = 0.0, antiperiodic: bool = True, recon: int = 18):
+    def __init__(self, L: Sequence[int], mass: float = 0.0, antiperiodic: bool = True, recon: int = 18,
+                 precisions: int = LQCD_PREC_F64):
         import torch
         if not torch.cuda.is_available():
             raise RuntimeError("paper_1801_01473_b200 needs a CUDA device (there is no CPU fallback)")
@@ -207,6 +267,7 @@ class Lattice:
         self.set_option(LQCD_OPT_MASS, mass)
         self.set_option(LQCD_OPT_ANTIPERIODIC_T, 1.0 if antiperiodic else 0.0)
         self.set_option(LQCD_OPT_RECON, recon)
+        self.set_option(LQCD_OPT_LINK_PRECISIONS, precisions)
 
     def close(self):
         if getattr(self, "ctx", None):
@@ -228,17 +289,23 @@ class Lattice:
     def _sync_stream(self):
         self._check(lqcd_set_stream(self.ctx, self._torch.cuda.current_stream().cuda_stream))
 
-    def _t(self, t, shape, device_type=None):
+    def _t(self, t, shape, device_type=None, dtype=None):
         torch = self._torch
-        assert t.dtype == torch.float64 and t.is_contiguous(), "float64 contiguous tensor expected"
+        dtype = torch.float64 if dtype is None else dtype
+        assert t.dtype == dtype and t.is_contiguous(), f"{dtype} contiguous tensor expected"
         assert tuple(t.shape) == tuple(shape), f"shape {tuple(t.shape)} != {tuple(shape)}"
         if device_type is not None:
             assert t.device.type == device_type
         return t.data_ptr()
 
-    def new_vector(self, n: Optional[int] = None):
+    def _f32(self, t) -> bool:
+        torch = self._torch
+        assert t.dtype in (torch.float64, torch.float32), "float64 or float32 tensor expected"
+        return t.dtype == torch.float32
+
+    def new_vector(self, n: Optional[int] = None, dtype=None):
         shape = (3, self.Vh, 2) if n is None else (n, 3, self.Vh, 2)
-        return self._torch.empty(shape, dtype=self._torch.float64, device="cuda")
+        return self._torch.empty(shape, dtype=dtype or self._torch.float64, device="cuda")
 
     # -- options / stats
     def set_option(self, key, value):
@@ -268,46 +335,50 @@ class Lattice:
         else:
             self._check(lqcd_set_gauge_host(self.ctx, p))
 
-    def _apply(self, fn_dev, fn_host, v, out):
+    def _apply(self, fns, v, out):
         torch = self._torch
-        pin = self._t(v, (3, self.Vh, 2))
+        f32 = self._f32(v)
+        pin = self._t(v, (3, self.Vh, 2), dtype=v.dtype)
         if out is None:
             out = torch.empty_like(v)
-        pout = self._t(out, (3, self.Vh, 2), v.device.type)
+        pout = self._t(out, (3, self.Vh, 2), v.device.type, v.dtype)
         self._sync_stream()
-        self._check((fn_dev if v.device.type == "cuda" else fn_host)(self.ctx, pout, pin))
+        self._check(fns[2 * f32 + (v.device.type != "cuda")](self.ctx, pout, pin))
         return out
 
     def doe(self, v_even, out=None):
         """D_oe: even -> odd parity vector."""
-        return self._apply(lqcd_doe, lqcd_doe_host, v_even, out)
+        return self._apply((lqcd_doe, lqcd_doe_host, lqcd_doe_f32, lqcd_doe_f32_host), v_even, out)
 
     def deo(self, v_odd, out=None):
         """D_eo: odd -> even parity vector."""
-        return self._apply(lqcd_deo, lqcd_deo_host, v_odd, out)
+        return self._apply((lqcd_deo, lqcd_deo_host, lqcd_deo_f32, lqcd_deo_f32_host), v_odd, out)
 
     def mdagm(self, v_even, sigma: float = 0.0, out=None):
         """(m^2 + sigma) v - D_eo D_oe v."""
-        pin = self._t(v_even, (3, self.Vh, 2), "cuda")
+        f32 = self._f32(v_even)
+        pin = self._t(v_even, (3, self.Vh, 2), "cuda", v_even.dtype)
         if out is None:
             out = self._torch.empty_like(v_even)
-        pout = self._t(out, (3, self.Vh, 2), "cuda")
+        pout = self._t(out, (3, self.Vh, 2), "cuda", v_even.dtype)
         self._sync_stream()
-        self._check(lqcd_mdagm(self.ctx, pout, pin, sigma))
+        self._check((lqcd_mdagm_f32 if f32 else lqcd_mdagm)(self.ctx, pout, pin, sigma))
         return out
 
     def mshift_cg(self, b_even, shifts: Sequence[float], tol: float, x=None, raise_on_noconv: bool = True):
         """Solve (m^2 - D_eo D_oe + shifts[i]) x[i] = b.  Returns (x, info); x is (nshift, 3, Vh, 2)."""
         torch = self._torch
         n = len(shifts)
-        pb = self._t(b_even, (3, self.Vh, 2))
+        f32 = self._f32(b_even)
+        pb = self._t(b_even, (3, self.Vh, 2), dtype=b_even.dtype)
         if x is None:
-            x = torch.empty((n, 3, self.Vh, 2), dtype=torch.float64, device=b_even.device,
+            x = torch.empty((n, 3, self.Vh, 2), dtype=b_even.dtype, device=b_even.device,
                             pin_memory=(b_even.device.type == "cpu"))
-        self._t(x, (n, 3, self.Vh, 2), b_even.device.type)
+        self._t(x, (n, 3, self.Vh, 2), b_even.device.type, b_even.dtype)
         ptrs = [x[i].data_ptr() for i in range(n)]
         self._sync_stream()
-        fn = lqcd_mshift_cg if b_even.device.type == "cuda" else lqcd_mshift_cg_host
+        fn = (lqcd_mshift_cg, lqcd_mshift_cg_host, lqcd_mshift_cg_f32, lqcd_mshift_cg_f32_host)[
+            2 * f32 + (b_even.device.type != "cuda")]
         rc = fn(self.ctx, pb, shifts, tol, ptrs)
         self._check(rc, allow=() if raise_on_noconv else (LQCD_ENOCONV,))
         return x, self._solve_info(rc, n)
@@ -327,30 +398,39 @@ class Lattice:
         """y = alpha0 b + sum_i alpha_i (m^2 - D_eo D_oe + shifts[i])^-1 b, accumulated
         during the multi-shift solve.  Returns (y, info)."""
         torch = self._torch
-        pb = self._t(b_even, (3, self.Vh, 2))
+        f32 = self._f32(b_even)
+        pb = self._t(b_even, (3, self.Vh, 2), dtype=b_even.dtype)
         host = b_even.device.type == "cpu"
+        assert not (f32 and host), "no host entry point for the single-precision rational sum"
         if y is None:
-            y = torch.empty((3, self.Vh, 2), dtype=torch.float64, device=b_even.device, pin_memory=host)
-        py = self._t(y, (3, self.Vh, 2), b_even.device.type)
+            y = torch.empty((3, self.Vh, 2), dtype=b_even.dtype, device=b_even.device, pin_memory=host)
+        py = self._t(y, (3, self.Vh, 2), b_even.device.type, b_even.dtype)
         self._sync_stream()
-        rc = lqcd_rational_apply(self.ctx, pb, alpha0, alpha, shifts, tol, py, host=host)
+        if f32:
+            rc = lqcd_rational_apply_f32(self.ctx, pb, alpha0, alpha, shifts, tol, py)
+        else:
+            rc = lqcd_rational_apply(self.ctx, pb, alpha0, alpha, shifts, tol, py, host=host)
         self._check(rc, allow=() if raise_on_noconv else (LQCD_ENOCONV,))
         return y, self._solve_info(rc, len(shifts))
 
     def pack(self, site_field, parity: int, out=None):
         """(V,3,2) site field -> (3,Vh,2) parity vector of the given parity."""
-        ps = self._t(site_field, (self.V, 3, 2), "cuda")
+        f32 = self._f32(site_field)
+        ps = self._t(site_field, (self.V, 3, 2), "cuda", site_field.dtype)
         if out is None:
-            out = self.new_vector()
+            out = self.new_vector(dtype=site_field.dtype)
         self._sync_stream()
-        self._check(lqcd_pack_vector(self.ctx, parity, ps, self._t(out, (3, self.Vh, 2), "cuda")))
+        fn = lqcd_pack_vector_f32 if f32 else lqcd_pack_vector
+        self._check(fn(self.ctx, parity, ps, self._t(out, (3, self.Vh, 2), "cuda", site_field.dtype)))
         return out
 
     def unpack(self, v, parity: int, out=None):
         """(3,Vh,2) parity vector -> (V,3,2) site field (other parity zero unless `out` is given)."""
-        pv = self._t(v, (3, self.Vh, 2), "cuda")
+        f32 = self._f32(v)
+        pv = self._t(v, (3, self.Vh, 2), "cuda", v.dtype)
         if out is None:
-            out = self._torch.zeros((self.V, 3, 2), dtype=self._torch.float64, device="cuda")
+            out = self._torch.zeros((self.V, 3, 2), dtype=v.dtype, device="cuda")
         self._sync_stream()
-        self._check(lqcd_unpack_vector(self.ctx, parity, pv, self._t(out, (self.V, 3, 2), "cuda")))
+        fn = lqcd_unpack_vector_f32 if f32 else lqcd_unpack_vector
+        self._check(fn(self.ctx, parity, pv, self._t(out, (self.V, 3, 2), "cuda", v.dtype)))
         return out

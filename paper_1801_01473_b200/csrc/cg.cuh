@@ -15,28 +15,29 @@
 
 #define CG_BLOCK 256
 
-// K0: r = p_i = b, x_i = 0, |b|^2
-__global__ void __launch_bounds__(CG_BLOCK) cg_init_kernel(const double2* __restrict__ b, double2* __restrict__ r,
+// K0: r = p_i = b, x_i = 0, |b|^2.  In every sweep the vectors are V2<T>; scalars and sums are double.
+template <typename T>
+__global__ void __launch_bounds__(CG_BLOCK) cg_init_kernel(const V2<T>* __restrict__ b, V2<T>* __restrict__ r,
                                                            CgState* st, double* partials, size_t n, double tol) {
     __shared__ double red[32];
     __shared__ int last_flag;
     const int ns = st->nshift;
     const int rational = st->rational;
-    const double alpha0 = st->alpha0;
-    double2* __restrict__ y = st->y;
+    const T alpha0 = (T)st->alpha0;
+    V2<T>* __restrict__ y = (V2<T>*)st->y;
     double acc = 0.0;
-    const double2 zero = make_double2(0.0, 0.0);
+    const V2<T> zero = make_v2((T)0, (T)0);
     for (size_t j = (size_t)blockIdx.x * CG_BLOCK + threadIdx.x; j < n; j += (size_t)gridDim.x * CG_BLOCK) {
-        const double2 v = b[j];
+        const V2<T> v = b[j];
         r[j] = v;
-        for (int i = 0; i < ns; ++i) st->p[i][j] = v;
+        for (int i = 0; i < ns; ++i) ((V2<T>*)st->p[i])[j] = v;
         if (rational) {
-            y[j] = make_double2(alpha0 * v.x, alpha0 * v.y);
+            y[j] = make_v2(alpha0 * v.x, alpha0 * v.y);
         } else {
-            for (int i = 0; i < ns; ++i) st->x[i][j] = zero;
+            for (int i = 0; i < ns; ++i) ((V2<T>*)st->x[i])[j] = zero;
         }
-        acc = fma(v.x, v.x, acc);
-        acc = fma(v.y, v.y, acc);
+        acc = fma((double)v.x, (double)v.x, acc);
+        acc = fma((double)v.y, (double)v.y, acc);
     }
     const double bsum = block_sum<CG_BLOCK>(acc, red);
     if (publish_partial<CG_BLOCK>(bsum, partials, &st->ticket[0], &last_flag)) {
@@ -49,17 +50,18 @@ __global__ void __launch_bounds__(CG_BLOCK) cg_init_kernel(const double2* __rest
 }
 
 // K3: r -= a s, |r|^2, then the scalar step that needs it
-__global__ void __launch_bounds__(CG_BLOCK) cg_update_r_kernel(double2* __restrict__ r, const double2* __restrict__ s,
+template <typename T>
+__global__ void __launch_bounds__(CG_BLOCK) cg_update_r_kernel(V2<T>* __restrict__ r, const V2<T>* __restrict__ s,
                                                                CgState* st, double* partials, size_t n) {
     if (st->stop) return;
     __shared__ double red[32];
     __shared__ int last_flag;
-    const double a = st->a;
+    const T a = (T)st->a;
     double acc = 0.0;
     const size_t stride = (size_t)gridDim.x * CG_BLOCK;
     size_t j = (size_t)blockIdx.x * CG_BLOCK + threadIdx.x;
     for (; j + 3 * stride < n; j += 4 * stride) {
-        double2 rv[4], sv[4];
+        V2<T> rv[4], sv[4];
 #pragma unroll
         for (int u = 0; u < 4; ++u) {
             rv[u] = r[j + u * stride];
@@ -70,18 +72,18 @@ __global__ void __launch_bounds__(CG_BLOCK) cg_update_r_kernel(double2* __restri
             rv[u].x = fma(-a, sv[u].x, rv[u].x);
             rv[u].y = fma(-a, sv[u].y, rv[u].y);
             r[j + u * stride] = rv[u];
-            acc = fma(rv[u].x, rv[u].x, acc);
-            acc = fma(rv[u].y, rv[u].y, acc);
+            acc = fma((double)rv[u].x, (double)rv[u].x, acc);
+            acc = fma((double)rv[u].y, (double)rv[u].y, acc);
         }
     }
     for (; j < n; j += stride) {
-        double2 rv = r[j];
-        const double2 sv = s[j];
+        V2<T> rv = r[j];
+        const V2<T> sv = s[j];
         rv.x = fma(-a, sv.x, rv.x);
         rv.y = fma(-a, sv.y, rv.y);
         r[j] = rv;
-        acc = fma(rv.x, rv.x, acc);
-        acc = fma(rv.y, rv.y, acc);
+        acc = fma((double)rv.x, (double)rv.x, acc);
+        acc = fma((double)rv.y, (double)rv.y, acc);
     }
     const double bsum = block_sum<CG_BLOCK>(acc, red);
     if (publish_partial<CG_BLOCK>(bsum, partials, &st->ticket[2], &last_flag)) {
@@ -94,27 +96,28 @@ __global__ void __launch_bounds__(CG_BLOCK) cg_update_r_kernel(double2* __restri
 }
 
 // K4: x_i += a_i p_i ; p_i = zeta_new_i r + b_i p_i   for the shifts on this iteration's list
-__global__ void __launch_bounds__(CG_BLOCK) cg_update_xp_kernel(const double2* __restrict__ r, const CgState* st, size_t n) {
+template <typename T>
+__global__ void __launch_bounds__(CG_BLOCK) cg_update_xp_kernel(const V2<T>* __restrict__ r, const CgState* st, size_t n) {
     if (st->stop4) return;
-    __shared__ double2* sx[LQCD_MAX_SHIFTS];
-    __shared__ double2* sp[LQCD_MAX_SHIFTS];
-    __shared__ double sa[LQCD_MAX_SHIFTS], sz[LQCD_MAX_SHIFTS], sb[LQCD_MAX_SHIFTS];
+    __shared__ V2<T>* sx[LQCD_MAX_SHIFTS];
+    __shared__ V2<T>* sp[LQCD_MAX_SHIFTS];
+    __shared__ T sa[LQCD_MAX_SHIFTS], sz[LQCD_MAX_SHIFTS], sb[LQCD_MAX_SHIFTS];
     const int nl = st->nlist;
     for (int e = threadIdx.x; e < nl; e += CG_BLOCK) {
         const int i = st->list_idx[e];
-        sx[e] = st->x[i];
-        sp[e] = st->p[i];
-        sa[e] = st->list_a[e];
-        sz[e] = st->list_zn[e];
-        sb[e] = st->list_b[e];
+        sx[e] = (V2<T>*)st->x[i];
+        sp[e] = (V2<T>*)st->p[i];
+        sa[e] = (T)st->list_a[e];
+        sz[e] = (T)st->list_zn[e];
+        sb[e] = (T)st->list_b[e];
     }
     __syncthreads();
     const size_t stride = (size_t)gridDim.x * CG_BLOCK;
     for (size_t j = (size_t)blockIdx.x * CG_BLOCK + threadIdx.x; j < n; j += stride) {
-        const double2 rv = r[j];
+        const V2<T> rv = r[j];
         int e = 0;
         for (; e + 4 <= nl; e += 4) {
-            double2 xv[4], pv[4];
+            V2<T> xv[4], pv[4];
 #pragma unroll
             for (int u = 0; u < 4; ++u) {
                 xv[u] = sx[e + u][j];
@@ -122,7 +125,7 @@ __global__ void __launch_bounds__(CG_BLOCK) cg_update_xp_kernel(const double2* _
             }
 #pragma unroll
             for (int u = 0; u < 4; ++u) {
-                const double a = sa[e + u], zn = sz[e + u], bi = sb[e + u];
+                const T a = sa[e + u], zn = sz[e + u], bi = sb[e + u];
                 xv[u].x = fma(a, pv[u].x, xv[u].x);
                 xv[u].y = fma(a, pv[u].y, xv[u].y);
                 pv[u].x = fma(zn, rv.x, bi * pv[u].x);
@@ -132,8 +135,8 @@ __global__ void __launch_bounds__(CG_BLOCK) cg_update_xp_kernel(const double2* _
             }
         }
         for (; e < nl; ++e) {
-            double2 xv = sx[e][j], pv = sp[e][j];
-            const double a = sa[e], zn = sz[e], bi = sb[e];
+            V2<T> xv = sx[e][j], pv = sp[e][j];
+            const T a = sa[e], zn = sz[e], bi = sb[e];
             xv.x = fma(a, pv.x, xv.x);
             xv.y = fma(a, pv.y, xv.y);
             pv.x = fma(zn, rv.x, bi * pv.x);
@@ -146,31 +149,32 @@ __global__ void __launch_bounds__(CG_BLOCK) cg_update_xp_kernel(const double2* _
 
 // K4 of lqcd_rational_apply: y += sum_i (alpha_i a_i) p_i ; p_i = zeta_new_i r + b_i p_i.  The x_i are never
 // stored: 96 B per site and active shift instead of 192 (the sum is taken in list order, per element).
-__global__ void __launch_bounds__(CG_BLOCK) cg_update_yp_kernel(const double2* __restrict__ r, const CgState* st, size_t n) {
+template <typename T>
+__global__ void __launch_bounds__(CG_BLOCK) cg_update_yp_kernel(const V2<T>* __restrict__ r, const CgState* st, size_t n) {
     if (st->stop4) return;
-    __shared__ double2* sp[LQCD_MAX_SHIFTS];
-    __shared__ double sa[LQCD_MAX_SHIFTS], sz[LQCD_MAX_SHIFTS], sb[LQCD_MAX_SHIFTS];
+    __shared__ V2<T>* sp[LQCD_MAX_SHIFTS];
+    __shared__ T sa[LQCD_MAX_SHIFTS], sz[LQCD_MAX_SHIFTS], sb[LQCD_MAX_SHIFTS];
     const int nl = st->nlist;
     for (int e = threadIdx.x; e < nl; e += CG_BLOCK) {
-        sp[e] = st->p[st->list_idx[e]];
-        sa[e] = st->list_a[e];
-        sz[e] = st->list_zn[e];
-        sb[e] = st->list_b[e];
+        sp[e] = (V2<T>*)st->p[st->list_idx[e]];
+        sa[e] = (T)st->list_a[e];
+        sz[e] = (T)st->list_zn[e];
+        sb[e] = (T)st->list_b[e];
     }
     __syncthreads();
-    double2* __restrict__ y = st->y;
+    V2<T>* __restrict__ y = (V2<T>*)st->y;
     const size_t stride = (size_t)gridDim.x * CG_BLOCK;
     for (size_t j = (size_t)blockIdx.x * CG_BLOCK + threadIdx.x; j < n; j += stride) {
-        const double2 rv = r[j];
-        double2 yv = y[j];
+        const V2<T> rv = r[j];
+        V2<T> yv = y[j];
         int e = 0;
         for (; e + 4 <= nl; e += 4) {
-            double2 pv[4];
+            V2<T> pv[4];
 #pragma unroll
             for (int u = 0; u < 4; ++u) pv[u] = sp[e + u][j];
 #pragma unroll
             for (int u = 0; u < 4; ++u) {
-                const double a = sa[e + u], zn = sz[e + u], bi = sb[e + u];
+                const T a = sa[e + u], zn = sz[e + u], bi = sb[e + u];
                 yv.x = fma(a, pv[u].x, yv.x);
                 yv.y = fma(a, pv[u].y, yv.y);
                 pv[u].x = fma(zn, rv.x, bi * pv[u].x);
@@ -179,8 +183,8 @@ __global__ void __launch_bounds__(CG_BLOCK) cg_update_yp_kernel(const double2* _
             }
         }
         for (; e < nl; ++e) {
-            double2 pv = sp[e][j];
-            const double a = sa[e], zn = sz[e], bi = sb[e];
+            V2<T> pv = sp[e][j];
+            const T a = sa[e], zn = sz[e], bi = sb[e];
             yv.x = fma(a, pv.x, yv.x);
             yv.y = fma(a, pv.y, yv.y);
             pv.x = fma(zn, rv.x, bi * pv.x);
@@ -210,8 +214,9 @@ __device__ __forceinline__ void atomic_max_nonneg(double* addr, double v) {
 
 // canonical links[mu][lex][3][3] -> W[((mu*2+par)*NE + e)*Vh + k]; one thread per (mu, par, k).
 // With RECON=12 also records max |r2 - conj(r0 x r1)| over all links.
-template <int RECON>
-__global__ void __launch_bounds__(256) repack_gauge_kernel(Geom g, const double2* __restrict__ links, double2* __restrict__ W,
+// The input is always the double-precision canonical field; T is the precision it is stored in.
+template <typename T, int RECON>
+__global__ void __launch_bounds__(256) repack_gauge_kernel(Geom g, const double2* __restrict__ links, V2<T>* __restrict__ W,
                                                            double* __restrict__ dev_max) {
     constexpr int NE = (RECON == 12) ? 6 : 9;
     const size_t vh = (size_t)g.Vh;
@@ -226,7 +231,7 @@ __global__ void __launch_bounds__(256) repack_gauge_kernel(Geom g, const double2
 #pragma unroll
     for (int e = 0; e < 9; ++e) u[e] = src[e];
 #pragma unroll
-    for (int e = 0; e < NE; ++e) W[((size_t)mp * NE + e) * vh + k] = u[e];
+    for (int e = 0; e < NE; ++e) W[((size_t)mp * NE + e) * vh + k] = make_v2((T)u[e].x, (T)u[e].y);
     if (RECON == 12) {
         double dev = 0.0;
         const int ia[3] = {1, 2, 0}, ib[3] = {2, 0, 1};
@@ -247,19 +252,30 @@ __global__ void __launch_bounds__(256) repack_gauge_kernel(Geom g, const double2
 }
 
 // site field [lex][3] <-> parity vector [c][k]
-__global__ void __launch_bounds__(256) pack_vector_kernel(Geom g, int par, const double2* __restrict__ site, double2* __restrict__ pv) {
+template <typename T>
+__global__ void __launch_bounds__(256) pack_vector_kernel(Geom g, int par, const V2<T>* __restrict__ site, V2<T>* __restrict__ pv) {
     const int k = blockIdx.x * 256 + threadIdx.x;
     if (k >= g.Vh) return;
     const size_t lex = lex_of(g, k, par);
 #pragma unroll
     for (int c = 0; c < 3; ++c) pv[(size_t)c * g.Vh + k] = site[lex * 3 + c];
 }
-__global__ void __launch_bounds__(256) unpack_vector_kernel(Geom g, int par, const double2* __restrict__ pv, double2* __restrict__ site) {
+template <typename T>
+__global__ void __launch_bounds__(256) unpack_vector_kernel(Geom g, int par, const V2<T>* __restrict__ pv, V2<T>* __restrict__ site) {
     const int k = blockIdx.x * 256 + threadIdx.x;
     if (k >= g.Vh) return;
     const size_t lex = lex_of(g, k, par);
 #pragma unroll
     for (int c = 0; c < 3; ++c) site[lex * 3 + c] = pv[(size_t)c * g.Vh + k];
+}
+
+// precision conversion of a parity vector (n complex numbers)
+template <typename TO, typename FROM>
+__global__ void __launch_bounds__(256) convert_vector_kernel(const V2<FROM>* __restrict__ in, V2<TO>* __restrict__ out, size_t n) {
+    for (size_t j = (size_t)blockIdx.x * 256 + threadIdx.x; j < n; j += (size_t)gridDim.x * 256) {
+        const V2<FROM> v = in[j];
+        out[j] = make_v2((TO)v.x, (TO)v.y);
+    }
 }
 
 #endif

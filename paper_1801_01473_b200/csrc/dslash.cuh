@@ -2,7 +2,9 @@
 //
 //   out(x) = 1/2 sum_mu [ s_mu(x) U_mu(x) in(x+mu) - s_mu(x-mu) U_mu(x-mu)^+ in(x-mu) ]
 //
-// One thread per output site.  All traffic is 128-bit (double2) and unit-stride in the site index k:
+// One thread per output site, in double or single precision (template parameter T).
+// All traffic is one complex number per thread and instruction (128-bit double2 / 64-bit float2) and
+// unit-stride in the site index k:
 //   links   W[((mu*2 + parity_of_origin)*NE + e)*Vh + k],  e = 3*row+col, NE = 9 (18-real) or 6 (12-real)
 //   vectors v[c*Vh + k]
 // Neighbour indices, staggered phases eta_mu and the antiperiodic sign are computed in registers from
@@ -27,6 +29,9 @@
 #ifndef DS_MINB
 #define DS_MINB 4
 #endif
+#ifndef DS_MINB_F32
+#define DS_MINB_F32 6
+#endif
 #ifndef EPI_PLOAD
 #define EPI_PLOAD 1      // 0: load p in the epilogue, 1: load p into registers up front, 2: L2 prefetch up front
 #endif
@@ -50,6 +55,13 @@ __device__ __forceinline__ double2 ld_stream(const double2* p, uint64_t pol) {
         : "l"(p), "l"(pol));
     return v;
 }
+__device__ __forceinline__ float2 ld_stream(const float2* p, uint64_t pol) {
+    float2 v;
+    asm("ld.global.nc.L1::no_allocate.L2::cache_hint.v2.f32 {%0, %1}, [%2], %3;"
+        : "=f"(v.x), "=f"(v.y)
+        : "l"(p), "l"(pol));
+    return v;
+}
 // re-used by neighbouring sites: allocate in L1, last to leave L2
 __device__ __forceinline__ double2 ld_reuse(const double2* p, uint64_t pol) {
     double2 v;
@@ -58,100 +70,119 @@ __device__ __forceinline__ double2 ld_reuse(const double2* p, uint64_t pol) {
         : "l"(p), "l"(pol));
     return v;
 }
+__device__ __forceinline__ float2 ld_reuse(const float2* p, uint64_t pol) {
+    float2 v;
+    asm("ld.global.nc.L1::evict_last.L2::cache_hint.v2.f32 {%0, %1}, [%2], %3;"
+        : "=f"(v.x), "=f"(v.y)
+        : "l"(p), "l"(pol));
+    return v;
+}
 
-// x -> +-x by flipping the sign bit (mask is 0 or 0x80000000); integer pipe, not FP64
+// x -> +-x by flipping the sign bit (mask is 0 or 0x80000000); integer pipe, not the FP pipe
 __device__ __forceinline__ double flip(double x, unsigned int mask) {
     return __hiloint2double(__double2hiint(x) ^ (int)mask, __double2loint(x));
 }
+__device__ __forceinline__ float flip(float x, unsigned int mask) {
+    return __int_as_float(__float_as_int(x) ^ (int)mask);
+}
 
 // acc += u * v
-__device__ __forceinline__ void cmad(double& ar, double& ai, const double2 u, const double vr, const double vi) {
+template <typename T>
+__device__ __forceinline__ void cmad(T& ar, T& ai, const V2<T> u, const T vr, const T vi) {
     ar = fma(u.x, vr, ar);
     ar = fma(-u.y, vi, ar);
     ai = fma(u.x, vi, ai);
     ai = fma(u.y, vr, ai);
 }
 // acc += conj(u) * v
-__device__ __forceinline__ void cmad_conj(double& ar, double& ai, const double2 u, const double vr, const double vi) {
+template <typename T>
+__device__ __forceinline__ void cmad_conj(T& ar, T& ai, const V2<T> u, const T vr, const T vi) {
     ar = fma(u.x, vr, ar);
     ar = fma(u.y, vi, ar);
     ai = fma(u.x, vi, ai);
     ai = fma(-u.y, vr, ai);
 }
 
-__device__ __forceinline__ double2 cmul(const double2 a, const double2 b) {
-    return make_double2(a.x * b.x - a.y * b.y, a.x * b.y + a.y * b.x);
+template <typename V>
+__device__ __forceinline__ V cmul(const V a, const V b) {
+    return make_v2(a.x * b.x - a.y * b.y, a.x * b.y + a.y * b.x);
 }
 
 // Load one link (9 complex).  12-real storage: rows 0,1 are read, r2 = conj(r0 x r1).
-template <int RECON>
-__device__ __forceinline__ void load_link(const double2* __restrict__ w, const size_t vh, uint64_t pol, double2 (&u)[9]) {
+template <typename T, int RECON>
+__device__ __forceinline__ void load_link(const V2<T>* __restrict__ w, const size_t vh, uint64_t pol, V2<T> (&u)[9]) {
     constexpr int NE = (RECON == 12) ? 6 : 9;
 #pragma unroll
     for (int e = 0; e < NE; ++e) u[e] = ld_stream(w + e * vh, pol);
     if (RECON == 12) {
-        double2 c;
-        c = cmul(u[1], u[5]); { const double2 d = cmul(u[2], u[4]); u[6] = make_double2(c.x - d.x, -(c.y - d.y)); }
-        c = cmul(u[2], u[3]); { const double2 d = cmul(u[0], u[5]); u[7] = make_double2(c.x - d.x, -(c.y - d.y)); }
-        c = cmul(u[0], u[4]); { const double2 d = cmul(u[1], u[3]); u[8] = make_double2(c.x - d.x, -(c.y - d.y)); }
+        V2<T> c;
+        c = cmul(u[1], u[5]); { const V2<T> d = cmul(u[2], u[4]); u[6] = make_v2(c.x - d.x, -(c.y - d.y)); }
+        c = cmul(u[2], u[3]); { const V2<T> d = cmul(u[0], u[5]); u[7] = make_v2(c.x - d.x, -(c.y - d.y)); }
+        c = cmul(u[0], u[4]); { const V2<T> d = cmul(u[1], u[3]); u[8] = make_v2(c.x - d.x, -(c.y - d.y)); }
     }
 }
 
-__device__ __forceinline__ void load_vec(const double2* __restrict__ v, const size_t vh, uint64_t pol, unsigned int mask,
-                                         double (&vr)[3], double (&vi)[3]) {
+template <typename T>
+__device__ __forceinline__ void load_vec(const V2<T>* __restrict__ v, const size_t vh, uint64_t pol, unsigned int mask,
+                                         T (&vr)[3], T (&vi)[3]) {
 #pragma unroll
     for (int c = 0; c < 3; ++c) {
-        const double2 t = ld_reuse(v + c * vh, pol);
+        const V2<T> t = ld_reuse(v + c * vh, pol);
         vr[c] = flip(t.x, mask);
         vi[c] = flip(t.y, mask);
     }
 }
 
 // acc += sign * U v          (forward hop; the sign is already folded into v)
-template <int RECON>
-__device__ __forceinline__ void hop_fwd(double (&ar)[3], double (&ai)[3], const double2* __restrict__ w,
-                                        const double2* __restrict__ v, const size_t vh, unsigned int mask,
+template <typename T, int RECON>
+__device__ __forceinline__ void hop_fwd(T (&ar)[3], T (&ai)[3], const V2<T>* __restrict__ w,
+                                        const V2<T>* __restrict__ v, const size_t vh, unsigned int mask,
                                         uint64_t pol_s, uint64_t pol_r) {
-    double2 u[9];
-    double vr[3], vi[3];
-    load_link<RECON>(w, vh, pol_s, u);
-    load_vec(v, vh, pol_r, mask, vr, vi);
+    V2<T> u[9];
+    T vr[3], vi[3];
+    load_link<T, RECON>(w, vh, pol_s, u);
+    load_vec<T>(v, vh, pol_r, mask, vr, vi);
 #pragma unroll
     for (int a = 0; a < 3; ++a)
 #pragma unroll
-        for (int b = 0; b < 3; ++b) cmad(ar[a], ai[a], u[3 * a + b], vr[b], vi[b]);
+        for (int b = 0; b < 3; ++b) cmad<T>(ar[a], ai[a], u[3 * a + b], vr[b], vi[b]);
 }
 
 // acc += sign * U^dagger v   (backward hop; caller passes the mask of -s)
-template <int RECON>
-__device__ __forceinline__ void hop_bwd(double (&ar)[3], double (&ai)[3], const double2* __restrict__ w,
-                                        const double2* __restrict__ v, const size_t vh, unsigned int mask,
+template <typename T, int RECON>
+__device__ __forceinline__ void hop_bwd(T (&ar)[3], T (&ai)[3], const V2<T>* __restrict__ w,
+                                        const V2<T>* __restrict__ v, const size_t vh, unsigned int mask,
                                         uint64_t pol_s, uint64_t pol_r) {
-    double2 u[9];
-    double vr[3], vi[3];
-    load_link<RECON>(w, vh, pol_s, u);
-    load_vec(v, vh, pol_r, mask, vr, vi);
+    V2<T> u[9];
+    T vr[3], vi[3];
+    load_link<T, RECON>(w, vh, pol_s, u);
+    load_vec<T>(v, vh, pol_r, mask, vr, vi);
 #pragma unroll
     for (int a = 0; a < 3; ++a)
 #pragma unroll
-        for (int b = 0; b < 3; ++b) cmad_conj(ar[a], ai[a], u[3 * b + a], vr[b], vi[b]);
+        for (int b = 0; b < 3; ++b) cmad_conj<T>(ar[a], ai[a], u[3 * b + a], vr[b], vi[b]);
 }
 
+template <typename T>
 struct DslashArgs {
     Geom g;
-    const double2* W;        // stored links
-    const double2* in;       // parity 1-par
-    double2* out;            // parity par
+    const V2<T>* W;          // stored links
+    const V2<T>* in;         // parity 1-par
+    V2<T>* out;              // parity par
     int par;                 // parity of the output sites
-    const double2* pv;       // EPI >= 1: vector of parity par
+    const V2<T>* pv;         // EPI >= 1: vector of parity par
     double coef;             // EPI >= 1: m^2 + sigma
     double* partials;        // EPI == 1
     CgState* st;             // EPI == 1, or any EPI with check_stop
     int check_stop;          // 1: return at once if st->stop (CG already converged)
 };
 
-template <int RECON, int EPI>
-__global__ void __launch_bounds__(DS_BLOCK, DS_MINB) dslash_kernel(const DslashArgs A) {
+// registers: double needs ~126 (4 blocks of 128 threads per SM); single fits 6 blocks
+template <typename T> struct DsOcc { static constexpr int minb = DS_MINB; };
+template <> struct DsOcc<float> { static constexpr int minb = DS_MINB_F32; };
+
+template <typename T, int RECON, int EPI>
+__global__ void __launch_bounds__(DS_BLOCK, DsOcc<T>::minb) dslash_kernel(const DslashArgs<T> A) {
     constexpr int NE = (RECON == 12) ? 6 : 9;
     if (A.check_stop) {
         if (A.st->stop) {
@@ -195,16 +226,16 @@ __global__ void __launch_bounds__(DS_BLOCK, DS_MINB) dslash_kernel(const DslashA
     const uint64_t pol_s = l2_policy_evict_first();
     const uint64_t pol_r = l2_policy_evict_last();
 
-    const double2* __restrict__ Wf = A.W + (size_t)A.par * NE * vh + k;          // links of the output parity
-    const double2* __restrict__ Wb = A.W + (size_t)(1 - A.par) * NE * vh;        // links of the input parity
+    const V2<T>* __restrict__ Wf = A.W + (size_t)A.par * NE * vh + k;            // links of the output parity
+    const V2<T>* __restrict__ Wb = A.W + (size_t)(1 - A.par) * NE * vh;          // links of the input parity
     const size_t mu_stride = (size_t)2 * NE * vh;
-    const double2* __restrict__ in = A.in;
+    const V2<T>* __restrict__ in = A.in;
 
     // epilogue operands are requested first, so that their latency hides behind the eight hops
-    double coef = 0.0;
-    double2 pv[3];
+    T coef = (T)0;
+    V2<T> pv[3];
     if (EPI != 0) {
-        coef = (EPI == 1) ? A.st->c0 : A.coef;     // CG: m^2 + sigma0 from the device state (graph-invariant)
+        coef = (T)((EPI == 1) ? A.st->c0 : A.coef);     // CG: m^2 + sigma0 from the device state (graph-invariant)
 #if EPI_PLOAD == 1
 #pragma unroll
         for (int c = 0; c < 3; ++c) pv[c] = A.pv[c * vh + k];
@@ -214,38 +245,38 @@ __global__ void __launch_bounds__(DS_BLOCK, DS_MINB) dslash_kernel(const DslashA
 #endif
     }
 
-    double ar[3] = {0.0, 0.0, 0.0}, ai[3] = {0.0, 0.0, 0.0};
-    hop_fwd<RECON>(ar, ai, Wf + 0 * mu_stride, in + kxf, vh, 0u, pol_s, pol_r);
-    hop_bwd<RECON>(ar, ai, Wb + 0 * mu_stride + kxb, in + kxb, vh, SB, pol_s, pol_r);
-    hop_fwd<RECON>(ar, ai, Wf + 1 * mu_stride, in + kyf, vh, my, pol_s, pol_r);
-    hop_bwd<RECON>(ar, ai, Wb + 1 * mu_stride + kyb, in + kyb, vh, my ^ SB, pol_s, pol_r);
-    hop_fwd<RECON>(ar, ai, Wf + 2 * mu_stride, in + kzf, vh, mz, pol_s, pol_r);
-    hop_bwd<RECON>(ar, ai, Wb + 2 * mu_stride + kzb, in + kzb, vh, mz ^ SB, pol_s, pol_r);
-    hop_fwd<RECON>(ar, ai, Wf + 3 * mu_stride, in + ktf, vh, mtf, pol_s, pol_r);
-    hop_bwd<RECON>(ar, ai, Wb + 3 * mu_stride + ktb, in + ktb, vh, mtb ^ SB, pol_s, pol_r);
+    T ar[3] = {(T)0, (T)0, (T)0}, ai[3] = {(T)0, (T)0, (T)0};
+    hop_fwd<T, RECON>(ar, ai, Wf + 0 * mu_stride, in + kxf, vh, 0u, pol_s, pol_r);
+    hop_bwd<T, RECON>(ar, ai, Wb + 0 * mu_stride + kxb, in + kxb, vh, SB, pol_s, pol_r);
+    hop_fwd<T, RECON>(ar, ai, Wf + 1 * mu_stride, in + kyf, vh, my, pol_s, pol_r);
+    hop_bwd<T, RECON>(ar, ai, Wb + 1 * mu_stride + kyb, in + kyb, vh, my ^ SB, pol_s, pol_r);
+    hop_fwd<T, RECON>(ar, ai, Wf + 2 * mu_stride, in + kzf, vh, mz, pol_s, pol_r);
+    hop_bwd<T, RECON>(ar, ai, Wb + 2 * mu_stride + kzb, in + kzb, vh, mz ^ SB, pol_s, pol_r);
+    hop_fwd<T, RECON>(ar, ai, Wf + 3 * mu_stride, in + ktf, vh, mtf, pol_s, pol_r);
+    hop_bwd<T, RECON>(ar, ai, Wb + 3 * mu_stride + ktb, in + ktb, vh, mtb ^ SB, pol_s, pol_r);
 
     if (EPI == 0) {
         if (valid) {
 #pragma unroll
-            for (int c = 0; c < 3; ++c) A.out[c * vh + k] = make_double2(0.5 * ar[c], 0.5 * ai[c]);
+            for (int c = 0; c < 3; ++c) A.out[c * vh + k] = make_v2((T)0.5 * ar[c], (T)0.5 * ai[c]);
         }
         return;
     }
 
-    // epilogue: out = coef*pv - D in;  Re<pv, out>
+    // epilogue: out = coef*pv - D in;  Re<pv, out> (summed in double whatever T is)
     double dot = 0.0;
 #pragma unroll
     for (int c = 0; c < 3; ++c) {
 #if EPI_PLOAD == 1
-        const double2 p = pv[c];
+        const V2<T> p = pv[c];
 #else
-        const double2 p = A.pv[c * vh + k];
+        const V2<T> p = A.pv[c * vh + k];
 #endif
-        const double2 o = make_double2(fma(-0.5, ar[c], coef * p.x), fma(-0.5, ai[c], coef * p.y));
+        const V2<T> o = make_v2(fma((T)-0.5, ar[c], coef * p.x), fma((T)-0.5, ai[c], coef * p.y));
         if (valid) {
             A.out[c * vh + k] = o;
-            dot = fma(p.x, o.x, dot);
-            dot = fma(p.y, o.y, dot);
+            dot = fma((double)p.x, (double)o.x, dot);
+            dot = fma((double)p.y, (double)o.y, dot);
         }
     }
     if (EPI == 1) {

@@ -27,6 +27,22 @@ inline size_t align_up(size_t b) { return (b + ALIGN - 1) / ALIGN * ALIGN; }
 
 }  // namespace
 
+// everything that exists once per precision T (double: the default path; float: the *_f32 entry points)
+template <typename T>
+struct PrecBufs {
+    V2<T>* W = nullptr;      // stored links
+    size_t W_bytes = 0;
+    int recon_stored = 0;    // 0 = no gauge in this precision, else 18 or 12
+    V2<T> *r = nullptr, *p = nullptr, *s = nullptr, *t = nullptr;
+    V2<T>* pextra[LQCD_MAX_SHIFTS] = {};
+    int n_pextra = 0;
+    cudaGraphExec_t graph_exec = nullptr;    // CUDA graph of `graph_iters` CG iterations
+    int graph_iters = 0, graph_rational = 0;
+    V2<T>* stage_b = nullptr;                // host-call staging (device copies of host arguments)
+    V2<T>* stage_x[LQCD_MAX_SHIFTS] = {};
+    int n_stage_x = 0;
+};
+
 struct lqcd_ctx {
     int L[4];
     Geom g;
@@ -43,16 +59,12 @@ struct lqcd_ctx {
     size_t arena_bytes, arena_used;
     std::vector<void*> owned;    // cudaMalloc'ed by us
 
-    // stored gauge field
-    double2* W;
-    size_t W_bytes;
-    int recon_stored;        // 0 = no gauge yet, else 18 or 12
+    // stored gauge field, operator / solver buffers, CG graph and host-call staging: one set per precision
+    PrecBufs<double> d;
+    PrecBufs<float> f;
+    int prec_opt;            // LQCD_OPT_LINK_PRECISIONS: which of them the next lqcd_set_gauge stores
     double* dev_max;
 
-    // operator / solver buffers
-    double2 *r, *p, *s, *t;
-    double2* pextra[LQCD_MAX_SHIFTS];
-    int n_pextra;
     double* partials;
     size_t n_partials;
     CgState* st_dev;
@@ -61,16 +73,6 @@ struct lqcd_ctx {
     double* max_host;        // pinned
     cudaEvent_t ev[2], ev_t0, ev_t1;
     bool basics;
-
-    // CUDA graph of `graph_iters` CG iterations
-    cudaGraphExec_t graph_exec;
-    int graph_iters, graph_rational;
-
-    // host-call staging (device copies of host arguments)
-    double2* stage_b;
-    double2* stage_x[LQCD_MAX_SHIFTS];
-    int n_stage_x;
-    double2* stage_links;
 
     // statistics
     int last_iters, last_i0, last_nshift;
@@ -130,16 +132,28 @@ void dev_free_owned(lqcd_ctx* c, void* p) {
         }
 }
 
+template <typename T> PrecBufs<T>& bufs(lqcd_ctx* c);
+template <> PrecBufs<double>& bufs<double>(lqcd_ctx* c) { return c->d; }
+template <> PrecBufs<float>& bufs<float>(lqcd_ctx* c) { return c->f; }
+
+template <typename T>
 void drop_graph(lqcd_ctx* c) {
-    if (c->graph_exec) {
-        cudaGraphExecDestroy(c->graph_exec);
-        c->graph_exec = nullptr;
+    PrecBufs<T>& B = bufs<T>(c);
+    if (B.graph_exec) {
+        cudaGraphExecDestroy(B.graph_exec);
+        B.graph_exec = nullptr;
     }
-    c->graph_iters = 0;
+    B.graph_iters = 0;
+}
+void drop_graphs(lqcd_ctx* c) {
+    drop_graph<double>(c);
+    drop_graph<float>(c);
 }
 
-size_t vec_bytes(const lqcd_ctx* c) { return c->Vh * 3 * sizeof(double2); }
-size_t links_bytes(const lqcd_ctx* c, int recon) { return (size_t)8 * (recon == 12 ? 6 : 9) * c->Vh * sizeof(double2); }
+template <typename T> size_t vec_bytes(const lqcd_ctx* c) { return c->Vh * 3 * sizeof(V2<T>); }
+template <typename T> size_t links_bytes(const lqcd_ctx* c, int recon) {
+    return (size_t)8 * (recon == 12 ? 6 : 9) * c->Vh * sizeof(V2<T>);
+}
 
 int ds_grid(const lqcd_ctx* c) { return (int)((c->Vh + DS_BLOCK - 1) / DS_BLOCK); }
 int cg_grid(const lqcd_ctx* c) {
@@ -149,11 +163,10 @@ int cg_grid(const lqcd_ctx* c) {
     return (int)(blocks < cap ? blocks : cap);
 }
 
-// buffers every operator call needs: the odd temporary, the CG state, pinned mirrors, events
+// buffers every call needs: the CG state, reduction partials, pinned mirrors, events
 int ensure_basics(lqcd_ctx* c) {
     if (c->basics) return LQCD_OK;
     int rc;
-    if ((rc = dev_alloc(c, (void**)&c->t, vec_bytes(c)))) return rc;
     if ((rc = dev_alloc(c, (void**)&c->st_dev, sizeof(CgState)))) return rc;
     c->n_partials = (size_t)(ds_grid(c) > cg_grid(c) ? ds_grid(c) : cg_grid(c));
     if ((rc = dev_alloc(c, (void**)&c->partials, c->n_partials * sizeof(double)))) return rc;
@@ -170,36 +183,47 @@ int ensure_basics(lqcd_ctx* c) {
     return LQCD_OK;
 }
 
-int ensure_solver(lqcd_ctx* c, int nshift) {
+// the odd-parity temporary of the two-launch operators
+template <typename T>
+int ensure_tmp(lqcd_ctx* c) {
     int rc;
     if ((rc = ensure_basics(c))) return rc;
-    if (!c->r) {
-        if ((rc = dev_alloc(c, (void**)&c->r, vec_bytes(c)))) return rc;
-        if ((rc = dev_alloc(c, (void**)&c->p, vec_bytes(c)))) return rc;
-        if ((rc = dev_alloc(c, (void**)&c->s, vec_bytes(c)))) return rc;
-    }
-    while (c->n_pextra < nshift - 1) {
-        if ((rc = dev_alloc(c, (void**)&c->pextra[c->n_pextra], vec_bytes(c)))) return rc;
-        ++c->n_pextra;
+    PrecBufs<T>& B = bufs<T>(c);
+    if (!B.t && (rc = dev_alloc(c, (void**)&B.t, vec_bytes<T>(c)))) return rc;
+    return LQCD_OK;
+}
+
+template <typename T>
+int ensure_solver(lqcd_ctx* c, int nshift) {
+    int rc;
+    if ((rc = ensure_tmp<T>(c))) return rc;
+    PrecBufs<T>& B = bufs<T>(c);
+    if (!B.r && (rc = dev_alloc(c, (void**)&B.r, vec_bytes<T>(c)))) return rc;
+    if (!B.p && (rc = dev_alloc(c, (void**)&B.p, vec_bytes<T>(c)))) return rc;
+    if (!B.s && (rc = dev_alloc(c, (void**)&B.s, vec_bytes<T>(c)))) return rc;
+    while (B.n_pextra < nshift - 1) {
+        if ((rc = dev_alloc(c, (void**)&B.pextra[B.n_pextra], vec_bytes<T>(c)))) return rc;
+        ++B.n_pextra;
     }
     return LQCD_OK;
 }
 
-template <int EPI>
-void launch_dslash_t(lqcd_ctx* c, const DslashArgs& a) {
-    if (c->recon_stored == 12)
-        dslash_kernel<12, EPI><<<ds_grid(c), DS_BLOCK, 0, c->stream>>>(a);
+template <typename T, int EPI>
+void launch_dslash_t(lqcd_ctx* c, const DslashArgs<T>& a) {
+    if (bufs<T>(c).recon_stored == 12)
+        dslash_kernel<T, 12, EPI><<<ds_grid(c), DS_BLOCK, 0, c->stream>>>(a);
     else
-        dslash_kernel<18, EPI><<<ds_grid(c), DS_BLOCK, 0, c->stream>>>(a);
+        dslash_kernel<T, 18, EPI><<<ds_grid(c), DS_BLOCK, 0, c->stream>>>(a);
     ++c->launches;
 }
 
 // out(par) = D in, optionally with the epilogue
-void launch_dslash(lqcd_ctx* c, int epi, double2* out, const double2* in, int par, const double2* pv, double coef,
+template <typename T>
+void launch_dslash(lqcd_ctx* c, int epi, V2<T>* out, const V2<T>* in, int par, const V2<T>* pv, double coef,
                    int check_stop) {
-    DslashArgs a;
+    DslashArgs<T> a;
     a.g = c->g;
-    a.W = c->W;
+    a.W = bufs<T>(c).W;
     a.in = in;
     a.out = out;
     a.par = par;
@@ -208,21 +232,23 @@ void launch_dslash(lqcd_ctx* c, int epi, double2* out, const double2* in, int pa
     a.partials = c->partials;
     a.st = c->st_dev;
     a.check_stop = check_stop;
-    if (epi == 0) launch_dslash_t<0>(c, a);
-    else if (epi == 1) launch_dslash_t<1>(c, a);
-    else launch_dslash_t<2>(c, a);
+    if (epi == 0) launch_dslash_t<T, 0>(c, a);
+    else if (epi == 1) launch_dslash_t<T, 1>(c, a);
+    else launch_dslash_t<T, 2>(c, a);
 }
 
 // one CG iteration = K1..K4 (cg.cuh)
+template <typename T>
 void launch_cg_iteration(lqcd_ctx* c, int rational) {
     const size_t n = c->Vh * 3;
-    launch_dslash(c, 0, c->t, c->p, 1, nullptr, 0.0, 1);
-    launch_dslash(c, 1, c->s, c->t, 0, c->p, 0.0, 1);
-    cg_update_r_kernel<<<cg_grid(c), CG_BLOCK, 0, c->stream>>>(c->r, c->s, c->st_dev, c->partials, n);
+    PrecBufs<T>& B = bufs<T>(c);
+    launch_dslash<T>(c, 0, B.t, B.p, 1, nullptr, 0.0, 1);
+    launch_dslash<T>(c, 1, B.s, B.t, 0, B.p, 0.0, 1);
+    cg_update_r_kernel<T><<<cg_grid(c), CG_BLOCK, 0, c->stream>>>(B.r, B.s, c->st_dev, c->partials, n);
     if (rational)
-        cg_update_yp_kernel<<<cg_grid(c), CG_BLOCK, 0, c->stream>>>(c->r, c->st_dev, n);
+        cg_update_yp_kernel<T><<<cg_grid(c), CG_BLOCK, 0, c->stream>>>(B.r, c->st_dev, n);
     else
-        cg_update_xp_kernel<<<cg_grid(c), CG_BLOCK, 0, c->stream>>>(c->r, c->st_dev, n);
+        cg_update_xp_kernel<T><<<cg_grid(c), CG_BLOCK, 0, c->stream>>>(B.r, c->st_dev, n);
     c->launches += 2;
 }
 
@@ -233,39 +259,90 @@ int default_check_every(const lqcd_ctx* c) {
     return (int)v;
 }
 
+template <typename T>
 int build_graph(lqcd_ctx* c, int iters, int rational) {
-    drop_graph(c);
+    drop_graph<T>(c);
+    PrecBufs<T>& B = bufs<T>(c);
     cudaGraph_t graph = nullptr;
     const long long before = c->launches;
     CU(cudaStreamBeginCapture(c->stream, cudaStreamCaptureModeThreadLocal));
-    for (int i = 0; i < iters; ++i) launch_cg_iteration(c, rational);
+    for (int i = 0; i < iters; ++i) launch_cg_iteration<T>(c, rational);
     cudaError_t e = cudaStreamEndCapture(c->stream, &graph);
     c->launches = before;     // capturing is not launching
     if (e != cudaSuccess) return fail(c, LQCD_ECUDA, "graph capture failed: %s", cudaGetErrorString(e));
-    e = cudaGraphInstantiate(&c->graph_exec, graph, 0);
+    e = cudaGraphInstantiate(&B.graph_exec, graph, 0);
     cudaGraphDestroy(graph);
     if (e != cudaSuccess) {
-        c->graph_exec = nullptr;
+        B.graph_exec = nullptr;
         return fail(c, LQCD_ECUDA, "graph instantiate failed: %s", cudaGetErrorString(e));
     }
-    c->graph_iters = iters;
-    c->graph_rational = rational;
+    B.graph_iters = iters;
+    B.graph_rational = rational;
     return LQCD_OK;
 }
 
+template <typename T>
 int check_ctx_gauge(lqcd_ctx* c) {
-    if (!c->recon_stored) return fail(c, LQCD_ENOGAUGE, "no gauge field set (call lqcd_set_gauge first)");
+    if (!bufs<T>(c).recon_stored)
+        return fail(c, LQCD_ENOGAUGE, "no %s-precision gauge field stored (lqcd_set_gauge, LQCD_OPT_LINK_PRECISIONS)",
+                    sizeof(T) == 8 ? "double" : "single");
     return LQCD_OK;
 }
 
+template <typename T>
 int ensure_stage(lqcd_ctx* c, int nx) {
     int rc;
-    if (!c->stage_b && (rc = dev_alloc(c, (void**)&c->stage_b, vec_bytes(c)))) return rc;
-    while (c->n_stage_x < nx) {
-        if ((rc = dev_alloc(c, (void**)&c->stage_x[c->n_stage_x], vec_bytes(c)))) return rc;
-        ++c->n_stage_x;
+    PrecBufs<T>& B = bufs<T>(c);
+    if (!B.stage_b && (rc = dev_alloc(c, (void**)&B.stage_b, vec_bytes<T>(c)))) return rc;
+    while (B.n_stage_x < nx) {
+        if ((rc = dev_alloc(c, (void**)&B.stage_x[B.n_stage_x], vec_bytes<T>(c)))) return rc;
+        ++B.n_stage_x;
     }
     return LQCD_OK;
+}
+
+// Store the links in precision T (step A1).  `links` is the canonical double-precision field on the device.
+template <typename T>
+int store_gauge(lqcd_ctx* c, const double* links, int recon) {
+    int rc;
+    PrecBufs<T>& B = bufs<T>(c);
+    const size_t need = links_bytes<T>(c, recon);
+    if (!B.W || B.W_bytes < need) {
+        if (B.W && !c->arena) dev_free_owned(c, B.W);
+        B.W = nullptr;
+        B.recon_stored = 0;
+        const size_t want = c->arena ? links_bytes<T>(c, 18) : need;   // an arena slot is sized for either format
+        if ((rc = dev_alloc(c, (void**)&B.W, want))) return rc;
+        B.W_bytes = align_up(want);
+    }
+    B.recon_stored = 0;
+    CU(cudaMemsetAsync(c->dev_max, 0, sizeof(double), c->stream));
+    const size_t nthreads = 8 * c->Vh;
+    const int grid = (int)((nthreads + 255) / 256);
+    if (recon == 12)
+        repack_gauge_kernel<T, 12><<<grid, 256, 0, c->stream>>>(c->g, (const double2*)links, B.W, c->dev_max);
+    else
+        repack_gauge_kernel<T, 18><<<grid, 256, 0, c->stream>>>(c->g, (const double2*)links, B.W, c->dev_max);
+    ++c->launches;
+    CU(cudaGetLastError());
+    CU(cudaMemcpyAsync(c->max_host, c->dev_max, sizeof(double), cudaMemcpyDeviceToHost, c->stream));
+    CU(cudaStreamSynchronize(c->stream));
+    if (recon == 12 && !(*c->max_host <= 1e-12))
+        return fail(c, LQCD_ENOTSU3, "RECON=12 but max|r2 - conj(r0 x r1)| = %.3e > 1e-12", *c->max_host);
+    B.recon_stored = recon;
+    return LQCD_OK;
+}
+
+// release the stored links of precision T (no longer requested by LQCD_OPT_LINK_PRECISIONS)
+template <typename T>
+void release_gauge(lqcd_ctx* c) {
+    PrecBufs<T>& B = bufs<T>(c);
+    B.recon_stored = 0;
+    if (B.W && !c->arena) {
+        dev_free_owned(c, B.W);
+        B.W = nullptr;
+        B.W_bytes = 0;
+    }
 }
 
 }  // namespace
@@ -319,6 +396,7 @@ lqcd_ctx* lqcd_create(int Lx, int Ly, int Lz, int Lt) {
     c->stream = nullptr;
     c->mass = 0.0;
     c->recon_opt = 18;
+    c->prec_opt = LQCD_PREC_F64;
     c->max_iter = 100000;
     c->check_every = 0;
     c->use_graph = 1;
@@ -329,7 +407,7 @@ lqcd_ctx* lqcd_create(int Lx, int Ly, int Lz, int Lt) {
 void lqcd_destroy(lqcd_ctx* c) {
     if (!c) return;
     cudaStreamSynchronize(c->stream);
-    drop_graph(c);
+    drop_graphs(c);
     for (void* p : c->owned) cudaFree(p);
     if (c->st_host) cudaFreeHost(c->st_host);
     if (c->flag_host) cudaFreeHost(c->flag_host);
@@ -362,7 +440,7 @@ int lqcd_set_option(lqcd_ctx* c, int key, double v) {
         case LQCD_OPT_ANTIPERIODIC_T:
             if (v != 0.0 && v != 1.0) return fail(c, LQCD_EINVAL, "ANTIPERIODIC_T must be 0 or 1");
             c->g.antiperiodic = (int)v;
-            drop_graph(c);        // Geom is a kernel argument baked into the graph
+            drop_graphs(c);       // Geom is a kernel argument baked into the graph
             break;
         case LQCD_OPT_RECON:
             if (v != 18.0 && v != 12.0) return fail(c, LQCD_EINVAL, "RECON must be 18 or 12");
@@ -380,6 +458,11 @@ int lqcd_set_option(lqcd_ctx* c, int key, double v) {
             if (v != 0.0 && v != 1.0) return fail(c, LQCD_EINVAL, "USE_GRAPH must be 0 or 1");
             c->use_graph = (int)v;
             break;
+        case LQCD_OPT_LINK_PRECISIONS:
+            if (v != 1.0 && v != 2.0 && v != 3.0)
+                return fail(c, LQCD_EINVAL, "LINK_PRECISIONS must be LQCD_PREC_F64 (1), LQCD_PREC_F32 (2) or both (3)");
+            c->prec_opt = (int)v;
+            break;
         default:
             return fail(c, LQCD_EINVAL, "unknown option key %d", key);
     }
@@ -395,6 +478,7 @@ int lqcd_get_option(const lqcd_ctx* c, int key, double* v) {
         case LQCD_OPT_MAX_ITER: *v = c->max_iter; break;
         case LQCD_OPT_CHECK_EVERY: *v = c->check_every ? c->check_every : default_check_every(c); break;
         case LQCD_OPT_USE_GRAPH: *v = c->use_graph; break;
+        case LQCD_OPT_LINK_PRECISIONS: *v = c->prec_opt; break;
         default: return LQCD_EINVAL;
     }
     return LQCD_OK;
@@ -402,9 +486,11 @@ int lqcd_get_option(const lqcd_ctx* c, int key, double* v) {
 
 size_t lqcd_workspace_bytes(const lqcd_ctx* c, int nshift) {
     if (!c || nshift < 1 || nshift > LQCD_MAX_SHIFTS) return 0;
-    const size_t vb = align_up(vec_bytes(c));
-    size_t b = align_up(links_bytes(c, 18));
-    b += vb * (size_t)(4 + (nshift - 1));                       // t, r, p, s, extra directions
+    size_t b = 0;
+    if (c->prec_opt & LQCD_PREC_F64)
+        b += align_up(links_bytes<double>(c, 18)) + align_up(vec_bytes<double>(c)) * (size_t)(4 + (nshift - 1));
+    if (c->prec_opt & LQCD_PREC_F32)
+        b += align_up(links_bytes<float>(c, 18)) + align_up(vec_bytes<float>(c)) * (size_t)(4 + (nshift - 1));
     b += align_up(sizeof(CgState)) + align_up(sizeof(double));
     const size_t np = (size_t)(ds_grid(c) > cg_grid(c) ? ds_grid(c) : cg_grid(c));
     b += align_up(np * sizeof(double));
@@ -413,7 +499,7 @@ size_t lqcd_workspace_bytes(const lqcd_ctx* c, int nshift) {
 
 int lqcd_set_workspace(lqcd_ctx* c, void* dev, size_t bytes) {
     if (!c) return LQCD_EINVAL;
-    if (c->recon_stored || c->basics || !c->owned.empty())
+    if (c->d.recon_stored || c->f.recon_stored || c->basics || !c->owned.empty())
         return fail(c, LQCD_EINVAL, "lqcd_set_workspace must be called before any other device work on the context");
     if (!dev || ((uintptr_t)dev % ALIGN) != 0) return fail(c, LQCD_EINVAL, "workspace must be a 256-byte aligned device pointer");
     c->arena = (char*)dev;
@@ -427,32 +513,22 @@ int lqcd_set_gauge(lqcd_ctx* c, const double* links) {
     if (!links) return fail(c, LQCD_EINVAL, "links is NULL");
     int rc;
     if ((rc = ensure_basics(c))) return rc;
-    const int recon = c->recon_opt;
-    const size_t need = links_bytes(c, recon);
-    if (!c->W || c->W_bytes < need) {
-        if (c->W && !c->arena) dev_free_owned(c, c->W);
-        c->W = nullptr;
-        c->recon_stored = 0;
-        const size_t want = c->arena ? links_bytes(c, 18) : need;   // an arena slot is sized for either format
-        if ((rc = dev_alloc(c, (void**)&c->W, want))) return rc;
-        c->W_bytes = align_up(want);
+    drop_graphs(c);
+    c->d.recon_stored = 0;
+    c->f.recon_stored = 0;
+    if (c->prec_opt & LQCD_PREC_F64) {
+        if ((rc = store_gauge<double>(c, links, c->recon_opt))) return rc;
+    } else {
+        release_gauge<double>(c);
     }
-    drop_graph(c);
-    c->recon_stored = 0;
-    CU(cudaMemsetAsync(c->dev_max, 0, sizeof(double), c->stream));
-    const size_t nthreads = 8 * c->Vh;
-    const int grid = (int)((nthreads + 255) / 256);
-    if (recon == 12)
-        repack_gauge_kernel<12><<<grid, 256, 0, c->stream>>>(c->g, (const double2*)links, c->W, c->dev_max);
-    else
-        repack_gauge_kernel<18><<<grid, 256, 0, c->stream>>>(c->g, (const double2*)links, c->W, c->dev_max);
-    ++c->launches;
-    CU(cudaGetLastError());
-    CU(cudaMemcpyAsync(c->max_host, c->dev_max, sizeof(double), cudaMemcpyDeviceToHost, c->stream));
-    CU(cudaStreamSynchronize(c->stream));
-    if (recon == 12 && !(*c->max_host <= 1e-12))
-        return fail(c, LQCD_ENOTSU3, "RECON=12 but max|r2 - conj(r0 x r1)| = %.3e > 1e-12", *c->max_host);
-    c->recon_stored = recon;
+    if (c->prec_opt & LQCD_PREC_F32) {
+        if ((rc = store_gauge<float>(c, links, c->recon_opt))) {
+            c->d.recon_stored = 0;
+            return rc;
+        }
+    } else {
+        release_gauge<float>(c);
+    }
     return LQCD_OK;
 }
 
@@ -475,52 +551,57 @@ int lqcd_set_gauge_host(lqcd_ctx* c, const double* links) {
     return rc;
 }
 
-static int apply_d(lqcd_ctx* c, double* out, const double* in, int par) {
+}  // extern "C"
+
+namespace {
+
+template <typename T>
+int apply_d(lqcd_ctx* c, T* out, const T* in, int par) {
     if (!c) return LQCD_EINVAL;
     if (!out || !in) return fail(c, LQCD_EINVAL, "NULL vector");
     if (out == in) return fail(c, LQCD_EINVAL, "in and out must not alias");
     int rc;
-    if ((rc = check_ctx_gauge(c))) return rc;
-    launch_dslash(c, 0, (double2*)out, (const double2*)in, par, nullptr, 0.0, 0);
+    if ((rc = check_ctx_gauge<T>(c))) return rc;
+    launch_dslash<T>(c, 0, (V2<T>*)out, (const V2<T>*)in, par, nullptr, 0.0, 0);
     CU(cudaGetLastError());
     return LQCD_OK;
 }
 
-int lqcd_doe(lqcd_ctx* c, double* out_odd, const double* in_even) { return apply_d(c, out_odd, in_even, 1); }
-int lqcd_deo(lqcd_ctx* c, double* out_even, const double* in_odd) { return apply_d(c, out_even, in_odd, 0); }
-
-static int apply_d_host(lqcd_ctx* c, double* out, const double* in, int par) {
+template <typename T>
+int apply_d_host(lqcd_ctx* c, T* out, const T* in, int par) {
     if (!c) return LQCD_EINVAL;
     if (!out || !in) return fail(c, LQCD_EINVAL, "NULL vector");
     int rc;
-    if ((rc = check_ctx_gauge(c))) return rc;
-    if ((rc = ensure_stage(c, 1))) return rc;
-    CU(cudaMemcpyAsync(c->stage_b, in, vec_bytes(c), cudaMemcpyHostToDevice, c->stream));
-    if ((rc = apply_d(c, (double*)c->stage_x[0], (const double*)c->stage_b, par))) return rc;
-    CU(cudaMemcpyAsync(out, c->stage_x[0], vec_bytes(c), cudaMemcpyDeviceToHost, c->stream));
+    if ((rc = check_ctx_gauge<T>(c))) return rc;
+    if ((rc = ensure_stage<T>(c, 1))) return rc;
+    PrecBufs<T>& B = bufs<T>(c);
+    CU(cudaMemcpyAsync(B.stage_b, in, vec_bytes<T>(c), cudaMemcpyHostToDevice, c->stream));
+    if ((rc = apply_d<T>(c, (T*)B.stage_x[0], (const T*)B.stage_b, par))) return rc;
+    CU(cudaMemcpyAsync(out, B.stage_x[0], vec_bytes<T>(c), cudaMemcpyDeviceToHost, c->stream));
     CU(cudaStreamSynchronize(c->stream));
     return LQCD_OK;
 }
 
-int lqcd_doe_host(lqcd_ctx* c, double* out_odd, const double* in_even) { return apply_d_host(c, out_odd, in_even, 1); }
-int lqcd_deo_host(lqcd_ctx* c, double* out_even, const double* in_odd) { return apply_d_host(c, out_even, in_odd, 0); }
-
-int lqcd_mdagm(lqcd_ctx* c, double* out_even, const double* in_even, double sigma) {
+template <typename T>
+int apply_mdagm(lqcd_ctx* c, T* out_even, const T* in_even, double sigma) {
     if (!c) return LQCD_EINVAL;
     if (!out_even || !in_even) return fail(c, LQCD_EINVAL, "NULL vector");
     if (out_even == in_even) return fail(c, LQCD_EINVAL, "in and out must not alias");
     int rc;
-    if ((rc = check_ctx_gauge(c))) return rc;
-    launch_dslash(c, 0, c->t, (const double2*)in_even, 1, nullptr, 0.0, 0);
-    launch_dslash(c, 2, (double2*)out_even, c->t, 0, (const double2*)in_even, c->mass * c->mass + sigma, 0);
+    if ((rc = check_ctx_gauge<T>(c))) return rc;
+    if ((rc = ensure_tmp<T>(c))) return rc;
+    PrecBufs<T>& B = bufs<T>(c);
+    launch_dslash<T>(c, 0, B.t, (const V2<T>*)in_even, 1, nullptr, 0.0, 0);
+    launch_dslash<T>(c, 2, (V2<T>*)out_even, B.t, 0, (const V2<T>*)in_even, c->mass * c->mass + sigma, 0);
     CU(cudaGetLastError());
     return LQCD_OK;
 }
 
 // The solver behind lqcd_mshift_cg (x != NULL: every x[i] is stored) and lqcd_rational_apply (y != NULL:
-// only y = alpha0 b + sum_i alpha[i] x_i is accumulated).
-static int solve(lqcd_ctx* c, const double* b_even, const double* shifts, int nshift, double tol, double* const* x,
-                 double* y, double alpha0, const double* alpha) {
+// only y = alpha0 b + sum_i alpha[i] x_i is accumulated), in precision T.
+template <typename T>
+int solve(lqcd_ctx* c, const T* b_even, const double* shifts, int nshift, double tol, T* const* x, T* y, double alpha0,
+          const double* alpha) {
     if (!c) return LQCD_EINVAL;
     if (!b_even || !shifts || (!x && !y) || (y && !alpha)) return fail(c, LQCD_EINVAL, "NULL argument");
     if (nshift < 1 || nshift > LQCD_MAX_SHIFTS) return fail(c, LQCD_EINVAL, "nshift must be in [1, %d]", LQCD_MAX_SHIFTS);
@@ -531,15 +612,16 @@ static int solve(lqcd_ctx* c, const double* b_even, const double* shifts, int ns
             if (!std::isfinite(alpha[i])) return fail(c, LQCD_EINVAL, "alpha[%d] must be finite", i);
             continue;
         }
-        if (!x[i] || (const double*)x[i] == b_even) return fail(c, LQCD_EINVAL, "x[%d] is NULL or aliases b", i);
+        if (!x[i] || (const T*)x[i] == b_even) return fail(c, LQCD_EINVAL, "x[%d] is NULL or aliases b", i);
         for (int j = 0; j < i; ++j)
             if (x[j] == x[i]) return fail(c, LQCD_EINVAL, "x[%d] aliases x[%d]", i, j);
     }
     if (y && (y == b_even || !std::isfinite(alpha0))) return fail(c, LQCD_EINVAL, "y aliases b, or alpha0 is not finite");
     const int rational = y ? 1 : 0;
     int rc;
-    if ((rc = check_ctx_gauge(c))) return rc;
-    if ((rc = ensure_solver(c, nshift))) return rc;
+    if ((rc = check_ctx_gauge<T>(c))) return rc;
+    if ((rc = ensure_solver<T>(c, nshift))) return rc;
+    PrecBufs<T>& B = bufs<T>(c);
 
     // base system = smallest shift (R5); ties: the first
     int i0 = 0;
@@ -555,35 +637,35 @@ static int solve(lqcd_ctx* c, const double* b_even, const double* shifts, int ns
     int extra = 0;
     for (int i = 0; i < nshift; ++i) {
         h->delta[i] = shifts[i] - shifts[i0];
-        h->x[i] = rational ? nullptr : (double2*)x[i];
+        h->x[i] = rational ? nullptr : (void*)x[i];
         h->alpha[i] = rational ? alpha[i] : 0.0;
-        h->p[i] = (i == i0) ? c->p : c->pextra[extra++];
+        h->p[i] = (i == i0) ? (void*)B.p : (void*)B.pextra[extra++];
     }
     h->rational = rational;
     h->alpha0 = alpha0;
-    h->y = (double2*)y;
+    h->y = (void*)y;
     const size_t n = c->Vh * 3;
     CU(cudaMemcpyAsync(c->st_dev, h, sizeof(CgState), cudaMemcpyHostToDevice, c->stream));
     CU(cudaEventRecord(c->ev_t0, c->stream));
-    cg_init_kernel<<<cg_grid(c), CG_BLOCK, 0, c->stream>>>((const double2*)b_even, c->r, c->st_dev, c->partials, n, tol);
+    cg_init_kernel<T><<<cg_grid(c), CG_BLOCK, 0, c->stream>>>((const V2<T>*)b_even, B.r, c->st_dev, c->partials, n, tol);
     ++c->launches;
     CU(cudaGetLastError());
 
     const int ce = c->check_every ? c->check_every : default_check_every(c);
     // the legacy default stream cannot be captured: plain launches there
     const bool use_graph = c->use_graph && c->stream != nullptr && c->stream != cudaStreamLegacy;
-    if (use_graph && (c->graph_iters != ce || c->graph_rational != rational)) {
-        if ((rc = build_graph(c, ce, rational))) return rc;
+    if (use_graph && (B.graph_iters != ce || B.graph_rational != rational)) {
+        if ((rc = build_graph<T>(c, ce, rational))) return rc;
     }
     c->flag_host[0] = c->flag_host[1] = 0;
     bool done = false;
     const long max_batches = (long)c->max_iter / ce + 3;
     for (long batch = 0; batch < max_batches && !done; ++batch) {
         if (use_graph) {
-            CU(cudaGraphLaunch(c->graph_exec, c->stream));
+            CU(cudaGraphLaunch(B.graph_exec, c->stream));
             c->launches += 4LL * ce;
         } else {
-            for (int i = 0; i < ce; ++i) launch_cg_iteration(c, rational);
+            for (int i = 0; i < ce; ++i) launch_cg_iteration<T>(c, rational);
             CU(cudaGetLastError());
         }
         const int slot = (int)(batch & 1);
@@ -611,51 +693,96 @@ static int solve(lqcd_ctx* c, const double* b_even, const double* shifts, int ns
     return LQCD_OK;
 }
 
+template <typename T>
+int solve_host(lqcd_ctx* c, const T* b_even, const double* shifts, int nshift, double tol, T* const* x, T* y,
+               double alpha0, const double* alpha) {
+    if (!c) return LQCD_EINVAL;
+    if (!b_even || !shifts || (!x && !y)) return fail(c, LQCD_EINVAL, "NULL argument");
+    if (nshift < 1 || nshift > LQCD_MAX_SHIFTS) return fail(c, LQCD_EINVAL, "nshift must be in [1, %d]", LQCD_MAX_SHIFTS);
+    const int nout = y ? 1 : nshift;
+    for (int i = 0; x && i < nshift; ++i)
+        if (!x[i]) return fail(c, LQCD_EINVAL, "x[%d] is NULL", i);
+    int rc;
+    if ((rc = check_ctx_gauge<T>(c))) return rc;
+    if ((rc = ensure_stage<T>(c, nout))) return rc;
+    PrecBufs<T>& B = bufs<T>(c);
+    CU(cudaMemcpyAsync(B.stage_b, b_even, vec_bytes<T>(c), cudaMemcpyHostToDevice, c->stream));
+    T* xd[LQCD_MAX_SHIFTS];
+    for (int i = 0; i < nout; ++i) xd[i] = (T*)B.stage_x[i];
+    const int status = y ? solve<T>(c, (const T*)B.stage_b, shifts, nshift, tol, nullptr, xd[0], alpha0, alpha)
+                         : solve<T>(c, (const T*)B.stage_b, shifts, nshift, tol, xd, nullptr, 0.0, nullptr);
+    if (status != LQCD_OK && status != LQCD_ENOCONV) return status;
+    for (int i = 0; i < nout; ++i)
+        CU(cudaMemcpyAsync(y ? y : x[i], B.stage_x[i], vec_bytes<T>(c), cudaMemcpyDeviceToHost, c->stream));
+    CU(cudaStreamSynchronize(c->stream));
+    return status;
+}
+
+template <typename T>
+int pack_unpack(lqcd_ctx* c, int parity, const T* in, T* out, bool pack) {
+    if (!c) return LQCD_EINVAL;
+    if (!in || !out || (parity != 0 && parity != 1)) return fail(c, LQCD_EINVAL, "bad argument");
+    const int grid = (int)((c->Vh + 255) / 256);
+    if (pack)
+        pack_vector_kernel<T><<<grid, 256, 0, c->stream>>>(c->g, parity, (const V2<T>*)in, (V2<T>*)out);
+    else
+        unpack_vector_kernel<T><<<grid, 256, 0, c->stream>>>(c->g, parity, (const V2<T>*)in, (V2<T>*)out);
+    ++c->launches;
+    CU(cudaGetLastError());
+    return LQCD_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+int lqcd_doe(lqcd_ctx* c, double* out_odd, const double* in_even) { return apply_d<double>(c, out_odd, in_even, 1); }
+int lqcd_deo(lqcd_ctx* c, double* out_even, const double* in_odd) { return apply_d<double>(c, out_even, in_odd, 0); }
+int lqcd_doe_host(lqcd_ctx* c, double* out_odd, const double* in_even) { return apply_d_host<double>(c, out_odd, in_even, 1); }
+int lqcd_deo_host(lqcd_ctx* c, double* out_even, const double* in_odd) { return apply_d_host<double>(c, out_even, in_odd, 0); }
+int lqcd_mdagm(lqcd_ctx* c, double* out_even, const double* in_even, double sigma) {
+    return apply_mdagm<double>(c, out_even, in_even, sigma);
+}
+
+int lqcd_doe_f32(lqcd_ctx* c, float* out_odd, const float* in_even) { return apply_d<float>(c, out_odd, in_even, 1); }
+int lqcd_deo_f32(lqcd_ctx* c, float* out_even, const float* in_odd) { return apply_d<float>(c, out_even, in_odd, 0); }
+int lqcd_doe_f32_host(lqcd_ctx* c, float* out_odd, const float* in_even) { return apply_d_host<float>(c, out_odd, in_even, 1); }
+int lqcd_deo_f32_host(lqcd_ctx* c, float* out_even, const float* in_odd) { return apply_d_host<float>(c, out_even, in_odd, 0); }
+int lqcd_mdagm_f32(lqcd_ctx* c, float* out_even, const float* in_even, double sigma) {
+    return apply_mdagm<float>(c, out_even, in_even, sigma);
+}
+
 int lqcd_mshift_cg(lqcd_ctx* c, const double* b_even, const double* shifts, int nshift, double tol, double* const* x) {
     if (c && !x) return fail(c, LQCD_EINVAL, "NULL argument");
-    return solve(c, b_even, shifts, nshift, tol, x, nullptr, 0.0, nullptr);
+    return solve<double>(c, b_even, shifts, nshift, tol, x, nullptr, 0.0, nullptr);
+}
+int lqcd_mshift_cg_host(lqcd_ctx* c, const double* b_even, const double* shifts, int nshift, double tol, double* const* x) {
+    if (c && !x) return fail(c, LQCD_EINVAL, "NULL argument");
+    return solve_host<double>(c, b_even, shifts, nshift, tol, x, nullptr, 0.0, nullptr);
+}
+int lqcd_mshift_cg_f32(lqcd_ctx* c, const float* b_even, const double* shifts, int nshift, double tol, float* const* x) {
+    if (c && !x) return fail(c, LQCD_EINVAL, "NULL argument");
+    return solve<float>(c, b_even, shifts, nshift, tol, x, nullptr, 0.0, nullptr);
+}
+int lqcd_mshift_cg_f32_host(lqcd_ctx* c, const float* b_even, const double* shifts, int nshift, double tol, float* const* x) {
+    if (c && !x) return fail(c, LQCD_EINVAL, "NULL argument");
+    return solve_host<float>(c, b_even, shifts, nshift, tol, x, nullptr, 0.0, nullptr);
 }
 
 int lqcd_rational_apply(lqcd_ctx* c, const double* b_even, double alpha0, const double* alpha, const double* shifts,
                         int nshift, double tol, double* y_even) {
-    if (c && !y_even) return fail(c, LQCD_EINVAL, "NULL argument");
-    return solve(c, b_even, shifts, nshift, tol, nullptr, y_even, alpha0, alpha);
+    if (c && (!y_even || !alpha)) return fail(c, LQCD_EINVAL, "NULL argument");
+    return solve<double>(c, b_even, shifts, nshift, tol, nullptr, y_even, alpha0, alpha);
 }
-
 int lqcd_rational_apply_host(lqcd_ctx* c, const double* b_even, double alpha0, const double* alpha,
                              const double* shifts, int nshift, double tol, double* y_even) {
-    if (!c) return LQCD_EINVAL;
-    if (!b_even || !y_even) return fail(c, LQCD_EINVAL, "NULL argument");
-    int rc;
-    if ((rc = check_ctx_gauge(c))) return rc;
-    if ((rc = ensure_stage(c, 1))) return rc;
-    CU(cudaMemcpyAsync(c->stage_b, b_even, vec_bytes(c), cudaMemcpyHostToDevice, c->stream));
-    const int status = lqcd_rational_apply(c, (const double*)c->stage_b, alpha0, alpha, shifts, nshift, tol,
-                                           (double*)c->stage_x[0]);
-    if (status != LQCD_OK && status != LQCD_ENOCONV) return status;
-    CU(cudaMemcpyAsync(y_even, c->stage_x[0], vec_bytes(c), cudaMemcpyDeviceToHost, c->stream));
-    CU(cudaStreamSynchronize(c->stream));
-    return status;
+    if (c && (!y_even || !alpha)) return fail(c, LQCD_EINVAL, "NULL argument");
+    return solve_host<double>(c, b_even, shifts, nshift, tol, nullptr, y_even, alpha0, alpha);
 }
-
-int lqcd_mshift_cg_host(lqcd_ctx* c, const double* b_even, const double* shifts, int nshift, double tol, double* const* x) {
-    if (!c) return LQCD_EINVAL;
-    if (!b_even || !shifts || !x) return fail(c, LQCD_EINVAL, "NULL argument");
-    if (nshift < 1 || nshift > LQCD_MAX_SHIFTS) return fail(c, LQCD_EINVAL, "nshift must be in [1, %d]", LQCD_MAX_SHIFTS);
-    for (int i = 0; i < nshift; ++i)
-        if (!x[i]) return fail(c, LQCD_EINVAL, "x[%d] is NULL", i);
-    int rc;
-    if ((rc = check_ctx_gauge(c))) return rc;
-    if ((rc = ensure_stage(c, nshift))) return rc;
-    CU(cudaMemcpyAsync(c->stage_b, b_even, vec_bytes(c), cudaMemcpyHostToDevice, c->stream));
-    double* xd[LQCD_MAX_SHIFTS];
-    for (int i = 0; i < nshift; ++i) xd[i] = (double*)c->stage_x[i];
-    const int status = lqcd_mshift_cg(c, (const double*)c->stage_b, shifts, nshift, tol, xd);
-    if (status != LQCD_OK && status != LQCD_ENOCONV) return status;
-    for (int i = 0; i < nshift; ++i)
-        CU(cudaMemcpyAsync(x[i], c->stage_x[i], vec_bytes(c), cudaMemcpyDeviceToHost, c->stream));
-    CU(cudaStreamSynchronize(c->stream));
-    return status;
+int lqcd_rational_apply_f32(lqcd_ctx* c, const float* b_even, double alpha0, const double* alpha, const double* shifts,
+                            int nshift, double tol, float* y_even) {
+    if (c && (!y_even || !alpha)) return fail(c, LQCD_EINVAL, "NULL argument");
+    return solve<float>(c, b_even, shifts, nshift, tol, nullptr, y_even, alpha0, alpha);
 }
 
 int lqcd_get_stat(const lqcd_ctx* c, int key, int idx, double* out) {
@@ -676,23 +803,16 @@ int lqcd_get_stat(const lqcd_ctx* c, int key, int idx, double* out) {
 }
 
 int lqcd_pack_vector(lqcd_ctx* c, int parity, const double* site_field, double* parity_vector) {
-    if (!c) return LQCD_EINVAL;
-    if (!site_field || !parity_vector || (parity != 0 && parity != 1)) return fail(c, LQCD_EINVAL, "bad argument");
-    pack_vector_kernel<<<(int)((c->Vh + 255) / 256), 256, 0, c->stream>>>(c->g, parity, (const double2*)site_field,
-                                                                         (double2*)parity_vector);
-    ++c->launches;
-    CU(cudaGetLastError());
-    return LQCD_OK;
+    return pack_unpack<double>(c, parity, site_field, parity_vector, true);
 }
-
 int lqcd_unpack_vector(lqcd_ctx* c, int parity, const double* parity_vector, double* site_field) {
-    if (!c) return LQCD_EINVAL;
-    if (!site_field || !parity_vector || (parity != 0 && parity != 1)) return fail(c, LQCD_EINVAL, "bad argument");
-    unpack_vector_kernel<<<(int)((c->Vh + 255) / 256), 256, 0, c->stream>>>(c->g, parity, (const double2*)parity_vector,
-                                                                           (double2*)site_field);
-    ++c->launches;
-    CU(cudaGetLastError());
-    return LQCD_OK;
+    return pack_unpack<double>(c, parity, parity_vector, site_field, false);
+}
+int lqcd_pack_vector_f32(lqcd_ctx* c, int parity, const float* site_field, float* parity_vector) {
+    return pack_unpack<float>(c, parity, site_field, parity_vector, true);
+}
+int lqcd_unpack_vector_f32(lqcd_ctx* c, int parity, const float* parity_vector, float* site_field) {
+    return pack_unpack<float>(c, parity, parity_vector, site_field, false);
 }
 
 }  // extern "C"

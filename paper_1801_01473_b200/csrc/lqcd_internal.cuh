@@ -9,6 +9,16 @@
 
 #define LQCD_MAX_SHIFTS 64          // r of Eq. 2; rational approximations use <= ~20
 
+// The path exists in the two precisions the paper runs in ("double (or float) C99 complex numbers",
+// PAPER.md:L147; single precision for the MD evolution).  Every kernel is a template on the
+// real type T; a complex number is the 2-vector V2<T> (128-bit loads in double, 64-bit in single).
+template <typename T> struct Cplx;
+template <> struct Cplx<double> { typedef double2 type; };
+template <> struct Cplx<float> { typedef float2 type; };
+template <typename T> using V2 = typename Cplx<T>::type;
+__host__ __device__ __forceinline__ double2 make_v2(double x, double y) { return make_double2(x, y); }
+__host__ __device__ __forceinline__ float2 make_v2(float x, float y) { return make_float2(x, y); }
+
 // Geometry of one parity of the lattice in the checkerboard index k = lex>>1 =
 // xh + Lxh*(y + Ly*(z + Lz*t)), xh = x>>1 ("Data layout").
 struct Geom {
@@ -31,14 +41,14 @@ struct CgState {
     // update list of the current iteration (shifts that were active when it started)
     int list_idx[LQCD_MAX_SHIFTS];
     double list_a[LQCD_MAX_SHIFTS], list_zn[LQCD_MAX_SHIFTS], list_b[LQCD_MAX_SHIFTS];
-    double2* x[LQCD_MAX_SHIFTS];
-    double2* p[LQCD_MAX_SHIFTS];
+    void* x[LQCD_MAX_SHIFTS];       // V2<T>* of the precision the solve runs in
+    void* p[LQCD_MAX_SHIFTS];
     // rational-sum mode (lqcd_rational_apply): y = alpha0 b + sum_i alpha_i x_i is accumulated during the
     // solve and the x_i are never stored; list_a then holds alpha_i * a_i
     int rational;
     double alpha0;
     double alpha[LQCD_MAX_SHIFTS];
-    double2* y;
+    void* y;
 };
 
 #endif
