@@ -6,6 +6,7 @@ the two kinds of input the path consumes, in the *canonical user layouts* of ``i
 
 * gauge links  ``links[mu, lex, row, col, {re,im}]``   float64, shape (4, V, 3, 3, 2)
 * a site field ``field[lex, colour, {re,im}]``          float64, shape (V, 3, 2)
+* (optional) U(1) link phases ``theta[mu, lex]``        float64, shape (4, V), radians
 
 with ``lex = x + Lx*(y + Ly*(z + Lz*t))`` and ``mu = 0..3 = x,y,z,t``.  The same bytes are handed to the
 CPU oracle (``oracle/``) and to the CUDA library through their public entry points; neither of them
@@ -44,6 +45,7 @@ SEED_SOURCE = 180101474
 _STREAM_LINKS = 1
 _STREAM_FIELD = 2
 _STREAM_GAUGE_XFORM = 3
+_STREAM_U1 = 4
 
 _MASK64 = (1 << 64) - 1
 
@@ -170,6 +172,15 @@ def random_gauge_transform(L: Sequence[int], seed: int, device="cpu") -> torch.T
     """One SU(3) matrix per site, float64 (V, 3, 3, 2) -- input of the gauge-covariance test."""
     V = volume(L)
     return torch.view_as_real(_random_su3(seed, _STREAM_GAUGE_XFORM, 0, V, device)).contiguous()
+
+
+def random_u1_phases(L: Sequence[int], seed: int = SEED_LINKS, device="cpu") -> torch.Tensor:
+    """U(1) phase field theta_mu(x), float64 (4, V), uniform in (-pi, pi): a stand-in for the imaginary chemical
+    potential / background field phases of PAPER.md:L159 (canonical layout: theta[mu, lex] belongs to the link
+    leaving lex along +mu)."""
+    V = volume(L)
+    ctr = torch.arange(4 * V, dtype=torch.int64, device=device)
+    return ((2.0 * uniform01(seed, _STREAM_U1, ctr) - 1.0) * math.pi).view(4, V)
 
 
 def shifts_geometric(first: float, last: float, n: int) -> list[float]:

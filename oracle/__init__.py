@@ -41,6 +41,11 @@ def lib():
         L.oracle_mshift_cg.argtypes = [_ip, _dp, ctypes.c_double, ctypes.c_int, _dp, _dp, ctypes.c_int,
                                        ctypes.c_double, ctypes.c_int, ctypes.c_int, _dp, _ip, _ip, _dp]
         L.oracle_mshift_cg.restype = ctypes.c_int
+        L.oracle_dslash_u1.argtypes = [_ip, _dp, _dp, _dp, _dp, ctypes.c_int, ctypes.c_int]
+        L.oracle_mdagm_u1.argtypes = [_ip, _dp, _dp, ctypes.c_double, ctypes.c_double, _dp, _dp, ctypes.c_int]
+        L.oracle_mshift_cg_u1.argtypes = [_ip, _dp, _dp, ctypes.c_double, ctypes.c_int, _dp, _dp, ctypes.c_int,
+                                          ctypes.c_double, ctypes.c_int, ctypes.c_int, _dp, _ip, _ip, _dp]
+        L.oracle_mshift_cg_u1.restype = ctypes.c_int
         L.oracle_rational_apply.argtypes = [_ip, _dp, ctypes.c_double, ctypes.c_int, _dp, ctypes.c_double, _dp, _dp,
                                             ctypes.c_int, ctypes.c_double, ctypes.c_int, _dp, _ip, _dp]
         L.oracle_rational_apply.restype = ctypes.c_int
@@ -72,29 +77,45 @@ def set_num_threads(n: int) -> None:
     lib().oracle_set_num_threads(int(n))
 
 
-def dslash(L, U, f_in, out_parity: int, antiperiodic: bool = True) -> np.ndarray:
+def _theta(L, theta):
+    """theta: None, or the U(1) phase field (4, V) in radians, u_mu(x) = exp(i theta_mu(x))."""
+    if theta is None:
+        return None
+    theta = _c(theta)
+    assert theta.shape == (4, 2 * _vh(L))
+    return theta
+
+
+def dslash(L, U, f_in, out_parity: int, antiperiodic: bool = True, theta=None) -> np.ndarray:
     """Parity field on `out_parity` = D applied to the parity field `f_in` on the other parity."""
-    U, f_in = _c(U), _c(f_in)
+    U, f_in, theta = _c(U), _c(f_in), _theta(L, theta)
     out = np.empty((_vh(L), 3, 2), dtype=np.float64)
-    lib().oracle_dslash(_L(L), _p(U), _p(f_in), _p(out), int(out_parity), int(antiperiodic))
+    if theta is None:
+        lib().oracle_dslash(_L(L), _p(U), _p(f_in), _p(out), int(out_parity), int(antiperiodic))
+    else:
+        lib().oracle_dslash_u1(_L(L), _p(U), _p(theta), _p(f_in), _p(out), int(out_parity), int(antiperiodic))
     return out
 
 
-def doe(L, U, f_even, antiperiodic: bool = True) -> np.ndarray:
+def doe(L, U, f_even, antiperiodic: bool = True, theta=None) -> np.ndarray:
     """D_oe: even -> odd (PAPER.md:L80)."""
-    return dslash(L, U, f_even, 1, antiperiodic)
+    return dslash(L, U, f_even, 1, antiperiodic, theta)
 
 
-def deo(L, U, f_odd, antiperiodic: bool = True) -> np.ndarray:
+def deo(L, U, f_odd, antiperiodic: bool = True, theta=None) -> np.ndarray:
     """D_eo: odd -> even (PAPER.md:L80)."""
-    return dslash(L, U, f_odd, 0, antiperiodic)
+    return dslash(L, U, f_odd, 0, antiperiodic, theta)
 
 
-def mdagm(L, U, mass: float, sigma: float, f_even, antiperiodic: bool = True) -> np.ndarray:
+def mdagm(L, U, mass: float, sigma: float, f_even, antiperiodic: bool = True, theta=None) -> np.ndarray:
     """(m^2 + sigma) f - D_eo D_oe f   (Eq. 2)."""
-    U, f_even = _c(U), _c(f_even)
+    U, f_even, theta = _c(U), _c(f_even), _theta(L, theta)
     out = np.empty_like(f_even)
-    lib().oracle_mdagm(_L(L), _p(U), float(mass), float(sigma), _p(f_even), _p(out), int(antiperiodic))
+    if theta is None:
+        lib().oracle_mdagm(_L(L), _p(U), float(mass), float(sigma), _p(f_even), _p(out), int(antiperiodic))
+    else:
+        lib().oracle_mdagm_u1(_L(L), _p(U), _p(theta), float(mass), float(sigma), _p(f_even), _p(out),
+                              int(antiperiodic))
     return out
 
 
@@ -139,7 +160,7 @@ def scatter(L, parity: int, f, full=None) -> np.ndarray:
 
 
 def mshift_cg(L, U, mass: float, b_even, shifts, tol: float, max_iter: int = 100000,
-              antiperiodic: bool = True, sum_order: int = 0):
+              antiperiodic: bool = True, sum_order: int = 0, theta=None):
     """Multi-shift CG for (m^2 - D_eo D_oe + sigma_i) x_i = b.
 
     sum_order 0 (default) adds the per-slice partials of each scalar product in increasing t, 1 in
@@ -152,9 +173,15 @@ def mshift_cg(L, U, mass: float, b_even, shifts, tol: float, max_iter: int = 100
     iters = ctypes.c_int(0)
     freeze = (ctypes.c_int * n)()
     rel = ctypes.c_double(0.0)
-    status = lib().oracle_mshift_cg(_L(L), _p(U), float(mass), int(antiperiodic), _p(b_even), _p(sh), n,
-                                    float(tol), int(max_iter), int(sum_order), _p(x), ctypes.byref(iters), freeze,
-                                    ctypes.byref(rel))
+    theta = _theta(L, theta)
+    if theta is None:
+        status = lib().oracle_mshift_cg(_L(L), _p(U), float(mass), int(antiperiodic), _p(b_even), _p(sh), n,
+                                        float(tol), int(max_iter), int(sum_order), _p(x), ctypes.byref(iters),
+                                        freeze, ctypes.byref(rel))
+    else:
+        status = lib().oracle_mshift_cg_u1(_L(L), _p(U), _p(theta), float(mass), int(antiperiodic), _p(b_even),
+                                           _p(sh), n, float(tol), int(max_iter), int(sum_order), _p(x),
+                                           ctypes.byref(iters), freeze, ctypes.byref(rel))
     return x, dict(status=status, iters=iters.value, freeze_iter=list(freeze), rel_res=rel.value)
 
 

@@ -16,7 +16,11 @@
 //         s_mu(x) = eta_mu(x) bc_mu(x); eta = (1, (-1)^x, (-1)^(x+y), (-1)^(x+y+z));
 //         bc_t(x) = -1 on links leaving the last time slice (antiperiodic), +1 otherwise.
 //     This is the plain definition written out: four nested coordinate loops, no blocking.
+//   * optionally (the *_u1 entry points) the general U(1) field u_mu(x) = cos(theta_mu(x)) + i sin(theta_mu(x))
+//     by which "pseudofermions must be multiplied" together with U_mu(x) -- imaginary chemical potential and
+//     background fields; theta is stored, u recomputed, as the paper does.
 //   * third-row reconstruction r2 = conj(r0 x r1) of a compressed link.
+//   * the rational function alpha0 b + sum_i alpha_i x_i of the Eq. 2 operator.
 //   * the shifted ("multimass") conjugate gradient for (m^2 - D_eo D_oe + sigma_i) x_i = b
 //     (Eq. 2; refs 32, 33).  The paper gives no pseudo-code; the algorithm is
 //     followed step by step in the order and notation of DESIGN.md reading R5.
@@ -79,8 +83,19 @@ double link_sign(const Lattice& lat, int mu, const int c[4], int antiperiodic) {
     return s;
 }
 
-// Apply D to a field living on parity 1-p, result on the sites of parity p.
-void dslash(const Lattice& lat, const cplx* U, const cplx* in, cplx* out, int p, int antiperiodic) {
+// U(1) factor of the link (site lex, direction mu) beyond the staggered phase and the boundary sign:
+// u = cos(theta) + i sin(theta) with theta_mu(x) stored, as the paper does for the imaginary chemical
+// potential and background fields.  theta == NULL means no such field (u = 1).
+cplx u1_factor(const double* theta, int64_t V, int mu, int64_t lex) {
+    if (!theta) return cplx(1.0, 0.0);
+    const double th = theta[(int64_t)mu * V + lex];
+    return cplx(std::cos(th), std::sin(th));
+}
+
+// Apply D to a field living on parity 1-p, result on the sites of parity p.  The hopping term between x and
+// x+mu is s_mu(x) u_mu(x) U_mu(x) forwards and its negative adjoint backwards.
+void dslash(const Lattice& lat, const cplx* U, const double* theta, const cplx* in, cplx* out, int p,
+            int antiperiodic) {
     const int64_t V = lat.V;
 #pragma omp parallel for collapse(2) schedule(static)
     for (int t = 0; t < lat.L[3]; ++t)
@@ -101,8 +116,8 @@ void dslash(const Lattice& lat, const cplx* U, const cplx* in, cplx* out, int p,
                         const cplx* Ub = U + ((int64_t)mu * V + bwd) * 9;    // U_mu(x-mu)
                         const cplx* vf = in + (fwd >> 1) * 3;
                         const cplx* vb = in + (bwd >> 1) * 3;
-                        const double sf = link_sign(lat, mu, c, antiperiodic);
-                        const double sb = link_sign(lat, mu, cb, antiperiodic);
+                        const cplx sf = link_sign(lat, mu, c, antiperiodic) * u1_factor(theta, V, mu, here);
+                        const cplx sb = link_sign(lat, mu, cb, antiperiodic) * std::conj(u1_factor(theta, V, mu, bwd));
                         for (int a = 0; a < 3; ++a) {
                             cplx f = 0.0, b = 0.0;
                             for (int bb = 0; bb < 3; ++bb) {
@@ -174,7 +189,14 @@ void oracle_set_num_threads(int n) {
 void oracle_dslash(const int* L, const double* U, const double* in, double* out, int out_parity,
                    int antiperiodic) {
     Lattice lat = make_lattice(L);
-    dslash(lat, (const cplx*)U, (const cplx*)in, (cplx*)out, out_parity, antiperiodic);
+    dslash(lat, (const cplx*)U, nullptr, (const cplx*)in, (cplx*)out, out_parity, antiperiodic);
+}
+
+// Same with the U(1) field u_mu(x) = exp(i theta_mu(x)), theta[mu][lex].
+void oracle_dslash_u1(const int* L, const double* U, const double* theta, const double* in, double* out,
+                      int out_parity, int antiperiodic) {
+    Lattice lat = make_lattice(L);
+    dslash(lat, (const cplx*)U, theta, (const cplx*)in, (cplx*)out, out_parity, antiperiodic);
 }
 
 // D_oe: even -> odd;  D_eo: odd -> even
@@ -186,17 +208,21 @@ void oracle_deo(const int* L, const double* U, const double* in_odd, double* out
 }
 
 // out = (m^2 + sigma) in - D_eo D_oe in       (Eq. 2; even -> even)
-void oracle_mdagm(const int* L, const double* U, double mass, double sigma, const double* in_even,
-                  double* out_even, int antiperiodic) {
+void oracle_mdagm_u1(const int* L, const double* U, const double* theta, double mass, double sigma,
+                     const double* in_even, double* out_even, int antiperiodic) {
     Lattice lat = make_lattice(L);
     std::vector<cplx> tmp(lat.Vh * 3);
     const cplx* in = (const cplx*)in_even;
     cplx* out = (cplx*)out_even;
-    dslash(lat, (const cplx*)U, in, tmp.data(), 1, antiperiodic);
-    dslash(lat, (const cplx*)U, tmp.data(), out, 0, antiperiodic);
+    dslash(lat, (const cplx*)U, theta, in, tmp.data(), 1, antiperiodic);
+    dslash(lat, (const cplx*)U, theta, tmp.data(), out, 0, antiperiodic);
     const double c = mass * mass + sigma;
 #pragma omp parallel for schedule(static)
     for (int64_t j = 0; j < lat.Vh * 3; ++j) out[j] = c * in[j] - out[j];
+}
+void oracle_mdagm(const int* L, const double* U, double mass, double sigma, const double* in_even,
+                  double* out_even, int antiperiodic) {
+    oracle_mdagm_u1(L, U, nullptr, mass, sigma, in_even, out_even, antiperiodic);
 }
 
 // Gauge-link compression: overwrite the third row of every link by conj(r0 x r1).
@@ -262,9 +288,10 @@ void oracle_scatter(const int* L, int parity, const double* aos, double* full) {
 //   final count if it never froze); *rel_res = sqrt(rr/bb) of the base recurrence residual.
 //   sum_order: order in which the per-slice partials of every scalar product are added (see re_dot).
 //   Returns 0 on convergence, 1 if max_iter was reached, 2 on breakdown (pAp <= 0 or non-finite).
-int oracle_mshift_cg(const int* L, const double* U, double mass, int antiperiodic, const double* b_even,
-                     const double* shifts, int nshift, double tol, int max_iter, int sum_order,
-                     double* x_out, int* iters, int* freeze_iter, double* rel_res) {
+//   theta: the U(1) field of oracle_dslash_u1, or NULL.
+int oracle_mshift_cg_u1(const int* L, const double* U, const double* theta, double mass, int antiperiodic,
+                        const double* b_even, const double* shifts, int nshift, double tol, int max_iter,
+                        int sum_order, double* x_out, int* iters, int* freeze_iter, double* rel_res) {
     Lattice lat = make_lattice(L);
     const int64_t n = lat.Vh * 3;
     const cplx* Uc = (const cplx*)U;
@@ -300,8 +327,8 @@ int oracle_mshift_cg(const int* L, const double* U, double mass, int antiperiodi
     for (;;) {
         // s = B(p) = (m^2 + sigma0) p - D_eo (D_oe p)
         cplx* pb = p[i0].data();
-        dslash(lat, Uc, pb, tmp.data(), 1, antiperiodic);
-        dslash(lat, Uc, tmp.data(), s.data(), 0, antiperiodic);
+        dslash(lat, Uc, theta, pb, tmp.data(), 1, antiperiodic);
+        dslash(lat, Uc, theta, tmp.data(), s.data(), 0, antiperiodic);
 #pragma omp parallel for schedule(static)
         for (int64_t j = 0; j < n; ++j) s[j] = c0 * pb[j] - s[j];
 
@@ -355,6 +382,13 @@ int oracle_mshift_cg(const int* L, const double* U, double mass, int antiperiodi
     *iters = it;
     *rel_res = std::sqrt(rr / bb);
     return status;
+}
+
+int oracle_mshift_cg(const int* L, const double* U, double mass, int antiperiodic, const double* b_even,
+                     const double* shifts, int nshift, double tol, int max_iter, int sum_order,
+                     double* x_out, int* iters, int* freeze_iter, double* rel_res) {
+    return oracle_mshift_cg_u1(L, U, nullptr, mass, antiperiodic, b_even, shifts, nshift, tol, max_iter, sum_order,
+                               x_out, iters, freeze_iter, rel_res);
 }
 
 // Rational function of the operator of Eq. 2 applied to a vector,

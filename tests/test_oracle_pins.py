@@ -386,3 +386,96 @@ def test_rational_apply_product_of_two_inverses():
     assert info["status"] == 0
     back = oracle.mdagm(L, U, mass, s2, oracle.mdagm(L, U, mass, s1, y))
     assert np.linalg.norm(back - b) <= 1e-10 * np.linalg.norm(b)
+
+
+# ---------------------------------------------------------------------------------------------------
+# general U(1) field u_mu(x) = exp(i theta_mu(x)) on the links
+# ---------------------------------------------------------------------------------------------------
+def u1_phases(L, seed=11):
+    return gen.random_u1_phases(L, seed).numpy()
+
+
+@pytest.mark.parametrize("L", [(2, 2, 2, 2), (4, 2, 4, 6), (4, 6, 4, 4)])
+@pytest.mark.parametrize("antiperiodic", [True, False])
+def test_u1_antihermiticity(L, antiperiodic):
+    """u is unitary, so D stays anti-Hermitian: the backward hop must carry conj(u) of the neighbour's link."""
+    U, th = links(L), u1_phases(L)
+    chi, psi = random_parity_field(L, 1), random_parity_field(L, 2)
+    lhs = vdot(chi, oracle.deo(L, U, psi, antiperiodic, theta=th))
+    rhs = -np.conj(vdot(psi, oracle.doe(L, U, chi, antiperiodic, theta=th)))
+    assert abs(lhs - rhs) < 1e-12 * abs(lhs)
+    # and the field does something
+    assert np.abs(oracle.deo(L, U, psi, antiperiodic, theta=th) - oracle.deo(L, U, psi, antiperiodic)).max() > 0.1
+
+
+@pytest.mark.parametrize("L", [(2, 2, 2, 2), (4, 2, 4, 6)])
+def test_u1_gauge_covariance(L):
+    """theta'_mu(x) = theta_mu(x) + a(x) - a(x+mu)  =>  D[theta'] (e^{ia} psi) = e^{ia} D[theta] psi.
+    Pins which site each theta belongs to and the direction of the phase on forward and backward hops."""
+    Lx, Ly, Lz, Lt = L
+    V = int(np.prod(L))
+    U, th = links(L), u1_phases(L)
+    a = np.random.default_rng(4).uniform(-np.pi, np.pi, V)
+    a4 = a.reshape(Lt, Lz, Ly, Lx)
+    th2 = np.stack([th[mu] + a - np.roll(a4, -1, axis=3 - mu).ravel() for mu in range(4)])
+    for p_in in (0, 1):
+        psi = random_parity_field(L, 5 + p_in)
+        m_in, m_out = parity_mask(L, p_in), parity_mask(L, 1 - p_in)
+        psi_g = r(np.exp(1j * a[m_in])[:, None] * c(psi))
+        lhs = c(oracle.dslash(L, U, psi_g, 1 - p_in, True, theta=th2))
+        rhs = np.exp(1j * a[m_out])[:, None] * c(oracle.dslash(L, U, psi, 1 - p_in, True, theta=th))
+        assert np.abs(lhs - rhs).max() < 1e-13
+
+
+@pytest.mark.parametrize("L,k", [((4, 6, 4, 4), (1, 2, 0, 3)), ((2, 4, 6, 8), (1, 0, 2, 5))])
+def test_u1_constant_phase_shifts_the_momentum(L, k):
+    """Unit links, periodic, theta_mu(x) = phi_mu: D_eo D_oe e^{ipx} = -sum_mu sin^2(p_mu + phi_mu) e^{ipx}
+    (an imaginary chemical potential is a constant theta_t).  Pins the sign of theta."""
+    U = gen.unit_links(L).numpy()
+    V = int(np.prod(L))
+    phi = np.array([0.3, -0.7, 1.1, 0.45])
+    th = np.repeat(phi[:, None], V, axis=1)
+    x = coords(L)
+    p = [2 * np.pi * k[mu] / L[mu] for mu in range(4)]
+    wave = np.exp(1j * sum(p[mu] * x[mu] for mu in range(4)))
+    col = np.array([0.3 - 0.2j, 1.0, -0.5j])
+    psi = r(wave[parity_mask(L, 0)][:, None] * col[None, :])
+    out = c(oracle.deo(L, U, oracle.doe(L, U, psi, False, theta=th), False, theta=th))
+    lam = -sum(np.sin(p[mu] + phi[mu]) ** 2 for mu in range(4))
+    assert np.abs(out - lam * c(psi)).max() < 1e-13
+    lam0 = -sum(np.sin(p[mu]) ** 2 for mu in range(4))
+    assert abs(lam - lam0) > 0.05
+
+
+def test_u1_phase_pi_on_the_last_time_links_is_the_antiperiodic_boundary():
+    """"by which we handle antiperiodic boundary conditions": theta = pi on the links leaving
+    t = Lt-1 with the periodic operator must equal the antiperiodic operator without theta."""
+    L = (4, 2, 4, 6)
+    U = links(L)
+    V = int(np.prod(L))
+    th = np.zeros((4, V))
+    th[3, coords(L)[3] == L[3] - 1] = np.pi
+    for p_in in (0, 1):
+        psi = random_parity_field(L, 8 + p_in)
+        a = oracle.dslash(L, U, psi, 1 - p_in, False, theta=th)
+        b = oracle.dslash(L, U, psi, 1 - p_in, True)
+        assert np.abs(a - b).max() < 1e-14
+
+
+def test_u1_mshift_cg_against_dense_solve():
+    L, mass, shifts = (4, 2, 2, 4), 0.05, [1e-2, 1e-1, 1.0]
+    U, th = links(L), u1_phases(L)
+    b = oracle.restrict(L, 0, gen.gaussian_field(L).numpy())
+    n = int(np.prod(L)) // 2 * 3
+    A = np.empty((n, n), dtype=np.complex128)
+    e = np.zeros((n, 2))
+    for j in range(n):
+        e[:] = 0.0
+        e[j, 0] = 1.0
+        A[:, j] = c(oracle.mdagm(L, U, mass, 0.0, e.reshape(-1, 3, 2), True, theta=th)).ravel()
+    assert np.abs(A - A.conj().T).max() < 1e-14 and np.linalg.eigvalsh(A).min() >= mass * mass * (1 - 1e-9)
+    x, info = oracle.mshift_cg(L, U, mass, b, shifts, 1e-11, theta=th)
+    assert info["status"] == 0
+    for i, sigma in enumerate(shifts):
+        ref = np.linalg.solve(A + sigma * np.eye(n), c(b).ravel())
+        assert np.linalg.norm(c(x[i]).ravel() - ref) <= 1e-8 * np.linalg.norm(ref)
