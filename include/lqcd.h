@@ -114,6 +114,19 @@ int    lqcd_set_workspace(lqcd_ctx* ctx, void* dev, size_t bytes);
 int lqcd_set_gauge(lqcd_ctx* ctx, const double* links);
 int lqcd_set_gauge_host(lqcd_ctx* ctx, const double* links /*HOST*/);
 
+/* General U(1) phase field: "we multiply the pseudofermion fields by u_mu(x) U_mu(x)", with
+ * u_mu(x) = exp(i theta_mu(x)) carrying, besides the staggered phases and the boundary sign (which this
+ * library computes from the coordinates), an imaginary chemical potential or a background electromagnetic
+ * field.  With a field set, every operator and solver of this context uses
+ *     (D psi)(x) = 1/2 sum_mu [ s_mu(x) u_mu(x) U_mu(x) psi(x+mu) - s_mu(x-mu) conj(u_mu(x-mu)) U_mu(x-mu)^+ psi(x-mu) ]
+ * (D_oe^dagger = -D_eo still holds).  As in the paper, theta is what is stored (8 bytes per link in double,
+ * 4 in single) and cos/sin are recomputed in the kernel: +64 bytes per site on 1584.
+ *   theta : 4*V doubles, theta[mu*V + lex], radians; copied (into every precision named by
+ *           LQCD_OPT_LINK_PRECISIONS at the time of the call).  NULL switches the field off (u = 1).
+ * Returns after the copy has completed.  Independent of lqcd_set_gauge (either order). */
+int lqcd_set_u1_phases(lqcd_ctx* ctx, const double* theta);
+int lqcd_set_u1_phases_host(lqcd_ctx* ctx, const double* theta /*HOST*/);
+
 /* out_odd = D_oe in_even;  out_even = D_eo in_odd.  Parity vectors. */
 int lqcd_doe(lqcd_ctx* ctx, double* out_odd, const double* in_even);
 int lqcd_deo(lqcd_ctx* ctx, double* out_even, const double* in_odd);

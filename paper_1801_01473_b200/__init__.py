@@ -16,7 +16,7 @@ from .binding import (  # noqa: F401
     LQCD_STAT_SOLVE_MS,
     LqcdError, Lattice, load_library, library_path, EXPORTS,
     lqcd_create, lqcd_destroy, lqcd_set_stream, lqcd_set_option, lqcd_get_option, lqcd_workspace_bytes,
-    lqcd_set_workspace, lqcd_set_gauge, lqcd_set_gauge_host, lqcd_doe, lqcd_deo, lqcd_doe_host, lqcd_deo_host,
+    lqcd_set_workspace, lqcd_set_gauge, lqcd_set_gauge_host, lqcd_set_u1_phases, lqcd_set_u1_phases_host, lqcd_doe, lqcd_deo, lqcd_doe_host, lqcd_deo_host,
     lqcd_mdagm, lqcd_mshift_cg, lqcd_mshift_cg_host, lqcd_rational_apply, lqcd_rational_apply_host, lqcd_get_stat, lqcd_pack_vector, lqcd_unpack_vector,
     lqcd_last_error,
     lqcd_doe_f32, lqcd_deo_f32, lqcd_doe_f32_host, lqcd_deo_f32_host, lqcd_mdagm_f32, lqcd_mshift_cg_f32,

@@ -33,6 +33,8 @@ EXPORTS = {
     "lqcd_set_workspace": (_i, [_vp, _vp, _sz]),
     "lqcd_set_gauge": (_i, [_vp, _dp]),
     "lqcd_set_gauge_host": (_i, [_vp, _dp]),
+    "lqcd_set_u1_phases": (_i, [_vp, _dp]),
+    "lqcd_set_u1_phases_host": (_i, [_vp, _dp]),
     "lqcd_doe": (_i, [_vp, _dp, _dp]),
     "lqcd_deo": (_i, [_vp, _dp, _dp]),
     "lqcd_doe_host": (_i, [_vp, _dp, _dp]),
@@ -127,6 +129,14 @@ def lqcd_set_gauge(ctx, links):
 
 def lqcd_set_gauge_host(ctx, links):
     return load_library().lqcd_set_gauge_host(ctx, links)
+
+
+def lqcd_set_u1_phases(ctx, theta):
+    return load_library().lqcd_set_u1_phases(ctx, theta)
+
+
+def lqcd_set_u1_phases_host(ctx, theta):
+    return load_library().lqcd_set_u1_phases_host(ctx, theta)
 
 
 def lqcd_doe(ctx, out_odd, in_even):
@@ -334,6 +344,19 @@ class Lattice:
             self._check(lqcd_set_gauge(self.ctx, p))
         else:
             self._check(lqcd_set_gauge_host(self.ctx, p))
+
+    def set_u1_phases(self, theta):
+        """theta: (4, V) float64 angles of u_mu(x) = exp(i theta_mu(x)) (PAPER.md:L159), CUDA or CPU tensor;
+        None switches the field off."""
+        self._sync_stream()
+        if theta is None:
+            self._check(lqcd_set_u1_phases(self.ctx, None))
+            return
+        p = self._t(theta, (4, self.V))
+        if theta.device.type == "cuda":
+            self._check(lqcd_set_u1_phases(self.ctx, p))
+        else:
+            self._check(lqcd_set_u1_phases_host(self.ctx, p))
 
     def _apply(self, fns, v, out):
         torch = self._torch

@@ -251,6 +251,17 @@ __global__ void __launch_bounds__(256) repack_gauge_kernel(Geom g, const double2
     }
 }
 
+// canonical U(1) angles theta[mu][lex] -> Th[(mu*2+par)*Vh + k] (theta is what is stored)
+template <typename T>
+__global__ void __launch_bounds__(256) repack_theta_kernel(Geom g, const double* __restrict__ theta, T* __restrict__ Th) {
+    const size_t vh = (size_t)g.Vh;
+    const size_t idx = (size_t)blockIdx.x * 256 + threadIdx.x;
+    if (idx >= 8 * vh) return;
+    const int k = (int)(idx % vh);
+    const int mp = (int)(idx / vh);          // mu*2 + par
+    Th[idx] = (T)theta[(size_t)(mp >> 1) * 2 * vh + lex_of(g, k, mp & 1)];
+}
+
 // site field [lex][3] <-> parity vector [c][k]
 template <typename T>
 __global__ void __launch_bounds__(256) pack_vector_kernel(Geom g, int par, const V2<T>* __restrict__ site, V2<T>* __restrict__ pv) {

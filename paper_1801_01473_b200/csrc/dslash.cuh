@@ -13,6 +13,11 @@
 // Links are streamed once (L1 no-allocate, L2 evict-first policy); neighbour vectors are re-used 8 times
 // across sites and are kept in L1/L2 (evict-last policy).
 //
+// U1 = 1 : every hop also carries the general U(1) factor u_mu(x) = exp(i theta_mu(x)) (imaginary chemical
+//          potential, background fields).  As in the paper theta is what is stored and read
+//          (8 B per link in double instead of 16 for u) and cos/sin are recomputed in registers: the kernel is
+//          HBM-bound, the FP pipes have room.  Th[(mu*2 + parity_of_origin)*Vh + k].
+//
 // EPI = 0 : out = D in
 // EPI = 1 : out = coef*pv - D in, plus the block partial of Re<pv, out> and the CG scalar step
 //           (this is the paper's separate zaxpy kernel, fused into the D_eo epilogue)
@@ -108,6 +113,35 @@ __device__ __forceinline__ V cmul(const V a, const V b) {
     return make_v2(a.x * b.x - a.y * b.y, a.x * b.y + a.y * b.x);
 }
 
+// streamed scalar (the U(1) angle of one link)
+__device__ __forceinline__ double ld_stream_scalar(const double* p, uint64_t pol) {
+    double v;
+    asm("ld.global.nc.L1::no_allocate.L2::cache_hint.f64 %0, [%1], %2;" : "=d"(v) : "l"(p), "l"(pol));
+    return v;
+}
+__device__ __forceinline__ float ld_stream_scalar(const float* p, uint64_t pol) {
+    float v;
+    asm("ld.global.nc.L1::no_allocate.L2::cache_hint.f32 %0, [%1], %2;" : "=f"(v) : "l"(p), "l"(pol));
+    return v;
+}
+__device__ __forceinline__ void sincos_t(double th, double* s, double* c) { sincos(th, s, c); }
+__device__ __forceinline__ void sincos_t(float th, float* s, float* c) { sincosf(th, s, c); }
+
+// v <- exp(+-i theta) v  (sgn = +1: forward hop, u; sgn = -1: backward hop, conj(u))
+template <typename T, int SGN>
+__device__ __forceinline__ void u1_rotate(const T* __restrict__ th, uint64_t pol, T (&vr)[3], T (&vi)[3]) {
+    T s, c;
+    sincos_t(ld_stream_scalar(th, pol), &s, &c);
+    if (SGN < 0) s = -s;
+#pragma unroll
+    for (int a = 0; a < 3; ++a) {
+        const T re = fma(c, vr[a], -(s * vi[a]));
+        const T im = fma(c, vi[a], s * vr[a]);
+        vr[a] = re;
+        vi[a] = im;
+    }
+}
+
 // Load one link (9 complex).  12-real storage: rows 0,1 are read, r2 = conj(r0 x r1).
 template <typename T, int RECON>
 __device__ __forceinline__ void load_link(const V2<T>* __restrict__ w, const size_t vh, uint64_t pol, V2<T> (&u)[9]) {
@@ -134,14 +168,15 @@ __device__ __forceinline__ void load_vec(const V2<T>* __restrict__ v, const size
 }
 
 // acc += sign * U v          (forward hop; the sign is already folded into v)
-template <typename T, int RECON>
+template <typename T, int RECON, int U1>
 __device__ __forceinline__ void hop_fwd(T (&ar)[3], T (&ai)[3], const V2<T>* __restrict__ w,
                                         const V2<T>* __restrict__ v, const size_t vh, unsigned int mask,
-                                        uint64_t pol_s, uint64_t pol_r) {
+                                        uint64_t pol_s, uint64_t pol_r, const T* __restrict__ th) {
     V2<T> u[9];
     T vr[3], vi[3];
     load_link<T, RECON>(w, vh, pol_s, u);
     load_vec<T>(v, vh, pol_r, mask, vr, vi);
+    if (U1) u1_rotate<T, +1>(th, pol_s, vr, vi);
 #pragma unroll
     for (int a = 0; a < 3; ++a)
 #pragma unroll
@@ -149,14 +184,15 @@ __device__ __forceinline__ void hop_fwd(T (&ar)[3], T (&ai)[3], const V2<T>* __r
 }
 
 // acc += sign * U^dagger v   (backward hop; caller passes the mask of -s)
-template <typename T, int RECON>
+template <typename T, int RECON, int U1>
 __device__ __forceinline__ void hop_bwd(T (&ar)[3], T (&ai)[3], const V2<T>* __restrict__ w,
                                         const V2<T>* __restrict__ v, const size_t vh, unsigned int mask,
-                                        uint64_t pol_s, uint64_t pol_r) {
+                                        uint64_t pol_s, uint64_t pol_r, const T* __restrict__ th) {
     V2<T> u[9];
     T vr[3], vi[3];
     load_link<T, RECON>(w, vh, pol_s, u);
     load_vec<T>(v, vh, pol_r, mask, vr, vi);
+    if (U1) u1_rotate<T, -1>(th, pol_s, vr, vi);
 #pragma unroll
     for (int a = 0; a < 3; ++a)
 #pragma unroll
@@ -167,6 +203,7 @@ template <typename T>
 struct DslashArgs {
     Geom g;
     const V2<T>* W;          // stored links
+    const T* Th;             // U1 == 1: stored U(1) angles theta_mu(x)
     const V2<T>* in;         // parity 1-par
     V2<T>* out;              // parity par
     int par;                 // parity of the output sites
@@ -181,7 +218,7 @@ struct DslashArgs {
 template <typename T> struct DsOcc { static constexpr int minb = DS_MINB; };
 template <> struct DsOcc<float> { static constexpr int minb = DS_MINB_F32; };
 
-template <typename T, int RECON, int EPI>
+template <typename T, int RECON, int EPI, int U1>
 __global__ void __launch_bounds__(DS_BLOCK, DsOcc<T>::minb) dslash_kernel(const DslashArgs<T> A) {
     constexpr int NE = (RECON == 12) ? 6 : 9;
     if (A.check_stop) {
@@ -246,14 +283,17 @@ __global__ void __launch_bounds__(DS_BLOCK, DsOcc<T>::minb) dslash_kernel(const 
     }
 
     T ar[3] = {(T)0, (T)0, (T)0}, ai[3] = {(T)0, (T)0, (T)0};
-    hop_fwd<T, RECON>(ar, ai, Wf + 0 * mu_stride, in + kxf, vh, 0u, pol_s, pol_r);
-    hop_bwd<T, RECON>(ar, ai, Wb + 0 * mu_stride + kxb, in + kxb, vh, SB, pol_s, pol_r);
-    hop_fwd<T, RECON>(ar, ai, Wf + 1 * mu_stride, in + kyf, vh, my, pol_s, pol_r);
-    hop_bwd<T, RECON>(ar, ai, Wb + 1 * mu_stride + kyb, in + kyb, vh, my ^ SB, pol_s, pol_r);
-    hop_fwd<T, RECON>(ar, ai, Wf + 2 * mu_stride, in + kzf, vh, mz, pol_s, pol_r);
-    hop_bwd<T, RECON>(ar, ai, Wb + 2 * mu_stride + kzb, in + kzb, vh, mz ^ SB, pol_s, pol_r);
-    hop_fwd<T, RECON>(ar, ai, Wf + 3 * mu_stride, in + ktf, vh, mtf, pol_s, pol_r);
-    hop_bwd<T, RECON>(ar, ai, Wb + 3 * mu_stride + ktb, in + ktb, vh, mtb ^ SB, pol_s, pol_r);
+    const T* __restrict__ Tf = U1 ? A.Th + (size_t)A.par * vh + k : nullptr;     // angles of the forward links
+    const T* __restrict__ Tb = U1 ? A.Th + (size_t)(1 - A.par) * vh : nullptr;   // angles of the backward links
+    const size_t th_stride = 2 * vh;
+    hop_fwd<T, RECON, U1>(ar, ai, Wf + 0 * mu_stride, in + kxf, vh, 0u, pol_s, pol_r, Tf + 0 * th_stride);
+    hop_bwd<T, RECON, U1>(ar, ai, Wb + 0 * mu_stride + kxb, in + kxb, vh, SB, pol_s, pol_r, Tb + 0 * th_stride + kxb);
+    hop_fwd<T, RECON, U1>(ar, ai, Wf + 1 * mu_stride, in + kyf, vh, my, pol_s, pol_r, Tf + 1 * th_stride);
+    hop_bwd<T, RECON, U1>(ar, ai, Wb + 1 * mu_stride + kyb, in + kyb, vh, my ^ SB, pol_s, pol_r, Tb + 1 * th_stride + kyb);
+    hop_fwd<T, RECON, U1>(ar, ai, Wf + 2 * mu_stride, in + kzf, vh, mz, pol_s, pol_r, Tf + 2 * th_stride);
+    hop_bwd<T, RECON, U1>(ar, ai, Wb + 2 * mu_stride + kzb, in + kzb, vh, mz ^ SB, pol_s, pol_r, Tb + 2 * th_stride + kzb);
+    hop_fwd<T, RECON, U1>(ar, ai, Wf + 3 * mu_stride, in + ktf, vh, mtf, pol_s, pol_r, Tf + 3 * th_stride);
+    hop_bwd<T, RECON, U1>(ar, ai, Wb + 3 * mu_stride + ktb, in + ktb, vh, mtb ^ SB, pol_s, pol_r, Tb + 3 * th_stride + ktb);
 
     if (EPI == 0) {
         if (valid) {

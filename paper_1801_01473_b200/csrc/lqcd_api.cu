@@ -33,6 +33,8 @@ struct PrecBufs {
     V2<T>* W = nullptr;      // stored links
     size_t W_bytes = 0;
     int recon_stored = 0;    // 0 = no gauge in this precision, else 18 or 12
+    T* Th = nullptr;         // stored U(1) angles theta_mu(x) (lqcd_set_u1_phases), [(mu*2+par)*Vh + k]
+    int u1_stored = 0;
     V2<T> *r = nullptr, *p = nullptr, *s = nullptr, *t = nullptr;
     V2<T>* pextra[LQCD_MAX_SHIFTS] = {};
     int n_pextra = 0;
@@ -63,6 +65,7 @@ struct lqcd_ctx {
     PrecBufs<double> d;
     PrecBufs<float> f;
     int prec_opt;            // LQCD_OPT_LINK_PRECISIONS: which of them the next lqcd_set_gauge stores
+    int u1_on;               // general U(1) phases in force (lqcd_set_u1_phases with a non-NULL field)
     double* dev_max;
 
     double* partials;
@@ -208,13 +211,18 @@ int ensure_solver(lqcd_ctx* c, int nshift) {
     return LQCD_OK;
 }
 
+template <typename T, int EPI, int U1>
+void launch_dslash_u(lqcd_ctx* c, const DslashArgs<T>& a) {
+    if (bufs<T>(c).recon_stored == 12)
+        dslash_kernel<T, 12, EPI, U1><<<ds_grid(c), DS_BLOCK, 0, c->stream>>>(a);
+    else
+        dslash_kernel<T, 18, EPI, U1><<<ds_grid(c), DS_BLOCK, 0, c->stream>>>(a);
+    ++c->launches;
+}
 template <typename T, int EPI>
 void launch_dslash_t(lqcd_ctx* c, const DslashArgs<T>& a) {
-    if (bufs<T>(c).recon_stored == 12)
-        dslash_kernel<T, 12, EPI><<<ds_grid(c), DS_BLOCK, 0, c->stream>>>(a);
-    else
-        dslash_kernel<T, 18, EPI><<<ds_grid(c), DS_BLOCK, 0, c->stream>>>(a);
-    ++c->launches;
+    if (c->u1_on) launch_dslash_u<T, EPI, 1>(c, a);
+    else launch_dslash_u<T, EPI, 0>(c, a);
 }
 
 // out(par) = D in, optionally with the epilogue
@@ -224,6 +232,7 @@ void launch_dslash(lqcd_ctx* c, int epi, V2<T>* out, const V2<T>* in, int par, c
     DslashArgs<T> a;
     a.g = c->g;
     a.W = bufs<T>(c).W;
+    a.Th = bufs<T>(c).Th;
     a.in = in;
     a.out = out;
     a.par = par;
@@ -286,6 +295,9 @@ int check_ctx_gauge(lqcd_ctx* c) {
     if (!bufs<T>(c).recon_stored)
         return fail(c, LQCD_ENOGAUGE, "no %s-precision gauge field stored (lqcd_set_gauge, LQCD_OPT_LINK_PRECISIONS)",
                     sizeof(T) == 8 ? "double" : "single");
+    if (c->u1_on && !bufs<T>(c).u1_stored)
+        return fail(c, LQCD_ENOGAUGE, "U(1) phases are on but not stored in %s precision (lqcd_set_u1_phases after "
+                    "LQCD_OPT_LINK_PRECISIONS)", sizeof(T) == 8 ? "double" : "single");
     return LQCD_OK;
 }
 
@@ -330,6 +342,21 @@ int store_gauge(lqcd_ctx* c, const double* links, int recon) {
     if (recon == 12 && !(*c->max_host <= 1e-12))
         return fail(c, LQCD_ENOTSU3, "RECON=12 but max|r2 - conj(r0 x r1)| = %.3e > 1e-12", *c->max_host);
     B.recon_stored = recon;
+    return LQCD_OK;
+}
+
+// Store the U(1) angles in precision T: canonical theta[mu][lex] -> Th[(mu*2+par)*Vh + k].
+template <typename T>
+int store_theta(lqcd_ctx* c, const double* theta) {
+    int rc;
+    PrecBufs<T>& B = bufs<T>(c);
+    B.u1_stored = 0;
+    if (!B.Th && (rc = dev_alloc(c, (void**)&B.Th, (size_t)8 * c->Vh * sizeof(T)))) return rc;
+    const size_t nthreads = 8 * c->Vh;
+    repack_theta_kernel<T><<<(int)((nthreads + 255) / 256), 256, 0, c->stream>>>(c->g, theta, B.Th);
+    ++c->launches;
+    CU(cudaGetLastError());
+    B.u1_stored = 1;
     return LQCD_OK;
 }
 
@@ -397,6 +424,7 @@ lqcd_ctx* lqcd_create(int Lx, int Ly, int Lz, int Lt) {
     c->mass = 0.0;
     c->recon_opt = 18;
     c->prec_opt = LQCD_PREC_F64;
+    c->u1_on = 0;
     c->max_iter = 100000;
     c->check_every = 0;
     c->use_graph = 1;
@@ -491,6 +519,8 @@ size_t lqcd_workspace_bytes(const lqcd_ctx* c, int nshift) {
         b += align_up(links_bytes<double>(c, 18)) + align_up(vec_bytes<double>(c)) * (size_t)(4 + (nshift - 1));
     if (c->prec_opt & LQCD_PREC_F32)
         b += align_up(links_bytes<float>(c, 18)) + align_up(vec_bytes<float>(c)) * (size_t)(4 + (nshift - 1));
+    if (c->prec_opt & LQCD_PREC_F64) b += align_up((size_t)8 * c->Vh * sizeof(double));   // U(1) angles, if set
+    if (c->prec_opt & LQCD_PREC_F32) b += align_up((size_t)8 * c->Vh * sizeof(float));
     b += align_up(sizeof(CgState)) + align_up(sizeof(double));
     const size_t np = (size_t)(ds_grid(c) > cg_grid(c) ? ds_grid(c) : cg_grid(c));
     b += align_up(np * sizeof(double));
@@ -530,6 +560,40 @@ int lqcd_set_gauge(lqcd_ctx* c, const double* links) {
         release_gauge<float>(c);
     }
     return LQCD_OK;
+}
+
+int lqcd_set_u1_phases(lqcd_ctx* c, const double* theta) {
+    if (!c) return LQCD_EINVAL;
+    int rc;
+    if ((rc = ensure_basics(c))) return rc;
+    drop_graphs(c);           // the kernel variant and its arguments are baked into the graph
+    c->u1_on = 0;
+    c->d.u1_stored = c->f.u1_stored = 0;
+    if (!theta) return LQCD_OK;
+    if ((c->prec_opt & LQCD_PREC_F64) && (rc = store_theta<double>(c, theta))) return rc;
+    if ((c->prec_opt & LQCD_PREC_F32) && (rc = store_theta<float>(c, theta))) return rc;
+    CU(cudaStreamSynchronize(c->stream));       // theta may be freed by the caller on return
+    c->u1_on = 1;
+    return LQCD_OK;
+}
+
+int lqcd_set_u1_phases_host(lqcd_ctx* c, const double* theta) {
+    if (!c) return LQCD_EINVAL;
+    if (!theta) return lqcd_set_u1_phases(c, nullptr);
+    const size_t bytes = (size_t)4 * c->V * sizeof(double);
+    void* tmp = nullptr;
+    cudaError_t e = cudaMalloc(&tmp, bytes);
+    if (e != cudaSuccess) {
+        cudaGetLastError();
+        return fail(c, LQCD_ENOMEM, "cudaMalloc(%zu) for the canonical U(1) angles failed", bytes);
+    }
+    e = cudaMemcpyAsync(tmp, theta, bytes, cudaMemcpyHostToDevice, c->stream);
+    int rc = LQCD_OK;
+    if (e != cudaSuccess) rc = fail(c, LQCD_ECUDA, "copy of the U(1) angles failed: %s", cudaGetErrorString(e));
+    if (!rc) rc = lqcd_set_u1_phases(c, (const double*)tmp);
+    cudaStreamSynchronize(c->stream);
+    cudaFree(tmp);
+    return rc;
 }
 
 int lqcd_set_gauge_host(lqcd_ctx* c, const double* links) {
