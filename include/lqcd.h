@@ -80,6 +80,11 @@ typedef struct lqcd_ctx lqcd_ctx;
 #define LQCD_OPT_LINK_PRECISIONS 6  /* which copies of the links the next lqcd_set_gauge stores: LQCD_PREC_F64
                                        (default; serves the double entry points), LQCD_PREC_F32 (serves the
                                        *_f32 entry points), or both OR-ed together                         */
+#define LQCD_OPT_SHIFT_BLOCK     7  /* m in [1,16], default 8: the x_i, p_i of the shifted systems are updated once
+                                       per block of m iterations from the m residuals of the block (kept in m
+                                       extra vectors) instead of once per iteration; same recurrences, same
+                                       iteration counts, x_i equal up to rounding.  m = 1: every iteration.
+                                       CHECK_EVERY is rounded up to a multiple of m.                        */
 #define LQCD_PREC_F64 1
 #define LQCD_PREC_F32 2
 

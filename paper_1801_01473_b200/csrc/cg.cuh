@@ -1,12 +1,18 @@
 // cg.cuh -- the vector sweeps of the multi-shift CG (steps A7, A8 of DESIGN.md) and layout kernels.
 //
-// One CG iteration is four launches ("scalar products and sums" + the two operators):
+// One CG iteration is four launches ("scalar products and sums" + the two operators), plus one
+// sweep over the shifted systems every m iterations:
 //   K1  t  = D_oe p                                         dslash_kernel<.,0>
-//   K2  s  = (m^2+sigma0) p - D_eo t ;  Re<p,s>  -> a, zeta_new_i, a_i      dslash_kernel<.,1>
-//   K3  r -= a s ;  |r|^2  -> beta, b_i, freeze flags, stop flag            cg_update_r_kernel
-//   K4  for every shift active in this iteration:  x_i += a_i p_i ;  p_i = zeta_new_i r + b_i p_i
-//                                                                           cg_update_xp_kernel
-// p_i is read once per iteration (x_i and p_i updates share the load).  All scalars stay on the device.
+//   K2  s  = (m^2+sigma0) p - D_eo t ;  Re<p,s>  -> a, zeta_new_i, block coefficients   dslash_kernel<.,1>
+//   K3  r_new = r - a s ;  |r_new|^2  -> beta, b_i, block coefficients, freeze flags, stop flag
+//                                                                           cg_update_r_kernel
+//   K4  base system only:  x_0 += a p ;  p = r_new + beta p                 cg_update_base_kernel
+//   K5  every m-th iteration (and once after the stop), for every shifted system of the block:
+//         x_i += CP_i p_i + sum_l D_il r_l ;  p_i = B_i p_i + sum_l E_il r_l      cg_flush_kernel
+// K3 writes r_new into a ring of m residual vectors instead of over r, so that the m residuals of a block
+// are still there when K5 runs: the 192 B per site and active shift of the x_i/p_i update are paid once per
+// block instead of once per iteration (CgState in lqcd_internal.cuh has the algebra).
+// All scalars stay on the device.
 #ifndef LQCD_CG_CUH
 #define LQCD_CG_CUH
 
@@ -14,8 +20,10 @@
 #include "reduce.cuh"
 
 #define CG_BLOCK 256
+static_assert(CG_BLOCK >= LQCD_MAX_SHIFTS, "the scalar step needs one thread per shift");
 
 // K0: r = p_i = b, x_i = 0, |b|^2.  In every sweep the vectors are V2<T>; scalars and sums are double.
+// r is the ring slot that holds r^(n0) of the first block.
 template <typename T>
 __global__ void __launch_bounds__(CG_BLOCK) cg_init_kernel(const V2<T>* __restrict__ b, V2<T>* __restrict__ r,
                                                            CgState* st, double* partials, size_t n, double tol) {
@@ -49,10 +57,11 @@ __global__ void __launch_bounds__(CG_BLOCK) cg_init_kernel(const V2<T>* __restri
     }
 }
 
-// K3: r -= a s, |r|^2, then the scalar step that needs it
+// K3: r_out = r_in - a s, |r_out|^2, then the scalar step that needs it
 template <typename T>
-__global__ void __launch_bounds__(CG_BLOCK) cg_update_r_kernel(V2<T>* __restrict__ r, const V2<T>* __restrict__ s,
-                                                               CgState* st, double* partials, size_t n) {
+__global__ void __launch_bounds__(CG_BLOCK) cg_update_r_kernel(const V2<T>* r_in, V2<T>* r_out,
+                                                               const V2<T>* __restrict__ s, CgState* st,
+                                                               double* partials, size_t n) {
     if (st->stop) return;
     __shared__ double red[32];
     __shared__ int last_flag;
@@ -64,134 +73,236 @@ __global__ void __launch_bounds__(CG_BLOCK) cg_update_r_kernel(V2<T>* __restrict
         V2<T> rv[4], sv[4];
 #pragma unroll
         for (int u = 0; u < 4; ++u) {
-            rv[u] = r[j + u * stride];
+            rv[u] = r_in[j + u * stride];
             sv[u] = s[j + u * stride];
         }
 #pragma unroll
         for (int u = 0; u < 4; ++u) {
             rv[u].x = fma(-a, sv[u].x, rv[u].x);
             rv[u].y = fma(-a, sv[u].y, rv[u].y);
-            r[j + u * stride] = rv[u];
+            r_out[j + u * stride] = rv[u];
             acc = fma((double)rv[u].x, (double)rv[u].x, acc);
             acc = fma((double)rv[u].y, (double)rv[u].y, acc);
         }
     }
     for (; j < n; j += stride) {
-        V2<T> rv = r[j];
+        V2<T> rv = r_in[j];
         const V2<T> sv = s[j];
         rv.x = fma(-a, sv.x, rv.x);
         rv.y = fma(-a, sv.y, rv.y);
-        r[j] = rv;
+        r_out[j] = rv;
         acc = fma((double)rv.x, (double)rv.x, acc);
         acc = fma((double)rv.y, (double)rv.y, acc);
     }
     const double bsum = block_sum<CG_BLOCK>(acc, red);
     if (publish_partial<CG_BLOCK>(bsum, partials, &st->ticket[2], &last_flag)) {
-        const double rr = final_sum<CG_BLOCK>(partials, gridDim.x, red);
-        if (threadIdx.x == 0) {
-            st->ticket[2] = 0;
-            cg_scalars_after_rr(st, rr);
-        }
+        const double rr = broadcast0(final_sum<CG_BLOCK>(partials, gridDim.x, red), red);
+        if (threadIdx.x == 0) st->ticket[2] = 0;
+        cg_scalars_after_rr(st, rr);
     }
 }
 
-// K4: x_i += a_i p_i ; p_i = zeta_new_i r + b_i p_i   for the shifts on this iteration's list
+// K4: the base system (zeta = 1):  x_0 += a p  (rational mode: y += alpha_0 a p) ;  p = r_new + beta p
 template <typename T>
-__global__ void __launch_bounds__(CG_BLOCK) cg_update_xp_kernel(const V2<T>* __restrict__ r, const CgState* st, size_t n) {
+__global__ void __launch_bounds__(CG_BLOCK) cg_update_base_kernel(const V2<T>* __restrict__ r, V2<T>* __restrict__ p,
+                                                                  const CgState* st, size_t n) {
     if (st->stop4) return;
-    __shared__ V2<T>* sx[LQCD_MAX_SHIFTS];
-    __shared__ V2<T>* sp[LQCD_MAX_SHIFTS];
-    __shared__ T sa[LQCD_MAX_SHIFTS], sz[LQCD_MAX_SHIFTS], sb[LQCD_MAX_SHIFTS];
-    const int nl = st->nlist;
-    for (int e = threadIdx.x; e < nl; e += CG_BLOCK) {
-        const int i = st->list_idx[e];
-        sx[e] = (V2<T>*)st->x[i];
-        sp[e] = (V2<T>*)st->p[i];
-        sa[e] = (T)st->list_a[e];
-        sz[e] = (T)st->list_zn[e];
-        sb[e] = (T)st->list_b[e];
+    const int i0 = st->i0;
+    const T bt = (T)st->b_prev;
+    const T a = (T)(st->rational ? st->alpha[i0] * st->a : st->a);
+    V2<T>* __restrict__ x = (V2<T>*)(st->rational ? st->y : st->x[i0]);
+    const size_t stride = (size_t)gridDim.x * CG_BLOCK;
+    size_t j = (size_t)blockIdx.x * CG_BLOCK + threadIdx.x;
+    for (; j + stride < n; j += 2 * stride) {
+        V2<T> rv[2], pv[2], xv[2];
+#pragma unroll
+        for (int u = 0; u < 2; ++u) {
+            rv[u] = r[j + u * stride];
+            pv[u] = p[j + u * stride];
+            xv[u] = x[j + u * stride];
+        }
+#pragma unroll
+        for (int u = 0; u < 2; ++u) {
+            xv[u].x = fma(a, pv[u].x, xv[u].x);
+            xv[u].y = fma(a, pv[u].y, xv[u].y);
+            pv[u].x = fma(bt, pv[u].x, rv[u].x);
+            pv[u].y = fma(bt, pv[u].y, rv[u].y);
+            x[j + u * stride] = xv[u];
+            p[j + u * stride] = pv[u];
+        }
     }
-    __syncthreads();
+    for (; j < n; j += stride) {
+        const V2<T> rv = r[j];
+        V2<T> pv = p[j], xv = x[j];
+        xv.x = fma(a, pv.x, xv.x);
+        xv.y = fma(a, pv.y, xv.y);
+        pv.x = fma(bt, pv.x, rv.x);
+        pv.y = fma(bt, pv.y, rv.y);
+        x[j] = xv;
+        p[j] = pv;
+    }
+}
+
+// K5: the deferred updates of one block, for every shifted system that was active when the block began.
+// nres = st->blk_j residuals r_l = hist[l] are used (nres = m for a full block, less after the stop).
+//   x_i += CP_i p_i + sum_l D_il r_l   (rational mode: y += sum_i of that; alpha_i is inside CP, D)
+//   p_i  = B_i p_i + sum_l E_il r_l
+// MM = compile-time bound on nres (registers for the residuals).  The block that finishes last closes the
+// block of iterations (blk_j = 0), which also makes a second launch of this kernel a no-op.
+template <typename T, int MM, bool RATIONAL, bool FULL>
+__device__ __forceinline__ void cg_flush_body(const int nres, const int nl, V2<T>* const* sx, V2<T>* const* sp,
+                                              const V2<T>* const* sr, const T* sCP, const T* sB, const V2<T>* sDE,
+                                              const T* sY, V2<T>* __restrict__ y, const size_t n) {
     const size_t stride = (size_t)gridDim.x * CG_BLOCK;
     for (size_t j = (size_t)blockIdx.x * CG_BLOCK + threadIdx.x; j < n; j += stride) {
-        const V2<T> rv = r[j];
-        int e = 0;
-        for (; e + 4 <= nl; e += 4) {
-            V2<T> xv[4], pv[4];
+        V2<T> rv[MM];
 #pragma unroll
-            for (int u = 0; u < 4; ++u) {
-                xv[u] = sx[e + u][j];
+        for (int l = 0; l < MM; ++l)
+            if (FULL || l < nres) rv[l] = sr[l][j];
+        V2<T> yv;
+        if (RATIONAL) {
+            yv = y[j];
+#pragma unroll
+            for (int l = 0; l < MM; ++l)
+                if (FULL || l < nres) {
+                    yv.x = fma(sY[l], rv[l].x, yv.x);
+                    yv.y = fma(sY[l], rv[l].y, yv.y);
+                }
+        }
+        int e = 0;
+        for (; e + 2 <= nl; e += 2) {
+            V2<T> pv[2], xv[2];
+#pragma unroll
+            for (int u = 0; u < 2; ++u) {
                 pv[u] = sp[e + u][j];
+                if (!RATIONAL) xv[u] = sx[e + u][j];
             }
 #pragma unroll
-            for (int u = 0; u < 4; ++u) {
-                const T a = sa[e + u], zn = sz[e + u], bi = sb[e + u];
-                xv[u].x = fma(a, pv[u].x, xv[u].x);
-                xv[u].y = fma(a, pv[u].y, xv[u].y);
-                pv[u].x = fma(zn, rv.x, bi * pv[u].x);
-                pv[u].y = fma(zn, rv.y, bi * pv[u].y);
-                sx[e + u][j] = xv[u];
-                sp[e + u][j] = pv[u];
+            for (int u = 0; u < 2; ++u) {
+                const T cp = sCP[e + u], bb = sB[e + u];
+                T dx = cp * pv[u].x, dy = cp * pv[u].y;
+                T px = bb * pv[u].x, py = bb * pv[u].y;
+                if (!RATIONAL) {
+#pragma unroll
+                    for (int l = 0; l < MM; ++l)
+                        if (FULL || l < nres) {
+                            const V2<T> de = sDE[(e + u) * MM + l];
+                            dx = fma(de.x, rv[l].x, dx);
+                            dy = fma(de.x, rv[l].y, dy);
+                            px = fma(de.y, rv[l].x, px);
+                            py = fma(de.y, rv[l].y, py);
+                        }
+                    xv[u].x += dx;
+                    xv[u].y += dy;
+                    sx[e + u][j] = xv[u];
+                } else {
+#pragma unroll
+                    for (int l = 0; l < MM; ++l)
+                        if (FULL || l < nres) {
+                            const V2<T> de = sDE[(e + u) * MM + l];
+                            px = fma(de.y, rv[l].x, px);
+                            py = fma(de.y, rv[l].y, py);
+                        }
+                    yv.x += dx;
+                    yv.y += dy;
+                }
+                sp[e + u][j] = make_v2(px, py);
             }
         }
         for (; e < nl; ++e) {
-            V2<T> xv = sx[e][j], pv = sp[e][j];
-            const T a = sa[e], zn = sz[e], bi = sb[e];
-            xv.x = fma(a, pv.x, xv.x);
-            xv.y = fma(a, pv.y, xv.y);
-            pv.x = fma(zn, rv.x, bi * pv.x);
-            pv.y = fma(zn, rv.y, bi * pv.y);
-            sx[e][j] = xv;
-            sp[e][j] = pv;
+            const V2<T> pv = sp[e][j];
+            const T cp = sCP[e], bb = sB[e];
+            T dx = cp * pv.x, dy = cp * pv.y;
+            T px = bb * pv.x, py = bb * pv.y;
+#pragma unroll
+            for (int l = 0; l < MM; ++l)
+                if (FULL || l < nres) {
+                    const V2<T> de = sDE[e * MM + l];
+                    if (!RATIONAL) {
+                        dx = fma(de.x, rv[l].x, dx);
+                        dy = fma(de.x, rv[l].y, dy);
+                    }
+                    px = fma(de.y, rv[l].x, px);
+                    py = fma(de.y, rv[l].y, py);
+                }
+            if (!RATIONAL) {
+                V2<T> xv = sx[e][j];
+                xv.x += dx;
+                xv.y += dy;
+                sx[e][j] = xv;
+            } else {
+                yv.x += dx;
+                yv.y += dy;
+            }
+            sp[e][j] = make_v2(px, py);
         }
+        if (RATIONAL) y[j] = yv;
     }
 }
 
-// K4 of lqcd_rational_apply: y += sum_i (alpha_i a_i) p_i ; p_i = zeta_new_i r + b_i p_i.  The x_i are never
-// stored: 96 B per site and active shift instead of 192 (the sum is taken in list order, per element).
-template <typename T>
-__global__ void __launch_bounds__(CG_BLOCK) cg_update_yp_kernel(const V2<T>* __restrict__ r, const CgState* st, size_t n) {
-    if (st->stop4) return;
+template <typename T, int MM>
+__global__ void __launch_bounds__(CG_BLOCK) cg_flush_kernel(CgState* st, size_t n) {
+    const int nres = st->blk_j;
+    if (nres == 0) return;                       // nothing accumulated (solve already over); same in every block
+    __shared__ V2<T>* sx[LQCD_MAX_SHIFTS];
     __shared__ V2<T>* sp[LQCD_MAX_SHIFTS];
-    __shared__ T sa[LQCD_MAX_SHIFTS], sz[LQCD_MAX_SHIFTS], sb[LQCD_MAX_SHIFTS];
-    const int nl = st->nlist;
-    for (int e = threadIdx.x; e < nl; e += CG_BLOCK) {
-        sp[e] = (V2<T>*)st->p[st->list_idx[e]];
-        sa[e] = (T)st->list_a[e];
-        sz[e] = (T)st->list_zn[e];
-        sb[e] = (T)st->list_b[e];
+    __shared__ const V2<T>* sr[MM];
+    __shared__ T sCP[LQCD_MAX_SHIFTS], sB[LQCD_MAX_SHIFTS], sY[MM];
+    __shared__ V2<T> sDE[LQCD_MAX_SHIFTS * MM];
+    __shared__ int cnt[2];
+    const int tid = threadIdx.x;
+    const int rational = st->rational;
+    // compact list of the shifts of this block (two warps, one thread per shift)
+    int inb = 0;
+    unsigned int bal = 0;
+    if (tid < LQCD_MAX_SHIFTS) {
+        inb = (tid < st->nshift) ? st->in_block[tid] : 0;
+        bal = __ballot_sync(0xffffffffu, inb);
+        if ((tid & 31) == 0) cnt[tid >> 5] = __popc(bal);
+    }
+    if (tid >= LQCD_MAX_SHIFTS && tid < LQCD_MAX_SHIFTS + MM) {
+        const int l = tid - LQCD_MAX_SHIFTS;
+        sr[l] = (const V2<T>*)st->hist[l < nres ? l : 0];
+    }
+    __syncthreads();
+    const int nl = cnt[0] + cnt[1];
+    if (inb) {
+        const int e = __popc(bal & ((1u << (tid & 31)) - 1u)) + ((tid >= 32) ? cnt[0] : 0);
+        sx[e] = (V2<T>*)st->x[tid];
+        sp[e] = (V2<T>*)st->p[tid];
+        sCP[e] = (T)st->blk_CP[tid];
+        sB[e] = (T)st->blk_B[tid];
+#pragma unroll
+        for (int l = 0; l < MM; ++l)
+            sDE[e * MM + l] = (l < nres) ? make_v2((T)st->blk_D[l * LQCD_MAX_SHIFTS + tid], (T)st->blk_E[l * LQCD_MAX_SHIFTS + tid])
+                                         : make_v2((T)0, (T)0);
+    }
+    __syncthreads();
+    if (rational && tid < MM) {                  // y += sum_l (sum_i D_il) r_l
+        T acc = (T)0;
+        for (int e = 0; e < nl; ++e) acc += sDE[e * MM + tid].x;
+        sY[tid] = acc;
     }
     __syncthreads();
     V2<T>* __restrict__ y = (V2<T>*)st->y;
-    const size_t stride = (size_t)gridDim.x * CG_BLOCK;
-    for (size_t j = (size_t)blockIdx.x * CG_BLOCK + threadIdx.x; j < n; j += stride) {
-        const V2<T> rv = r[j];
-        V2<T> yv = y[j];
-        int e = 0;
-        for (; e + 4 <= nl; e += 4) {
-            V2<T> pv[4];
-#pragma unroll
-            for (int u = 0; u < 4; ++u) pv[u] = sp[e + u][j];
-#pragma unroll
-            for (int u = 0; u < 4; ++u) {
-                const T a = sa[e + u], zn = sz[e + u], bi = sb[e + u];
-                yv.x = fma(a, pv[u].x, yv.x);
-                yv.y = fma(a, pv[u].y, yv.y);
-                pv[u].x = fma(zn, rv.x, bi * pv[u].x);
-                pv[u].y = fma(zn, rv.y, bi * pv[u].y);
-                sp[e + u][j] = pv[u];
-            }
+    if (nl > 0) {
+        if (rational) {
+            if (nres == MM) cg_flush_body<T, MM, true, true>(nres, nl, sx, sp, sr, sCP, sB, sDE, sY, y, n);
+            else cg_flush_body<T, MM, true, false>(nres, nl, sx, sp, sr, sCP, sB, sDE, sY, y, n);
+        } else {
+            if (nres == MM) cg_flush_body<T, MM, false, true>(nres, nl, sx, sp, sr, sCP, sB, sDE, sY, y, n);
+            else cg_flush_body<T, MM, false, false>(nres, nl, sx, sp, sr, sCP, sB, sDE, sY, y, n);
         }
-        for (; e < nl; ++e) {
-            V2<T> pv = sp[e][j];
-            const T a = sa[e], zn = sz[e], bi = sb[e];
-            yv.x = fma(a, pv.x, yv.x);
-            yv.y = fma(a, pv.y, yv.y);
-            pv.x = fma(zn, rv.x, bi * pv.x);
-            pv.y = fma(zn, rv.y, bi * pv.y);
-            sp[e][j] = pv;
+    }
+    // the last block to finish closes the block of iterations; every block has read the state by then
+    __syncthreads();
+    if (tid == 0) {
+        __threadfence();
+        const unsigned int t = atomicAdd(&st->ticket[3], 1u);
+        if (t == gridDim.x - 1) {
+            st->ticket[3] = 0;
+            st->blk_j = 0;
         }
-        y[j] = yv;
     }
 }
 

@@ -37,6 +37,7 @@
 #ifndef DS_MINB_F32
 #define DS_MINB_F32 6
 #endif
+static_assert(DS_BLOCK >= LQCD_MAX_SHIFTS, "the scalar step of the epilogue needs one thread per shift");
 #ifndef EPI_PLOAD
 #define EPI_PLOAD 1      // 0: load p in the epilogue, 1: load p into registers up front, 2: L2 prefetch up front
 #endif
@@ -324,11 +325,9 @@ __global__ void __launch_bounds__(DS_BLOCK, DsOcc<T>::minb) dslash_kernel(const 
         __shared__ int last_flag;
         const double bsum = block_sum<DS_BLOCK>(dot, red);
         if (publish_partial<DS_BLOCK>(bsum, A.partials, &A.st->ticket[1], &last_flag)) {
-            const double pAp = final_sum<DS_BLOCK>(A.partials, gridDim.x, red);
-            if (threadIdx.x == 0) {
-                A.st->ticket[1] = 0;
-                cg_scalars_after_pAp(A.st, pAp);
-            }
+            const double pAp = broadcast0(final_sum<DS_BLOCK>(A.partials, gridDim.x, red), red);
+            if (threadIdx.x == 0) A.st->ticket[1] = 0;
+            cg_scalars_after_pAp(A.st, pAp);
         }
     }
 }

@@ -35,11 +35,13 @@ struct PrecBufs {
     int recon_stored = 0;    // 0 = no gauge in this precision, else 18 or 12
     T* Th = nullptr;         // stored U(1) angles theta_mu(x) (lqcd_set_u1_phases), [(mu*2+par)*Vh + k]
     int u1_stored = 0;
-    V2<T> *r = nullptr, *p = nullptr, *s = nullptr, *t = nullptr;
+    V2<T> *p = nullptr, *s = nullptr, *t = nullptr;
+    V2<T>* hist[LQCD_MAX_BLOCK] = {};        // ring of residual vectors (cg.cuh)
+    int n_hist = 0;
     V2<T>* pextra[LQCD_MAX_SHIFTS] = {};
     int n_pextra = 0;
     cudaGraphExec_t graph_exec = nullptr;    // CUDA graph of `graph_iters` CG iterations
-    int graph_iters = 0, graph_rational = 0;
+    int graph_iters = 0, graph_rational = 0, graph_block = 0;
     V2<T>* stage_b = nullptr;                // host-call staging (device copies of host arguments)
     V2<T>* stage_x[LQCD_MAX_SHIFTS] = {};
     int n_stage_x = 0;
@@ -54,7 +56,7 @@ struct lqcd_ctx {
 
     // options
     double mass;
-    int recon_opt, max_iter, check_every, use_graph;
+    int recon_opt, max_iter, check_every, use_graph, shift_block;
 
     // memory
     char* arena;             // caller workspace (not owned) or NULL
@@ -201,7 +203,10 @@ int ensure_solver(lqcd_ctx* c, int nshift) {
     int rc;
     if ((rc = ensure_tmp<T>(c))) return rc;
     PrecBufs<T>& B = bufs<T>(c);
-    if (!B.r && (rc = dev_alloc(c, (void**)&B.r, vec_bytes<T>(c)))) return rc;
+    while (B.n_hist < c->shift_block) {
+        if ((rc = dev_alloc(c, (void**)&B.hist[B.n_hist], vec_bytes<T>(c)))) return rc;
+        ++B.n_hist;
+    }
     if (!B.p && (rc = dev_alloc(c, (void**)&B.p, vec_bytes<T>(c)))) return rc;
     if (!B.s && (rc = dev_alloc(c, (void**)&B.s, vec_bytes<T>(c)))) return rc;
     while (B.n_pextra < nshift - 1) {
@@ -246,36 +251,50 @@ void launch_dslash(lqcd_ctx* c, int epi, V2<T>* out, const V2<T>* in, int par, c
     else launch_dslash_t<T, 2>(c, a);
 }
 
-// one CG iteration = K1..K4 (cg.cuh)
+// the sweep over the shifted systems that closes a block of iterations (K5 of cg.cuh)
 template <typename T>
-void launch_cg_iteration(lqcd_ctx* c, int rational) {
+void launch_flush(lqcd_ctx* c) {
     const size_t n = c->Vh * 3;
+    const int m = c->shift_block;
+    if (m <= 4) cg_flush_kernel<T, 4><<<cg_grid(c), CG_BLOCK, 0, c->stream>>>(c->st_dev, n);
+    else if (m <= 8) cg_flush_kernel<T, 8><<<cg_grid(c), CG_BLOCK, 0, c->stream>>>(c->st_dev, n);
+    else cg_flush_kernel<T, 16><<<cg_grid(c), CG_BLOCK, 0, c->stream>>>(c->st_dev, n);
+    ++c->launches;
+}
+
+// one CG iteration = K1..K4 (cg.cuh), plus K5 when it is the last of a block; pos = iteration index mod m
+template <typename T>
+void launch_cg_iteration(lqcd_ctx* c, int pos) {
+    const size_t n = c->Vh * 3;
+    const int m = c->shift_block;
     PrecBufs<T>& B = bufs<T>(c);
     launch_dslash<T>(c, 0, B.t, B.p, 1, nullptr, 0.0, 1);
     launch_dslash<T>(c, 1, B.s, B.t, 0, B.p, 0.0, 1);
-    cg_update_r_kernel<T><<<cg_grid(c), CG_BLOCK, 0, c->stream>>>(B.r, B.s, c->st_dev, c->partials, n);
-    if (rational)
-        cg_update_yp_kernel<T><<<cg_grid(c), CG_BLOCK, 0, c->stream>>>(B.r, c->st_dev, n);
-    else
-        cg_update_xp_kernel<T><<<cg_grid(c), CG_BLOCK, 0, c->stream>>>(B.r, c->st_dev, n);
+    cg_update_r_kernel<T><<<cg_grid(c), CG_BLOCK, 0, c->stream>>>(B.hist[(pos + m - 1) % m], B.hist[pos], B.s, c->st_dev,
+                                                                  c->partials, n);
+    cg_update_base_kernel<T><<<cg_grid(c), CG_BLOCK, 0, c->stream>>>(B.hist[pos], B.p, c->st_dev, n);
     c->launches += 2;
+    if (pos == m - 1) launch_flush<T>(c);
 }
 
-int default_check_every(const lqcd_ctx* c) {
-    long v = (long)(4000000 / (long)c->Vh);
+// the host looks at the stop flag every this many iterations: a whole number of blocks
+int check_every(const lqcd_ctx* c) {
+    long v = c->check_every ? (long)c->check_every : (long)(4000000 / (long)c->Vh);
     if (v < 1) v = 1;
-    if (v > 64) v = 64;
-    return (int)v;
+    if (!c->check_every && v > 64) v = 64;
+    const long m = c->shift_block;
+    return (int)((v + m - 1) / m * m);
 }
 
 template <typename T>
 int build_graph(lqcd_ctx* c, int iters, int rational) {
+    (void)rational;                  // the kernels read the mode from the device state
     drop_graph<T>(c);
     PrecBufs<T>& B = bufs<T>(c);
     cudaGraph_t graph = nullptr;
     const long long before = c->launches;
     CU(cudaStreamBeginCapture(c->stream, cudaStreamCaptureModeThreadLocal));
-    for (int i = 0; i < iters; ++i) launch_cg_iteration<T>(c, rational);
+    for (int i = 0; i < iters; ++i) launch_cg_iteration<T>(c, i % c->shift_block);
     cudaError_t e = cudaStreamEndCapture(c->stream, &graph);
     c->launches = before;     // capturing is not launching
     if (e != cudaSuccess) return fail(c, LQCD_ECUDA, "graph capture failed: %s", cudaGetErrorString(e));
@@ -287,6 +306,7 @@ int build_graph(lqcd_ctx* c, int iters, int rational) {
     }
     B.graph_iters = iters;
     B.graph_rational = rational;
+    B.graph_block = c->shift_block;
     return LQCD_OK;
 }
 
@@ -428,6 +448,7 @@ lqcd_ctx* lqcd_create(int Lx, int Ly, int Lz, int Lt) {
     c->max_iter = 100000;
     c->check_every = 0;
     c->use_graph = 1;
+    c->shift_block = 8;
     c->err[0] = 0;
     return c;
 }
@@ -486,6 +507,11 @@ int lqcd_set_option(lqcd_ctx* c, int key, double v) {
             if (v != 0.0 && v != 1.0) return fail(c, LQCD_EINVAL, "USE_GRAPH must be 0 or 1");
             c->use_graph = (int)v;
             break;
+        case LQCD_OPT_SHIFT_BLOCK:
+            if (!(v >= 1.0) || v > (double)LQCD_MAX_BLOCK || v != std::floor(v))
+                return fail(c, LQCD_EINVAL, "SHIFT_BLOCK must be an integer in [1, %d]", LQCD_MAX_BLOCK);
+            c->shift_block = (int)v;
+            break;
         case LQCD_OPT_LINK_PRECISIONS:
             if (v != 1.0 && v != 2.0 && v != 3.0)
                 return fail(c, LQCD_EINVAL, "LINK_PRECISIONS must be LQCD_PREC_F64 (1), LQCD_PREC_F32 (2) or both (3)");
@@ -504,7 +530,8 @@ int lqcd_get_option(const lqcd_ctx* c, int key, double* v) {
         case LQCD_OPT_ANTIPERIODIC_T: *v = c->g.antiperiodic; break;
         case LQCD_OPT_RECON: *v = c->recon_opt; break;
         case LQCD_OPT_MAX_ITER: *v = c->max_iter; break;
-        case LQCD_OPT_CHECK_EVERY: *v = c->check_every ? c->check_every : default_check_every(c); break;
+        case LQCD_OPT_CHECK_EVERY: *v = check_every(c); break;
+        case LQCD_OPT_SHIFT_BLOCK: *v = c->shift_block; break;
         case LQCD_OPT_USE_GRAPH: *v = c->use_graph; break;
         case LQCD_OPT_LINK_PRECISIONS: *v = c->prec_opt; break;
         default: return LQCD_EINVAL;
@@ -516,9 +543,9 @@ size_t lqcd_workspace_bytes(const lqcd_ctx* c, int nshift) {
     if (!c || nshift < 1 || nshift > LQCD_MAX_SHIFTS) return 0;
     size_t b = 0;
     if (c->prec_opt & LQCD_PREC_F64)
-        b += align_up(links_bytes<double>(c, 18)) + align_up(vec_bytes<double>(c)) * (size_t)(4 + (nshift - 1));
+        b += align_up(links_bytes<double>(c, 18)) + align_up(vec_bytes<double>(c)) * (size_t)(3 + c->shift_block + (nshift - 1));
     if (c->prec_opt & LQCD_PREC_F32)
-        b += align_up(links_bytes<float>(c, 18)) + align_up(vec_bytes<float>(c)) * (size_t)(4 + (nshift - 1));
+        b += align_up(links_bytes<float>(c, 18)) + align_up(vec_bytes<float>(c)) * (size_t)(3 + c->shift_block + (nshift - 1));
     if (c->prec_opt & LQCD_PREC_F64) b += align_up((size_t)8 * c->Vh * sizeof(double));   // U(1) angles, if set
     if (c->prec_opt & LQCD_PREC_F32) b += align_up((size_t)8 * c->Vh * sizeof(float));
     b += align_up(sizeof(CgState)) + align_up(sizeof(double));
@@ -705,20 +732,23 @@ int solve(lqcd_ctx* c, const T* b_even, const double* shifts, int nshift, double
         h->alpha[i] = rational ? alpha[i] : 0.0;
         h->p[i] = (i == i0) ? (void*)B.p : (void*)B.pextra[extra++];
     }
+    const int m = c->shift_block;
+    h->blk_m = m;
+    for (int l = 0; l < m; ++l) h->hist[l] = (void*)B.hist[l];
     h->rational = rational;
     h->alpha0 = alpha0;
     h->y = (void*)y;
     const size_t n = c->Vh * 3;
     CU(cudaMemcpyAsync(c->st_dev, h, sizeof(CgState), cudaMemcpyHostToDevice, c->stream));
     CU(cudaEventRecord(c->ev_t0, c->stream));
-    cg_init_kernel<T><<<cg_grid(c), CG_BLOCK, 0, c->stream>>>((const V2<T>*)b_even, B.r, c->st_dev, c->partials, n, tol);
+    cg_init_kernel<T><<<cg_grid(c), CG_BLOCK, 0, c->stream>>>((const V2<T>*)b_even, B.hist[m - 1], c->st_dev, c->partials, n, tol);
     ++c->launches;
     CU(cudaGetLastError());
 
-    const int ce = c->check_every ? c->check_every : default_check_every(c);
+    const int ce = check_every(c);
     // the legacy default stream cannot be captured: plain launches there
     const bool use_graph = c->use_graph && c->stream != nullptr && c->stream != cudaStreamLegacy;
-    if (use_graph && (B.graph_iters != ce || B.graph_rational != rational)) {
+    if (use_graph && (B.graph_iters != ce || B.graph_block != m)) {
         if ((rc = build_graph<T>(c, ce, rational))) return rc;
     }
     c->flag_host[0] = c->flag_host[1] = 0;
@@ -727,9 +757,9 @@ int solve(lqcd_ctx* c, const T* b_even, const double* shifts, int nshift, double
     for (long batch = 0; batch < max_batches && !done; ++batch) {
         if (use_graph) {
             CU(cudaGraphLaunch(B.graph_exec, c->stream));
-            c->launches += 4LL * ce;
+            c->launches += 4LL * ce + ce / m;
         } else {
-            for (int i = 0; i < ce; ++i) launch_cg_iteration<T>(c, rational);
+            for (int i = 0; i < ce; ++i) launch_cg_iteration<T>(c, i % m);
             CU(cudaGetLastError());
         }
         const int slot = (int)(batch & 1);

@@ -29,22 +29,35 @@ struct Geom {
     int antiperiodic;               // bc_t = -1 on links leaving t = Lt-1
 };
 
+#define LQCD_MAX_BLOCK 16           // longest block of iterations whose shift updates are applied in one sweep
+
 // Device-resident state of one multi-shift CG solve (steps A6, A9): every scalar of the recurrence
 // lives here, so an iteration needs no host round trip.
+//
+// Block-deferred shift updates.  Within a block of m iterations that starts at
+// iteration n0 with P = p_i, X = x_i, the recurrences  x_i += a_i p_i ;  p_i = zeta_i r + b_i p_i  unroll to
+//     p_i^(n0+j) = B_j P + sum_{l=1..j} E_{j,l} r^(n0+l)
+//     x_i^(n0+j) = X + CP_j P + sum_{l=1..j-1} D_{j,l} r^(n0+l)
+// so the shifted x_i, p_i need not be touched until the block ends if the m residuals of the block are kept
+// (m x 48 B per site, shared by all shifts) and the scalar coefficients B, E, CP, D are carried along.
+// The base system's p is needed by the operator every iteration and is updated every iteration.
 struct CgState {
     double rr, bb, pAp, a, a_prev, b_prev, tol2bb, c0;
-    int iter, max_iter, stop, stop4, status, nshift, i0, nlist;
-    unsigned int ticket[4];
+    int iter, max_iter, stop, stop4, status, nshift, i0, blk_m;
+    int blk_j;                      // iterations accumulated in the current block (0..blk_m)
+    unsigned int ticket[5];
     double delta[LQCD_MAX_SHIFTS];
     double zeta[LQCD_MAX_SHIFTS], zeta_prev[LQCD_MAX_SHIFTS], zeta_new[LQCD_MAX_SHIFTS];
     int active[LQCD_MAX_SHIFTS], freeze_iter[LQCD_MAX_SHIFTS];
-    // update list of the current iteration (shifts that were active when it started)
-    int list_idx[LQCD_MAX_SHIFTS];
-    double list_a[LQCD_MAX_SHIFTS], list_zn[LQCD_MAX_SHIFTS], list_b[LQCD_MAX_SHIFTS];
+    // block coefficients, per shift i (index [l*LQCD_MAX_SHIFTS + i] so that a warp's accesses coalesce)
+    int in_block[LQCD_MAX_SHIFTS];  // shift takes part in the current block (was active at its start, not the base)
+    double blk_B[LQCD_MAX_SHIFTS], blk_CP[LQCD_MAX_SHIFTS];
+    double blk_E[LQCD_MAX_BLOCK * LQCD_MAX_SHIFTS], blk_D[LQCD_MAX_BLOCK * LQCD_MAX_SHIFTS];
     void* x[LQCD_MAX_SHIFTS];       // V2<T>* of the precision the solve runs in
     void* p[LQCD_MAX_SHIFTS];
+    void* hist[LQCD_MAX_BLOCK];     // residual ring: r^(n0+l) is in hist[l-1], l = 1..m; r^(n0) in hist[m-1]
     // rational-sum mode (lqcd_rational_apply): y = alpha0 b + sum_i alpha_i x_i is accumulated during the
-    // solve and the x_i are never stored; list_a then holds alpha_i * a_i
+    // solve and the x_i are never stored; blk_CP, blk_D then carry the factor alpha_i
     int rational;
     double alpha0;
     double alpha[LQCD_MAX_SHIFTS];

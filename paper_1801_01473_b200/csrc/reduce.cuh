@@ -72,9 +72,21 @@ __device__ __forceinline__ double final_sum(const double* partials, int n, doubl
     return block_sum<BLOCK>(a[0], red);
 }
 
-// ---- scalar recurrences (SURVEY.md §8(c2) / DESIGN.md R5), run by thread 0 of the last block ------
+// value of thread 0 -> every thread of the block (red is the scratch of the block_sum that produced it)
+__device__ __forceinline__ double broadcast0(double v, double* red) {
+    __syncthreads();
+    if (threadIdx.x == 0) red[0] = v;
+    __syncthreads();
+    return red[0];
+}
 
-// after |b|^2 is known (solve start)
+// ---- scalar recurrences (SURVEY.md §8(c2) / DESIGN.md R5) ------------------------------------------
+// Run by the block that finished last, ALL its threads calling (blockDim.x >= LQCD_MAX_SHIFTS): thread i
+// carries shift i, thread 0 also the scalars of the base system, so the tail of the kernel costs one chain
+// of dependent operations instead of nshift of them.  Besides the zeta recurrences the threads carry the
+// block coefficients B, E, CP, D of the deferred shift updates (lqcd_internal.cuh, CgState).
+
+// after |b|^2 is known (solve start); thread 0 only
 __device__ inline void cg_scalars_init(CgState* st, double bb, double tol) {
     st->rr = bb;
     st->bb = bb;
@@ -83,7 +95,7 @@ __device__ inline void cg_scalars_init(CgState* st, double bb, double tol) {
     st->b_prev = 0.0;
     st->iter = 0;
     st->status = 0;
-    st->nlist = 0;
+    st->blk_j = 0;
     const int stop = (bb == 0.0) ? 1 : 0;       // zero source: x_i = 0 is the answer
     st->stop = stop;
     st->stop4 = stop;
@@ -92,64 +104,115 @@ __device__ inline void cg_scalars_init(CgState* st, double bb, double tol) {
         st->zeta_prev[i] = 1.0;
         st->zeta_new[i] = 1.0;
         st->active[i] = 1;
+        st->in_block[i] = 0;
         st->freeze_iter[i] = 0;
     }
 }
 
-// after pAp = Re<p, B p> is known: step length and the shifted coefficients
-__device__ inline void cg_scalars_after_pAp(CgState* st, double pAp) {
-    st->pAp = pAp;
+// after pAp = Re<p, B p> is known: step length, zeta_new_i, and the x-part of the block coefficients
+//   x_i += a_i p_i  with  p_i = B P + sum_l E_l r_l   =>   CP += a_i B ;  D_l += a_i E_l  (l < j)
+__device__ __noinline__ void cg_scalars_after_pAp(CgState* st, double pAp) {
+    const int tid = threadIdx.x;
+    const double rr = st->rr, a_prev = st->a_prev, b_prev = st->b_prev;
+    const int j = st->blk_j, ns = st->nshift, i0 = st->i0, rational = st->rational;
     if (!(pAp > 0.0) || !isfinite(pAp)) {
-        st->status = -6;                         // LQCD_EBREAKDOWN
-        st->stop = 1;
-        st->stop4 = 1;
-        st->nlist = 0;
+        if (tid == 0) {
+            st->pAp = pAp;
+            st->status = -6;                     // LQCD_EBREAKDOWN
+            st->stop = 1;
+            st->stop4 = 1;
+        }
         return;
     }
-    const double a = st->rr / pAp;
-    st->a = a;
-    const double a_prev = st->a_prev, b_prev = st->b_prev;
-    int n = 0;
-    for (int i = 0; i < st->nshift; ++i) {
-        if (!st->active[i]) continue;
-        const double z = st->zeta[i], zp = st->zeta_prev[i];
-        const double zn = z * zp * a_prev / (a_prev * zp * (1.0 + st->delta[i] * a) + a * b_prev * (zp - z));
-        st->zeta_new[i] = zn;
-        st->list_idx[n] = i;
-        st->list_a[n] = st->rational ? st->alpha[i] * (a * zn / z) : a * zn / z;
-        st->list_zn[n] = zn;
-        ++n;
-    }
-    st->nlist = n;
-}
-
-// after |r_new|^2 is known: direction coefficients, shift of the recurrence, freezing, stopping rule
-__device__ inline void cg_scalars_after_rr(CgState* st, double rr_new) {
-    const double bt = rr_new / st->rr;
-    for (int e = 0; e < st->nlist; ++e) {
-        const int i = st->list_idx[e];
-        const double ratio = st->zeta_new[i] / st->zeta[i];
-        st->list_b[e] = bt * ratio * ratio;
-        st->zeta_prev[i] = st->zeta[i];
-        st->zeta[i] = st->zeta_new[i];
-    }
-    st->a_prev = st->a;
-    st->b_prev = bt;
-    st->rr = rr_new;
-    const int it = st->iter + 1;
-    st->iter = it;
-    for (int i = 0; i < st->nshift; ++i) {
-        if (!st->active[i]) continue;
-        if (st->zeta[i] * st->zeta[i] * rr_new <= st->tol2bb) {
-            st->active[i] = 0;
-            st->freeze_iter[i] = it;
+    const double a = rr / pAp;
+    if (tid < ns) {
+        const int i = tid;
+        const int act = st->active[i];
+        const int inb = (j == 0) ? (act && i != i0) : st->in_block[i];
+        if (j == 0) st->in_block[i] = inb;
+        if (act) {
+            const double z = st->zeta[i], zp = st->zeta_prev[i];
+            const double zn = z * zp * a_prev / (a_prev * zp * (1.0 + st->delta[i] * a) + a * b_prev * (zp - z));
+            st->zeta_new[i] = zn;
+            if (inb) {
+                double ai = a * zn / z;
+                if (rational) ai *= st->alpha[i];
+                if (j == 0) {
+                    st->blk_B[i] = 1.0;
+                    st->blk_CP[i] = ai;
+                } else {
+                    st->blk_CP[i] = fma(ai, st->blk_B[i], st->blk_CP[i]);
+                    double e[LQCD_MAX_BLOCK], d[LQCD_MAX_BLOCK];
+#pragma unroll
+                    for (int l = 0; l < LQCD_MAX_BLOCK; ++l)
+                        if (l < j) {
+                            e[l] = st->blk_E[l * LQCD_MAX_SHIFTS + i];
+                            d[l] = st->blk_D[l * LQCD_MAX_SHIFTS + i];
+                        }
+#pragma unroll
+                    for (int l = 0; l < LQCD_MAX_BLOCK; ++l)
+                        if (l < j) st->blk_D[l * LQCD_MAX_SHIFTS + i] = fma(ai, e[l], d[l]);
+                }
+            }
         }
     }
-    if (rr_new <= st->tol2bb) {
-        st->stop = 1;
-    } else if (it >= st->max_iter) {
-        st->stop = 1;
-        st->status = -5;                         // LQCD_ENOCONV
+    if (tid == 0) {
+        st->pAp = pAp;
+        st->a = a;
+    }
+}
+
+// after |r_new|^2 is known: beta, b_i, the p-part of the block coefficients
+//   p_i = zeta_new_i r_new + b_i p_i   =>   B *= b_i ;  E_l *= b_i (l < j) ;  E_j = zeta_new_i ;  D_j = 0
+// then the shift of the recurrence, freezing and the stopping rule
+__device__ __noinline__ void cg_scalars_after_rr(CgState* st, double rr_new) {
+    const int tid = threadIdx.x;
+    const double rr_old = st->rr, a = st->a, tol2bb = st->tol2bb;
+    const int j = st->blk_j, ns = st->nshift, it = st->iter + 1, max_iter = st->max_iter;
+    const double bt = rr_new / rr_old;
+    if (tid < ns) {
+        const int i = tid;
+        const int act = st->active[i], inb = st->in_block[i];
+        if (act) {
+            const double z = st->zeta[i], zn = st->zeta_new[i];
+            const double ratio = zn / z;
+            const double bi = bt * ratio * ratio;
+            if (inb) {
+                st->blk_B[i] = (j == 0 ? 1.0 : st->blk_B[i]) * bi;
+                double e[LQCD_MAX_BLOCK];
+#pragma unroll
+                for (int l = 0; l < LQCD_MAX_BLOCK; ++l)
+                    if (l < j) e[l] = st->blk_E[l * LQCD_MAX_SHIFTS + i];
+#pragma unroll
+                for (int l = 0; l < LQCD_MAX_BLOCK; ++l)
+                    if (l < j) st->blk_E[l * LQCD_MAX_SHIFTS + i] = e[l] * bi;
+                st->blk_E[j * LQCD_MAX_SHIFTS + i] = zn;
+                st->blk_D[j * LQCD_MAX_SHIFTS + i] = 0.0;
+            }
+            st->zeta_prev[i] = z;
+            st->zeta[i] = zn;
+            if (zn * zn * rr_new <= tol2bb) {
+                st->active[i] = 0;
+                st->freeze_iter[i] = it;
+            }
+        } else if (inb) {                        // frozen earlier in this block: its x_i no longer moves
+            st->blk_E[j * LQCD_MAX_SHIFTS + i] = 0.0;
+            st->blk_D[j * LQCD_MAX_SHIFTS + i] = 0.0;
+        }
+    }
+    __syncthreads();                             // every thread has read the old scalars
+    if (tid == 0) {
+        st->a_prev = a;
+        st->b_prev = bt;
+        st->rr = rr_new;
+        st->iter = it;
+        st->blk_j = j + 1;
+        if (rr_new <= tol2bb) {
+            st->stop = 1;
+        } else if (it >= max_iter) {
+            st->stop = 1;
+            st->status = -5;                     // LQCD_ENOCONV
+        }
     }
 }
 
