@@ -52,8 +52,24 @@ NCU_DRAM_BYTES_PER_LAUNCH = {
 
 
 def cg_bytes_per_site(n_active: int, recon: int) -> int:
-    """One CG iteration per even site: two Dslash + p in the epilogue + r update + shift updates."""
+    """SURVEY.md §8(d) model of one CG iteration per even site, shift updates applied every iteration:
+    two Dslash + p in the epilogue + r update + base x/p + 192 B per further active shift."""
     return 2 * DSLASH_BYTES[recon] + 48 + 144 + 240 + 192 * (n_active - 1)
+
+
+def cg_bytes_moved(freeze_iter, iters: int, m: int, recon: int) -> int:
+    """Bytes per even site the library actually moves in `iters` iterations with block-deferred shift updates
+    (DESIGN.md "CG iteration"): per iteration two Dslash + p (48) + r update (144) + base x/p (240); per block of
+    m iterations one sweep reading the block's residuals (48 each) and updating x_i, p_i (192) of every shifted
+    system that was active when the block began."""
+    base = max(range(len(freeze_iter)), key=lambda i: freeze_iter[i])
+    total = iters * (2 * DSLASH_BYTES[recon] + 48 + 144 + 240)
+    for n0 in range(0, iters, m):
+        nres = min(m, iters - n0)
+        n_in = sum(1 for i, fz in enumerate(freeze_iter) if i != base and fz > n0)
+        if n_in:
+            total += 48 * nres + 192 * n_in
+    return total
 
 
 def load_peaks():
@@ -259,9 +275,12 @@ def run_ours(args, world, rank, local):
         launches = lat.launches - n0
         sched = n_active_schedule(info["freeze_iter"], K)
         bytes_total = sum(cg_bytes_per_site(n, recon) for n in sched) * lat.Vh
+        m_blk = int(lat.get_option(lq.LQCD_OPT_SHIFT_BLOCK))
+        bytes_moved = cg_bytes_moved(info["freeze_iter"], K, m_blk, recon) * lat.Vh
         out["timed"] = dict(ms_total=ms_total, launches=launches, launches_all=int(sum_over_ranks(world, launches)),
-                            n_active_mean=sum(sched) / K,
-                            gbs_algorithmic=bytes_total / (ms_total * 1e6), kernel_ms=info["solve_ms"])
+                            n_active_mean=sum(sched) / K, shift_block=m_blk,
+                            gbs_algorithmic=bytes_total / (ms_total * 1e6),
+                            gbs_moved=bytes_moved / (ms_total * 1e6), kernel_ms=info["solve_ms"])
 
         # ---- e2e: same K iterations through the host-pointer entry point (rank-local, then max)
         b_host = torch.empty(b.shape, dtype=torch.float64, pin_memory=True)
@@ -290,10 +309,12 @@ def run_ours(args, world, rank, local):
             _, full = lat.mshift_cg(b, shifts, tol, x=x, raise_on_noconv=False)
             sched_f = n_active_schedule(full["freeze_iter"], full["iters"])
             bytes_f = sum(cg_bytes_per_site(n, recon) for n in sched_f) * lat.Vh
+            moved_f = cg_bytes_moved(full["freeze_iter"], full["iters"], m_blk, recon) * lat.Vh
             out["full_solve"] = dict(iters=full["iters"], status=full["status"], rel_res=full["rel_res"],
                                      s_per_iter=full["solve_ms"] * 1e-3 / max(full["iters"], 1),
                                      solve_s=full["solve_ms"] * 1e-3, n_active_mean=sum(sched_f) / max(len(sched_f), 1),
                                      gbs_algorithmic=bytes_f / (full["solve_ms"] * 1e6),
+                                     gbs_moved=moved_f / (full["solve_ms"] * 1e6),
                                      freeze_iter=full["freeze_iter"])
         lat.close()
         del x
@@ -377,7 +398,8 @@ def main():
     config = {"workload": f"{args.workload}: {lname} lattice, multi-shift CG with {len(cfg['shifts'])} shifts "
                           f"(geometric {cfg['shifts'][0]:g}..{cfg['shifts'][-1]:g}), m={cfg['mass']}, tol={cfg['tol']:g}, "
                           f"{args.recon}-real links, seeded random SU(3) links + Gaussian even-site source",
-              "step": "one multi-shift CG iteration (D_oe, D_eo+epilogue, scalar recurrences, r update, x_i/p_i updates)",
+              "step": "one multi-shift CG iteration (D_oe, D_eo+epilogue, scalar recurrences, r update, base x/p update, "
+                      "1/m of the block sweep over the shifted x_i/p_i)",
               "lattice": list(cfg["L"]), "nshift": len(cfg["shifts"]), "mass": cfg["mass"], "tol": cfg["tol"],
               "recon": args.recon, "parallelism": "replicas only" if world > 1 else "single GPU",
               "l2": "inputs larger than L2 (links 3.06 GB vs 126 MB); no flush needed"}
@@ -425,8 +447,11 @@ def main():
                      "note": "achieved = algorithmic bytes (8 links + 8 neighbour vectors + 1 output per site) / event "
                              "time; the 8 neighbour-vector reads are mostly L2 hits, achieved_dram_model counts each "
                              "input vector once (what DRAM must deliver)"},
-        "cg": {"n_active_mean": res["timed"]["n_active_mean"], "gbs_algorithmic": res["timed"]["gbs_algorithmic"],
-               "frac_of_peak": res["timed"]["gbs_algorithmic"] / peak},
+        "cg": {"n_active_mean": res["timed"]["n_active_mean"], "shift_block": res["timed"]["shift_block"],
+               "gbs_algorithmic": res["timed"]["gbs_algorithmic"], "gbs_moved": res["timed"]["gbs_moved"],
+               "frac_of_peak_moved": res["timed"]["gbs_moved"] / peak,
+               "note": "gbs_algorithmic: bytes of the per-iteration method (SURVEY.md 8(d): 3600+192(n_act-1) B/site) / time, "
+                       "an equivalent rate; gbs_moved: bytes the block-deferred updates actually move / time"},
         "dslash": res["dslash"],
     }
     if "full_solve" in res:
