@@ -67,6 +67,7 @@ typedef struct lqcd_ctx lqcd_ctx;
 #define LQCD_ENOCONV     -5   /* MAX_ITER reached; x[] holds the last iterate */
 #define LQCD_EBREAKDOWN  -6   /* <p,Ap> <= 0 or non-finite (cannot happen for SU(3) links) */
 #define LQCD_ENOTSU3     -7   /* RECON=12 and some link has max|r2 - conj(r0 x r1)| > 1e-12 */
+#define LQCD_ECOMM       -8   /* slab context: no transport set, or the transport failed */
 
 /* option keys for lqcd_set_option / lqcd_get_option */
 #define LQCD_OPT_MASS            0  /* m of Eq. 2; default 0                               */
@@ -189,6 +190,62 @@ int lqcd_rational_apply_host(lqcd_ctx* ctx, const double* b_even /*HOST*/, doubl
 
 int lqcd_rational_apply_f32(lqcd_ctx* ctx, const float* b_even, double alpha0, const double* alpha /*HOST*/,
                             const double* shifts /*HOST*/, int nshift, double tol, float* y_even);
+
+/* ---- 1-D slab decomposition over several GPUs (Alg. 1) --------------------------
+ * The paper cuts the lattice along one direction, one MPI rank (one GPU) per slab: each application of D_oe / D_eo
+ * then needs the faces of the input vector from the two neighbouring ranks ("a pseudofermion border ... 48 bytes
+ * per even site"), and each scalar product of the CG a global reduction.  The
+ * operator is applied to the interior of the slab while the faces travel and to the two border slices afterwards
+ * (Alg. 1).
+ *
+ * Here: one process per GPU, the cut is along t (the slowest index, so a face is contiguous per colour), rank r of
+ * nranks owns the time slices [r*Lt/nranks, (r+1)*Lt/nranks).  Lt/nranks must be even (then local and global site
+ * parities agree).  A slab context is used through the SAME calls as a whole-lattice one, on the rank's local
+ * data: lqcd_set_gauge takes the links that leave the slab's sites (canonical layout of the local
+ * Lx*Ly*Lz*(Lt/nranks) lattice), vectors are parity vectors of the local lattice, lqcd_mshift_cg solves the global
+ * system (its statistics are identical on every rank).  Every rank must make the same sequence of calls with the
+ * same options, shifts and tol.  The antiperiodic boundary sits on the links that leave the last time slice of the
+ * whole lattice.  Not available on a slab context: lqcd_set_u1_phases (LQCD_EINVAL).
+ *
+ * A transport must be set before lqcd_set_gauge (which exchanges the t-links of the face once):
+ *   lqcd_comm_init_nccl   NCCL send/recv + all-reduce on the GPU (NVLink 5 / NVSwitch between the GPUs of a node),
+ *                         enqueued on streams, captured into the CUDA graph of the CG iteration;
+ *   lqcd_set_comm         caller-supplied functions, e.g. on top of MPI or torch.distributed.
+ */
+lqcd_ctx* lqcd_create_slab(int Lx, int Ly, int Lz, int Lt_global, int rank, int nranks);
+
+/* A transport = the two communication steps of the path.  All ranks call them in the same order.
+ *   exchange(user, send_lo, send_hi, recv_lo, recv_hi, bytes, stream)
+ *       ring along t: send_lo goes to rank-1, send_hi to rank+1; recv_lo receives what rank-1 sent as its
+ *       send_hi, recv_hi what rank+1 sent as its send_lo (with nranks = 1 or 2 both neighbours may be the same
+ *       rank, possibly myself).  `bytes` per buffer.
+ *   allreduce_sum(user, buf, n, stream)
+ *       buf[0..n) <- sum over ranks, in place, the same bits on every rank.
+ * host_staged = 0: the buffers are DEVICE memory; the functions enqueue on `stream` (a cudaStream_t) or complete
+ *                  before returning, and are ordered after the work already enqueued on `stream`.
+ * host_staged = 1: the buffers are pinned HOST memory whose contents are complete on entry and are consumed after
+ *                  return (the library does the copies and synchronises); `stream` is NULL.  Blocking.
+ * graph_safe  = 1: the functions only enqueue stream work that CUDA graph capture accepts.
+ * Return 0 on success; anything else makes the calling lqcd_* function return LQCD_ECOMM. */
+typedef struct lqcd_comm_ops {
+    void* user;
+    int (*exchange)(void* user, const void* send_lo, const void* send_hi, void* recv_lo, void* recv_hi, size_t bytes,
+                    void* stream);
+    int (*allreduce_sum)(void* user, double* buf, int n, void* stream);
+    int host_staged;
+    int graph_safe;
+} lqcd_comm_ops;
+int lqcd_set_comm(lqcd_ctx* ctx, const lqcd_comm_ops* ops /*HOST; copied*/);
+
+/* NCCL transport.  One rank obtains an id (128 bytes, HOST) with lqcd_nccl_unique_id and hands it to the others by
+ * any means (e.g. a torch.distributed broadcast); then every rank calls lqcd_comm_init_nccl (collective: it
+ * returns once all ranks of the slab context's nranks have joined).  LQCD_ECOMM if NCCL cannot be loaded or fails. */
+#define LQCD_NCCL_ID_BYTES 128
+int lqcd_nccl_unique_id(void* id /*HOST, 128 bytes*/);
+int lqcd_comm_init_nccl(lqcd_ctx* ctx, const void* id /*HOST, 128 bytes*/);
+
+/* rank, nranks, first global time slice and global Lt of a context (0, 1, 0, Lt for a whole-lattice one) */
+int lqcd_slab_info(const lqcd_ctx* ctx, int* rank, int* nranks, int* t_offset, int* Lt_global /*HOST, may be NULL*/);
 
 /* Statistics of the last solve; *out is HOST. idx is used by LQCD_STAT_FREEZE_ITER only. */
 int lqcd_get_stat(const lqcd_ctx* ctx, int key, int idx, double* out /*HOST*/);

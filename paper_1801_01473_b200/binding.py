@@ -9,7 +9,8 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 
 # ---- constants of include/lqcd.h ---------------------------------------------------------------------
 LQCD_OK, LQCD_EINVAL, LQCD_ENOGAUGE, LQCD_ENOMEM, LQCD_ECUDA = 0, -1, -2, -3, -4
-LQCD_ENOCONV, LQCD_EBREAKDOWN, LQCD_ENOTSU3 = -5, -6, -7
+LQCD_ENOCONV, LQCD_EBREAKDOWN, LQCD_ENOTSU3, LQCD_ECOMM = -5, -6, -7, -8
+LQCD_NCCL_ID_BYTES = 128
 LQCD_OPT_MASS, LQCD_OPT_ANTIPERIODIC_T, LQCD_OPT_RECON, LQCD_OPT_MAX_ITER = 0, 1, 2, 3
 LQCD_OPT_CHECK_EVERY, LQCD_OPT_USE_GRAPH, LQCD_OPT_LINK_PRECISIONS, LQCD_OPT_SHIFT_BLOCK = 4, 5, 6, 7
 LQCD_PREC_F64, LQCD_PREC_F32 = 1, 2
@@ -17,10 +18,21 @@ LQCD_STAT_ITERS, LQCD_STAT_REL_RES, LQCD_STAT_FREEZE_ITER, LQCD_STAT_BASE_SHIFT 
 LQCD_STAT_GPU_LAUNCHES, LQCD_STAT_SOLVE_MS = 4, 5
 
 _ERRNAMES = {0: "LQCD_OK", -1: "LQCD_EINVAL", -2: "LQCD_ENOGAUGE", -3: "LQCD_ENOMEM", -4: "LQCD_ECUDA",
-             -5: "LQCD_ENOCONV", -6: "LQCD_EBREAKDOWN", -7: "LQCD_ENOTSU3"}
+             -5: "LQCD_ENOCONV", -6: "LQCD_EBREAKDOWN", -7: "LQCD_ENOTSU3", -8: "LQCD_ECOMM"}
 
 _vp, _dp, _sz, _i, _d = ctypes.c_void_p, ctypes.c_void_p, ctypes.c_size_t, ctypes.c_int, ctypes.c_double
 _pd = ctypes.POINTER(ctypes.c_double)
+_pi = ctypes.POINTER(ctypes.c_int)
+
+# lqcd_comm_ops of include/lqcd.h
+EXCHANGE_FN = ctypes.CFUNCTYPE(_i, _vp, _vp, _vp, _vp, _vp, _sz, _vp)
+ALLREDUCE_FN = ctypes.CFUNCTYPE(_i, _vp, _pd, _i, _vp)
+
+
+class lqcd_comm_ops(ctypes.Structure):
+    _fields_ = [("user", _vp), ("exchange", EXCHANGE_FN), ("allreduce_sum", ALLREDUCE_FN),
+                ("host_staged", _i), ("graph_safe", _i)]
+
 
 # every symbol include/lqcd.h declares: name -> (restype, argtypes)
 EXPORTS = {
@@ -58,6 +70,11 @@ EXPORTS = {
     "lqcd_pack_vector_f32": (_i, [_vp, _i, _dp, _dp]),
     "lqcd_unpack_vector_f32": (_i, [_vp, _i, _dp, _dp]),
     "lqcd_last_error": (ctypes.c_char_p, [_vp]),
+    "lqcd_create_slab": (_vp, [_i, _i, _i, _i, _i, _i]),
+    "lqcd_set_comm": (_i, [_vp, ctypes.POINTER(lqcd_comm_ops)]),
+    "lqcd_nccl_unique_id": (_i, [_vp]),
+    "lqcd_comm_init_nccl": (_i, [_vp, _vp]),
+    "lqcd_slab_info": (_i, [_vp, _pi, _pi, _pi, _pi]),
 }
 
 _lib = None
@@ -255,6 +272,105 @@ def lqcd_last_error(ctx) -> str:
     return s.decode() if s else ""
 
 
+def lqcd_create_slab(Lx, Ly, Lz, Lt_global, rank, nranks):
+    return load_library().lqcd_create_slab(int(Lx), int(Ly), int(Lz), int(Lt_global), int(rank), int(nranks))
+
+
+def lqcd_set_comm(ctx, ops: "lqcd_comm_ops"):
+    return load_library().lqcd_set_comm(ctx, ctypes.byref(ops))
+
+
+def lqcd_nccl_unique_id():
+    """-> (rc, 128 bytes)"""
+    buf = ctypes.create_string_buffer(LQCD_NCCL_ID_BYTES)
+    rc = load_library().lqcd_nccl_unique_id(ctypes.cast(buf, _vp))
+    return rc, buf.raw
+
+
+def lqcd_comm_init_nccl(ctx, nccl_id: bytes):
+    assert len(nccl_id) == LQCD_NCCL_ID_BYTES
+    buf = ctypes.create_string_buffer(bytes(nccl_id), LQCD_NCCL_ID_BYTES)
+    return load_library().lqcd_comm_init_nccl(ctx, ctypes.cast(buf, _vp))
+
+
+def lqcd_slab_info(ctx):
+    """-> (rc, rank, nranks, t_offset, Lt_global)"""
+    v = [ctypes.c_int(0) for _ in range(4)]
+    rc = load_library().lqcd_slab_info(ctx, *[ctypes.byref(x) for x in v])
+    return (rc,) + tuple(x.value for x in v)
+
+
+# ---- a transport on top of torch.distributed (include/lqcd.h: lqcd_comm_ops, host_staged = 1) ----------------
+class TorchTransport:
+    """The two communication steps of the slab path (ring exchange of the faces along t, all-reduce of a scalar
+    product) carried by ``torch.distributed`` on HOST buffers -- any backend that moves CPU tensors (gloo).  The
+    library stages device data through pinned host memory around the calls, so ranks never wait on one another
+    inside a kernel and may even share a GPU (tests).  The production transport is ``lqcd_comm_init_nccl``.
+
+    Messages that travel up the ring (to rank+1) carry tag 1, those that travel down tag 2: with two ranks both
+    neighbours are the same peer and only the tag tells the two faces apart."""
+
+    def __init__(self, group=None):
+        import torch.distributed as dist
+        self.dist = dist
+        self.group = group
+        if dist.is_initialized():
+            self.rank, self.nranks = dist.get_rank(group), dist.get_world_size(group)
+        else:                       # a single process: the ring closes on itself
+            self.rank, self.nranks = 0, 1
+        self.error = None
+        self._fx = EXCHANGE_FN(self._exchange)
+        self._fa = ALLREDUCE_FN(self._allreduce)
+        self.ops = lqcd_comm_ops(None, self._fx, self._fa, 1, 0)
+        self.n_exchange = 0
+        self.n_allreduce = 0
+
+    @staticmethod
+    def _bytes(ptr, n):
+        import numpy as np
+        import torch
+        return torch.from_numpy(np.ctypeslib.as_array((ctypes.c_uint8 * n).from_address(ptr)))
+
+    def exchange(self, send_lo, send_hi, recv_lo, recv_hi):
+        """uint8 CPU tensors of equal size: send_lo -> rank-1, send_hi -> rank+1; recv_lo <- rank-1's send_hi,
+        recv_hi <- rank+1's send_lo."""
+        dist, g = self.dist, self.group
+        up, dn = (self.rank + 1) % self.nranks, (self.rank - 1) % self.nranks
+        self.n_exchange += 1
+        if self.nranks == 1:
+            recv_lo.copy_(send_hi)
+            recv_hi.copy_(send_lo)
+            return
+        reqs = [dist.irecv(recv_lo, src=dn, group=g, tag=1), dist.irecv(recv_hi, src=up, group=g, tag=2),
+                dist.isend(send_hi, dst=up, group=g, tag=1), dist.isend(send_lo, dst=dn, group=g, tag=2)]
+        for r in reqs:
+            r.wait()
+
+    def allreduce(self, buf):
+        self.n_allreduce += 1
+        if self.nranks > 1:
+            self.dist.all_reduce(buf, op=self.dist.ReduceOp.SUM, group=self.group)
+
+    def _exchange(self, user, slo, shi, rlo, rhi, nbytes, stream):
+        try:
+            self.exchange(self._bytes(slo, nbytes), self._bytes(shi, nbytes), self._bytes(rlo, nbytes),
+                          self._bytes(rhi, nbytes))
+            return 0
+        except Exception as e:  # an exception must not cross the C frame
+            self.error = e
+            return 1
+
+    def _allreduce(self, user, buf, n, stream):
+        try:
+            import numpy as np
+            import torch
+            self.allreduce(torch.from_numpy(np.ctypeslib.as_array(buf, shape=(n,))))
+            return 0
+        except Exception as e:
+            self.error = e
+            return 1
+
+
 # ---- torch-tensor convenience wrapper ------------------------------------------------------------------
 class Lattice:
     """One lqcd_ctx.  float64 tensors go to the double entry points, float32 tensors to the ``*_f32`` ones
@@ -263,21 +379,81 @@ class Lattice:
     inside the call)."""
 
     def __init__(self, L: Sequence[int], mass: float = 0.0, antiperiodic: bool = True, recon: int = 18,
-                 precisions: int = LQCD_PREC_F64):
+                 precisions: int = LQCD_PREC_F64, slab: Optional[Sequence[int]] = None, comm: Optional[str] = None,
+                 group=None):
+        """``slab=(rank, nranks)``: this process owns time slices [rank*Lt/nranks, (rank+1)*Lt/nranks) of the
+        lattice ``L`` (include/lqcd.h, slab decomposition); all tensors are then those of the local lattice
+        ``self.L`` = (Lx, Ly, Lz, Lt/nranks).  ``comm``: "nccl" (the library's own NCCL communicator; the id is
+        handed round with ``torch.distributed``) or "torch" (:class:`TorchTransport`, host-staged)."""
         import torch
         if not torch.cuda.is_available():
             raise RuntimeError("paper_1801_01473_b200 needs a CUDA device (there is no CPU fallback)")
         self._torch = torch
-        self.L = tuple(int(v) for v in L)
-        self.V = self.L[0] * self.L[1] * self.L[2] * self.L[3]
-        self.Vh = self.V // 2
-        self.ctx = lqcd_create(*self.L)
+        self.L_global = tuple(int(v) for v in L)
+        self.transport = None
+        if slab is None:
+            self.L = self.L_global
+            self.ctx = lqcd_create(*self.L)
+        else:
+            rank, nranks = int(slab[0]), int(slab[1])
+            self.ctx = lqcd_create_slab(*self.L_global, rank, nranks)
+            self.L = self.L_global[:3] + (self.L_global[3] // max(nranks, 1),)
         if not self.ctx:
             raise LqcdError(LQCD_EINVAL, lqcd_last_error(None))
+        self.V = self.L[0] * self.L[1] * self.L[2] * self.L[3]
+        self.Vh = self.V // 2
+        if slab is not None:
+            self._init_comm(comm or "nccl", rank, nranks, group)
         self.set_option(LQCD_OPT_MASS, mass)
         self.set_option(LQCD_OPT_ANTIPERIODIC_T, 1.0 if antiperiodic else 0.0)
         self.set_option(LQCD_OPT_RECON, recon)
         self.set_option(LQCD_OPT_LINK_PRECISIONS, precisions)
+
+    def _init_comm(self, comm: str, rank: int, nranks: int, group):
+        torch = self._torch
+        if comm == "torch":
+            self.transport = TorchTransport(group)
+            assert (self.transport.rank, self.transport.nranks) == (rank, nranks), "slab != torch.distributed rank"
+            self._check(lqcd_set_comm(self.ctx, self.transport.ops))
+        elif comm == "nccl":
+            import torch.distributed as dist
+            if nranks > 1:
+                assert dist.is_initialized() and dist.get_world_size(group) == nranks and dist.get_rank(group) == rank
+            if rank == 0:
+                rc, nccl_id = lqcd_nccl_unique_id()
+                if rc != LQCD_OK:
+                    raise LqcdError(rc, lqcd_last_error(None))
+            else:
+                nccl_id = None
+            if nranks > 1:
+                box = [nccl_id]
+                dist.broadcast_object_list(box, src=dist.get_global_rank(group, 0) if group is not None else 0,
+                                           group=group)
+                nccl_id = box[0]
+            self._check(lqcd_comm_init_nccl(self.ctx, nccl_id))
+        else:
+            raise ValueError(f"unknown transport {comm!r}")
+
+    # -- slab bookkeeping (slicing only): the part of a whole-lattice tensor this rank owns.  The cut is along t,
+    # the slowest index, so a slab is one contiguous range of sites.
+    @staticmethod
+    def slab_range(L_global: Sequence[int], rank: int, nranks: int):
+        """(first, last+1) lexicographic site index of the slab."""
+        v3 = int(L_global[0]) * int(L_global[1]) * int(L_global[2])
+        lt = int(L_global[3]) // nranks
+        return rank * lt * v3, (rank + 1) * lt * v3
+
+    @staticmethod
+    def slab_of_links(links, L_global, rank, nranks):
+        """(4, V, 3, 3, 2) -> (4, V_local, 3, 3, 2), contiguous"""
+        a, b = Lattice.slab_range(L_global, rank, nranks)
+        return links[:, a:b].contiguous()
+
+    @staticmethod
+    def slab_of_vector(v, L_global, rank, nranks):
+        """parity vector (3, Vh, 2) -> (3, Vh_local, 2), contiguous"""
+        a, b = Lattice.slab_range(L_global, rank, nranks)
+        return v[:, a // 2:b // 2].contiguous()
 
     def close(self):
         if getattr(self, "ctx", None):

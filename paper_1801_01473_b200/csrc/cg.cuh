@@ -24,7 +24,9 @@ static_assert(CG_BLOCK >= LQCD_MAX_SHIFTS, "the scalar step needs one thread per
 
 // K0: r = p_i = b, x_i = 0, |b|^2.  In every sweep the vectors are V2<T>; scalars and sums are double.
 // r is the ring slot that holds r^(n0) of the first block.
-template <typename T>
+// FUSED = false (slab mode): only the block partial is written; the sum over blocks and ranks and the scalar
+// step follow in sum_partials_kernel / cg_scalar_kernel.
+template <typename T, bool FUSED = true>
 __global__ void __launch_bounds__(CG_BLOCK) cg_init_kernel(const V2<T>* __restrict__ b, V2<T>* __restrict__ r,
                                                            CgState* st, double* partials, size_t n, double tol) {
     __shared__ double red[32];
@@ -48,6 +50,10 @@ __global__ void __launch_bounds__(CG_BLOCK) cg_init_kernel(const V2<T>* __restri
         acc = fma((double)v.y, (double)v.y, acc);
     }
     const double bsum = block_sum<CG_BLOCK>(acc, red);
+    if (!FUSED) {
+        if (threadIdx.x == 0) partials[blockIdx.x] = bsum;
+        return;
+    }
     if (publish_partial<CG_BLOCK>(bsum, partials, &st->ticket[0], &last_flag)) {
         const double bb = final_sum<CG_BLOCK>(partials, gridDim.x, red);
         if (threadIdx.x == 0) {
@@ -58,7 +64,7 @@ __global__ void __launch_bounds__(CG_BLOCK) cg_init_kernel(const V2<T>* __restri
 }
 
 // K3: r_out = r_in - a s, |r_out|^2, then the scalar step that needs it
-template <typename T>
+template <typename T, bool FUSED = true>
 __global__ void __launch_bounds__(CG_BLOCK) cg_update_r_kernel(const V2<T>* r_in, V2<T>* r_out,
                                                                const V2<T>* __restrict__ s, CgState* st,
                                                                double* partials, size_t n) {
@@ -95,11 +101,43 @@ __global__ void __launch_bounds__(CG_BLOCK) cg_update_r_kernel(const V2<T>* r_in
         acc = fma((double)rv.y, (double)rv.y, acc);
     }
     const double bsum = block_sum<CG_BLOCK>(acc, red);
+    if (!FUSED) {
+        if (threadIdx.x == 0) partials[blockIdx.x] = bsum;
+        return;
+    }
     if (publish_partial<CG_BLOCK>(bsum, partials, &st->ticket[2], &last_flag)) {
         const double rr = broadcast0(final_sum<CG_BLOCK>(partials, gridDim.x, red), red);
         if (threadIdx.x == 0) st->ticket[2] = 0;
         cg_scalars_after_rr(st, rr);
     }
+}
+
+// ---- slab mode (1-D decomposition along t): a scalar product is the sum over the blocks of
+// this rank (sum_partials_kernel, fixed order), then over the ranks (all-reduce of one double: "global
+// reductions" of PAPER.md:L112), then the scalar step runs on every rank on bit-identical input
+// (cg_scalar_kernel), so that all ranks take the same decisions.
+__global__ void __launch_bounds__(CG_BLOCK) sum_partials_kernel(const double* __restrict__ partials, int n,
+                                                                double* __restrict__ out, const CgState* st,
+                                                                int check_stop) {
+    if (check_stop && st->stop) return;
+    __shared__ double red[32];
+    const double v = final_sum<CG_BLOCK>(partials, n, red);
+    if (threadIdx.x == 0) *out = v;
+}
+// which = 0: after |b|^2 ; 1: after <p,Ap> ; 2: after |r_new|^2.  One block of >= LQCD_MAX_SHIFTS threads.
+__global__ void __launch_bounds__(64) cg_scalar_kernel(CgState* st, const double* __restrict__ value, int which,
+                                                       double tol) {
+    const double v = *value;
+    if (which == 0) {
+        if (threadIdx.x == 0) cg_scalars_init(st, v, tol);
+        return;
+    }
+    if (st->stop) {
+        if (which == 1 && threadIdx.x == 0) st->stop4 = 1;
+        return;
+    }
+    if (which == 1) cg_scalars_after_pAp(st, v);
+    else cg_scalars_after_rr(st, v);
 }
 
 // K4: the base system (zeta = 1):  x_0 += a p  (rational mode: y += alpha_0 a p) ;  p = r_new + beta p
@@ -149,10 +187,15 @@ __global__ void __launch_bounds__(CG_BLOCK) cg_update_base_kernel(const V2<T>* _
 //   p_i  = B_i p_i + sum_l E_il r_l
 // MM = compile-time bound on nres (registers for the residuals).  The block that finishes last closes the
 // block of iterations (blk_j = 0), which also makes a second launch of this kernel a no-op.
+// FLUSH_UNR = shifted systems whose x_i, p_i loads are in flight together.  The sweep is latency-bound at the
+// 2 blocks per SM its registers allow (ncu: long-scoreboard stalls, 25 % occupancy): 4 shifts (8 x 16 B per
+// thread) in flight instead of 2 took it from 5.6 to 6.3 TB/s at 48^4 (profiles/ncu_full_r01.md).
+#define FLUSH_UNR 4
 template <typename T, int MM, bool RATIONAL, bool FULL>
 __device__ __forceinline__ void cg_flush_body(const int nres, const int nl, V2<T>* const* sx, V2<T>* const* sp,
                                               const V2<T>* const* sr, const T* sCP, const T* sB, const V2<T>* sDE,
                                               const T* sY, V2<T>* __restrict__ y, const size_t n) {
+    constexpr int U = FLUSH_UNR;
     const size_t stride = (size_t)gridDim.x * CG_BLOCK;
     for (size_t j = (size_t)blockIdx.x * CG_BLOCK + threadIdx.x; j < n; j += stride) {
         V2<T> rv[MM];
@@ -169,79 +212,51 @@ __device__ __forceinline__ void cg_flush_body(const int nres, const int nl, V2<T
                     yv.y = fma(sY[l], rv[l].y, yv.y);
                 }
         }
-        int e = 0;
-        for (; e + 2 <= nl; e += 2) {
-            V2<T> pv[2], xv[2];
+        // U shifts at a time (the last group is clamped to the last shift and its surplus lanes are not stored)
+        for (int e0 = 0; e0 < nl; e0 += U) {
+            V2<T> pv[U], xv[U];
 #pragma unroll
-            for (int u = 0; u < 2; ++u) {
-                pv[u] = sp[e + u][j];
-                if (!RATIONAL) xv[u] = sx[e + u][j];
+            for (int u = 0; u < U; ++u) {
+                const int e = min(e0 + u, nl - 1);
+                pv[u] = sp[e][j];
+                if (!RATIONAL) xv[u] = sx[e][j];
             }
 #pragma unroll
-            for (int u = 0; u < 2; ++u) {
-                const T cp = sCP[e + u], bb = sB[e + u];
-                T dx = cp * pv[u].x, dy = cp * pv[u].y;
-                T px = bb * pv[u].x, py = bb * pv[u].y;
-                if (!RATIONAL) {
+            for (int u = 0; u < U; ++u) {
+                const int e = e0 + u;
+                if (e < nl) {
+                    const T cp = sCP[e], bb = sB[e];
+                    T dx = cp * pv[u].x, dy = cp * pv[u].y;
+                    T px = bb * pv[u].x, py = bb * pv[u].y;
 #pragma unroll
                     for (int l = 0; l < MM; ++l)
                         if (FULL || l < nres) {
-                            const V2<T> de = sDE[(e + u) * MM + l];
-                            dx = fma(de.x, rv[l].x, dx);
-                            dy = fma(de.x, rv[l].y, dy);
+                            const V2<T> de = sDE[e * MM + l];
+                            if (!RATIONAL) {
+                                dx = fma(de.x, rv[l].x, dx);
+                                dy = fma(de.x, rv[l].y, dy);
+                            }
                             px = fma(de.y, rv[l].x, px);
                             py = fma(de.y, rv[l].y, py);
                         }
-                    xv[u].x += dx;
-                    xv[u].y += dy;
-                    sx[e + u][j] = xv[u];
-                } else {
-#pragma unroll
-                    for (int l = 0; l < MM; ++l)
-                        if (FULL || l < nres) {
-                            const V2<T> de = sDE[(e + u) * MM + l];
-                            px = fma(de.y, rv[l].x, px);
-                            py = fma(de.y, rv[l].y, py);
-                        }
-                    yv.x += dx;
-                    yv.y += dy;
-                }
-                sp[e + u][j] = make_v2(px, py);
-            }
-        }
-        for (; e < nl; ++e) {
-            const V2<T> pv = sp[e][j];
-            const T cp = sCP[e], bb = sB[e];
-            T dx = cp * pv.x, dy = cp * pv.y;
-            T px = bb * pv.x, py = bb * pv.y;
-#pragma unroll
-            for (int l = 0; l < MM; ++l)
-                if (FULL || l < nres) {
-                    const V2<T> de = sDE[e * MM + l];
                     if (!RATIONAL) {
-                        dx = fma(de.x, rv[l].x, dx);
-                        dy = fma(de.x, rv[l].y, dy);
+                        xv[u].x += dx;
+                        xv[u].y += dy;
+                        sx[e][j] = xv[u];
+                    } else {
+                        yv.x += dx;
+                        yv.y += dy;
                     }
-                    px = fma(de.y, rv[l].x, px);
-                    py = fma(de.y, rv[l].y, py);
+                    sp[e][j] = make_v2(px, py);
                 }
-            if (!RATIONAL) {
-                V2<T> xv = sx[e][j];
-                xv.x += dx;
-                xv.y += dy;
-                sx[e][j] = xv;
-            } else {
-                yv.x += dx;
-                yv.y += dy;
             }
-            sp[e][j] = make_v2(px, py);
         }
         if (RATIONAL) y[j] = yv;
     }
 }
 
 template <typename T, int MM>
-__global__ void __launch_bounds__(CG_BLOCK) cg_flush_kernel(CgState* st, size_t n) {
+__global__ void __launch_bounds__(CG_BLOCK, (MM <= 8 ? 2 : 1)) cg_flush_kernel(CgState* st, size_t n) {
     const int nres = st->blk_j;
     if (nres == 0) return;                       // nothing accumulated (solve already over); same in every block
     __shared__ V2<T>* sx[LQCD_MAX_SHIFTS];

@@ -18,10 +18,19 @@
 //          (8 B per link in double instead of 16 for u) and cos/sin are recomputed in registers: the kernel is
 //          HBM-bound, the FP pipes have room.  Th[(mu*2 + parity_of_origin)*Vh + k].
 //
+// SLAB = 1 : the lattice is one slab [t_off, t_off + Lt) of a lattice cut along t over several GPUs (the paper's
+//          1-D decomposition).  The input vector's time slices t_off-1 and t_off+Lt live in
+//          two halo buffers filled by the neighbour ranks (layout [c][face], face = Lxh*Ly*Lz), and the t-links
+//          that leave the slice below the slab in a third one (filled once, at lqcd_set_gauge).  The launch covers
+//          one or two ranges of sites, so that the interior (t = 1..Lt-2, no halo needed) runs while the faces
+//          are in flight and the two border slices afterwards (Alg. 1).
+//
 // EPI = 0 : out = D in
 // EPI = 1 : out = coef*pv - D in, plus the block partial of Re<pv, out> and the CG scalar step
 //           (this is the paper's separate zaxpy kernel, fused into the D_eo epilogue)
 // EPI = 2 : out = coef*pv - D in only
+// EPI = 3 : as 1, but only the block partial is written (at partials[part_off + blockIdx.x]); the sum over
+//           blocks, launches and ranks and the scalar step follow in their own small kernels (slab mode)
 #ifndef LQCD_DSLASH_CUH
 #define LQCD_DSLASH_CUH
 
@@ -200,6 +209,34 @@ __device__ __forceinline__ void hop_bwd(T (&ar)[3], T (&ai)[3], const V2<T>* __r
         for (int b = 0; b < 3; ++b) cmad_conj<T>(ar[a], ai[a], u[3 * b + a], vr[b], vi[b]);
 }
 
+// the same two hops with separate element strides for the link and the vector (slab faces: halo buffers)
+template <typename T, int RECON>
+__device__ __forceinline__ void hop_fwd_s(T (&ar)[3], T (&ai)[3], const V2<T>* __restrict__ w, const size_t ws,
+                                          const V2<T>* __restrict__ v, const size_t vs, unsigned int mask,
+                                          uint64_t pol_s, uint64_t pol_r) {
+    V2<T> u[9];
+    T vr[3], vi[3];
+    load_link<T, RECON>(w, ws, pol_s, u);
+    load_vec<T>(v, vs, pol_r, mask, vr, vi);
+#pragma unroll
+    for (int a = 0; a < 3; ++a)
+#pragma unroll
+        for (int b = 0; b < 3; ++b) cmad<T>(ar[a], ai[a], u[3 * a + b], vr[b], vi[b]);
+}
+template <typename T, int RECON>
+__device__ __forceinline__ void hop_bwd_s(T (&ar)[3], T (&ai)[3], const V2<T>* __restrict__ w, const size_t ws,
+                                          const V2<T>* __restrict__ v, const size_t vs, unsigned int mask,
+                                          uint64_t pol_s, uint64_t pol_r) {
+    V2<T> u[9];
+    T vr[3], vi[3];
+    load_link<T, RECON>(w, ws, pol_s, u);
+    load_vec<T>(v, vs, pol_r, mask, vr, vi);
+#pragma unroll
+    for (int a = 0; a < 3; ++a)
+#pragma unroll
+        for (int b = 0; b < 3; ++b) cmad_conj<T>(ar[a], ai[a], u[3 * b + a], vr[b], vi[b]);
+}
+
 template <typename T>
 struct DslashArgs {
     Geom g;
@@ -213,13 +250,19 @@ struct DslashArgs {
     double* partials;        // EPI == 1
     CgState* st;             // EPI == 1, or any EPI with check_stop
     int check_stop;          // 1: return at once if st->stop (CG already converged)
+    // SLAB == 1 only
+    const V2<T>* in_lo;      // halo: time slice t_off-1 of `in`, [c][face]
+    const V2<T>* in_hi;      // halo: time slice t_off+Lt of `in`, [c][face]
+    const V2<T>* Wt_lo;      // halo: t-links leaving slice t_off-1, [parity of origin][e][face]
+    int k0a, na, k0b, nsites;    // thread idx < na: site k0a+idx; else site k0b+(idx-na); nsites in all
+    int part_off;            // EPI == 3: first slot of this launch in `partials`
 };
 
 // registers: double needs ~126 (4 blocks of 128 threads per SM); single fits 6 blocks
 template <typename T> struct DsOcc { static constexpr int minb = DS_MINB; };
 template <> struct DsOcc<float> { static constexpr int minb = DS_MINB_F32; };
 
-template <typename T, int RECON, int EPI, int U1>
+template <typename T, int RECON, int EPI, int U1, int SLAB = 0>
 __global__ void __launch_bounds__(DS_BLOCK, DsOcc<T>::minb) dslash_kernel(const DslashArgs<T> A) {
     constexpr int NE = (RECON == 12) ? 6 : 9;
     if (A.check_stop) {
@@ -231,8 +274,16 @@ __global__ void __launch_bounds__(DS_BLOCK, DsOcc<T>::minb) dslash_kernel(const 
     }
     const Geom& g = A.g;
     const int kraw = blockIdx.x * DS_BLOCK + threadIdx.x;
-    const bool valid = kraw < g.Vh;
-    const int k = valid ? kraw : g.Vh - 1;
+    bool valid;
+    int k;
+    if (SLAB) {
+        valid = kraw < A.nsites;
+        const int i = valid ? kraw : A.nsites - 1;
+        k = (i < A.na) ? A.k0a + i : A.k0b + (i - A.na);
+    } else {
+        valid = kraw < g.Vh;
+        k = valid ? kraw : g.Vh - 1;
+    }
     const size_t vh = (size_t)g.Vh;
 
     // step A3: coordinates, neighbours, phases
@@ -258,8 +309,11 @@ __global__ void __launch_bounds__(DS_BLOCK, DsOcc<T>::minb) dslash_kernel(const 
     const unsigned int my = (unsigned)(x & 1) << 31;                    // eta_y = (-1)^x
     const unsigned int mz = (unsigned)((x + y) & 1) << 31;              // eta_z = (-1)^(x+y)
     const unsigned int mt = (unsigned)((x + y + z) & 1) << 31;          // eta_t = (-1)^(x+y+z)
-    const unsigned int mtf = mt ^ ((g.antiperiodic && t == g.Lt - 1) ? SB : 0u);   // link (x,t) leaves Lt-1
-    const unsigned int mtb = mt ^ ((g.antiperiodic && t == 0) ? SB : 0u);          // link (x-t,t) leaves Lt-1
+    // the boundary sign sits on the links that leave the last time slice of the WHOLE lattice
+    const int tg = SLAB ? t + g.t_off : t;
+    const int Ltg = SLAB ? g.Lt_glob : g.Lt;
+    const unsigned int mtf = mt ^ ((g.antiperiodic && tg == Ltg - 1) ? SB : 0u);   // link (x,t) leaves Lt-1
+    const unsigned int mtb = mt ^ ((g.antiperiodic && tg == 0) ? SB : 0u);         // link (x-t,t) leaves Lt-1
 
     const uint64_t pol_s = l2_policy_evict_first();
     const uint64_t pol_r = l2_policy_evict_last();
@@ -273,7 +327,7 @@ __global__ void __launch_bounds__(DS_BLOCK, DsOcc<T>::minb) dslash_kernel(const 
     T coef = (T)0;
     V2<T> pv[3];
     if (EPI != 0) {
-        coef = (T)((EPI == 1) ? A.st->c0 : A.coef);     // CG: m^2 + sigma0 from the device state (graph-invariant)
+        coef = (T)((EPI == 1 || EPI == 3) ? A.st->c0 : A.coef);     // CG: m^2 + sigma0 from the device state (graph-invariant)
 #if EPI_PLOAD == 1
 #pragma unroll
         for (int c = 0; c < 3; ++c) pv[c] = A.pv[c * vh + k];
@@ -293,8 +347,20 @@ __global__ void __launch_bounds__(DS_BLOCK, DsOcc<T>::minb) dslash_kernel(const 
     hop_bwd<T, RECON, U1>(ar, ai, Wb + 1 * mu_stride + kyb, in + kyb, vh, my ^ SB, pol_s, pol_r, Tb + 1 * th_stride + kyb);
     hop_fwd<T, RECON, U1>(ar, ai, Wf + 2 * mu_stride, in + kzf, vh, mz, pol_s, pol_r, Tf + 2 * th_stride);
     hop_bwd<T, RECON, U1>(ar, ai, Wb + 2 * mu_stride + kzb, in + kzb, vh, mz ^ SB, pol_s, pol_r, Tb + 2 * th_stride + kzb);
-    hop_fwd<T, RECON, U1>(ar, ai, Wf + 3 * mu_stride, in + ktf, vh, mtf, pol_s, pol_r, Tf + 3 * th_stride);
-    hop_bwd<T, RECON, U1>(ar, ai, Wb + 3 * mu_stride + ktb, in + ktb, vh, mtb ^ SB, pol_s, pol_r, Tb + 3 * th_stride + ktb);
+    if (!SLAB) {
+        hop_fwd<T, RECON, U1>(ar, ai, Wf + 3 * mu_stride, in + ktf, vh, mtf, pol_s, pol_r, Tf + 3 * th_stride);
+        hop_bwd<T, RECON, U1>(ar, ai, Wb + 3 * mu_stride + ktb, in + ktb, vh, mtb ^ SB, pol_s, pol_r, Tb + 3 * th_stride + ktb);
+    } else {
+        // across the slab faces the neighbour vector (and, downwards, the link) comes from the halo buffers
+        const size_t face = (size_t)g.st;
+        const int kf = k - t * g.st;                                  // index inside a time slice
+        const bool top = (t == g.Lt - 1), bot = (t == 0);
+        const V2<T>* vf = top ? A.in_hi + kf : in + k + g.st;
+        hop_fwd_s<T, RECON>(ar, ai, Wf + 3 * mu_stride, vh, vf, top ? face : vh, mtf, pol_s, pol_r);
+        const V2<T>* vb = bot ? A.in_lo + kf : in + k - g.st;
+        const V2<T>* wb = bot ? A.Wt_lo + (size_t)(1 - A.par) * NE * face + kf : Wb + 3 * mu_stride + k - g.st;
+        hop_bwd_s<T, RECON>(ar, ai, wb, bot ? face : vh, vb, bot ? face : vh, mtb ^ SB, pol_s, pol_r);
+    }
 
     if (EPI == 0) {
         if (valid) {
@@ -319,6 +385,11 @@ __global__ void __launch_bounds__(DS_BLOCK, DsOcc<T>::minb) dslash_kernel(const 
             dot = fma((double)p.x, (double)o.x, dot);
             dot = fma((double)p.y, (double)o.y, dot);
         }
+    }
+    if (EPI == 3) {
+        __shared__ double red3[32];
+        const double bsum = block_sum<DS_BLOCK>(dot, red3);
+        if (threadIdx.x == 0) A.partials[A.part_off + blockIdx.x] = bsum;
     }
     if (EPI == 1) {
         __shared__ double red[32];

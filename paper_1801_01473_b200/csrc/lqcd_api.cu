@@ -15,6 +15,7 @@
 #include <vector>
 
 #include "cg.cuh"
+#include "comm.h"
 #include "dslash.cuh"
 #include "lqcd_internal.cuh"
 
@@ -42,6 +43,12 @@ struct PrecBufs {
     int n_pextra = 0;
     cudaGraphExec_t graph_exec = nullptr;    // CUDA graph of `graph_iters` CG iterations
     int graph_iters = 0, graph_rational = 0, graph_block = 0;
+    int graph_launches = 0;                  // kernels one replay of the graph launches
+    // slab mode: faces of the input vector, [lo|hi][c][face] each; t-links leaving the slice below the slab
+    V2<T>* halo_send = nullptr;
+    V2<T>* halo_recv = nullptr;
+    V2<T>* Wt_lo = nullptr;                  // [parity of origin][e][face]
+    V2<T>* Wt_send = nullptr;                // one-time staging of my top t-links (+ a dummy receive buffer behind it)
     V2<T>* stage_b = nullptr;                // host-call staging (device copies of host arguments)
     V2<T>* stage_x[LQCD_MAX_SHIFTS] = {};
     int n_stage_x = 0;
@@ -69,6 +76,18 @@ struct lqcd_ctx {
     int prec_opt;            // LQCD_OPT_LINK_PRECISIONS: which of them the next lqcd_set_gauge stores
     int u1_on;               // general U(1) phases in force (lqcd_set_u1_phases with a non-NULL field)
     double* dev_max;
+
+    // slab decomposition (lqcd_create_slab): rank of nranks along t, transport, its stream and events
+    int slab, rank, nranks;
+    lqcd_comm_ops comm;
+    bool has_comm;
+    lqcd_nccl::Transport nccl;
+    cudaStream_t comm_stream;
+    cudaEvent_t ev_pack, ev_halo;
+    double* red;             // device: the scalar product being reduced over ranks
+    char* host_stage;        // pinned: staging of a host_staged transport (4 faces, or the link faces)
+    size_t host_stage_bytes;
+    double* red_host;        // pinned
 
     double* partials;
     size_t n_partials;
@@ -173,8 +192,15 @@ int ensure_basics(lqcd_ctx* c) {
     if (c->basics) return LQCD_OK;
     int rc;
     if ((rc = dev_alloc(c, (void**)&c->st_dev, sizeof(CgState)))) return rc;
-    c->n_partials = (size_t)(ds_grid(c) > cg_grid(c) ? ds_grid(c) : cg_grid(c));
+    c->n_partials = (size_t)(ds_grid(c) > cg_grid(c) ? ds_grid(c) : cg_grid(c)) + 4;
     if ((rc = dev_alloc(c, (void**)&c->partials, c->n_partials * sizeof(double)))) return rc;
+    if (c->slab) {
+        if ((rc = dev_alloc(c, (void**)&c->red, 2 * sizeof(double)))) return rc;
+        CU(cudaMallocHost((void**)&c->red_host, 2 * sizeof(double)));
+        CU(cudaStreamCreateWithFlags(&c->comm_stream, cudaStreamNonBlocking));
+        CU(cudaEventCreateWithFlags(&c->ev_pack, cudaEventDisableTiming));
+        CU(cudaEventCreateWithFlags(&c->ev_halo, cudaEventDisableTiming));
+    }
     if ((rc = dev_alloc(c, (void**)&c->dev_max, sizeof(double)))) return rc;
     CU(cudaMemsetAsync(c->st_dev, 0, sizeof(CgState), c->stream));
     CU(cudaMallocHost((void**)&c->st_host, sizeof(CgState)));
@@ -230,11 +256,162 @@ void launch_dslash_t(lqcd_ctx* c, const DslashArgs<T>& a) {
     else launch_dslash_u<T, EPI, 0>(c, a);
 }
 
+// ---- slab mode ------------------------------------------------------------------------------------------------
+#define COMM(expr)                                                                                   \
+    do {                                                                                             \
+        if ((expr) != 0) return fail(c, LQCD_ECOMM, "transport failed in %s (%s:%d)", #expr, __FILE__, __LINE__); \
+    } while (0)
+
+size_t face_sites(const lqcd_ctx* c) { return (size_t)c->g.st; }
+
+int ensure_host_stage(lqcd_ctx* c, size_t bytes) {
+    if (c->host_stage_bytes >= bytes) return LQCD_OK;
+    if (c->host_stage) cudaFreeHost(c->host_stage);
+    c->host_stage = nullptr;
+    c->host_stage_bytes = 0;
+    CU(cudaMallocHost((void**)&c->host_stage, bytes));
+    c->host_stage_bytes = bytes;
+    return LQCD_OK;
+}
+
+// ring exchange of two device buffers of `bytes` each, ordered after the work enqueued on c->comm_stream
+int comm_exchange(lqcd_ctx* c, const void* send_lo, const void* send_hi, void* recv_lo, void* recv_hi, size_t bytes) {
+    if (!c->comm.host_staged) {
+        COMM(c->comm.exchange(c->comm.user, send_lo, send_hi, recv_lo, recv_hi, bytes, (void*)c->comm_stream));
+        return LQCD_OK;
+    }
+    int rc;
+    if ((rc = ensure_host_stage(c, 4 * bytes))) return rc;
+    char* h = c->host_stage;
+    CU(cudaMemcpyAsync(h, send_lo, bytes, cudaMemcpyDeviceToHost, c->comm_stream));
+    CU(cudaMemcpyAsync(h + bytes, send_hi, bytes, cudaMemcpyDeviceToHost, c->comm_stream));
+    CU(cudaStreamSynchronize(c->comm_stream));
+    COMM(c->comm.exchange(c->comm.user, h, h + bytes, h + 2 * bytes, h + 3 * bytes, bytes, nullptr));
+    CU(cudaMemcpyAsync(recv_lo, h + 2 * bytes, bytes, cudaMemcpyHostToDevice, c->comm_stream));
+    CU(cudaMemcpyAsync(recv_hi, h + 3 * bytes, bytes, cudaMemcpyHostToDevice, c->comm_stream));
+    CU(cudaStreamSynchronize(c->comm_stream));       // the staging buffer is free again on return
+    return LQCD_OK;
+}
+
+// c->red[0] <- sum over ranks, on the compute stream
+int comm_allreduce(lqcd_ctx* c) {
+    if (!c->comm.host_staged) {
+        COMM(c->comm.allreduce_sum(c->comm.user, c->red, 1, (void*)c->stream));
+        return LQCD_OK;
+    }
+    CU(cudaMemcpyAsync(c->red_host, c->red, sizeof(double), cudaMemcpyDeviceToHost, c->stream));
+    CU(cudaStreamSynchronize(c->stream));
+    COMM(c->comm.allreduce_sum(c->comm.user, c->red_host, 1, nullptr));
+    CU(cudaMemcpyAsync(c->red, c->red_host, sizeof(double), cudaMemcpyHostToDevice, c->stream));
+    CU(cudaStreamSynchronize(c->stream));            // red_host may be rewritten by the next reduction
+    return LQCD_OK;
+}
+
+template <typename T>
+int ensure_halo(lqcd_ctx* c) {
+    int rc;
+    PrecBufs<T>& B = bufs<T>(c);
+    const size_t fb = 2 * 3 * face_sites(c) * sizeof(V2<T>);
+    if (!B.halo_send && (rc = dev_alloc(c, (void**)&B.halo_send, fb))) return rc;
+    if (!B.halo_recv && (rc = dev_alloc(c, (void**)&B.halo_recv, fb))) return rc;
+    return LQCD_OK;
+}
+
+template <typename T, int EPI>
+void launch_dslash_slab_k(lqcd_ctx* c, const DslashArgs<T>& a, int grid) {
+    if (bufs<T>(c).recon_stored == 12)
+        dslash_kernel<T, 12, EPI, 0, 1><<<grid, DS_BLOCK, 0, c->stream>>>(a);
+    else
+        dslash_kernel<T, 18, EPI, 0, 1><<<grid, DS_BLOCK, 0, c->stream>>>(a);
+    ++c->launches;
+}
+
+// One operator application on a slab (Alg. 1 of the paper): the two faces of `in` are packed
+// and sent, the interior time slices are computed meanwhile, the two border slices once the halos have arrived.
+// EPI == 1 becomes EPI == 3: block partials in c->partials[0 .. *n_part), summed by the caller.
+template <typename T>
+int slab_dslash(lqcd_ctx* c, int epi, V2<T>* out, const V2<T>* in, int par, const V2<T>* pv, double coef, int check_stop,
+                int* n_part) {
+    int rc;
+    if (!c->has_comm) return fail(c, LQCD_ECOMM, "slab context without a transport (lqcd_comm_init_nccl / lqcd_set_comm)");
+    if ((rc = ensure_halo<T>(c))) return rc;
+    PrecBufs<T>& B = bufs<T>(c);
+    const size_t face = face_sites(c), vh = c->Vh;
+    const size_t row = face * sizeof(V2<T>), pitch = vh * sizeof(V2<T>);
+    V2<T>* send_lo = B.halo_send;
+    V2<T>* send_hi = B.halo_send + 3 * face;
+    V2<T>* recv_lo = B.halo_recv;
+    V2<T>* recv_hi = B.halo_recv + 3 * face;
+    // a face is three contiguous runs (one per colour) of the vector: strided copies, no kernel
+    CU(cudaMemcpy2DAsync(send_lo, row, in, pitch, row, 3, cudaMemcpyDeviceToDevice, c->stream));
+    CU(cudaMemcpy2DAsync(send_hi, row, in + (vh - face), pitch, row, 3, cudaMemcpyDeviceToDevice, c->stream));
+    CU(cudaEventRecord(c->ev_pack, c->stream));
+
+    DslashArgs<T> a{};
+    a.g = c->g;
+    a.W = B.W;
+    a.Th = nullptr;
+    a.in = in;
+    a.out = out;
+    a.par = par;
+    a.pv = pv;
+    a.coef = coef;
+    a.partials = c->partials;
+    a.st = c->st_dev;
+    a.check_stop = check_stop;
+    a.in_lo = recv_lo;
+    a.in_hi = recv_hi;
+    a.Wt_lo = B.Wt_lo;
+    const int kepi = (epi == 1) ? 3 : epi;
+    int part = 0;
+    auto launch = [&](int grid) {
+        a.part_off = part;
+        if (kepi == 0) launch_dslash_slab_k<T, 0>(c, a, grid);
+        else if (kepi == 2) launch_dslash_slab_k<T, 2>(c, a, grid);
+        else launch_dslash_slab_k<T, 3>(c, a, grid);
+        part += grid;
+    };
+    // interior: t = 1 .. Lt-2
+    const int n_int = (int)(vh - 2 * face);
+    if (n_int > 0) {
+        a.k0a = (int)face;
+        a.na = n_int;
+        a.k0b = 0;
+        a.nsites = n_int;
+        launch((n_int + DS_BLOCK - 1) / DS_BLOCK);
+    }
+    // faces in flight on the communication stream
+    CU(cudaStreamWaitEvent(c->comm_stream, c->ev_pack, 0));
+    if ((rc = comm_exchange(c, send_lo, send_hi, recv_lo, recv_hi, 3 * row))) return rc;
+    CU(cudaEventRecord(c->ev_halo, c->comm_stream));
+    CU(cudaStreamWaitEvent(c->stream, c->ev_halo, 0));
+    // borders: t = 0 and t = Lt-1
+    a.k0a = 0;
+    a.na = (int)face;
+    a.k0b = (int)(vh - face);
+    a.nsites = (int)(2 * face);
+    launch((a.nsites + DS_BLOCK - 1) / DS_BLOCK);
+    CU(cudaGetLastError());
+    if (n_part) *n_part = part;
+    return LQCD_OK;
+}
+
+// sum of c->partials[0..n) over this rank's blocks, then over the ranks, then the scalar step `which`
+int slab_reduce_step(lqcd_ctx* c, int n, int which, double tol, int check_stop) {
+    int rc;
+    sum_partials_kernel<<<1, CG_BLOCK, 0, c->stream>>>(c->partials, n, c->red, c->st_dev, check_stop);
+    if ((rc = comm_allreduce(c))) return rc;
+    cg_scalar_kernel<<<1, 64, 0, c->stream>>>(c->st_dev, c->red, which, tol);
+    c->launches += 2;
+    CU(cudaGetLastError());
+    return LQCD_OK;
+}
+
 // out(par) = D in, optionally with the epilogue
 template <typename T>
 void launch_dslash(lqcd_ctx* c, int epi, V2<T>* out, const V2<T>* in, int par, const V2<T>* pv, double coef,
                    int check_stop) {
-    DslashArgs<T> a;
+    DslashArgs<T> a{};
     a.g = c->g;
     a.W = bufs<T>(c).W;
     a.Th = bufs<T>(c).Th;
@@ -264,10 +441,26 @@ void launch_flush(lqcd_ctx* c) {
 
 // one CG iteration = K1..K4 (cg.cuh), plus K5 when it is the last of a block; pos = iteration index mod m
 template <typename T>
-void launch_cg_iteration(lqcd_ctx* c, int pos) {
+int launch_cg_iteration(lqcd_ctx* c, int pos) {
     const size_t n = c->Vh * 3;
     const int m = c->shift_block;
     PrecBufs<T>& B = bufs<T>(c);
+    if (c->slab) {
+        // the same iteration with the two exchange steps of the slab decomposition: faces before each operator,
+        // one all-reduced double after each scalar product
+        int rc, np = 0;
+        if ((rc = slab_dslash<T>(c, 0, B.t, B.p, 1, nullptr, 0.0, 1, nullptr))) return rc;
+        if ((rc = slab_dslash<T>(c, 1, B.s, B.t, 0, B.p, 0.0, 1, &np))) return rc;
+        if ((rc = slab_reduce_step(c, np, 1, 0.0, 1))) return rc;
+        cg_update_r_kernel<T, false><<<cg_grid(c), CG_BLOCK, 0, c->stream>>>(B.hist[(pos + m - 1) % m], B.hist[pos], B.s,
+                                                                             c->st_dev, c->partials, n);
+        ++c->launches;
+        if ((rc = slab_reduce_step(c, cg_grid(c), 2, 0.0, 1))) return rc;
+        cg_update_base_kernel<T><<<cg_grid(c), CG_BLOCK, 0, c->stream>>>(B.hist[pos], B.p, c->st_dev, n);
+        ++c->launches;
+        if (pos == m - 1) launch_flush<T>(c);
+        return LQCD_OK;
+    }
     launch_dslash<T>(c, 0, B.t, B.p, 1, nullptr, 0.0, 1);
     launch_dslash<T>(c, 1, B.s, B.t, 0, B.p, 0.0, 1);
     cg_update_r_kernel<T><<<cg_grid(c), CG_BLOCK, 0, c->stream>>>(B.hist[(pos + m - 1) % m], B.hist[pos], B.s, c->st_dev,
@@ -275,6 +468,7 @@ void launch_cg_iteration(lqcd_ctx* c, int pos) {
     cg_update_base_kernel<T><<<cg_grid(c), CG_BLOCK, 0, c->stream>>>(B.hist[pos], B.p, c->st_dev, n);
     c->launches += 2;
     if (pos == m - 1) launch_flush<T>(c);
+    return LQCD_OK;
 }
 
 // the host looks at the stop flag every this many iterations: a whole number of blocks
@@ -294,9 +488,15 @@ int build_graph(lqcd_ctx* c, int iters, int rational) {
     cudaGraph_t graph = nullptr;
     const long long before = c->launches;
     CU(cudaStreamBeginCapture(c->stream, cudaStreamCaptureModeThreadLocal));
-    for (int i = 0; i < iters; ++i) launch_cg_iteration<T>(c, i % c->shift_block);
+    int rc_it = LQCD_OK;
+    for (int i = 0; i < iters && !rc_it; ++i) rc_it = launch_cg_iteration<T>(c, i % c->shift_block);
     cudaError_t e = cudaStreamEndCapture(c->stream, &graph);
+    B.graph_launches = (int)(c->launches - before);
     c->launches = before;     // capturing is not launching
+    if (rc_it) {
+        if (graph) cudaGraphDestroy(graph);
+        return rc_it;
+    }
     if (e != cudaSuccess) return fail(c, LQCD_ECUDA, "graph capture failed: %s", cudaGetErrorString(e));
     e = cudaGraphInstantiate(&B.graph_exec, graph, 0);
     cudaGraphDestroy(graph);
@@ -361,6 +561,27 @@ int store_gauge(lqcd_ctx* c, const double* links, int recon) {
     CU(cudaStreamSynchronize(c->stream));
     if (recon == 12 && !(*c->max_host <= 1e-12))
         return fail(c, LQCD_ENOTSU3, "RECON=12 but max|r2 - conj(r0 x r1)| = %.3e > 1e-12", *c->max_host);
+    if (c->slab) {
+        // the backward t-hop of my lowest time slice needs the t-links that leave the slice below it: the top
+        // t-links of rank-1, sent up the ring once (both origin parities, NE elements, stored format)
+        const int NE = (recon == 12) ? 6 : 9;
+        const size_t face = face_sites(c), vh = c->Vh;
+        const size_t n = (size_t)2 * NE * face;
+        if (!B.Wt_lo) {
+            const size_t n18 = (size_t)2 * 9 * face;             // sized for either format
+            if ((rc = dev_alloc(c, (void**)&B.Wt_lo, n18 * sizeof(V2<T>)))) return rc;
+            if ((rc = dev_alloc(c, (void**)&B.Wt_send, 2 * n18 * sizeof(V2<T>)))) return rc;
+        }
+        const size_t row = face * sizeof(V2<T>);
+        // rows (3*2 + parity)*NE + e of W, last time slice
+        CU(cudaMemcpy2DAsync(B.Wt_send, row, B.W + (size_t)6 * NE * vh + (vh - face), vh * sizeof(V2<T>), row, 2 * NE,
+                             cudaMemcpyDeviceToDevice, c->stream));
+        CU(cudaEventRecord(c->ev_pack, c->stream));
+        CU(cudaStreamWaitEvent(c->comm_stream, c->ev_pack, 0));
+        V2<T>* dummy = B.Wt_send + (size_t)2 * 9 * face;        // what comes down the ring is not needed
+        if ((rc = comm_exchange(c, B.Wt_send, B.Wt_send, B.Wt_lo, dummy, n * sizeof(V2<T>)))) return rc;
+        CU(cudaStreamSynchronize(c->comm_stream));
+    }
     B.recon_stored = recon;
     return LQCD_OK;
 }
@@ -438,6 +659,12 @@ lqcd_ctx* lqcd_create(int Lx, int Ly, int Lz, int Lt) {
     g.dy = make_fastdiv((uint32_t)Ly);
     g.dz = make_fastdiv((uint32_t)Lz);
     g.antiperiodic = 1;
+    g.t_off = 0;
+    g.Lt_glob = Lt;
+    c->slab = 0;
+    c->rank = 0;
+    c->nranks = 1;
+    c->has_comm = false;
     c->device = dev;
     c->num_sms = prop.multiProcessorCount;
     c->stream = nullptr;
@@ -461,6 +688,17 @@ void lqcd_destroy(lqcd_ctx* c) {
     if (c->st_host) cudaFreeHost(c->st_host);
     if (c->flag_host) cudaFreeHost(c->flag_host);
     if (c->max_host) cudaFreeHost(c->max_host);
+    if (c->nccl.comm) {
+        lqcd_nccl::Api* a = lqcd_nccl::api(nullptr);
+        if (a) a->CommDestroy(c->nccl.comm);
+    }
+    if (c->host_stage) cudaFreeHost(c->host_stage);
+    if (c->red_host) cudaFreeHost(c->red_host);
+    if (c->basics && c->slab) {
+        cudaStreamDestroy(c->comm_stream);
+        cudaEventDestroy(c->ev_pack);
+        cudaEventDestroy(c->ev_halo);
+    }
     if (c->basics) {
         cudaEventDestroy(c->ev[0]);
         cudaEventDestroy(c->ev[1]);
@@ -472,6 +710,90 @@ void lqcd_destroy(lqcd_ctx* c) {
 }
 
 const char* lqcd_last_error(const lqcd_ctx* c) { return c ? c->err : g_create_error; }
+
+lqcd_ctx* lqcd_create_slab(int Lx, int Ly, int Lz, int Lt_global, int rank, int nranks) {
+    if (nranks < 1 || rank < 0 || rank >= nranks) {
+        snprintf(g_create_error, sizeof(g_create_error), "rank %d of %d is not a valid slab", rank, nranks);
+        return nullptr;
+    }
+    if (Lt_global < 2 || Lt_global % nranks != 0 || ((Lt_global / nranks) & 1)) {
+        snprintf(g_create_error, sizeof(g_create_error), "Lt = %d over %d ranks: every slab needs an even number of time slices",
+                 Lt_global, nranks);
+        return nullptr;
+    }
+    const int Lt_loc = Lt_global / nranks;
+    lqcd_ctx* c = lqcd_create(Lx, Ly, Lz, Lt_loc);
+    if (!c) return nullptr;
+    c->slab = 1;
+    c->rank = rank;
+    c->nranks = nranks;
+    c->g.t_off = rank * Lt_loc;
+    c->g.Lt_glob = Lt_global;
+    return c;
+}
+
+int lqcd_slab_info(const lqcd_ctx* c, int* rank, int* nranks, int* t_offset, int* Lt_global) {
+    if (!c) return LQCD_EINVAL;
+    if (rank) *rank = c->rank;
+    if (nranks) *nranks = c->nranks;
+    if (t_offset) *t_offset = c->g.t_off;
+    if (Lt_global) *Lt_global = c->g.Lt_glob;
+    return LQCD_OK;
+}
+
+int lqcd_set_comm(lqcd_ctx* c, const lqcd_comm_ops* ops) {
+    if (!c) return LQCD_EINVAL;
+    if (!c->slab) return fail(c, LQCD_EINVAL, "not a slab context (lqcd_create_slab)");
+    if (!ops || !ops->exchange || !ops->allreduce_sum) return fail(c, LQCD_EINVAL, "transport functions missing");
+    drop_graphs(c);
+    c->comm = *ops;
+    c->has_comm = true;
+    return LQCD_OK;
+}
+
+int lqcd_nccl_unique_id(void* id) {
+    if (!id) return LQCD_EINVAL;
+    const char* why = nullptr;
+    lqcd_nccl::Api* a = lqcd_nccl::api(&why);
+    if (!a) {
+        snprintf(g_create_error, sizeof(g_create_error), "NCCL unavailable: %s", why ? why : "?");
+        return LQCD_ECOMM;
+    }
+    lqcd_nccl::unique_id u;
+    const int rc = a->GetUniqueId(&u);
+    if (rc) {
+        snprintf(g_create_error, sizeof(g_create_error), "ncclGetUniqueId: %s", a->GetErrorString(rc));
+        return LQCD_ECOMM;
+    }
+    memcpy(id, &u, sizeof(u));
+    return LQCD_OK;
+}
+
+int lqcd_comm_init_nccl(lqcd_ctx* c, const void* id) {
+    if (!c) return LQCD_EINVAL;
+    if (!c->slab) return fail(c, LQCD_EINVAL, "not a slab context (lqcd_create_slab)");
+    if (!id) return fail(c, LQCD_EINVAL, "id is NULL");
+    if (c->nccl.comm) return fail(c, LQCD_EINVAL, "NCCL transport already initialised");
+    const char* why = nullptr;
+    lqcd_nccl::Api* a = lqcd_nccl::api(&why);
+    if (!a) return fail(c, LQCD_ECOMM, "NCCL unavailable: %s", why ? why : "?");
+    lqcd_nccl::unique_id u;
+    memcpy(&u, id, sizeof(u));
+    c->nccl.rank = c->rank;
+    c->nccl.nranks = c->nranks;
+    const int rc = a->CommInitRank(&c->nccl.comm, c->nranks, u, c->rank);
+    if (rc) {
+        c->nccl.comm = nullptr;
+        return fail(c, LQCD_ECOMM, "ncclCommInitRank: %s", a->GetErrorString(rc));
+    }
+    lqcd_comm_ops ops;
+    ops.user = &c->nccl;
+    ops.exchange = lqcd_nccl::exchange;
+    ops.allreduce_sum = lqcd_nccl::allreduce_sum;
+    ops.host_staged = 0;
+    ops.graph_safe = 1;
+    return lqcd_set_comm(c, &ops);
+}
 
 int lqcd_set_stream(lqcd_ctx* c, void* cuda_stream) {
     if (!c) return LQCD_EINVAL;
@@ -549,7 +871,13 @@ size_t lqcd_workspace_bytes(const lqcd_ctx* c, int nshift) {
     if (c->prec_opt & LQCD_PREC_F64) b += align_up((size_t)8 * c->Vh * sizeof(double));   // U(1) angles, if set
     if (c->prec_opt & LQCD_PREC_F32) b += align_up((size_t)8 * c->Vh * sizeof(float));
     b += align_up(sizeof(CgState)) + align_up(sizeof(double));
-    const size_t np = (size_t)(ds_grid(c) > cg_grid(c) ? ds_grid(c) : cg_grid(c));
+    if (c->slab) {
+        const size_t face = face_sites(c);
+        b += align_up(2 * sizeof(double));
+        if (c->prec_opt & LQCD_PREC_F64) b += 2 * align_up(6 * face * sizeof(double2)) + align_up(18 * face * sizeof(double2)) + align_up(36 * face * sizeof(double2));
+        if (c->prec_opt & LQCD_PREC_F32) b += 2 * align_up(6 * face * sizeof(float2)) + align_up(18 * face * sizeof(float2)) + align_up(36 * face * sizeof(float2));
+    }
+    const size_t np = (size_t)(ds_grid(c) > cg_grid(c) ? ds_grid(c) : cg_grid(c)) + 4;
     b += align_up(np * sizeof(double));
     return b;
 }
@@ -568,6 +896,8 @@ int lqcd_set_workspace(lqcd_ctx* c, void* dev, size_t bytes) {
 int lqcd_set_gauge(lqcd_ctx* c, const double* links) {
     if (!c) return LQCD_EINVAL;
     if (!links) return fail(c, LQCD_EINVAL, "links is NULL");
+    if (c->slab && !c->has_comm)
+        return fail(c, LQCD_ECOMM, "slab context: set a transport (lqcd_comm_init_nccl / lqcd_set_comm) before lqcd_set_gauge");
     int rc;
     if ((rc = ensure_basics(c))) return rc;
     drop_graphs(c);
@@ -591,6 +921,7 @@ int lqcd_set_gauge(lqcd_ctx* c, const double* links) {
 
 int lqcd_set_u1_phases(lqcd_ctx* c, const double* theta) {
     if (!c) return LQCD_EINVAL;
+    if (c->slab && theta) return fail(c, LQCD_EINVAL, "general U(1) phases are not available on a slab context");
     int rc;
     if ((rc = ensure_basics(c))) return rc;
     drop_graphs(c);           // the kernel variant and its arguments are baked into the graph
@@ -653,6 +984,10 @@ int apply_d(lqcd_ctx* c, T* out, const T* in, int par) {
     if (out == in) return fail(c, LQCD_EINVAL, "in and out must not alias");
     int rc;
     if ((rc = check_ctx_gauge<T>(c))) return rc;
+    if (c->slab) {
+        if ((rc = ensure_basics(c))) return rc;
+        return slab_dslash<T>(c, 0, (V2<T>*)out, (const V2<T>*)in, par, nullptr, 0.0, 0, nullptr);
+    }
     launch_dslash<T>(c, 0, (V2<T>*)out, (const V2<T>*)in, par, nullptr, 0.0, 0);
     CU(cudaGetLastError());
     return LQCD_OK;
@@ -682,6 +1017,10 @@ int apply_mdagm(lqcd_ctx* c, T* out_even, const T* in_even, double sigma) {
     if ((rc = check_ctx_gauge<T>(c))) return rc;
     if ((rc = ensure_tmp<T>(c))) return rc;
     PrecBufs<T>& B = bufs<T>(c);
+    if (c->slab) {
+        if ((rc = slab_dslash<T>(c, 0, B.t, (const V2<T>*)in_even, 1, nullptr, 0.0, 0, nullptr))) return rc;
+        return slab_dslash<T>(c, 2, (V2<T>*)out_even, B.t, 0, (const V2<T>*)in_even, c->mass * c->mass + sigma, 0, nullptr);
+    }
     launch_dslash<T>(c, 0, B.t, (const V2<T>*)in_even, 1, nullptr, 0.0, 0);
     launch_dslash<T>(c, 2, (V2<T>*)out_even, B.t, 0, (const V2<T>*)in_even, c->mass * c->mass + sigma, 0);
     CU(cudaGetLastError());
@@ -712,6 +1051,7 @@ int solve(lqcd_ctx* c, const T* b_even, const double* shifts, int nshift, double
     int rc;
     if ((rc = check_ctx_gauge<T>(c))) return rc;
     if ((rc = ensure_solver<T>(c, nshift))) return rc;
+    if (c->slab && (rc = ensure_halo<T>(c))) return rc;      // nothing may be allocated while the graph is captured
     PrecBufs<T>& B = bufs<T>(c);
 
     // base system = smallest shift (R5); ties: the first
@@ -741,13 +1081,22 @@ int solve(lqcd_ctx* c, const T* b_even, const double* shifts, int nshift, double
     const size_t n = c->Vh * 3;
     CU(cudaMemcpyAsync(c->st_dev, h, sizeof(CgState), cudaMemcpyHostToDevice, c->stream));
     CU(cudaEventRecord(c->ev_t0, c->stream));
-    cg_init_kernel<T><<<cg_grid(c), CG_BLOCK, 0, c->stream>>>((const V2<T>*)b_even, B.hist[m - 1], c->st_dev, c->partials, n, tol);
-    ++c->launches;
+    if (c->slab) {
+        if (!c->has_comm) return fail(c, LQCD_ECOMM, "slab context without a transport (lqcd_comm_init_nccl / lqcd_set_comm)");
+        cg_init_kernel<T, false><<<cg_grid(c), CG_BLOCK, 0, c->stream>>>((const V2<T>*)b_even, B.hist[m - 1], c->st_dev,
+                                                                         c->partials, n, tol);
+        ++c->launches;
+        if ((rc = slab_reduce_step(c, cg_grid(c), 0, tol, 0))) return rc;
+    } else {
+        cg_init_kernel<T><<<cg_grid(c), CG_BLOCK, 0, c->stream>>>((const V2<T>*)b_even, B.hist[m - 1], c->st_dev, c->partials, n, tol);
+        ++c->launches;
+    }
     CU(cudaGetLastError());
 
     const int ce = check_every(c);
     // the legacy default stream cannot be captured: plain launches there
-    const bool use_graph = c->use_graph && c->stream != nullptr && c->stream != cudaStreamLegacy;
+    const bool use_graph = c->use_graph && c->stream != nullptr && c->stream != cudaStreamLegacy &&
+                           (!c->slab || c->comm.graph_safe);
     if (use_graph && (B.graph_iters != ce || B.graph_block != m)) {
         if ((rc = build_graph<T>(c, ce, rational))) return rc;
     }
@@ -757,9 +1106,10 @@ int solve(lqcd_ctx* c, const T* b_even, const double* shifts, int nshift, double
     for (long batch = 0; batch < max_batches && !done; ++batch) {
         if (use_graph) {
             CU(cudaGraphLaunch(B.graph_exec, c->stream));
-            c->launches += 4LL * ce + ce / m;
+            c->launches += B.graph_launches;
         } else {
-            for (int i = 0; i < ce; ++i) launch_cg_iteration<T>(c, i % m);
+            for (int i = 0; i < ce; ++i)
+                if ((rc = launch_cg_iteration<T>(c, i % m))) return rc;
             CU(cudaGetLastError());
         }
         const int slot = (int)(batch & 1);

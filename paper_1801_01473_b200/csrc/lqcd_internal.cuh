@@ -27,6 +27,7 @@ struct Geom {
     int Vh;                         // sites per parity
     int sy, sz, st;                 // strides of y, z, t in k
     int antiperiodic;               // bc_t = -1 on links leaving t = Lt-1
+    int t_off, Lt_glob;             // slab mode: this lattice is time slices [t_off, t_off+Lt) of Lt_glob
 };
 
 #define LQCD_MAX_BLOCK 16           // longest block of iterations whose shift updates are applied in one sweep

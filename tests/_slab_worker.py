@@ -1,0 +1,70 @@
+"""Worker of tests/test_gpu_slab.py: 2 ranks under torch.distributed.run (gloo), both on cuda:0, the slab path with
+the host-staged torch transport.  Rank 0 gathers the slabs and compares with the oracle on the whole lattice."""
+import json
+import os
+import sys
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+sys.path.insert(0, ROOT)
+sys.path.insert(0, os.path.join(ROOT, "tests"))
+
+import numpy as np  # noqa: E402
+import torch  # noqa: E402
+import torch.distributed as dist  # noqa: E402
+
+import paper_1801_01473_b200 as lq  # noqa: E402
+from helpers import make_inputs, oracle_parity_vector, rel_l2  # noqa: E402
+import oracle  # noqa: E402
+
+L = tuple(int(v) for v in sys.argv[1:5])
+dist.init_process_group("gloo", init_method="env://")
+rank, world = dist.get_rank(), dist.get_world_size()
+torch.cuda.set_device(0)
+
+mass, tol, shifts = 0.05, 1e-10, [1e-3, 1e-2, 1e-1, 1.0]
+U, f = make_inputs(L)                                   # every rank draws the same whole-lattice inputs
+b_soa, b_aos = oracle_parity_vector(L, f.numpy(), 0)
+b_glob = torch.as_tensor(b_soa)
+
+lat = lq.Lattice(L, mass=mass, slab=(rank, world), comm="torch")
+lat.set_gauge(lq.Lattice.slab_of_links(U, L, rank, world).cuda())
+b = lq.Lattice.slab_of_vector(b_glob, L, rank, world).cuda()
+with torch.cuda.stream(torch.cuda.Stream()):
+    t = lat.doe(b)
+    u = lat.deo(t)
+    a = lat.mdagm(b, 0.3)
+    x, info = lat.mshift_cg(b, shifts, tol)
+torch.cuda.synchronize()
+assert lat.transport.error is None, lat.transport.error
+
+
+def gather(v):
+    """local parity vector (3, Vh_loc, 2) -> whole-lattice parity vector on rank 0"""
+    v = v.cpu().contiguous()
+    parts = [torch.empty_like(v) for _ in range(world)] if rank == 0 else None
+    dist.gather(v, parts, dst=0)
+    return torch.cat(parts, dim=1).numpy() if rank == 0 else None
+
+
+tg, ug, ag = gather(t), gather(u), gather(a)
+xg = [gather(x[i]) for i in range(len(shifts))]
+stats = [None] * world
+dist.all_gather_object(stats, (info["iters"], info["freeze_iter"], info["rel_res"]))
+if rank == 0:
+    Un = U.numpy()
+    t_ref = oracle.doe(L, Un, b_aos)
+    u_ref = oracle.deo(L, Un, t_ref)
+    a_ref = oracle.mdagm(L, Un, mass, 0.3, b_aos)
+    x_ref, info_ref = oracle.mshift_cg(L, Un, mass, b_aos, shifts, tol)
+    res = dict(
+        doe=rel_l2(oracle.soa_to_aos(tg), t_ref), deo=rel_l2(oracle.soa_to_aos(ug), u_ref),
+        mdagm=rel_l2(oracle.soa_to_aos(ag), a_ref),
+        x=[rel_l2(oracle.soa_to_aos(xg[i]), x_ref[i]) for i in range(len(shifts))],
+        iters=info["iters"], iters_ref=info_ref["iters"],
+        iters_equal_on_ranks=all(s[0] == stats[0][0] for s in stats),
+        freeze_equal_on_ranks=all(s[1] == stats[0][1] and s[2] == stats[0][2] for s in stats),
+        exchanges=lat.transport.n_exchange, allreduces=lat.transport.n_allreduce)
+    print("RESULT " + json.dumps(res))
+lat.close()
+dist.barrier()
+dist.destroy_process_group()

@@ -1,0 +1,149 @@
+"""NEXT-3: the path on a 1-D slab decomposition along t (Alg. 1), against
+the oracle applied to the WHOLE lattice.
+
+One GPU is all there is here, so:
+  * one rank, ring closed on itself, over the library's own NCCL transport (send/recv to self, all-reduce of one
+    rank, CUDA graph with the NCCL operations captured) and over the host-staged torch transport: exercises the
+    interior/border split, the halo buffers, the link halo and the unfused reductions;
+  * two ranks as two processes that share the GPU, host-staged through gloo (tests/_slab_worker.py): exercises
+    t_off != 0, the antiperiodic sign on the right rank, the ring order of the faces.  No kernel ever waits on
+    another rank: the processes only block on the host.
+"""
+import json
+import os
+import socket
+import subprocess
+import sys
+
+import numpy as np
+import pytest
+import torch
+
+import lqcd_inputs as gen
+import oracle
+import paper_1801_01473_b200 as lq
+from helpers import make_inputs, oracle_parity_vector, rel_l2, soa_gpu_to_aos
+
+pytestmark = pytest.mark.gpu
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+SHIFTS = [1e-3, 1e-2, 1e-1, 1.0]
+
+
+@pytest.mark.parametrize("comm", ["nccl", "torch"])
+@pytest.mark.parametrize("L,recon", [((4, 6, 8, 10), 18), ((8, 4, 6, 2), 18), ((4, 4, 4, 4), 12)])
+def test_one_rank_slab_operators_and_cg(L, recon, comm):
+    U, f = make_inputs(L)
+    b_soa, b_aos = oracle_parity_vector(L, f.numpy(), 0)
+    mass, tol = 0.05, 1e-10
+    lat = lq.Lattice(L, mass=mass, recon=recon, slab=(0, 1), comm=comm)
+    assert lq.lqcd_slab_info(lat.ctx) == (0, 0, 1, 0, L[3])
+    lat.set_gauge(U.cuda())
+    b = torch.as_tensor(b_soa).cuda()
+    with torch.cuda.stream(torch.cuda.Stream()):
+        t = lat.doe(b)
+        u = lat.deo(t)
+        a = lat.mdagm(b, 0.3)
+        x, info = lat.mshift_cg(b, SHIFTS, tol)
+    torch.cuda.synchronize()
+    t_ref = oracle.doe(L, U.numpy(), b_aos)
+    u_ref = oracle.deo(L, U.numpy(), t_ref)
+    a_ref = oracle.mdagm(L, U.numpy(), mass, 0.3, b_aos)
+    assert rel_l2(soa_gpu_to_aos(t), t_ref) <= 1e-12
+    assert rel_l2(soa_gpu_to_aos(u), u_ref) <= 1e-12
+    assert rel_l2(soa_gpu_to_aos(a), a_ref) <= 1e-12
+    x_ref, info_ref = oracle.mshift_cg(L, U.numpy(), mass, b_aos, SHIFTS, tol)
+    assert abs(info["iters"] - info_ref["iters"]) <= 1
+    for i in range(len(SHIFTS)):
+        assert rel_l2(soa_gpu_to_aos(x[i]), x_ref[i]) <= 1e-8
+    if comm == "torch":
+        assert lat.transport.error is None
+        # two exchanges and two reductions per iteration (+ the link halo, 3 operator calls, |b|^2)
+        assert lat.transport.n_exchange >= 2 * info["iters"] + 1 + 4
+        assert lat.transport.n_allreduce >= 2 * info["iters"] + 1
+    lat.close()
+
+
+def test_one_rank_slab_equals_whole_lattice_bitwise():
+    """Same arithmetic per site, whichever launch computes it: the operator on a one-rank slab is bit-identical to
+    the whole-lattice kernel; so are the CG iterates up to the (different, still deterministic) summation order."""
+    L = (8, 8, 8, 8)
+    U, f = make_inputs(L)
+    b_soa, _ = oracle_parity_vector(L, f.numpy(), 0)
+    b = torch.as_tensor(b_soa).cuda()
+    whole = lq.Lattice(L, mass=0.05)
+    whole.set_gauge(U.cuda())
+    slab = lq.Lattice(L, mass=0.05, slab=(0, 1), comm="nccl")
+    slab.set_gauge(U.cuda())
+    with torch.cuda.stream(torch.cuda.Stream()):
+        t0, t1 = whole.doe(b), slab.doe(b)
+        u0, u1 = whole.deo(t0), slab.deo(t1)
+        x0, i0 = whole.mshift_cg(b, SHIFTS, 1e-10)
+        x1, i1 = slab.mshift_cg(b, SHIFTS, 1e-10)
+    torch.cuda.synchronize()
+    assert torch.equal(t0, t1) and torch.equal(u0, u1)
+    assert abs(i0["iters"] - i1["iters"]) <= 1
+    for a, c in zip(x0, x1):
+        assert rel_l2(a.cpu().numpy(), c.cpu().numpy()) <= 1e-9
+    whole.close()
+    slab.close()
+
+
+def test_slab_f32_and_rational():
+    L = (4, 4, 6, 8)
+    U, f = make_inputs(L)
+    b_soa, b_aos = oracle_parity_vector(L, f.numpy(), 0)
+    lat = lq.Lattice(L, mass=0.1, slab=(0, 1), comm="nccl", precisions=lq.LQCD_PREC_F64 | lq.LQCD_PREC_F32)
+    lat.set_gauge(U.cuda())
+    b = torch.as_tensor(b_soa).cuda()
+    alpha = [0.3, -0.2, 0.7, 0.1]
+    with torch.cuda.stream(torch.cuda.Stream()):
+        y = lat.rational_apply(b, 0.5, alpha, SHIFTS, 1e-10)[0]
+        t32 = lat.doe(b.float())
+    torch.cuda.synchronize()
+    y_ref = oracle.rational_apply(L, U.numpy(), 0.1, b_aos, 0.5, alpha, SHIFTS, 1e-10)[0]
+    assert rel_l2(soa_gpu_to_aos(y), y_ref) <= 1e-8
+    Uf = U.float().double()
+    t_ref = oracle.doe(L, Uf.numpy(), oracle.soa_to_aos(b.float().double().cpu().numpy()))
+    assert rel_l2(soa_gpu_to_aos(t32.double()), t_ref) <= 2e-6
+    lat.close()
+
+
+def test_slab_errors():
+    assert not lq.lqcd_create_slab(4, 4, 4, 6, 0, 2)          # 3 time slices per rank: odd
+    assert "even" in lq.lqcd_last_error(None)
+    assert not lq.lqcd_create_slab(4, 4, 4, 8, 2, 2)
+    ctx = lq.lqcd_create_slab(4, 4, 4, 8, 1, 2)
+    assert ctx and lq.lqcd_slab_info(ctx) == (0, 1, 2, 4, 8)
+    U = gen.random_su3_links((4, 4, 4, 4)).cuda()
+    assert lq.lqcd_set_gauge(ctx, U.data_ptr()) == lq.LQCD_ECOMM      # no transport yet
+    th = torch.zeros(4 * 256, dtype=torch.float64, device="cuda")
+    assert lq.lqcd_set_u1_phases(ctx, th.data_ptr()) == lq.LQCD_EINVAL
+    lq.lqcd_destroy(ctx)
+    whole = lq.lqcd_create(4, 4, 4, 4)
+    rc, nid = lq.lqcd_nccl_unique_id()
+    assert rc == 0 and lq.lqcd_comm_init_nccl(whole, nid) == lq.LQCD_EINVAL
+    lq.lqcd_destroy(whole)
+
+
+def _free_port():
+    with socket.socket() as s:
+        s.bind(("127.0.0.1", 0))
+        return s.getsockname()[1]
+
+
+@pytest.mark.parametrize("L", [(4, 6, 4, 8), (4, 4, 4, 4)])
+def test_two_ranks_share_the_gpu_host_staged(L):
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", "2",
+           "--master-addr", "127.0.0.1", "--master-port", str(_free_port()),
+           os.path.join("tests", "_slab_worker.py"), *[str(v) for v in L]]
+    out = subprocess.run(cmd, cwd=ROOT, env=dict(os.environ, OMP_NUM_THREADS="4"), capture_output=True, text=True,
+                         timeout=600)
+    assert out.returncode == 0, out.stdout[-2000:] + out.stderr[-3000:]
+    line = [l for l in out.stdout.splitlines() if l.startswith("RESULT ")]
+    assert len(line) == 1, out.stdout[-2000:]
+    r = json.loads(line[0][7:])
+    assert r["doe"] <= 1e-12 and r["deo"] <= 1e-12 and r["mdagm"] <= 1e-12, r
+    assert abs(r["iters"] - r["iters_ref"]) <= 1 and r["iters_equal_on_ranks"], r
+    assert max(r["x"]) <= 1e-8, r
+    assert r["freeze_equal_on_ranks"], r
