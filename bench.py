@@ -196,12 +196,13 @@ def sum_over_ranks(world, value: float) -> float:
 # ---------------------------------------------------------------------------------------------------
 # our arm
 # ---------------------------------------------------------------------------------------------------
-def time_dslash(lq, L, recon, reps, warm, links=None, field=None):
+def time_dslash(lq, L, recon, reps, warm, links=None, field=None, slab=None):
     """ns/site and GB/s of one parity application: reps x (D_oe: b->t, D_eo: t->u) with fixed b
-    (never fed back: |D| ~ 2.6 on random links would overflow)."""
+    (never fed back: |D| ~ 2.6 on random links would overflow).  slab = (L_global, rank, nranks): the same on a slab
+    context (two face exchanges over NCCL, interior and border launches per application); collective."""
     U = links if links is not None else gen.random_su3_links(L, device="cuda")
     f = field if field is not None else gen.gaussian_field(L, device="cuda")
-    lat = lq.Lattice(L, recon=recon)
+    lat = lq.Lattice(L, recon=recon) if slab is None else lq.Lattice(slab[0], recon=recon, slab=slab[1:], comm="nccl")
     lat.set_gauge(U)
     b = lat.pack(f, 0)
     t = torch.empty_like(b)
@@ -219,7 +220,7 @@ def time_dslash(lq, L, recon, reps, warm, links=None, field=None):
     e1.record()
     torch.cuda.current_stream().synchronize()
     launches = lat.launches - n0
-    ms = e0.elapsed_time(e1) / launches
+    ms = e0.elapsed_time(e1) / (2 * reps)
     lat.close()
     ns_site = ms * 1e6 / lat.Vh
     return {"us_per_application": ms * 1e3, "ns_per_site": ns_site,
@@ -246,10 +247,17 @@ def run_ours(args, world, rank, local):
     peak, peak_src = load_peaks()
     stream = torch.cuda.Stream()
     out = {}
+    slab = args.parallel == "slab"
+    Lg = tuple(L[:3]) + (L[3] * world,)                 # slab mode: weak scaling, the lattice grows along t
     with torch.cuda.stream(stream):
-        U = gen.random_su3_links(L, device="cuda")
-        f = gen.gaussian_field(L, device="cuda")
-        lat = lq.Lattice(L, mass=mass, recon=recon)
+        if slab:
+            U = gen.random_su3_links_slab(Lg, rank, world, device="cuda")
+            f = gen.gaussian_field_slab(Lg, rank, world, device="cuda")
+            lat = lq.Lattice(Lg, mass=mass, recon=recon, slab=(rank, world), comm="nccl")
+        else:
+            U = gen.random_su3_links(L, device="cuda")
+            f = gen.gaussian_field(L, device="cuda")
+            lat = lq.Lattice(L, mass=mass, recon=recon)
         lat.set_gauge(U)
         b = lat.pack(f, 0)
         x = lat.new_vector(len(shifts))
@@ -303,7 +311,7 @@ def run_ours(args, world, rank, local):
         out["e2e"] = dict(ms_total=e2e_ms, h2d=b_host.numel() * 8, d2h=x_host.numel() * 8)
         del b_host, x_host
 
-        if rank == 0 and not args.quick:
+        if (rank == 0 or slab) and not args.quick:
             # ---- the same solve to convergence (what a user runs): average s/iter, iteration count
             lat.set_option(lq.LQCD_OPT_MAX_ITER, 100000)
             _, full = lat.mshift_cg(b, shifts, tol, x=x, raise_on_noconv=False)
@@ -328,6 +336,8 @@ def run_ours(args, world, rank, local):
             if not args.quick:
                 other = 12 if recon == 18 else 18
                 ds[name][f"recon{other}"] = time_dslash(lq, L, other, reps, 5, U, f)
+        if slab:
+            out["dslash_slab"] = time_dslash(lq, L, recon, reps, 5, U, f, slab=(Lg, rank, world))
         del U, f
         if rank == 0 and not args.quick and args.workload == "config4_48^4":
             L3 = gen.CONFIGS["config3_32^4"]["L"]
@@ -384,6 +394,10 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="config4_48^4", choices=sorted(gen.CONFIGS))
     ap.add_argument("--recon", type=int, default=18, choices=[18, 12])
+    ap.add_argument("--parallel", default="replicas", choices=["replicas", "slab"],
+                    help="N > 1: independent replicas (default; north_star: no sharding) or ONE lattice of N times "
+                         "the time extent cut into N slabs (NEXT-3; faces over NCCL, all-reduced scalar products). "
+                         "With N = 1, slab runs the slab code path on one rank (ring closed on itself).")
     ap.add_argument("--quick", action="store_true", help="skip the full solve, the 32^4 table and the CPU baseline")
     ap.add_argument("--cpu-budget", type=float, default=20.0, help="seconds of oracle time for cpu_baseline")
     args = ap.parse_args()
@@ -401,7 +415,10 @@ def main():
               "step": "one multi-shift CG iteration (D_oe, D_eo+epilogue, scalar recurrences, r update, base x/p update, "
                       "1/m of the block sweep over the shifted x_i/p_i)",
               "lattice": list(cfg["L"]), "nshift": len(cfg["shifts"]), "mass": cfg["mass"], "tol": cfg["tol"],
-              "recon": args.recon, "parallelism": "replicas only" if world > 1 else "single GPU",
+              "recon": args.recon,
+              "parallelism": (f"1-D slabs along t: ONE {lname[:lname.rfind('x')]}x{cfg['L'][3] * world} lattice over {world} "
+                              f"rank(s), value = s/iter of that solve / {world}") if args.parallel == "slab"
+              else ("replicas only" if world > 1 else "single GPU"),
               "l2": "inputs larger than L2 (links 3.06 GB vs 126 MB); no flush needed"}
 
     if args.impl == "reference":
@@ -456,6 +473,8 @@ def main():
     }
     if "full_solve" in res:
         line["full_solve"] = res["full_solve"]
+    if "dslash_slab" in res:
+        line["dslash_slab"] = res["dslash_slab"]
     if not args.quick and world == 1:
         s_iter, cores, sample, _ = run_oracle(args.workload, budget_s=args.cpu_budget, steps=None)
         line["cpu_baseline"] = {"value": s_iter, "unit": "s/iter", "cores": cores, "kind": "oracle", "sample": sample}

@@ -143,6 +143,36 @@ def random_su3_links(L: Sequence[int], seed: int = SEED_LINKS, device="cpu",
     return out
 
 
+def slab_sites(L: Sequence[int], rank: int, nranks: int) -> tuple[int, int]:
+    """(first lexicographic site, number of sites) of the slab of time slices rank r of nranks owns (the slab
+    decomposition cuts the slowest index t into nranks equal parts)."""
+    V = volume(L)
+    assert L[3] % nranks == 0
+    return rank * (V // nranks), V // nranks
+
+
+def random_su3_links_slab(L: Sequence[int], rank: int, nranks: int, seed: int = SEED_LINKS, device="cpu",
+                          chunk: int = 1 << 20) -> torch.Tensor:
+    """The part of ``random_su3_links(L)`` that leaves the sites of one slab, (4, V/nranks, 3, 3, 2), drawn
+    directly (same counters, hence the same values) so that no rank ever holds the whole field."""
+    V = volume(L)
+    first_site, n = slab_sites(L, rank, nranks)
+    out = torch.empty((4, n, 3, 3, 2), dtype=torch.float64, device=device)
+    for mu in range(4):
+        for a in range(0, n, chunk):
+            count = min(chunk, n - a)
+            u = _random_su3(seed, _STREAM_LINKS, mu * V + first_site + a, count, out.device)
+            out[mu, a:a + count] = torch.view_as_real(u)
+    return out
+
+
+def gaussian_field_slab(L: Sequence[int], rank: int, nranks: int, seed: int = SEED_SOURCE, device="cpu") -> torch.Tensor:
+    """The part of ``gaussian_field(L)`` on the sites of one slab, (V/nranks, 3, 2)."""
+    first_site, n = slab_sites(L, rank, nranks)
+    ctr = torch.arange(3 * first_site, 3 * (first_site + n), dtype=torch.int64, device=device)
+    return torch.view_as_real(complex_gaussian(seed, _STREAM_FIELD, ctr)).reshape(n, 3, 2).contiguous()
+
+
 def unit_links(L: Sequence[int], device="cpu") -> torch.Tensor:
     """Free field: every link is the identity."""
     V = volume(L)
