@@ -46,8 +46,8 @@ DSLASH_FLOPS = {18: 570, 12: 570 + 8 * 42}
 # DRAM bytes per launch of dslash_kernel<18,0> measured by `ncu --set full` (dram__bytes_read.sum +
 # dram__bytes_write.sum), keyed by workload; source file under profiles/.  None until captured.
 NCU_DRAM_BYTES_PER_LAUNCH = {
-    ("config4_48^4", 18): 3.190935e9 + 0.102704e9,     # profiles/ncu_full_r01.md, dslash_kernel<18,0>
-    ("config4_48^4", 12): 2.171263e9 + 0.100277e9,     # profiles/ncu_full_r01.md, dslash_kernel<12,0>
+    ("config4_48^4", 18): 3.190834e9 + 0.103419e9,     # profiles/ncu_full_r01.md, dslash_kernel<double,18,0>
+    ("config4_48^4", 12): 2.171204e9 + 0.101689e9,     # profiles/ncu_full_r01.md, dslash_kernel<double,12,0>
 }
 
 
@@ -325,6 +325,20 @@ def run_ours(args, world, rank, local):
                                      gbs_moved=moved_f / (full["solve_ms"] * 1e6),
                                      freeze_iter=full["freeze_iter"])
         lat.close()
+
+        if rank == 0 and not args.quick and not slab:
+            # ---- the same K iterations with the other link format (BASELINE config 3 compares the two; the paper
+            # always runs with two-row links)
+            other = 12 if recon == 18 else 18
+            lat2 = lq.Lattice(L, mass=mass, recon=other)
+            lat2.set_gauge(U)
+            lat2.set_option(lq.LQCD_OPT_MAX_ITER, max(W, 3))
+            lat2.mshift_cg(b, shifts, tol, x=x, raise_on_noconv=False)
+            lat2.set_option(lq.LQCD_OPT_MAX_ITER, K)
+            _, info2 = lat2.mshift_cg(b, shifts, tol, x=x, raise_on_noconv=False)
+            out[f"cg_recon{other}"] = dict(s_per_iter=info2["solve_ms"] * 1e-3 / max(info2["iters"], 1), iters=info2["iters"],
+                                           note=f"same {K} iterations with {other}-real links, device time of the solve")
+            lat2.close()
         del x
 
         # ---- the dominant kernel alone: D_oe / D_eo at the workload size, live CUDA events
@@ -475,6 +489,9 @@ def main():
         line["full_solve"] = res["full_solve"]
     if "dslash_slab" in res:
         line["dslash_slab"] = res["dslash_slab"]
+    for key in ("cg_recon12", "cg_recon18"):
+        if key in res:
+            line[key] = res[key]
     if not args.quick and world == 1:
         s_iter, cores, sample, _ = run_oracle(args.workload, budget_s=args.cpu_budget, steps=None)
         line["cpu_baseline"] = {"value": s_iter, "unit": "s/iter", "cores": cores, "kind": "oracle", "sample": sample}
