@@ -230,6 +230,66 @@ def time_dslash(lq, L, recon, reps, warm, links=None, field=None, slab=None):
             "bytes_per_launch": DSLASH_BYTES[recon] * lat.Vh}
 
 
+def time_next_rows(lq, L, mass, shifts, tol, K, W, U, f):
+    """The widened rows on the same workload, K iterations / applications each, device time:
+    NEXT-1 rational sum, NEXT-2 single precision (Dslash and CG), NEXT-4 general U(1) phases (Dslash)."""
+    res = {}
+    ev = lambda: torch.cuda.Event(enable_timing=True)
+
+    def dslash_ns(lat, b, reps=max(K // 2, 20)):
+        t, u = torch.empty_like(b), torch.empty_like(b)
+        for _ in range(5):
+            lat.doe(b, out=t)
+            lat.deo(t, out=u)
+        e0, e1 = ev(), ev()
+        torch.cuda.current_stream().synchronize()
+        e0.record()
+        for _ in range(reps):
+            lat.doe(b, out=t)
+            lat.deo(t, out=u)
+        e1.record()
+        torch.cuda.current_stream().synchronize()
+        return e0.elapsed_time(e1) * 1e6 / (2 * reps) / lat.Vh
+
+    def cg_s_per_iter(lat, solve):
+        lat.set_option(lq.LQCD_OPT_MAX_ITER, max(W, 3))
+        solve()
+        lat.set_option(lq.LQCD_OPT_MAX_ITER, K)
+        info = solve()
+        return info["solve_ms"] * 1e-3 / max(info["iters"], 1), info["iters"]
+
+    # NEXT-1 and NEXT-4 on a double-precision context
+    lat = lq.Lattice(L, mass=mass)
+    lat.set_gauge(U)
+    b = lat.pack(f, 0)
+    alpha = [1.0 / (1 + i) for i in range(len(shifts))]
+    y = torch.empty_like(b)
+    s_it, n = cg_s_per_iter(lat, lambda: lat.rational_apply(b, 0.5, alpha, shifts, tol, y=y, raise_on_noconv=False)[1])
+    res["next1_rational_apply"] = {"s_per_iter": s_it, "iters": n,
+                                   "note": "y = alpha0 b + sum_i alpha_i x_i accumulated in the solve, x_i never stored"}
+    theta = gen.random_u1_phases(L, device="cuda")
+    lat.set_u1_phases(theta)
+    ns = dslash_ns(lat, b)
+    res["next4_u1_dslash"] = {"ns_per_site": ns, "gbs_algorithmic": (DSLASH_BYTES[18] + 64) / ns,
+                              "gbs_dram_model": (DSLASH_DRAM_MODEL[18] + 64) / ns,
+                              "note": "18-real links + theta_mu(x) (8 B/link), sincos in the kernel"}
+    lat.close()
+    del theta, y
+    # NEXT-2: single precision
+    lat = lq.Lattice(L, mass=mass, precisions=lq.LQCD_PREC_F32)
+    lat.set_gauge(U)
+    b32 = b.float()
+    ns = dslash_ns(lat, b32)
+    res["next2_f32_dslash"] = {"ns_per_site": ns, "gbs_algorithmic": DSLASH_BYTES[18] / 2 / ns,
+                               "gbs_dram_model": DSLASH_DRAM_MODEL[18] / 2 / ns}
+    x32 = lat.new_vector(len(shifts), dtype=torch.float32)
+    s_it, n = cg_s_per_iter(lat, lambda: lat.mshift_cg(b32, shifts, tol, x=x32, raise_on_noconv=False)[1])
+    res["next2_f32_mshift_cg"] = {"s_per_iter": s_it, "iters": n,
+                                  "note": "float links, vectors and sweeps; scalar products and recurrences in double"}
+    lat.close()
+    return res
+
+
 def n_active_schedule(freeze_iter, iters):
     """number of shifts updated in iteration j = 1..iters (shift i is updated while j <= freeze_iter[i])"""
     return [sum(1 for fz in freeze_iter if j <= fz) for j in range(1, iters + 1)]
@@ -352,6 +412,8 @@ def run_ours(args, world, rank, local):
                 ds[name][f"recon{other}"] = time_dslash(lq, L, other, reps, 5, U, f)
         if slab:
             out["dslash_slab"] = time_dslash(lq, L, recon, reps, 5, U, f, slab=(Lg, rank, world))
+        if rank == 0 and not args.quick and not slab:
+            out["next_rows"] = time_next_rows(lq, L, mass, shifts, tol, K, W, U, f)
         del U, f
         if rank == 0 and not args.quick and args.workload == "config4_48^4":
             L3 = gen.CONFIGS["config3_32^4"]["L"]
@@ -489,7 +551,7 @@ def main():
         line["full_solve"] = res["full_solve"]
     if "dslash_slab" in res:
         line["dslash_slab"] = res["dslash_slab"]
-    for key in ("cg_recon12", "cg_recon18"):
+    for key in ("cg_recon12", "cg_recon18", "next_rows"):
         if key in res:
             line[key] = res[key]
     if not args.quick and world == 1:
