@@ -205,7 +205,8 @@ int lqcd_rational_apply_f32(lqcd_ctx* ctx, const float* b_even, double alpha0, c
  * Lx*Ly*Lz*(Lt/nranks) lattice), vectors are parity vectors of the local lattice, lqcd_mshift_cg solves the global
  * system (its statistics are identical on every rank).  Every rank must make the same sequence of calls with the
  * same options, shifts and tol.  The antiperiodic boundary sits on the links that leave the last time slice of the
- * whole lattice.  Not available on a slab context: lqcd_set_u1_phases (LQCD_EINVAL).
+ * whole lattice.  lqcd_set_u1_phases takes the angles of the slab's own links (4 * V_local) and, like lqcd_set_gauge,
+ * needs the transport (the t-links below the slab, and their angles, come from rank-1 once).
  *
  * A transport must be set before lqcd_set_gauge (which exchanges the t-links of the face once):
  *   lqcd_comm_init_nccl   NCCL send/recv + all-reduce on the GPU (NVLink 5 / NVSwitch between the GPUs of a node),

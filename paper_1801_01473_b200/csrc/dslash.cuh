@@ -210,27 +210,29 @@ __device__ __forceinline__ void hop_bwd(T (&ar)[3], T (&ai)[3], const V2<T>* __r
 }
 
 // the same two hops with separate element strides for the link and the vector (slab faces: halo buffers)
-template <typename T, int RECON>
+template <typename T, int RECON, int U1>
 __device__ __forceinline__ void hop_fwd_s(T (&ar)[3], T (&ai)[3], const V2<T>* __restrict__ w, const size_t ws,
                                           const V2<T>* __restrict__ v, const size_t vs, unsigned int mask,
-                                          uint64_t pol_s, uint64_t pol_r) {
+                                          uint64_t pol_s, uint64_t pol_r, const T* __restrict__ th) {
     V2<T> u[9];
     T vr[3], vi[3];
     load_link<T, RECON>(w, ws, pol_s, u);
     load_vec<T>(v, vs, pol_r, mask, vr, vi);
+    if (U1) u1_rotate<T, +1>(th, pol_s, vr, vi);
 #pragma unroll
     for (int a = 0; a < 3; ++a)
 #pragma unroll
         for (int b = 0; b < 3; ++b) cmad<T>(ar[a], ai[a], u[3 * a + b], vr[b], vi[b]);
 }
-template <typename T, int RECON>
+template <typename T, int RECON, int U1>
 __device__ __forceinline__ void hop_bwd_s(T (&ar)[3], T (&ai)[3], const V2<T>* __restrict__ w, const size_t ws,
                                           const V2<T>* __restrict__ v, const size_t vs, unsigned int mask,
-                                          uint64_t pol_s, uint64_t pol_r) {
+                                          uint64_t pol_s, uint64_t pol_r, const T* __restrict__ th) {
     V2<T> u[9];
     T vr[3], vi[3];
     load_link<T, RECON>(w, ws, pol_s, u);
     load_vec<T>(v, vs, pol_r, mask, vr, vi);
+    if (U1) u1_rotate<T, -1>(th, pol_s, vr, vi);
 #pragma unroll
     for (int a = 0; a < 3; ++a)
 #pragma unroll
@@ -254,6 +256,7 @@ struct DslashArgs {
     const V2<T>* in_lo;      // halo: time slice t_off-1 of `in`, [c][face]
     const V2<T>* in_hi;      // halo: time slice t_off+Lt of `in`, [c][face]
     const V2<T>* Wt_lo;      // halo: t-links leaving slice t_off-1, [parity of origin][e][face]
+    const T* Th_lo;          // halo (U1): their U(1) angles, [parity of origin][face]
     int k0a, na, k0b, nsites;    // thread idx < na: site k0a+idx; else site k0b+(idx-na); nsites in all
     int part_off;            // EPI == 3: first slot of this launch in `partials`
 };
@@ -356,10 +359,11 @@ __global__ void __launch_bounds__(DS_BLOCK, DsOcc<T>::minb) dslash_kernel(const 
         const int kf = k - t * g.st;                                  // index inside a time slice
         const bool top = (t == g.Lt - 1), bot = (t == 0);
         const V2<T>* vf = top ? A.in_hi + kf : in + k + g.st;
-        hop_fwd_s<T, RECON>(ar, ai, Wf + 3 * mu_stride, vh, vf, top ? face : vh, mtf, pol_s, pol_r);
+        hop_fwd_s<T, RECON, U1>(ar, ai, Wf + 3 * mu_stride, vh, vf, top ? face : vh, mtf, pol_s, pol_r, Tf + 3 * th_stride);
         const V2<T>* vb = bot ? A.in_lo + kf : in + k - g.st;
         const V2<T>* wb = bot ? A.Wt_lo + (size_t)(1 - A.par) * NE * face + kf : Wb + 3 * mu_stride + k - g.st;
-        hop_bwd_s<T, RECON>(ar, ai, wb, bot ? face : vh, vb, bot ? face : vh, mtb ^ SB, pol_s, pol_r);
+        const T* tb = U1 ? (bot ? A.Th_lo + (size_t)(1 - A.par) * face + kf : Tb + 3 * th_stride + k - g.st) : nullptr;
+        hop_bwd_s<T, RECON, U1>(ar, ai, wb, bot ? face : vh, vb, bot ? face : vh, mtb ^ SB, pol_s, pol_r, tb);
     }
 
     if (EPI == 0) {

@@ -49,6 +49,8 @@ struct PrecBufs {
     V2<T>* halo_recv = nullptr;
     V2<T>* Wt_lo = nullptr;                  // [parity of origin][e][face]
     V2<T>* Wt_send = nullptr;                // one-time staging of my top t-links (+ a dummy receive buffer behind it)
+    T* Th_lo = nullptr;                      // U(1) angles of those links, [parity of origin][face]
+    T* Th_send = nullptr;
     V2<T>* stage_b = nullptr;                // host-call staging (device copies of host arguments)
     V2<T>* stage_x[LQCD_MAX_SHIFTS] = {};
     int n_stage_x = 0;
@@ -317,13 +319,18 @@ int ensure_halo(lqcd_ctx* c) {
     return LQCD_OK;
 }
 
+template <typename T, int EPI, int U1>
+void launch_dslash_slab_u(lqcd_ctx* c, const DslashArgs<T>& a, int grid) {
+    if (bufs<T>(c).recon_stored == 12)
+        dslash_kernel<T, 12, EPI, U1, 1><<<grid, DS_BLOCK, 0, c->stream>>>(a);
+    else
+        dslash_kernel<T, 18, EPI, U1, 1><<<grid, DS_BLOCK, 0, c->stream>>>(a);
+    ++c->launches;
+}
 template <typename T, int EPI>
 void launch_dslash_slab_k(lqcd_ctx* c, const DslashArgs<T>& a, int grid) {
-    if (bufs<T>(c).recon_stored == 12)
-        dslash_kernel<T, 12, EPI, 0, 1><<<grid, DS_BLOCK, 0, c->stream>>>(a);
-    else
-        dslash_kernel<T, 18, EPI, 0, 1><<<grid, DS_BLOCK, 0, c->stream>>>(a);
-    ++c->launches;
+    if (c->u1_on) launch_dslash_slab_u<T, EPI, 1>(c, a, grid);
+    else launch_dslash_slab_u<T, EPI, 0>(c, a, grid);
 }
 
 // One operator application on a slab (Alg. 1 of the paper): the two faces of `in` are packed
@@ -350,7 +357,8 @@ int slab_dslash(lqcd_ctx* c, int epi, V2<T>* out, const V2<T>* in, int par, cons
     DslashArgs<T> a{};
     a.g = c->g;
     a.W = B.W;
-    a.Th = nullptr;
+    a.Th = B.Th;
+    a.Th_lo = B.Th_lo;
     a.in = in;
     a.out = out;
     a.par = par;
@@ -597,6 +605,21 @@ int store_theta(lqcd_ctx* c, const double* theta) {
     repack_theta_kernel<T><<<(int)((nthreads + 255) / 256), 256, 0, c->stream>>>(c->g, theta, B.Th);
     ++c->launches;
     CU(cudaGetLastError());
+    if (c->slab) {
+        // the angles of the t-links that leave the slice below the slab (cf. the link halo in store_gauge)
+        const size_t face = face_sites(c), vh = c->Vh;
+        if (!B.Th_lo) {
+            if ((rc = dev_alloc(c, (void**)&B.Th_lo, 2 * face * sizeof(T)))) return rc;
+            if ((rc = dev_alloc(c, (void**)&B.Th_send, 4 * face * sizeof(T)))) return rc;
+        }
+        // rows (3*2 + parity) of Th, last time slice
+        CU(cudaMemcpy2DAsync(B.Th_send, face * sizeof(T), B.Th + (size_t)6 * vh + (vh - face), vh * sizeof(T),
+                             face * sizeof(T), 2, cudaMemcpyDeviceToDevice, c->stream));
+        CU(cudaEventRecord(c->ev_pack, c->stream));
+        CU(cudaStreamWaitEvent(c->comm_stream, c->ev_pack, 0));
+        if ((rc = comm_exchange(c, B.Th_send, B.Th_send, B.Th_lo, B.Th_send + 2 * face, 2 * face * sizeof(T)))) return rc;
+        CU(cudaStreamSynchronize(c->comm_stream));
+    }
     B.u1_stored = 1;
     return LQCD_OK;
 }
@@ -921,7 +944,8 @@ int lqcd_set_gauge(lqcd_ctx* c, const double* links) {
 
 int lqcd_set_u1_phases(lqcd_ctx* c, const double* theta) {
     if (!c) return LQCD_EINVAL;
-    if (c->slab && theta) return fail(c, LQCD_EINVAL, "general U(1) phases are not available on a slab context");
+    if (c->slab && theta && !c->has_comm)
+        return fail(c, LQCD_ECOMM, "slab context: set a transport before lqcd_set_u1_phases");
     int rc;
     if ((rc = ensure_basics(c))) return rc;
     drop_graphs(c);           // the kernel variant and its arguments are baked into the graph

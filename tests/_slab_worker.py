@@ -14,19 +14,21 @@ import torch.distributed as dist  # noqa: E402
 
 import paper_1801_01473_b200 as lq  # noqa: E402
 from helpers import make_inputs, oracle_parity_vector, rel_l2  # noqa: E402
+import lqcd_inputs as gen  # noqa: E402
 import oracle  # noqa: E402
 
 L = tuple(int(v) for v in sys.argv[1:5])
+COMM = sys.argv[5] if len(sys.argv) > 5 else "torch"      # "torch": host-staged, ranks share cuda:0; "nccl": one GPU each
 dist.init_process_group("gloo", init_method="env://")
 rank, world = dist.get_rank(), dist.get_world_size()
-torch.cuda.set_device(0)
+torch.cuda.set_device(int(os.environ.get("LOCAL_RANK", "0")) if COMM == "nccl" else 0)
 
 mass, tol, shifts = 0.05, 1e-10, [1e-3, 1e-2, 1e-1, 1.0]
 U, f = make_inputs(L)                                   # every rank draws the same whole-lattice inputs
 b_soa, b_aos = oracle_parity_vector(L, f.numpy(), 0)
 b_glob = torch.as_tensor(b_soa)
 
-lat = lq.Lattice(L, mass=mass, slab=(rank, world), comm="torch")
+lat = lq.Lattice(L, mass=mass, slab=(rank, world), comm=COMM)
 lat.set_gauge(lq.Lattice.slab_of_links(U, L, rank, world).cuda())
 b = lq.Lattice.slab_of_vector(b_glob, L, rank, world).cuda()
 with torch.cuda.stream(torch.cuda.Stream()):
@@ -34,8 +36,14 @@ with torch.cuda.stream(torch.cuda.Stream()):
     u = lat.deo(t)
     a = lat.mdagm(b, 0.3)
     x, info = lat.mshift_cg(b, shifts, tol)
+    # the same operator with general U(1) phases (the angles of the t-links below the slab come from rank-1)
+    theta = gen.random_u1_phases(L)
+    a0, a1 = lq.Lattice.slab_range(L, rank, world)
+    lat.set_u1_phases(theta[:, a0:a1].contiguous().cuda())
+    tu = lat.doe(b)
+    uu = lat.deo(tu)
 torch.cuda.synchronize()
-assert lat.transport.error is None, lat.transport.error
+assert lat.transport is None or lat.transport.error is None, lat.transport.error
 
 
 def gather(v):
@@ -47,6 +55,7 @@ def gather(v):
 
 
 tg, ug, ag = gather(t), gather(u), gather(a)
+tug, uug = gather(tu), gather(uu)
 xg = [gather(x[i]) for i in range(len(shifts))]
 stats = [None] * world
 dist.all_gather_object(stats, (info["iters"], info["freeze_iter"], info["rel_res"]))
@@ -56,14 +65,17 @@ if rank == 0:
     u_ref = oracle.deo(L, Un, t_ref)
     a_ref = oracle.mdagm(L, Un, mass, 0.3, b_aos)
     x_ref, info_ref = oracle.mshift_cg(L, Un, mass, b_aos, shifts, tol)
+    tu_ref = oracle.doe(L, Un, b_aos, theta=theta.numpy())
+    uu_ref = oracle.deo(L, Un, tu_ref, theta=theta.numpy())
     res = dict(
         doe=rel_l2(oracle.soa_to_aos(tg), t_ref), deo=rel_l2(oracle.soa_to_aos(ug), u_ref),
+        doe_u1=rel_l2(oracle.soa_to_aos(tug), tu_ref), deo_u1=rel_l2(oracle.soa_to_aos(uug), uu_ref),
         mdagm=rel_l2(oracle.soa_to_aos(ag), a_ref),
         x=[rel_l2(oracle.soa_to_aos(xg[i]), x_ref[i]) for i in range(len(shifts))],
         iters=info["iters"], iters_ref=info_ref["iters"],
         iters_equal_on_ranks=all(s[0] == stats[0][0] for s in stats),
         freeze_equal_on_ranks=all(s[1] == stats[0][1] and s[2] == stats[0][2] for s in stats),
-        exchanges=lat.transport.n_exchange, allreduces=lat.transport.n_allreduce)
+        exchanges=lat.transport.n_exchange if lat.transport else None)
     print("RESULT " + json.dumps(res))
 lat.close()
 dist.barrier()

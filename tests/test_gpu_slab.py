@@ -109,6 +109,29 @@ def test_slab_f32_and_rational():
     lat.close()
 
 
+def test_slab_with_u1_phases():
+    L = (4, 6, 4, 6)
+    U, f = make_inputs(L)
+    theta = gen.random_u1_phases(L)
+    b_soa, b_aos = oracle_parity_vector(L, f.numpy(), 0)
+    lat = lq.Lattice(L, mass=0.1, slab=(0, 1), comm="nccl")
+    lat.set_gauge(U.cuda())
+    lat.set_u1_phases(theta.cuda())
+    b = torch.as_tensor(b_soa).cuda()
+    with torch.cuda.stream(torch.cuda.Stream()):
+        t = lat.doe(b)
+        u = lat.deo(t)
+        x, info = lat.mshift_cg(b, SHIFTS, 1e-10)
+    torch.cuda.synchronize()
+    t_ref = oracle.doe(L, U.numpy(), b_aos, theta=theta.numpy())
+    u_ref = oracle.deo(L, U.numpy(), t_ref, theta=theta.numpy())
+    assert rel_l2(soa_gpu_to_aos(t), t_ref) <= 1e-12 and rel_l2(soa_gpu_to_aos(u), u_ref) <= 1e-12
+    x_ref, info_ref = oracle.mshift_cg(L, U.numpy(), 0.1, b_aos, SHIFTS, 1e-10, theta=theta.numpy())
+    assert abs(info["iters"] - info_ref["iters"]) <= 1
+    assert max(rel_l2(soa_gpu_to_aos(x[i]), x_ref[i]) for i in range(len(SHIFTS))) <= 1e-8
+    lat.close()
+
+
 def test_slab_errors():
     assert not lq.lqcd_create_slab(4, 4, 4, 6, 0, 2)          # 3 time slices per rank: odd
     assert "even" in lq.lqcd_last_error(None)
@@ -118,7 +141,7 @@ def test_slab_errors():
     U = gen.random_su3_links((4, 4, 4, 4)).cuda()
     assert lq.lqcd_set_gauge(ctx, U.data_ptr()) == lq.LQCD_ECOMM      # no transport yet
     th = torch.zeros(4 * 256, dtype=torch.float64, device="cuda")
-    assert lq.lqcd_set_u1_phases(ctx, th.data_ptr()) == lq.LQCD_EINVAL
+    assert lq.lqcd_set_u1_phases(ctx, th.data_ptr()) == lq.LQCD_ECOMM
     lq.lqcd_destroy(ctx)
     whole = lq.lqcd_create(4, 4, 4, 4)
     rc, nid = lq.lqcd_nccl_unique_id()
@@ -132,11 +155,10 @@ def _free_port():
         return s.getsockname()[1]
 
 
-@pytest.mark.parametrize("L", [(4, 6, 4, 8), (4, 4, 4, 4)])
-def test_two_ranks_share_the_gpu_host_staged(L):
-    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", "2",
+def _run_ranks(world, L, comm):
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", str(world),
            "--master-addr", "127.0.0.1", "--master-port", str(_free_port()),
-           os.path.join("tests", "_slab_worker.py"), *[str(v) for v in L]]
+           os.path.join("tests", "_slab_worker.py"), *[str(v) for v in L], comm]
     out = subprocess.run(cmd, cwd=ROOT, env=dict(os.environ, OMP_NUM_THREADS="4"), capture_output=True, text=True,
                          timeout=600)
     assert out.returncode == 0, out.stdout[-2000:] + out.stderr[-3000:]
@@ -144,6 +166,20 @@ def test_two_ranks_share_the_gpu_host_staged(L):
     assert len(line) == 1, out.stdout[-2000:]
     r = json.loads(line[0][7:])
     assert r["doe"] <= 1e-12 and r["deo"] <= 1e-12 and r["mdagm"] <= 1e-12, r
+    assert r["doe_u1"] <= 1e-12 and r["deo_u1"] <= 1e-12, r
     assert abs(r["iters"] - r["iters_ref"]) <= 1 and r["iters_equal_on_ranks"], r
     assert max(r["x"]) <= 1e-8, r
     assert r["freeze_equal_on_ranks"], r
+
+
+@pytest.mark.parametrize("L", [(4, 6, 4, 8), (4, 4, 4, 4)])
+def test_two_ranks_share_the_gpu_host_staged(L):
+    _run_ranks(2, L, "torch")
+
+
+@pytest.mark.parametrize("world,L", [(2, (8, 8, 8, 8)), (4, (4, 6, 8, 16))])
+def test_ranks_on_their_own_gpus_over_nccl(world, L):
+    """The production transport between GPUs: needs `world` devices, skipped on a one-GPU box."""
+    if torch.cuda.device_count() < world:
+        pytest.skip(f"needs {world} GPUs")
+    _run_ranks(world, L, "nccl")
