@@ -230,6 +230,24 @@ def time_dslash(lq, L, recon, reps, warm, links=None, field=None, slab=None):
             "bytes_per_launch": DSLASH_BYTES[recon] * lat.Vh}
 
 
+def read_only_reference_gbs():
+    """Context for the roofline: what a plain read-only stream reaches on this GPU (torch.sum over 4 GiB of doubles,
+    best of 10, CUDA events).  The measured peak of MEASURED_PEAKS.json is a COPY (half writes); the Dslash is 97 %
+    reads."""
+    a = torch.ones(1 << 29, dtype=torch.float64, device="cuda")
+    best = 0.0
+    for i in range(13):
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        a.sum()
+        e1.record()
+        torch.cuda.current_stream().synchronize()
+        if i >= 3:
+            best = max(best, a.numel() * 8 / (e0.elapsed_time(e1) * 1e6))
+    del a
+    return best
+
+
 def time_next_rows(lq, L, mass, shifts, tol, K, W, U, f):
     """The widened rows on the same workload, K iterations / applications each, device time:
     NEXT-1 rational sum, NEXT-2 single precision (Dslash and CG), NEXT-4 general U(1) phases (Dslash)."""
@@ -414,6 +432,7 @@ def run_ours(args, world, rank, local):
             out["dslash_slab"] = time_dslash(lq, L, recon, reps, 5, U, f, slab=(Lg, rank, world))
         if rank == 0 and not args.quick and not slab:
             out["next_rows"] = time_next_rows(lq, L, mass, shifts, tol, K, W, U, f)
+            out["read_only_gbs"] = read_only_reference_gbs()
         del U, f
         if rank == 0 and not args.quick and args.workload == "config4_48^4":
             L3 = gen.CONFIGS["config3_32^4"]["L"]
@@ -537,6 +556,7 @@ def main():
                      "ns_per_site": ds_main["ns_per_site"],
                      "achieved_dram_model": ds_main["gbs_dram_model"], "frac_dram_model": ds_main["gbs_dram_model"] / peak,
                      "frac_of_nominal_8000": achieved / 8000.0,
+                     "read_only_reference_gbs": res.get("read_only_gbs"),
                      "note": "achieved = algorithmic bytes (8 links + 8 neighbour vectors + 1 output per site) / event "
                              "time; the 8 neighbour-vector reads are mostly L2 hits, achieved_dram_model counts each "
                              "input vector once (what DRAM must deliver)"},
