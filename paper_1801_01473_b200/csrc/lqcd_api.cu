@@ -320,17 +320,17 @@ int ensure_halo(lqcd_ctx* c) {
 }
 
 template <typename T, int EPI, int U1>
-void launch_dslash_slab_u(lqcd_ctx* c, const DslashArgs<T>& a, int grid) {
+void launch_dslash_slab_u(lqcd_ctx* c, const DslashArgs<T>& a, int grid, cudaStream_t stream) {
     if (bufs<T>(c).recon_stored == 12)
-        dslash_kernel<T, 12, EPI, U1, 1><<<grid, DS_BLOCK, 0, c->stream>>>(a);
+        dslash_kernel<T, 12, EPI, U1, 1><<<grid, DS_BLOCK, 0, stream>>>(a);
     else
-        dslash_kernel<T, 18, EPI, U1, 1><<<grid, DS_BLOCK, 0, c->stream>>>(a);
+        dslash_kernel<T, 18, EPI, U1, 1><<<grid, DS_BLOCK, 0, stream>>>(a);
     ++c->launches;
 }
 template <typename T, int EPI>
-void launch_dslash_slab_k(lqcd_ctx* c, const DslashArgs<T>& a, int grid) {
-    if (c->u1_on) launch_dslash_slab_u<T, EPI, 1>(c, a, grid);
-    else launch_dslash_slab_u<T, EPI, 0>(c, a, grid);
+void launch_dslash_slab_k(lqcd_ctx* c, const DslashArgs<T>& a, int grid, cudaStream_t stream) {
+    if (c->u1_on) launch_dslash_slab_u<T, EPI, 1>(c, a, grid, stream);
+    else launch_dslash_slab_u<T, EPI, 0>(c, a, grid, stream);
 }
 
 // One operator application on a slab (Alg. 1 of the paper): the two faces of `in` are packed
@@ -349,10 +349,13 @@ int slab_dslash(lqcd_ctx* c, int epi, V2<T>* out, const V2<T>* in, int par, cons
     V2<T>* send_hi = B.halo_send + 3 * face;
     V2<T>* recv_lo = B.halo_recv;
     V2<T>* recv_hi = B.halo_recv + 3 * face;
-    // a face is three contiguous runs (one per colour) of the vector: strided copies, no kernel
-    CU(cudaMemcpy2DAsync(send_lo, row, in, pitch, row, 3, cudaMemcpyDeviceToDevice, c->stream));
-    CU(cudaMemcpy2DAsync(send_hi, row, in + (vh - face), pitch, row, 3, cudaMemcpyDeviceToDevice, c->stream));
+    // `in` is complete at this point of the compute stream; everything about the faces happens on the
+    // communication stream from here on, beside the interior launch
     CU(cudaEventRecord(c->ev_pack, c->stream));
+    CU(cudaStreamWaitEvent(c->comm_stream, c->ev_pack, 0));
+    // a face is three contiguous runs (one per colour) of the vector: strided copies, no kernel
+    CU(cudaMemcpy2DAsync(send_lo, row, in, pitch, row, 3, cudaMemcpyDeviceToDevice, c->comm_stream));
+    CU(cudaMemcpy2DAsync(send_hi, row, in + (vh - face), pitch, row, 3, cudaMemcpyDeviceToDevice, c->comm_stream));
 
     DslashArgs<T> a{};
     a.g = c->g;
@@ -372,11 +375,11 @@ int slab_dslash(lqcd_ctx* c, int epi, V2<T>* out, const V2<T>* in, int par, cons
     a.Wt_lo = B.Wt_lo;
     const int kepi = (epi == 1) ? 3 : epi;
     int part = 0;
-    auto launch = [&](int grid) {
+    auto launch = [&](int grid, cudaStream_t stream) {
         a.part_off = part;
-        if (kepi == 0) launch_dslash_slab_k<T, 0>(c, a, grid);
-        else if (kepi == 2) launch_dslash_slab_k<T, 2>(c, a, grid);
-        else launch_dslash_slab_k<T, 3>(c, a, grid);
+        if (kepi == 0) launch_dslash_slab_k<T, 0>(c, a, grid, stream);
+        else if (kepi == 2) launch_dslash_slab_k<T, 2>(c, a, grid, stream);
+        else launch_dslash_slab_k<T, 3>(c, a, grid, stream);
         part += grid;
     };
     // interior: t = 1 .. Lt-2
@@ -386,19 +389,18 @@ int slab_dslash(lqcd_ctx* c, int epi, V2<T>* out, const V2<T>* in, int par, cons
         a.na = n_int;
         a.k0b = 0;
         a.nsites = n_int;
-        launch((n_int + DS_BLOCK - 1) / DS_BLOCK);
+        launch((n_int + DS_BLOCK - 1) / DS_BLOCK, c->stream);
     }
-    // faces in flight on the communication stream
-    CU(cudaStreamWaitEvent(c->comm_stream, c->ev_pack, 0));
+    // faces in flight on the communication stream; the two border slices (t = 0 and t = Lt-1) follow them on
+    // that stream, so they run beside the interior (disjoint outputs and partial slots) instead of after it
     if ((rc = comm_exchange(c, send_lo, send_hi, recv_lo, recv_hi, 3 * row))) return rc;
-    CU(cudaEventRecord(c->ev_halo, c->comm_stream));
-    CU(cudaStreamWaitEvent(c->stream, c->ev_halo, 0));
-    // borders: t = 0 and t = Lt-1
     a.k0a = 0;
     a.na = (int)face;
     a.k0b = (int)(vh - face);
     a.nsites = (int)(2 * face);
-    launch((a.nsites + DS_BLOCK - 1) / DS_BLOCK);
+    launch((a.nsites + DS_BLOCK - 1) / DS_BLOCK, c->comm_stream);
+    CU(cudaEventRecord(c->ev_halo, c->comm_stream));
+    CU(cudaStreamWaitEvent(c->stream, c->ev_halo, 0));
     CU(cudaGetLastError());
     if (n_part) *n_part = part;
     return LQCD_OK;
