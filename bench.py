@@ -493,9 +493,21 @@ def main():
                     help="N > 1: independent replicas (default; north_star: no sharding) or ONE lattice of N times "
                          "the time extent cut into N slabs (NEXT-3; faces over NCCL, all-reduced scalar products). "
                          "With N = 1, slab runs the slab code path on one rank (ring closed on itself).")
+    ap.add_argument("--next-rows-only", action="store_true",
+                    help="run only the widened rows (rational sum, f32, U(1) phases) and print their JSON object "
+                         "(used for the ncu captures of those kernels)")
     ap.add_argument("--quick", action="store_true", help="skip the full solve, the 32^4 table and the CPU baseline")
     ap.add_argument("--cpu-budget", type=float, default=20.0, help="seconds of oracle time for cpu_baseline")
     args = ap.parse_args()
+    if args.next_rows_only:
+        import paper_1801_01473_b200 as lq
+        cfg = gen.CONFIGS[args.workload]
+        with torch.cuda.stream(torch.cuda.Stream()):
+            U = gen.random_su3_links(cfg["L"], device="cuda")
+            f = gen.gaussian_field(cfg["L"], device="cuda")
+            res = time_next_rows(lq, cfg["L"], cfg["mass"], cfg["shifts"], cfg["tol"], args.steps, args.warmup, U, f)
+        print(json.dumps({"next_rows": res}))
+        return 0
     if args.impl == "reference" and int(os.environ.get("RANK", "0")) != 0:
         return 0                                   # the oracle arm runs on rank 0 alone, no process group
     if args.impl == "reference":
