@@ -305,6 +305,23 @@ def time_next_rows(lq, L, mass, shifts, tol, K, W, U, f):
     res["next2_f32_mshift_cg"] = {"s_per_iter": s_it, "iters": n,
                                   "note": "float links, vectors and sweeps; scalar products and recurrences in double"}
     lat.close()
+    # NEXT-2, mixed precision: full solves to tol on the true residual, against the double-precision solver
+    lat = lq.Lattice(L, mass=mass, precisions=lq.LQCD_PREC_F64 | lq.LQCD_PREC_F32)
+    lat.set_gauge(U)
+    lat.set_option(lq.LQCD_OPT_MAX_ITER, 100000)
+    mixed = {}
+    for name, sh in (("one_system", shifts[:1]), ("all_systems", shifts)):
+        xm = lat.new_vector(len(sh))
+        _, im = lat.mshift_cg_mixed(b, sh, tol, x=xm, raise_on_noconv=False)
+        _, idb = lat.mshift_cg(b, sh, tol, x=xm, raise_on_noconv=False)
+        mixed[name] = {"nshift": len(sh), "mixed_s": im["solve_ms"] * 1e-3, "mixed_float_iters": im["iters"],
+                       "reliable_updates": im["reliable_updates"], "mixed_true_rel_res": im["rel_res"],
+                       "double_s": idb["solve_ms"] * 1e-3, "double_iters": idb["iters"]}
+        del xm
+    mixed["note"] = ("lqcd_mshift_cg_mixed (float CG + double reliable updates; with several systems a float "
+                     "multi-shift phase, then each system finished alone) against lqcd_mshift_cg, solves to convergence")
+    res["next2_mixed"] = mixed
+    lat.close()
     return res
 
 

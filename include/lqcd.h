@@ -96,6 +96,7 @@ typedef struct lqcd_ctx lqcd_ctx;
 #define LQCD_STAT_BASE_SHIFT     3  /* index of the shift used as base system (the smallest)              */
 #define LQCD_STAT_GPU_LAUNCHES   4  /* kernels launched by this context since creation                    */
 #define LQCD_STAT_SOLVE_MS       5  /* device time of the last solve between CUDA events, milliseconds     */
+#define LQCD_STAT_RELIABLE_UPDATES 6 /* lqcd_mshift_cg_mixed: double-precision residual replacements performed */
 
 /* Create a context for an Lx*Ly*Lz*Lt lattice on the current CUDA device.  NULL on error
  * (extent odd or < 2, volume too large, no device). */
@@ -172,6 +173,23 @@ int lqcd_mshift_cg_f32(lqcd_ctx* ctx, const float* b_even, const double* shifts 
                        double tol, float* const* x /*HOST array of DEVICE pointers*/);
 int lqcd_mshift_cg_f32_host(lqcd_ctx* ctx, const float* b_even /*HOST*/, const double* shifts /*HOST*/,
                             int nshift, double tol, float* const* x /*HOST array of HOST pointers*/);
+
+/* Mixed precision: the systems of lqcd_mshift_cg solved to a DOUBLE-precision tolerance with the iterations in
+ * single precision (the paper keeps its fields "double (or float)", and mixes the two at the level of
+ * the algorithm; here they are mixed inside one solve).  A float CG iterates on a recurrence residual;
+ * whenever that has dropped by a factor 10 since the last time, the float partial solution is added to the double
+ * one and the residual is REPLACED by the true residual b - (m^2 - D_eo D_oe + sigma) x computed with the double
+ * operator, the search direction being kept ("reliable updates").  The stopping rule is on that true residual:
+ * |b - (A + shifts[i]) x[i]| <= tol |b| for every i.  With nshift > 1 a float multi-shift solve first brings all
+ * systems to a relative residual ~1e-5, then each system is finished on its own: the shifted systems cannot share
+ * residual replacements (they would lose r_i = zeta_i r), so with many light shifts and a tight tol this costs MORE
+ * than lqcd_mshift_cg; with one or few systems it is up to ~2x faster.
+ * Needs both link copies (LQCD_OPT_LINK_PRECISIONS = LQCD_PREC_F64 | LQCD_PREC_F32 at lqcd_set_gauge time), else
+ * LQCD_ENOGAUGE.  Arguments as lqcd_mshift_cg.  Statistics: LQCD_STAT_ITERS = float iterations in all phases,
+ * LQCD_STAT_FREEZE_ITER[i] = float iterations spent finishing system i, LQCD_STAT_REL_RES = the largest final true
+ * relative residual, LQCD_STAT_RELIABLE_UPDATES.  Not available on a slab context (LQCD_EINVAL). */
+int lqcd_mshift_cg_mixed(lqcd_ctx* ctx, const double* b_even, const double* shifts /*HOST*/, int nshift,
+                         double tol, double* const* x /*HOST array of DEVICE pointers*/);
 
 /* Rational function of the Eq. 2 operator applied to b,
  *     y = alpha0 b + sum_i alpha[i] (m^2 - D_eo D_oe + shifts[i])^{-1} b ,

@@ -15,7 +15,7 @@ LQCD_OPT_MASS, LQCD_OPT_ANTIPERIODIC_T, LQCD_OPT_RECON, LQCD_OPT_MAX_ITER = 0, 1
 LQCD_OPT_CHECK_EVERY, LQCD_OPT_USE_GRAPH, LQCD_OPT_LINK_PRECISIONS, LQCD_OPT_SHIFT_BLOCK = 4, 5, 6, 7
 LQCD_PREC_F64, LQCD_PREC_F32 = 1, 2
 LQCD_STAT_ITERS, LQCD_STAT_REL_RES, LQCD_STAT_FREEZE_ITER, LQCD_STAT_BASE_SHIFT = 0, 1, 2, 3
-LQCD_STAT_GPU_LAUNCHES, LQCD_STAT_SOLVE_MS = 4, 5
+LQCD_STAT_GPU_LAUNCHES, LQCD_STAT_SOLVE_MS, LQCD_STAT_RELIABLE_UPDATES = 4, 5, 6
 
 _ERRNAMES = {0: "LQCD_OK", -1: "LQCD_EINVAL", -2: "LQCD_ENOGAUGE", -3: "LQCD_ENOMEM", -4: "LQCD_ECUDA",
              -5: "LQCD_ENOCONV", -6: "LQCD_EBREAKDOWN", -7: "LQCD_ENOTSU3", -8: "LQCD_ECOMM"}
@@ -54,6 +54,7 @@ EXPORTS = {
     "lqcd_mdagm": (_i, [_vp, _dp, _dp, _d]),
     "lqcd_mshift_cg": (_i, [_vp, _dp, _pd, _i, _d, ctypes.POINTER(ctypes.c_void_p)]),
     "lqcd_mshift_cg_host": (_i, [_vp, _dp, _pd, _i, _d, ctypes.POINTER(ctypes.c_void_p)]),
+    "lqcd_mshift_cg_mixed": (_i, [_vp, _dp, _pd, _i, _d, ctypes.POINTER(ctypes.c_void_p)]),
     "lqcd_rational_apply": (_i, [_vp, _dp, _d, _pd, _pd, _i, _d, _dp]),
     "lqcd_rational_apply_host": (_i, [_vp, _dp, _d, _pd, _pd, _i, _d, _dp]),
     "lqcd_doe_f32": (_i, [_vp, _dp, _dp]),
@@ -211,6 +212,11 @@ def lqcd_mshift_cg(ctx, b_even, shifts: Sequence[float], tol: float, x_ptrs: Seq
 def lqcd_mshift_cg_host(ctx, b_even, shifts: Sequence[float], tol: float, x_ptrs: Sequence[int]):
     n, sh, xs = _cg_args(shifts, x_ptrs)
     return load_library().lqcd_mshift_cg_host(ctx, b_even, sh, n, float(tol), xs)
+
+
+def lqcd_mshift_cg_mixed(ctx, b_even, shifts: Sequence[float], tol: float, x_ptrs: Sequence[int]):
+    n, sh, xs = _cg_args(shifts, x_ptrs)
+    return load_library().lqcd_mshift_cg_mixed(ctx, b_even, sh, n, float(tol), xs)
 
 
 def lqcd_mshift_cg_f32(ctx, b_even, shifts: Sequence[float], tol: float, x_ptrs: Sequence[int]):
@@ -581,6 +587,22 @@ class Lattice:
         rc = fn(self.ctx, pb, shifts, tol, ptrs)
         self._check(rc, allow=() if raise_on_noconv else (LQCD_ENOCONV,))
         return x, self._solve_info(rc, n)
+
+    def mshift_cg_mixed(self, b_even, shifts: Sequence[float], tol: float, x=None, raise_on_noconv: bool = True):
+        """The same systems to a double-precision tolerance on the TRUE residual, iterating in single precision with
+        double-precision reliable updates (include/lqcd.h: lqcd_mshift_cg_mixed).  float64 CUDA tensors."""
+        torch = self._torch
+        n = len(shifts)
+        pb = self._t(b_even, (3, self.Vh, 2), "cuda")
+        if x is None:
+            x = torch.empty((n, 3, self.Vh, 2), dtype=torch.float64, device="cuda")
+        self._t(x, (n, 3, self.Vh, 2), "cuda")
+        self._sync_stream()
+        rc = lqcd_mshift_cg_mixed(self.ctx, pb, shifts, tol, [x[i].data_ptr() for i in range(n)])
+        self._check(rc, allow=() if raise_on_noconv else (LQCD_ENOCONV,))
+        info = self._solve_info(rc, n)
+        info["reliable_updates"] = int(self.stat(LQCD_STAT_RELIABLE_UPDATES))
+        return x, info
 
     def _solve_info(self, rc, n):
         return dict(

@@ -321,6 +321,71 @@ __global__ void __launch_bounds__(CG_BLOCK, (MM <= 8 ? 2 : 1)) cg_flush_kernel(C
     }
 }
 
+// ---- mixed precision: single-precision CG with double-precision reliable updates -------------------------------
+// ("fp32 inner, fp64 reliable updates"; the paper keeps its fields in either precision,
+// PAPER.md:L147, and runs MD in single, Metropolis in double.)
+// The float CG iterates on a recurrence residual r and accumulates its solution in a float vector y.  At a
+// reliable update the accumulated y is added to the double-precision solution x (and cleared), the TRUE residual
+// b - (A + sigma) x is computed with the double-precision operator, and replaces r; the search direction is kept
+// (p += r_true - r_recurrence, i.e. p = r_true + beta p_old), so the Krylov sequence is not restarted.
+
+// x64 += y32 ; y32 = 0
+__global__ void __launch_bounds__(CG_BLOCK) mixed_accumulate_kernel(double2* __restrict__ x, float2* __restrict__ y, size_t n) {
+    for (size_t j = (size_t)blockIdx.x * CG_BLOCK + threadIdx.x; j < n; j += (size_t)gridDim.x * CG_BLOCK) {
+        const float2 v = y[j];
+        double2 xv = x[j];
+        xv.x += (double)v.x;
+        xv.y += (double)v.y;
+        x[j] = xv;
+        y[j] = make_float2(0.f, 0.f);
+    }
+}
+
+// r_true = b - ax (double; ax == NULL: r_true = b);  |r_true|^2 -> st->rr and *rr_out;  r_out = float(r_true);
+// if p != NULL: p += float(r_true) - r_rec  (r_rec = the recurrence residual being replaced).
+// resume != 0: the float solver had stopped on its recurrence residual and is started again.
+__global__ void __launch_bounds__(CG_BLOCK) mixed_residual_kernel(const double2* __restrict__ b, const double2* __restrict__ ax,
+                                                                  const float2* r_rec, float2* r_out, float2* __restrict__ p,
+                                                                  CgState* st, double* partials, double* rr_out, size_t n,
+                                                                  int resume) {
+    __shared__ double red[32];
+    __shared__ int last_flag;
+    double acc = 0.0;
+    for (size_t j = (size_t)blockIdx.x * CG_BLOCK + threadIdx.x; j < n; j += (size_t)gridDim.x * CG_BLOCK) {
+        double2 r = b[j];
+        if (ax) {
+            const double2 a = ax[j];
+            r.x -= a.x;
+            r.y -= a.y;
+        }
+        acc = fma(r.x, r.x, acc);
+        acc = fma(r.y, r.y, acc);
+        const float2 rf = make_float2((float)r.x, (float)r.y);
+        if (p) {
+            const float2 old = r_rec[j];
+            float2 pv = p[j];
+            pv.x += rf.x - old.x;
+            pv.y += rf.y - old.y;
+            p[j] = pv;
+        }
+        r_out[j] = rf;
+    }
+    const double bsum = block_sum<CG_BLOCK>(acc, red);
+    if (publish_partial<CG_BLOCK>(bsum, partials, &st->ticket[4], &last_flag)) {
+        const double rr = final_sum<CG_BLOCK>(partials, gridDim.x, red);
+        if (threadIdx.x == 0) {
+            st->ticket[4] = 0;
+            *rr_out = rr;
+            if (p) st->rr = rr;
+            if (resume) {
+                st->stop = 0;
+                st->stop4 = 0;
+                st->active[st->i0] = 1;
+            }
+        }
+    }
+}
+
 // ---- layout kernels (step A1 and the pack/unpack convenience calls) -------------------------------
 
 __device__ __forceinline__ size_t lex_of(const Geom& g, int k, int par) {

@@ -97,7 +97,7 @@ struct lqcd_ctx {
     CgState* st_host;        // pinned
     int* flag_host;          // pinned, 2 ints
     double* max_host;        // pinned
-    cudaEvent_t ev[2], ev_t0, ev_t1;
+    cudaEvent_t ev[2], ev_t0, ev_t1, ev_m0, ev_m1;
     bool basics;
 
     // statistics
@@ -105,6 +105,7 @@ struct lqcd_ctx {
     double last_rel;
     int last_freeze[LQCD_MAX_SHIFTS];
     float last_ms;
+    int last_updates;        // reliable updates of the last mixed-precision solve
     long long launches;
 
     char err[256];
@@ -212,6 +213,8 @@ int ensure_basics(lqcd_ctx* c) {
     CU(cudaEventCreateWithFlags(&c->ev[1], cudaEventDisableTiming));
     CU(cudaEventCreate(&c->ev_t0));
     CU(cudaEventCreate(&c->ev_t1));
+    CU(cudaEventCreate(&c->ev_m0));
+    CU(cudaEventCreate(&c->ev_m1));
     c->basics = true;
     return LQCD_OK;
 }
@@ -729,6 +732,8 @@ void lqcd_destroy(lqcd_ctx* c) {
         cudaEventDestroy(c->ev[1]);
         cudaEventDestroy(c->ev_t0);
         cudaEventDestroy(c->ev_t1);
+        cudaEventDestroy(c->ev_m0);
+        cudaEventDestroy(c->ev_m1);
     }
     cudaGetLastError();
     delete c;
@@ -1188,6 +1193,197 @@ int solve_host(lqcd_ctx* c, const T* b_even, const double* shifts, int nshift, d
     return status;
 }
 
+// ---- mixed precision (NEXT-2): float CG with double-precision reliable updates ---------------------------------
+// One system (A + sigma) x = b, A = m^2 - D_eo D_oe, to the tolerance tol on the TRUE residual computed in double.
+// x holds the initial guess on entry when have_guess (it is then improved), else it is overwritten.
+// The float iterations run as the ordinary single-shift solver (same kernels, same CUDA graph); between batches of
+// CHECK_EVERY iterations the host looks at the recurrence residual and triggers a reliable update (cg.cuh) when it
+// has dropped by RELIABLE_DELTA since the last one, or when the float solver has stopped.
+constexpr double RELIABLE_DELTA = 0.1;
+constexpr double MIXED_TOL_F32 = 1e-5;     // relative recurrence residual asked of the float multi-shift phase
+
+int mixed_solve_one(lqcd_ctx* c, const double* b, double sigma, double tol, double* x, bool have_guess, double bb,
+                    int* iters_out, int* updates_out, double* rel_out) {
+    int rc;
+    PrecBufs<float>& F = bufs<float>(c);
+    PrecBufs<double>& D = bufs<double>(c);
+    const size_t n = c->Vh * 3;
+    const int m = c->shift_block;
+    const double2* b2 = (const double2*)b;
+    double2* x2 = (double2*)x;
+    double2* ax = D.stage_x[0];           // (A + sigma) x
+    float2* r0 = F.stage_b;               // float copy of the starting residual
+    float2* y = F.stage_x[0];             // float partial solution since the last reliable update
+
+    // device state of a single-shift float solve; the starting vector is the (true) starting residual
+    CgState* h = c->st_host;
+    memset(h, 0, sizeof(CgState));
+    h->nshift = 1;
+    h->i0 = 0;
+    h->max_iter = c->max_iter;
+    h->c0 = c->mass * c->mass + sigma;
+    h->x[0] = (void*)y;
+    h->p[0] = (void*)F.p;
+    h->blk_m = m;
+    for (int l = 0; l < m; ++l) h->hist[l] = (void*)F.hist[l];
+    CU(cudaMemcpyAsync(c->st_dev, h, sizeof(CgState), cudaMemcpyHostToDevice, c->stream));
+
+    if (have_guess) {
+        if ((rc = apply_mdagm<double>(c, (double*)ax, x, sigma))) return rc;
+    } else {
+        CU(cudaMemsetAsync(x, 0, n * sizeof(double2), c->stream));
+    }
+    mixed_residual_kernel<<<cg_grid(c), CG_BLOCK, 0, c->stream>>>(b2, have_guess ? ax : nullptr, nullptr, r0, nullptr, c->st_dev,
+                                                                c->partials, c->red, n, 0);
+    ++c->launches;
+    CU(cudaMemcpyAsync(c->red_host, c->red, sizeof(double), cudaMemcpyDeviceToHost, c->stream));
+    CU(cudaStreamSynchronize(c->stream));
+    double rr_true = c->red_host[0];
+    const double target = tol * tol * bb;
+    *iters_out = 0;
+    *updates_out = 0;
+    *rel_out = std::sqrt(rr_true / bb);
+    if (rr_true <= target) return LQCD_OK;
+
+    // tol of the float solver is relative to ITS source (the starting residual): same absolute target
+    cg_init_kernel<float><<<cg_grid(c), CG_BLOCK, 0, c->stream>>>(r0, F.hist[m - 1], c->st_dev, c->partials, n,
+                                                                 tol * std::sqrt(bb / rr_true));
+    ++c->launches;
+    CU(cudaGetLastError());
+
+    const int ce = check_every(c);
+    const bool use_graph = c->use_graph && c->stream != nullptr && c->stream != cudaStreamLegacy;
+    if (use_graph && (F.graph_iters != ce || F.graph_block != m)) {
+        if ((rc = build_graph<float>(c, ce, 0))) return rc;
+    }
+    double maxrr = rr_true;
+    const long max_batches = (long)c->max_iter / ce + 3;
+    for (long batch = 0; batch < max_batches; ++batch) {
+        if (use_graph) {
+            CU(cudaGraphLaunch(F.graph_exec, c->stream));
+            c->launches += F.graph_launches;
+        } else {
+            for (int i = 0; i < ce; ++i)
+                if ((rc = launch_cg_iteration<float>(c, i % m))) return rc;
+            CU(cudaGetLastError());
+        }
+        // the head of the state: rr, ..., iter, stop, status
+        CU(cudaMemcpyAsync(h, c->st_dev, offsetof(CgState, ticket), cudaMemcpyDeviceToHost, c->stream));
+        CU(cudaStreamSynchronize(c->stream));
+        if (h->status == LQCD_EBREAKDOWN) return fail(c, LQCD_EBREAKDOWN, "<p,Ap> = %g at iteration %d", h->pAp, h->iter);
+        if (h->rr > maxrr) maxrr = h->rr;
+        if (!h->stop && !(h->rr < RELIABLE_DELTA * RELIABLE_DELTA * maxrr)) continue;
+
+        // reliable update: x += y, y = 0, r <- b - (A + sigma) x in double, p keeps its direction
+        mixed_accumulate_kernel<<<cg_grid(c), CG_BLOCK, 0, c->stream>>>(x2, y, n);
+        ++c->launches;
+        if ((rc = apply_mdagm<double>(c, (double*)ax, x, sigma))) return rc;
+        const int cur = (h->iter + m - 1) % m;          // ring slot of the current recurrence residual
+        const int resume = (h->stop && h->status == 0) ? 1 : 0;
+        mixed_residual_kernel<<<cg_grid(c), CG_BLOCK, 0, c->stream>>>(b2, ax, F.hist[cur], F.hist[m - 1], F.p, c->st_dev,
+                                                                    c->partials, c->red, n, resume);
+        ++c->launches;
+        CU(cudaMemcpyAsync(c->red_host, c->red, sizeof(double), cudaMemcpyDeviceToHost, c->stream));
+        CU(cudaStreamSynchronize(c->stream));
+        rr_true = c->red_host[0];
+        maxrr = rr_true;
+        ++*updates_out;
+        *iters_out = h->iter;
+        *rel_out = std::sqrt(rr_true / bb);
+        if (rr_true <= target) return LQCD_OK;
+        if (h->stop && h->status == LQCD_ENOCONV)
+            return fail(c, LQCD_ENOCONV, "no convergence in %d iterations, |r|/|b| = %.3e", h->iter, *rel_out);
+    }
+    return fail(c, LQCD_ENOCONV, "no convergence within the iteration cap, |r|/|b| = %.3e", *rel_out);
+}
+
+// Multi-shift front end: one float multi-shift solve brings every system to a loose tolerance, then each system is
+// refined on its own (the shifted systems cannot share reliable updates: replacing r breaks r_i = zeta_i r).
+int solve_mixed(lqcd_ctx* c, const double* b_even, const double* shifts, int nshift, double tol, double* const* x) {
+    if (!c) return LQCD_EINVAL;
+    if (!b_even || !shifts || !x) return fail(c, LQCD_EINVAL, "NULL argument");
+    if (nshift < 1 || nshift > LQCD_MAX_SHIFTS) return fail(c, LQCD_EINVAL, "nshift must be in [1, %d]", LQCD_MAX_SHIFTS);
+    if (!(tol > 0.0) || !std::isfinite(tol)) return fail(c, LQCD_EINVAL, "tol must be positive");
+    for (int i = 0; i < nshift; ++i) {
+        if (!(shifts[i] >= 0.0) || !std::isfinite(shifts[i])) return fail(c, LQCD_EINVAL, "shift %d must be >= 0", i);
+        if (!x[i] || (const double*)x[i] == b_even) return fail(c, LQCD_EINVAL, "x[%d] is NULL or aliases b", i);
+        for (int j = 0; j < i; ++j)
+            if (x[j] == x[i]) return fail(c, LQCD_EINVAL, "x[%d] aliases x[%d]", i, j);
+    }
+    if (c->slab) return fail(c, LQCD_EINVAL, "the mixed-precision solver is not available on a slab context");
+    int rc;
+    if ((rc = check_ctx_gauge<double>(c)) || (rc = check_ctx_gauge<float>(c))) return rc;
+    if ((rc = ensure_solver<float>(c, nshift)) || (rc = ensure_tmp<double>(c))) return rc;
+    if ((rc = ensure_stage<float>(c, nshift)) || (rc = ensure_stage<double>(c, 1))) return rc;
+    if (!c->red) {
+        if ((rc = dev_alloc(c, (void**)&c->red, 2 * sizeof(double)))) return rc;
+        CU(cudaMallocHost((void**)&c->red_host, 2 * sizeof(double)));
+    }
+    PrecBufs<float>& F = bufs<float>(c);
+    PrecBufs<double>& D = bufs<double>(c);
+    const size_t n = c->Vh * 3;
+    const int cgrid = cg_grid(c);
+    cudaEvent_t t0 = c->ev_m0, t1 = c->ev_m1;
+    CU(cudaEventRecord(t0, c->stream));
+
+    // |b|^2 in double (the residual kernel with nothing subtracted), and the float copy of b
+    CU(cudaMemsetAsync(c->st_dev, 0, sizeof(CgState), c->stream));
+    mixed_residual_kernel<<<cgrid, CG_BLOCK, 0, c->stream>>>((const double2*)b_even, nullptr, nullptr, F.stage_b, nullptr,
+                                                           c->st_dev, c->partials, c->red, n, 0);
+    ++c->launches;
+    CU(cudaMemcpyAsync(c->red_host, c->red, sizeof(double), cudaMemcpyDeviceToHost, c->stream));
+    CU(cudaStreamSynchronize(c->stream));
+    const double bb = c->red_host[0];
+    int total_iters = 0, total_updates = 0;
+    double worst = 0.0;
+    c->last_nshift = nshift;
+    if (bb == 0.0) {
+        for (int i = 0; i < nshift; ++i) CU(cudaMemsetAsync(x[i], 0, n * sizeof(double2), c->stream));
+        for (int i = 0; i < nshift; ++i) c->last_freeze[i] = 0;
+    } else {
+        bool guess = false;
+        if (nshift > 1) {
+            // phase 1: every system at once in single precision, to what single precision can deliver
+            const double tol1 = tol > MIXED_TOL_F32 ? tol : MIXED_TOL_F32;
+            float* xf[LQCD_MAX_SHIFTS];
+            for (int i = 0; i < nshift; ++i) xf[i] = (float*)F.stage_x[i];
+            rc = solve<float>(c, (const float*)F.stage_b, shifts, nshift, tol1, xf, nullptr, 0.0, nullptr);
+            if (rc != LQCD_OK && rc != LQCD_ENOCONV) return rc;
+            total_iters += c->last_iters;
+            for (int i = 0; i < nshift; ++i) {
+                convert_vector_kernel<double, float><<<cgrid, 256, 0, c->stream>>>(F.stage_x[i], (double2*)x[i], n);
+                ++c->launches;
+            }
+            guess = true;
+        }
+        // phase 2: each system to the double-precision tolerance
+        for (int i = 0; i < nshift; ++i) {
+            int it = 0, up = 0;
+            double rel = 0.0;
+            rc = mixed_solve_one(c, b_even, shifts[i], tol, x[i], guess, bb, &it, &up, &rel);
+            total_iters += it;
+            total_updates += up;
+            c->last_freeze[i] = it;
+            if (rel > worst) worst = rel;
+            if (rc != LQCD_OK) {
+                c->last_iters = total_iters;
+                c->last_rel = worst;
+                c->last_updates = total_updates;
+                return rc;
+            }
+        }
+    }
+    CU(cudaEventRecord(t1, c->stream));
+    CU(cudaStreamSynchronize(c->stream));
+    CU(cudaEventElapsedTime(&c->last_ms, t0, t1));
+    c->last_iters = total_iters;
+    c->last_rel = worst;
+    c->last_updates = total_updates;
+    c->last_i0 = 0;
+    (void)D;
+    return LQCD_OK;
+}
+
 template <typename T>
 int pack_unpack(lqcd_ctx* c, int parity, const T* in, T* out, bool pack) {
     if (!c) return LQCD_EINVAL;
@@ -1239,6 +1435,10 @@ int lqcd_mshift_cg_f32_host(lqcd_ctx* c, const float* b_even, const double* shif
     return solve_host<float>(c, b_even, shifts, nshift, tol, x, nullptr, 0.0, nullptr);
 }
 
+int lqcd_mshift_cg_mixed(lqcd_ctx* c, const double* b_even, const double* shifts, int nshift, double tol, double* const* x) {
+    return solve_mixed(c, b_even, shifts, nshift, tol, x);
+}
+
 int lqcd_rational_apply(lqcd_ctx* c, const double* b_even, double alpha0, const double* alpha, const double* shifts,
                         int nshift, double tol, double* y_even) {
     if (c && (!y_even || !alpha)) return fail(c, LQCD_EINVAL, "NULL argument");
@@ -1267,6 +1467,7 @@ int lqcd_get_stat(const lqcd_ctx* c, int key, int idx, double* out) {
         case LQCD_STAT_BASE_SHIFT: *out = c->last_i0; break;
         case LQCD_STAT_GPU_LAUNCHES: *out = (double)c->launches; break;
         case LQCD_STAT_SOLVE_MS: *out = c->last_ms; break;
+        case LQCD_STAT_RELIABLE_UPDATES: *out = c->last_updates; break;
         default: return LQCD_EINVAL;
     }
     return LQCD_OK;
