@@ -72,6 +72,15 @@ def cg_bytes_moved(freeze_iter, iters: int, m: int, recon: int) -> int:
     return total
 
 
+_T0 = time.perf_counter()
+
+
+def phase(name: str):
+    """wall-clock phase marks on stderr (BENCH_TIMING=1), to keep the default run within a few minutes"""
+    if os.environ.get("BENCH_TIMING"):
+        print(f"[bench {time.perf_counter() - _T0:7.1f} s] {name}", file=sys.stderr, flush=True)
+
+
 def load_peaks():
     path = os.path.join(ROOT, "MEASURED_PEAKS.json")
     if os.path.exists(path):
@@ -357,6 +366,7 @@ def run_ours(args, world, rank, local):
         b = lat.pack(f, 0)
         x = lat.new_vector(len(shifts))
 
+        phase('inputs drawn, gauge stored')
         # ---- warm-up: W iterations (also builds the CUDA graph)
         lat.set_option(lq.LQCD_OPT_MAX_ITER, max(W, 3))
         lat.mshift_cg(b, shifts, tol, x=x, raise_on_noconv=False)
@@ -385,6 +395,7 @@ def run_ours(args, world, rank, local):
                             gbs_algorithmic=bytes_total / (ms_total * 1e6),
                             gbs_moved=bytes_moved / (ms_total * 1e6), kernel_ms=info["solve_ms"])
 
+        phase('timed region done')
         # ---- e2e: same K iterations through the host-pointer entry point (rank-local, then max)
         b_host = torch.empty(b.shape, dtype=torch.float64, pin_memory=True)
         b_host.copy_(b)
@@ -406,6 +417,7 @@ def run_ours(args, world, rank, local):
         out["e2e"] = dict(ms_total=e2e_ms, h2d=b_host.numel() * 8, d2h=x_host.numel() * 8)
         del b_host, x_host
 
+        phase('e2e done')
         if (rank == 0 or slab) and not args.quick:
             # ---- the same solve to convergence (what a user runs): average s/iter, iteration count
             lat.set_option(lq.LQCD_OPT_MAX_ITER, 100000)
@@ -436,6 +448,7 @@ def run_ours(args, world, rank, local):
             lat2.close()
         del x
 
+        phase('full solve / other link format done')
         # ---- the dominant kernel alone: D_oe / D_eo at the workload size, live CUDA events
         reps = max(K // 2, 20)
         ds = {}
@@ -447,10 +460,12 @@ def run_ours(args, world, rank, local):
                 ds[name][f"recon{other}"] = time_dslash(lq, L, other, reps, 5, U, f)
         if slab:
             out["dslash_slab"] = time_dslash(lq, L, recon, reps, 5, U, f, slab=(Lg, rank, world))
+        phase('dslash at workload size done')
         if rank == 0 and not args.quick and not slab:
             out["next_rows"] = time_next_rows(lq, L, mass, shifts, tol, K, W, U, f)
             out["read_only_gbs"] = read_only_reference_gbs()
         del U, f
+        phase('next rows done')
         if rank == 0 and not args.quick and args.workload == "config4_48^4":
             L3 = gen.CONFIGS["config3_32^4"]["L"]
             U3, f3 = gen.random_su3_links(L3, device="cuda"), gen.gaussian_field(L3, device="cuda")
@@ -603,9 +618,11 @@ def main():
     for key in ("cg_recon12", "cg_recon18", "next_rows"):
         if key in res:
             line[key] = res[key]
+    phase("GPU part done")
     if not args.quick and world == 1:
         s_iter, cores, sample, _ = run_oracle(args.workload, budget_s=args.cpu_budget, steps=None)
         line["cpu_baseline"] = {"value": s_iter, "unit": "s/iter", "cores": cores, "kind": "oracle", "sample": sample}
+    phase("CPU baseline done")
     print(json.dumps(line))
     barrier(world)
     return 0

@@ -155,10 +155,10 @@ def _free_port():
         return s.getsockname()[1]
 
 
-def _run_ranks(world, L, comm):
+def _run_ranks(world, L, comm, recon=18):
     cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", str(world),
            "--master-addr", "127.0.0.1", "--master-port", str(_free_port()),
-           os.path.join("tests", "_slab_worker.py"), *[str(v) for v in L], comm]
+           os.path.join("tests", "_slab_worker.py"), *[str(v) for v in L], comm, str(recon)]
     out = subprocess.run(cmd, cwd=ROOT, env=dict(os.environ, OMP_NUM_THREADS="4"), capture_output=True, text=True,
                          timeout=600)
     assert out.returncode == 0, out.stdout[-2000:] + out.stderr[-3000:]
@@ -167,14 +167,21 @@ def _run_ranks(world, L, comm):
     r = json.loads(line[0][7:])
     assert r["doe"] <= 1e-12 and r["deo"] <= 1e-12 and r["mdagm"] <= 1e-12, r
     assert r["doe_u1"] <= 1e-12 and r["deo_u1"] <= 1e-12, r
-    assert abs(r["iters"] - r["iters_ref"]) <= 1 and r["iters_equal_on_ranks"], r
+    # single precision on the slabs (tolerances of tests/test_gpu_f32.py: 24 eps32 for the operator; the float solve
+    # to 1e-5 against the double solutions)
+    assert r["doe_f32"] <= 2e-6 and max(r["x_f32"]) <= 1e-3, r
+    assert r["band"][0] - 1 <= r["iters"] <= r["band"][1] + 1 and r["iters_equal_on_ranks"], r
     assert max(r["x"]) <= 1e-8, r
     assert r["freeze_equal_on_ranks"], r
 
 
-@pytest.mark.parametrize("L", [(4, 6, 4, 8), (4, 4, 4, 4)])
-def test_two_ranks_share_the_gpu_host_staged(L):
-    _run_ranks(2, L, "torch")
+@pytest.mark.parametrize("L,recon", [((4, 6, 4, 8), 18), ((4, 4, 4, 4), 18), ((4, 4, 6, 8), 12)])
+def test_two_ranks_share_the_gpu_host_staged(L, recon):
+    _run_ranks(2, L, "torch", recon)
+
+
+def test_four_ranks_share_the_gpu_host_staged():
+    _run_ranks(4, (4, 4, 4, 8), "torch")            # two time slices per rank: no interior
 
 
 @pytest.mark.parametrize("world,L", [(2, (8, 8, 8, 8)), (4, (4, 6, 8, 16))])
