@@ -27,7 +27,8 @@
 //
 // Pins (tests/test_oracle_pins.py, all CPU): anti-hermiticity, gauge covariance, free-field closed form
 // (periodic and antiperiodic), dense 2^4 / small-lattice inversion with numpy for every shift, unitarity
-// of reconstructed links, CG invariants.  No function here is "parity unpinned".
+// of reconstructed links, CG invariants, and the stop / freeze iterations and the frozen iterates against an
+// independent textbook CG per shifted system on the dense matrix.  No function here is "parity unpinned".
 //
 // Storage conventions of this file:
 //   lex = x + Lx*(y + Ly*(z + Lz*t)),  parity(lex) = (x+y+z+t)&1, even = 0.

@@ -275,6 +275,83 @@ def test_mshift_cg_against_dense_solve(L, mass, shifts):
     assert np.all(np.diff(fr) <= 0) and fr[0] == info["iters"]
 
 
+def dense_A_linkwise(L, U, mass, antiperiodic=True):
+    """A = m^2 - D_eo D_oe from the link-centric numpy assembly of D: shares nothing with the oracle."""
+    D = dense_D_linkwise(L, U, antiperiodic)
+    me3, mo3 = np.repeat(parity_mask(L, 0), 3), np.repeat(parity_mask(L, 1), 3)
+    D_oe, D_eo = D[np.ix_(mo3, me3)], D[np.ix_(me3, mo3)]
+    return mass * mass * np.eye(D_oe.shape[1]) - D_eo @ D_oe
+
+
+def textbook_cg(M, b, nit):
+    """Plain CG (Hestenes-Stiefel) on one dense Hermitian system M x = b, zero initial guess, own loop and own
+    dot products.  Returns the relative residual norms |r_n|/|b| and the iterates x_n for n = 0..nit."""
+    x, res, p = np.zeros_like(b), b.copy(), b.copy()
+    rr = np.vdot(res, res).real
+    bb = rr
+    norms, iterates = [1.0], [x.copy()]
+    for _ in range(nit):
+        Mp = M @ p
+        a = rr / np.vdot(p, Mp).real
+        x = x + a * p
+        res = res - a * Mp
+        rr_new = np.vdot(res, res).real
+        p = res + (rr_new / rr) * p
+        rr = rr_new
+        norms.append(np.sqrt(rr / bb))
+        iterates.append(x.copy())
+    return np.array(norms), iterates
+
+
+# (lattice, mass, shifts, slack): slack = allowed distance between the oracle's freeze iteration and the first
+# iteration at which the independent CG's residual is below tol.  +-1 is rounding (the two programs add in a
+# different order); the 600-iteration solve on 4^4 at m = 0.01 moves by 2 (cf. DESIGN.md R9).
+STOP_CASES = [
+    ((2, 2, 2, 2), 0.01, [1e-4 * 10 ** (i / 2) for i in range(8)], 1),
+    ((2, 2, 2, 2), 0.05, [0.3, 0.0, 2.0, 1e-3], 1),
+    ((4, 2, 2, 4), 0.02, [1e-3, 1e-2, 1e-1, 1.0], 1),
+    ((4, 4, 4, 4), 0.1, [1e-2 * 10 ** (i / 2) for i in range(6)], 1),
+    ((4, 4, 4, 4), 0.01, [1e-4 * 10 ** (i / 2) for i in range(8)], 2),
+]
+
+
+@pytest.mark.parametrize("L,mass,shifts,slack", STOP_CASES)
+def test_stop_and_freeze_iterations_against_independent_cg_per_shift(L, mass, shifts, slack):
+    """In exact arithmetic the multi-shift iterate of system i IS the CG iterate of (A + sigma_i) x = b, and its
+    residual is zeta_i r (refs 32/33; R5).  So the rules R6/R7 say: shift i is frozen at
+    the FIRST iteration n at which a plain CG on that system alone has |r_n| <= tol |b|, its solution is that
+    CG's n-th iterate, and the solve stops when the smallest shift gets there.  Checked against a textbook CG in
+    numpy on the dense matrix assembled link by link (no oracle code on that side).  This pins the freeze test
+    (zeta_i^2 |r|^2 against tol^2 |b|^2), the stopping test and the reported counts from BOTH sides: freezing
+    or stopping later than necessary fails as well as earlier ("stopping residuals")."""
+    U = links(L)
+    b = oracle.restrict(L, 0, gen.gaussian_field(L).numpy())
+    bv = c(b).ravel()
+    A = dense_A_linkwise(L, U, mass)
+    tol = 1e-10
+    x, info = oracle.mshift_cg(L, U, mass, b, shifts, tol)
+    assert info["status"] == 0
+    i0 = int(np.argmin(shifts))
+    assert info["freeze_iter"][i0] == info["iters"] == max(info["freeze_iter"])
+    for i, sigma in enumerate(shifts):
+        M = A + sigma * np.eye(A.shape[0])
+        fz = info["freeze_iter"][i]
+        norms, iterates = textbook_cg(M, bv, fz + slack + 1)
+        first = int(np.argmax(norms <= tol))
+        assert norms[first] <= tol and abs(first - fz) <= slack, (i, sigma, first, fz)
+        # not later than necessary: well before the freeze iteration the system had NOT converged ...
+        assert norms[fz - slack - 1] > tol, (i, norms[fz - slack - 1])
+        # ... and the frozen x_i is that CG's iterate of the same iteration, not a later (more accurate) one
+        xi = c(x[i]).ravel()
+        assert np.linalg.norm(xi - iterates[fz]) <= 1e-9 * np.linalg.norm(iterates[fz]), (i, sigma)
+        true_res = np.linalg.norm(bv - M @ xi) / np.linalg.norm(bv)
+        # zeta_i |r| at the freeze iteration = |r_n| of the system's own CG (the recurrences differ by rounding)
+        band = norms[fz - slack:fz + slack + 1]
+        assert 0.5 * band.min() <= true_res <= 2.0 * band.max() and true_res <= tol * 1.01, (i, true_res, band)
+        if i == i0:      # the reported residual is that of the base system at the stop
+            assert 0.5 * band.min() <= info["rel_res"] <= 2.0 * band.max() and info["rel_res"] <= tol
+
+
 def test_mshift_cg_fixed_iteration_count_and_first_step():
     # after exactly one iteration x_i = a_0/(1 + delta_i a_0) b with a_0 = <b,b>/<b,B b>: the exact
     # first CG step of every shifted system (closed form, independent of the zeta recurrence code path)
