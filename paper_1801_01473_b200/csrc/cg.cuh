@@ -192,7 +192,7 @@ __global__ void __launch_bounds__(CG_BLOCK) cg_update_base_kernel(const V2<T>* _
 // thread) in flight instead of 2 took it from 5.6 to 6.3 TB/s at 48^4 (profiles/ncu_full_r01.md).
 #define FLUSH_UNR 4
 template <typename T, int MM, bool RATIONAL, bool FULL>
-__device__ __forceinline__ void cg_flush_body(const int nres, const int nl, V2<T>* const* sx, V2<T>* const* sp,
+__device__ __forceinline__ void cg_flush_body(const int nres, const int nl, const int e_base, V2<T>* const* sx, V2<T>* const* sp,
                                               const V2<T>* const* sr, const T* sCP, const T* sB, const V2<T>* sDE,
                                               const T* sY, V2<T>* __restrict__ y, const size_t n) {
     constexpr int U = FLUSH_UNR;
@@ -247,7 +247,7 @@ __device__ __forceinline__ void cg_flush_body(const int nres, const int nl, V2<T
                         yv.x += dx;
                         yv.y += dy;
                     }
-                    sp[e][j] = make_v2(px, py);
+                    if (e != e_base) sp[e][j] = make_v2(px, py);      // the base system's p is kept by K2
                 }
             }
         }
@@ -265,7 +265,9 @@ __global__ void __launch_bounds__(CG_BLOCK, (MM <= 8 ? 2 : 1)) cg_flush_kernel(C
     __shared__ T sCP[LQCD_MAX_SHIFTS], sB[LQCD_MAX_SHIFTS], sY[MM];
     __shared__ V2<T> sDE[LQCD_MAX_SHIFTS * MM];
     __shared__ int cnt[2];
+    __shared__ int s_ebase;
     const int tid = threadIdx.x;
+    if (tid == 0) s_ebase = -1;
     const int rational = st->rational;
     // compact list of the shifts of this block (two warps, one thread per shift)
     int inb = 0;
@@ -284,7 +286,12 @@ __global__ void __launch_bounds__(CG_BLOCK, (MM <= 8 ? 2 : 1)) cg_flush_kernel(C
     if (inb) {
         const int e = __popc(bal & ((1u << (tid & 31)) - 1u)) + ((tid >= 32) ? cnt[0] : 0);
         sx[e] = (V2<T>*)st->x[tid];
-        sp[e] = (V2<T>*)st->p[tid];
+        if (tid == st->i0) {                     // block-deferred base system: P = p^(n0), read only
+            sp[e] = (V2<T>*)st->p_keep;
+            s_ebase = e;
+        } else {
+            sp[e] = (V2<T>*)st->p[tid];
+        }
         sCP[e] = (T)st->blk_CP[tid];
         sB[e] = (T)st->blk_B[tid];
 #pragma unroll
@@ -302,11 +309,11 @@ __global__ void __launch_bounds__(CG_BLOCK, (MM <= 8 ? 2 : 1)) cg_flush_kernel(C
     V2<T>* __restrict__ y = (V2<T>*)st->y;
     if (nl > 0) {
         if (rational) {
-            if (nres == MM) cg_flush_body<T, MM, true, true>(nres, nl, sx, sp, sr, sCP, sB, sDE, sY, y, n);
-            else cg_flush_body<T, MM, true, false>(nres, nl, sx, sp, sr, sCP, sB, sDE, sY, y, n);
+            if (nres == MM) cg_flush_body<T, MM, true, true>(nres, nl, s_ebase, sx, sp, sr, sCP, sB, sDE, sY, y, n);
+            else cg_flush_body<T, MM, true, false>(nres, nl, s_ebase, sx, sp, sr, sCP, sB, sDE, sY, y, n);
         } else {
-            if (nres == MM) cg_flush_body<T, MM, false, true>(nres, nl, sx, sp, sr, sCP, sB, sDE, sY, y, n);
-            else cg_flush_body<T, MM, false, false>(nres, nl, sx, sp, sr, sCP, sB, sDE, sY, y, n);
+            if (nres == MM) cg_flush_body<T, MM, false, true>(nres, nl, s_ebase, sx, sp, sr, sCP, sB, sDE, sY, y, n);
+            else cg_flush_body<T, MM, false, false>(nres, nl, s_ebase, sx, sp, sr, sCP, sB, sDE, sY, y, n);
         }
     }
     // the last block to finish closes the block of iterations; every block has read the state by then
@@ -327,7 +334,7 @@ __global__ void __launch_bounds__(CG_BLOCK, (MM <= 8 ? 2 : 1)) cg_flush_kernel(C
 // The float CG iterates on a recurrence residual r and accumulates its solution in a float vector y.  At a
 // reliable update the accumulated y is added to the double-precision solution x (and cleared), the TRUE residual
 // b - (A + sigma) x is computed with the double-precision operator, and replaces r; the search direction is kept
-// (p += r_true - r_recurrence, i.e. p = r_true + beta p_old), so the Krylov sequence is not restarted.
+// (p = r_true + beta p_old), so the Krylov sequence is not restarted.
 
 // x64 += y32 ; y32 = 0
 __global__ void __launch_bounds__(CG_BLOCK) mixed_accumulate_kernel(double2* __restrict__ x, float2* __restrict__ y, size_t n) {
@@ -341,13 +348,15 @@ __global__ void __launch_bounds__(CG_BLOCK) mixed_accumulate_kernel(double2* __r
     }
 }
 
-// r_true = b - ax (double; ax == NULL: r_true = b);  |r_true|^2 -> st->rr and *rr_out;  r_out = float(r_true);
-// if p != NULL: p += float(r_true) - r_rec  (r_rec = the recurrence residual being replaced).
+// r_true = b - ax (double; ax == NULL: r_true = b);  |r_true|^2 -> *rr_out;  r_out = float(r_true).
+// replace != 0: r_out is the ring slot the next iteration reads its residual from, and |r_true|^2 replaces the
+// recurrence value on the device.  The search direction needs no correction: the fused iteration forms
+// p = r + beta p_old from whatever residual it finds there, so p = r_true + beta p_old, the direction is kept and
+// the Krylov sequence is not restarted.
 // resume != 0: the float solver had stopped on its recurrence residual and is started again.
 __global__ void __launch_bounds__(CG_BLOCK) mixed_residual_kernel(const double2* __restrict__ b, const double2* __restrict__ ax,
-                                                                  const float2* r_rec, float2* r_out, float2* __restrict__ p,
-                                                                  CgState* st, double* partials, double* rr_out, size_t n,
-                                                                  int resume) {
+                                                                  float2* __restrict__ r_out, CgState* st, double* partials,
+                                                                  double* rr_out, size_t n, int replace, int resume) {
     __shared__ double red[32];
     __shared__ int last_flag;
     double acc = 0.0;
@@ -360,15 +369,7 @@ __global__ void __launch_bounds__(CG_BLOCK) mixed_residual_kernel(const double2*
         }
         acc = fma(r.x, r.x, acc);
         acc = fma(r.y, r.y, acc);
-        const float2 rf = make_float2((float)r.x, (float)r.y);
-        if (p) {
-            const float2 old = r_rec[j];
-            float2 pv = p[j];
-            pv.x += rf.x - old.x;
-            pv.y += rf.y - old.y;
-            p[j] = pv;
-        }
-        r_out[j] = rf;
+        r_out[j] = make_float2((float)r.x, (float)r.y);
     }
     const double bsum = block_sum<CG_BLOCK>(acc, red);
     if (publish_partial<CG_BLOCK>(bsum, partials, &st->ticket[4], &last_flag)) {
@@ -376,7 +377,7 @@ __global__ void __launch_bounds__(CG_BLOCK) mixed_residual_kernel(const double2*
         if (threadIdx.x == 0) {
             st->ticket[4] = 0;
             *rr_out = rr;
-            if (p) st->rr = rr;
+            if (replace) st->rr = rr;
             if (resume) {
                 st->stop = 0;
                 st->stop4 = 0;

@@ -31,6 +31,18 @@
 // EPI = 2 : out = coef*pv - D in only
 // EPI = 3 : as 1, but only the block partial is written (at partials[part_off + blockIdx.x]); the sum over
 //           blocks, launches and ranks and the scalar step follow in their own small kernels (slab mode)
+//
+// The two launches of one fused CG iteration (cg.cuh has the whole picture; "scalar products and sums"
+// + the two operators, with every sum and scalar product folded into the operators' own sweeps):
+// EPI = 4 : K1.  The input is not a stored vector: it is the search direction p = r + beta p_old formed in
+//           registers at each of the eight neighbours from the residual `in` and the previous direction `in2`.
+//           out = D p (odd sites), and the block partial of  <p, A p> = c0 |p|^2 + |D_oe p|^2  (D_eo = -D_oe^+,
+//           PAPER.md:L80): |out|^2 of the site plus c0/8 |p|^2 of each neighbour (every even site is the
+//           neighbour of exactly eight odd sites).  The last block sums and runs the scalar step (a, zeta_i).
+// EPI = 5 : K2.  in = t = D_oe p.  At its own (even) site the thread forms p = r + beta p_old again and stores
+//           it (p_out), s = c0 p - D_eo t (never stored), r_new = r - a s (r_out, the next ring slot),
+//           x_0 += a p (unless the base system is block-deferred like the shifted ones), and the block partial of
+//           |r_new|^2.  The last block sums and runs the scalar step (beta, b_i, freeze and stop flags).
 #ifndef LQCD_DSLASH_CUH
 #define LQCD_DSLASH_CUH
 
@@ -166,77 +178,59 @@ __device__ __forceinline__ void load_link(const V2<T>* __restrict__ w, const siz
     }
 }
 
-template <typename T>
-__device__ __forceinline__ void load_vec(const V2<T>* __restrict__ v, const size_t vh, uint64_t pol, unsigned int mask,
-                                         T (&vr)[3], T (&vi)[3]) {
+// the vector operand of a hop: a stored vector, or (FLY) p = r + beta p_old formed in registers from the residual v
+// and the previous search direction v2 (same index); pp accumulates |p|^2 for the <p,Ap> identity of EPI = 4
+template <typename T, bool FLY>
+__device__ __forceinline__ void load_vec(const V2<T>* __restrict__ v, const V2<T>* __restrict__ v2, const size_t vs,
+                                         uint64_t pol, unsigned int mask, const T beta, T (&vr)[3], T (&vi)[3],
+                                         double& pp) {
+    if (!FLY) {
 #pragma unroll
-    for (int c = 0; c < 3; ++c) {
-        const V2<T> t = ld_reuse(v + c * vh, pol);
-        vr[c] = flip(t.x, mask);
-        vi[c] = flip(t.y, mask);
+        for (int c = 0; c < 3; ++c) {
+            const V2<T> t = ld_reuse(v + c * vs, pol);
+            vr[c] = flip(t.x, mask);
+            vi[c] = flip(t.y, mask);
+        }
+    } else {
+        V2<T> r[3], q[3];
+#pragma unroll
+        for (int c = 0; c < 3; ++c) {
+            r[c] = ld_reuse(v + c * vs, pol);
+            q[c] = ld_reuse(v2 + c * vs, pol);
+        }
+        T n2 = (T)0;
+#pragma unroll
+        for (int c = 0; c < 3; ++c) {
+            const T x = fma(beta, q[c].x, r[c].x), y = fma(beta, q[c].y, r[c].y);
+            n2 = fma(x, x, n2);
+            n2 = fma(y, y, n2);
+            vr[c] = flip(x, mask);
+            vi[c] = flip(y, mask);
+        }
+        pp += (double)n2;
     }
 }
 
-// acc += sign * U v          (forward hop; the sign is already folded into v)
-template <typename T, int RECON, int U1>
-__device__ __forceinline__ void hop_fwd(T (&ar)[3], T (&ai)[3], const V2<T>* __restrict__ w,
-                                        const V2<T>* __restrict__ v, const size_t vh, unsigned int mask,
-                                        uint64_t pol_s, uint64_t pol_r, const T* __restrict__ th) {
-    V2<T> u[9];
-    T vr[3], vi[3];
-    load_link<T, RECON>(w, vh, pol_s, u);
-    load_vec<T>(v, vh, pol_r, mask, vr, vi);
-    if (U1) u1_rotate<T, +1>(th, pol_s, vr, vi);
-#pragma unroll
-    for (int a = 0; a < 3; ++a)
-#pragma unroll
-        for (int b = 0; b < 3; ++b) cmad<T>(ar[a], ai[a], u[3 * a + b], vr[b], vi[b]);
-}
-
-// acc += sign * U^dagger v   (backward hop; caller passes the mask of -s)
-template <typename T, int RECON, int U1>
-__device__ __forceinline__ void hop_bwd(T (&ar)[3], T (&ai)[3], const V2<T>* __restrict__ w,
-                                        const V2<T>* __restrict__ v, const size_t vh, unsigned int mask,
-                                        uint64_t pol_s, uint64_t pol_r, const T* __restrict__ th) {
-    V2<T> u[9];
-    T vr[3], vi[3];
-    load_link<T, RECON>(w, vh, pol_s, u);
-    load_vec<T>(v, vh, pol_r, mask, vr, vi);
-    if (U1) u1_rotate<T, -1>(th, pol_s, vr, vi);
-#pragma unroll
-    for (int a = 0; a < 3; ++a)
-#pragma unroll
-        for (int b = 0; b < 3; ++b) cmad_conj<T>(ar[a], ai[a], u[3 * b + a], vr[b], vi[b]);
-}
-
-// the same two hops with separate element strides for the link and the vector (slab faces: halo buffers)
-template <typename T, int RECON, int U1>
-__device__ __forceinline__ void hop_fwd_s(T (&ar)[3], T (&ai)[3], const V2<T>* __restrict__ w, const size_t ws,
-                                          const V2<T>* __restrict__ v, const size_t vs, unsigned int mask,
-                                          uint64_t pol_s, uint64_t pol_r, const T* __restrict__ th) {
+// One hop.  FWD: acc += sign * U v (the sign is already folded into v);  !FWD: acc += sign * U^dagger v (the caller
+// passes the mask of -s).  ws, vs: element strides of the link and of the vector (they differ from Vh only for the
+// halo buffers of a slab face).
+template <typename T, int RECON, int U1, bool FWD, bool FLY>
+__device__ __forceinline__ void hop(T (&ar)[3], T (&ai)[3], const V2<T>* __restrict__ w, const size_t ws,
+                                    const V2<T>* __restrict__ v, const V2<T>* __restrict__ v2, const size_t vs,
+                                    unsigned int mask, uint64_t pol_s, uint64_t pol_r, const T* __restrict__ th,
+                                    const T beta, double& pp) {
     V2<T> u[9];
     T vr[3], vi[3];
     load_link<T, RECON>(w, ws, pol_s, u);
-    load_vec<T>(v, vs, pol_r, mask, vr, vi);
-    if (U1) u1_rotate<T, +1>(th, pol_s, vr, vi);
+    load_vec<T, FLY>(v, v2, vs, pol_r, mask, beta, vr, vi, pp);
+    if (U1) u1_rotate<T, FWD ? +1 : -1>(th, pol_s, vr, vi);
 #pragma unroll
     for (int a = 0; a < 3; ++a)
 #pragma unroll
-        for (int b = 0; b < 3; ++b) cmad<T>(ar[a], ai[a], u[3 * a + b], vr[b], vi[b]);
-}
-template <typename T, int RECON, int U1>
-__device__ __forceinline__ void hop_bwd_s(T (&ar)[3], T (&ai)[3], const V2<T>* __restrict__ w, const size_t ws,
-                                          const V2<T>* __restrict__ v, const size_t vs, unsigned int mask,
-                                          uint64_t pol_s, uint64_t pol_r, const T* __restrict__ th) {
-    V2<T> u[9];
-    T vr[3], vi[3];
-    load_link<T, RECON>(w, ws, pol_s, u);
-    load_vec<T>(v, vs, pol_r, mask, vr, vi);
-    if (U1) u1_rotate<T, -1>(th, pol_s, vr, vi);
-#pragma unroll
-    for (int a = 0; a < 3; ++a)
-#pragma unroll
-        for (int b = 0; b < 3; ++b) cmad_conj<T>(ar[a], ai[a], u[3 * b + a], vr[b], vi[b]);
+        for (int b = 0; b < 3; ++b) {
+            if (FWD) cmad<T>(ar[a], ai[a], u[3 * a + b], vr[b], vi[b]);
+            else cmad_conj<T>(ar[a], ai[a], u[3 * b + a], vr[b], vi[b]);
+        }
 }
 
 template <typename T>
@@ -244,14 +238,21 @@ struct DslashArgs {
     Geom g;
     const V2<T>* W;          // stored links
     const T* Th;             // U1 == 1: stored U(1) angles theta_mu(x)
-    const V2<T>* in;         // parity 1-par
-    V2<T>* out;              // parity par
+    const V2<T>* in;         // parity 1-par (EPI == 4: the residual r)
+    const V2<T>* in2;        // EPI == 4: the previous search direction p_old, parity 1-par
+    V2<T>* out;              // parity par (not written by EPI == 5)
     int par;                 // parity of the output sites
-    const V2<T>* pv;         // EPI >= 1: vector of parity par
-    double coef;             // EPI >= 1: m^2 + sigma
-    double* partials;        // EPI == 1
-    CgState* st;             // EPI == 1, or any EPI with check_stop
+    const V2<T>* pv;         // EPI 1,2,3: vector of parity par;  EPI == 5: p_old
+    double coef;             // EPI == 2: m^2 + sigma
+    double* partials;        // EPI 1,3,4,5
+    CgState* st;             // EPI 1,3,4,5, or any EPI with check_stop
     int check_stop;          // 1: return at once if st->stop (CG already converged)
+    // EPI == 5 only (all of parity par)
+    const V2<T>* r_in;       // residual r^(n)
+    V2<T>* r_out;            // residual r^(n+1): the next slot of the ring (may be r_in itself)
+    V2<T>* p_out;            // search direction p^(n) (may be pv itself)
+    V2<T>* p_keep;           // not NULL: p^(n) is also stored here (first iteration of a block, base system deferred)
+    int defer_base;          // 1: x_0 is updated by the block sweep like the shifted systems, not here
     // SLAB == 1 only
     const V2<T>* in_lo;      // halo: time slice t_off-1 of `in`, [c][face]
     const V2<T>* in_hi;      // halo: time slice t_off+Lt of `in`, [c][face]
@@ -262,12 +263,20 @@ struct DslashArgs {
 };
 
 // registers: double needs ~126 (4 blocks of 128 threads per SM); single fits 6 blocks
-template <typename T> struct DsOcc { static constexpr int minb = DS_MINB; };
-template <> struct DsOcc<float> { static constexpr int minb = DS_MINB_F32; };
+#ifndef DS_MINB_K1
+#define DS_MINB_K1 DS_MINB
+#endif
+#ifndef DS_MINB_K2
+#define DS_MINB_K2 DS_MINB
+#endif
+template <typename T, int EPI> struct DsOcc { static constexpr int minb = (EPI == 4) ? DS_MINB_K1 : (EPI == 5) ? DS_MINB_K2 : DS_MINB; };
+template <int EPI> struct DsOcc<float, EPI> { static constexpr int minb = DS_MINB_F32; };
 
 template <typename T, int RECON, int EPI, int U1, int SLAB = 0>
-__global__ void __launch_bounds__(DS_BLOCK, DsOcc<T>::minb) dslash_kernel(const DslashArgs<T> A) {
+__global__ void __launch_bounds__(DS_BLOCK, (DsOcc<T, EPI>::minb)) dslash_kernel(const DslashArgs<T> A) {
     constexpr int NE = (RECON == 12) ? 6 : 9;
+    constexpr bool FLY = (EPI == 4);
+    static_assert(!(SLAB && EPI >= 4), "the fused CG launches exist for the whole-lattice path only");
     if (A.check_stop) {
         if (A.st->stop) {
             // tell the x/p update kernel of the *following* iterations to do nothing (see cg.cuh)
@@ -325,46 +334,66 @@ __global__ void __launch_bounds__(DS_BLOCK, DsOcc<T>::minb) dslash_kernel(const 
     const V2<T>* __restrict__ Wb = A.W + (size_t)(1 - A.par) * NE * vh;          // links of the input parity
     const size_t mu_stride = (size_t)2 * NE * vh;
     const V2<T>* __restrict__ in = A.in;
+    const V2<T>* __restrict__ in2 = FLY ? A.in2 : A.in;
 
     // epilogue operands are requested first, so that their latency hides behind the eight hops
-    T coef = (T)0;
-    V2<T> pv[3];
+    T coef = (T)0, beta = (T)0;
+    V2<T> pv[3], rv[3];
     if (EPI != 0) {
-        coef = (T)((EPI == 1 || EPI == 3) ? A.st->c0 : A.coef);     // CG: m^2 + sigma0 from the device state (graph-invariant)
+        // CG: m^2 + sigma0 from the device state (graph-invariant)
+        coef = (T)((EPI == 2) ? A.coef : A.st->c0);
+        if (EPI >= 4) beta = (T)A.st->b_prev;
+        if (EPI != 4) {
 #if EPI_PLOAD == 1
 #pragma unroll
-        for (int c = 0; c < 3; ++c) pv[c] = A.pv[c * vh + k];
+            for (int c = 0; c < 3; ++c) pv[c] = A.pv[c * vh + k];
 #elif EPI_PLOAD == 2
 #pragma unroll
-        for (int c = 0; c < 3; ++c) asm volatile("prefetch.global.L2 [%0];" ::"l"(A.pv + c * vh + k));
+            for (int c = 0; c < 3; ++c) asm volatile("prefetch.global.L2 [%0];" ::"l"(A.pv + c * vh + k));
 #endif
+        }
+        if (EPI == 5) {
+#pragma unroll
+            for (int c = 0; c < 3; ++c) rv[c] = A.r_in[c * vh + k];
+        }
     }
 
     T ar[3] = {(T)0, (T)0, (T)0}, ai[3] = {(T)0, (T)0, (T)0};
+    double pp = 0.0;                                                             // EPI == 4: sum of |p|^2 over the neighbours
     const T* __restrict__ Tf = U1 ? A.Th + (size_t)A.par * vh + k : nullptr;     // angles of the forward links
     const T* __restrict__ Tb = U1 ? A.Th + (size_t)(1 - A.par) * vh : nullptr;   // angles of the backward links
     const size_t th_stride = 2 * vh;
-    hop_fwd<T, RECON, U1>(ar, ai, Wf + 0 * mu_stride, in + kxf, vh, 0u, pol_s, pol_r, Tf + 0 * th_stride);
-    hop_bwd<T, RECON, U1>(ar, ai, Wb + 0 * mu_stride + kxb, in + kxb, vh, SB, pol_s, pol_r, Tb + 0 * th_stride + kxb);
-    hop_fwd<T, RECON, U1>(ar, ai, Wf + 1 * mu_stride, in + kyf, vh, my, pol_s, pol_r, Tf + 1 * th_stride);
-    hop_bwd<T, RECON, U1>(ar, ai, Wb + 1 * mu_stride + kyb, in + kyb, vh, my ^ SB, pol_s, pol_r, Tb + 1 * th_stride + kyb);
-    hop_fwd<T, RECON, U1>(ar, ai, Wf + 2 * mu_stride, in + kzf, vh, mz, pol_s, pol_r, Tf + 2 * th_stride);
-    hop_bwd<T, RECON, U1>(ar, ai, Wb + 2 * mu_stride + kzb, in + kzb, vh, mz ^ SB, pol_s, pol_r, Tb + 2 * th_stride + kzb);
+#define HOP_F(mu, kn, mask) \
+    hop<T, RECON, U1, true, FLY>(ar, ai, Wf + (mu) * mu_stride, vh, in + (kn), in2 + (kn), vh, mask, pol_s, pol_r, \
+                                 Tf + (mu) * th_stride, beta, pp)
+#define HOP_B(mu, kn, mask) \
+    hop<T, RECON, U1, false, FLY>(ar, ai, Wb + (mu) * mu_stride + (kn), vh, in + (kn), in2 + (kn), vh, (mask) ^ SB, pol_s, \
+                                  pol_r, Tb + (mu) * th_stride + (kn), beta, pp)
+    HOP_F(0, kxf, 0u);
+    HOP_B(0, kxb, 0u);
+    HOP_F(1, kyf, my);
+    HOP_B(1, kyb, my);
+    HOP_F(2, kzf, mz);
+    HOP_B(2, kzb, mz);
     if (!SLAB) {
-        hop_fwd<T, RECON, U1>(ar, ai, Wf + 3 * mu_stride, in + ktf, vh, mtf, pol_s, pol_r, Tf + 3 * th_stride);
-        hop_bwd<T, RECON, U1>(ar, ai, Wb + 3 * mu_stride + ktb, in + ktb, vh, mtb ^ SB, pol_s, pol_r, Tb + 3 * th_stride + ktb);
+        HOP_F(3, ktf, mtf);
+        HOP_B(3, ktb, mtb);
     } else {
         // across the slab faces the neighbour vector (and, downwards, the link) comes from the halo buffers
         const size_t face = (size_t)g.st;
         const int kf = k - t * g.st;                                  // index inside a time slice
         const bool top = (t == g.Lt - 1), bot = (t == 0);
         const V2<T>* vf = top ? A.in_hi + kf : in + k + g.st;
-        hop_fwd_s<T, RECON, U1>(ar, ai, Wf + 3 * mu_stride, vh, vf, top ? face : vh, mtf, pol_s, pol_r, Tf + 3 * th_stride);
+        hop<T, RECON, U1, true, false>(ar, ai, Wf + 3 * mu_stride, vh, vf, vf, top ? face : vh, mtf, pol_s, pol_r,
+                                       Tf + 3 * th_stride, beta, pp);
         const V2<T>* vb = bot ? A.in_lo + kf : in + k - g.st;
         const V2<T>* wb = bot ? A.Wt_lo + (size_t)(1 - A.par) * NE * face + kf : Wb + 3 * mu_stride + k - g.st;
         const T* tb = U1 ? (bot ? A.Th_lo + (size_t)(1 - A.par) * face + kf : Tb + 3 * th_stride + k - g.st) : nullptr;
-        hop_bwd_s<T, RECON, U1>(ar, ai, wb, bot ? face : vh, vb, bot ? face : vh, mtb ^ SB, pol_s, pol_r, tb);
+        hop<T, RECON, U1, false, false>(ar, ai, wb, bot ? face : vh, vb, vb, bot ? face : vh, mtb ^ SB, pol_s, pol_r, tb,
+                                        beta, pp);
     }
+#undef HOP_F
+#undef HOP_B
 
     if (EPI == 0) {
         if (valid) {
@@ -374,20 +403,66 @@ __global__ void __launch_bounds__(DS_BLOCK, DsOcc<T>::minb) dslash_kernel(const 
         return;
     }
 
-    // epilogue: out = coef*pv - D in;  Re<pv, out> (summed in double whatever T is)
-    double dot = 0.0;
+    double dot = 0.0;                           // scalar products are summed in double whatever T is
+    if (EPI == 4) {
+        // K1: t = D_oe p;  this site's share of <p, A p> = c0 |p|^2 + |t|^2
 #pragma unroll
-    for (int c = 0; c < 3; ++c) {
+        for (int c = 0; c < 3; ++c) {
+            const V2<T> o = make_v2((T)0.5 * ar[c], (T)0.5 * ai[c]);
+            if (valid) {
+                A.out[c * vh + k] = o;
+                dot = fma((double)o.x, (double)o.x, dot);
+                dot = fma((double)o.y, (double)o.y, dot);
+            }
+        }
+        if (valid) dot = fma(0.125 * A.st->c0, pp, dot);
+    } else if (EPI == 5) {
+        // K2: p = r + beta p_old;  s = c0 p - D_eo t;  r_new = r - a s;  x_0 += a p
+        const CgState* st = A.st;
+        const T a = (T)st->a;
+        const int rational = st->rational, i0 = st->i0;
+        const T ax = (T)(rational ? st->alpha[i0] * st->a : st->a);
+        V2<T>* __restrict__ xp = (V2<T>*)(rational ? st->y : st->x[i0]);
+#pragma unroll
+        for (int c = 0; c < 3; ++c) {
 #if EPI_PLOAD == 1
-        const V2<T> p = pv[c];
+            const V2<T> po = pv[c];
 #else
-        const V2<T> p = A.pv[c * vh + k];
+            const V2<T> po = A.pv[c * vh + k];
 #endif
-        const V2<T> o = make_v2(fma((T)-0.5, ar[c], coef * p.x), fma((T)-0.5, ai[c], coef * p.y));
-        if (valid) {
-            A.out[c * vh + k] = o;
-            dot = fma((double)p.x, (double)o.x, dot);
-            dot = fma((double)p.y, (double)o.y, dot);
+            const V2<T> r = rv[c];
+            const V2<T> p = make_v2(fma(beta, po.x, r.x), fma(beta, po.y, r.y));
+            const V2<T> sv = make_v2(fma((T)-0.5, ar[c], coef * p.x), fma((T)-0.5, ai[c], coef * p.y));
+            const V2<T> rn = make_v2(fma(-a, sv.x, r.x), fma(-a, sv.y, r.y));
+            if (valid) {
+                A.p_out[c * vh + k] = p;
+                A.r_out[c * vh + k] = rn;
+                if (A.p_keep) A.p_keep[c * vh + k] = p;
+                if (!A.defer_base) {
+                    V2<T> xv = xp[c * vh + k];
+                    xv.x = fma(ax, p.x, xv.x);
+                    xv.y = fma(ax, p.y, xv.y);
+                    xp[c * vh + k] = xv;
+                }
+                dot = fma((double)rn.x, (double)rn.x, dot);
+                dot = fma((double)rn.y, (double)rn.y, dot);
+            }
+        }
+    } else {
+        // out = coef*pv - D in;  Re<pv, out>
+#pragma unroll
+        for (int c = 0; c < 3; ++c) {
+#if EPI_PLOAD == 1
+            const V2<T> p = pv[c];
+#else
+            const V2<T> p = A.pv[c * vh + k];
+#endif
+            const V2<T> o = make_v2(fma((T)-0.5, ar[c], coef * p.x), fma((T)-0.5, ai[c], coef * p.y));
+            if (valid) {
+                A.out[c * vh + k] = o;
+                dot = fma((double)p.x, (double)o.x, dot);
+                dot = fma((double)p.y, (double)o.y, dot);
+            }
         }
     }
     if (EPI == 3) {
@@ -395,7 +470,7 @@ __global__ void __launch_bounds__(DS_BLOCK, DsOcc<T>::minb) dslash_kernel(const 
         const double bsum = block_sum<DS_BLOCK>(dot, red3);
         if (threadIdx.x == 0) A.partials[A.part_off + blockIdx.x] = bsum;
     }
-    if (EPI == 1) {
+    if (EPI == 1 || EPI == 4) {
         __shared__ double red[32];
         __shared__ int last_flag;
         const double bsum = block_sum<DS_BLOCK>(dot, red);
@@ -403,6 +478,16 @@ __global__ void __launch_bounds__(DS_BLOCK, DsOcc<T>::minb) dslash_kernel(const 
             const double pAp = broadcast0(final_sum<DS_BLOCK>(A.partials, gridDim.x, red), red);
             if (threadIdx.x == 0) A.st->ticket[1] = 0;
             cg_scalars_after_pAp(A.st, pAp);
+        }
+    }
+    if (EPI == 5) {
+        __shared__ double red5[32];
+        __shared__ int last_flag5;
+        const double bsum = block_sum<DS_BLOCK>(dot, red5);
+        if (publish_partial<DS_BLOCK>(bsum, A.partials, &A.st->ticket[2], &last_flag5)) {
+            const double rr = broadcast0(final_sum<DS_BLOCK>(A.partials, gridDim.x, red5), red5);
+            if (threadIdx.x == 0) A.st->ticket[2] = 0;
+            cg_scalars_after_rr(A.st, rr);
         }
     }
 }

@@ -37,6 +37,7 @@ struct PrecBufs {
     T* Th = nullptr;         // stored U(1) angles theta_mu(x) (lqcd_set_u1_phases), [(mu*2+par)*Vh + k]
     int u1_stored = 0;
     V2<T> *p = nullptr, *s = nullptr, *t = nullptr;
+    V2<T>* p_keep = nullptr;                 // p of the first iteration of the current block (CgState::p_keep)
     V2<T>* hist[LQCD_MAX_BLOCK] = {};        // ring of residual vectors (cg.cuh)
     int n_hist = 0;
     V2<T>* pextra[LQCD_MAX_SHIFTS] = {};
@@ -239,7 +240,8 @@ int ensure_solver(lqcd_ctx* c, int nshift) {
         ++B.n_hist;
     }
     if (!B.p && (rc = dev_alloc(c, (void**)&B.p, vec_bytes<T>(c)))) return rc;
-    if (!B.s && (rc = dev_alloc(c, (void**)&B.s, vec_bytes<T>(c)))) return rc;
+    if (c->slab && !B.s && (rc = dev_alloc(c, (void**)&B.s, vec_bytes<T>(c)))) return rc;    // s is stored on slabs only
+    if (!c->slab && !B.p_keep && (rc = dev_alloc(c, (void**)&B.p_keep, vec_bytes<T>(c)))) return rc;
     while (B.n_pextra < nshift - 1) {
         if ((rc = dev_alloc(c, (void**)&B.pextra[B.n_pextra], vec_bytes<T>(c)))) return rc;
         ++B.n_pextra;
@@ -441,6 +443,40 @@ void launch_dslash(lqcd_ctx* c, int epi, V2<T>* out, const V2<T>* in, int par, c
     else launch_dslash_t<T, 2>(c, a);
 }
 
+// The two launches of a fused CG iteration (dslash.cuh, EPI = 4 and 5; cg.cuh has the whole picture).
+//   K1: t = D_oe p with p = r + beta p_old formed at the neighbours; <p,Ap>; a, zeta_i
+//   K2: p, s = c0 p - D_eo t, r_new = r - a s, x_0 += a p at the thread's own site; |r_new|^2; beta, b_i, flags
+template <typename T>
+void launch_cg_fused(lqcd_ctx* c, const V2<T>* r_in, V2<T>* r_out, V2<T>* p_keep, int defer_base) {
+    PrecBufs<T>& B = bufs<T>(c);
+    DslashArgs<T> a{};
+    a.g = c->g;
+    a.W = B.W;
+    a.Th = B.Th;
+    a.partials = c->partials;
+    a.st = c->st_dev;
+    a.check_stop = 1;
+    a.in = r_in;
+    a.in2 = B.p;
+    a.out = B.t;
+    a.par = 1;
+    launch_dslash_t<T, 4>(c, a);
+    a.in = B.t;
+    a.in2 = nullptr;
+    a.out = nullptr;
+    a.par = 0;
+    a.pv = B.p;
+    a.r_in = r_in;
+    a.r_out = r_out;
+    a.p_out = B.p;
+    a.p_keep = p_keep;
+    a.defer_base = defer_base;
+    launch_dslash_t<T, 5>(c, a);
+}
+
+// whole lattice, m >= 2: x_0 of the base system is updated by the block sweep too (CgState::defer_base)
+int defer_base(const lqcd_ctx* c) { return (!c->slab && c->shift_block >= 2) ? 1 : 0; }
+
 // the sweep over the shifted systems that closes a block of iterations (K5 of cg.cuh)
 template <typename T>
 void launch_flush(lqcd_ctx* c) {
@@ -474,12 +510,8 @@ int launch_cg_iteration(lqcd_ctx* c, int pos) {
         if (pos == m - 1) launch_flush<T>(c);
         return LQCD_OK;
     }
-    launch_dslash<T>(c, 0, B.t, B.p, 1, nullptr, 0.0, 1);
-    launch_dslash<T>(c, 1, B.s, B.t, 0, B.p, 0.0, 1);
-    cg_update_r_kernel<T><<<cg_grid(c), CG_BLOCK, 0, c->stream>>>(B.hist[(pos + m - 1) % m], B.hist[pos], B.s, c->st_dev,
-                                                                  c->partials, n);
-    cg_update_base_kernel<T><<<cg_grid(c), CG_BLOCK, 0, c->stream>>>(B.hist[pos], B.p, c->st_dev, n);
-    c->launches += 2;
+    const int defer = defer_base(c);
+    launch_cg_fused<T>(c, B.hist[(pos + m - 1) % m], B.hist[pos], (defer && pos == 0) ? B.p_keep : nullptr, defer);
     if (pos == m - 1) launch_flush<T>(c);
     return LQCD_OK;
 }
@@ -1109,6 +1141,8 @@ int solve(lqcd_ctx* c, const T* b_even, const double* shifts, int nshift, double
     h->rational = rational;
     h->alpha0 = alpha0;
     h->y = (void*)y;
+    h->defer_base = defer_base(c);
+    h->p_keep = (void*)B.p_keep;
     const size_t n = c->Vh * 3;
     CU(cudaMemcpyAsync(c->st_dev, h, sizeof(CgState), cudaMemcpyHostToDevice, c->stream));
     CU(cudaEventRecord(c->ev_t0, c->stream));
@@ -1226,6 +1260,8 @@ int mixed_solve_one(lqcd_ctx* c, const double* b, double sigma, double tol, doub
     h->p[0] = (void*)F.p;
     h->blk_m = m;
     for (int l = 0; l < m; ++l) h->hist[l] = (void*)F.hist[l];
+    h->defer_base = defer_base(c);
+    h->p_keep = (void*)F.p_keep;
     CU(cudaMemcpyAsync(c->st_dev, h, sizeof(CgState), cudaMemcpyHostToDevice, c->stream));
 
     if (have_guess) {
@@ -1233,8 +1269,8 @@ int mixed_solve_one(lqcd_ctx* c, const double* b, double sigma, double tol, doub
     } else {
         CU(cudaMemsetAsync(x, 0, n * sizeof(double2), c->stream));
     }
-    mixed_residual_kernel<<<cg_grid(c), CG_BLOCK, 0, c->stream>>>(b2, have_guess ? ax : nullptr, nullptr, r0, nullptr, c->st_dev,
-                                                                c->partials, c->red, n, 0);
+    mixed_residual_kernel<<<cg_grid(c), CG_BLOCK, 0, c->stream>>>(b2, have_guess ? ax : nullptr, r0, c->st_dev, c->partials,
+                                                                c->red, n, 0, 0);
     ++c->launches;
     CU(cudaMemcpyAsync(c->red_host, c->red, sizeof(double), cudaMemcpyDeviceToHost, c->stream));
     CU(cudaStreamSynchronize(c->stream));
@@ -1278,10 +1314,11 @@ int mixed_solve_one(lqcd_ctx* c, const double* b, double sigma, double tol, doub
         mixed_accumulate_kernel<<<cg_grid(c), CG_BLOCK, 0, c->stream>>>(x2, y, n);
         ++c->launches;
         if ((rc = apply_mdagm<double>(c, (double*)ax, x, sigma))) return rc;
-        const int cur = (h->iter + m - 1) % m;          // ring slot of the current recurrence residual
+        // every batch starts at ring position 0 (a batch is a whole number of blocks, and a stop inside a block closes
+        // it), i.e. its first iteration reads the residual from slot m-1 whatever slot the recurrence wrote last
         const int resume = (h->stop && h->status == 0) ? 1 : 0;
-        mixed_residual_kernel<<<cg_grid(c), CG_BLOCK, 0, c->stream>>>(b2, ax, F.hist[cur], F.hist[m - 1], F.p, c->st_dev,
-                                                                    c->partials, c->red, n, resume);
+        mixed_residual_kernel<<<cg_grid(c), CG_BLOCK, 0, c->stream>>>(b2, ax, F.hist[m - 1], c->st_dev, c->partials, c->red, n,
+                                                                    1, resume);
         ++c->launches;
         CU(cudaMemcpyAsync(c->red_host, c->red, sizeof(double), cudaMemcpyDeviceToHost, c->stream));
         CU(cudaStreamSynchronize(c->stream));
@@ -1328,8 +1365,8 @@ int solve_mixed(lqcd_ctx* c, const double* b_even, const double* shifts, int nsh
 
     // |b|^2 in double (the residual kernel with nothing subtracted), and the float copy of b
     CU(cudaMemsetAsync(c->st_dev, 0, sizeof(CgState), c->stream));
-    mixed_residual_kernel<<<cgrid, CG_BLOCK, 0, c->stream>>>((const double2*)b_even, nullptr, nullptr, F.stage_b, nullptr,
-                                                           c->st_dev, c->partials, c->red, n, 0);
+    mixed_residual_kernel<<<cgrid, CG_BLOCK, 0, c->stream>>>((const double2*)b_even, nullptr, F.stage_b, c->st_dev, c->partials,
+                                                           c->red, n, 0, 0);
     ++c->launches;
     CU(cudaMemcpyAsync(c->red_host, c->red, sizeof(double), cudaMemcpyDeviceToHost, c->stream));
     CU(cudaStreamSynchronize(c->stream));

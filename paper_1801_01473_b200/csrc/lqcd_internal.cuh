@@ -63,6 +63,11 @@ struct CgState {
     double alpha0;
     double alpha[LQCD_MAX_SHIFTS];
     void* y;
+    // fused iteration with m >= 2: the base system's x_0 is block-deferred like the shifted ones (zeta = 1).  Its p
+    // is still formed every iteration (the operator needs it); p_keep holds p^(n0), the direction of the block's
+    // first iteration, which is what the sweep needs besides the block's residuals.
+    int defer_base;
+    void* p_keep;
 };
 
 #endif

@@ -128,7 +128,7 @@ __device__ __noinline__ void cg_scalars_after_pAp(CgState* st, double pAp) {
     if (tid < ns) {
         const int i = tid;
         const int act = st->active[i];
-        const int inb = (j == 0) ? (act && i != i0) : st->in_block[i];
+        const int inb = (j == 0) ? (act && (i != i0 || st->defer_base)) : st->in_block[i];
         if (j == 0) st->in_block[i] = inb;
         if (act) {
             const double z = st->zeta[i], zp = st->zeta_prev[i];

@@ -167,7 +167,7 @@ def test_mshift_cg_small(lq, L, mass, shifts, mode):
     assert info["rel_res"] <= 1e-10
     assert info["base_shift"] == int(np.argmin(shifts))
     check_cg(x, info, x_ref, info_ref, shifts)
-    assert launches >= 4 * info["iters"] + 2
+    assert launches >= 2 * info["iters"] + 2          # two launches per iteration (K1, K2 of cg.cuh) + init + sweeps
 
 
 def test_mshift_cg_config2_16x4(lq):

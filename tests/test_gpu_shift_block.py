@@ -1,5 +1,6 @@
 """Block-deferred shift updates (LQCD_OPT_SHIFT_BLOCK = m): the x_i, p_i of the
-shifted systems are updated once per block of m iterations from the m residuals of the block.
+systems (for m >= 2 the base system's x_0 too) are updated once per block of m iterations from the m residuals
+of the block.
 
 What must hold, and is checked against the CPU oracle (which follows SURVEY.md §8(c2) iteration by iteration
 and knows nothing about blocks):
@@ -82,8 +83,7 @@ def test_every_block_length_gives_the_same_solve(lq, L, mass, shifts):
         assert info["status"] == 0
         assert info["iters"] == i1["iters"] and info["freeze_iter"] == i1["freeze_iter"], (m, info, i1)
         assert info["rel_res"] == i1["rel_res"]
-        i0 = info["base_shift"]
-        assert torch.equal(x[i0], x1[i0])                          # the base system does not see m at all
+        # (for m >= 2 the base system's x_0 is block-deferred like the shifted ones: equal up to rounding, below)
         for i in range(len(shifts)):
             assert rel_l2(x[i].cpu().numpy(), x1[i].cpu().numpy()) <= 1e-12, (m, i)
             assert rel_l2(soa_gpu_to_aos(x[i]), x_ref[i]) <= TOL_CG, (m, i)
