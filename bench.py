@@ -1,22 +1,33 @@
 #!/usr/bin/env python
-"""bench.py -- the BASELINE.json metric on one B200 (or N independent replicas under torchrun).
+"""bench.py -- the BASELINE.json metric on one B200 (or on N GPUs of one node).
 
 Metric (BASELINE.json): "Dslash ns/site and HBM GB/s (fraction of peak), 1xB200 double; mshift-CG s/iter".
 
   step      one iteration of the multi-shift CG = one pass of the whole hot path (DESIGN.md rows A2-A9:
-            D_oe, D_eo + fused zaxpy/dot epilogue, scalar recurrences, residual update + norm, x_i/p_i
-            updates of every active shift, loop control); A1 (link storage) is one-time set-up.
+            D_oe, D_eo with every sum and scalar product fused into the two operator sweeps, scalar recurrences,
+            1/m of the block sweep over the x_i/p_i of the active shifts, loop control); A1 (link storage) is
+            one-time set-up.
   workload  BASELINE config 4: 48^4, 16 shifts geometric 1e-5..1, m = 0.0075, tol 1e-10, 18-real links,
             seeded random SU(3) links + Gaussian even-site source (lqcd_inputs).  Links (3.06 GB) are far
             larger than L2, so no explicit L2 flush is needed between iterations.
-  value     seconds per CG iteration over exactly K iterations (device time, CUDA events), inputs
-            resident in HBM.  `dslash` holds ns/site and GB/s of the operator alone at 32^4 and 48^4,
-            18- and 12-real links; `roofline` is the D_oe/D_eo kernel at 48^4 (18-real) against the
-            measured HBM copy bandwidth; `full_solve` is the same solve run to convergence.
-  e2e       the same K iterations through lqcd_mshift_cg_host: b read from pinned host memory, all 16
-            solutions written back to pinned host memory, copies inside the timed region.
-  cpu_baseline  the CPU oracle (oracle/, as it stands) timed on the host cores on a few iterations of the
-            same workload.  `--impl reference` runs only that.
+  value     seconds per CG iteration over exactly K iterations (device time, CUDA events), inputs resident in
+            HBM; `value_steady` is the same over 96 iterations (a whole number of shift blocks).
+  roofline  the D_oe/D_eo kernel alone at 48^4 (18-real): DRAM-compulsory bytes (every link, every
+            input vector and the output once = 1248 B/site) / live CUDA-event time, against the measured HBM
+            copy bandwidth; the algorithmic rate (1584 B/site, neighbour re-reads served by L1/L2) beside it.
+  cg_roofline  the same for the timed CG iterations, bytes from the recorded freeze schedule.
+  dslash    ns/site and GB/s of the operator alone at 32^4 and 48^4, 18- and 12-real links.
+  small     BASELINE config 2 (16^4, whole solve) and the same shifts at 32^4: s/iter, against an L2 read stream.
+  e2e       the same K iterations through lqcd_mshift_cg_host: b from pinned host memory, all 16 solutions back to
+            pinned host memory, copies inside the timed region; `e2e_rational`: lqcd_rational_apply_host (what the
+            RHMC calls: one vector in, one vector back).
+  cpu_baseline  the CPU oracle (oracle/, as it stands) on the host cores: CG s/iter on a few iterations of the
+            same workload, Dslash ns/site at 32^4 (all cores and 1 thread), the whole 16^4 solve.
+            `--impl reference` runs only the CG part.
+
+N > 1: `python bench.py --gpus N` starts its own N ranks (torch.distributed.run) unless it already runs under
+torchrun.  Replicas are the headline (north_star: no sharding); rank 0 then runs the 1-D slab path (NEXT-3) on all N
+GPUs as a guarded sub-run and reports it under `slab`.
 
 Usage:  python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--workload NAME]
 """
@@ -25,7 +36,9 @@ from __future__ import annotations
 import argparse
 import json
 import os
+import socket
 import statistics
+import subprocess
 import sys
 import threading
 import time
@@ -38,37 +51,44 @@ import torch  # noqa: E402
 
 import lqcd_inputs as gen  # noqa: E402
 
-# Algorithmic bytes, per output site of one parity application.
-DSLASH_BYTES = {18: 8 * 144 + 8 * 48 + 48, 12: 8 * 96 + 8 * 48 + 48}      # 1584 / 1200
-DSLASH_DRAM_MODEL = {18: 8 * 144 + 48 + 48, 12: 8 * 96 + 48 + 48}         # each input read from DRAM once
+# Bytes per output site of one parity application.
+LINK_BYTES = {18: 144, 12: 96}
+DSLASH_BYTES = {r: 8 * LINK_BYTES[r] + 8 * 48 + 48 for r in (18, 12)}            # algorithmic: 1584 / 1200
+DSLASH_DRAM_MODEL = {r: 8 * LINK_BYTES[r] + 48 + 48 for r in (18, 12)}          # DRAM-compulsory: 1248 / 864
 DSLASH_FLOPS = {18: 570, 12: 570 + 8 * 42}
 
-# DRAM bytes per launch of dslash_kernel<18,0> measured by `ncu --set full` (dram__bytes_read.sum +
-# dram__bytes_write.sum), keyed by workload; source file under profiles/.  None until captured.
-NCU_DRAM_BYTES_PER_LAUNCH = {
-    ("config4_48^4", 18): 3.190834e9 + 0.103419e9,     # profiles/ncu_full_r01.md, dslash_kernel<double,18,0>
-    ("config4_48^4", 12): 2.171204e9 + 0.101689e9,     # profiles/ncu_full_r01.md, dslash_kernel<double,12,0>
+# DRAM bytes per launch of the plain D_oe/D_eo kernel measured by `ncu --set full` (dram__bytes_read.sum +
+# dram__bytes_write.sum), keyed by (workload, recon): (read GB, write GB, file under profiles/ that holds them).
+# tests/test_host_logic.py checks these constants against that file.
+NCU_DRAM_GB_PER_LAUNCH = {
+    ("config4_48^4", 18): (3.190834, 0.103419, "profiles/ncu_full_r01.md"),
+    ("config4_48^4", 12): (2.171204, 0.101689, "profiles/ncu_full_r01.md"),
 }
 
 
 def cg_bytes_per_site(n_active: int, recon: int) -> int:
-    """SURVEY.md §8(d) model of one CG iteration per even site, shift updates applied every iteration:
-    two Dslash + p in the epilogue + r update + base x/p + 192 B per further active shift."""
+    """SURVEY.md §8(d) model of one CG iteration per even site of the METHOD as the paper states it (shift updates
+    applied every iteration, one sweep per BLAS-1 operation): two Dslash + p in the epilogue + r update + base x/p
+    + 192 B per further active shift.  An equivalent rate only: the library moves fewer bytes (cg_dram_bytes)."""
     return 2 * DSLASH_BYTES[recon] + 48 + 144 + 240 + 192 * (n_active - 1)
 
 
-def cg_bytes_moved(freeze_iter, iters: int, m: int, recon: int) -> int:
-    """Bytes per even site the library actually moves in `iters` iterations with block-deferred shift updates
-    (DESIGN.md "CG iteration"): per iteration two Dslash + p (48) + r update (144) + base x/p (240); per block of
-    m iterations one sweep reading the block's residuals (48 each) and updating x_i, p_i (192) of every shifted
-    system that was active when the block began."""
+def cg_dram_bytes(freeze_iter, iters: int, m: int, recon: int) -> int:
+    """DRAM-compulsory bytes per even site of `iters` iterations as the library runs them:
+      K1  8 links + r + p_old in, t out;   K2  8 links + t + r + p_old in, p + r_new out;
+      m >= 2: per block of m iterations p_keep out (48), and one sweep: the block's residuals in (48 each), x_i, p_i
+              in and out (192) of every shifted system active when the block began, p_keep in + x_0 in/out (144);
+      m == 1: x_0 in/out in K2 (96); per iteration the residual (48) + 192 per active shifted system."""
+    links = 8 * LINK_BYTES[recon]
     base = max(range(len(freeze_iter)), key=lambda i: freeze_iter[i])
-    total = iters * (2 * DSLASH_BYTES[recon] + 48 + 144 + 240)
+    total = iters * (2 * links + 3 * 48 + 5 * 48)
     for n0 in range(0, iters, m):
         nres = min(m, iters - n0)
         n_in = sum(1 for i, fz in enumerate(freeze_iter) if i != base and fz > n0)
-        if n_in:
-            total += 48 * nres + 192 * n_in
+        if m >= 2:
+            total += 48 + 48 * nres + 192 * n_in + 144
+        else:
+            total += 96 + (48 + 192 * n_in if n_in else 0)
     return total
 
 
@@ -86,14 +106,14 @@ def load_peaks():
     if os.path.exists(path):
         with open(path) as fh:
             d = json.load(fh)
-        return float(d["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs, copy read+write)"
+        return float(d["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs: copy, read+write bytes, best of 10)"
     return 6650.0, "fallback (B200_PROFILING.md: 6.65 TB/s)"
 
 
 class ClockSampler:
     """Samples SM clock and throttle reasons of one GPU while the timed region runs (pynvml thread)."""
 
-    def __init__(self, index: int, period: float = 0.02):
+    def __init__(self, index: int, period: float = 0.005):
         self.index, self.period = index, period
         self.samples, self.reasons, self.max_mhz = [], set(), None
         self._stop = threading.Event()
@@ -154,10 +174,41 @@ class ClockSampler:
                 "reasons": sorted(self.reasons), "samples": len(self.samples)}
 
 
+# ---------------------------------------------------------------------------------------------------
+# ranks
+# ---------------------------------------------------------------------------------------------------
+def free_port() -> int:
+    with socket.socket() as s:
+        s.bind(("127.0.0.1", 0))
+        return s.getsockname()[1]
+
+
+def torchrun_cmd(n: int, script_args: list[str]) -> list[str]:
+    return [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={n}",
+            "--master-addr", "127.0.0.1", "--master-port", str(free_port()), os.path.abspath(__file__)] + script_args
+
+
+def self_launch(args, argv: list[str]):
+    """`python bench.py --gpus N` with N > 1 outside torchrun: become N ranks.  Never runs fewer GPUs than asked."""
+    if args.gpus <= 1 or "WORLD_SIZE" in os.environ or args.impl == "reference":
+        return
+    if not args.plumbing_check:
+        have = torch.cuda.device_count() if torch.cuda.is_available() else 0
+        if have < args.gpus:
+            print(f"bench.py: --gpus {args.gpus} needs {args.gpus} CUDA devices, this machine has {have}",
+                  file=sys.stderr)
+            sys.exit(2)
+    cmd = torchrun_cmd(args.gpus, argv)
+    os.execv(sys.executable, cmd)
+
+
 def dist_setup(n_gpus: int):
     world = int(os.environ.get("WORLD_SIZE", "1"))
     rank = int(os.environ.get("RANK", "0"))
     local = int(os.environ.get("LOCAL_RANK", "0"))
+    if world != max(n_gpus, 1):
+        print(f"bench.py: --gpus {n_gpus} but WORLD_SIZE={world}", file=sys.stderr)
+        sys.exit(2)
     if world > 1:
         import torch.distributed as dist
         os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
@@ -166,6 +217,13 @@ def dist_setup(n_gpus: int):
             torch.cuda.set_device(local)
         dist.init_process_group(backend=backend)
     return world, rank, local
+
+
+def dist_teardown(world):
+    if world > 1:
+        import torch.distributed as dist
+        if dist.is_initialized():
+            dist.destroy_process_group()
 
 
 def barrier(world):
@@ -186,7 +244,7 @@ def max_over_ranks(world, value: float) -> float:
 
 def aggregate_replicas(world: int, local_ms_total: float, steps: int):
     """N independent replicas: the timed region lasts as long as the slowest rank; in that
-    time the job advanced world*steps iterations.  Returns (ms_per_step of one replica, aggregate s/iter)."""
+    time the job advanced world*steps iterations.  Returns (ms_total, ms_per_step of one replica, aggregate s/iter)."""
     ms_total = max_over_ranks(world, local_ms_total)
     ms_step = ms_total / steps
     return ms_total, ms_step, ms_step * 1e-3 / world
@@ -202,9 +260,28 @@ def sum_over_ranks(world, value: float) -> float:
     return float(t.item())
 
 
+def run_plumbing_check(args):
+    """The multi-rank plumbing of this file without a GPU or the library (gloo on the CPU box): launch, process
+    group, barriers, max / sum over ranks, the replica normalisation.  tests/test_bench_dist.py runs it."""
+    world, rank, local = dist_setup(args.gpus)
+    barrier(world)
+    ms_total, ms_step, value = aggregate_replicas(world, 10.0 * (rank + 1), args.steps)
+    launches = sum_over_ranks(world, 100 + rank)
+    barrier(world)
+    if rank == 0:
+        print(json.dumps({"plumbing_check": True, "n_gpus": world, "steps": args.steps, "ms_total": ms_total,
+                          "ms_per_step": ms_step, "value": value, "launches": launches}))
+    dist_teardown(world)
+    return 0
+
+
 # ---------------------------------------------------------------------------------------------------
 # our arm
 # ---------------------------------------------------------------------------------------------------
+def ev():
+    return torch.cuda.Event(enable_timing=True)
+
+
 def time_dslash(lq, L, recon, reps, warm, links=None, field=None, slab=None):
     """ns/site and GB/s of one parity application: reps x (D_oe: b->t, D_eo: t->u) with fixed b
     (never fed back: |D| ~ 2.6 on random links would overflow).  slab = (L_global, rank, nranks): the same on a slab
@@ -219,7 +296,7 @@ def time_dslash(lq, L, recon, reps, warm, links=None, field=None, slab=None):
     for _ in range(warm):
         lat.doe(b, out=t)
         lat.deo(t, out=u)
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0, e1 = ev(), ev()
     torch.cuda.current_stream().synchronize()
     n0 = lat.launches
     e0.record()
@@ -233,20 +310,21 @@ def time_dslash(lq, L, recon, reps, warm, links=None, field=None, slab=None):
     lat.close()
     ns_site = ms * 1e6 / lat.Vh
     return {"us_per_application": ms * 1e3, "ns_per_site": ns_site,
-            "gbs_algorithmic": DSLASH_BYTES[recon] / ns_site,
             "gbs_dram_model": DSLASH_DRAM_MODEL[recon] / ns_site,
+            "gbs_algorithmic": DSLASH_BYTES[recon] / ns_site,
             "gflops": DSLASH_FLOPS[recon] / ns_site, "launches": launches,
-            "bytes_per_launch": DSLASH_BYTES[recon] * lat.Vh}
+            "dram_bytes_per_launch": DSLASH_DRAM_MODEL[recon] * lat.Vh,
+            "algorithmic_bytes_per_launch": DSLASH_BYTES[recon] * lat.Vh}
 
 
-def read_only_reference_gbs():
-    """Context for the roofline: what a plain read-only stream reaches on this GPU (torch.sum over 4 GiB of doubles,
-    best of 10, CUDA events).  The measured peak of MEASURED_PEAKS.json is a COPY (half writes); the Dslash is 97 %
-    reads."""
-    a = torch.ones(1 << 29, dtype=torch.float64, device="cuda")
+def read_stream_gbs(nbytes: int, reps: int = 10):
+    """What a plain read-only stream reaches on this GPU over a buffer of nbytes (torch.sum over doubles, best of
+    `reps` after 3 warm-up passes, CUDA events).  4 GiB: HBM (the measured peak of MEASURED_PEAKS.json is a COPY, half
+    writes; the Dslash is 97 % reads).  40 MB: the buffer stays in L2 (126 MB), i.e. an L2 read stream."""
+    a = torch.ones(nbytes // 8, dtype=torch.float64, device="cuda")
     best = 0.0
-    for i in range(13):
-        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    for i in range(reps + 3):
+        e0, e1 = ev(), ev()
         e0.record()
         a.sum()
         e1.record()
@@ -257,11 +335,46 @@ def read_only_reference_gbs():
     return best
 
 
+def time_small(lq, peak):
+    """The small-lattice regime (SURVEY.md §7 "Small lattices are launch-bound", BASELINE config 2): the whole 16^4
+    solve, and the same 8 shifts at 32^4 (400 iterations, then the whole solve).  At 16^4 links (37.7 MB) and
+    vectors live in L2, so the rate is quoted against an L2 read stream measured here, not against HBM."""
+    cfg = gen.CONFIGS["config2_16^4"]
+    out = {"l2_read_stream_gbs_40MB": read_stream_gbs(40 << 20, reps=20)}
+    for name, L in (("16x16x16x16", cfg["L"]), ("32x32x32x32", (32, 32, 32, 32))):
+        U, f = gen.random_su3_links(L, device="cuda"), gen.gaussian_field(L, device="cuda")
+        lat = lq.Lattice(L, mass=cfg["mass"])
+        lat.set_gauge(U)
+        b = lat.pack(f, 0)
+        x = lat.new_vector(len(cfg["shifts"]))
+        m = int(lat.get_option(lq.LQCD_OPT_SHIFT_BLOCK))
+        lat.set_option(lq.LQCD_OPT_MAX_ITER, 32)
+        lat.mshift_cg(b, cfg["shifts"], cfg["tol"], x=x, raise_on_noconv=False)
+        lat.set_option(lq.LQCD_OPT_MAX_ITER, 400)
+        _, first = lat.mshift_cg(b, cfg["shifts"], cfg["tol"], x=x, raise_on_noconv=False)
+        lat.set_option(lq.LQCD_OPT_MAX_ITER, 100000)
+        _, full = lat.mshift_cg(b, cfg["shifts"], cfg["tol"], x=x, raise_on_noconv=False)
+        moved = cg_dram_bytes(full["freeze_iter"], full["iters"], m, 18) * lat.Vh
+        gbs = moved / (full["solve_ms"] * 1e6)
+        out[name] = {"iters": full["iters"], "status": full["status"], "rel_res": full["rel_res"],
+                     "s_per_iter": full["solve_ms"] * 1e-3 / max(full["iters"], 1),
+                     "s_per_iter_first_400": first["solve_ms"] * 1e-3 / max(first["iters"], 1),
+                     "solve_s": full["solve_ms"] * 1e-3, "freeze_iter": full["freeze_iter"],
+                     "gbs_moved": gbs, "frac_of_hbm_peak": gbs / peak,
+                     "frac_of_l2_read_stream": gbs / out["l2_read_stream_gbs_40MB"],
+                     "launches_per_iter": 2 + 1.0 / m}
+        lat.close()
+        del U, f, x, b
+    out["note"] = ("config 2 (16^4, m=0.01, 8 shifts, tol 1e-10) whole solve, and the same at 32^4; gbs_moved = bytes the "
+                   "iteration touches (cg_dram_bytes) / time: at 16^4 they are served by L2, hence the L2 read stream "
+                   "beside it")
+    return out
+
+
 def time_next_rows(lq, L, mass, shifts, tol, K, W, U, f):
     """The widened rows on the same workload, K iterations / applications each, device time:
     NEXT-1 rational sum, NEXT-2 single precision (Dslash and CG), NEXT-4 general U(1) phases (Dslash)."""
     res = {}
-    ev = lambda: torch.cuda.Event(enable_timing=True)
 
     def dslash_ns(lat, b, reps=max(K // 2, 20)):
         t, u = torch.empty_like(b), torch.empty_like(b)
@@ -365,6 +478,7 @@ def run_ours(args, world, rank, local):
         lat.set_gauge(U)
         b = lat.pack(f, 0)
         x = lat.new_vector(len(shifts))
+        m_blk = int(lat.get_option(lq.LQCD_OPT_SHIFT_BLOCK))
 
         phase('inputs drawn, gauge stored')
         # ---- warm-up: W iterations (also builds the CUDA graph)
@@ -376,7 +490,7 @@ def run_ours(args, world, rank, local):
         torch.cuda.synchronize()
         barrier(world)
         n0 = lat.launches
-        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0, e1 = ev(), ev()
         with ClockSampler(local) as clocks:
             e0.record()
             _, info = lat.mshift_cg(b, shifts, tol, x=x, raise_on_noconv=False)
@@ -387,13 +501,12 @@ def run_ours(args, world, rank, local):
         ms_total, _, _ = aggregate_replicas(world, e0.elapsed_time(e1), K)
         launches = lat.launches - n0
         sched = n_active_schedule(info["freeze_iter"], K)
-        bytes_total = sum(cg_bytes_per_site(n, recon) for n in sched) * lat.Vh
-        m_blk = int(lat.get_option(lq.LQCD_OPT_SHIFT_BLOCK))
-        bytes_moved = cg_bytes_moved(info["freeze_iter"], K, m_blk, recon) * lat.Vh
+        bytes_method = sum(cg_bytes_per_site(n, recon) for n in sched) * lat.Vh
+        bytes_dram = cg_dram_bytes(info["freeze_iter"], K, m_blk, recon) * lat.Vh
         out["timed"] = dict(ms_total=ms_total, launches=launches, launches_all=int(sum_over_ranks(world, launches)),
-                            n_active_mean=sum(sched) / K, shift_block=m_blk,
-                            gbs_algorithmic=bytes_total / (ms_total * 1e6),
-                            gbs_moved=bytes_moved / (ms_total * 1e6), kernel_ms=info["solve_ms"])
+                            n_active_mean=sum(sched) / K, shift_block=m_blk, bytes_dram=bytes_dram,
+                            gbs_method_equivalent=bytes_method / (ms_total * 1e6),
+                            gbs_dram=bytes_dram / (ms_total * 1e6), kernel_ms=info["solve_ms"])
 
         phase('timed region done')
         # ---- e2e: same K iterations through the host-pointer entry point (rank-local, then max)
@@ -415,21 +528,48 @@ def run_ours(args, world, rank, local):
         assert info_h["iters"] == K
         assert torch.equal(x_host, x.cpu()), "host entry point and device entry point disagree"
         out["e2e"] = dict(ms_total=e2e_ms, h2d=b_host.numel() * 8, d2h=x_host.numel() * 8)
-        del b_host, x_host
+        del x_host
+        # what the RHMC calls: the rational function applied to a host vector, one vector back
+        if not slab:
+            alpha = [1.0 / (1 + i) for i in range(len(shifts))]
+            y_host = torch.empty(b.shape, dtype=torch.float64, pin_memory=True)
+            lat.set_option(lq.LQCD_OPT_MAX_ITER, max(W, 3))
+            lat.rational_apply(b_host, 0.5, alpha, shifts, tol, y=y_host, raise_on_noconv=False)
+            lat.set_option(lq.LQCD_OPT_MAX_ITER, K)
+            torch.cuda.synchronize()
+            t0 = time.perf_counter()
+            e0.record()
+            _, info_r = lat.rational_apply(b_host, 0.5, alpha, shifts, tol, y=y_host, raise_on_noconv=False)
+            e1.record()
+            torch.cuda.synchronize()
+            wall_ms = (time.perf_counter() - t0) * 1e3
+            out["e2e_rational"] = dict(ms_total=max(e0.elapsed_time(e1), wall_ms), iters=info_r["iters"],
+                                       h2d=b_host.numel() * 8, d2h=y_host.numel() * 8, kernel_ms=info_r["solve_ms"])
+            del y_host
+        del b_host
 
         phase('e2e done')
+        if rank == 0 or slab:
+            # ---- the same over a whole number of shift blocks (the driver's K need not be one)
+            Ks = 96
+            lat.set_option(lq.LQCD_OPT_MAX_ITER, Ks)
+            _, st = lat.mshift_cg(b, shifts, tol, x=x, raise_on_noconv=False)
+            out["steady"] = dict(iters=st["iters"], s_per_iter=st["solve_ms"] * 1e-3 / max(st["iters"], 1),
+                                 gbs_dram=cg_dram_bytes(st["freeze_iter"], st["iters"], m_blk, recon) * lat.Vh
+                                 / (st["solve_ms"] * 1e6))
         if (rank == 0 or slab) and not args.quick:
             # ---- the same solve to convergence (what a user runs): average s/iter, iteration count
             lat.set_option(lq.LQCD_OPT_MAX_ITER, 100000)
             _, full = lat.mshift_cg(b, shifts, tol, x=x, raise_on_noconv=False)
             sched_f = n_active_schedule(full["freeze_iter"], full["iters"])
             bytes_f = sum(cg_bytes_per_site(n, recon) for n in sched_f) * lat.Vh
-            moved_f = cg_bytes_moved(full["freeze_iter"], full["iters"], m_blk, recon) * lat.Vh
+            moved_f = cg_dram_bytes(full["freeze_iter"], full["iters"], m_blk, recon) * lat.Vh
             out["full_solve"] = dict(iters=full["iters"], status=full["status"], rel_res=full["rel_res"],
                                      s_per_iter=full["solve_ms"] * 1e-3 / max(full["iters"], 1),
                                      solve_s=full["solve_ms"] * 1e-3, n_active_mean=sum(sched_f) / max(len(sched_f), 1),
-                                     gbs_algorithmic=bytes_f / (full["solve_ms"] * 1e6),
-                                     gbs_moved=moved_f / (full["solve_ms"] * 1e6),
+                                     gbs_method_equivalent=bytes_f / (full["solve_ms"] * 1e6),
+                                     gbs_dram=moved_f / (full["solve_ms"] * 1e6),
+                                     frac_of_peak_dram=moved_f / (full["solve_ms"] * 1e6) / peak,
                                      freeze_iter=full["freeze_iter"])
         lat.close()
 
@@ -441,10 +581,12 @@ def run_ours(args, world, rank, local):
             lat2.set_gauge(U)
             lat2.set_option(lq.LQCD_OPT_MAX_ITER, max(W, 3))
             lat2.mshift_cg(b, shifts, tol, x=x, raise_on_noconv=False)
-            lat2.set_option(lq.LQCD_OPT_MAX_ITER, K)
+            lat2.set_option(lq.LQCD_OPT_MAX_ITER, max(K, 96))
             _, info2 = lat2.mshift_cg(b, shifts, tol, x=x, raise_on_noconv=False)
-            out[f"cg_recon{other}"] = dict(s_per_iter=info2["solve_ms"] * 1e-3 / max(info2["iters"], 1), iters=info2["iters"],
-                                           note=f"same {K} iterations with {other}-real links, device time of the solve")
+            out[f"cg_recon{other}"] = dict(
+                s_per_iter=info2["solve_ms"] * 1e-3 / max(info2["iters"], 1), iters=info2["iters"],
+                gbs_dram=cg_dram_bytes(info2["freeze_iter"], info2["iters"], m_blk, other) * lat2.Vh / (info2["solve_ms"] * 1e6),
+                note=f"{info2['iters']} iterations with {other}-real links, device time of the solve")
             lat2.close()
         del x
 
@@ -463,15 +605,17 @@ def run_ours(args, world, rank, local):
         phase('dslash at workload size done')
         if rank == 0 and not args.quick and not slab:
             out["next_rows"] = time_next_rows(lq, L, mass, shifts, tol, K, W, U, f)
-            out["read_only_gbs"] = read_only_reference_gbs()
-        del U, f
+            out["read_only_gbs"] = read_stream_gbs(4 << 30)
+        del U, f, b
         phase('next rows done')
         if rank == 0 and not args.quick and args.workload == "config4_48^4":
             L3 = gen.CONFIGS["config3_32^4"]["L"]
             U3, f3 = gen.random_su3_links(L3, device="cuda"), gen.gaussian_field(L3, device="cuda")
             ds["32x32x32x32"] = {f"recon{r}": time_dslash(lq, L3, r, 500, 20, U3, f3) for r in (18, 12)}
             del U3, f3
+            out["small"] = time_small(lq, peak)
         out["dslash"] = ds
+        phase('small lattices done')
     out["clocks"] = clocks.summary()
     out["peak"] = (peak, peak_src)
     out["cfg"] = dict(L=L, mass=mass, nshift=len(shifts), tol=tol, recon=recon)
@@ -479,10 +623,152 @@ def run_ours(args, world, rank, local):
 
 
 # ---------------------------------------------------------------------------------------------------
+# NEXT-3 on the GPUs of this node: a guarded sub-run (a hang in a collective cannot lose the headline line)
+# ---------------------------------------------------------------------------------------------------
+def run_slab_check(args):
+    """Runs as its own set of N ranks (`bench.py --slab-check --gpus N` under torchrun; N = 1 closes the ring on
+    itself).  (1) parity on a 16^3 x 4N lattice: the gathered D_oe of the N slabs against the single-GPU kernel
+    (bit for bit) and against the oracle, then 20 CG iterations against the oracle at a fixed count; (2) timing of
+    ONE Lx*Ly*Lz*(Lt*N) lattice of the workload: operator us, CG s/iter, face bytes.  Prints {"slab": {...}}."""
+    import numpy as np
+    import oracle
+    import paper_1801_01473_b200 as lq
+    import torch.distributed as dist
+    world, rank, local = dist_setup(args.gpus)
+    torch.cuda.set_device(local)
+    res = {"n_ranks": world}
+    with torch.cuda.stream(torch.cuda.Stream()):
+        # ---- (1) parity
+        Lp = (16, 16, 16, 4 * world)
+        mass, shifts = 0.05, [1e-3, 1e-2, 1e-1, 1.0]
+        U, f = gen.random_su3_links(Lp), gen.gaussian_field(Lp)
+        b_aos = oracle.restrict(Lp, 0, f.numpy())
+        b_whole = torch.as_tensor(oracle.aos_to_soa(b_aos)).cuda()
+        lat = lq.Lattice(Lp, mass=mass, slab=(rank, world), comm="nccl")
+        lat.set_gauge(lq.Lattice.slab_of_links(U, Lp, rank, world).cuda())
+        b = lq.Lattice.slab_of_vector(b_whole, Lp, rank, world)
+        t = lat.doe(b)
+        lat.set_option(lq.LQCD_OPT_MAX_ITER, 20)
+        x, info = lat.mshift_cg(b, shifts, 1e-30, raise_on_noconv=False)
+        torch.cuda.synchronize()
+
+        def gather(v):                      # (..., 3, Vh_loc, 2) slabs -> whole-lattice vector on every rank
+            if world == 1:
+                return v
+            parts = [torch.empty_like(v) for _ in range(world)]
+            dist.all_gather(parts, v.contiguous())
+            return torch.cat(parts, dim=-2)
+
+        t_all, x_all = gather(t), gather(x)
+        lat.close()
+        if rank == 0:
+            whole = lq.Lattice(Lp, mass=mass)
+            whole.set_gauge(U.cuda())
+            t_one = whole.doe(b_whole)
+            whole.close()
+            rel = lambda a, r: float(np.linalg.norm(a - r) / np.linalg.norm(r))
+            t_ref = oracle.doe(Lp, U.numpy(), b_aos)
+            x_ref, i_ref = oracle.mshift_cg(Lp, U.numpy(), mass, b_aos, shifts, 1e-30, max_iter=20)
+            res["parity"] = {
+                "lattice": list(Lp),
+                "doe_bit_identical_to_single_gpu_kernel": bool(torch.equal(t_all, t_one)),
+                "doe_rel_err_vs_oracle": rel(oracle.soa_to_aos(t_all.cpu().numpy()), t_ref),
+                "cg20_max_rel_err_vs_oracle": max(rel(oracle.soa_to_aos(x_all[i].cpu().numpy()), x_ref[i])
+                                                  for i in range(len(shifts))),
+                "cg_iters": info["iters"], "oracle_iters": i_ref["iters"]}
+            p = res["parity"]
+            p["ok"] = bool(p["doe_bit_identical_to_single_gpu_kernel"] and p["doe_rel_err_vs_oracle"] <= 1e-12
+                           and p["cg20_max_rel_err_vs_oracle"] <= 1e-11 and p["cg_iters"] == p["oracle_iters"] == 20)
+        del U, f
+        # ---- (2) timing at the workload size, weak scaling along t
+        cfg = gen.CONFIGS[args.workload]
+        L = cfg["L"]
+        Lg = tuple(L[:3]) + (L[3] * world,)
+        U = gen.random_su3_links_slab(Lg, rank, world, device="cuda")
+        f = gen.gaussian_field_slab(Lg, rank, world, device="cuda")
+        lat = lq.Lattice(Lg, mass=cfg["mass"], recon=args.recon, slab=(rank, world), comm="nccl")
+        lat.set_gauge(U)
+        b = lat.pack(f, 0)
+        x = lat.new_vector(len(cfg["shifts"]))
+        lat.set_option(lq.LQCD_OPT_MAX_ITER, max(args.warmup, 3))
+        lat.mshift_cg(b, cfg["shifts"], cfg["tol"], x=x, raise_on_noconv=False)
+        lat.set_option(lq.LQCD_OPT_MAX_ITER, args.steps)
+        torch.cuda.synchronize()
+        barrier(world)
+        e0, e1 = ev(), ev()
+        e0.record()
+        _, info = lat.mshift_cg(b, cfg["shifts"], cfg["tol"], x=x, raise_on_noconv=False)
+        e1.record()
+        torch.cuda.synchronize()
+        barrier(world)
+        ms = max_over_ranks(world, e0.elapsed_time(e1))
+        tt, uu = torch.empty_like(b), torch.empty_like(b)
+        for _ in range(3):
+            lat.doe(b, out=tt)
+            lat.deo(tt, out=uu)
+        torch.cuda.synchronize()
+        barrier(world)
+        reps = 20
+        e0.record()
+        for _ in range(reps):
+            lat.doe(b, out=tt)
+            lat.deo(tt, out=uu)
+        e1.record()
+        torch.cuda.synchronize()
+        op_us = max_over_ranks(world, e0.elapsed_time(e1)) * 1e3 / (2 * reps)
+        face = L[0] * L[1] * L[2] // 2 * 48
+        res["timing"] = {"lattice": list(Lg), "iters": info["iters"], "s_per_iter": ms * 1e-3 / max(info["iters"], 1),
+                         "s_per_iter_per_gpu_volume": ms * 1e-3 / max(info["iters"], 1) / world,
+                         "operator_us": op_us, "face_bytes_each_way": face,
+                         "face_bytes_per_application": 2 * face, "transport": "NCCL send/recv + all-reduce"}
+        lat.close()
+    barrier(world)
+    if rank == 0:
+        print(json.dumps({"slab": res}))
+    dist_teardown(world)
+    return 0
+
+
+def guarded_slab_run(args, n: int, timeout_s: float = 600.0):
+    """rank 0 of the headline run: start the slab check as a separate set of n ranks and wait at most timeout_s."""
+    argv = ["--slab-check", "--gpus", str(n), "--steps", str(args.steps), "--warmup", str(args.warmup),
+            "--workload", args.workload, "--recon", str(args.recon)]
+    cmd = torchrun_cmd(n, argv) if n > 1 else [sys.executable, os.path.abspath(__file__)] + argv
+    env = {k: v for k, v in os.environ.items()
+           if k not in ("RANK", "LOCAL_RANK", "WORLD_SIZE", "MASTER_ADDR", "MASTER_PORT", "GROUP_RANK", "ROLE_RANK",
+                        "LOCAL_WORLD_SIZE", "ROLE_WORLD_SIZE", "TORCHELASTIC_RUN_ID", "TORCHELASTIC_RESTART_COUNT",
+                        "TORCHELASTIC_MAX_RESTARTS", "TORCHELASTIC_USE_AGENT_STORE", "TORCHELASTIC_ERROR_FILE")}
+    env.setdefault("NCCL_DEBUG", "INFO")                 # NCCL's own log (rank count, transports) goes to stderr
+    env.setdefault("NCCL_DEBUG_SUBSYS", "INIT")
+    t0 = time.perf_counter()
+    try:
+        p = subprocess.run(cmd, env=env, stdout=subprocess.PIPE, stderr=sys.stderr, timeout=timeout_s, text=True)
+    except subprocess.TimeoutExpired:
+        return {"error": f"slab sub-run did not finish within {timeout_s:.0f} s (killed)", "n_ranks": n}
+    for line in reversed(p.stdout.splitlines()):
+        if line.startswith("{") and '"slab"' in line:
+            d = json.loads(line)["slab"]
+            d["wall_s"] = time.perf_counter() - t0
+            return d
+    return {"error": f"slab sub-run exited {p.returncode} without a result", "n_ranks": n}
+
+
+# ---------------------------------------------------------------------------------------------------
 # the CPU oracle (cpu_baseline leg, and the whole of --impl reference)
 # ---------------------------------------------------------------------------------------------------
+def cpu_model() -> str:
+    try:
+        with open("/proc/cpuinfo") as fh:
+            for line in fh:
+                if line.startswith("model name"):
+                    return line.split(":", 1)[1].strip()
+    except OSError:
+        pass
+    return "unknown"
+
+
 def run_oracle(workload: str, budget_s: float, steps: int | None, warmup: int = 0):
-    """Times the oracle's multi-shift CG on the workload's inputs.  Returns (s_per_iter, description).
+    """Times the oracle's multi-shift CG on the workload's inputs.  Returns (s_per_iter, cores, description, iters).
     Without `steps`, the number of iterations is chosen so that the run takes about budget_s."""
     import oracle
     cfg = gen.CONFIGS[workload]
@@ -513,6 +799,48 @@ def run_oracle(workload: str, budget_s: float, steps: int | None, warmup: int = 
     return dt / info["iters"], cores, sample, info["iters"]
 
 
+def run_oracle_extras():
+    """SURVEY.md §8(d) "Oracle timing": the oracle's D_oe/D_eo pair at 32^4 -> ns/site on all cores and on one
+    thread; the whole BASELINE config 2 solve (16^4) -> s/iter and iteration count."""
+    import oracle
+    out = {"nproc": os.cpu_count(), "cpu_model": cpu_model()}
+    dev = "cuda" if torch.cuda.is_available() else "cpu"
+    cores = oracle.num_threads()
+    L = gen.CONFIGS["config3_32^4"]["L"]
+    U = gen.random_su3_links(L, device=dev).cpu().numpy()
+    b = oracle.restrict(L, 0, gen.gaussian_field(L, device=dev).cpu().numpy())
+    vh = b.shape[0]
+
+    def pair_ns(reps):
+        t = oracle.doe(L, U, b)
+        oracle.deo(L, U, t)
+        t0 = time.perf_counter()
+        for _ in range(reps):
+            t = oracle.doe(L, U, b)
+            oracle.deo(L, U, t)
+        return (time.perf_counter() - t0) / (2 * reps) / vh * 1e9
+
+    out["dslash_ns_per_site"] = pair_ns(10)
+    out["dslash_sample"] = f"10 x (D_oe, D_eo) at 32^4 on {cores} threads"
+    try:
+        oracle.set_num_threads(1)
+        out["dslash_ns_per_site_1thread"] = pair_ns(2)
+    finally:
+        oracle.set_num_threads(cores)
+    del U, b
+    cfg = gen.CONFIGS["config2_16^4"]
+    L = cfg["L"]
+    U = gen.random_su3_links(L, device=dev).cpu().numpy()
+    b = oracle.restrict(L, 0, gen.gaussian_field(L, device=dev).cpu().numpy())
+    t0 = time.perf_counter()
+    _, info = oracle.mshift_cg(L, U, cfg["mass"], b, cfg["shifts"], cfg["tol"])
+    dt = time.perf_counter() - t0
+    out["cg16_s_per_iter"] = dt / max(info["iters"], 1)
+    out["cg16_iters"] = info["iters"]
+    out["cg16_sample"] = f"whole config-2 solve (16^4, 8 shifts, tol 1e-10) on {cores} threads, {dt:.1f} s"
+    return out
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -528,9 +856,18 @@ def main():
     ap.add_argument("--next-rows-only", action="store_true",
                     help="run only the widened rows (rational sum, f32, U(1) phases) and print their JSON object "
                          "(used for the ncu captures of those kernels)")
-    ap.add_argument("--quick", action="store_true", help="skip the full solve, the 32^4 table and the CPU baseline")
+    ap.add_argument("--quick", action="store_true", help="skip the full solve, the 32^4 / small tables and the CPU baseline")
     ap.add_argument("--cpu-budget", type=float, default=20.0, help="seconds of oracle time for cpu_baseline")
+    ap.add_argument("--with-slab", action="store_true",
+                    help="also run the guarded slab sub-run when N = 1 (it always runs when N > 1)")
+    ap.add_argument("--slab-check", action="store_true", help=argparse.SUPPRESS)
+    ap.add_argument("--plumbing-check", action="store_true", help=argparse.SUPPRESS)
     args = ap.parse_args()
+    self_launch(args, sys.argv[1:])
+    if args.plumbing_check:
+        return run_plumbing_check(args)
+    if args.slab_check:
+        return run_slab_check(args)
     if args.next_rows_only:
         import paper_1801_01473_b200 as lq
         cfg = gen.CONFIGS[args.workload]
@@ -551,8 +888,8 @@ def main():
     config = {"workload": f"{args.workload}: {lname} lattice, multi-shift CG with {len(cfg['shifts'])} shifts "
                           f"(geometric {cfg['shifts'][0]:g}..{cfg['shifts'][-1]:g}), m={cfg['mass']}, tol={cfg['tol']:g}, "
                           f"{args.recon}-real links, seeded random SU(3) links + Gaussian even-site source",
-              "step": "one multi-shift CG iteration (D_oe, D_eo+epilogue, scalar recurrences, r update, base x/p update, "
-                      "1/m of the block sweep over the shifted x_i/p_i)",
+              "step": "one multi-shift CG iteration (D_oe and D_eo with all sums and scalar products fused in, scalar "
+                      "recurrences, 1/m of the block sweep over the x_i/p_i)",
               "lattice": list(cfg["L"]), "nshift": len(cfg["shifts"]), "mass": cfg["mass"], "tol": cfg["tol"],
               "recon": args.recon,
               "parallelism": (f"1-D slabs along t: ONE {lname[:lname.rfind('x')]}x{cfg['L'][3] * world} lattice over {world} "
@@ -573,58 +910,81 @@ def main():
         return 0
 
     res = run_ours(args, world, rank, local)
+    # the headline is complete on every rank; the other ranks are done (rank 0 alone finishes the report, and the slab
+    # sub-run needs their GPUs idle)
+    barrier(world)
+    dist_teardown(world)
     if rank != 0:
-        barrier(world)
         return 0
     K, W = args.steps, args.warmup
     peak, peak_src = res["peak"]
     ms_step = res["timed"]["ms_total"] / K
     value = ms_step * 1e-3 / world                     # replicas: N solves advance one iteration per ms_step
     ds_main = res["dslash"][lname][f"recon{args.recon}"]
-    bytes_per_launch = ds_main["bytes_per_launch"]
-    achieved = ds_main["gbs_algorithmic"]
-    traffic = NCU_DRAM_BYTES_PER_LAUNCH.get((args.workload, args.recon))
+    achieved = ds_main["gbs_dram_model"]
+    ncu = NCU_DRAM_GB_PER_LAUNCH.get((args.workload, args.recon))
+    read_ref = res.get("read_only_gbs")
     line = {
         "metric": "mshift_cg_s_per_iter", "value": value, "unit": "s/iter", "n_gpus": world, "steps": K, "warmup": W,
         "ms_per_step": ms_step, "higher_is_better": False, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
         "data": "synthetic", "config": config,
         "clocks": res["clocks"],
+        "value_steady": res["steady"]["s_per_iter"] / world if "steady" in res else None,
         "e2e": {"value": res["e2e"]["ms_total"] * 1e-3 / K / world, "unit": "s/iter",
                 "h2d_bytes_per_step": res["e2e"]["h2d"] / K, "d2h_bytes_per_step": res["e2e"]["d2h"] / K,
                 "note": "lqcd_mshift_cg_host: pinned-host b in, 16 pinned-host solutions out, K iterations per call"},
         "gpu_launches": res["timed"]["launches_all"],
-        "roofline": {"bound": "hbm", "kernel": f"dslash_kernel<{args.recon},0|1> (D_oe / D_eo) at {lname}",
+        "roofline": {"bound": "hbm", "kernel": f"dslash_kernel<{args.recon},0> (D_oe / D_eo) at {lname}",
                      "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                     "traffic": traffic, "peak_source": peak_src,
-                     "bytes_per_launch": bytes_per_launch, "us_per_launch": ds_main["us_per_application"],
+                     "traffic": (ncu[0] + ncu[1]) * 1e9 if ncu else None,
+                     "traffic_source": ncu[2] if ncu else None,
+                     "peak_source": peak_src,
+                     "bytes_per_launch": ds_main["dram_bytes_per_launch"], "us_per_launch": ds_main["us_per_application"],
                      "ns_per_site": ds_main["ns_per_site"],
-                     "achieved_dram_model": ds_main["gbs_dram_model"], "frac_dram_model": ds_main["gbs_dram_model"] / peak,
+                     "bytes_per_site": DSLASH_DRAM_MODEL[args.recon],
+                     "achieved_algorithmic": ds_main["gbs_algorithmic"], "frac_algorithmic": ds_main["gbs_algorithmic"] / peak,
+                     "algorithmic_bytes_per_site": DSLASH_BYTES[args.recon],
                      "frac_of_nominal_8000": achieved / 8000.0,
-                     "read_only_reference_gbs": res.get("read_only_gbs"),
-                     "note": "achieved = algorithmic bytes (8 links + 8 neighbour vectors + 1 output per site) / event "
-                             "time; the 8 neighbour-vector reads are mostly L2 hits, achieved_dram_model counts each "
-                             "input vector once (what DRAM must deliver)"},
-        "cg": {"n_active_mean": res["timed"]["n_active_mean"], "shift_block": res["timed"]["shift_block"],
-               "gbs_algorithmic": res["timed"]["gbs_algorithmic"], "gbs_moved": res["timed"]["gbs_moved"],
-               "frac_of_peak_moved": res["timed"]["gbs_moved"] / peak,
-               "note": "gbs_algorithmic: bytes of the per-iteration method (SURVEY.md 8(d): 3600+192(n_act-1) B/site) / time, "
-                       "an equivalent rate; gbs_moved: bytes the block-deferred updates actually move / time"},
+                     "read_only_reference_gbs": read_ref,
+                     "frac_of_read_only_stream": achieved / read_ref if read_ref else None,
+                     "note": "achieved = DRAM-compulsory bytes (8 links + 1 input vector + 1 output per site, SURVEY.md "
+                             "8(d) 'each input once') / event time; peak is a COPY (half writes) while this kernel is 96 % "
+                             "reads, hence frac slightly above 1 -- see frac_of_read_only_stream and frac_of_nominal_8000; "
+                             "achieved_algorithmic also counts the 8 neighbour-vector reads that L1/L2 serve and is not an "
+                             "HBM fraction"},
+        "cg_roofline": {"bound": "hbm", "achieved": res["timed"]["gbs_dram"], "peak": peak, "unit": "GB/s",
+                        "frac": res["timed"]["gbs_dram"] / peak,
+                        "bytes_per_iteration": res["timed"]["bytes_dram"] / K, "n_active_mean": res["timed"]["n_active_mean"],
+                        "shift_block": res["timed"]["shift_block"],
+                        "steady_achieved": res["steady"]["gbs_dram"] if "steady" in res else None,
+                        "method_equivalent_gbs": res["timed"]["gbs_method_equivalent"],
+                        "note": "achieved = DRAM-compulsory bytes of the K timed iterations as the library runs them "
+                                "(cg_dram_bytes: two fused operator sweeps + block sweeps, from the recorded freeze schedule) "
+                                "/ time; method_equivalent_gbs = bytes of the method as the paper states it (SURVEY.md 8(d): "
+                                "3600+192(n_act-1) B/site per iteration) / time, an equivalent rate, not an HBM fraction"},
         "dslash": res["dslash"],
     }
-    if "full_solve" in res:
-        line["full_solve"] = res["full_solve"]
-    if "dslash_slab" in res:
-        line["dslash_slab"] = res["dslash_slab"]
-    for key in ("cg_recon12", "cg_recon18", "next_rows"):
+    if "e2e_rational" in res:
+        er = res["e2e_rational"]
+        line["e2e_rational"] = {"value": er["ms_total"] * 1e-3 / max(er["iters"], 1), "unit": "s/iter", "iters": er["iters"],
+                                "h2d_bytes_per_step": er["h2d"] / max(er["iters"], 1),
+                                "d2h_bytes_per_step": er["d2h"] / max(er["iters"], 1),
+                                "device_s_per_iter": er["kernel_ms"] * 1e-3 / max(er["iters"], 1),
+                                "note": "lqcd_rational_apply_host: pinned-host b in, ONE pinned-host vector out (the call "
+                                        "the RHMC makes, PAPER.md:L82), K iterations per call, wall clock"}
+    for key in ("full_solve", "dslash_slab", "cg_recon12", "cg_recon18", "next_rows", "small"):
         if key in res:
             line[key] = res[key]
     phase("GPU part done")
+    if world > 1 or args.with_slab:
+        line["slab"] = guarded_slab_run(args, world)
+        phase("slab sub-run done")
     if not args.quick and world == 1:
         s_iter, cores, sample, _ = run_oracle(args.workload, budget_s=args.cpu_budget, steps=None)
         line["cpu_baseline"] = {"value": s_iter, "unit": "s/iter", "cores": cores, "kind": "oracle", "sample": sample}
+        line["cpu_baseline"].update(run_oracle_extras())
     phase("CPU baseline done")
     print(json.dumps(line))
-    barrier(world)
     return 0
 
 

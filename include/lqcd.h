@@ -81,11 +81,11 @@ typedef struct lqcd_ctx lqcd_ctx;
 #define LQCD_OPT_LINK_PRECISIONS 6  /* which copies of the links the next lqcd_set_gauge stores: LQCD_PREC_F64
                                        (default; serves the double entry points), LQCD_PREC_F32 (serves the
                                        *_f32 entry points), or both OR-ed together                         */
-#define LQCD_OPT_SHIFT_BLOCK     7  /* m in [1,16], default 8: the x_i, p_i of the shifted systems are updated once
-                                       per block of m iterations from the m residuals of the block (kept in m
-                                       extra vectors) instead of once per iteration; same recurrences, same
-                                       iteration counts, x_i equal up to rounding.  m = 1: every iteration.
-                                       CHECK_EVERY is rounded up to a multiple of m.                        */
+#define LQCD_OPT_SHIFT_BLOCK     7  /* m in [1,16], default 16: the x_i, p_i of the shifted systems (and x_0 of the
+                                       base system) are updated once per block of m iterations from the m
+                                       residuals of the block (kept in m vectors) instead of once per iteration;
+                                       same recurrences, same iteration counts, x_i equal up to rounding.
+                                       m = 1: every iteration.  CHECK_EVERY is rounded up to a multiple of m. */
 #define LQCD_PREC_F64 1
 #define LQCD_PREC_F32 2
 
@@ -111,7 +111,11 @@ int lqcd_get_option(const lqcd_ctx* ctx, int key, double* value /*HOST*/);
 /* Device memory.  By default the library allocates what it needs with cudaMalloc.  Alternatively the
  * caller provides one arena of at least lqcd_workspace_bytes(ctx, nshift) bytes (256-byte aligned) that
  * then holds the stored links and all solver temporaries for up to nshift shifts; it must stay valid
- * until lqcd_destroy or the next lqcd_set_workspace.  Must be called before lqcd_set_gauge. */
+ * until lqcd_destroy or the next lqcd_set_workspace.  Must be called before lqcd_set_gauge.
+ * The size depends on LQCD_OPT_SHIFT_BLOCK and LQCD_OPT_LINK_PRECISIONS: set both BEFORE the query and do not
+ * raise them afterwards (lqcd_mshift_cg_mixed needs both precisions).  The device staging copies of the *_host
+ * entry points and of lqcd_mshift_cg_mixed (up to nshift + 2 vectors) are not part of the arena: the library
+ * allocates them with cudaMalloc on first use. */
 size_t lqcd_workspace_bytes(const lqcd_ctx* ctx, int nshift);
 int    lqcd_set_workspace(lqcd_ctx* ctx, void* dev, size_t bytes);
 

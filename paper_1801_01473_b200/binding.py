@@ -86,15 +86,14 @@ def library_path() -> str:
 
 
 def load_library():
-    """dlopen liblqcd_b200.so (building it with nvcc if it is not there).  Raises if that fails: there is
-    no other implementation to fall back to."""
+    """dlopen liblqcd_b200.so (building it with nvcc if it is missing or was built from other sources than the
+    ones in the tree now).  Raises if that fails: there is no other implementation to fall back to."""
     global _lib
     if _lib is not None:
         return _lib
     path = library_path()
-    if not os.path.exists(path):
-        from .build import build
-        build()
+    from .build import build
+    build()                              # returns at once when the library matches the sources
     lib = ctypes.CDLL(path)
     for name, (res, args) in EXPORTS.items():
         fn = getattr(lib, name)          # AttributeError if the symbol is missing

@@ -151,6 +151,16 @@ int dev_alloc(lqcd_ctx* c, void** out, size_t bytes) {
     return LQCD_OK;
 }
 
+// memory outside the caller's arena even when there is one: the staging copies of the *_host entry points
+// (lqcd_workspace_bytes does not count them)
+int dev_alloc_own(lqcd_ctx* c, void** out, size_t bytes) {
+    char* arena = c->arena;
+    c->arena = nullptr;
+    const int rc = dev_alloc(c, out, bytes);
+    c->arena = arena;
+    return rc;
+}
+
 void dev_free_owned(lqcd_ctx* c, void* p) {
     for (size_t i = 0; i < c->owned.size(); ++i)
         if (c->owned[i] == p) {
@@ -194,28 +204,33 @@ int cg_grid(const lqcd_ctx* c) {
 // buffers every call needs: the CG state, reduction partials, pinned mirrors, events
 int ensure_basics(lqcd_ctx* c) {
     if (c->basics) return LQCD_OK;
+    // every resource is created only if it does not exist yet: a call that failed half way can be repeated
     int rc;
-    if ((rc = dev_alloc(c, (void**)&c->st_dev, sizeof(CgState)))) return rc;
-    c->n_partials = (size_t)(ds_grid(c) > cg_grid(c) ? ds_grid(c) : cg_grid(c)) + 4;
-    if ((rc = dev_alloc(c, (void**)&c->partials, c->n_partials * sizeof(double)))) return rc;
-    if (c->slab) {
-        if ((rc = dev_alloc(c, (void**)&c->red, 2 * sizeof(double)))) return rc;
-        CU(cudaMallocHost((void**)&c->red_host, 2 * sizeof(double)));
-        CU(cudaStreamCreateWithFlags(&c->comm_stream, cudaStreamNonBlocking));
-        CU(cudaEventCreateWithFlags(&c->ev_pack, cudaEventDisableTiming));
-        CU(cudaEventCreateWithFlags(&c->ev_halo, cudaEventDisableTiming));
+    if (!c->st_dev) {
+        if ((rc = dev_alloc(c, (void**)&c->st_dev, sizeof(CgState)))) return rc;
+        CU(cudaMemsetAsync(c->st_dev, 0, sizeof(CgState), c->stream));
     }
-    if ((rc = dev_alloc(c, (void**)&c->dev_max, sizeof(double)))) return rc;
-    CU(cudaMemsetAsync(c->st_dev, 0, sizeof(CgState), c->stream));
-    CU(cudaMallocHost((void**)&c->st_host, sizeof(CgState)));
-    CU(cudaMallocHost((void**)&c->flag_host, 2 * sizeof(int)));
-    CU(cudaMallocHost((void**)&c->max_host, sizeof(double)));
-    CU(cudaEventCreateWithFlags(&c->ev[0], cudaEventDisableTiming));
-    CU(cudaEventCreateWithFlags(&c->ev[1], cudaEventDisableTiming));
-    CU(cudaEventCreate(&c->ev_t0));
-    CU(cudaEventCreate(&c->ev_t1));
-    CU(cudaEventCreate(&c->ev_m0));
-    CU(cudaEventCreate(&c->ev_m1));
+    if (!c->partials) {
+        c->n_partials = (size_t)(ds_grid(c) > cg_grid(c) ? ds_grid(c) : cg_grid(c)) + 4;
+        if ((rc = dev_alloc(c, (void**)&c->partials, c->n_partials * sizeof(double)))) return rc;
+    }
+    if (!c->red && (rc = dev_alloc(c, (void**)&c->red, 2 * sizeof(double)))) return rc;
+    if (!c->red_host) CU(cudaMallocHost((void**)&c->red_host, 2 * sizeof(double)));
+    if (c->slab) {
+        if (!c->comm_stream) CU(cudaStreamCreateWithFlags(&c->comm_stream, cudaStreamNonBlocking));
+        if (!c->ev_pack) CU(cudaEventCreateWithFlags(&c->ev_pack, cudaEventDisableTiming));
+        if (!c->ev_halo) CU(cudaEventCreateWithFlags(&c->ev_halo, cudaEventDisableTiming));
+    }
+    if (!c->dev_max && (rc = dev_alloc(c, (void**)&c->dev_max, sizeof(double)))) return rc;
+    if (!c->st_host) CU(cudaMallocHost((void**)&c->st_host, sizeof(CgState)));
+    if (!c->flag_host) CU(cudaMallocHost((void**)&c->flag_host, 2 * sizeof(int)));
+    if (!c->max_host) CU(cudaMallocHost((void**)&c->max_host, sizeof(double)));
+    for (int i = 0; i < 2; ++i)
+        if (!c->ev[i]) CU(cudaEventCreateWithFlags(&c->ev[i], cudaEventDisableTiming));
+    if (!c->ev_t0) CU(cudaEventCreate(&c->ev_t0));
+    if (!c->ev_t1) CU(cudaEventCreate(&c->ev_t1));
+    if (!c->ev_m0) CU(cudaEventCreate(&c->ev_m0));
+    if (!c->ev_m1) CU(cudaEventCreate(&c->ev_m1));
     c->basics = true;
     return LQCD_OK;
 }
@@ -570,9 +585,9 @@ template <typename T>
 int ensure_stage(lqcd_ctx* c, int nx) {
     int rc;
     PrecBufs<T>& B = bufs<T>(c);
-    if (!B.stage_b && (rc = dev_alloc(c, (void**)&B.stage_b, vec_bytes<T>(c)))) return rc;
+    if (!B.stage_b && (rc = dev_alloc_own(c, (void**)&B.stage_b, vec_bytes<T>(c)))) return rc;
     while (B.n_stage_x < nx) {
-        if ((rc = dev_alloc(c, (void**)&B.stage_x[B.n_stage_x], vec_bytes<T>(c)))) return rc;
+        if ((rc = dev_alloc_own(c, (void**)&B.stage_x[B.n_stage_x], vec_bytes<T>(c)))) return rc;
         ++B.n_stage_x;
     }
     return LQCD_OK;
@@ -626,6 +641,11 @@ int store_gauge(lqcd_ctx* c, const double* links, int recon) {
         V2<T>* dummy = B.Wt_send + (size_t)2 * 9 * face;        // what comes down the ring is not needed
         if ((rc = comm_exchange(c, B.Wt_send, B.Wt_send, B.Wt_lo, dummy, n * sizeof(V2<T>)))) return rc;
         CU(cudaStreamSynchronize(c->comm_stream));
+        // first use of the all-reduce here, outside any stream capture: a transport that sets up connections or
+        // buffers lazily (NCCL) has then done so before the CG iteration is captured into a CUDA graph
+        CU(cudaMemsetAsync(c->red, 0, 2 * sizeof(double), c->stream));
+        if ((rc = comm_allreduce(c))) return rc;
+        CU(cudaStreamSynchronize(c->stream));
     }
     B.recon_stored = recon;
     return LQCD_OK;
@@ -735,7 +755,7 @@ lqcd_ctx* lqcd_create(int Lx, int Ly, int Lz, int Lt) {
     c->max_iter = 100000;
     c->check_every = 0;
     c->use_graph = 1;
-    c->shift_block = 8;
+    c->shift_block = 16;
     c->err[0] = 0;
     return c;
 }
@@ -754,19 +774,10 @@ void lqcd_destroy(lqcd_ctx* c) {
     }
     if (c->host_stage) cudaFreeHost(c->host_stage);
     if (c->red_host) cudaFreeHost(c->red_host);
-    if (c->basics && c->slab) {
-        cudaStreamDestroy(c->comm_stream);
-        cudaEventDestroy(c->ev_pack);
-        cudaEventDestroy(c->ev_halo);
-    }
-    if (c->basics) {
-        cudaEventDestroy(c->ev[0]);
-        cudaEventDestroy(c->ev[1]);
-        cudaEventDestroy(c->ev_t0);
-        cudaEventDestroy(c->ev_t1);
-        cudaEventDestroy(c->ev_m0);
-        cudaEventDestroy(c->ev_m1);
-    }
+    if (c->comm_stream) cudaStreamDestroy(c->comm_stream);
+    cudaEvent_t evs[] = {c->ev_pack, c->ev_halo, c->ev[0], c->ev[1], c->ev_t0, c->ev_t1, c->ev_m0, c->ev_m1};
+    for (cudaEvent_t e : evs)
+        if (e) cudaEventDestroy(e);
     cudaGetLastError();
     delete c;
 }
@@ -932,10 +943,9 @@ size_t lqcd_workspace_bytes(const lqcd_ctx* c, int nshift) {
         b += align_up(links_bytes<float>(c, 18)) + align_up(vec_bytes<float>(c)) * (size_t)(3 + c->shift_block + (nshift - 1));
     if (c->prec_opt & LQCD_PREC_F64) b += align_up((size_t)8 * c->Vh * sizeof(double));   // U(1) angles, if set
     if (c->prec_opt & LQCD_PREC_F32) b += align_up((size_t)8 * c->Vh * sizeof(float));
-    b += align_up(sizeof(CgState)) + align_up(sizeof(double));
+    b += align_up(sizeof(CgState)) + align_up(sizeof(double)) + align_up(2 * sizeof(double));
     if (c->slab) {
         const size_t face = face_sites(c);
-        b += align_up(2 * sizeof(double));
         if (c->prec_opt & LQCD_PREC_F64) b += 2 * align_up(6 * face * sizeof(double2)) + align_up(18 * face * sizeof(double2)) + align_up(36 * face * sizeof(double2));
         if (c->prec_opt & LQCD_PREC_F32) b += 2 * align_up(6 * face * sizeof(float2)) + align_up(18 * face * sizeof(float2)) + align_up(36 * face * sizeof(float2));
     }
@@ -1352,10 +1362,6 @@ int solve_mixed(lqcd_ctx* c, const double* b_even, const double* shifts, int nsh
     if ((rc = check_ctx_gauge<double>(c)) || (rc = check_ctx_gauge<float>(c))) return rc;
     if ((rc = ensure_solver<float>(c, nshift)) || (rc = ensure_tmp<double>(c))) return rc;
     if ((rc = ensure_stage<float>(c, nshift)) || (rc = ensure_stage<double>(c, 1))) return rc;
-    if (!c->red) {
-        if ((rc = dev_alloc(c, (void**)&c->red, 2 * sizeof(double)))) return rc;
-        CU(cudaMallocHost((void**)&c->red_host, 2 * sizeof(double)));
-    }
     PrecBufs<float>& F = bufs<float>(c);
     PrecBufs<double>& D = bufs<double>(c);
     const size_t n = c->Vh * 3;

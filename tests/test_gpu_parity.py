@@ -293,6 +293,20 @@ def test_caller_workspace(lq):
     ir["band"] = oracle_iteration_band(L, U.numpy(), mass, b_aos, shifts, 1e-10, ir["iters"], 3)
     check_cg(x, info, xr, ir, shifts)
     lat.close()
+    # an arena of exactly the documented size also serves the host entry points and the mixed-precision solver
+    # (their staging copies are allocated outside it); both link precisions are named BEFORE the query
+    lat = lq.Lattice(L, mass=mass, precisions=lq.LQCD_PREC_F64 | lq.LQCD_PREC_F32)
+    need2 = lq.lqcd_workspace_bytes(lat.ctx, len(shifts))
+    assert need2 > need
+    ws = torch.empty(need2, dtype=torch.uint8, device="cuda")
+    assert lq.lqcd_set_workspace(lat.ctx, ws.data_ptr(), ws.numel()) == 0
+    lat.set_gauge(U.cuda())
+    xh, ih = lat.mshift_cg(torch.as_tensor(b_soa).pin_memory(), shifts, 1e-10)
+    assert torch.equal(xh, x.cpu()) and ih["iters"] == info["iters"]
+    xm, im = lat.mshift_cg_mixed(cuda(b_soa), shifts, 1e-10)
+    for i in range(len(shifts)):
+        assert rel_l2(soa_gpu_to_aos(xm[i]), xr[i]) <= TOL_CG
+    lat.close()
 
 
 # ---- rational function of the Eq. 2 operator, accumulated during the solve ------

@@ -56,7 +56,7 @@ def solve(lq, lat, b, shifts, tol, m, use_graph=True, max_iter=None):
 
 def test_option_range(lq):
     lat = lq.Lattice((4, 4, 4, 4))
-    assert lat.get_option(lq.LQCD_OPT_SHIFT_BLOCK) == 8
+    assert lat.get_option(lq.LQCD_OPT_SHIFT_BLOCK) == 16
     for bad in (0, 17, 2.5, -1):
         assert lq.lqcd_set_option(lat.ctx, lq.LQCD_OPT_SHIFT_BLOCK, bad) == lq.LQCD_EINVAL
     lat.set_option(lq.LQCD_OPT_SHIFT_BLOCK, 5)

@@ -79,3 +79,19 @@ int main() {
     subprocess.run(["g++", "-O2", "-I", inc, "-o", str(exe), str(src)], check=True)
     out = subprocess.run([str(exe)], capture_output=True, text=True, check=True)
     assert out.stdout.strip() == "ok"
+
+
+def test_ncu_traffic_constants_of_bench_match_the_profile_they_cite():
+    """bench.py reports `roofline.traffic` from a constant measured once under `ncu --set full`; the constant and
+    the file it names must say the same thing (it would otherwise go stale silently when the kernel changes)."""
+    sys.path.insert(0, ROOT)
+    import bench
+    unit = {"Gbyte": 1.0, "Mbyte": 1e-3, "Kbyte": 1e-6, "byte": 1e-9}
+    assert bench.NCU_DRAM_GB_PER_LAUNCH
+    for (workload, recon), (rd, wr, path) in bench.NCU_DRAM_GB_PER_LAUNCH.items():
+        text = open(os.path.join(ROOT, path)).read()
+        m = re.search(r"dslash_kernel<double, %d, 0, 0, 0>.*?dram__bytes_read\.sum\s+([0-9.]+) (\w+).*?"
+                      r"dram__bytes_write\.sum\s+([0-9.]+) (\w+)" % recon, text, flags=re.S)
+        assert m, (workload, recon, path)
+        assert abs(float(m.group(1)) * unit[m.group(2)] - rd) <= 1e-5 * rd
+        assert abs(float(m.group(3)) * unit[m.group(4)] - wr) <= 1e-5 * wr
