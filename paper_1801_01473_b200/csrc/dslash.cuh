@@ -247,6 +247,7 @@ struct DslashArgs {
     double* partials;        // EPI 1,3,4,5
     CgState* st;             // EPI 1,3,4,5, or any EPI with check_stop
     int check_stop;          // 1: return at once if st->stop (CG already converged)
+    int links_resident;      // 1: the stored links are small enough to live in L2 (cache policy of the link loads)
     // EPI == 5 only (all of parity par)
     const V2<T>* r_in;       // residual r^(n)
     V2<T>* r_out;            // residual r^(n+1): the next slot of the ring (may be r_in itself)
@@ -327,8 +328,10 @@ __global__ void __launch_bounds__(DS_BLOCK, (DsOcc<T, EPI>::minb)) dslash_kernel
     const unsigned int mtf = mt ^ ((g.antiperiodic && tg == Ltg - 1) ? SB : 0u);   // link (x,t) leaves Lt-1
     const unsigned int mtb = mt ^ ((g.antiperiodic && tg == 0) ? SB : 0u);         // link (x-t,t) leaves Lt-1
 
-    const uint64_t pol_s = l2_policy_evict_first();
+    // links: streamed once per application -- first to leave L2; unless the whole gauge field fits in L2 beside the
+    // vectors (small lattices), where it is what should stay for the next application
     const uint64_t pol_r = l2_policy_evict_last();
+    const uint64_t pol_s = A.links_resident ? pol_r : l2_policy_evict_first();
 
     const V2<T>* __restrict__ Wf = A.W + (size_t)A.par * NE * vh + k;            // links of the output parity
     const V2<T>* __restrict__ Wb = A.W + (size_t)(1 - A.par) * NE * vh;          // links of the input parity

@@ -170,6 +170,9 @@ void dev_free_owned(lqcd_ctx* c, void* p) {
         }
 }
 
+template <typename T> const PrecBufs<T>& bufs_c(const lqcd_ctx* c);
+template <> const PrecBufs<double>& bufs_c<double>(const lqcd_ctx* c) { return c->d; }
+template <> const PrecBufs<float>& bufs_c<float>(const lqcd_ctx* c) { return c->f; }
 template <typename T> PrecBufs<T>& bufs(lqcd_ctx* c);
 template <> PrecBufs<double>& bufs<double>(lqcd_ctx* c) { return c->d; }
 template <> PrecBufs<float>& bufs<float>(lqcd_ctx* c) { return c->f; }
@@ -191,6 +194,18 @@ void drop_graphs(lqcd_ctx* c) {
 template <typename T> size_t vec_bytes(const lqcd_ctx* c) { return c->Vh * 3 * sizeof(V2<T>); }
 template <typename T> size_t links_bytes(const lqcd_ctx* c, int recon) {
     return (size_t)8 * (recon == 12 ? 6 : 9) * c->Vh * sizeof(V2<T>);
+}
+
+// The stored links of precision T fit in L2 beside the solver's vectors (B200: 126 MB in two halves, and a line
+// read by SMs of both dies may sit in both).  Measured at 16^4 (37.7 MB of links): with the streaming policy every
+// application re-read them from DRAM (40 MB per launch under ncu --cache-control none); kept, one application in a
+// graph takes 4.5 us = 9.6 TB/s out of L2.
+#ifndef LINKS_RESIDENT_MAX
+#define LINKS_RESIDENT_MAX (48u << 20)
+#endif
+template <typename T> int links_resident(const lqcd_ctx* c) {
+    const int ne = (bufs_c<T>(c).recon_stored == 12) ? 6 : 9;
+    return (size_t)8 * ne * c->Vh * sizeof(V2<T>) <= LINKS_RESIDENT_MAX ? 1 : 0;
 }
 
 int ds_grid(const lqcd_ctx* c) { return (int)((c->Vh + DS_BLOCK - 1) / DS_BLOCK); }
@@ -380,6 +395,7 @@ int slab_dslash(lqcd_ctx* c, int epi, V2<T>* out, const V2<T>* in, int par, cons
     DslashArgs<T> a{};
     a.g = c->g;
     a.W = B.W;
+    a.links_resident = links_resident<T>(c);
     a.Th = B.Th;
     a.Th_lo = B.Th_lo;
     a.in = in;
@@ -444,6 +460,7 @@ void launch_dslash(lqcd_ctx* c, int epi, V2<T>* out, const V2<T>* in, int par, c
     DslashArgs<T> a{};
     a.g = c->g;
     a.W = bufs<T>(c).W;
+    a.links_resident = links_resident<T>(c);
     a.Th = bufs<T>(c).Th;
     a.in = in;
     a.out = out;
@@ -467,6 +484,7 @@ void launch_cg_fused(lqcd_ctx* c, const V2<T>* r_in, V2<T>* r_out, V2<T>* p_keep
     DslashArgs<T> a{};
     a.g = c->g;
     a.W = B.W;
+    a.links_resident = links_resident<T>(c);
     a.Th = B.Th;
     a.partials = c->partials;
     a.st = c->st_dev;

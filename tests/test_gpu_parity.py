@@ -443,7 +443,7 @@ def large_config_protocol(lq, name, n_it, residual_shifts):
 
 def test_mshift_cg_config4_48x4(lq):
     """BASELINE config 4: 48^4, 16 shifts 1e-5..1, m = 0.0075, tol 1e-10."""
-    large_config_protocol(lq, "config4_48^4", n_it=12, residual_shifts=(0, 7, 15))
+    large_config_protocol(lq, "config4_48^4", n_it=20, residual_shifts=(0, 7, 15))      # one whole shift block + 4
 
 
 def test_mshift_cg_config5_64x4(lq):
