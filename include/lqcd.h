@@ -86,6 +86,12 @@ typedef struct lqcd_ctx lqcd_ctx;
                                        residuals of the block (kept in m vectors) instead of once per iteration;
                                        same recurrences, same iteration counts, x_i equal up to rounding.
                                        m = 1: every iteration.  CHECK_EVERY is rounded up to a multiple of m. */
+#define LQCD_OPT_PERSISTENT      8  /* -1 (default): lattices whose stored links stay in L2 (e.g. 16^4) are solved by ONE
+                                       cooperative kernel that runs all iterations with grid-wide barriers between the
+                                       sweeps (no launch gaps, no host polling); larger ones by two launches per
+                                       iteration replayed as a CUDA graph.  0: never, 1: always the persistent kernel.
+                                       Same arithmetic per site; the scalar products are added over a different grid,
+                                       so results agree to rounding.  Whole-lattice contexts only.            */
 #define LQCD_PREC_F64 1
 #define LQCD_PREC_F32 2
 

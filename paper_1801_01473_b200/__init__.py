@@ -11,7 +11,7 @@ takes torch tensors (device memory and streams are torch's job, nothing else is)
 from .binding import (  # noqa: F401
     LQCD_OK, LQCD_EINVAL, LQCD_ENOGAUGE, LQCD_ENOMEM, LQCD_ECUDA, LQCD_ENOCONV, LQCD_EBREAKDOWN, LQCD_ENOTSU3, LQCD_ECOMM, LQCD_NCCL_ID_BYTES,
     LQCD_OPT_MASS, LQCD_OPT_ANTIPERIODIC_T, LQCD_OPT_RECON, LQCD_OPT_MAX_ITER, LQCD_OPT_CHECK_EVERY,
-    LQCD_OPT_USE_GRAPH, LQCD_OPT_LINK_PRECISIONS, LQCD_OPT_SHIFT_BLOCK, LQCD_PREC_F64, LQCD_PREC_F32,
+    LQCD_OPT_USE_GRAPH, LQCD_OPT_LINK_PRECISIONS, LQCD_OPT_SHIFT_BLOCK, LQCD_OPT_PERSISTENT, LQCD_PREC_F64, LQCD_PREC_F32,
     LQCD_STAT_ITERS, LQCD_STAT_REL_RES, LQCD_STAT_FREEZE_ITER, LQCD_STAT_BASE_SHIFT, LQCD_STAT_GPU_LAUNCHES,
     LQCD_STAT_SOLVE_MS, LQCD_STAT_RELIABLE_UPDATES,
     LqcdError, Lattice, load_library, library_path, EXPORTS,

@@ -13,6 +13,7 @@ LQCD_ENOCONV, LQCD_EBREAKDOWN, LQCD_ENOTSU3, LQCD_ECOMM = -5, -6, -7, -8
 LQCD_NCCL_ID_BYTES = 128
 LQCD_OPT_MASS, LQCD_OPT_ANTIPERIODIC_T, LQCD_OPT_RECON, LQCD_OPT_MAX_ITER = 0, 1, 2, 3
 LQCD_OPT_CHECK_EVERY, LQCD_OPT_USE_GRAPH, LQCD_OPT_LINK_PRECISIONS, LQCD_OPT_SHIFT_BLOCK = 4, 5, 6, 7
+LQCD_OPT_PERSISTENT = 8
 LQCD_PREC_F64, LQCD_PREC_F32 = 1, 2
 LQCD_STAT_ITERS, LQCD_STAT_REL_RES, LQCD_STAT_FREEZE_ITER, LQCD_STAT_BASE_SHIFT = 0, 1, 2, 3
 LQCD_STAT_GPU_LAUNCHES, LQCD_STAT_SOLVE_MS, LQCD_STAT_RELIABLE_UPDATES = 4, 5, 6
@@ -383,6 +384,9 @@ class Lattice:
     entry points on torch's current stream, CPU tensors to the ``*_host`` entry points (the copies happen
     inside the call)."""
 
+    # options applied to every context at creation, {key: value} (tests use it to run whole modules on one solver path)
+    default_options: dict = {}
+
     def __init__(self, L: Sequence[int], mass: float = 0.0, antiperiodic: bool = True, recon: int = 18,
                  precisions: int = LQCD_PREC_F64, slab: Optional[Sequence[int]] = None, comm: Optional[str] = None,
                  group=None):
@@ -409,6 +413,8 @@ class Lattice:
         self.Vh = self.V // 2
         if slab is not None:
             self._init_comm(comm or "nccl", rank, nranks, group)
+        for key, value in self.default_options.items():
+            self.set_option(key, value)
         self.set_option(LQCD_OPT_MASS, mass)
         self.set_option(LQCD_OPT_ANTIPERIODIC_T, 1.0 if antiperiodic else 0.0)
         self.set_option(LQCD_OPT_RECON, recon)

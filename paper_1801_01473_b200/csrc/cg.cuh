@@ -196,8 +196,8 @@ __device__ __forceinline__ void cg_flush_body(const int nres, const int nl, cons
                                               const V2<T>* const* sr, const T* sCP, const T* sB, const V2<T>* sDE,
                                               const T* sY, V2<T>* __restrict__ y, const size_t n) {
     constexpr int U = FLUSH_UNR;
-    const size_t stride = (size_t)gridDim.x * CG_BLOCK;
-    for (size_t j = (size_t)blockIdx.x * CG_BLOCK + threadIdx.x; j < n; j += stride) {
+    const size_t stride = (size_t)gridDim.x * blockDim.x;
+    for (size_t j = (size_t)blockIdx.x * blockDim.x + threadIdx.x; j < n; j += stride) {
         V2<T> rv[MM];
 #pragma unroll
         for (int l = 0; l < MM; ++l)
@@ -255,10 +255,10 @@ __device__ __forceinline__ void cg_flush_body(const int nres, const int nl, cons
     }
 }
 
+// The sweep as a block-level function (every thread of every block of the grid calls it; blockDim.x >=
+// LQCD_MAX_SHIFTS + MM): used by cg_flush_kernel and, between grid-wide barriers, by the persistent solver.
 template <typename T, int MM>
-__global__ void __launch_bounds__(CG_BLOCK, (MM <= 8 ? 2 : 1)) cg_flush_kernel(CgState* st, size_t n) {
-    const int nres = st->blk_j;
-    if (nres == 0) return;                       // nothing accumulated (solve already over); same in every block
+__device__ __forceinline__ void cg_flush_block(const CgState* st, const size_t n, const int nres) {
     __shared__ V2<T>* sx[LQCD_MAX_SHIFTS];
     __shared__ V2<T>* sp[LQCD_MAX_SHIFTS];
     __shared__ const V2<T>* sr[MM];
@@ -316,9 +316,16 @@ __global__ void __launch_bounds__(CG_BLOCK, (MM <= 8 ? 2 : 1)) cg_flush_kernel(C
             else cg_flush_body<T, MM, false, false>(nres, nl, s_ebase, sx, sp, sr, sCP, sB, sDE, sY, y, n);
         }
     }
+}
+
+template <typename T, int MM>
+__global__ void __launch_bounds__(CG_BLOCK, (MM <= 8 ? 2 : 1)) cg_flush_kernel(CgState* st, size_t n) {
+    const int nres = st->blk_j;
+    if (nres == 0) return;                       // nothing accumulated (solve already over); same in every block
+    cg_flush_block<T, MM>(st, n, nres);
     // the last block to finish closes the block of iterations; every block has read the state by then
     __syncthreads();
-    if (tid == 0) {
+    if (threadIdx.x == 0) {
         __threadfence();
         const unsigned int t = atomicAdd(&st->ticket[3], 1u);
         if (t == gridDim.x - 1) {

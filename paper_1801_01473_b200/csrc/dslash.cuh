@@ -59,19 +59,27 @@
 #define DS_MINB_F32 6
 #endif
 static_assert(DS_BLOCK >= LQCD_MAX_SHIFTS, "the scalar step of the epilogue needs one thread per shift");
-#ifndef EPI_PLOAD
-#define EPI_PLOAD 1      // 0: load p in the epilogue, 1: load p into registers up front, 2: L2 prefetch up front
-#endif
 
 __device__ __forceinline__ uint64_t l2_policy_evict_first() {
     uint64_t p;
     asm("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(p));
     return p;
 }
+__device__ __forceinline__ uint64_t l2_policy_evict_normal() {
+    uint64_t p;
+    asm("createpolicy.fractional.L2::evict_normal.b64 %0, 1.0;" : "=l"(p));
+    return p;
+}
+// 0: evict_first, 1: evict_normal, 2: evict_last
+__device__ __forceinline__ uint64_t l2_policy(int code);
 __device__ __forceinline__ uint64_t l2_policy_evict_last() {
     uint64_t p;
     asm("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(p));
     return p;
+}
+
+__device__ __forceinline__ uint64_t l2_policy(int code) {
+    return code == 0 ? l2_policy_evict_first() : (code == 1 ? l2_policy_evict_normal() : l2_policy_evict_last());
 }
 
 // streamed once: bypass L1 allocation, first to leave L2
@@ -103,6 +111,30 @@ __device__ __forceinline__ float2 ld_reuse(const float2* p, uint64_t pol) {
         : "=f"(v.x), "=f"(v.y)
         : "l"(p), "l"(pol));
     return v;
+}
+
+// The same without .nc, for vectors that other blocks of the SAME kernel write between grid-wide barriers (the
+// persistent solver): .nc data must be read-only for the lifetime of the kernel, an ordinary load is ordered by
+// the barrier's fence.
+__device__ __forceinline__ double2 ld_reuse_coherent(const double2* p, uint64_t pol) {
+    double2 v;
+    asm volatile("ld.global.L1::evict_last.L2::cache_hint.v2.f64 {%0, %1}, [%2], %3;"
+                 : "=d"(v.x), "=d"(v.y)
+                 : "l"(p), "l"(pol)
+                 : "memory");
+    return v;
+}
+__device__ __forceinline__ float2 ld_reuse_coherent(const float2* p, uint64_t pol) {
+    float2 v;
+    asm volatile("ld.global.L1::evict_last.L2::cache_hint.v2.f32 {%0, %1}, [%2], %3;"
+                 : "=f"(v.x), "=f"(v.y)
+                 : "l"(p), "l"(pol)
+                 : "memory");
+    return v;
+}
+template <bool COH, typename V>
+__device__ __forceinline__ V ld_vec(const V* p, uint64_t pol) {
+    return COH ? ld_reuse_coherent(p, pol) : ld_reuse(p, pol);
 }
 
 // x -> +-x by flipping the sign bit (mask is 0 or 0x80000000); integer pipe, not the FP pipe
@@ -180,14 +212,14 @@ __device__ __forceinline__ void load_link(const V2<T>* __restrict__ w, const siz
 
 // the vector operand of a hop: a stored vector, or (FLY) p = r + beta p_old formed in registers from the residual v
 // and the previous search direction v2 (same index); pp accumulates |p|^2 for the <p,Ap> identity of EPI = 4
-template <typename T, bool FLY>
+template <typename T, bool FLY, bool COH>
 __device__ __forceinline__ void load_vec(const V2<T>* __restrict__ v, const V2<T>* __restrict__ v2, const size_t vs,
                                          uint64_t pol, unsigned int mask, const T beta, T (&vr)[3], T (&vi)[3],
                                          double& pp) {
     if (!FLY) {
 #pragma unroll
         for (int c = 0; c < 3; ++c) {
-            const V2<T> t = ld_reuse(v + c * vs, pol);
+            const V2<T> t = ld_vec<COH>(v + c * vs, pol);
             vr[c] = flip(t.x, mask);
             vi[c] = flip(t.y, mask);
         }
@@ -195,8 +227,8 @@ __device__ __forceinline__ void load_vec(const V2<T>* __restrict__ v, const V2<T
         V2<T> r[3], q[3];
 #pragma unroll
         for (int c = 0; c < 3; ++c) {
-            r[c] = ld_reuse(v + c * vs, pol);
-            q[c] = ld_reuse(v2 + c * vs, pol);
+            r[c] = ld_vec<COH>(v + c * vs, pol);
+            q[c] = ld_vec<COH>(v2 + c * vs, pol);
         }
         T n2 = (T)0;
 #pragma unroll
@@ -214,7 +246,7 @@ __device__ __forceinline__ void load_vec(const V2<T>* __restrict__ v, const V2<T
 // One hop.  FWD: acc += sign * U v (the sign is already folded into v);  !FWD: acc += sign * U^dagger v (the caller
 // passes the mask of -s).  ws, vs: element strides of the link and of the vector (they differ from Vh only for the
 // halo buffers of a slab face).
-template <typename T, int RECON, int U1, bool FWD, bool FLY>
+template <typename T, int RECON, int U1, bool FWD, bool FLY, bool COH = false>
 __device__ __forceinline__ void hop(T (&ar)[3], T (&ai)[3], const V2<T>* __restrict__ w, const size_t ws,
                                     const V2<T>* __restrict__ v, const V2<T>* __restrict__ v2, const size_t vs,
                                     unsigned int mask, uint64_t pol_s, uint64_t pol_r, const T* __restrict__ th,
@@ -222,7 +254,7 @@ __device__ __forceinline__ void hop(T (&ar)[3], T (&ai)[3], const V2<T>* __restr
     V2<T> u[9];
     T vr[3], vi[3];
     load_link<T, RECON>(w, ws, pol_s, u);
-    load_vec<T, FLY>(v, v2, vs, pol_r, mask, beta, vr, vi, pp);
+    load_vec<T, FLY, COH>(v, v2, vs, pol_r, mask, beta, vr, vi, pp);
     if (U1) u1_rotate<T, FWD ? +1 : -1>(th, pol_s, vr, vi);
 #pragma unroll
     for (int a = 0; a < 3; ++a)
@@ -247,7 +279,7 @@ struct DslashArgs {
     double* partials;        // EPI 1,3,4,5
     CgState* st;             // EPI 1,3,4,5, or any EPI with check_stop
     int check_stop;          // 1: return at once if st->stop (CG already converged)
-    int links_resident;      // 1: the stored links are small enough to live in L2 (cache policy of the link loads)
+    int pol_links, pol_vecs; // L2 eviction priority of the link / neighbour-vector loads (l2_policy codes)
     // EPI == 5 only (all of parity par)
     const V2<T>* r_in;       // residual r^(n)
     V2<T>* r_out;            // residual r^(n+1): the next slot of the ring (may be r_in itself)
@@ -273,30 +305,15 @@ struct DslashArgs {
 template <typename T, int EPI> struct DsOcc { static constexpr int minb = (EPI == 4) ? DS_MINB_K1 : (EPI == 5) ? DS_MINB_K2 : DS_MINB; };
 template <int EPI> struct DsOcc<float, EPI> { static constexpr int minb = DS_MINB_F32; };
 
-template <typename T, int RECON, int EPI, int U1, int SLAB = 0>
-__global__ void __launch_bounds__(DS_BLOCK, (DsOcc<T, EPI>::minb)) dslash_kernel(const DslashArgs<T> A) {
+// The eight hops of one output site k of parity `par`: acc = sum_mu [ s U in(x+mu) - s U^+ in(x-mu) ] (without the
+// factor 1/2).  FLY: the input is p = in + beta in2 formed at each neighbour, and pp accumulates its |p|^2.
+// COH: the input vectors are written by other blocks of the same kernel (see ld_reuse_coherent).
+template <typename T, int RECON, int U1, int SLAB, bool FLY, bool COH = false>
+__device__ __forceinline__ void dslash_hops(const DslashArgs<T>& A, const int par, const int k,
+                                            const V2<T>* __restrict__ in, const V2<T>* __restrict__ in2, const T beta,
+                                            T (&ar)[3], T (&ai)[3], double& pp) {
     constexpr int NE = (RECON == 12) ? 6 : 9;
-    constexpr bool FLY = (EPI == 4);
-    static_assert(!(SLAB && EPI >= 4), "the fused CG launches exist for the whole-lattice path only");
-    if (A.check_stop) {
-        if (A.st->stop) {
-            // tell the x/p update kernel of the *following* iterations to do nothing (see cg.cuh)
-            if (EPI == 0 && blockIdx.x == 0 && threadIdx.x == 0) A.st->stop4 = 1;
-            return;
-        }
-    }
     const Geom& g = A.g;
-    const int kraw = blockIdx.x * DS_BLOCK + threadIdx.x;
-    bool valid;
-    int k;
-    if (SLAB) {
-        valid = kraw < A.nsites;
-        const int i = valid ? kraw : A.nsites - 1;
-        k = (i < A.na) ? A.k0a + i : A.k0b + (i - A.na);
-    } else {
-        valid = kraw < g.Vh;
-        k = valid ? kraw : g.Vh - 1;
-    }
     const size_t vh = (size_t)g.Vh;
 
     // step A3: coordinates, neighbours, phases
@@ -306,7 +323,7 @@ __global__ void __launch_bounds__(DS_BLOCK, (DsOcc<T, EPI>::minb)) dslash_kernel
     const int y = (int)r1 - (int)r2 * g.Ly;
     const int t = (int)fastdiv(r2, g.dz);
     const int z = (int)r2 - t * g.Lz;
-    const int q = (y + z + t + A.par) & 1;
+    const int q = (y + z + t + par) & 1;
     const int x = 2 * xh + q;
 
     const int kxf = k + (q ? ((xh == g.Lxh - 1) ? 1 - g.Lxh : 1) : 0);
@@ -330,47 +347,20 @@ __global__ void __launch_bounds__(DS_BLOCK, (DsOcc<T, EPI>::minb)) dslash_kernel
 
     // links: streamed once per application -- first to leave L2; unless the whole gauge field fits in L2 beside the
     // vectors (small lattices), where it is what should stay for the next application
-    const uint64_t pol_r = l2_policy_evict_last();
-    const uint64_t pol_s = A.links_resident ? pol_r : l2_policy_evict_first();
+    const uint64_t pol_r = l2_policy(A.pol_vecs);
+    const uint64_t pol_s = l2_policy(A.pol_links);
 
-    const V2<T>* __restrict__ Wf = A.W + (size_t)A.par * NE * vh + k;            // links of the output parity
-    const V2<T>* __restrict__ Wb = A.W + (size_t)(1 - A.par) * NE * vh;          // links of the input parity
+    const V2<T>* __restrict__ Wf = A.W + (size_t)par * NE * vh + k;              // links of the output parity
+    const V2<T>* __restrict__ Wb = A.W + (size_t)(1 - par) * NE * vh;            // links of the input parity
     const size_t mu_stride = (size_t)2 * NE * vh;
-    const V2<T>* __restrict__ in = A.in;
-    const V2<T>* __restrict__ in2 = FLY ? A.in2 : A.in;
-
-    // epilogue operands are requested first, so that their latency hides behind the eight hops
-    T coef = (T)0, beta = (T)0;
-    V2<T> pv[3], rv[3];
-    if (EPI != 0) {
-        // CG: m^2 + sigma0 from the device state (graph-invariant)
-        coef = (T)((EPI == 2) ? A.coef : A.st->c0);
-        if (EPI >= 4) beta = (T)A.st->b_prev;
-        if (EPI != 4) {
-#if EPI_PLOAD == 1
-#pragma unroll
-            for (int c = 0; c < 3; ++c) pv[c] = A.pv[c * vh + k];
-#elif EPI_PLOAD == 2
-#pragma unroll
-            for (int c = 0; c < 3; ++c) asm volatile("prefetch.global.L2 [%0];" ::"l"(A.pv + c * vh + k));
-#endif
-        }
-        if (EPI == 5) {
-#pragma unroll
-            for (int c = 0; c < 3; ++c) rv[c] = A.r_in[c * vh + k];
-        }
-    }
-
-    T ar[3] = {(T)0, (T)0, (T)0}, ai[3] = {(T)0, (T)0, (T)0};
-    double pp = 0.0;                                                             // EPI == 4: sum of |p|^2 over the neighbours
-    const T* __restrict__ Tf = U1 ? A.Th + (size_t)A.par * vh + k : nullptr;     // angles of the forward links
-    const T* __restrict__ Tb = U1 ? A.Th + (size_t)(1 - A.par) * vh : nullptr;   // angles of the backward links
+    const T* __restrict__ Tf = U1 ? A.Th + (size_t)par * vh + k : nullptr;       // angles of the forward links
+    const T* __restrict__ Tb = U1 ? A.Th + (size_t)(1 - par) * vh : nullptr;     // angles of the backward links
     const size_t th_stride = 2 * vh;
 #define HOP_F(mu, kn, mask) \
-    hop<T, RECON, U1, true, FLY>(ar, ai, Wf + (mu) * mu_stride, vh, in + (kn), in2 + (kn), vh, mask, pol_s, pol_r, \
+    hop<T, RECON, U1, true, FLY, COH>(ar, ai, Wf + (mu) * mu_stride, vh, in + (kn), in2 + (kn), vh, mask, pol_s, pol_r, \
                                  Tf + (mu) * th_stride, beta, pp)
 #define HOP_B(mu, kn, mask) \
-    hop<T, RECON, U1, false, FLY>(ar, ai, Wb + (mu) * mu_stride + (kn), vh, in + (kn), in2 + (kn), vh, (mask) ^ SB, pol_s, \
+    hop<T, RECON, U1, false, FLY, COH>(ar, ai, Wb + (mu) * mu_stride + (kn), vh, in + (kn), in2 + (kn), vh, (mask) ^ SB, pol_s, \
                                   pol_r, Tb + (mu) * th_stride + (kn), beta, pp)
     HOP_F(0, kxf, 0u);
     HOP_B(0, kxb, 0u);
@@ -390,13 +380,137 @@ __global__ void __launch_bounds__(DS_BLOCK, (DsOcc<T, EPI>::minb)) dslash_kernel
         hop<T, RECON, U1, true, false>(ar, ai, Wf + 3 * mu_stride, vh, vf, vf, top ? face : vh, mtf, pol_s, pol_r,
                                        Tf + 3 * th_stride, beta, pp);
         const V2<T>* vb = bot ? A.in_lo + kf : in + k - g.st;
-        const V2<T>* wb = bot ? A.Wt_lo + (size_t)(1 - A.par) * NE * face + kf : Wb + 3 * mu_stride + k - g.st;
-        const T* tb = U1 ? (bot ? A.Th_lo + (size_t)(1 - A.par) * face + kf : Tb + 3 * th_stride + k - g.st) : nullptr;
+        const V2<T>* wb = bot ? A.Wt_lo + (size_t)(1 - par) * NE * face + kf : Wb + 3 * mu_stride + k - g.st;
+        const T* tb = U1 ? (bot ? A.Th_lo + (size_t)(1 - par) * face + kf : Tb + 3 * th_stride + k - g.st) : nullptr;
         hop<T, RECON, U1, false, false>(ar, ai, wb, bot ? face : vh, vb, vb, bot ? face : vh, mtb ^ SB, pol_s, pol_r, tb,
                                         beta, pp);
     }
 #undef HOP_F
 #undef HOP_B
+}
+
+// K1 of the fused iteration, after the hops: t = D_oe p is stored; returns this site's share of
+// <p, A p> = c0 |p|^2 + |t|^2 (|p|^2 of the eight neighbours, each counted 1/8)
+template <typename T>
+__device__ __forceinline__ double k1_finish(V2<T>* __restrict__ out, const size_t vh, const int k, const bool valid,
+                                            const T (&ar)[3], const T (&ai)[3], const double pp, const double c0) {
+    double dot = 0.0;
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+        const V2<T> o = make_v2((T)0.5 * ar[c], (T)0.5 * ai[c]);
+        if (valid) {
+            out[c * vh + k] = o;
+            dot = fma((double)o.x, (double)o.x, dot);
+            dot = fma((double)o.y, (double)o.y, dot);
+        }
+    }
+    if (valid) dot = fma(0.125 * c0, pp, dot);
+    return dot;
+}
+
+// What K2 needs besides the hops, the same for every site of a launch
+template <typename T>
+struct K2Coef {
+    T beta, a, c0, ax;       // ax: coefficient of p in the update of x_0 (alpha_i0 * a in rational-sum mode)
+    V2<T>* xp;               // x_0 (or y in rational-sum mode)
+    V2<T>* p_out;
+    V2<T>* r_out;
+    V2<T>* p_keep;           // may be NULL
+    int defer_base;
+};
+
+// K2 of the fused iteration, after the hops (acc = 2 D_eo t): p = r + beta p_old;  s = c0 p - D_eo t;
+// r_new = r - a s;  x_0 += a p;  returns |r_new|^2 of the site
+template <typename T>
+__device__ __forceinline__ double k2_finish(const K2Coef<T>& C, const size_t vh, const int k, const bool valid,
+                                            const V2<T> (&pold)[3], const V2<T> (&rv)[3], const T (&ar)[3],
+                                            const T (&ai)[3]) {
+    double dot = 0.0;
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+        const V2<T> r = rv[c];
+        const V2<T> p = make_v2(fma(C.beta, pold[c].x, r.x), fma(C.beta, pold[c].y, r.y));
+        const V2<T> sv = make_v2(fma((T)-0.5, ar[c], C.c0 * p.x), fma((T)-0.5, ai[c], C.c0 * p.y));
+        const V2<T> rn = make_v2(fma(-C.a, sv.x, r.x), fma(-C.a, sv.y, r.y));
+        if (valid) {
+            C.p_out[c * vh + k] = p;
+            C.r_out[c * vh + k] = rn;
+            if (C.p_keep) C.p_keep[c * vh + k] = p;
+            if (!C.defer_base) {
+                V2<T> xv = C.xp[c * vh + k];
+                xv.x = fma(C.ax, p.x, xv.x);
+                xv.y = fma(C.ax, p.y, xv.y);
+                C.xp[c * vh + k] = xv;
+            }
+            dot = fma((double)rn.x, (double)rn.x, dot);
+            dot = fma((double)rn.y, (double)rn.y, dot);
+        }
+    }
+    return dot;
+}
+
+template <typename T>
+__device__ __forceinline__ K2Coef<T> k2_coef_from_state(const CgState* st, V2<T>* p_out, V2<T>* r_out, V2<T>* p_keep,
+                                                        int defer_base) {
+    K2Coef<T> C;
+    const int rational = st->rational, i0 = st->i0;
+    C.beta = (T)st->b_prev;
+    C.a = (T)st->a;
+    C.c0 = (T)st->c0;
+    C.ax = (T)(rational ? st->alpha[i0] * st->a : st->a);
+    C.xp = (V2<T>*)(rational ? st->y : st->x[i0]);
+    C.p_out = p_out;
+    C.r_out = r_out;
+    C.p_keep = p_keep;
+    C.defer_base = defer_base;
+    return C;
+}
+
+template <typename T, int RECON, int EPI, int U1, int SLAB = 0>
+__global__ void __launch_bounds__(DS_BLOCK, (DsOcc<T, EPI>::minb)) dslash_kernel(const DslashArgs<T> A) {
+    constexpr bool FLY = (EPI == 4);
+    static_assert(!(SLAB && EPI >= 4), "the fused CG launches exist for the whole-lattice path only");
+    if (A.check_stop) {
+        if (A.st->stop) {
+            // tell the x/p update kernel of the *following* iterations to do nothing (see cg.cuh)
+            if (EPI == 0 && blockIdx.x == 0 && threadIdx.x == 0) A.st->stop4 = 1;
+            return;
+        }
+    }
+    const Geom& g = A.g;
+    const int kraw = blockIdx.x * DS_BLOCK + threadIdx.x;
+    bool valid;
+    int k;
+    if (SLAB) {
+        valid = kraw < A.nsites;
+        const int i = valid ? kraw : A.nsites - 1;
+        k = (i < A.na) ? A.k0a + i : A.k0b + (i - A.na);
+    } else {
+        valid = kraw < g.Vh;
+        k = valid ? kraw : g.Vh - 1;
+    }
+    const size_t vh = (size_t)g.Vh;
+
+    // epilogue operands are requested first, so that their latency hides behind the eight hops
+    T coef = (T)0, beta = (T)0;
+    V2<T> pv[3], rv[3];
+    if (EPI != 0) {
+        // CG: m^2 + sigma0 from the device state (graph-invariant)
+        coef = (T)((EPI == 2) ? A.coef : A.st->c0);
+        if (EPI == 4) beta = (T)A.st->b_prev;
+        if (EPI != 4) {
+#pragma unroll
+            for (int c = 0; c < 3; ++c) pv[c] = A.pv[c * vh + k];
+        }
+        if (EPI == 5) {
+#pragma unroll
+            for (int c = 0; c < 3; ++c) rv[c] = A.r_in[c * vh + k];
+        }
+    }
+
+    T ar[3] = {(T)0, (T)0, (T)0}, ai[3] = {(T)0, (T)0, (T)0};
+    double pp = 0.0;                            // EPI == 4: sum of |p|^2 over the neighbours
+    dslash_hops<T, RECON, U1, SLAB, FLY>(A, A.par, k, A.in, FLY ? A.in2 : A.in, beta, ar, ai, pp);
 
     if (EPI == 0) {
         if (valid) {
@@ -408,58 +522,15 @@ __global__ void __launch_bounds__(DS_BLOCK, (DsOcc<T, EPI>::minb)) dslash_kernel
 
     double dot = 0.0;                           // scalar products are summed in double whatever T is
     if (EPI == 4) {
-        // K1: t = D_oe p;  this site's share of <p, A p> = c0 |p|^2 + |t|^2
-#pragma unroll
-        for (int c = 0; c < 3; ++c) {
-            const V2<T> o = make_v2((T)0.5 * ar[c], (T)0.5 * ai[c]);
-            if (valid) {
-                A.out[c * vh + k] = o;
-                dot = fma((double)o.x, (double)o.x, dot);
-                dot = fma((double)o.y, (double)o.y, dot);
-            }
-        }
-        if (valid) dot = fma(0.125 * A.st->c0, pp, dot);
+        dot = k1_finish<T>(A.out, vh, k, valid, ar, ai, pp, A.st->c0);
     } else if (EPI == 5) {
-        // K2: p = r + beta p_old;  s = c0 p - D_eo t;  r_new = r - a s;  x_0 += a p
-        const CgState* st = A.st;
-        const T a = (T)st->a;
-        const int rational = st->rational, i0 = st->i0;
-        const T ax = (T)(rational ? st->alpha[i0] * st->a : st->a);
-        V2<T>* __restrict__ xp = (V2<T>*)(rational ? st->y : st->x[i0]);
-#pragma unroll
-        for (int c = 0; c < 3; ++c) {
-#if EPI_PLOAD == 1
-            const V2<T> po = pv[c];
-#else
-            const V2<T> po = A.pv[c * vh + k];
-#endif
-            const V2<T> r = rv[c];
-            const V2<T> p = make_v2(fma(beta, po.x, r.x), fma(beta, po.y, r.y));
-            const V2<T> sv = make_v2(fma((T)-0.5, ar[c], coef * p.x), fma((T)-0.5, ai[c], coef * p.y));
-            const V2<T> rn = make_v2(fma(-a, sv.x, r.x), fma(-a, sv.y, r.y));
-            if (valid) {
-                A.p_out[c * vh + k] = p;
-                A.r_out[c * vh + k] = rn;
-                if (A.p_keep) A.p_keep[c * vh + k] = p;
-                if (!A.defer_base) {
-                    V2<T> xv = xp[c * vh + k];
-                    xv.x = fma(ax, p.x, xv.x);
-                    xv.y = fma(ax, p.y, xv.y);
-                    xp[c * vh + k] = xv;
-                }
-                dot = fma((double)rn.x, (double)rn.x, dot);
-                dot = fma((double)rn.y, (double)rn.y, dot);
-            }
-        }
+        const K2Coef<T> C = k2_coef_from_state<T>(A.st, A.p_out, A.r_out, A.p_keep, A.defer_base);
+        dot = k2_finish<T>(C, vh, k, valid, pv, rv, ar, ai);
     } else {
         // out = coef*pv - D in;  Re<pv, out>
 #pragma unroll
         for (int c = 0; c < 3; ++c) {
-#if EPI_PLOAD == 1
             const V2<T> p = pv[c];
-#else
-            const V2<T> p = A.pv[c * vh + k];
-#endif
             const V2<T> o = make_v2(fma((T)-0.5, ar[c], coef * p.x), fma((T)-0.5, ai[c], coef * p.y));
             if (valid) {
                 A.out[c * vh + k] = o;

@@ -18,6 +18,7 @@
 #include "comm.h"
 #include "dslash.cuh"
 #include "lqcd_internal.cuh"
+#include "persist.cuh"
 
 namespace {
 
@@ -62,11 +63,13 @@ struct lqcd_ctx {
     Geom g;
     size_t V, Vh;
     int device, num_sms;
+    int coop_launch;         // the device supports cooperative launches (the persistent solver needs one)
     cudaStream_t stream;
 
     // options
     double mass;
     int recon_opt, max_iter, check_every, use_graph, shift_block;
+    int persistent_opt;      // LQCD_OPT_PERSISTENT: -1 = the library decides (lattices that live in L2), 0 = never, 1 = always
 
     // memory
     char* arena;             // caller workspace (not owned) or NULL
@@ -208,12 +211,30 @@ template <typename T> int links_resident(const lqcd_ctx* c) {
     return (size_t)8 * ne * c->Vh * sizeof(V2<T>) <= LINKS_RESIDENT_MAX ? 1 : 0;
 }
 
+// L2 eviction priorities of the operator's loads (dslash.cuh, l2_policy codes).  Neighbour vectors are re-used by 8
+// sites: last to go.  Links: streamed once per application, first to go -- unless the whole stored field is small
+// enough to stay in L2 for the next application (links_resident), where they too are last to go.  Measured at 16^4,
+// whole CG iteration: links evict_first 36 us, evict_normal or evict_last 19 us, whatever the vectors' priority;
+// pinning the links with a persisting access-policy window on the stream (40 or 79 MB set aside) changed nothing.
+template <typename T> void set_policies(const lqcd_ctx* c, DslashArgs<T>& a) {
+    a.pol_links = links_resident<T>(c) ? 2 : 0;
+    a.pol_vecs = 2;
+}
+
 int ds_grid(const lqcd_ctx* c) { return (int)((c->Vh + DS_BLOCK - 1) / DS_BLOCK); }
 int cg_grid(const lqcd_ctx* c) {
     const size_t n = c->Vh * 3;
     size_t blocks = (n + CG_BLOCK - 1) / CG_BLOCK;
     const size_t cap = (size_t)c->num_sms * 8;
     return (int)(blocks < cap ? blocks : cap);
+}
+
+// one partial per block of the largest launch; the persistent solver keeps two arrays of its grid
+size_t n_partials_needed(const lqcd_ctx* c) {
+    size_t n = (size_t)(ds_grid(c) > cg_grid(c) ? ds_grid(c) : cg_grid(c));
+    const size_t resident = (size_t)c->num_sms * 16;       // no kernel of the library has more blocks per SM than this
+    if (n < resident) n = resident;
+    return 2 * n + 8;
 }
 
 // buffers every call needs: the CG state, reduction partials, pinned mirrors, events
@@ -226,7 +247,7 @@ int ensure_basics(lqcd_ctx* c) {
         CU(cudaMemsetAsync(c->st_dev, 0, sizeof(CgState), c->stream));
     }
     if (!c->partials) {
-        c->n_partials = (size_t)(ds_grid(c) > cg_grid(c) ? ds_grid(c) : cg_grid(c)) + 4;
+        c->n_partials = n_partials_needed(c);
         if ((rc = dev_alloc(c, (void**)&c->partials, c->n_partials * sizeof(double)))) return rc;
     }
     if (!c->red && (rc = dev_alloc(c, (void**)&c->red, 2 * sizeof(double)))) return rc;
@@ -395,7 +416,7 @@ int slab_dslash(lqcd_ctx* c, int epi, V2<T>* out, const V2<T>* in, int par, cons
     DslashArgs<T> a{};
     a.g = c->g;
     a.W = B.W;
-    a.links_resident = links_resident<T>(c);
+    set_policies<T>(c, a);
     a.Th = B.Th;
     a.Th_lo = B.Th_lo;
     a.in = in;
@@ -460,7 +481,7 @@ void launch_dslash(lqcd_ctx* c, int epi, V2<T>* out, const V2<T>* in, int par, c
     DslashArgs<T> a{};
     a.g = c->g;
     a.W = bufs<T>(c).W;
-    a.links_resident = links_resident<T>(c);
+    set_policies<T>(c, a);
     a.Th = bufs<T>(c).Th;
     a.in = in;
     a.out = out;
@@ -484,7 +505,7 @@ void launch_cg_fused(lqcd_ctx* c, const V2<T>* r_in, V2<T>* r_out, V2<T>* p_keep
     DslashArgs<T> a{};
     a.g = c->g;
     a.W = B.W;
-    a.links_resident = links_resident<T>(c);
+    set_policies<T>(c, a);
     a.Th = B.Th;
     a.partials = c->partials;
     a.st = c->st_dev;
@@ -547,6 +568,62 @@ int launch_cg_iteration(lqcd_ctx* c, int pos) {
     launch_cg_fused<T>(c, B.hist[(pos + m - 1) % m], B.hist[pos], (defer && pos == 0) ? B.p_keep : nullptr, defer);
     if (pos == m - 1) launch_flush<T>(c);
     return LQCD_OK;
+}
+
+// ---- the whole solve as one cooperative kernel (persist.cuh) -----------------------------------------------------
+template <typename T, int RECON, int U1>
+int persistent_grid(const lqcd_ctx* c) {
+    int per_sm = 0;
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, cg_persistent_kernel<T, RECON, U1>, PS_BLOCK, 0) != cudaSuccess) {
+        cudaGetLastError();
+        return 0;
+    }
+    // every resident slot is used (the sites are dealt out evenly over the blocks, persist.cuh); one of the blocks
+    // runs the scalar recurrences instead of sites; never more site blocks than sites
+    const long cap = (long)per_sm * c->num_sms - 1;
+    if (cap < 1) return 0;
+    const long want = (long)((c->Vh + PS_BLOCK - 1) / PS_BLOCK);       // no more blocks than one site per thread needs
+    return (int)(want < cap ? want : cap) + 1;
+}
+
+template <typename T, int RECON, int U1>
+int launch_persistent_k(lqcd_ctx* c, PersistArgs<T>& P) {
+    const int grid = persistent_grid<T, RECON, U1>(c);
+    if (grid < 2) return fail(c, LQCD_ECUDA, "the persistent solver does not fit on this device");
+    void* args[] = {(void*)&P};
+    CU(cudaLaunchCooperativeKernel((const void*)cg_persistent_kernel<T, RECON, U1>, dim3(grid), dim3(PS_BLOCK), args, 0,
+                                   c->stream));
+    ++c->launches;
+    return LQCD_OK;
+}
+
+template <typename T>
+int launch_persistent(lqcd_ctx* c) {
+    PrecBufs<T>& B = bufs<T>(c);
+    PersistArgs<T> P{};
+    P.D.g = c->g;
+    P.D.W = B.W;
+    P.D.Th = B.Th;
+    set_policies<T>(c, P.D);
+    P.st = c->st_dev;
+    P.partials = c->partials;
+    P.p = B.p;
+    P.t = B.t;
+    P.p_keep = B.p_keep;
+    P.m = c->shift_block;
+    P.defer_base = defer_base(c);
+    const bool r12 = B.recon_stored == 12;
+    if (c->u1_on) return r12 ? launch_persistent_k<T, 12, 1>(c, P) : launch_persistent_k<T, 18, 1>(c, P);
+    return r12 ? launch_persistent_k<T, 12, 0>(c, P) : launch_persistent_k<T, 18, 0>(c, P);
+}
+
+// The persistent solver pays when the iteration is bound by launch gaps and kernel tails rather than by bandwidth:
+// lattices whose links stay in L2 (links_resident).  LQCD_OPT_PERSISTENT overrides.
+template <typename T>
+bool use_persistent(const lqcd_ctx* c) {
+    if (c->slab || c->persistent_opt == 0) return false;
+    if (!c->coop_launch) return false;
+    return c->persistent_opt == 1 || links_resident<T>(c);
 }
 
 // the host looks at the stop flag every this many iterations: a whole number of blocks
@@ -765,6 +842,7 @@ lqcd_ctx* lqcd_create(int Lx, int Ly, int Lz, int Lt) {
     c->has_comm = false;
     c->device = dev;
     c->num_sms = prop.multiProcessorCount;
+    c->coop_launch = prop.cooperativeLaunch;
     c->stream = nullptr;
     c->mass = 0.0;
     c->recon_opt = 18;
@@ -774,6 +852,7 @@ lqcd_ctx* lqcd_create(int Lx, int Ly, int Lz, int Lt) {
     c->check_every = 0;
     c->use_graph = 1;
     c->shift_block = 16;
+    c->persistent_opt = -1;
     c->err[0] = 0;
     return c;
 }
@@ -925,6 +1004,10 @@ int lqcd_set_option(lqcd_ctx* c, int key, double v) {
                 return fail(c, LQCD_EINVAL, "SHIFT_BLOCK must be an integer in [1, %d]", LQCD_MAX_BLOCK);
             c->shift_block = (int)v;
             break;
+        case LQCD_OPT_PERSISTENT:
+            if (v != -1.0 && v != 0.0 && v != 1.0) return fail(c, LQCD_EINVAL, "PERSISTENT must be -1 (auto), 0 or 1");
+            c->persistent_opt = (int)v;
+            break;
         case LQCD_OPT_LINK_PRECISIONS:
             if (v != 1.0 && v != 2.0 && v != 3.0)
                 return fail(c, LQCD_EINVAL, "LINK_PRECISIONS must be LQCD_PREC_F64 (1), LQCD_PREC_F32 (2) or both (3)");
@@ -947,6 +1030,7 @@ int lqcd_get_option(const lqcd_ctx* c, int key, double* v) {
         case LQCD_OPT_SHIFT_BLOCK: *v = c->shift_block; break;
         case LQCD_OPT_USE_GRAPH: *v = c->use_graph; break;
         case LQCD_OPT_LINK_PRECISIONS: *v = c->prec_opt; break;
+        case LQCD_OPT_PERSISTENT: *v = c->persistent_opt; break;
         default: return LQCD_EINVAL;
     }
     return LQCD_OK;
@@ -967,8 +1051,7 @@ size_t lqcd_workspace_bytes(const lqcd_ctx* c, int nshift) {
         if (c->prec_opt & LQCD_PREC_F64) b += 2 * align_up(6 * face * sizeof(double2)) + align_up(18 * face * sizeof(double2)) + align_up(36 * face * sizeof(double2));
         if (c->prec_opt & LQCD_PREC_F32) b += 2 * align_up(6 * face * sizeof(float2)) + align_up(18 * face * sizeof(float2)) + align_up(36 * face * sizeof(float2));
     }
-    const size_t np = (size_t)(ds_grid(c) > cg_grid(c) ? ds_grid(c) : cg_grid(c)) + 4;
-    b += align_up(np * sizeof(double));
+    b += align_up(n_partials_needed(c) * sizeof(double));
     return b;
 }
 
@@ -1187,14 +1270,20 @@ int solve(lqcd_ctx* c, const T* b_even, const double* shifts, int nshift, double
     CU(cudaGetLastError());
 
     const int ce = check_every(c);
+    const bool persistent = use_persistent<T>(c);
     // the legacy default stream cannot be captured: plain launches there
-    const bool use_graph = c->use_graph && c->stream != nullptr && c->stream != cudaStreamLegacy &&
+    const bool use_graph = !persistent && c->use_graph && c->stream != nullptr && c->stream != cudaStreamLegacy &&
                            (!c->slab || c->comm.graph_safe);
     if (use_graph && (B.graph_iters != ce || B.graph_block != m)) {
         if ((rc = build_graph<T>(c, ce, rational))) return rc;
     }
     c->flag_host[0] = c->flag_host[1] = 0;
     bool done = false;
+    if (persistent) {
+        // one cooperative kernel runs the iterations until the device-side stop (persist.cuh)
+        if ((rc = launch_persistent<T>(c))) return rc;
+        done = true;
+    }
     const long max_batches = (long)c->max_iter / ce + 3;
     for (long batch = 0; batch < max_batches && !done; ++batch) {
         if (use_graph) {

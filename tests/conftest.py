@@ -26,3 +26,20 @@ def pytest_collection_modifyitems(config, items):
     for item in items:
         if "gpu" in item.keywords:
             item.add_marker(skip)
+
+
+@pytest.fixture
+def solver_path(request):
+    """Which of the two drivers of the CG iteration a test runs on (helpers.both_solvers parametrizes it):
+    "launches" = two launches per iteration, as a CUDA graph or plainly (what large lattices get);
+    "persistent" = the whole solve in one cooperative kernel (what lattices that live in L2 get by default)."""
+    import paper_1801_01473_b200 as lq
+    mode = getattr(request, "param", "auto")
+    saved = dict(lq.Lattice.default_options)
+    if mode == "launches":
+        lq.Lattice.default_options[lq.LQCD_OPT_PERSISTENT] = 0
+    elif mode == "persistent":
+        lq.Lattice.default_options[lq.LQCD_OPT_PERSISTENT] = 1
+    yield mode
+    lq.Lattice.default_options.clear()
+    lq.Lattice.default_options.update(saved)

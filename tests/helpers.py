@@ -1,6 +1,7 @@
 """Shared test plumbing: inputs from lqcd_inputs, conversions through the ORACLE's layout helpers.
 Nothing here is used by the product."""
 import numpy as np
+import pytest
 import torch
 
 import lqcd_inputs as gen
@@ -30,3 +31,7 @@ def oracle_parity_vector(L, site_field_np, parity):
 def soa_gpu_to_aos(v) -> np.ndarray:
     """GPU parity vector (3,Vh,2) -> oracle AoS parity field (Vh,3,2), via the oracle's own helper."""
     return oracle.soa_to_aos(v.detach().cpu().numpy())
+
+
+# run a test once on each driver of the CG iteration (conftest.solver_path)
+both_solvers = pytest.mark.parametrize("solver_path", ["launches", "persistent"], indirect=True)

@@ -21,7 +21,7 @@ import torch
 
 import lqcd_inputs as gen
 import oracle
-from helpers import make_inputs, oracle_parity_vector, rel_l2, soa_gpu_to_aos
+from helpers import both_solvers, make_inputs, oracle_parity_vector, rel_l2, soa_gpu_to_aos
 
 pytestmark = pytest.mark.gpu
 
@@ -149,7 +149,10 @@ def check_cg_f32(L, U, mass, b_aos, shifts, tol, x, info, x_ref, info_ref):
 
 @pytest.mark.parametrize("L,mass,shifts,tol", CG_CASES)
 @pytest.mark.parametrize("mode", ["graph", "plain", "recon12", "host"])
-def test_mshift_cg_f32(lq, L, mass, shifts, tol, mode):
+@both_solvers
+def test_mshift_cg_f32(lq, L, mass, shifts, tol, mode, solver_path):
+    if solver_path == "persistent" and mode == "plain":
+        pytest.skip("graph or plain launches: a property of the launch path only")
     if mode != "graph" and L[0] == 16:
         pytest.skip("the 16^4 case runs once")
     U, U32, f = f32_inputs(L)
@@ -169,7 +172,8 @@ def test_mshift_cg_f32(lq, L, mass, shifts, tol, mode):
     lat.close()
 
 
-def test_mshift_cg_f32_fixed_iteration_count_and_rational(lq):
+@both_solvers
+def test_mshift_cg_f32_fixed_iteration_count_and_rational(lq, solver_path):
     """Exactly 30 iterations on both sides (no stopping decision involved): x_i within 30 eps32-ish of the
     oracle; the fused rational sum equals the sum of the stored x_i."""
     L, mass = (8, 8, 8, 8), 0.0075

@@ -10,7 +10,7 @@ import torch
 
 import lqcd_inputs as gen
 import oracle
-from helpers import make_inputs, oracle_parity_vector, rel_l2, soa_gpu_to_aos
+from helpers import both_solvers, make_inputs, oracle_parity_vector, rel_l2, soa_gpu_to_aos
 
 pytestmark = pytest.mark.gpu
 
@@ -158,7 +158,10 @@ def check_cg(x, info, x_ref, info_ref, shifts):
     ((8, 8, 8, 8), 0.01, [1e-4 * 10 ** (i / 2) for i in range(8)]),
 ])
 @pytest.mark.parametrize("mode", ["graph", "plain", "legacy_stream", "recon12", "host"])
-def test_mshift_cg_small(lq, L, mass, shifts, mode):
+@both_solvers
+def test_mshift_cg_small(lq, L, mass, shifts, mode, solver_path):
+    if solver_path == "persistent" and mode == "plain":
+        pytest.skip("graph or plain launches: a property of the launch path only")
     s = None if mode == "legacy_stream" else torch.cuda.Stream()
     x, info, x_ref, info_ref, launches = run_cg_both(
         lq, L, mass, shifts, 1e-10, recon=12 if mode == "recon12" else 18, use_graph=(mode != "plain"),
@@ -167,10 +170,14 @@ def test_mshift_cg_small(lq, L, mass, shifts, mode):
     assert info["rel_res"] <= 1e-10
     assert info["base_shift"] == int(np.argmin(shifts))
     check_cg(x, info, x_ref, info_ref, shifts)
-    assert launches >= 2 * info["iters"] + 2          # two launches per iteration (K1, K2 of cg.cuh) + init + sweeps
+    if solver_path == "launches":
+        assert launches >= 2 * info["iters"] + 2      # two launches per iteration (K1, K2 of cg.cuh) + init + sweeps
+    else:
+        assert launches <= 8                          # links, pack, |b|^2 + ONE kernel for all iterations
 
 
-def test_mshift_cg_config2_16x4(lq):
+@both_solvers
+def test_mshift_cg_config2_16x4(lq, solver_path):
     """BASELINE config 2: 16^4, m = 0.01, 8 shifts 1e-4*10^(i/2), tol 1e-10 -- full solve on both sides."""
     cfg = gen.CONFIGS["config2_16^4"]
     x, info, x_ref, info_ref, _ = run_cg_both(lq, cfg["L"], cfg["mass"], cfg["shifts"], cfg["tol"],
@@ -190,7 +197,8 @@ def test_mshift_cg_config2_16x4(lq):
         assert np.linalg.norm(res) / bn <= 3 * cfg["tol"], (i, np.linalg.norm(res) / bn)
 
 
-def test_mshift_cg_fixed_iteration_count(lq):
+@both_solvers
+def test_mshift_cg_fixed_iteration_count(lq, solver_path):
     """The protocol used at the large configs (R9): both sides run exactly n iterations."""
     L, mass = (8, 8, 8, 8), 0.0075
     shifts = gen.shifts_geometric(1e-5, 1.0, 16)
@@ -203,14 +211,16 @@ def test_mshift_cg_fixed_iteration_count(lq):
 
 
 @pytest.mark.parametrize("check_every", [1, 3, 64])
-def test_mshift_cg_check_every_does_not_change_the_result(lq, check_every):
+@pytest.mark.parametrize("solver_path", ["launches"], indirect=True)      # the host polls only on the launch path
+def test_mshift_cg_check_every_does_not_change_the_result(lq, check_every, solver_path):
     L, mass, shifts = (4, 4, 4, 4), 0.05, [1e-3, 1e-1]
     x, info, x_ref, info_ref, _ = run_cg_both(lq, L, mass, shifts, 1e-10, stream=torch.cuda.Stream(),
                                               check_every=check_every)
     check_cg(x, info, x_ref, info_ref, shifts)
 
 
-def test_mshift_cg_is_bit_reproducible(lq):
+@both_solvers
+def test_mshift_cg_is_bit_reproducible(lq, solver_path):
     L, mass, shifts = (8, 8, 8, 8), 0.02, [1e-3, 1e-2, 1e-1]
     U, f = make_inputs(L)
     b_soa, _ = oracle_parity_vector(L, f.numpy(), 0)
@@ -226,7 +236,8 @@ def test_mshift_cg_is_bit_reproducible(lq):
     lat.close()
 
 
-def test_edge_cases_and_errors(lq):
+@both_solvers
+def test_edge_cases_and_errors(lq, solver_path):
     L = (4, 4, 4, 4)
     U, f = make_inputs(L)
     b_soa, b_aos = oracle_parity_vector(L, f.numpy(), 0)
@@ -273,7 +284,8 @@ def test_edge_cases_and_errors(lq):
     lat.close()
 
 
-def test_caller_workspace(lq):
+@both_solvers
+def test_caller_workspace(lq, solver_path):
     L, mass, shifts = (4, 6, 8, 10), 0.05, [1e-2, 1e-1, 1.0]
     U, f = make_inputs(L)
     b_soa, b_aos = oracle_parity_vector(L, f.numpy(), 0)
@@ -326,7 +338,10 @@ def rational_coefficients(n):
 
 @pytest.mark.parametrize("L,mass,shifts", RATIONAL_CASES)
 @pytest.mark.parametrize("mode", ["graph", "plain", "recon12", "host"])
-def test_rational_apply_small(lq, L, mass, shifts, mode):
+@both_solvers
+def test_rational_apply_small(lq, L, mass, shifts, mode, solver_path):
+    if solver_path == "persistent" and mode == "plain":
+        pytest.skip("graph or plain launches: a property of the launch path only")
     U, f = make_inputs(L)
     b_soa, b_aos = oracle_parity_vector(L, f.numpy(), 0)
     a0, al = rational_coefficients(len(shifts))
@@ -352,7 +367,8 @@ def test_rational_apply_small(lq, L, mass, shifts, mode):
     lat.close()
 
 
-def test_rational_apply_fixed_iteration_count_and_errors(lq):
+@both_solvers
+def test_rational_apply_fixed_iteration_count_and_errors(lq, solver_path):
     L, mass = (8, 8, 8, 8), 0.0075
     shifts = gen.shifts_geometric(1e-5, 1.0, 16)
     a0, al = rational_coefficients(16)

@@ -18,7 +18,7 @@ import torch
 
 import lqcd_inputs as gen
 import oracle
-from helpers import make_inputs, oracle_parity_vector, rel_l2, soa_gpu_to_aos
+from helpers import both_solvers, make_inputs, oracle_parity_vector, rel_l2, soa_gpu_to_aos
 
 pytestmark = pytest.mark.gpu
 
@@ -65,12 +65,13 @@ def test_option_range(lq):
     lat.close()
 
 
+@both_solvers
 @pytest.mark.parametrize("L,mass,shifts", [
     ((4, 4, 4, 4), 0.05, [1e-3, 1e-2, 1e-1, 1.0]),
     ((4, 6, 8, 10), 0.02, [1e-2, 1e-3, 1e-1, 1.0, 0.5]),
     ((8, 8, 8, 8), 0.01, [1e-4 * 10 ** (i / 2) for i in range(8)]),
 ])
-def test_every_block_length_gives_the_same_solve(lq, L, mass, shifts):
+def test_every_block_length_gives_the_same_solve(lq, L, mass, shifts, solver_path):
     U, f = make_inputs(L)
     b_soa, b_aos = oracle_parity_vector(L, f.numpy(), 0)
     x_ref, info_ref = oracle.mshift_cg(L, U.numpy(), mass, b_aos, shifts, 1e-10)
@@ -90,8 +91,9 @@ def test_every_block_length_gives_the_same_solve(lq, L, mass, shifts):
     lat.close()
 
 
+@both_solvers
 @pytest.mark.parametrize("n_iter", [1, 2, 7, 8, 9, 15, 16, 17, 23, 40])
-def test_stop_in_the_middle_of_a_block(lq, n_iter):
+def test_stop_in_the_middle_of_a_block(lq, n_iter, solver_path):
     """MAX_ITER = n_iter with tol tiny: both sides do exactly n_iter iterations; for m = 8 and 16 the stop falls
     at every position of a block (including its first and last iteration); some shifts freeze on the way."""
     L, mass = (8, 8, 8, 8), 0.0075
@@ -110,7 +112,8 @@ def test_stop_in_the_middle_of_a_block(lq, n_iter):
     lat.close()
 
 
-def test_freeze_in_the_middle_of_a_block(lq):
+@both_solvers
+def test_freeze_in_the_middle_of_a_block(lq, solver_path):
     """Loose tolerance: the large shifts freeze after a handful of iterations, i.e. inside the first blocks;
     their x_i must stop moving exactly there (the oracle's do)."""
     L, mass = (8, 8, 8, 8), 0.05
@@ -135,8 +138,9 @@ def test_freeze_in_the_middle_of_a_block(lq):
     lat.close()
 
 
+@both_solvers
 @pytest.mark.parametrize("m", [1, 4, 7, 16])
-def test_rational_sum_with_blocks(lq, m):
+def test_rational_sum_with_blocks(lq, m, solver_path):
     L, mass = (8, 8, 8, 8), 0.01
     shifts = [1e-4 * 10 ** (i / 2) for i in range(8)]
     a0, al = rational_coefficients(len(shifts))
@@ -165,7 +169,8 @@ def test_rational_sum_with_blocks(lq, m):
     lat.close()
 
 
-def test_single_precision_with_blocks(lq):
+@both_solvers
+def test_single_precision_with_blocks(lq, solver_path):
     L, mass, shifts = (8, 8, 8, 8), 0.05, [1e-3, 1e-2, 1e-1, 1.0]
     U, f = make_inputs(L)
     U32 = U.float().double()

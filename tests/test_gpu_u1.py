@@ -13,7 +13,7 @@ import torch
 
 import lqcd_inputs as gen
 import oracle
-from helpers import make_inputs, oracle_parity_vector, rel_l2, soa_gpu_to_aos
+from helpers import both_solvers, make_inputs, oracle_parity_vector, rel_l2, soa_gpu_to_aos
 
 pytestmark = pytest.mark.gpu
 
@@ -126,7 +126,8 @@ def test_dslash_f32_with_u1_phases(lq, recon):
 
 
 @pytest.mark.parametrize("use_graph", [True, False])
-def test_mshift_cg_with_u1_phases(lq, use_graph):
+@both_solvers
+def test_mshift_cg_with_u1_phases(lq, use_graph, solver_path):
     L, mass, tol = (8, 8, 8, 8), 0.05, 1e-10
     shifts = [1e-3, 1e-2, 1e-1, 1.0]
     U, f = make_inputs(L)
