@@ -81,11 +81,13 @@ typedef struct lqcd_ctx lqcd_ctx;
 #define LQCD_OPT_LINK_PRECISIONS 6  /* which copies of the links the next lqcd_set_gauge stores: LQCD_PREC_F64
                                        (default; serves the double entry points), LQCD_PREC_F32 (serves the
                                        *_f32 entry points), or both OR-ed together                         */
-#define LQCD_OPT_SHIFT_BLOCK     7  /* m in [1,16], default 16: the x_i, p_i of the shifted systems (and x_0 of the
-                                       base system) are updated once per block of m iterations from the m
-                                       residuals of the block (kept in m vectors) instead of once per iteration;
-                                       same recurrences, same iteration counts, x_i equal up to rounding.
-                                       m = 1: every iteration.  CHECK_EVERY is rounded up to a multiple of m. */
+#define LQCD_OPT_SHIFT_BLOCK     7  /* m in [1,32]; 0 (default) = chosen by the library (32; 16 on lattices small enough
+                                       to live in L2).  The x_i, p_i of the shifted systems (and x_0 of the base
+                                       system) are updated once per block of m iterations from the m residuals of the
+                                       block (kept in m vectors) instead of once per iteration; same recurrences, same
+                                       iteration counts, x_i equal up to rounding.  m = 1: every iteration.
+                                       CHECK_EVERY is rounded up to a multiple of m.  lqcd_get_option returns the
+                                       value in force.                                                         */
 #define LQCD_OPT_PERSISTENT      8  /* -1 (default): lattices whose stored links stay in L2 (e.g. 16^4) are solved by ONE
                                        cooperative kernel that runs all iterations with grid-wide barriers between the
                                        sweeps (no launch gaps, no host polling); larger ones by two launches per

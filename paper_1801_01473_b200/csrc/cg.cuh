@@ -190,12 +190,16 @@ __global__ void __launch_bounds__(CG_BLOCK) cg_update_base_kernel(const V2<T>* _
 // FLUSH_UNR = shifted systems whose x_i, p_i loads are in flight together.  The sweep is latency-bound at the
 // 2 blocks per SM its registers allow (ncu: long-scoreboard stalls, 25 % occupancy): 4 shifts (8 x 16 B per
 // thread) in flight instead of 2 took it from 5.6 to 6.3 TB/s at 48^4 (profiles/ncu_full_r01.md).
-#define FLUSH_UNR 4
-template <typename T, int MM, bool RATIONAL, bool FULL>
+#ifndef FLUSH_UNR
+#define FLUSH_UNR 8          // MM <= 16
+#endif
+#ifndef FLUSH_UNR_LONG
+#define FLUSH_UNR_LONG 4     // MM = 32: the 32 residuals of a site already take 128 registers
+#endif
+template <typename T, int MM, bool RATIONAL, bool FULL, int U>
 __device__ __forceinline__ void cg_flush_body(const int nres, const int nl, const int e_base, V2<T>* const* sx, V2<T>* const* sp,
                                               const V2<T>* const* sr, const T* sCP, const T* sB, const V2<T>* sDE,
                                               const T* sY, V2<T>* __restrict__ y, const size_t n) {
-    constexpr int U = FLUSH_UNR;
     const size_t stride = (size_t)gridDim.x * blockDim.x;
     for (size_t j = (size_t)blockIdx.x * blockDim.x + threadIdx.x; j < n; j += stride) {
         V2<T> rv[MM];
@@ -257,7 +261,7 @@ __device__ __forceinline__ void cg_flush_body(const int nres, const int nl, cons
 
 // The sweep as a block-level function (every thread of every block of the grid calls it; blockDim.x >=
 // LQCD_MAX_SHIFTS + MM): used by cg_flush_kernel and, between grid-wide barriers, by the persistent solver.
-template <typename T, int MM>
+template <typename T, int MM, int U = ((MM <= 16) ? FLUSH_UNR : FLUSH_UNR_LONG)>
 __device__ __forceinline__ void cg_flush_block(const CgState* st, const size_t n, const int nres) {
     __shared__ V2<T>* sx[LQCD_MAX_SHIFTS];
     __shared__ V2<T>* sp[LQCD_MAX_SHIFTS];
@@ -309,11 +313,11 @@ __device__ __forceinline__ void cg_flush_block(const CgState* st, const size_t n
     V2<T>* __restrict__ y = (V2<T>*)st->y;
     if (nl > 0) {
         if (rational) {
-            if (nres == MM) cg_flush_body<T, MM, true, true>(nres, nl, s_ebase, sx, sp, sr, sCP, sB, sDE, sY, y, n);
-            else cg_flush_body<T, MM, true, false>(nres, nl, s_ebase, sx, sp, sr, sCP, sB, sDE, sY, y, n);
+            if (nres == MM) cg_flush_body<T, MM, true, true, U>(nres, nl, s_ebase, sx, sp, sr, sCP, sB, sDE, sY, y, n);
+            else cg_flush_body<T, MM, true, false, U>(nres, nl, s_ebase, sx, sp, sr, sCP, sB, sDE, sY, y, n);
         } else {
-            if (nres == MM) cg_flush_body<T, MM, false, true>(nres, nl, s_ebase, sx, sp, sr, sCP, sB, sDE, sY, y, n);
-            else cg_flush_body<T, MM, false, false>(nres, nl, s_ebase, sx, sp, sr, sCP, sB, sDE, sY, y, n);
+            if (nres == MM) cg_flush_body<T, MM, false, true, U>(nres, nl, s_ebase, sx, sp, sr, sCP, sB, sDE, sY, y, n);
+            else cg_flush_body<T, MM, false, false, U>(nres, nl, s_ebase, sx, sp, sr, sCP, sB, sDE, sY, y, n);
         }
     }
 }

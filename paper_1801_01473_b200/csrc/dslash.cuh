@@ -297,7 +297,7 @@ struct DslashArgs {
 
 // registers: double needs ~126 (4 blocks of 128 threads per SM); single fits 6 blocks
 #ifndef DS_MINB_K1
-#define DS_MINB_K1 DS_MINB
+#define DS_MINB_K1 3     // K1 loads two vectors per neighbour: 168 registers (3 blocks) keep more loads in flight than 128
 #endif
 #ifndef DS_MINB_K2
 #define DS_MINB_K2 DS_MINB

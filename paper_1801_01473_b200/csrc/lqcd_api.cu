@@ -27,6 +27,10 @@ thread_local char g_create_error[256] = "";
 constexpr size_t ALIGN = 256;
 inline size_t align_up(size_t b) { return (b + ALIGN - 1) / ALIGN * ALIGN; }
 
+#ifndef LINKS_RESIDENT_MAX
+#define LINKS_RESIDENT_MAX (48u << 20)
+#endif
+
 }  // namespace
 
 // everything that exists once per precision T (double: the default path; float: the *_f32 entry points)
@@ -68,7 +72,8 @@ struct lqcd_ctx {
 
     // options
     double mass;
-    int recon_opt, max_iter, check_every, use_graph, shift_block;
+    int recon_opt, max_iter, check_every, use_graph;
+    int shift_block_opt;     // LQCD_OPT_SHIFT_BLOCK: 0 = chosen from the lattice size (block_len())
     int persistent_opt;      // LQCD_OPT_PERSISTENT: -1 = the library decides (lattices that live in L2), 0 = never, 1 = always
 
     // memory
@@ -194,6 +199,15 @@ void drop_graphs(lqcd_ctx* c) {
     drop_graph<float>(c);
 }
 
+// Block length m of the deferred shift updates (cg.cuh).  Default: 32 -- the longer the block, the fewer bytes per
+// iteration (48 + 192 (n_act-1)/m + 144/m per site) -- except on lattices small enough to live in L2, which get 16,
+// the longest block the persistent solver handles (persist.cuh).
+int block_len(const lqcd_ctx* c) {
+    if (c->shift_block_opt) return c->shift_block_opt;
+    const size_t smallest_links = (size_t)8 * 6 * c->Vh * sizeof(float2);          // float, two rows
+    return smallest_links <= LINKS_RESIDENT_MAX ? 16 : 32;
+}
+
 template <typename T> size_t vec_bytes(const lqcd_ctx* c) { return c->Vh * 3 * sizeof(V2<T>); }
 template <typename T> size_t links_bytes(const lqcd_ctx* c, int recon) {
     return (size_t)8 * (recon == 12 ? 6 : 9) * c->Vh * sizeof(V2<T>);
@@ -203,9 +217,6 @@ template <typename T> size_t links_bytes(const lqcd_ctx* c, int recon) {
 // read by SMs of both dies may sit in both).  Measured at 16^4 (37.7 MB of links): with the streaming policy every
 // application re-read them from DRAM (40 MB per launch under ncu --cache-control none); kept, one application in a
 // graph takes 4.5 us = 9.6 TB/s out of L2.
-#ifndef LINKS_RESIDENT_MAX
-#define LINKS_RESIDENT_MAX (48u << 20)
-#endif
 template <typename T> int links_resident(const lqcd_ctx* c) {
     const int ne = (bufs_c<T>(c).recon_stored == 12) ? 6 : 9;
     return (size_t)8 * ne * c->Vh * sizeof(V2<T>) <= LINKS_RESIDENT_MAX ? 1 : 0;
@@ -286,7 +297,7 @@ int ensure_solver(lqcd_ctx* c, int nshift) {
     int rc;
     if ((rc = ensure_tmp<T>(c))) return rc;
     PrecBufs<T>& B = bufs<T>(c);
-    while (B.n_hist < c->shift_block) {
+    while (B.n_hist < block_len(c)) {
         if ((rc = dev_alloc(c, (void**)&B.hist[B.n_hist], vec_bytes<T>(c)))) return rc;
         ++B.n_hist;
     }
@@ -529,16 +540,17 @@ void launch_cg_fused(lqcd_ctx* c, const V2<T>* r_in, V2<T>* r_out, V2<T>* p_keep
 }
 
 // whole lattice, m >= 2: x_0 of the base system is updated by the block sweep too (CgState::defer_base)
-int defer_base(const lqcd_ctx* c) { return (!c->slab && c->shift_block >= 2) ? 1 : 0; }
+int defer_base(const lqcd_ctx* c) { return (!c->slab && block_len(c) >= 2) ? 1 : 0; }
 
 // the sweep over the shifted systems that closes a block of iterations (K5 of cg.cuh)
 template <typename T>
 void launch_flush(lqcd_ctx* c) {
     const size_t n = c->Vh * 3;
-    const int m = c->shift_block;
+    const int m = block_len(c);
     if (m <= 4) cg_flush_kernel<T, 4><<<cg_grid(c), CG_BLOCK, 0, c->stream>>>(c->st_dev, n);
     else if (m <= 8) cg_flush_kernel<T, 8><<<cg_grid(c), CG_BLOCK, 0, c->stream>>>(c->st_dev, n);
-    else cg_flush_kernel<T, 16><<<cg_grid(c), CG_BLOCK, 0, c->stream>>>(c->st_dev, n);
+    else if (m <= 16) cg_flush_kernel<T, 16><<<cg_grid(c), CG_BLOCK, 0, c->stream>>>(c->st_dev, n);
+    else cg_flush_kernel<T, 32><<<cg_grid(c), CG_BLOCK, 0, c->stream>>>(c->st_dev, n);
     ++c->launches;
 }
 
@@ -546,7 +558,7 @@ void launch_flush(lqcd_ctx* c) {
 template <typename T>
 int launch_cg_iteration(lqcd_ctx* c, int pos) {
     const size_t n = c->Vh * 3;
-    const int m = c->shift_block;
+    const int m = block_len(c);
     PrecBufs<T>& B = bufs<T>(c);
     if (c->slab) {
         // the same iteration with the two exchange steps of the slab decomposition: faces before each operator,
@@ -610,7 +622,7 @@ int launch_persistent(lqcd_ctx* c) {
     P.p = B.p;
     P.t = B.t;
     P.p_keep = B.p_keep;
-    P.m = c->shift_block;
+    P.m = block_len(c);
     P.defer_base = defer_base(c);
     const bool r12 = B.recon_stored == 12;
     if (c->u1_on) return r12 ? launch_persistent_k<T, 12, 1>(c, P) : launch_persistent_k<T, 18, 1>(c, P);
@@ -622,7 +634,7 @@ int launch_persistent(lqcd_ctx* c) {
 template <typename T>
 bool use_persistent(const lqcd_ctx* c) {
     if (c->slab || c->persistent_opt == 0) return false;
-    if (!c->coop_launch) return false;
+    if (!c->coop_launch || block_len(c) > PS_MAX_BLOCK) return false;
     return c->persistent_opt == 1 || links_resident<T>(c);
 }
 
@@ -631,7 +643,7 @@ int check_every(const lqcd_ctx* c) {
     long v = c->check_every ? (long)c->check_every : (long)(4000000 / (long)c->Vh);
     if (v < 1) v = 1;
     if (!c->check_every && v > 64) v = 64;
-    const long m = c->shift_block;
+    const long m = block_len(c);
     return (int)((v + m - 1) / m * m);
 }
 
@@ -644,7 +656,7 @@ int build_graph(lqcd_ctx* c, int iters, int rational) {
     const long long before = c->launches;
     CU(cudaStreamBeginCapture(c->stream, cudaStreamCaptureModeThreadLocal));
     int rc_it = LQCD_OK;
-    for (int i = 0; i < iters && !rc_it; ++i) rc_it = launch_cg_iteration<T>(c, i % c->shift_block);
+    for (int i = 0; i < iters && !rc_it; ++i) rc_it = launch_cg_iteration<T>(c, i % block_len(c));
     cudaError_t e = cudaStreamEndCapture(c->stream, &graph);
     B.graph_launches = (int)(c->launches - before);
     c->launches = before;     // capturing is not launching
@@ -661,7 +673,7 @@ int build_graph(lqcd_ctx* c, int iters, int rational) {
     }
     B.graph_iters = iters;
     B.graph_rational = rational;
-    B.graph_block = c->shift_block;
+    B.graph_block = block_len(c);
     return LQCD_OK;
 }
 
@@ -851,7 +863,7 @@ lqcd_ctx* lqcd_create(int Lx, int Ly, int Lz, int Lt) {
     c->max_iter = 100000;
     c->check_every = 0;
     c->use_graph = 1;
-    c->shift_block = 16;
+    c->shift_block_opt = 0;
     c->persistent_opt = -1;
     c->err[0] = 0;
     return c;
@@ -1000,9 +1012,9 @@ int lqcd_set_option(lqcd_ctx* c, int key, double v) {
             c->use_graph = (int)v;
             break;
         case LQCD_OPT_SHIFT_BLOCK:
-            if (!(v >= 1.0) || v > (double)LQCD_MAX_BLOCK || v != std::floor(v))
-                return fail(c, LQCD_EINVAL, "SHIFT_BLOCK must be an integer in [1, %d]", LQCD_MAX_BLOCK);
-            c->shift_block = (int)v;
+            if (!(v >= 0.0) || v > (double)LQCD_MAX_BLOCK || v != std::floor(v))
+                return fail(c, LQCD_EINVAL, "SHIFT_BLOCK must be an integer in [1, %d], or 0 (chosen by the library)", LQCD_MAX_BLOCK);
+            c->shift_block_opt = (int)v;
             break;
         case LQCD_OPT_PERSISTENT:
             if (v != -1.0 && v != 0.0 && v != 1.0) return fail(c, LQCD_EINVAL, "PERSISTENT must be -1 (auto), 0 or 1");
@@ -1027,7 +1039,7 @@ int lqcd_get_option(const lqcd_ctx* c, int key, double* v) {
         case LQCD_OPT_RECON: *v = c->recon_opt; break;
         case LQCD_OPT_MAX_ITER: *v = c->max_iter; break;
         case LQCD_OPT_CHECK_EVERY: *v = check_every(c); break;
-        case LQCD_OPT_SHIFT_BLOCK: *v = c->shift_block; break;
+        case LQCD_OPT_SHIFT_BLOCK: *v = block_len(c); break;
         case LQCD_OPT_USE_GRAPH: *v = c->use_graph; break;
         case LQCD_OPT_LINK_PRECISIONS: *v = c->prec_opt; break;
         case LQCD_OPT_PERSISTENT: *v = c->persistent_opt; break;
@@ -1040,9 +1052,9 @@ size_t lqcd_workspace_bytes(const lqcd_ctx* c, int nshift) {
     if (!c || nshift < 1 || nshift > LQCD_MAX_SHIFTS) return 0;
     size_t b = 0;
     if (c->prec_opt & LQCD_PREC_F64)
-        b += align_up(links_bytes<double>(c, 18)) + align_up(vec_bytes<double>(c)) * (size_t)(3 + c->shift_block + (nshift - 1));
+        b += align_up(links_bytes<double>(c, 18)) + align_up(vec_bytes<double>(c)) * (size_t)(3 + block_len(c) + (nshift - 1));
     if (c->prec_opt & LQCD_PREC_F32)
-        b += align_up(links_bytes<float>(c, 18)) + align_up(vec_bytes<float>(c)) * (size_t)(3 + c->shift_block + (nshift - 1));
+        b += align_up(links_bytes<float>(c, 18)) + align_up(vec_bytes<float>(c)) * (size_t)(3 + block_len(c) + (nshift - 1));
     if (c->prec_opt & LQCD_PREC_F64) b += align_up((size_t)8 * c->Vh * sizeof(double));   // U(1) angles, if set
     if (c->prec_opt & LQCD_PREC_F32) b += align_up((size_t)8 * c->Vh * sizeof(float));
     b += align_up(sizeof(CgState)) + align_up(sizeof(double)) + align_up(2 * sizeof(double));
@@ -1246,7 +1258,7 @@ int solve(lqcd_ctx* c, const T* b_even, const double* shifts, int nshift, double
         h->alpha[i] = rational ? alpha[i] : 0.0;
         h->p[i] = (i == i0) ? (void*)B.p : (void*)B.pextra[extra++];
     }
-    const int m = c->shift_block;
+    const int m = block_len(c);
     h->blk_m = m;
     for (int l = 0; l < m; ++l) h->hist[l] = (void*)B.hist[l];
     h->rational = rational;
@@ -1284,7 +1296,9 @@ int solve(lqcd_ctx* c, const T* b_even, const double* shifts, int nshift, double
         if ((rc = launch_persistent<T>(c))) return rc;
         done = true;
     }
-    const long max_batches = (long)c->max_iter / ce + 3;
+    // MAX_ITER is reached inside batch number ceil(MAX_ITER / ce) at the latest: nothing is launched beyond it (the
+    // kernels of a launch whose solve is over return at once, but 2 x 20,000 empty blocks per iteration are not free)
+    const long max_batches = ((long)c->max_iter + ce - 1) / ce;
     for (long batch = 0; batch < max_batches && !done; ++batch) {
         if (use_graph) {
             CU(cudaGraphLaunch(B.graph_exec, c->stream));
@@ -1359,7 +1373,7 @@ int mixed_solve_one(lqcd_ctx* c, const double* b, double sigma, double tol, doub
     PrecBufs<float>& F = bufs<float>(c);
     PrecBufs<double>& D = bufs<double>(c);
     const size_t n = c->Vh * 3;
-    const int m = c->shift_block;
+    const int m = block_len(c);
     const double2* b2 = (const double2*)b;
     double2* x2 = (double2*)x;
     double2* ax = D.stage_x[0];           // (A + sigma) x

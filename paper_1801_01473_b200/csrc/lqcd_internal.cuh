@@ -30,7 +30,9 @@ struct Geom {
     int t_off, Lt_glob;             // slab mode: this lattice is time slices [t_off, t_off+Lt) of Lt_glob
 };
 
-#define LQCD_MAX_BLOCK 16           // longest block of iterations whose shift updates are applied in one sweep
+#ifndef LQCD_MAX_BLOCK
+#define LQCD_MAX_BLOCK 32           // longest block of iterations whose shift updates are applied in one sweep
+#endif
 
 // Device-resident state of one multi-shift CG solve (steps A6, A9): every scalar of the recurrence
 // lives here, so an iteration needs no host round trip.

@@ -34,6 +34,8 @@
 #ifndef PS_BLOCK
 #define PS_BLOCK 256
 #endif
+// longest block of deferred updates the persistent solver handles (registers of the sweep)
+#define PS_MAX_BLOCK 16
 static_assert(PS_BLOCK >= LQCD_MAX_SHIFTS + LQCD_MAX_BLOCK, "scalar step and sweep set-up need one thread per shift / residual");
 
 template <typename T>
@@ -66,7 +68,7 @@ __global__ void __launch_bounds__(PS_BLOCK, 1) cg_persistent_kernel(const Persis
     const int nsb = (int)gridDim.x - 1;                     // blocks that own sites
     const bool scalar_block = ((int)blockIdx.x == nsb);
     // sites are dealt out evenly: block b owns the contiguous range [b*chunk, (b+1)*chunk), so that every SM carries
-    // the same load even when there are fewer sites than resident threads (16^4: 111 sites for each of 295 blocks)
+    // the same load even when there are fewer sites than resident threads (16^4: 223 sites for each of 147 blocks)
     const int chunk = (g.Vh + nsb - 1) / nsb;
     const int k_begin = scalar_block ? g.Vh : min((int)blockIdx.x * chunk, g.Vh);
     const int k_end = scalar_block ? g.Vh : min(k_begin + chunk, g.Vh);
@@ -74,7 +76,7 @@ __global__ void __launch_bounds__(PS_BLOCK, 1) cg_persistent_kernel(const Persis
     double* part1 = P.partials;
     double* part2 = P.partials + gridDim.x;
 
-    // the scalars every block carries (block 0 keeps the device state in step with them)
+    // the scalars every block carries (the scalar block keeps the device state in step with them)
     double rr = st->rr, beta = st->b_prev;
     const double tol2bb = st->tol2bb, c0 = st->c0;
     const int max_iter = st->max_iter, rational = st->rational, i0 = st->i0;
@@ -154,7 +156,7 @@ __global__ void __launch_bounds__(PS_BLOCK, 1) cg_persistent_kernel(const Persis
         const int nres = breakdown ? pos : pos + 1;          // iterations accumulated in the current block
         if ((pos == m - 1 || stop) && nres > 0) {
             grid.sync();                                     // the scalar block's coefficients are visible
-            cg_flush_block<T, LQCD_MAX_BLOCK>(st, 3 * vh, nres);
+            cg_flush_block<T, PS_MAX_BLOCK, 4>(st, 3 * vh, nres);     // 4 systems in flight: the registers this kernel has
             close_block = true;
         }
         if (stop) break;
