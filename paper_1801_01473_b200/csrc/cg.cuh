@@ -22,8 +22,11 @@
 #define CG_BLOCK 256
 static_assert(CG_BLOCK >= LQCD_MAX_SHIFTS, "the scalar step needs one thread per shift");
 
-// K0: r = p_i = b, x_i = 0, |b|^2.  In every sweep the vectors are V2<T>; scalars and sums are double.
-// r is the ring slot that holds r^(n0) of the first block.
+// K0: r = p = b (base system), |b|^2.  In every sweep the vectors are V2<T>; scalars and sums are double.
+// r is the ring slot that holds r^(n0) of the first block.  The shifted p_i = b and the x_i = 0 are NOT written here:
+// the first block sweep produces them (CgState::first_block), which saves 2 x nshift vector writes and nshift + 1
+// vector reads per solve.  Only what is read before that sweep is initialised: the base p, x_0 when it is updated
+// every iteration (no deferral), and y = alpha0 b in rational-sum mode.
 // FUSED = false (slab mode): only the block partial is written; the sum over blocks and ranks and the scalar
 // step follow in sum_partials_kernel / cg_scalar_kernel.
 template <typename T, bool FUSED = true>
@@ -31,21 +34,19 @@ __global__ void __launch_bounds__(CG_BLOCK) cg_init_kernel(const V2<T>* __restri
                                                            CgState* st, double* partials, size_t n, double tol) {
     __shared__ double red[32];
     __shared__ int last_flag;
-    const int ns = st->nshift;
     const int rational = st->rational;
     const T alpha0 = (T)st->alpha0;
     V2<T>* __restrict__ y = (V2<T>*)st->y;
+    V2<T>* __restrict__ p0 = (V2<T>*)st->p[st->i0];
+    V2<T>* __restrict__ x0 = (!rational && !st->defer_base) ? (V2<T>*)st->x[st->i0] : nullptr;
     double acc = 0.0;
     const V2<T> zero = make_v2((T)0, (T)0);
     for (size_t j = (size_t)blockIdx.x * CG_BLOCK + threadIdx.x; j < n; j += (size_t)gridDim.x * CG_BLOCK) {
         const V2<T> v = b[j];
         r[j] = v;
-        for (int i = 0; i < ns; ++i) ((V2<T>*)st->p[i])[j] = v;
-        if (rational) {
-            y[j] = make_v2(alpha0 * v.x, alpha0 * v.y);
-        } else {
-            for (int i = 0; i < ns; ++i) ((V2<T>*)st->x[i])[j] = zero;
-        }
+        p0[j] = v;
+        if (rational) y[j] = make_v2(alpha0 * v.x, alpha0 * v.y);
+        if (x0) x0[j] = zero;
         acc = fma((double)v.x, (double)v.x, acc);
         acc = fma((double)v.y, (double)v.y, acc);
     }
@@ -197,7 +198,8 @@ __global__ void __launch_bounds__(CG_BLOCK) cg_update_base_kernel(const V2<T>* _
 #define FLUSH_UNR_LONG 4     // MM = 32: the 32 residuals of a site already take 128 registers
 #endif
 template <typename T, int MM, bool RATIONAL, bool FULL, int U>
-__device__ __forceinline__ void cg_flush_body(const int nres, const int nl, const int e_base, V2<T>* const* sx, V2<T>* const* sp,
+__device__ __forceinline__ void cg_flush_body(const int nres, const int nl, const int e_base, const bool first,
+                                              V2<T>* const* sx, V2<T>* const* sp, const V2<T>* const* sq,
                                               const V2<T>* const* sr, const T* sCP, const T* sB, const V2<T>* sDE,
                                               const T* sY, V2<T>* __restrict__ y, const size_t n) {
     const size_t stride = (size_t)gridDim.x * blockDim.x;
@@ -222,8 +224,8 @@ __device__ __forceinline__ void cg_flush_body(const int nres, const int nl, cons
 #pragma unroll
             for (int u = 0; u < U; ++u) {
                 const int e = min(e0 + u, nl - 1);
-                pv[u] = sp[e][j];
-                if (!RATIONAL) xv[u] = sx[e][j];
+                pv[u] = sq[e][j];                              // first block: the source b for every shifted system
+                if (!RATIONAL) xv[u] = first ? make_v2((T)0, (T)0) : sx[e][j];
             }
 #pragma unroll
             for (int u = 0; u < U; ++u) {
@@ -264,7 +266,9 @@ __device__ __forceinline__ void cg_flush_body(const int nres, const int nl, cons
 template <typename T, int MM, int U = ((MM <= 16) ? FLUSH_UNR : FLUSH_UNR_LONG)>
 __device__ __forceinline__ void cg_flush_block(const CgState* st, const size_t n, const int nres) {
     __shared__ V2<T>* sx[LQCD_MAX_SHIFTS];
-    __shared__ V2<T>* sp[LQCD_MAX_SHIFTS];
+    __shared__ V2<T>* sp[LQCD_MAX_SHIFTS];           // p_i as written
+    __shared__ const V2<T>* sq[LQCD_MAX_SHIFTS];     // P as read: p_i, p_keep (base system), or b in the first block
+    const bool first = st->first_block != 0;
     __shared__ const V2<T>* sr[MM];
     __shared__ T sCP[LQCD_MAX_SHIFTS], sB[LQCD_MAX_SHIFTS], sY[MM];
     __shared__ V2<T> sDE[LQCD_MAX_SHIFTS * MM];
@@ -290,11 +294,12 @@ __device__ __forceinline__ void cg_flush_block(const CgState* st, const size_t n
     if (inb) {
         const int e = __popc(bal & ((1u << (tid & 31)) - 1u)) + ((tid >= 32) ? cnt[0] : 0);
         sx[e] = (V2<T>*)st->x[tid];
+        sp[e] = (V2<T>*)st->p[tid];
         if (tid == st->i0) {                     // block-deferred base system: P = p^(n0), read only
-            sp[e] = (V2<T>*)st->p_keep;
+            sq[e] = (const V2<T>*)st->p_keep;
             s_ebase = e;
         } else {
-            sp[e] = (V2<T>*)st->p[tid];
+            sq[e] = first ? (const V2<T>*)st->b_src : (const V2<T>*)st->p[tid];
         }
         sCP[e] = (T)st->blk_CP[tid];
         sB[e] = (T)st->blk_B[tid];
@@ -313,11 +318,11 @@ __device__ __forceinline__ void cg_flush_block(const CgState* st, const size_t n
     V2<T>* __restrict__ y = (V2<T>*)st->y;
     if (nl > 0) {
         if (rational) {
-            if (nres == MM) cg_flush_body<T, MM, true, true, U>(nres, nl, s_ebase, sx, sp, sr, sCP, sB, sDE, sY, y, n);
-            else cg_flush_body<T, MM, true, false, U>(nres, nl, s_ebase, sx, sp, sr, sCP, sB, sDE, sY, y, n);
+            if (nres == MM) cg_flush_body<T, MM, true, true, U>(nres, nl, s_ebase, first, sx, sp, sq, sr, sCP, sB, sDE, sY, y, n);
+            else cg_flush_body<T, MM, true, false, U>(nres, nl, s_ebase, first, sx, sp, sq, sr, sCP, sB, sDE, sY, y, n);
         } else {
-            if (nres == MM) cg_flush_body<T, MM, false, true, U>(nres, nl, s_ebase, sx, sp, sr, sCP, sB, sDE, sY, y, n);
-            else cg_flush_body<T, MM, false, false, U>(nres, nl, s_ebase, sx, sp, sr, sCP, sB, sDE, sY, y, n);
+            if (nres == MM) cg_flush_body<T, MM, false, true, U>(nres, nl, s_ebase, first, sx, sp, sq, sr, sCP, sB, sDE, sY, y, n);
+            else cg_flush_body<T, MM, false, false, U>(nres, nl, s_ebase, first, sx, sp, sq, sr, sCP, sB, sDE, sY, y, n);
         }
     }
 }
@@ -335,6 +340,7 @@ __global__ void __launch_bounds__(CG_BLOCK, (MM <= 8 ? 2 : 1)) cg_flush_kernel(C
         if (t == gridDim.x - 1) {
             st->ticket[3] = 0;
             st->blk_j = 0;
+            st->first_block = 0;
         }
     }
 }

@@ -1266,6 +1266,7 @@ int solve(lqcd_ctx* c, const T* b_even, const double* shifts, int nshift, double
     h->y = (void*)y;
     h->defer_base = defer_base(c);
     h->p_keep = (void*)B.p_keep;
+    h->b_src = (const void*)b_even;
     const size_t n = c->Vh * 3;
     CU(cudaMemcpyAsync(c->st_dev, h, sizeof(CgState), cudaMemcpyHostToDevice, c->stream));
     CU(cudaEventRecord(c->ev_t0, c->stream));
@@ -1321,6 +1322,11 @@ int solve(lqcd_ctx* c, const T* b_even, const double* shifts, int nshift, double
     CU(cudaStreamSynchronize(c->stream));
     CU(cudaEventElapsedTime(&c->last_ms, c->ev_t0, c->ev_t1));
 
+    if (h->iter == 0 && !rational) {
+        // nothing was ever accumulated (zero source, or breakdown in the first iteration): no sweep has written the x_i
+        for (int i = 0; i < nshift; ++i) CU(cudaMemsetAsync(x[i], 0, n * sizeof(V2<T>), c->stream));
+        CU(cudaStreamSynchronize(c->stream));
+    }
     c->last_iters = h->iter;
     c->last_i0 = i0;
     c->last_nshift = nshift;
@@ -1393,6 +1399,7 @@ int mixed_solve_one(lqcd_ctx* c, const double* b, double sigma, double tol, doub
     for (int l = 0; l < m; ++l) h->hist[l] = (void*)F.hist[l];
     h->defer_base = defer_base(c);
     h->p_keep = (void*)F.p_keep;
+    h->b_src = (const void*)r0;
     CU(cudaMemcpyAsync(c->st_dev, h, sizeof(CgState), cudaMemcpyHostToDevice, c->stream));
 
     if (have_guess) {
@@ -1412,6 +1419,7 @@ int mixed_solve_one(lqcd_ctx* c, const double* b, double sigma, double tol, doub
     *rel_out = std::sqrt(rr_true / bb);
     if (rr_true <= target) return LQCD_OK;
 
+    CU(cudaMemsetAsync(y, 0, n * sizeof(float2), c->stream));       // should the float solver stop before its first sweep
     // tol of the float solver is relative to ITS source (the starting residual): same absolute target
     cg_init_kernel<float><<<cg_grid(c), CG_BLOCK, 0, c->stream>>>(r0, F.hist[m - 1], c->st_dev, c->partials, n,
                                                                  tol * std::sqrt(bb / rr_true));

@@ -70,6 +70,10 @@ struct CgState {
     // first iteration, which is what the sweep needs besides the block's residuals.
     int defer_base;
     void* p_keep;
+    // Until the first block sweep every shifted system still has p_i = b, x_i = 0: cg_init does not write those 2 x
+    // nshift vectors; the first sweep reads P from the source b_src (one vector, shared) and X as zero, and writes them.
+    int first_block;
+    const void* b_src;
 };
 
 #endif

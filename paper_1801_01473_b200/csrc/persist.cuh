@@ -111,7 +111,10 @@ __global__ void __launch_bounds__(PS_BLOCK, 1) cg_persistent_kernel(const Persis
         grid.sync();
         const double pAp = persist_sum(part1, nsb, red);
         if (scalar_block) {
-            if (close_block && threadIdx.x == 0) st->blk_j = 0;     // every block is past the sweep by now
+            if (close_block && threadIdx.x == 0) {                  // every block is past the sweep by now
+                st->blk_j = 0;
+                st->first_block = 0;
+            }
             __syncthreads();
             cg_scalars_after_pAp(st, pAp);
         }
@@ -164,7 +167,10 @@ __global__ void __launch_bounds__(PS_BLOCK, 1) cg_persistent_kernel(const Persis
     }
     if (close_block) {
         grid.sync();                                         // every block has read the coefficients
-        if (scalar_block && threadIdx.x == 0) st->blk_j = 0;
+        if (scalar_block && threadIdx.x == 0) {
+            st->blk_j = 0;
+            st->first_block = 0;
+        }
     }
 }
 

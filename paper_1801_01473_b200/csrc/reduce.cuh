@@ -96,6 +96,7 @@ __device__ inline void cg_scalars_init(CgState* st, double bb, double tol) {
     st->iter = 0;
     st->status = 0;
     st->blk_j = 0;
+    st->first_block = 1;
     const int stop = (bb == 0.0) ? 1 : 0;       // zero source: x_i = 0 is the answer
     st->stop = stop;
     st->stop4 = stop;
