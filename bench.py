@@ -85,7 +85,10 @@ def cg_dram_bytes(freeze_iter, iters: int, m: int, recon: int) -> int:
     for n0 in range(0, iters, m):
         nres = min(m, iters - n0)
         n_in = sum(1 for i, fz in enumerate(freeze_iter) if i != base and fz > n0)
-        if m >= 2:
+        if m >= 2 and n0 == 0:
+            # first sweep of a solve: P = b read once for all shifted systems, X = 0 not read (cg.cuh, first_block)
+            total += 48 + 48 * nres + 48 + 96 * n_in + 96
+        elif m >= 2:
             total += 48 + 48 * nres + 192 * n_in + 144
         else:
             total += 96 + (48 + 192 * n_in if n_in else 0)

@@ -1301,12 +1301,17 @@ int solve(lqcd_ctx* c, const T* b_even, const double* shifts, int nshift, double
     // kernels of a launch whose solve is over return at once, but 2 x 20,000 empty blocks per iteration are not free)
     const long max_batches = ((long)c->max_iter + ce - 1) / ce;
     for (long batch = 0; batch < max_batches && !done; ++batch) {
-        if (use_graph) {
+        // the batch in which MAX_ITER falls is launched plainly, only as far as the cap: the iterations of a graph
+        // replay beyond it would all return at once, at 27 us each (48^4)
+        const long left = (long)c->max_iter - batch * ce;
+        const int nit = (left < ce && !c->slab) ? (int)left : ce;
+        if (use_graph && nit == ce) {
             CU(cudaGraphLaunch(B.graph_exec, c->stream));
             c->launches += B.graph_launches;
         } else {
-            for (int i = 0; i < ce; ++i)
+            for (int i = 0; i < nit; ++i)
                 if ((rc = launch_cg_iteration<T>(c, i % m))) return rc;
+            if (nit % m != 0) launch_flush<T>(c);            // the stop falls inside a block: close it
             CU(cudaGetLastError());
         }
         const int slot = (int)(batch & 1);
