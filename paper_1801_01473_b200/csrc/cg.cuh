@@ -1,16 +1,15 @@
 // cg.cuh -- the vector sweeps of the multi-shift CG (steps A7, A8 of DESIGN.md) and layout kernels.
 //
-// One CG iteration is four launches ("scalar products and sums" + the two operators), plus one
-// sweep over the shifted systems every m iterations:
-//   K1  t  = D_oe p                                         dslash_kernel<.,0>
-//   K2  s  = (m^2+sigma0) p - D_eo t ;  Re<p,s>  -> a, zeta_new_i, block coefficients   dslash_kernel<.,1>
-//   K3  r_new = r - a s ;  |r_new|^2  -> beta, b_i, block coefficients, freeze flags, stop flag
-//                                                                           cg_update_r_kernel
-//   K4  base system only:  x_0 += a p ;  p = r_new + beta p                 cg_update_base_kernel
-//   K5  every m-th iteration (and once after the stop), for every shifted system of the block:
-//         x_i += CP_i p_i + sum_l D_il r_l ;  p_i = B_i p_i + sum_l E_il r_l      cg_flush_kernel
-// K3 writes r_new into a ring of m residual vectors instead of over r, so that the m residuals of a block
-// are still there when K5 runs: the 192 B per site and active shift of the x_i/p_i update are paid once per
+// One CG iteration is the two operator launches of dslash.cuh ("scalar products and sums" + the two
+// operators, every sum and scalar product of the base system folded into the operators' own sweeps), plus one sweep
+// over all systems every m iterations:
+//   K1  t = D_oe p with p = r + beta p_old formed at the neighbours;  <p,Ap>  -> a, zeta_new_i   dslash_kernel<.,4>
+//   K2  p, s = (m^2+sigma0) p - D_eo t, r_new = r - a s at the own site;  |r_new|^2
+//       -> beta, b_i, block coefficients, freeze flags, stop flag                                 dslash_kernel<.,5>
+//   every m-th iteration (and once after the stop), for every system of the block:
+//         x_i += CP_i p_i + sum_l D_il r_l ;  p_i = B_i p_i + sum_l E_il r_l                      cg_flush_kernel
+// K2 writes r_new into a ring of m residual vectors instead of over r, so that the m residuals of a block
+// are still there when the sweep runs: the 192 B per site and active shift of the x_i/p_i update are paid once per
 // block instead of once per iteration (CgState in lqcd_internal.cuh has the algebra).
 // All scalars stay on the device.
 #ifndef LQCD_CG_CUH
@@ -64,55 +63,6 @@ __global__ void __launch_bounds__(CG_BLOCK) cg_init_kernel(const V2<T>* __restri
     }
 }
 
-// K3: r_out = r_in - a s, |r_out|^2, then the scalar step that needs it
-template <typename T, bool FUSED = true>
-__global__ void __launch_bounds__(CG_BLOCK) cg_update_r_kernel(const V2<T>* r_in, V2<T>* r_out,
-                                                               const V2<T>* __restrict__ s, CgState* st,
-                                                               double* partials, size_t n) {
-    if (st->stop) return;
-    __shared__ double red[32];
-    __shared__ int last_flag;
-    const T a = (T)st->a;
-    double acc = 0.0;
-    const size_t stride = (size_t)gridDim.x * CG_BLOCK;
-    size_t j = (size_t)blockIdx.x * CG_BLOCK + threadIdx.x;
-    for (; j + 3 * stride < n; j += 4 * stride) {
-        V2<T> rv[4], sv[4];
-#pragma unroll
-        for (int u = 0; u < 4; ++u) {
-            rv[u] = r_in[j + u * stride];
-            sv[u] = s[j + u * stride];
-        }
-#pragma unroll
-        for (int u = 0; u < 4; ++u) {
-            rv[u].x = fma(-a, sv[u].x, rv[u].x);
-            rv[u].y = fma(-a, sv[u].y, rv[u].y);
-            r_out[j + u * stride] = rv[u];
-            acc = fma((double)rv[u].x, (double)rv[u].x, acc);
-            acc = fma((double)rv[u].y, (double)rv[u].y, acc);
-        }
-    }
-    for (; j < n; j += stride) {
-        V2<T> rv = r_in[j];
-        const V2<T> sv = s[j];
-        rv.x = fma(-a, sv.x, rv.x);
-        rv.y = fma(-a, sv.y, rv.y);
-        r_out[j] = rv;
-        acc = fma((double)rv.x, (double)rv.x, acc);
-        acc = fma((double)rv.y, (double)rv.y, acc);
-    }
-    const double bsum = block_sum<CG_BLOCK>(acc, red);
-    if (!FUSED) {
-        if (threadIdx.x == 0) partials[blockIdx.x] = bsum;
-        return;
-    }
-    if (publish_partial<CG_BLOCK>(bsum, partials, &st->ticket[2], &last_flag)) {
-        const double rr = broadcast0(final_sum<CG_BLOCK>(partials, gridDim.x, red), red);
-        if (threadIdx.x == 0) st->ticket[2] = 0;
-        cg_scalars_after_rr(st, rr);
-    }
-}
-
 // ---- slab mode (1-D decomposition along t): a scalar product is the sum over the blocks of
 // this rank (sum_partials_kernel, fixed order), then over the ranks (all-reduce of one double: "global
 // reductions" of PAPER.md:L112), then the scalar step runs on every rank on bit-identical input
@@ -133,56 +83,12 @@ __global__ void __launch_bounds__(64) cg_scalar_kernel(CgState* st, const double
         if (threadIdx.x == 0) cg_scalars_init(st, v, tol);
         return;
     }
-    if (st->stop) {
-        if (which == 1 && threadIdx.x == 0) st->stop4 = 1;
-        return;
-    }
+    if (st->stop) return;
     if (which == 1) cg_scalars_after_pAp(st, v);
     else cg_scalars_after_rr(st, v);
 }
 
-// K4: the base system (zeta = 1):  x_0 += a p  (rational mode: y += alpha_0 a p) ;  p = r_new + beta p
-template <typename T>
-__global__ void __launch_bounds__(CG_BLOCK) cg_update_base_kernel(const V2<T>* __restrict__ r, V2<T>* __restrict__ p,
-                                                                  const CgState* st, size_t n) {
-    if (st->stop4) return;
-    const int i0 = st->i0;
-    const T bt = (T)st->b_prev;
-    const T a = (T)(st->rational ? st->alpha[i0] * st->a : st->a);
-    V2<T>* __restrict__ x = (V2<T>*)(st->rational ? st->y : st->x[i0]);
-    const size_t stride = (size_t)gridDim.x * CG_BLOCK;
-    size_t j = (size_t)blockIdx.x * CG_BLOCK + threadIdx.x;
-    for (; j + stride < n; j += 2 * stride) {
-        V2<T> rv[2], pv[2], xv[2];
-#pragma unroll
-        for (int u = 0; u < 2; ++u) {
-            rv[u] = r[j + u * stride];
-            pv[u] = p[j + u * stride];
-            xv[u] = x[j + u * stride];
-        }
-#pragma unroll
-        for (int u = 0; u < 2; ++u) {
-            xv[u].x = fma(a, pv[u].x, xv[u].x);
-            xv[u].y = fma(a, pv[u].y, xv[u].y);
-            pv[u].x = fma(bt, pv[u].x, rv[u].x);
-            pv[u].y = fma(bt, pv[u].y, rv[u].y);
-            x[j + u * stride] = xv[u];
-            p[j + u * stride] = pv[u];
-        }
-    }
-    for (; j < n; j += stride) {
-        const V2<T> rv = r[j];
-        V2<T> pv = p[j], xv = x[j];
-        xv.x = fma(a, pv.x, xv.x);
-        xv.y = fma(a, pv.y, xv.y);
-        pv.x = fma(bt, pv.x, rv.x);
-        pv.y = fma(bt, pv.y, rv.y);
-        x[j] = xv;
-        p[j] = pv;
-    }
-}
-
-// K5: the deferred updates of one block, for every shifted system that was active when the block began.
+// The block sweep: the deferred updates of one block, for every shifted system that was active when the block began.
 // nres = st->blk_j residuals r_l = hist[l] are used (nres = m for a full block, less after the stop).
 //   x_i += CP_i p_i + sum_l D_il r_l   (rational mode: y += sum_i of that; alpha_i is inside CP, D)
 //   p_i  = B_i p_i + sum_l E_il r_l
@@ -397,7 +303,6 @@ __global__ void __launch_bounds__(CG_BLOCK) mixed_residual_kernel(const double2*
             if (replace) st->rr = rr;
             if (resume) {
                 st->stop = 0;
-                st->stop4 = 0;
                 st->active[st->i0] = 1;
             }
         }

@@ -26,11 +26,7 @@
 //          are in flight and the two border slices afterwards (Alg. 1).
 //
 // EPI = 0 : out = D in
-// EPI = 1 : out = coef*pv - D in, plus the block partial of Re<pv, out> and the CG scalar step
-//           (this is the paper's separate zaxpy kernel, fused into the D_eo epilogue)
-// EPI = 2 : out = coef*pv - D in only
-// EPI = 3 : as 1, but only the block partial is written (at partials[part_off + blockIdx.x]); the sum over
-//           blocks, launches and ranks and the scalar step follow in their own small kernels (slab mode)
+// EPI = 2 : out = coef*pv - D in  (the paper's separate zaxpy kernel, fused into the D_eo epilogue)
 //
 // The two launches of one fused CG iteration (cg.cuh has the whole picture; "scalar products and sums"
 // + the two operators, with every sum and scalar product folded into the operators' own sweeps):
@@ -43,6 +39,9 @@
 //           it (p_out), s = c0 p - D_eo t (never stored), r_new = r - a s (r_out, the next ring slot),
 //           x_0 += a p (unless the base system is block-deferred like the shifted ones), and the block partial of
 //           |r_new|^2.  The last block sums and runs the scalar step (beta, b_i, freeze and stop flags).
+// With SLAB = 1 the launches of EPI 4, 5 only write their block partials (at partials[part_off + blockIdx.x]); the
+// sum over blocks, launches and ranks and the scalar step follow in their own small kernels, and across the slab
+// faces K1 finds p itself in the halo (formed by its owner, slab_pack_p_kernel).
 #ifndef LQCD_DSLASH_CUH
 #define LQCD_DSLASH_CUH
 
@@ -210,19 +209,27 @@ __device__ __forceinline__ void load_link(const V2<T>* __restrict__ w, const siz
     }
 }
 
-// the vector operand of a hop: a stored vector, or (FLY) p = r + beta p_old formed in registers from the residual v
-// and the previous search direction v2 (same index); pp accumulates |p|^2 for the <p,Ap> identity of EPI = 4
-template <typename T, bool FLY, bool COH>
+// the vector operand of a hop.  MODE 0: a stored vector.  MODE 1: p = r + beta p_old formed in registers from the
+// residual v and the previous search direction v2 (same index); pp accumulates |p|^2 for the <p,Ap> identity of
+// EPI = 4.  MODE 2: p was formed by the rank that owns the site and arrived in a halo buffer (slab faces of
+// EPI = 4): a stored vector whose |p|^2 is accumulated all the same.
+template <typename T, int MODE, bool COH>
 __device__ __forceinline__ void load_vec(const V2<T>* __restrict__ v, const V2<T>* __restrict__ v2, const size_t vs,
                                          uint64_t pol, unsigned int mask, const T beta, T (&vr)[3], T (&vi)[3],
                                          double& pp) {
-    if (!FLY) {
+    if (MODE != 1) {
+        T n2 = (T)0;
 #pragma unroll
         for (int c = 0; c < 3; ++c) {
             const V2<T> t = ld_vec<COH>(v + c * vs, pol);
+            if (MODE == 2) {
+                n2 = fma(t.x, t.x, n2);
+                n2 = fma(t.y, t.y, n2);
+            }
             vr[c] = flip(t.x, mask);
             vi[c] = flip(t.y, mask);
         }
+        if (MODE == 2) pp += (double)n2;
     } else {
         V2<T> r[3], q[3];
 #pragma unroll
@@ -246,7 +253,7 @@ __device__ __forceinline__ void load_vec(const V2<T>* __restrict__ v, const V2<T
 // One hop.  FWD: acc += sign * U v (the sign is already folded into v);  !FWD: acc += sign * U^dagger v (the caller
 // passes the mask of -s).  ws, vs: element strides of the link and of the vector (they differ from Vh only for the
 // halo buffers of a slab face).
-template <typename T, int RECON, int U1, bool FWD, bool FLY, bool COH = false>
+template <typename T, int RECON, int U1, bool FWD, int MODE, bool COH = false>
 __device__ __forceinline__ void hop(T (&ar)[3], T (&ai)[3], const V2<T>* __restrict__ w, const size_t ws,
                                     const V2<T>* __restrict__ v, const V2<T>* __restrict__ v2, const size_t vs,
                                     unsigned int mask, uint64_t pol_s, uint64_t pol_r, const T* __restrict__ th,
@@ -254,7 +261,7 @@ __device__ __forceinline__ void hop(T (&ar)[3], T (&ai)[3], const V2<T>* __restr
     V2<T> u[9];
     T vr[3], vi[3];
     load_link<T, RECON>(w, ws, pol_s, u);
-    load_vec<T, FLY, COH>(v, v2, vs, pol_r, mask, beta, vr, vi, pp);
+    load_vec<T, MODE, COH>(v, v2, vs, pol_r, mask, beta, vr, vi, pp);
     if (U1) u1_rotate<T, FWD ? +1 : -1>(th, pol_s, vr, vi);
 #pragma unroll
     for (int a = 0; a < 3; ++a)
@@ -274,10 +281,10 @@ struct DslashArgs {
     const V2<T>* in2;        // EPI == 4: the previous search direction p_old, parity 1-par
     V2<T>* out;              // parity par (not written by EPI == 5)
     int par;                 // parity of the output sites
-    const V2<T>* pv;         // EPI 1,2,3: vector of parity par;  EPI == 5: p_old
+    const V2<T>* pv;         // EPI == 2: vector of parity par;  EPI == 5: p_old
     double coef;             // EPI == 2: m^2 + sigma
-    double* partials;        // EPI 1,3,4,5
-    CgState* st;             // EPI 1,3,4,5, or any EPI with check_stop
+    double* partials;        // EPI 4,5
+    CgState* st;             // EPI 4,5, or any EPI with check_stop
     int check_stop;          // 1: return at once if st->stop (CG already converged)
     int pol_links, pol_vecs; // L2 eviction priority of the link / neighbour-vector loads (l2_policy codes)
     // EPI == 5 only (all of parity par)
@@ -292,7 +299,7 @@ struct DslashArgs {
     const V2<T>* Wt_lo;      // halo: t-links leaving slice t_off-1, [parity of origin][e][face]
     const T* Th_lo;          // halo (U1): their U(1) angles, [parity of origin][face]
     int k0a, na, k0b, nsites;    // thread idx < na: site k0a+idx; else site k0b+(idx-na); nsites in all
-    int part_off;            // EPI == 3: first slot of this launch in `partials`
+    int part_off;            // EPI 4,5: first slot of this launch in `partials`
 };
 
 // registers: double needs ~126 (4 blocks of 128 threads per SM); single fits 6 blocks
@@ -357,10 +364,10 @@ __device__ __forceinline__ void dslash_hops(const DslashArgs<T>& A, const int pa
     const T* __restrict__ Tb = U1 ? A.Th + (size_t)(1 - par) * vh : nullptr;     // angles of the backward links
     const size_t th_stride = 2 * vh;
 #define HOP_F(mu, kn, mask) \
-    hop<T, RECON, U1, true, FLY, COH>(ar, ai, Wf + (mu) * mu_stride, vh, in + (kn), in2 + (kn), vh, mask, pol_s, pol_r, \
+    hop<T, RECON, U1, true, FLY ? 1 : 0, COH>(ar, ai, Wf + (mu) * mu_stride, vh, in + (kn), in2 + (kn), vh, mask, pol_s, pol_r, \
                                  Tf + (mu) * th_stride, beta, pp)
 #define HOP_B(mu, kn, mask) \
-    hop<T, RECON, U1, false, FLY, COH>(ar, ai, Wb + (mu) * mu_stride + (kn), vh, in + (kn), in2 + (kn), vh, (mask) ^ SB, pol_s, \
+    hop<T, RECON, U1, false, FLY ? 1 : 0, COH>(ar, ai, Wb + (mu) * mu_stride + (kn), vh, in + (kn), in2 + (kn), vh, (mask) ^ SB, pol_s, \
                                   pol_r, Tb + (mu) * th_stride + (kn), beta, pp)
     HOP_F(0, kxf, 0u);
     HOP_B(0, kxb, 0u);
@@ -372,18 +379,27 @@ __device__ __forceinline__ void dslash_hops(const DslashArgs<T>& A, const int pa
         HOP_F(3, ktf, mtf);
         HOP_B(3, ktb, mtb);
     } else {
-        // across the slab faces the neighbour vector (and, downwards, the link) comes from the halo buffers
+        // across the slab faces the neighbour vector (and, downwards, the link) comes from the halo buffers; with
+        // FLY the halo holds p itself, formed by the rank that owns those sites (slab_pack_p_kernel)
         const size_t face = (size_t)g.st;
         const int kf = k - t * g.st;                                  // index inside a time slice
         const bool top = (t == g.Lt - 1), bot = (t == 0);
-        const V2<T>* vf = top ? A.in_hi + kf : in + k + g.st;
-        hop<T, RECON, U1, true, false>(ar, ai, Wf + 3 * mu_stride, vh, vf, vf, top ? face : vh, mtf, pol_s, pol_r,
-                                       Tf + 3 * th_stride, beta, pp);
-        const V2<T>* vb = bot ? A.in_lo + kf : in + k - g.st;
+        const V2<T>* wf = Wf + 3 * mu_stride;
+        const T* tf = Tf + 3 * th_stride;
         const V2<T>* wb = bot ? A.Wt_lo + (size_t)(1 - par) * NE * face + kf : Wb + 3 * mu_stride + k - g.st;
         const T* tb = U1 ? (bot ? A.Th_lo + (size_t)(1 - par) * face + kf : Tb + 3 * th_stride + k - g.st) : nullptr;
-        hop<T, RECON, U1, false, false>(ar, ai, wb, bot ? face : vh, vb, vb, bot ? face : vh, mtb ^ SB, pol_s, pol_r, tb,
-                                        beta, pp);
+        const size_t wbs = bot ? face : vh;
+        if (!FLY) {
+            const V2<T>* vf = top ? A.in_hi + kf : in + k + g.st;
+            hop<T, RECON, U1, true, 0>(ar, ai, wf, vh, vf, vf, top ? face : vh, mtf, pol_s, pol_r, tf, beta, pp);
+            const V2<T>* vb = bot ? A.in_lo + kf : in + k - g.st;
+            hop<T, RECON, U1, false, 0>(ar, ai, wb, wbs, vb, vb, bot ? face : vh, mtb ^ SB, pol_s, pol_r, tb, beta, pp);
+        } else {
+            if (top) hop<T, RECON, U1, true, 2>(ar, ai, wf, vh, A.in_hi + kf, A.in_hi + kf, face, mtf, pol_s, pol_r, tf, beta, pp);
+            else hop<T, RECON, U1, true, 1>(ar, ai, wf, vh, in + k + g.st, in2 + k + g.st, vh, mtf, pol_s, pol_r, tf, beta, pp);
+            if (bot) hop<T, RECON, U1, false, 2>(ar, ai, wb, wbs, A.in_lo + kf, A.in_lo + kf, face, mtb ^ SB, pol_s, pol_r, tb, beta, pp);
+            else hop<T, RECON, U1, false, 1>(ar, ai, wb, wbs, in + k - g.st, in2 + k - g.st, vh, mtb ^ SB, pol_s, pol_r, tb, beta, pp);
+        }
     }
 #undef HOP_F
 #undef HOP_B
@@ -469,14 +485,8 @@ __device__ __forceinline__ K2Coef<T> k2_coef_from_state(const CgState* st, V2<T>
 template <typename T, int RECON, int EPI, int U1, int SLAB = 0>
 __global__ void __launch_bounds__(DS_BLOCK, (DsOcc<T, EPI>::minb)) dslash_kernel(const DslashArgs<T> A) {
     constexpr bool FLY = (EPI == 4);
-    static_assert(!(SLAB && EPI >= 4), "the fused CG launches exist for the whole-lattice path only");
-    if (A.check_stop) {
-        if (A.st->stop) {
-            // tell the x/p update kernel of the *following* iterations to do nothing (see cg.cuh)
-            if (EPI == 0 && blockIdx.x == 0 && threadIdx.x == 0) A.st->stop4 = 1;
-            return;
-        }
-    }
+    static_assert(EPI == 0 || EPI == 2 || EPI == 4 || EPI == 5, "EPI");
+    if (A.check_stop && A.st->stop) return;      // iterations launched beyond the one that converged
     const Geom& g = A.g;
     const int kraw = blockIdx.x * DS_BLOCK + threadIdx.x;
     bool valid;
@@ -527,43 +537,48 @@ __global__ void __launch_bounds__(DS_BLOCK, (DsOcc<T, EPI>::minb)) dslash_kernel
         const K2Coef<T> C = k2_coef_from_state<T>(A.st, A.p_out, A.r_out, A.p_keep, A.defer_base);
         dot = k2_finish<T>(C, vh, k, valid, pv, rv, ar, ai);
     } else {
-        // out = coef*pv - D in;  Re<pv, out>
+        // out = coef*pv - D in
+        if (valid) {
 #pragma unroll
-        for (int c = 0; c < 3; ++c) {
-            const V2<T> p = pv[c];
-            const V2<T> o = make_v2(fma((T)-0.5, ar[c], coef * p.x), fma((T)-0.5, ai[c], coef * p.y));
-            if (valid) {
-                A.out[c * vh + k] = o;
-                dot = fma((double)p.x, (double)o.x, dot);
-                dot = fma((double)p.y, (double)o.y, dot);
+            for (int c = 0; c < 3; ++c) {
+                const V2<T> p = pv[c];
+                A.out[c * vh + k] = make_v2(fma((T)-0.5, ar[c], coef * p.x), fma((T)-0.5, ai[c], coef * p.y));
             }
         }
+        return;
     }
-    if (EPI == 3) {
-        __shared__ double red3[32];
-        const double bsum = block_sum<DS_BLOCK>(dot, red3);
+    __shared__ double red[32];
+    __shared__ int last_flag;
+    const double bsum = block_sum<DS_BLOCK>(dot, red);
+    if (SLAB) {
+        // a slab's launches (interior, borders) each write their block partials; the sum over blocks, launches and
+        // ranks and the scalar step follow in their own small kernels (sum_partials_kernel, cg_scalar_kernel)
         if (threadIdx.x == 0) A.partials[A.part_off + blockIdx.x] = bsum;
+        return;
     }
-    if (EPI == 1 || EPI == 4) {
-        __shared__ double red[32];
-        __shared__ int last_flag;
-        const double bsum = block_sum<DS_BLOCK>(dot, red);
-        if (publish_partial<DS_BLOCK>(bsum, A.partials, &A.st->ticket[1], &last_flag)) {
-            const double pAp = broadcast0(final_sum<DS_BLOCK>(A.partials, gridDim.x, red), red);
-            if (threadIdx.x == 0) A.st->ticket[1] = 0;
-            cg_scalars_after_pAp(A.st, pAp);
-        }
+    if (publish_partial<DS_BLOCK>(bsum, A.partials, &A.st->ticket[EPI == 4 ? 1 : 2], &last_flag)) {
+        const double sum = broadcast0(final_sum<DS_BLOCK>(A.partials, gridDim.x, red), red);
+        if (threadIdx.x == 0) A.st->ticket[EPI == 4 ? 1 : 2] = 0;
+        if (EPI == 4) cg_scalars_after_pAp(A.st, sum);
+        else cg_scalars_after_rr(A.st, sum);
     }
-    if (EPI == 5) {
-        __shared__ double red5[32];
-        __shared__ int last_flag5;
-        const double bsum = block_sum<DS_BLOCK>(dot, red5);
-        if (publish_partial<DS_BLOCK>(bsum, A.partials, &A.st->ticket[2], &last_flag5)) {
-            const double rr = broadcast0(final_sum<DS_BLOCK>(A.partials, gridDim.x, red5), red5);
-            if (threadIdx.x == 0) A.st->ticket[2] = 0;
-            cg_scalars_after_rr(A.st, rr);
-        }
-    }
+}
+
+// Slab mode, before K1: the two faces (time slices 0 and Lt-1) of p = r + beta p_old, formed by the rank that owns the
+// sites with the formula K1 uses at the neighbours (load_vec, MODE 1: same operands, same bits), packed for the ring
+// exchange as [lo|hi][c][face].  One thread per complex number.
+template <typename T>
+__global__ void __launch_bounds__(256) slab_pack_p_kernel(const V2<T>* __restrict__ r, const V2<T>* __restrict__ p_old,
+                                                          V2<T>* __restrict__ send, const CgState* st, size_t vh, size_t face) {
+    if (st->stop) return;
+    const size_t i = (size_t)blockIdx.x * 256 + threadIdx.x;
+    if (i >= 6 * face) return;
+    const T beta = (T)st->b_prev;
+    const size_t hi = i / (3 * face), rem = i - hi * 3 * face;
+    const size_t c = rem / face, kf = rem - c * face;
+    const size_t src = c * vh + (hi ? vh - face : 0) + kf;
+    const V2<T> rv = r[src], q = p_old[src];
+    send[i] = make_v2(fma(beta, q.x, rv.x), fma(beta, q.y, rv.y));
 }
 
 #endif

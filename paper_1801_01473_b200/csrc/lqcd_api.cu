@@ -41,7 +41,7 @@ struct PrecBufs {
     int recon_stored = 0;    // 0 = no gauge in this precision, else 18 or 12
     T* Th = nullptr;         // stored U(1) angles theta_mu(x) (lqcd_set_u1_phases), [(mu*2+par)*Vh + k]
     int u1_stored = 0;
-    V2<T> *p = nullptr, *s = nullptr, *t = nullptr;
+    V2<T> *p = nullptr, *t = nullptr;
     V2<T>* p_keep = nullptr;                 // p of the first iteration of the current block (CgState::p_keep)
     V2<T>* hist[LQCD_MAX_BLOCK] = {};        // ring of residual vectors (cg.cuh)
     int n_hist = 0;
@@ -302,8 +302,7 @@ int ensure_solver(lqcd_ctx* c, int nshift) {
         ++B.n_hist;
     }
     if (!B.p && (rc = dev_alloc(c, (void**)&B.p, vec_bytes<T>(c)))) return rc;
-    if (c->slab && !B.s && (rc = dev_alloc(c, (void**)&B.s, vec_bytes<T>(c)))) return rc;    // s is stored on slabs only
-    if (!c->slab && !B.p_keep && (rc = dev_alloc(c, (void**)&B.p_keep, vec_bytes<T>(c)))) return rc;
+    if (!B.p_keep && (rc = dev_alloc(c, (void**)&B.p_keep, vec_bytes<T>(c)))) return rc;
     while (B.n_pextra < nshift - 1) {
         if ((rc = dev_alloc(c, (void**)&B.pextra[B.n_pextra], vec_bytes<T>(c)))) return rc;
         ++B.n_pextra;
@@ -400,12 +399,14 @@ void launch_dslash_slab_k(lqcd_ctx* c, const DslashArgs<T>& a, int grid, cudaStr
     else launch_dslash_slab_u<T, EPI, 0>(c, a, grid, stream);
 }
 
-// One operator application on a slab (Alg. 1 of the paper): the two faces of `in` are packed
-// and sent, the interior time slices are computed meanwhile, the two border slices once the halos have arrived.
-// EPI == 1 becomes EPI == 3: block partials in c->partials[0 .. *n_part), summed by the caller.
+// One operator sweep on a slab (Alg. 1 of the paper): the two faces of the input are packed and
+// sent, the interior time slices are computed meanwhile, the two border slices once the halos have arrived.
+// `a` carries everything but the slab fields; kepi is the kernel's EPI (0, 2: operators; 4, 5: the two launches of the
+// fused CG iteration, which write block partials to c->partials[0 .. *n_part), summed by the caller).
+// The faces that travel are those of `face_v`, or, with face_v2, of face_v + beta face_v2 (K1: p = r + beta p_old,
+// formed by the owner of the sites).
 template <typename T>
-int slab_dslash(lqcd_ctx* c, int epi, V2<T>* out, const V2<T>* in, int par, const V2<T>* pv, double coef, int check_stop,
-                int* n_part) {
+int slab_apply(lqcd_ctx* c, DslashArgs<T>& a, int kepi, const V2<T>* face_v, const V2<T>* face_v2, int* n_part) {
     int rc;
     if (!c->has_comm) return fail(c, LQCD_ECOMM, "slab context without a transport (lqcd_comm_init_nccl / lqcd_set_comm)");
     if ((rc = ensure_halo<T>(c))) return rc;
@@ -416,38 +417,36 @@ int slab_dslash(lqcd_ctx* c, int epi, V2<T>* out, const V2<T>* in, int par, cons
     V2<T>* send_hi = B.halo_send + 3 * face;
     V2<T>* recv_lo = B.halo_recv;
     V2<T>* recv_hi = B.halo_recv + 3 * face;
-    // `in` is complete at this point of the compute stream; everything about the faces happens on the
+    // the input is complete at this point of the compute stream; everything about the faces happens on the
     // communication stream from here on, beside the interior launch
     CU(cudaEventRecord(c->ev_pack, c->stream));
     CU(cudaStreamWaitEvent(c->comm_stream, c->ev_pack, 0));
-    // a face is three contiguous runs (one per colour) of the vector: strided copies, no kernel
-    CU(cudaMemcpy2DAsync(send_lo, row, in, pitch, row, 3, cudaMemcpyDeviceToDevice, c->comm_stream));
-    CU(cudaMemcpy2DAsync(send_hi, row, in + (vh - face), pitch, row, 3, cudaMemcpyDeviceToDevice, c->comm_stream));
+    if (face_v2) {
+        slab_pack_p_kernel<T><<<(int)((6 * face + 255) / 256), 256, 0, c->comm_stream>>>(face_v, face_v2, B.halo_send, c->st_dev, vh, face);
+        ++c->launches;
+    } else {
+        // a face is three contiguous runs (one per colour) of the vector: strided copies, no kernel
+        CU(cudaMemcpy2DAsync(send_lo, row, face_v, pitch, row, 3, cudaMemcpyDeviceToDevice, c->comm_stream));
+        CU(cudaMemcpy2DAsync(send_hi, row, face_v + (vh - face), pitch, row, 3, cudaMemcpyDeviceToDevice, c->comm_stream));
+    }
 
-    DslashArgs<T> a{};
     a.g = c->g;
     a.W = B.W;
     set_policies<T>(c, a);
     a.Th = B.Th;
     a.Th_lo = B.Th_lo;
-    a.in = in;
-    a.out = out;
-    a.par = par;
-    a.pv = pv;
-    a.coef = coef;
     a.partials = c->partials;
     a.st = c->st_dev;
-    a.check_stop = check_stop;
     a.in_lo = recv_lo;
     a.in_hi = recv_hi;
     a.Wt_lo = B.Wt_lo;
-    const int kepi = (epi == 1) ? 3 : epi;
     int part = 0;
     auto launch = [&](int grid, cudaStream_t stream) {
         a.part_off = part;
         if (kepi == 0) launch_dslash_slab_k<T, 0>(c, a, grid, stream);
         else if (kepi == 2) launch_dslash_slab_k<T, 2>(c, a, grid, stream);
-        else launch_dslash_slab_k<T, 3>(c, a, grid, stream);
+        else if (kepi == 4) launch_dslash_slab_k<T, 4>(c, a, grid, stream);
+        else launch_dslash_slab_k<T, 5>(c, a, grid, stream);
         part += grid;
     };
     // interior: t = 1 .. Lt-2
@@ -472,6 +471,18 @@ int slab_dslash(lqcd_ctx* c, int epi, V2<T>* out, const V2<T>* in, int par, cons
     CU(cudaGetLastError());
     if (n_part) *n_part = part;
     return LQCD_OK;
+}
+
+// out(par) = D in on a slab, optionally with the epilogue out = coef pv - D in (epi == 2)
+template <typename T>
+int slab_dslash(lqcd_ctx* c, int epi, V2<T>* out, const V2<T>* in, int par, const V2<T>* pv, double coef) {
+    DslashArgs<T> a{};
+    a.in = in;
+    a.out = out;
+    a.par = par;
+    a.pv = pv;
+    a.coef = coef;
+    return slab_apply<T>(c, a, epi, in, nullptr, nullptr);
 }
 
 // sum of c->partials[0..n) over this rank's blocks, then over the ranks, then the scalar step `which`
@@ -503,7 +514,6 @@ void launch_dslash(lqcd_ctx* c, int epi, V2<T>* out, const V2<T>* in, int par, c
     a.st = c->st_dev;
     a.check_stop = check_stop;
     if (epi == 0) launch_dslash_t<T, 0>(c, a);
-    else if (epi == 1) launch_dslash_t<T, 1>(c, a);
     else launch_dslash_t<T, 2>(c, a);
 }
 
@@ -539,8 +549,8 @@ void launch_cg_fused(lqcd_ctx* c, const V2<T>* r_in, V2<T>* r_out, V2<T>* p_keep
     launch_dslash_t<T, 5>(c, a);
 }
 
-// whole lattice, m >= 2: x_0 of the base system is updated by the block sweep too (CgState::defer_base)
-int defer_base(const lqcd_ctx* c) { return (!c->slab && block_len(c) >= 2) ? 1 : 0; }
+// m >= 2: x_0 of the base system is updated by the block sweep too (CgState::defer_base)
+int defer_base(const lqcd_ctx* c) { return block_len(c) >= 2 ? 1 : 0; }
 
 // the sweep over the shifted systems that closes a block of iterations (K5 of cg.cuh)
 template <typename T>
@@ -554,30 +564,44 @@ void launch_flush(lqcd_ctx* c) {
     ++c->launches;
 }
 
-// one CG iteration = K1..K4 (cg.cuh), plus K5 when it is the last of a block; pos = iteration index mod m
+// one CG iteration = K1, K2 (dslash.cuh), plus the block sweep when it is the last of a block; pos = iteration index mod m
 template <typename T>
 int launch_cg_iteration(lqcd_ctx* c, int pos) {
-    const size_t n = c->Vh * 3;
     const int m = block_len(c);
     PrecBufs<T>& B = bufs<T>(c);
+    const int defer = defer_base(c);
+    const V2<T>* r_in = B.hist[(pos + m - 1) % m];
+    V2<T>* r_out = B.hist[pos];
+    V2<T>* p_keep = (defer && pos == 0) ? B.p_keep : nullptr;
     if (c->slab) {
-        // the same iteration with the two exchange steps of the slab decomposition: faces before each operator,
-        // one all-reduced double after each scalar product
+        // the same two launches with the two exchange steps of the slab decomposition: faces before each operator
+        // sweep (of p, formed by its owner, before K1; of t before K2), one all-reduced double after each scalar
+        // product, then the scalar step on every rank
         int rc, np = 0;
-        if ((rc = slab_dslash<T>(c, 0, B.t, B.p, 1, nullptr, 0.0, 1, nullptr))) return rc;
-        if ((rc = slab_dslash<T>(c, 1, B.s, B.t, 0, B.p, 0.0, 1, &np))) return rc;
+        DslashArgs<T> a{};
+        a.check_stop = 1;
+        a.in = r_in;
+        a.in2 = B.p;
+        a.out = B.t;
+        a.par = 1;
+        if ((rc = slab_apply<T>(c, a, 4, r_in, B.p, &np))) return rc;
         if ((rc = slab_reduce_step(c, np, 1, 0.0, 1))) return rc;
-        cg_update_r_kernel<T, false><<<cg_grid(c), CG_BLOCK, 0, c->stream>>>(B.hist[(pos + m - 1) % m], B.hist[pos], B.s,
-                                                                             c->st_dev, c->partials, n);
-        ++c->launches;
-        if ((rc = slab_reduce_step(c, cg_grid(c), 2, 0.0, 1))) return rc;
-        cg_update_base_kernel<T><<<cg_grid(c), CG_BLOCK, 0, c->stream>>>(B.hist[pos], B.p, c->st_dev, n);
-        ++c->launches;
+        a.in = B.t;
+        a.in2 = nullptr;
+        a.out = nullptr;
+        a.par = 0;
+        a.pv = B.p;
+        a.r_in = r_in;
+        a.r_out = r_out;
+        a.p_out = B.p;
+        a.p_keep = p_keep;
+        a.defer_base = defer;
+        if ((rc = slab_apply<T>(c, a, 5, B.t, nullptr, &np))) return rc;
+        if ((rc = slab_reduce_step(c, np, 2, 0.0, 1))) return rc;
         if (pos == m - 1) launch_flush<T>(c);
         return LQCD_OK;
     }
-    const int defer = defer_base(c);
-    launch_cg_fused<T>(c, B.hist[(pos + m - 1) % m], B.hist[pos], (defer && pos == 0) ? B.p_keep : nullptr, defer);
+    launch_cg_fused<T>(c, r_in, r_out, p_keep, defer);
     if (pos == m - 1) launch_flush<T>(c);
     return LQCD_OK;
 }
@@ -1172,7 +1196,7 @@ int apply_d(lqcd_ctx* c, T* out, const T* in, int par) {
     if ((rc = check_ctx_gauge<T>(c))) return rc;
     if (c->slab) {
         if ((rc = ensure_basics(c))) return rc;
-        return slab_dslash<T>(c, 0, (V2<T>*)out, (const V2<T>*)in, par, nullptr, 0.0, 0, nullptr);
+        return slab_dslash<T>(c, 0, (V2<T>*)out, (const V2<T>*)in, par, nullptr, 0.0);
     }
     launch_dslash<T>(c, 0, (V2<T>*)out, (const V2<T>*)in, par, nullptr, 0.0, 0);
     CU(cudaGetLastError());
@@ -1204,8 +1228,8 @@ int apply_mdagm(lqcd_ctx* c, T* out_even, const T* in_even, double sigma) {
     if ((rc = ensure_tmp<T>(c))) return rc;
     PrecBufs<T>& B = bufs<T>(c);
     if (c->slab) {
-        if ((rc = slab_dslash<T>(c, 0, B.t, (const V2<T>*)in_even, 1, nullptr, 0.0, 0, nullptr))) return rc;
-        return slab_dslash<T>(c, 2, (V2<T>*)out_even, B.t, 0, (const V2<T>*)in_even, c->mass * c->mass + sigma, 0, nullptr);
+        if ((rc = slab_dslash<T>(c, 0, B.t, (const V2<T>*)in_even, 1, nullptr, 0.0))) return rc;
+        return slab_dslash<T>(c, 2, (V2<T>*)out_even, B.t, 0, (const V2<T>*)in_even, c->mass * c->mass + sigma);
     }
     launch_dslash<T>(c, 0, B.t, (const V2<T>*)in_even, 1, nullptr, 0.0, 0);
     launch_dslash<T>(c, 2, (V2<T>*)out_even, B.t, 0, (const V2<T>*)in_even, c->mass * c->mass + sigma, 0);

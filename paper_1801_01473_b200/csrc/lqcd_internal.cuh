@@ -46,7 +46,7 @@ struct Geom {
 // The base system's p is needed by the operator every iteration and is updated every iteration.
 struct CgState {
     double rr, bb, pAp, a, a_prev, b_prev, tol2bb, c0;
-    int iter, max_iter, stop, stop4, status, nshift, i0, blk_m;
+    int iter, max_iter, stop, status, nshift, i0, blk_m;
     int blk_j;                      // iterations accumulated in the current block (0..blk_m)
     unsigned int ticket[5];
     double delta[LQCD_MAX_SHIFTS];

@@ -99,7 +99,6 @@ __device__ inline void cg_scalars_init(CgState* st, double bb, double tol) {
     st->first_block = 1;
     const int stop = (bb == 0.0) ? 1 : 0;       // zero source: x_i = 0 is the answer
     st->stop = stop;
-    st->stop4 = stop;
     for (int i = 0; i < st->nshift; ++i) {
         st->zeta[i] = 1.0;
         st->zeta_prev[i] = 1.0;
@@ -121,7 +120,6 @@ __device__ __noinline__ void cg_scalars_after_pAp(CgState* st, double pAp) {
             st->pAp = pAp;
             st->status = -6;                     // LQCD_EBREAKDOWN
             st->stop = 1;
-            st->stop4 = 1;
         }
         return;
     }
