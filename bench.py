@@ -36,6 +36,7 @@ from __future__ import annotations
 import argparse
 import json
 import os
+import signal
 import socket
 import statistics
 import subprocess
@@ -647,7 +648,7 @@ def run_slab_check(args):
         U, f = gen.random_su3_links(Lp), gen.gaussian_field(Lp)
         b_aos = oracle.restrict(Lp, 0, f.numpy())
         b_whole = torch.as_tensor(oracle.aos_to_soa(b_aos)).cuda()
-        lat = lq.Lattice(Lp, mass=mass, slab=(rank, world), comm="nccl")
+        lat = lq.Lattice(Lp, mass=mass, slab=(rank, world), comm=args.slab_comm)
         lat.set_gauge(lq.Lattice.slab_of_links(U, Lp, rank, world).cuda())
         b = lq.Lattice.slab_of_vector(b_whole, Lp, rank, world)
         t = lat.doe(b)
@@ -689,7 +690,7 @@ def run_slab_check(args):
         Lg = tuple(L[:3]) + (L[3] * world,)
         U = gen.random_su3_links_slab(Lg, rank, world, device="cuda")
         f = gen.gaussian_field_slab(Lg, rank, world, device="cuda")
-        lat = lq.Lattice(Lg, mass=cfg["mass"], recon=args.recon, slab=(rank, world), comm="nccl")
+        lat = lq.Lattice(Lg, mass=cfg["mass"], recon=args.recon, slab=(rank, world), comm=args.slab_comm)
         lat.set_gauge(U)
         b = lat.pack(f, 0)
         x = lat.new_vector(len(cfg["shifts"]))
@@ -723,7 +724,10 @@ def run_slab_check(args):
         res["timing"] = {"lattice": list(Lg), "iters": info["iters"], "s_per_iter": ms * 1e-3 / max(info["iters"], 1),
                          "s_per_iter_per_gpu_volume": ms * 1e-3 / max(info["iters"], 1) / world,
                          "operator_us": op_us, "face_bytes_each_way": face,
-                         "face_bytes_per_application": 2 * face, "transport": "NCCL send/recv + all-reduce"}
+                         "face_bytes_per_application": 2 * face,
+                         "transport": {"nccl": "NCCL send/recv + all-reduce",
+                                       "p2p": "peer-mapped windows: faces stored into the neighbours' halo buffers, "
+                                              "stream memory operations, slot all-reduce"}[args.slab_comm]}
         lat.close()
     barrier(world)
     if rank == 0:
@@ -732,9 +736,9 @@ def run_slab_check(args):
     return 0
 
 
-def guarded_slab_run(args, n: int, timeout_s: float = 600.0):
+def guarded_slab_run(args, n: int, comm: str = "nccl", timeout_s: float = 600.0):
     """rank 0 of the headline run: start the slab check as a separate set of n ranks and wait at most timeout_s."""
-    argv = ["--slab-check", "--gpus", str(n), "--steps", str(args.steps), "--warmup", str(args.warmup),
+    argv = ["--slab-check", "--slab-comm", comm, "--gpus", str(n), "--steps", str(args.steps), "--warmup", str(args.warmup),
             "--workload", args.workload, "--recon", str(args.recon)]
     cmd = torchrun_cmd(n, argv) if n > 1 else [sys.executable, os.path.abspath(__file__)] + argv
     env = {k: v for k, v in os.environ.items()
@@ -745,7 +749,15 @@ def guarded_slab_run(args, n: int, timeout_s: float = 600.0):
     env.setdefault("NCCL_DEBUG_SUBSYS", "INIT")
     t0 = time.perf_counter()
     try:
-        p = subprocess.run(cmd, env=env, stdout=subprocess.PIPE, stderr=sys.stderr, timeout=timeout_s, text=True)
+        # its own process group: a rank that hangs is killed together with its launcher
+        proc = subprocess.Popen(cmd, env=env, stdout=subprocess.PIPE, stderr=sys.stderr, text=True, start_new_session=True)
+        try:
+            stdout, _ = proc.communicate(timeout=timeout_s)
+        except subprocess.TimeoutExpired:
+            os.killpg(proc.pid, signal.SIGKILL)
+            proc.communicate()
+            raise
+        p = subprocess.CompletedProcess(cmd, proc.returncode, stdout, None)
     except subprocess.TimeoutExpired:
         return {"error": f"slab sub-run did not finish within {timeout_s:.0f} s (killed)", "n_ranks": n}
     for line in reversed(p.stdout.splitlines()):
@@ -864,6 +876,7 @@ def main():
     ap.add_argument("--with-slab", action="store_true",
                     help="also run the guarded slab sub-run when N = 1 (it always runs when N > 1)")
     ap.add_argument("--slab-check", action="store_true", help=argparse.SUPPRESS)
+    ap.add_argument("--slab-comm", default="nccl", choices=["nccl", "p2p"], help=argparse.SUPPRESS)
     ap.add_argument("--plumbing-check", action="store_true", help=argparse.SUPPRESS)
     args = ap.parse_args()
     self_launch(args, sys.argv[1:])
@@ -980,8 +993,9 @@ def main():
             line[key] = res[key]
     phase("GPU part done")
     if world > 1 or args.with_slab:
-        line["slab"] = guarded_slab_run(args, world)
-        phase("slab sub-run done")
+        line["slab"] = guarded_slab_run(args, world, "nccl")
+        line["slab_p2p"] = guarded_slab_run(args, world, "p2p")
+        phase("slab sub-runs done")
     if not args.quick and world == 1:
         s_iter, cores, sample, _ = run_oracle(args.workload, budget_s=args.cpu_budget, steps=None)
         line["cpu_baseline"] = {"value": s_iter, "unit": "s/iter", "cores": cores, "kind": "oracle", "sample": sample}

@@ -245,6 +245,10 @@ int lqcd_rational_apply_f32(lqcd_ctx* ctx, const float* b_even, double alpha0, c
  * so that the transport's connections exist before any CUDA graph is captured):
  *   lqcd_comm_init_nccl   NCCL send/recv + all-reduce on the GPU (NVLink 5 / NVSwitch between the GPUs of a node),
  *                         enqueued on streams, captured into the CUDA graph of the CG iteration;
+ *   lqcd_comm_init_p2p    peer-mapped memory between the GPUs of one node (CUDA IPC): the faces are
+ *                         written straight into the neighbours' halo buffers, arrival is a stream memory operation,
+ *                         the scalar products are summed through slots in every rank's window; no transport kernel
+ *                         on the path of the faces, no CUDA graph (the iteration is launched plainly);
  *   lqcd_set_comm         caller-supplied functions, e.g. on top of MPI or torch.distributed.
  */
 lqcd_ctx* lqcd_create_slab(int Lx, int Ly, int Lz, int Lt_global, int rank, int nranks);
@@ -278,6 +282,18 @@ int lqcd_set_comm(lqcd_ctx* ctx, const lqcd_comm_ops* ops /*HOST; copied*/);
 #define LQCD_NCCL_ID_BYTES 128
 int lqcd_nccl_unique_id(void* id /*HOST, 128 bytes*/);
 int lqcd_comm_init_nccl(lqcd_ctx* ctx, const void* id /*HOST, 128 bytes*/);
+
+/* Peer-memory transport (GPUs of one node that can map each other's memory; also ranks that share a GPU).
+ * Every rank calls lqcd_p2p_export, which allocates its window (header + four face buffers, each the size of the
+ * largest face message: 288 bytes x Lx/2*Ly*Lz) and writes LQCD_P2P_HANDLE_BYTES describing it; the caller gathers
+ * the handles of all ranks by any means (e.g. torch.distributed.all_gather_object) and hands every rank the table of
+ * all of them, in rank order, through lqcd_comm_init_p2p (not collective: it only maps the windows).  At most 16
+ * ranks.  LQCD_ECOMM if a window cannot be mapped (no peer access, other node) or stream memory operations are
+ * unavailable.  STATUS: verified on one GPU (one rank; two and four ranks as processes sharing the GPU over CUDA IPC);
+ * not run between two or more GPUs. */
+#define LQCD_P2P_HANDLE_BYTES 96
+int lqcd_p2p_export(lqcd_ctx* ctx, void* handle /*HOST, LQCD_P2P_HANDLE_BYTES*/);
+int lqcd_comm_init_p2p(lqcd_ctx* ctx, const void* handles /*HOST, nranks * LQCD_P2P_HANDLE_BYTES, rank order*/);
 
 /* rank, nranks, first global time slice and global Lt of a context (0, 1, 0, Lt for a whole-lattice one) */
 int lqcd_slab_info(const lqcd_ctx* ctx, int* rank, int* nranks, int* t_offset, int* Lt_global /*HOST, may be NULL*/);

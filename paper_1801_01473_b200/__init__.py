@@ -9,7 +9,7 @@ Functions carry the C names (``lqcd_create`` ...); :class:`Lattice` is a small c
 takes torch tensors (device memory and streams are torch's job, nothing else is).
 """
 from .binding import (  # noqa: F401
-    LQCD_OK, LQCD_EINVAL, LQCD_ENOGAUGE, LQCD_ENOMEM, LQCD_ECUDA, LQCD_ENOCONV, LQCD_EBREAKDOWN, LQCD_ENOTSU3, LQCD_ECOMM, LQCD_NCCL_ID_BYTES,
+    LQCD_OK, LQCD_EINVAL, LQCD_ENOGAUGE, LQCD_ENOMEM, LQCD_ECUDA, LQCD_ENOCONV, LQCD_EBREAKDOWN, LQCD_ENOTSU3, LQCD_ECOMM, LQCD_NCCL_ID_BYTES, LQCD_P2P_HANDLE_BYTES,
     LQCD_OPT_MASS, LQCD_OPT_ANTIPERIODIC_T, LQCD_OPT_RECON, LQCD_OPT_MAX_ITER, LQCD_OPT_CHECK_EVERY,
     LQCD_OPT_USE_GRAPH, LQCD_OPT_LINK_PRECISIONS, LQCD_OPT_SHIFT_BLOCK, LQCD_OPT_PERSISTENT, LQCD_PREC_F64, LQCD_PREC_F32,
     LQCD_STAT_ITERS, LQCD_STAT_REL_RES, LQCD_STAT_FREEZE_ITER, LQCD_STAT_BASE_SHIFT, LQCD_STAT_GPU_LAUNCHES,
@@ -21,6 +21,6 @@ from .binding import (  # noqa: F401
     lqcd_last_error,
     lqcd_doe_f32, lqcd_deo_f32, lqcd_doe_f32_host, lqcd_deo_f32_host, lqcd_mdagm_f32, lqcd_mshift_cg_f32,
     lqcd_mshift_cg_f32_host, lqcd_rational_apply_f32, lqcd_pack_vector_f32, lqcd_unpack_vector_f32,
-    lqcd_create_slab, lqcd_set_comm, lqcd_nccl_unique_id, lqcd_comm_init_nccl, lqcd_slab_info, lqcd_comm_ops,
+    lqcd_create_slab, lqcd_set_comm, lqcd_nccl_unique_id, lqcd_comm_init_nccl, lqcd_p2p_export, lqcd_comm_init_p2p, lqcd_slab_info, lqcd_comm_ops,
     TorchTransport, lqcd_mshift_cg_mixed,
 )

@@ -11,6 +11,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 LQCD_OK, LQCD_EINVAL, LQCD_ENOGAUGE, LQCD_ENOMEM, LQCD_ECUDA = 0, -1, -2, -3, -4
 LQCD_ENOCONV, LQCD_EBREAKDOWN, LQCD_ENOTSU3, LQCD_ECOMM = -5, -6, -7, -8
 LQCD_NCCL_ID_BYTES = 128
+LQCD_P2P_HANDLE_BYTES = 96
 LQCD_OPT_MASS, LQCD_OPT_ANTIPERIODIC_T, LQCD_OPT_RECON, LQCD_OPT_MAX_ITER = 0, 1, 2, 3
 LQCD_OPT_CHECK_EVERY, LQCD_OPT_USE_GRAPH, LQCD_OPT_LINK_PRECISIONS, LQCD_OPT_SHIFT_BLOCK = 4, 5, 6, 7
 LQCD_OPT_PERSISTENT = 8
@@ -76,6 +77,8 @@ EXPORTS = {
     "lqcd_set_comm": (_i, [_vp, ctypes.POINTER(lqcd_comm_ops)]),
     "lqcd_nccl_unique_id": (_i, [_vp]),
     "lqcd_comm_init_nccl": (_i, [_vp, _vp]),
+    "lqcd_p2p_export": (_i, [_vp, _vp]),
+    "lqcd_comm_init_p2p": (_i, [_vp, _vp]),
     "lqcd_slab_info": (_i, [_vp, _pi, _pi, _pi, _pi]),
 }
 
@@ -299,6 +302,20 @@ def lqcd_comm_init_nccl(ctx, nccl_id: bytes):
     return load_library().lqcd_comm_init_nccl(ctx, ctypes.cast(buf, _vp))
 
 
+def lqcd_p2p_export(ctx):
+    """-> (rc, LQCD_P2P_HANDLE_BYTES bytes)"""
+    buf = ctypes.create_string_buffer(LQCD_P2P_HANDLE_BYTES)
+    rc = load_library().lqcd_p2p_export(ctx, ctypes.cast(buf, _vp))
+    return rc, buf.raw
+
+
+def lqcd_comm_init_p2p(ctx, handles: bytes):
+    """``handles``: the LQCD_P2P_HANDLE_BYTES of every rank, concatenated in rank order"""
+    assert len(handles) % LQCD_P2P_HANDLE_BYTES == 0
+    buf = ctypes.create_string_buffer(bytes(handles), len(handles))
+    return load_library().lqcd_comm_init_p2p(ctx, ctypes.cast(buf, _vp))
+
+
 def lqcd_slab_info(ctx):
     """-> (rc, rank, nranks, t_offset, Lt_global)"""
     v = [ctypes.c_int(0) for _ in range(4)]
@@ -393,6 +410,7 @@ class Lattice:
         """``slab=(rank, nranks)``: this process owns time slices [rank*Lt/nranks, (rank+1)*Lt/nranks) of the
         lattice ``L`` (include/lqcd.h, slab decomposition); all tensors are then those of the local lattice
         ``self.L`` = (Lx, Ly, Lz, Lt/nranks).  ``comm``: "nccl" (the library's own NCCL communicator; the id is
+        handed round with ``torch.distributed``), "p2p" (the library's peer-memory transport; the window handles are
         handed round with ``torch.distributed``) or "torch" (:class:`TorchTransport`, host-staged)."""
         import torch
         if not torch.cuda.is_available():
@@ -442,6 +460,16 @@ class Lattice:
                                            group=group)
                 nccl_id = box[0]
             self._check(lqcd_comm_init_nccl(self.ctx, nccl_id))
+        elif comm == "p2p":
+            import torch.distributed as dist
+            rc, mine = lqcd_p2p_export(self.ctx)
+            self._check(rc)
+            handles = [mine]
+            if nranks > 1:
+                assert dist.is_initialized() and dist.get_world_size(group) == nranks and dist.get_rank(group) == rank
+                handles = [None] * nranks
+                dist.all_gather_object(handles, mine, group=group)
+            self._check(lqcd_comm_init_p2p(self.ctx, b"".join(handles)))
         else:
             raise ValueError(f"unknown transport {comm!r}")
 

@@ -565,11 +565,13 @@ __global__ void __launch_bounds__(DS_BLOCK, (DsOcc<T, EPI>::minb)) dslash_kernel
 }
 
 // Slab mode, before K1: the two faces (time slices 0 and Lt-1) of p = r + beta p_old, formed by the rank that owns the
-// sites with the formula K1 uses at the neighbours (load_vec, MODE 1: same operands, same bits), packed for the ring
-// exchange as [lo|hi][c][face].  One thread per complex number.
+// sites with the formula K1 uses at the neighbours (load_vec, MODE 1: same operands, same bits), packed as [c][face]
+// each: into the send buffers of the ring exchange, or (peer-memory transport) straight into the neighbours' halo
+// buffers over NVLink.  One thread per complex number.
 template <typename T>
 __global__ void __launch_bounds__(256) slab_pack_p_kernel(const V2<T>* __restrict__ r, const V2<T>* __restrict__ p_old,
-                                                          V2<T>* __restrict__ send, const CgState* st, size_t vh, size_t face) {
+                                                          V2<T>* __restrict__ send_lo, V2<T>* __restrict__ send_hi,
+                                                          const CgState* st, size_t vh, size_t face) {
     if (st->stop) return;
     const size_t i = (size_t)blockIdx.x * 256 + threadIdx.x;
     if (i >= 6 * face) return;
@@ -578,7 +580,7 @@ __global__ void __launch_bounds__(256) slab_pack_p_kernel(const V2<T>* __restric
     const size_t c = rem / face, kf = rem - c * face;
     const size_t src = c * vh + (hi ? vh - face : 0) + kf;
     const V2<T> rv = r[src], q = p_old[src];
-    send[i] = make_v2(fma(beta, q.x, rv.x), fma(beta, q.y, rv.y));
+    (hi ? send_hi : send_lo)[rem] = make_v2(fma(beta, q.x, rv.x), fma(beta, q.y, rv.y));
 }
 
 #endif

@@ -18,6 +18,7 @@
 #include "comm.h"
 #include "dslash.cuh"
 #include "lqcd_internal.cuh"
+#include "p2p.cuh"
 #include "persist.cuh"
 
 namespace {
@@ -93,6 +94,7 @@ struct lqcd_ctx {
     lqcd_comm_ops comm;
     bool has_comm;
     lqcd_nccl::Transport nccl;
+    lqcd_p2p::Transport p2p;     // peer-memory transport (lqcd_comm_init_p2p)
     cudaStream_t comm_stream;
     cudaEvent_t ev_pack, ev_halo;
     double* red;             // device: the scalar product being reduced over ranks
@@ -417,17 +419,27 @@ int slab_apply(lqcd_ctx* c, DslashArgs<T>& a, int kepi, const V2<T>* face_v, con
     V2<T>* send_hi = B.halo_send + 3 * face;
     V2<T>* recv_lo = B.halo_recv;
     V2<T>* recv_hi = B.halo_recv + 3 * face;
+    // peer-memory transport: the faces are written straight into the neighbours' halo buffers (no send buffer, no
+    // transport kernel), and the border launch reads my halos where the neighbours wrote them (p2p.cuh)
+    const bool p2p = c->p2p.active && c->comm.user == (void*)&c->p2p;
+    if (p2p) {
+        const lqcd_p2p::Slots o = lqcd_p2p::begin(&c->p2p);
+        send_lo = (V2<T>*)o.dst_dn;
+        send_hi = (V2<T>*)o.dst_up;
+        recv_lo = (V2<T>*)o.recv_lo;
+        recv_hi = (V2<T>*)o.recv_hi;
+    }
     // the input is complete at this point of the compute stream; everything about the faces happens on the
     // communication stream from here on, beside the interior launch
     CU(cudaEventRecord(c->ev_pack, c->stream));
     CU(cudaStreamWaitEvent(c->comm_stream, c->ev_pack, 0));
     if (face_v2) {
-        slab_pack_p_kernel<T><<<(int)((6 * face + 255) / 256), 256, 0, c->comm_stream>>>(face_v, face_v2, B.halo_send, c->st_dev, vh, face);
+        slab_pack_p_kernel<T><<<(int)((6 * face + 255) / 256), 256, 0, c->comm_stream>>>(face_v, face_v2, send_lo, send_hi, c->st_dev, vh, face);
         ++c->launches;
     } else {
         // a face is three contiguous runs (one per colour) of the vector: strided copies, no kernel
-        CU(cudaMemcpy2DAsync(send_lo, row, face_v, pitch, row, 3, cudaMemcpyDeviceToDevice, c->comm_stream));
-        CU(cudaMemcpy2DAsync(send_hi, row, face_v + (vh - face), pitch, row, 3, cudaMemcpyDeviceToDevice, c->comm_stream));
+        CU(cudaMemcpy2DAsync(send_lo, row, face_v, pitch, row, 3, cudaMemcpyDefault, c->comm_stream));
+        CU(cudaMemcpy2DAsync(send_hi, row, face_v + (vh - face), pitch, row, 3, cudaMemcpyDefault, c->comm_stream));
     }
 
     a.g = c->g;
@@ -460,7 +472,11 @@ int slab_apply(lqcd_ctx* c, DslashArgs<T>& a, int kepi, const V2<T>* face_v, con
     }
     // faces in flight on the communication stream; the two border slices (t = 0 and t = Lt-1) follow them on
     // that stream, so they run beside the interior (disjoint outputs and partial slots) instead of after it
-    if ((rc = comm_exchange(c, send_lo, send_hi, recv_lo, recv_hi, 3 * row))) return rc;
+    if (p2p) {
+        if (lqcd_p2p::signal_wait(&c->p2p, c->comm_stream)) return fail(c, LQCD_ECOMM, "peer-memory transport: %s", c->p2p.error);
+    } else if ((rc = comm_exchange(c, send_lo, send_hi, recv_lo, recv_hi, 3 * row))) {
+        return rc;
+    }
     a.k0a = 0;
     a.na = (int)face;
     a.k0b = (int)(vh - face);
@@ -905,6 +921,7 @@ void lqcd_destroy(lqcd_ctx* c) {
         lqcd_nccl::Api* a = lqcd_nccl::api(nullptr);
         if (a) a->CommDestroy(c->nccl.comm);
     }
+    lqcd_p2p::destroy(&c->p2p);
     if (c->host_stage) cudaFreeHost(c->host_stage);
     if (c->red_host) cudaFreeHost(c->red_host);
     if (c->comm_stream) cudaStreamDestroy(c->comm_stream);
@@ -998,6 +1015,36 @@ int lqcd_comm_init_nccl(lqcd_ctx* c, const void* id) {
     ops.allreduce_sum = lqcd_nccl::allreduce_sum;
     ops.host_staged = 0;
     ops.graph_safe = 1;
+    return lqcd_set_comm(c, &ops);
+}
+
+int lqcd_p2p_export(lqcd_ctx* c, void* handle) {
+    if (!c) return LQCD_EINVAL;
+    if (!c->slab) return fail(c, LQCD_EINVAL, "not a slab context (lqcd_create_slab)");
+    if (!handle) return fail(c, LQCD_EINVAL, "handle is NULL");
+    // a face buffer holds the largest message of the path: the t-links of one face, both parities, 18 reals, double
+    const size_t cap = (size_t)2 * 9 * face_sites(c) * sizeof(double2);
+    lqcd_p2p::Blob b;
+    if (lqcd_p2p::create_window(&c->p2p, c->rank, c->nranks, cap, &b)) return fail(c, LQCD_ECOMM, "peer-memory transport: %s", c->p2p.error);
+    memcpy(handle, &b, sizeof(b));
+    return LQCD_OK;
+}
+
+int lqcd_comm_init_p2p(lqcd_ctx* c, const void* handles) {
+    if (!c) return LQCD_EINVAL;
+    if (!c->slab) return fail(c, LQCD_EINVAL, "not a slab context (lqcd_create_slab)");
+    if (!handles) return fail(c, LQCD_EINVAL, "handles is NULL");
+    if (c->p2p.active) return fail(c, LQCD_EINVAL, "peer-memory transport already initialised");
+    static_assert(sizeof(lqcd_p2p::Blob) == LQCD_P2P_HANDLE_BYTES, "LQCD_P2P_HANDLE_BYTES");
+    std::vector<lqcd_p2p::Blob> blobs((size_t)c->nranks);
+    memcpy(blobs.data(), handles, blobs.size() * sizeof(lqcd_p2p::Blob));
+    if (lqcd_p2p::connect(&c->p2p, blobs.data())) return fail(c, LQCD_ECOMM, "peer-memory transport: %s", c->p2p.error);
+    lqcd_comm_ops ops;
+    ops.user = &c->p2p;
+    ops.exchange = lqcd_p2p::exchange;
+    ops.allreduce_sum = lqcd_p2p::allreduce_sum;
+    ops.host_staged = 0;
+    ops.graph_safe = 0;          // the sequence numbers of the stream memory operations change from call to call
     return lqcd_set_comm(c, &ops);
 }
 

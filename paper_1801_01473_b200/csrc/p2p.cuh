@@ -1,0 +1,254 @@
+// p2p.cuh -- the two exchange steps of the slab-decomposed path over peer-mapped memory (NVLink 5 / NVSwitch
+// between the GPUs of a node; the paper: "CUDA-aware MPI ... CUDA inter-process communication between GPUs attached
+// to the same host").  No NCCL kernel, no staging buffer:
+//
+//   * every rank owns ONE device allocation, its WINDOW: a header of flag words and all-reduce slots, then four face
+//     buffers ([from rank-1 | from rank+1] x two generations).  The window is exported with cudaIpcGetMemHandle; the
+//     handles travel once over the caller's channel (lqcd_p2p_export / lqcd_comm_init_p2p), and every rank maps every
+//     other rank's window (cudaIpcOpenMemHandle enables peer access over NVLink);
+//   * face exchange of application number s (one counter per rank, the same on all of them): the sender WRITES its
+//     two faces straight into the neighbours' face buffers of generation s&1 -- strided copies or the stores of the
+//     pack kernel, from the vector itself -- then writes s into the neighbours' `arrived` words with a stream memory
+//     operation (cuStreamWriteValue32, ordered after the copies), and waits for its own two `arrived` words to reach s
+//     (cuStreamWaitValue32 on LOCAL memory).  The border launch reads the halo in place, in the window;
+//   * no flow control is needed beyond the two generations: a rank that sends face s has received face s-1 from that
+//     neighbour, which the neighbour sent (stream order) after the launch that consumed ITS halo of s-2, the last
+//     tenant of the buffer now being overwritten;
+//   * all-reduce of the scalar products: one kernel of one warp stores this rank's value into slot [generation][rank]
+//     of every rank's window (itself included) and then, after a system-wide fence, the sequence number into their
+//     `red_arrived[rank]` words; nranks stream waits on the local words; one kernel adds the slots in rank order, so
+//     every rank holds the same bits (R8).  The same two-generation argument applies.
+//
+// Nothing here spins inside a kernel: every wait is a stream memory operation on the waiting rank's own memory, so
+// several ranks may share one GPU (tests) without any kernel of one waiting for a kernel of another.
+// The waits are not captured into CUDA graphs (graph_safe = 0): the sequence numbers change from call to call.
+#ifndef LQCD_P2P_CUH
+#define LQCD_P2P_CUH
+
+#include <cuda.h>
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <string.h>
+#include <unistd.h>
+
+namespace lqcd_p2p {
+
+constexpr int MAX_RANKS = 16;
+constexpr int RED_MAX = 4;                 // doubles per all-reduce
+constexpr size_t HDR_BYTES = 2048;
+
+struct Header {                            // start of every window
+    unsigned int arrived[2];               // [0]: number of the last exchange whose face from rank-1 is complete; [1]: rank+1
+    unsigned int pad[14];
+    unsigned int red_arrived[MAX_RANKS];   // number of the last all-reduce whose contribution from rank q is complete
+    double red[2][MAX_RANKS][RED_MAX];     // [generation][rank][value]
+};
+static_assert(sizeof(Header) <= HDR_BYTES, "window header");
+
+// what travels between the ranks (LQCD_P2P_HANDLE_BYTES of include/lqcd.h)
+struct Blob {
+    cudaIpcMemHandle_t ipc;                // 64 bytes
+    long long pid;
+    unsigned long long ptr;                // the window in the exporting process (used when it is this process)
+    unsigned long long cap;
+    int device;
+    int rank;
+};
+static_assert(sizeof(Blob) == 96, "LQCD_P2P_HANDLE_BYTES");
+
+typedef CUresult (*mem_op32_fn)(CUstream, CUdeviceptr, cuuint32_t, unsigned int);
+
+struct Transport {
+    bool active = false;
+    int rank = 0, nranks = 1, device = 0;
+    char* win[MAX_RANKS] = {};             // every rank's window as mapped in this process; win[rank] is mine
+    bool opened[MAX_RANKS] = {};           // mapped with cudaIpcOpenMemHandle (to be closed)
+    size_t cap = 0;                        // bytes of one face buffer
+    unsigned int seq = 0, rseq = 0;        // exchanges / all-reduces issued so far
+    mem_op32_fn wait32 = nullptr, write32 = nullptr;
+    const char* error = "";
+
+    Header* hdr(int r) const { return (Header*)win[r]; }
+    // face buffer of rank r: side 0 = halo below its slab (filled by r-1), 1 = above (filled by r+1)
+    char* face(int r, int side, unsigned int s) const { return win[r] + HDR_BYTES + ((size_t)side * 2 + (s & 1)) * cap; }
+    int dn() const { return (rank + nranks - 1) % nranks; }
+    int up() const { return (rank + 1) % nranks; }
+};
+
+inline size_t window_bytes(size_t cap) { return HDR_BYTES + 4 * cap; }
+
+inline int fail(Transport* t, const char* why) {
+    t->error = why;
+    cudaGetLastError();
+    return -1;
+}
+
+// allocate this rank's window and describe it
+inline int create_window(Transport* t, int rank, int nranks, size_t cap, Blob* out) {
+    if (nranks > MAX_RANKS) return fail(t, "more ranks than the peer-memory transport handles");
+    if (t->win[rank]) return fail(t, "window already exported");
+    void* fn = nullptr;
+    cudaDriverEntryPointQueryResult q;
+    if (cudaGetDriverEntryPoint("cuStreamWaitValue32", &fn, cudaEnableDefault, &q) != cudaSuccess || !fn)
+        return fail(t, "cuStreamWaitValue32 not available");
+    t->wait32 = (mem_op32_fn)fn;
+    if (cudaGetDriverEntryPoint("cuStreamWriteValue32", &fn, cudaEnableDefault, &q) != cudaSuccess || !fn)
+        return fail(t, "cuStreamWriteValue32 not available");
+    t->write32 = (mem_op32_fn)fn;
+    t->rank = rank;
+    t->nranks = nranks;
+    t->cap = (cap + 255) / 256 * 256;
+    if (cudaGetDevice(&t->device) != cudaSuccess) return fail(t, "cudaGetDevice");
+    void* w = nullptr;
+    if (cudaMalloc(&w, window_bytes(t->cap)) != cudaSuccess) return fail(t, "cudaMalloc of the window");
+    if (cudaMemset(w, 0, HDR_BYTES) != cudaSuccess || cudaDeviceSynchronize() != cudaSuccess) {
+        cudaFree(w);
+        return fail(t, "clearing the window");
+    }
+    t->win[rank] = (char*)w;
+    memset(out, 0, sizeof(Blob));
+    if (cudaIpcGetMemHandle(&out->ipc, w) != cudaSuccess) {
+        // a device without IPC support can still run ranks of one process
+        cudaGetLastError();
+    }
+    out->pid = (long long)getpid();
+    out->ptr = (unsigned long long)(uintptr_t)w;
+    out->cap = t->cap;
+    out->device = t->device;
+    out->rank = rank;
+    return 0;
+}
+
+// map every rank's window
+inline int connect(Transport* t, const Blob* blobs) {
+    if (!t->win[t->rank]) return fail(t, "lqcd_p2p_export first");
+    for (int r = 0; r < t->nranks; ++r) {
+        const Blob& b = blobs[r];
+        if (b.rank != r || b.cap != t->cap) return fail(t, "handle table does not match this lattice / rank order");
+        if (r == t->rank) continue;
+        if (b.pid == (long long)getpid()) {
+            // another context of this process: its pointer is valid here; peer access if it sits on another device
+            if (b.device != t->device) {
+                const cudaError_t e = cudaDeviceEnablePeerAccess(b.device, 0);
+                if (e != cudaSuccess && e != cudaErrorPeerAccessAlreadyEnabled) return fail(t, "no peer access to a rank of this process");
+                cudaGetLastError();
+            }
+            t->win[r] = (char*)(uintptr_t)b.ptr;
+        } else {
+            void* p = nullptr;
+            if (cudaIpcOpenMemHandle(&p, b.ipc, cudaIpcMemLazyEnablePeerAccess) != cudaSuccess)
+                return fail(t, "cudaIpcOpenMemHandle failed (ranks must be on GPUs of one node with peer access)");
+            t->win[r] = (char*)p;
+            t->opened[r] = true;
+        }
+    }
+    t->active = true;
+    return 0;
+}
+
+inline void destroy(Transport* t) {
+    for (int r = 0; r < t->nranks; ++r)
+        if (t->opened[r]) cudaIpcCloseMemHandle(t->win[r]);
+    if (t->win[t->rank]) cudaFree(t->win[t->rank]);
+    for (int r = 0; r < MAX_RANKS; ++r) {
+        t->win[r] = nullptr;
+        t->opened[r] = false;
+    }
+    t->active = false;
+    cudaGetLastError();
+}
+
+// Where the faces of the NEXT exchange go and arrive: the sender writes its lowest slice to dst_dn and its highest to
+// dst_up (peer memory); recv_lo / recv_hi are this rank's own halo buffers of that exchange.
+struct Slots {
+    void *dst_dn, *dst_up, *recv_lo, *recv_hi;
+};
+inline Slots begin(Transport* t) {
+    const unsigned int s = ++t->seq;
+    Slots o;
+    o.dst_dn = t->face(t->dn(), 1, s);       // my lowest slice is the halo ABOVE the slab of rank-1
+    o.dst_up = t->face(t->up(), 0, s);       // my highest slice is the halo BELOW the slab of rank+1
+    o.recv_lo = t->face(t->rank, 0, s);
+    o.recv_hi = t->face(t->rank, 1, s);
+    return o;
+}
+// after the writes to dst_dn / dst_up have been enqueued on `stream`: tell the neighbours, wait for mine
+inline int signal_wait(Transport* t, cudaStream_t stream) {
+    const unsigned int s = t->seq;
+    CUstream cs = (CUstream)stream;
+    if (t->write32(cs, (CUdeviceptr)(uintptr_t)&t->hdr(t->dn())->arrived[1], s, CU_STREAM_WRITE_VALUE_DEFAULT) != CUDA_SUCCESS ||
+        t->write32(cs, (CUdeviceptr)(uintptr_t)&t->hdr(t->up())->arrived[0], s, CU_STREAM_WRITE_VALUE_DEFAULT) != CUDA_SUCCESS)
+        return fail(t, "cuStreamWriteValue32 on a neighbour's window failed");
+    if (t->wait32(cs, (CUdeviceptr)(uintptr_t)&t->hdr(t->rank)->arrived[0], s, CU_STREAM_WAIT_VALUE_GEQ) != CUDA_SUCCESS ||
+        t->wait32(cs, (CUdeviceptr)(uintptr_t)&t->hdr(t->rank)->arrived[1], s, CU_STREAM_WAIT_VALUE_GEQ) != CUDA_SUCCESS)
+        return fail(t, "cuStreamWaitValue32 failed");
+    return 0;
+}
+
+// lqcd_comm_ops::exchange for arbitrary buffers (the one-time link faces): through the window, then out of it
+inline int exchange(void* user, const void* send_lo, const void* send_hi, void* recv_lo, void* recv_hi, size_t bytes,
+                    void* stream) {
+    Transport* t = (Transport*)user;
+    if (!t->active) return fail(t, "transport not connected");
+    if (bytes > t->cap) return fail(t, "message larger than a face buffer of the window");
+    cudaStream_t s = (cudaStream_t)stream;
+    const Slots o = begin(t);
+    if (cudaMemcpyAsync(o.dst_dn, send_lo, bytes, cudaMemcpyDefault, s) != cudaSuccess ||
+        cudaMemcpyAsync(o.dst_up, send_hi, bytes, cudaMemcpyDefault, s) != cudaSuccess)
+        return fail(t, "copy into a neighbour's window failed");
+    if (signal_wait(t, s)) return -1;
+    if (cudaMemcpyAsync(recv_lo, o.recv_lo, bytes, cudaMemcpyDeviceToDevice, s) != cudaSuccess ||
+        cudaMemcpyAsync(recv_hi, o.recv_hi, bytes, cudaMemcpyDeviceToDevice, s) != cudaSuccess)
+        return fail(t, "copy out of the window failed");
+    return 0;
+}
+
+struct PushArgs {
+    double* slot[MAX_RANKS];
+    unsigned int* flag[MAX_RANKS];
+    int nranks, n;
+    unsigned int seq;
+};
+// thread q: my value into rank q's slot, then (system-wide fence) the sequence number into its flag word
+__global__ void __launch_bounds__(32) p2p_push_kernel(const PushArgs a, const double* __restrict__ value) {
+    const int q = threadIdx.x;
+    if (q >= a.nranks) return;
+    for (int j = 0; j < a.n; ++j) ((volatile double*)a.slot[q])[j] = value[j];
+    __threadfence_system();
+    *(volatile unsigned int*)a.flag[q] = a.seq;
+}
+// out[j] = sum over ranks, in rank order: the same bits on every rank
+__global__ void __launch_bounds__(32) p2p_sum_kernel(const double* slots, int nranks, int n, double* __restrict__ out) {
+    const int j = threadIdx.x;
+    if (j >= n) return;
+    double acc = 0.0;
+    for (int r = 0; r < nranks; ++r) acc += __ldcv(slots + r * RED_MAX + j);
+    out[j] = acc;
+}
+
+inline int allreduce_sum(void* user, double* dev_buf, int n, void* stream) {
+    Transport* t = (Transport*)user;
+    if (!t->active) return fail(t, "transport not connected");
+    if (n < 1 || n > RED_MAX) return fail(t, "all-reduce of more values than a slot holds");
+    cudaStream_t s = (cudaStream_t)stream;
+    const unsigned int q = ++t->rseq, g = q & 1;
+    PushArgs a;
+    for (int r = 0; r < t->nranks; ++r) {
+        a.slot[r] = &t->hdr(r)->red[g][t->rank][0];
+        a.flag[r] = &t->hdr(r)->red_arrived[t->rank];
+    }
+    a.nranks = t->nranks;
+    a.n = n;
+    a.seq = q;
+    p2p_push_kernel<<<1, 32, 0, s>>>(a, dev_buf);
+    for (int r = 0; r < t->nranks; ++r)
+        if (t->wait32((CUstream)s, (CUdeviceptr)(uintptr_t)&t->hdr(t->rank)->red_arrived[r], q, CU_STREAM_WAIT_VALUE_GEQ) != CUDA_SUCCESS)
+            return fail(t, "cuStreamWaitValue32 failed");
+    p2p_sum_kernel<<<1, 32, 0, s>>>(&t->hdr(t->rank)->red[g][0][0], t->nranks, n, dev_buf);
+    if (cudaGetLastError() != cudaSuccess) return fail(t, "launch of the all-reduce kernels failed");
+    return 0;
+}
+
+}  // namespace lqcd_p2p
+
+#endif

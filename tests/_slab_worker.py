@@ -19,10 +19,13 @@ import oracle  # noqa: E402
 
 L = tuple(int(v) for v in sys.argv[1:5])
 RECON = int(sys.argv[6]) if len(sys.argv) > 6 else 18
-COMM = sys.argv[5] if len(sys.argv) > 5 else "torch"      # "torch": host-staged, ranks share cuda:0; "nccl": one GPU each
+# "torch": host-staged, ranks share cuda:0; "nccl": one GPU each; "p2p": peer-mapped windows, one GPU each when there
+# are enough of them, else the ranks share the GPUs there are (CUDA IPC between processes on one device)
+COMM = sys.argv[5] if len(sys.argv) > 5 else "torch"
 dist.init_process_group("gloo", init_method="env://")
 rank, world = dist.get_rank(), dist.get_world_size()
-torch.cuda.set_device(int(os.environ.get("LOCAL_RANK", "0")) if COMM == "nccl" else 0)
+_lr = int(os.environ.get("LOCAL_RANK", "0"))
+torch.cuda.set_device(_lr if COMM == "nccl" else (_lr % torch.cuda.device_count() if COMM == "p2p" else 0))
 
 mass, tol, shifts = 0.05, 1e-10, [1e-3, 1e-2, 1e-1, 1.0]
 U, f = make_inputs(L)                                   # every rank draws the same whole-lattice inputs
@@ -96,6 +99,7 @@ if rank == 0:
         freeze_equal_on_ranks=all(s[1] == stats[0][1] and s[2] == stats[0][2] for s in stats),
         exchanges=lat.transport.n_exchange if lat.transport else None)
     print("RESULT " + json.dumps(res))
+dist.barrier()          # nobody unmaps a window another rank may still be writing to
 lat.close()
 dist.barrier()
 dist.destroy_process_group()

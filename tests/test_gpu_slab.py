@@ -7,10 +7,14 @@ One GPU is all there is here, so:
     interior/border split, the halo buffers, the link halo and the unfused reductions;
   * two ranks as two processes that share the GPU, host-staged through gloo (tests/_slab_worker.py): exercises
     t_off != 0, the antiperiodic sign on the right rank, the ring order of the faces.  No kernel ever waits on
-    another rank: the processes only block on the host.
+    another rank: the processes only block on the host;
+  * the peer-memory transport (csrc/p2p.cuh): one rank (its own window as both neighbours), and two / four ranks as
+    processes that share the GPU and map each other's windows over CUDA IPC.  Its waits are stream memory operations on
+    the waiting rank's own memory, never a kernel.
 """
 import json
 import os
+import signal
 import socket
 import subprocess
 import sys
@@ -30,7 +34,7 @@ ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 SHIFTS = [1e-3, 1e-2, 1e-1, 1.0]
 
 
-@pytest.mark.parametrize("comm", ["nccl", "torch"])
+@pytest.mark.parametrize("comm", ["nccl", "torch", "p2p"])
 @pytest.mark.parametrize("L,recon", [((4, 6, 8, 10), 18), ((8, 4, 6, 2), 18), ((4, 4, 4, 4), 12)])
 def test_one_rank_slab_operators_and_cg(L, recon, comm):
     U, f = make_inputs(L)
@@ -155,12 +159,20 @@ def _free_port():
         return s.getsockname()[1]
 
 
-def _run_ranks(world, L, comm, recon=18):
+def _run_ranks(world, L, comm, recon=18, timeout=600):
     cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", str(world),
            "--master-addr", "127.0.0.1", "--master-port", str(_free_port()),
            os.path.join("tests", "_slab_worker.py"), *[str(v) for v in L], comm, str(recon)]
-    out = subprocess.run(cmd, cwd=ROOT, env=dict(os.environ, OMP_NUM_THREADS="4"), capture_output=True, text=True,
-                         timeout=600)
+    # its own process group, so that a rank that hangs can be killed together with its launcher
+    proc = subprocess.Popen(cmd, cwd=ROOT, env=dict(os.environ, OMP_NUM_THREADS="4"), stdout=subprocess.PIPE,
+                            stderr=subprocess.PIPE, text=True, start_new_session=True)
+    try:
+        stdout, stderr = proc.communicate(timeout=timeout)
+    except subprocess.TimeoutExpired:
+        os.killpg(proc.pid, signal.SIGKILL)
+        stdout, stderr = proc.communicate()
+        raise AssertionError(f"{world} ranks over {comm} timed out\n" + stdout[-2000:] + stderr[-3000:])
+    out = subprocess.CompletedProcess(cmd, proc.returncode, stdout, stderr)
     assert out.returncode == 0, out.stdout[-2000:] + out.stderr[-3000:]
     line = [l for l in out.stdout.splitlines() if l.startswith("RESULT ")]
     assert len(line) == 1, out.stdout[-2000:]
@@ -184,9 +196,21 @@ def test_four_ranks_share_the_gpu_host_staged():
     _run_ranks(4, (4, 4, 4, 8), "torch")            # two time slices per rank: no interior
 
 
+@pytest.mark.parametrize("L,recon", [((4, 6, 4, 8), 18), ((4, 4, 6, 8), 12)])
+def test_two_ranks_share_the_gpu_over_peer_memory(L, recon):
+    """Two processes on one GPU map each other's windows over CUDA IPC: faces written into the neighbour's window,
+    arrival flags by stream memory operations, scalar products through the windows' slots."""
+    _run_ranks(2, L, "p2p", recon, timeout=300)
+
+
+def test_four_ranks_share_the_gpu_over_peer_memory():
+    _run_ranks(4, (4, 4, 4, 8), "p2p", timeout=300)     # two time slices per rank: no interior, four-way all-reduce
+
+
+@pytest.mark.parametrize("comm", ["nccl", "p2p"])
 @pytest.mark.parametrize("world,L", [(2, (8, 8, 8, 8)), (4, (4, 6, 8, 16))])
-def test_ranks_on_their_own_gpus_over_nccl(world, L):
-    """The production transport between GPUs: needs `world` devices, skipped on a one-GPU box."""
+def test_ranks_on_their_own_gpus_over_nccl(world, L, comm):
+    """The production transports between GPUs: needs `world` devices, skipped on a one-GPU box."""
     if torch.cuda.device_count() < world:
         pytest.skip(f"needs {world} GPUs")
-    _run_ranks(world, L, "nccl")
+    _run_ranks(world, L, comm)
