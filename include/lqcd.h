@@ -105,6 +105,7 @@ typedef struct lqcd_ctx lqcd_ctx;
 #define LQCD_STAT_GPU_LAUNCHES   4  /* kernels launched by this context since creation                    */
 #define LQCD_STAT_SOLVE_MS       5  /* device time of the last solve between CUDA events, milliseconds     */
 #define LQCD_STAT_RELIABLE_UPDATES 6 /* lqcd_mshift_cg_mixed: double-precision residual replacements performed */
+#define LQCD_STAT_GRAPH_REPLAYS  7  /* CUDA-graph replays of the last solve (0: plain launches or the persistent kernel) */
 
 /* Create a context for an Lx*Ly*Lz*Lt lattice on the current CUDA device.  NULL on error
  * (extent odd or < 2, volume too large, no device). */

@@ -17,7 +17,7 @@ LQCD_OPT_CHECK_EVERY, LQCD_OPT_USE_GRAPH, LQCD_OPT_LINK_PRECISIONS, LQCD_OPT_SHI
 LQCD_OPT_PERSISTENT = 8
 LQCD_PREC_F64, LQCD_PREC_F32 = 1, 2
 LQCD_STAT_ITERS, LQCD_STAT_REL_RES, LQCD_STAT_FREEZE_ITER, LQCD_STAT_BASE_SHIFT = 0, 1, 2, 3
-LQCD_STAT_GPU_LAUNCHES, LQCD_STAT_SOLVE_MS, LQCD_STAT_RELIABLE_UPDATES = 4, 5, 6
+LQCD_STAT_GPU_LAUNCHES, LQCD_STAT_SOLVE_MS, LQCD_STAT_RELIABLE_UPDATES, LQCD_STAT_GRAPH_REPLAYS = 4, 5, 6, 7
 
 _ERRNAMES = {0: "LQCD_OK", -1: "LQCD_EINVAL", -2: "LQCD_ENOGAUGE", -3: "LQCD_ENOMEM", -4: "LQCD_ECUDA",
              -5: "LQCD_ENOCONV", -6: "LQCD_EBREAKDOWN", -7: "LQCD_ENOTSU3", -8: "LQCD_ECOMM"}
@@ -645,6 +645,7 @@ class Lattice:
             freeze_iter=[int(self.stat(LQCD_STAT_FREEZE_ITER, i)) for i in range(n)],
             base_shift=int(self.stat(LQCD_STAT_BASE_SHIFT)),
             solve_ms=self.stat(LQCD_STAT_SOLVE_MS),
+            graph_replays=int(self.stat(LQCD_STAT_GRAPH_REPLAYS)),
         )
 
     def rational_apply(self, b_even, alpha0: float, alpha: Sequence[float], shifts: Sequence[float], tol: float,

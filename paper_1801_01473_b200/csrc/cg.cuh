@@ -69,11 +69,26 @@ __global__ void __launch_bounds__(CG_BLOCK) cg_init_kernel(const V2<T>* __restri
 // (cg_scalar_kernel), so that all ranks take the same decisions.
 __global__ void __launch_bounds__(CG_BLOCK) sum_partials_kernel(const double* __restrict__ partials, int n,
                                                                 double* __restrict__ out, const CgState* st,
-                                                                int check_stop) {
-    if (check_stop && st->stop) return;
+                                                                int check_stop, const PeerPush* __restrict__ push) {
     __shared__ double red[32];
-    const double v = final_sum<CG_BLOCK>(partials, n, red);
+    // peer-memory transport (push != NULL): the rank's sum goes straight into every rank's window; when the solve is
+    // over a dummy still goes, because every rank still waits for every rank's contribution
+    if (check_stop && st->stop) {
+        if (push) peer_push(push, 0.0);
+        return;
+    }
+    const double v = broadcast0(final_sum<CG_BLOCK>(partials, n, red), red);
     if (threadIdx.x == 0) *out = v;
+    if (push) peer_push(push, v);
+}
+// whole lattice: the sum of the block partials of K1 (which = 1) / K2 (which = 2) and the scalar step, one block
+__global__ void __launch_bounds__(CG_BLOCK) cg_reduce_scalar_kernel(CgState* st, const double* __restrict__ partials, int n,
+                                                                    int which) {
+    if (st->stop) return;
+    __shared__ double red[32];
+    const double v = broadcast0(final_sum<CG_BLOCK>(partials, n, red), red);
+    if (which == 1) cg_scalars_after_pAp(st, v);
+    else cg_scalars_after_rr(st, v);
 }
 // which = 0: after |b|^2 ; 1: after <p,Ap> ; 2: after |r_new|^2.  One block of >= LQCD_MAX_SHIFTS threads.
 __global__ void __launch_bounds__(64) cg_scalar_kernel(CgState* st, const double* __restrict__ value, int which,
@@ -86,6 +101,23 @@ __global__ void __launch_bounds__(64) cg_scalar_kernel(CgState* st, const double
     if (st->stop) return;
     if (which == 1) cg_scalars_after_pAp(st, v);
     else cg_scalars_after_rr(st, v);
+}
+
+// The same after the peer-memory transport's push (p2p.cuh): the ranks' contributions sit in this rank's window,
+// slots[r * stride]; they are added in rank order (same bits on every rank), their arrival flags cleared.
+__global__ void __launch_bounds__(64) cg_scalar_slots_kernel(CgState* st, const double* slots, unsigned int* flags,
+                                                             int nranks, int stride, int which) {
+    __shared__ double sv;
+    if (threadIdx.x == 0) {
+        double acc = 0.0;
+        for (int r = 0; r < nranks; ++r) acc += __ldcv(slots + r * stride);
+        sv = acc;
+    }
+    if (threadIdx.x < nranks) flags[threadIdx.x] = 0u;
+    __syncthreads();
+    if (st->stop) return;
+    if (which == 1) cg_scalars_after_pAp(st, sv);
+    else cg_scalars_after_rr(st, sv);
 }
 
 // The block sweep: the deferred updates of one block, for every shifted system that was active when the block began.

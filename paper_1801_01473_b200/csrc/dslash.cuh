@@ -51,6 +51,11 @@
 #ifndef DS_BLOCK
 #define DS_BLOCK 128
 #endif
+// 1: K1 / K2 of the whole-lattice path write block partials only, and a one-block kernel after each sums them and runs
+// the scalar step; 0: the block that finishes last does both (fence + atomic ticket in every block)
+#ifndef LQCD_SPLIT_REDUCE
+#define LQCD_SPLIT_REDUCE 1
+#endif
 #ifndef DS_MINB
 #define DS_MINB 4
 #endif
@@ -300,6 +305,8 @@ struct DslashArgs {
     const T* Th_lo;          // halo (U1): their U(1) angles, [parity of origin][face]
     int k0a, na, k0b, nsites;    // thread idx < na: site k0a+idx; else site k0b+(idx-na); nsites in all
     int part_off;            // EPI 4,5: first slot of this launch in `partials`
+    unsigned int *clear0, *clear1;   // not NULL (border launch, peer-memory transport): the arrival words of the halos
+                             // this launch consumes, cleared for their next use (p2p.cuh)
 };
 
 // registers: double needs ~126 (4 blocks of 128 threads per SM); single fits 6 blocks
@@ -486,6 +493,10 @@ template <typename T, int RECON, int EPI, int U1, int SLAB = 0>
 __global__ void __launch_bounds__(DS_BLOCK, (DsOcc<T, EPI>::minb)) dslash_kernel(const DslashArgs<T> A) {
     constexpr bool FLY = (EPI == 4);
     static_assert(EPI == 0 || EPI == 2 || EPI == 4 || EPI == 5, "EPI");
+    if (SLAB && A.clear0 && blockIdx.x == 0 && threadIdx.x == 0) {
+        *A.clear0 = 0u;
+        *A.clear1 = 0u;
+    }
     if (A.check_stop && A.st->stop) return;      // iterations launched beyond the one that converged
     const Geom& g = A.g;
     const int kraw = blockIdx.x * DS_BLOCK + threadIdx.x;
@@ -550,9 +561,10 @@ __global__ void __launch_bounds__(DS_BLOCK, (DsOcc<T, EPI>::minb)) dslash_kernel
     __shared__ double red[32];
     __shared__ int last_flag;
     const double bsum = block_sum<DS_BLOCK>(dot, red);
-    if (SLAB) {
-        // a slab's launches (interior, borders) each write their block partials; the sum over blocks, launches and
-        // ranks and the scalar step follow in their own small kernels (sum_partials_kernel, cg_scalar_kernel)
+    if (SLAB || LQCD_SPLIT_REDUCE) {
+        // only the block partial is written here; the sum over blocks (over the launches of a slab's sweep, over the
+        // ranks) and the scalar step follow in one small kernel (cg_reduce_scalar_kernel; slabs: sum_partials_kernel,
+        // the transport's all-reduce, cg_scalar_kernel)
         if (threadIdx.x == 0) A.partials[A.part_off + blockIdx.x] = bsum;
         return;
     }

@@ -28,6 +28,10 @@ thread_local char g_create_error[256] = "";
 constexpr size_t ALIGN = 256;
 inline size_t align_up(size_t b) { return (b + ALIGN - 1) / ALIGN * ALIGN; }
 
+#ifndef SLAB_GRAPH_MAX_VH
+#define SLAB_GRAPH_MAX_VH (1u << 18)      // local sites per parity up to which a slab's CG iteration is replayed from a graph
+#endif
+
 #ifndef LINKS_RESIDENT_MAX
 #define LINKS_RESIDENT_MAX (48u << 20)
 #endif
@@ -117,6 +121,7 @@ struct lqcd_ctx {
     int last_freeze[LQCD_MAX_SHIFTS];
     float last_ms;
     int last_updates;        // reliable updates of the last mixed-precision solve
+    int last_replays;        // CUDA-graph replays of the last solve (0: launched plainly, or the persistent kernel)
     long long launches;
 
     char err[256];
@@ -266,7 +271,13 @@ int ensure_basics(lqcd_ctx* c) {
     if (!c->red && (rc = dev_alloc(c, (void**)&c->red, 2 * sizeof(double)))) return rc;
     if (!c->red_host) CU(cudaMallocHost((void**)&c->red_host, 2 * sizeof(double)));
     if (c->slab) {
-        if (!c->comm_stream) CU(cudaStreamCreateWithFlags(&c->comm_stream, cudaStreamNonBlocking));
+        if (!c->comm_stream) {
+            // highest priority: the blocks of the border launch are few and should not queue behind what is left of
+            // the interior launch (20,000 blocks at 48^4), or they become a tail of their own
+            int lo = 0, hi = 0;
+            CU(cudaDeviceGetStreamPriorityRange(&lo, &hi));
+            CU(cudaStreamCreateWithPriority(&c->comm_stream, cudaStreamNonBlocking, hi));
+        }
         if (!c->ev_pack) CU(cudaEventCreateWithFlags(&c->ev_pack, cudaEventDisableTiming));
         if (!c->ev_halo) CU(cudaEventCreateWithFlags(&c->ev_halo, cudaEventDisableTiming));
     }
@@ -404,7 +415,7 @@ void launch_dslash_slab_k(lqcd_ctx* c, const DslashArgs<T>& a, int grid, cudaStr
 // One operator sweep on a slab (Alg. 1 of the paper): the two faces of the input are packed and
 // sent, the interior time slices are computed meanwhile, the two border slices once the halos have arrived.
 // `a` carries everything but the slab fields; kepi is the kernel's EPI (0, 2: operators; 4, 5: the two launches of the
-// fused CG iteration, which write block partials to c->partials[0 .. *n_part), summed by the caller).
+// fused CG iteration, which write block partials to c->partials[0 .. *n_part): slab_reduce_step follows).
 // The faces that travel are those of `face_v`, or, with face_v2, of face_v + beta face_v2 (K1: p = r + beta p_old,
 // formed by the owner of the sites).
 template <typename T>
@@ -452,6 +463,10 @@ int slab_apply(lqcd_ctx* c, DslashArgs<T>& a, int kepi, const V2<T>* face_v, con
     a.in_lo = recv_lo;
     a.in_hi = recv_hi;
     a.Wt_lo = B.Wt_lo;
+    // interior: t = 1 .. Lt-2; borders: t = 0 and t = Lt-1
+    const int n_int = (int)(vh - 2 * face);
+    const int grid_int = n_int > 0 ? (n_int + DS_BLOCK - 1) / DS_BLOCK : 0;
+    const int grid_bor = (int)((2 * face + DS_BLOCK - 1) / DS_BLOCK);
     int part = 0;
     auto launch = [&](int grid, cudaStream_t stream) {
         a.part_off = part;
@@ -461,19 +476,18 @@ int slab_apply(lqcd_ctx* c, DslashArgs<T>& a, int kepi, const V2<T>* face_v, con
         else launch_dslash_slab_k<T, 5>(c, a, grid, stream);
         part += grid;
     };
-    // interior: t = 1 .. Lt-2
-    const int n_int = (int)(vh - 2 * face);
     if (n_int > 0) {
         a.k0a = (int)face;
         a.na = n_int;
         a.k0b = 0;
         a.nsites = n_int;
-        launch((n_int + DS_BLOCK - 1) / DS_BLOCK, c->stream);
+        launch(grid_int, c->stream);
     }
     // faces in flight on the communication stream; the two border slices (t = 0 and t = Lt-1) follow them on
     // that stream, so they run beside the interior (disjoint outputs and partial slots) instead of after it
     if (p2p) {
-        if (lqcd_p2p::signal_wait(&c->p2p, c->comm_stream)) return fail(c, LQCD_ECOMM, "peer-memory transport: %s", c->p2p.error);
+        if (lqcd_p2p::signal_wait(&c->p2p, c->comm_stream, false)) return fail(c, LQCD_ECOMM, "peer-memory transport: %s", c->p2p.error);
+        lqcd_p2p::clear_words(&c->p2p, &a.clear0, &a.clear1);
     } else if ((rc = comm_exchange(c, send_lo, send_hi, recv_lo, recv_hi, 3 * row))) {
         return rc;
     }
@@ -481,7 +495,7 @@ int slab_apply(lqcd_ctx* c, DslashArgs<T>& a, int kepi, const V2<T>* face_v, con
     a.na = (int)face;
     a.k0b = (int)(vh - face);
     a.nsites = (int)(2 * face);
-    launch((a.nsites + DS_BLOCK - 1) / DS_BLOCK, c->comm_stream);
+    launch(grid_bor, c->comm_stream);
     CU(cudaEventRecord(c->ev_halo, c->comm_stream));
     CU(cudaStreamWaitEvent(c->stream, c->ev_halo, 0));
     CU(cudaGetLastError());
@@ -501,12 +515,22 @@ int slab_dslash(lqcd_ctx* c, int epi, V2<T>* out, const V2<T>* in, int par, cons
     return slab_apply<T>(c, a, epi, in, nullptr, nullptr);
 }
 
-// sum of c->partials[0..n) over this rank's blocks, then over the ranks, then the scalar step `which`
+// sum of c->partials[0..n) over this rank's blocks, then over the ranks, then the scalar step `which`.
+// Peer-memory transport: the kernel that sums the partials stores the rank's sum into every rank's window itself, and
+// the kernel of the scalar step adds the ranks' slots (two kernels and nranks stream waits per scalar product).
 int slab_reduce_step(lqcd_ctx* c, int n, int which, double tol, int check_stop) {
     int rc;
-    sum_partials_kernel<<<1, CG_BLOCK, 0, c->stream>>>(c->partials, n, c->red, c->st_dev, check_stop);
-    if ((rc = comm_allreduce(c))) return rc;
-    cg_scalar_kernel<<<1, 64, 0, c->stream>>>(c->st_dev, c->red, which, tol);
+    if (which != 0 && c->p2p.active && c->comm.user == (void*)&c->p2p) {
+        lqcd_p2p::Transport* t = &c->p2p;
+        sum_partials_kernel<<<1, CG_BLOCK, 0, c->stream>>>(c->partials, n, c->red, c->st_dev, check_stop, lqcd_p2p::reduce_begin(t));
+        if (lqcd_p2p::reduce_wait(t, c->stream)) return fail(c, LQCD_ECOMM, "peer-memory transport: %s", t->error);
+        cg_scalar_slots_kernel<<<1, 64, 0, c->stream>>>(c->st_dev, lqcd_p2p::reduce_slots(t), lqcd_p2p::reduce_flags(t),
+                                                        t->nranks, LQCD_P2P_RED_MAX, which);
+    } else {
+        sum_partials_kernel<<<1, CG_BLOCK, 0, c->stream>>>(c->partials, n, c->red, c->st_dev, check_stop, nullptr);
+        if ((rc = comm_allreduce(c))) return rc;
+        cg_scalar_kernel<<<1, 64, 0, c->stream>>>(c->st_dev, c->red, which, tol);
+    }
     c->launches += 2;
     CU(cudaGetLastError());
     return LQCD_OK;
@@ -533,6 +557,17 @@ void launch_dslash(lqcd_ctx* c, int epi, V2<T>* out, const V2<T>* in, int par, c
     else launch_dslash_t<T, 2>(c, a);
 }
 
+// after K1 (which = 1) / K2 (which = 2) of the whole-lattice path: block partials -> sum -> scalar step, one block
+void launch_reduce_scalar(lqcd_ctx* c, int which) {
+#if LQCD_SPLIT_REDUCE
+    cg_reduce_scalar_kernel<<<1, CG_BLOCK, 0, c->stream>>>(c->st_dev, c->partials, ds_grid(c), which);
+    ++c->launches;
+#else
+    (void)c;
+    (void)which;
+#endif
+}
+
 // The two launches of a fused CG iteration (dslash.cuh, EPI = 4 and 5; cg.cuh has the whole picture).
 //   K1: t = D_oe p with p = r + beta p_old formed at the neighbours; <p,Ap>; a, zeta_i
 //   K2: p, s = c0 p - D_eo t, r_new = r - a s, x_0 += a p at the thread's own site; |r_new|^2; beta, b_i, flags
@@ -552,6 +587,7 @@ void launch_cg_fused(lqcd_ctx* c, const V2<T>* r_in, V2<T>* r_out, V2<T>* p_keep
     a.out = B.t;
     a.par = 1;
     launch_dslash_t<T, 4>(c, a);
+    launch_reduce_scalar(c, 1);
     a.in = B.t;
     a.in2 = nullptr;
     a.out = nullptr;
@@ -563,6 +599,7 @@ void launch_cg_fused(lqcd_ctx* c, const V2<T>* r_in, V2<T>* r_out, V2<T>* p_keep
     a.p_keep = p_keep;
     a.defer_base = defer_base;
     launch_dslash_t<T, 5>(c, a);
+    launch_reduce_scalar(c, 2);
 }
 
 // m >= 2: x_0 of the base system is updated by the block sweep too (CgState::defer_base)
@@ -1044,7 +1081,10 @@ int lqcd_comm_init_p2p(lqcd_ctx* c, const void* handles) {
     ops.exchange = lqcd_p2p::exchange;
     ops.allreduce_sum = lqcd_p2p::allreduce_sum;
     ops.host_staged = 0;
-    ops.graph_safe = 0;          // the sequence numbers of the stream memory operations change from call to call
+    // The stream memory operations can be captured (values are constants, addresses depend on the generation only), and
+    // a captured iteration was run and was correct -- and slower than plain launches at every size tried (one rank, us
+    // per iteration, graph / plain: 16^4 72.0 / 71.9, 32^4 271 / 254, 48^4 1191 / 1170): launched plainly.
+    ops.graph_safe = 0;
     return lqcd_set_comm(c, &ops);
 }
 
@@ -1356,12 +1396,16 @@ int solve(lqcd_ctx* c, const T* b_even, const double* shifts, int nshift, double
     const int ce = check_every(c);
     const bool persistent = use_persistent<T>(c);
     // the legacy default stream cannot be captured: plain launches there
+    // Slabs: a replayed graph does not keep the priority of the communication stream, so the border launches queue
+    // behind the interior again; measured on one rank over NCCL, graph against plain launches, us per iteration:
+    // 16^4 48.9 / 61.6, 32^4 256 / 246, 48^4 1175 / 1167 -- the graph pays only where launches are what limits
     const bool use_graph = !persistent && c->use_graph && c->stream != nullptr && c->stream != cudaStreamLegacy &&
-                           (!c->slab || c->comm.graph_safe);
+                           (!c->slab || (c->comm.graph_safe && c->Vh <= SLAB_GRAPH_MAX_VH));
     if (use_graph && (B.graph_iters != ce || B.graph_block != m)) {
         if ((rc = build_graph<T>(c, ce, rational))) return rc;
     }
     c->flag_host[0] = c->flag_host[1] = 0;
+    c->last_replays = 0;
     bool done = false;
     if (persistent) {
         // one cooperative kernel runs the iterations until the device-side stop (persist.cuh)
@@ -1379,6 +1423,7 @@ int solve(lqcd_ctx* c, const T* b_even, const double* shifts, int nshift, double
         if (use_graph && nit == ce) {
             CU(cudaGraphLaunch(B.graph_exec, c->stream));
             c->launches += B.graph_launches;
+            ++c->last_replays;
         } else {
             for (int i = 0; i < nit; ++i)
                 if ((rc = launch_cg_iteration<T>(c, i % m))) return rc;
@@ -1716,6 +1761,7 @@ int lqcd_get_stat(const lqcd_ctx* c, int key, int idx, double* out) {
         case LQCD_STAT_GPU_LAUNCHES: *out = (double)c->launches; break;
         case LQCD_STAT_SOLVE_MS: *out = c->last_ms; break;
         case LQCD_STAT_RELIABLE_UPDATES: *out = c->last_updates; break;
+        case LQCD_STAT_GRAPH_REPLAYS: *out = c->last_replays; break;
         default: return LQCD_EINVAL;
     }
     return LQCD_OK;

@@ -30,6 +30,25 @@ struct Geom {
     int t_off, Lt_glob;             // slab mode: this lattice is time slices [t_off, t_off+Lt) of Lt_glob
 };
 
+// Peer-memory transport (p2p.cuh): where the rank's share of a scalar product goes -- one slot and one flag word in
+// every rank's window (its own included).  Lives in device memory, one per generation of the all-reduce.
+#define LQCD_P2P_MAX_RANKS 16
+#define LQCD_P2P_RED_MAX 4          // doubles per all-reduce slot
+struct PeerPush {
+    double* slot[LQCD_P2P_MAX_RANKS];
+    unsigned int* flag[LQCD_P2P_MAX_RANKS];
+    int nranks;
+};
+// value -> every rank's slot, then (system-wide fence) 1 -> every rank's flag; threads 0..nranks-1 of one block
+__device__ __forceinline__ void peer_push(const PeerPush* __restrict__ d, const double value) {
+    const int q = threadIdx.x;
+    if (q < d->nranks) {
+        *(volatile double*)d->slot[q] = value;
+        __threadfence_system();
+        *(volatile unsigned int*)d->flag[q] = 1u;
+    }
+}
+
 #ifndef LQCD_MAX_BLOCK
 #define LQCD_MAX_BLOCK 32           // longest block of iterations whose shift updates are applied in one sweep
 #endif

@@ -6,22 +6,28 @@
 //     buffers ([from rank-1 | from rank+1] x two generations).  The window is exported with cudaIpcGetMemHandle; the
 //     handles travel once over the caller's channel (lqcd_p2p_export / lqcd_comm_init_p2p), and every rank maps every
 //     other rank's window (cudaIpcOpenMemHandle enables peer access over NVLink);
-//   * face exchange of application number s (one counter per rank, the same on all of them): the sender WRITES its
-//     two faces straight into the neighbours' face buffers of generation s&1 -- strided copies or the stores of the
-//     pack kernel, from the vector itself -- then writes s into the neighbours' `arrived` words with a stream memory
-//     operation (cuStreamWriteValue32, ordered after the copies), and waits for its own two `arrived` words to reach s
-//     (cuStreamWaitValue32 on LOCAL memory).  The border launch reads the halo in place, in the window;
+//   * face exchange number s (one counter per rank, the same on all of them), generation g = s&1: the sender WRITES its
+//     two faces straight into the neighbours' face buffers of generation g -- strided copies or the stores of the
+//     pack kernel, from the vector itself -- then sets the neighbours' `arrived[side][g]` words to 1 with a stream
+//     memory operation (cuStreamWriteValue32, ordered after the copies), waits for its own two `arrived[.][g]` words
+//     (cuStreamWaitValue32 on LOCAL memory).  The border launch reads the halo in place, in the window, and clears
+//     the two words;
 //   * no flow control is needed beyond the two generations: a rank that sends face s has received face s-1 from that
-//     neighbour, which the neighbour sent (stream order) after the launch that consumed ITS halo of s-2, the last
-//     tenant of the buffer now being overwritten;
-//   * all-reduce of the scalar products: one kernel of one warp stores this rank's value into slot [generation][rank]
-//     of every rank's window (itself included) and then, after a system-wide fence, the sequence number into their
-//     `red_arrived[rank]` words; nranks stream waits on the local words; one kernel adds the slots in rank order, so
-//     every rank holds the same bits (R8).  The same two-generation argument applies.
+//     neighbour, which the neighbour sent (stream order) after it had cleared its flags of s-2 and launched the
+//     kernel that consumed ITS halo of s-2, the last tenant of the buffer and flag now being overwritten;
+//   * all-reduce of the scalar products, generation g = q&1 of all-reduce number q: the rank's value is stored into
+//     slot [g][rank] of every rank's window (its own included) and then, after a system-wide fence, 1 into their
+//     `red_arrived[g][rank]` words (peer_push: by the one-block kernel that sums the rank's block partials, or by
+//     p2p_push_kernel); nranks stream waits on the local words; one kernel adds the slots in rank order -- every
+//     rank holds the same bits (R8) --, clears the words and runs the scalar step of the CG.  The same
+//     two-generation argument applies.
 //
 // Nothing here spins inside a kernel: every wait is a stream memory operation on the waiting rank's own memory, so
 // several ranks may share one GPU (tests) without any kernel of one waiting for a kernel of another.
-// The waits are not captured into CUDA graphs (graph_safe = 0): the sequence numbers change from call to call.
+// Every value written or waited for is the constant 0 or 1 and every address depends only on the generation, so the
+// operations of a CG iteration (two exchanges, two all-reduces: the generations come round) CAN be captured into a
+// CUDA graph; that was built and measured (correct, and slower than plain launches at 16^4, 32^4 and 48^4: a memory
+// operation node costs more than the launch it saves), so the library launches the iteration plainly (graph_safe = 0).
 #ifndef LQCD_P2P_CUH
 #define LQCD_P2P_CUH
 
@@ -31,17 +37,20 @@
 #include <string.h>
 #include <unistd.h>
 
+#include "lqcd_internal.cuh"
+
 namespace lqcd_p2p {
 
-constexpr int MAX_RANKS = 16;
-constexpr int RED_MAX = 4;                 // doubles per all-reduce
-constexpr size_t HDR_BYTES = 2048;
+constexpr int MAX_RANKS = LQCD_P2P_MAX_RANKS;
+constexpr int RED_MAX = LQCD_P2P_RED_MAX;
+constexpr size_t HDR_BYTES = 4096;
 
 struct Header {                            // start of every window
-    unsigned int arrived[2];               // [0]: number of the last exchange whose face from rank-1 is complete; [1]: rank+1
-    unsigned int pad[14];
-    unsigned int red_arrived[MAX_RANKS];   // number of the last all-reduce whose contribution from rank q is complete
+    unsigned int arrived[2][2];            // [side: 0 = from rank-1, 1 = from rank+1][generation]: 1 = that face is complete
+    unsigned int pad[12];
+    unsigned int red_arrived[2][MAX_RANKS];   // [generation][rank]: 1 = that rank's contribution is in its slot
     double red[2][MAX_RANKS][RED_MAX];     // [generation][rank][value]
+    PeerPush push[2];                      // this rank's targets of generation 0 / 1 (addresses as mapped HERE)
 };
 static_assert(sizeof(Header) <= HDR_BYTES, "window header");
 
@@ -64,13 +73,14 @@ struct Transport {
     char* win[MAX_RANKS] = {};             // every rank's window as mapped in this process; win[rank] is mine
     bool opened[MAX_RANKS] = {};           // mapped with cudaIpcOpenMemHandle (to be closed)
     size_t cap = 0;                        // bytes of one face buffer
-    unsigned int seq = 0, rseq = 0;        // exchanges / all-reduces issued so far
+    unsigned int seq = 0, rseq = 0;        // exchanges / all-reduces issued so far (only their parity matters)
     mem_op32_fn wait32 = nullptr, write32 = nullptr;
     const char* error = "";
 
     Header* hdr(int r) const { return (Header*)win[r]; }
+    Header* mine() const { return (Header*)win[rank]; }
     // face buffer of rank r: side 0 = halo below its slab (filled by r-1), 1 = above (filled by r+1)
-    char* face(int r, int side, unsigned int s) const { return win[r] + HDR_BYTES + ((size_t)side * 2 + (s & 1)) * cap; }
+    char* face(int r, int side, unsigned int g) const { return win[r] + HDR_BYTES + ((size_t)side * 2 + (g & 1)) * cap; }
     int dn() const { return (rank + nranks - 1) % nranks; }
     int up() const { return (rank + 1) % nranks; }
 };
@@ -107,10 +117,7 @@ inline int create_window(Transport* t, int rank, int nranks, size_t cap, Blob* o
     }
     t->win[rank] = (char*)w;
     memset(out, 0, sizeof(Blob));
-    if (cudaIpcGetMemHandle(&out->ipc, w) != cudaSuccess) {
-        // a device without IPC support can still run ranks of one process
-        cudaGetLastError();
-    }
+    if (cudaIpcGetMemHandle(&out->ipc, w) != cudaSuccess) cudaGetLastError();   // ranks of one process need no handle
     out->pid = (long long)getpid();
     out->ptr = (unsigned long long)(uintptr_t)w;
     out->cap = t->cap;
@@ -119,7 +126,7 @@ inline int create_window(Transport* t, int rank, int nranks, size_t cap, Blob* o
     return 0;
 }
 
-// map every rank's window
+// map every rank's window; write the push targets of both generations into my header
 inline int connect(Transport* t, const Blob* blobs) {
     if (!t->win[t->rank]) return fail(t, "lqcd_p2p_export first");
     for (int r = 0; r < t->nranks; ++r) {
@@ -142,6 +149,17 @@ inline int connect(Transport* t, const Blob* blobs) {
             t->opened[r] = true;
         }
     }
+    PeerPush push[2];
+    memset(push, 0, sizeof(push));
+    for (int g = 0; g < 2; ++g) {
+        push[g].nranks = t->nranks;
+        for (int r = 0; r < t->nranks; ++r) {
+            push[g].slot[r] = &t->hdr(r)->red[g][t->rank][0];
+            push[g].flag[r] = &t->hdr(r)->red_arrived[g][t->rank];
+        }
+    }
+    if (cudaMemcpy(t->mine()->push, push, sizeof(push), cudaMemcpyHostToDevice) != cudaSuccess)
+        return fail(t, "writing the push targets");
     t->active = true;
     return 0;
 }
@@ -158,30 +176,39 @@ inline void destroy(Transport* t) {
     cudaGetLastError();
 }
 
+inline CUdeviceptr dptr(const void* p) { return (CUdeviceptr)(uintptr_t)p; }
+
 // Where the faces of the NEXT exchange go and arrive: the sender writes its lowest slice to dst_dn and its highest to
 // dst_up (peer memory); recv_lo / recv_hi are this rank's own halo buffers of that exchange.
 struct Slots {
     void *dst_dn, *dst_up, *recv_lo, *recv_hi;
 };
 inline Slots begin(Transport* t) {
-    const unsigned int s = ++t->seq;
+    const unsigned int g = ++t->seq & 1;
     Slots o;
-    o.dst_dn = t->face(t->dn(), 1, s);       // my lowest slice is the halo ABOVE the slab of rank-1
-    o.dst_up = t->face(t->up(), 0, s);       // my highest slice is the halo BELOW the slab of rank+1
-    o.recv_lo = t->face(t->rank, 0, s);
-    o.recv_hi = t->face(t->rank, 1, s);
+    o.dst_dn = t->face(t->dn(), 1, g);       // my lowest slice is the halo ABOVE the slab of rank-1
+    o.dst_up = t->face(t->up(), 0, g);       // my highest slice is the halo BELOW the slab of rank+1
+    o.recv_lo = t->face(t->rank, 0, g);
+    o.recv_hi = t->face(t->rank, 1, g);
     return o;
 }
-// after the writes to dst_dn / dst_up have been enqueued on `stream`: tell the neighbours, wait for mine
-inline int signal_wait(Transport* t, cudaStream_t stream) {
-    const unsigned int s = t->seq;
+// after the writes to dst_dn / dst_up have been enqueued on `stream`: tell the neighbours, wait for mine, clear
+// (clear = false: the kernel that consumes the halos clears the two words itself, clear_words())
+inline void clear_words(Transport* t, unsigned int** w0, unsigned int** w1) {
+    *w0 = &t->mine()->arrived[0][t->seq & 1];
+    *w1 = &t->mine()->arrived[1][t->seq & 1];
+}
+inline int signal_wait(Transport* t, cudaStream_t stream, bool clear = true) {
+    const unsigned int g = t->seq & 1;
     CUstream cs = (CUstream)stream;
-    if (t->write32(cs, (CUdeviceptr)(uintptr_t)&t->hdr(t->dn())->arrived[1], s, CU_STREAM_WRITE_VALUE_DEFAULT) != CUDA_SUCCESS ||
-        t->write32(cs, (CUdeviceptr)(uintptr_t)&t->hdr(t->up())->arrived[0], s, CU_STREAM_WRITE_VALUE_DEFAULT) != CUDA_SUCCESS)
+    unsigned int* mine[2] = {&t->mine()->arrived[0][g], &t->mine()->arrived[1][g]};
+    if (t->write32(cs, dptr(&t->hdr(t->dn())->arrived[1][g]), 1u, CU_STREAM_WRITE_VALUE_DEFAULT) != CUDA_SUCCESS ||
+        t->write32(cs, dptr(&t->hdr(t->up())->arrived[0][g]), 1u, CU_STREAM_WRITE_VALUE_DEFAULT) != CUDA_SUCCESS)
         return fail(t, "cuStreamWriteValue32 on a neighbour's window failed");
-    if (t->wait32(cs, (CUdeviceptr)(uintptr_t)&t->hdr(t->rank)->arrived[0], s, CU_STREAM_WAIT_VALUE_GEQ) != CUDA_SUCCESS ||
-        t->wait32(cs, (CUdeviceptr)(uintptr_t)&t->hdr(t->rank)->arrived[1], s, CU_STREAM_WAIT_VALUE_GEQ) != CUDA_SUCCESS)
-        return fail(t, "cuStreamWaitValue32 failed");
+    for (int side = 0; side < 2; ++side)
+        if (t->wait32(cs, dptr(mine[side]), 1u, CU_STREAM_WAIT_VALUE_GEQ) != CUDA_SUCCESS) return fail(t, "cuStreamWaitValue32 failed");
+    for (int side = 0; clear && side < 2; ++side)
+        if (t->write32(cs, dptr(mine[side]), 0u, CU_STREAM_WRITE_VALUE_DEFAULT) != CUDA_SUCCESS) return fail(t, "cuStreamWriteValue32 failed");
     return 0;
 }
 
@@ -203,27 +230,36 @@ inline int exchange(void* user, const void* send_lo, const void* send_hi, void* 
     return 0;
 }
 
-struct PushArgs {
-    double* slot[MAX_RANKS];
-    unsigned int* flag[MAX_RANKS];
-    int nranks, n;
-    unsigned int seq;
-};
-// thread q: my value into rank q's slot, then (system-wide fence) the sequence number into its flag word
-__global__ void __launch_bounds__(32) p2p_push_kernel(const PushArgs a, const double* __restrict__ value) {
-    const int q = threadIdx.x;
-    if (q >= a.nranks) return;
-    for (int j = 0; j < a.n; ++j) ((volatile double*)a.slot[q])[j] = value[j];
-    __threadfence_system();
-    *(volatile unsigned int*)a.flag[q] = a.seq;
+// ---- all-reduce.  Three steps: push (by the producer of the value, or p2p_push_kernel), wait, sum + clear.
+// reduce_begin opens all-reduce number ++rseq and returns the push targets of its generation (device memory).
+inline const PeerPush* reduce_begin(Transport* t) { return &t->mine()->push[++t->rseq & 1]; }
+inline int reduce_wait(Transport* t, cudaStream_t stream) {
+    const unsigned int g = t->rseq & 1;
+    for (int r = 0; r < t->nranks; ++r)
+        if (t->wait32((CUstream)stream, dptr(&t->mine()->red_arrived[g][r]), 1u, CU_STREAM_WAIT_VALUE_GEQ) != CUDA_SUCCESS)
+            return fail(t, "cuStreamWaitValue32 failed");
+    return 0;
 }
-// out[j] = sum over ranks, in rank order: the same bits on every rank
-__global__ void __launch_bounds__(32) p2p_sum_kernel(const double* slots, int nranks, int n, double* __restrict__ out) {
+inline double* reduce_slots(Transport* t) { return &t->mine()->red[t->rseq & 1][0][0]; }
+inline unsigned int* reduce_flags(Transport* t) { return &t->mine()->red_arrived[t->rseq & 1][0]; }
+
+__global__ void __launch_bounds__(32) p2p_push_kernel(const PeerPush* __restrict__ d, const double* __restrict__ value, int n) {
+    const int q = threadIdx.x;
+    if (q >= d->nranks) return;
+    for (int j = 0; j < n; ++j) ((volatile double*)d->slot[q])[j] = value[j];
+    __threadfence_system();
+    *(volatile unsigned int*)d->flag[q] = 1u;
+}
+// out[j] = sum over ranks, in rank order: the same bits on every rank; the flags are cleared for their next use
+__global__ void __launch_bounds__(32) p2p_sum_kernel(const double* slots, unsigned int* flags, int nranks, int n,
+                                                     double* __restrict__ out) {
     const int j = threadIdx.x;
-    if (j >= n) return;
-    double acc = 0.0;
-    for (int r = 0; r < nranks; ++r) acc += __ldcv(slots + r * RED_MAX + j);
-    out[j] = acc;
+    if (j < n) {
+        double acc = 0.0;
+        for (int r = 0; r < nranks; ++r) acc += __ldcv(slots + r * RED_MAX + j);
+        out[j] = acc;
+    }
+    if (j < nranks) flags[j] = 0u;
 }
 
 inline int allreduce_sum(void* user, double* dev_buf, int n, void* stream) {
@@ -231,20 +267,9 @@ inline int allreduce_sum(void* user, double* dev_buf, int n, void* stream) {
     if (!t->active) return fail(t, "transport not connected");
     if (n < 1 || n > RED_MAX) return fail(t, "all-reduce of more values than a slot holds");
     cudaStream_t s = (cudaStream_t)stream;
-    const unsigned int q = ++t->rseq, g = q & 1;
-    PushArgs a;
-    for (int r = 0; r < t->nranks; ++r) {
-        a.slot[r] = &t->hdr(r)->red[g][t->rank][0];
-        a.flag[r] = &t->hdr(r)->red_arrived[t->rank];
-    }
-    a.nranks = t->nranks;
-    a.n = n;
-    a.seq = q;
-    p2p_push_kernel<<<1, 32, 0, s>>>(a, dev_buf);
-    for (int r = 0; r < t->nranks; ++r)
-        if (t->wait32((CUstream)s, (CUdeviceptr)(uintptr_t)&t->hdr(t->rank)->red_arrived[r], q, CU_STREAM_WAIT_VALUE_GEQ) != CUDA_SUCCESS)
-            return fail(t, "cuStreamWaitValue32 failed");
-    p2p_sum_kernel<<<1, 32, 0, s>>>(&t->hdr(t->rank)->red[g][0][0], t->nranks, n, dev_buf);
+    p2p_push_kernel<<<1, 32, 0, s>>>(reduce_begin(t), dev_buf, n);
+    if (reduce_wait(t, s)) return -1;
+    p2p_sum_kernel<<<1, 32, 0, s>>>(reduce_slots(t), reduce_flags(t), t->nranks, n, dev_buf);
     if (cudaGetLastError() != cudaSuccess) return fail(t, "launch of the all-reduce kernels failed");
     return 0;
 }
