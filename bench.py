@@ -62,7 +62,7 @@ DSLASH_FLOPS = {18: 570, 12: 570 + 8 * 42}
 # dram__bytes_write.sum), keyed by (workload, recon): (read GB, write GB, file under profiles/ that holds them).
 # tests/test_host_logic.py checks these constants against that file.
 NCU_DRAM_GB_PER_LAUNCH = {
-    ("config4_48^4", 18): (3.190604, 0.104271, "profiles/ncu_full_r02.md"),
+    ("config4_48^4", 18): (3.190561, 0.104241, "profiles/ncu_full_r02.md"),
     ("config4_48^4", 12): (2.171204, 0.101689, "profiles/ncu_full_r01.md"),
 }
 
@@ -286,13 +286,13 @@ def ev():
     return torch.cuda.Event(enable_timing=True)
 
 
-def time_dslash(lq, L, recon, reps, warm, links=None, field=None, slab=None):
+def time_dslash(lq, L, recon, reps, warm, links=None, field=None, slab=None, comm="nccl"):
     """ns/site and GB/s of one parity application: reps x (D_oe: b->t, D_eo: t->u) with fixed b
     (never fed back: |D| ~ 2.6 on random links would overflow).  slab = (L_global, rank, nranks): the same on a slab
     context (two face exchanges over NCCL, interior and border launches per application); collective."""
     U = links if links is not None else gen.random_su3_links(L, device="cuda")
     f = field if field is not None else gen.gaussian_field(L, device="cuda")
-    lat = lq.Lattice(L, recon=recon) if slab is None else lq.Lattice(slab[0], recon=recon, slab=slab[1:], comm="nccl")
+    lat = lq.Lattice(L, recon=recon) if slab is None else lq.Lattice(slab[0], recon=recon, slab=slab[1:], comm=comm)
     lat.set_gauge(U)
     b = lat.pack(f, 0)
     t = torch.empty_like(b)
@@ -474,7 +474,7 @@ def run_ours(args, world, rank, local):
         if slab:
             U = gen.random_su3_links_slab(Lg, rank, world, device="cuda")
             f = gen.gaussian_field_slab(Lg, rank, world, device="cuda")
-            lat = lq.Lattice(Lg, mass=mass, recon=recon, slab=(rank, world), comm="nccl")
+            lat = lq.Lattice(Lg, mass=mass, recon=recon, slab=(rank, world), comm=args.slab_comm)
         else:
             U = gen.random_su3_links(L, device="cuda")
             f = gen.gaussian_field(L, device="cuda")
@@ -605,7 +605,7 @@ def run_ours(args, world, rank, local):
                 other = 12 if recon == 18 else 18
                 ds[name][f"recon{other}"] = time_dslash(lq, L, other, reps, 5, U, f)
         if slab:
-            out["dslash_slab"] = time_dslash(lq, L, recon, reps, 5, U, f, slab=(Lg, rank, world))
+            out["dslash_slab"] = time_dslash(lq, L, recon, reps, 5, U, f, slab=(Lg, rank, world), comm=args.slab_comm)
         phase('dslash at workload size done')
         if rank == 0 and not args.quick and not slab:
             out["next_rows"] = time_next_rows(lq, L, mass, shifts, tol, K, W, U, f)
@@ -876,7 +876,8 @@ def main():
     ap.add_argument("--with-slab", action="store_true",
                     help="also run the guarded slab sub-run when N = 1 (it always runs when N > 1)")
     ap.add_argument("--slab-check", action="store_true", help=argparse.SUPPRESS)
-    ap.add_argument("--slab-comm", default="nccl", choices=["nccl", "p2p"], help=argparse.SUPPRESS)
+    ap.add_argument("--slab-comm", default="nccl", choices=["nccl", "p2p"],
+                    help="transport of --parallel slab: the library's NCCL transport or its peer-memory transport")
     ap.add_argument("--plumbing-check", action="store_true", help=argparse.SUPPRESS)
     args = ap.parse_args()
     self_launch(args, sys.argv[1:])

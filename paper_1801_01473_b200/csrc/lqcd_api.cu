@@ -1419,7 +1419,7 @@ int solve(lqcd_ctx* c, const T* b_even, const double* shifts, int nshift, double
         // the batch in which MAX_ITER falls is launched plainly, only as far as the cap: the iterations of a graph
         // replay beyond it would all return at once, at 27 us each (48^4)
         const long left = (long)c->max_iter - batch * ce;
-        const int nit = (left < ce && !c->slab) ? (int)left : ce;
+        const int nit = (left < ce) ? (int)left : ce;       // the same on every rank of a slab decomposition
         if (use_graph && nit == ce) {
             CU(cudaGraphLaunch(B.graph_exec, c->stream));
             c->launches += B.graph_launches;
