@@ -239,8 +239,9 @@ int lqcd_rational_apply_f32(lqcd_ctx* ctx, const float* b_even, double alpha0, c
  * whole lattice.  lqcd_set_u1_phases takes the angles of the slab's own links (4 * V_local) and, like lqcd_set_gauge,
  * needs the transport (the t-links below the slab, and their angles, come from rank-1 once).
  *
- * STATUS: verified on one GPU only (one rank over NCCL with the ring closed on itself; several ranks sharing the GPU
- * through a host-staged transport).  NCCL between two or more GPUs has not been run.
+ * STATUS: verified on one GPU only (one rank with the ring closed on itself, over NCCL and over peer memory; several
+ * ranks sharing the GPU, over peer memory (CUDA IPC) and through a host-staged transport).  Neither NCCL nor the
+ * peer-memory transport has been run between two or more GPUs.
  *
  * A transport must be set before lqcd_set_gauge (which exchanges the t-links of the face once, and runs one all-reduce
  * so that the transport's connections exist before any CUDA graph is captured):
