@@ -290,7 +290,8 @@ int lqcd_comm_init_nccl(lqcd_ctx* ctx, const void* id /*HOST, 128 bytes*/);
  * largest face message: 288 bytes x Lx/2*Ly*Lz) and writes LQCD_P2P_HANDLE_BYTES describing it; the caller gathers
  * the handles of all ranks by any means (e.g. torch.distributed.all_gather_object) and hands every rank the table of
  * all of them, in rank order, through lqcd_comm_init_p2p (not collective: it only maps the windows).  At most 16
- * ranks.  LQCD_ECOMM if a window cannot be mapped (no peer access, other node) or stream memory operations are
+ * ranks.  The window is allocated with cudaMalloc (CUDA IPC exports whole allocations): it is not part of a caller
+ * workspace and is released by lqcd_destroy.  LQCD_ECOMM if a window cannot be mapped (no peer access, other node) or stream memory operations are
  * unavailable.  STATUS: verified on one GPU (one rank; two and four ranks as processes sharing the GPU over CUDA IPC);
  * not run between two or more GPUs. */
 #define LQCD_P2P_HANDLE_BYTES 96

@@ -3,9 +3,11 @@
 // One CG iteration is the two operator launches of dslash.cuh ("scalar products and sums" + the two
 // operators, every sum and scalar product of the base system folded into the operators' own sweeps), plus one sweep
 // over all systems every m iterations:
-//   K1  t = D_oe p with p = r + beta p_old formed at the neighbours;  <p,Ap>  -> a, zeta_new_i   dslash_kernel<.,4>
-//   K2  p, s = (m^2+sigma0) p - D_eo t, r_new = r - a s at the own site;  |r_new|^2
-//       -> beta, b_i, block coefficients, freeze flags, stop flag                                 dslash_kernel<.,5>
+//   K1  t = D_oe p with p = r + beta p_old formed at the neighbours;  block partials of <p,Ap>    dslash_kernel<.,4>
+//       sum -> a, zeta_new_i                                                          cg_reduce_scalar_kernel (1 block)
+//   K2  p, s = (m^2+sigma0) p - D_eo t, r_new = r - a s at the own site;  block partials of |r_new|^2
+//                                                                                                 dslash_kernel<.,5>
+//       sum -> beta, b_i, block coefficients, freeze flags, stop flag                 cg_reduce_scalar_kernel (1 block)
 //   every m-th iteration (and once after the stop), for every system of the block:
 //         x_i += CP_i p_i + sum_l D_il r_l ;  p_i = B_i p_i + sum_l E_il r_l                      cg_flush_kernel
 // K2 writes r_new into a ring of m residual vectors instead of over r, so that the m residuals of a block

@@ -34,13 +34,13 @@
 //           registers at each of the eight neighbours from the residual `in` and the previous direction `in2`.
 //           out = D p (odd sites), and the block partial of  <p, A p> = c0 |p|^2 + |D_oe p|^2  (D_eo = -D_oe^+,
 //           PAPER.md:L80): |out|^2 of the site plus c0/8 |p|^2 of each neighbour (every even site is the
-//           neighbour of exactly eight odd sites).  The last block sums and runs the scalar step (a, zeta_i).
+//           neighbour of exactly eight odd sites).  cg_reduce_scalar_kernel sums and runs the scalar step (a, zeta_i).
 // EPI = 5 : K2.  in = t = D_oe p.  At its own (even) site the thread forms p = r + beta p_old again and stores
 //           it (p_out), s = c0 p - D_eo t (never stored), r_new = r - a s (r_out, the next ring slot),
 //           x_0 += a p (unless the base system is block-deferred like the shifted ones), and the block partial of
-//           |r_new|^2.  The last block sums and runs the scalar step (beta, b_i, freeze and stop flags).
-// With SLAB = 1 the launches of EPI 4, 5 only write their block partials (at partials[part_off + blockIdx.x]); the
-// sum over blocks, launches and ranks and the scalar step follow in their own small kernels, and across the slab
+//           |r_new|^2.  cg_reduce_scalar_kernel sums and runs the scalar step (beta, b_i, freeze and stop flags).
+// With SLAB = 1 a sweep is two launches (interior, borders) that write their partials at partials[part_off + blockIdx.x];
+// the sum over blocks, launches and ranks and the scalar step follow in their own small kernels, and across the slab
 // faces K1 finds p itself in the halo (formed by its owner, slab_pack_p_kernel).
 #ifndef LQCD_DSLASH_CUH
 #define LQCD_DSLASH_CUH
@@ -50,11 +50,6 @@
 
 #ifndef DS_BLOCK
 #define DS_BLOCK 128
-#endif
-// 1: K1 / K2 of the whole-lattice path write block partials only, and a one-block kernel after each sums them and runs
-// the scalar step; 0: the block that finishes last does both (fence + atomic ticket in every block)
-#ifndef LQCD_SPLIT_REDUCE
-#define LQCD_SPLIT_REDUCE 1
 #endif
 #ifndef DS_MINB
 #define DS_MINB 4
@@ -558,22 +553,13 @@ __global__ void __launch_bounds__(DS_BLOCK, (DsOcc<T, EPI>::minb)) dslash_kernel
         }
         return;
     }
+    // Only the block partial is written here; the sum over blocks (over the launches of a slab's sweep, over the ranks)
+    // and the scalar step follow in one small kernel (cg_reduce_scalar_kernel; slabs: sum_partials_kernel, the
+    // transport's all-reduce, cg_scalar_kernel).  Having the block that finishes last do it instead (partial, fence,
+    // atomic ticket in every block) saved the launch and cost 10-12 us per sweep of 20,736 blocks.
     __shared__ double red[32];
-    __shared__ int last_flag;
     const double bsum = block_sum<DS_BLOCK>(dot, red);
-    if (SLAB || LQCD_SPLIT_REDUCE) {
-        // only the block partial is written here; the sum over blocks (over the launches of a slab's sweep, over the
-        // ranks) and the scalar step follow in one small kernel (cg_reduce_scalar_kernel; slabs: sum_partials_kernel,
-        // the transport's all-reduce, cg_scalar_kernel)
-        if (threadIdx.x == 0) A.partials[A.part_off + blockIdx.x] = bsum;
-        return;
-    }
-    if (publish_partial<DS_BLOCK>(bsum, A.partials, &A.st->ticket[EPI == 4 ? 1 : 2], &last_flag)) {
-        const double sum = broadcast0(final_sum<DS_BLOCK>(A.partials, gridDim.x, red), red);
-        if (threadIdx.x == 0) A.st->ticket[EPI == 4 ? 1 : 2] = 0;
-        if (EPI == 4) cg_scalars_after_pAp(A.st, sum);
-        else cg_scalars_after_rr(A.st, sum);
-    }
+    if (threadIdx.x == 0) A.partials[A.part_off + blockIdx.x] = bsum;
 }
 
 // Slab mode, before K1: the two faces (time slices 0 and Lt-1) of p = r + beta p_old, formed by the rank that owns the

@@ -559,13 +559,8 @@ void launch_dslash(lqcd_ctx* c, int epi, V2<T>* out, const V2<T>* in, int par, c
 
 // after K1 (which = 1) / K2 (which = 2) of the whole-lattice path: block partials -> sum -> scalar step, one block
 void launch_reduce_scalar(lqcd_ctx* c, int which) {
-#if LQCD_SPLIT_REDUCE
     cg_reduce_scalar_kernel<<<1, CG_BLOCK, 0, c->stream>>>(c->st_dev, c->partials, ds_grid(c), which);
     ++c->launches;
-#else
-    (void)c;
-    (void)which;
-#endif
 }
 
 // The two launches of a fused CG iteration (dslash.cuh, EPI = 4 and 5; cg.cuh has the whole picture).

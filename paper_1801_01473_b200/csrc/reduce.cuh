@@ -1,9 +1,11 @@
 // reduce.cuh -- deterministic two-stage reductions and the device-side CG scalar recurrences.
 //
 // Stage 1: every block reduces its threads' values with a fixed shuffle tree and writes ONE partial.
-// Stage 2: the block that finishes last (atomic ticket) adds all partials in a fixed order.  No
-// floating-point atomics anywhere, so a solve is bit-reproducible for a given lattice (R8).
-// The same last block then runs the scalar part of the iteration (steps A6 and A9).
+// Stage 2: ONE block adds all partials in a fixed order (final_sum) -- a one-block kernel launched after the sweep
+// (the CG iteration: cg_reduce_scalar_kernel, sum_partials_kernel), or, in the kernels that run once per solve, the
+// block that finishes last (publish_partial: fence + atomic ticket in every block, too dear for 20,000 blocks twice
+// per iteration).  No floating-point atomics anywhere, so a solve is bit-reproducible for a given lattice
+// (R8).  The block that holds the sum then runs the scalar part of the iteration (steps A6 and A9).
 #ifndef LQCD_REDUCE_CUH
 #define LQCD_REDUCE_CUH
 
@@ -81,7 +83,7 @@ __device__ __forceinline__ double broadcast0(double v, double* red) {
 }
 
 // ---- scalar recurrences (SURVEY.md §8(c2) / DESIGN.md R5) ------------------------------------------
-// Run by the block that finished last, ALL its threads calling (blockDim.x >= LQCD_MAX_SHIFTS): thread i
+// Run by the block that holds the sum, ALL its threads calling (blockDim.x >= LQCD_MAX_SHIFTS): thread i
 // carries shift i, thread 0 also the scalars of the base system, so the tail of the kernel costs one chain
 // of dependent operations instead of nshift of them.  Besides the zeta recurrences the threads carry the
 // block coefficients B, E, CP, D of the deferred shift updates (lqcd_internal.cuh, CgState).

@@ -153,6 +153,43 @@ def test_slab_errors():
     lq.lqcd_destroy(whole)
 
 
+def test_peer_memory_transport_errors_and_determinism():
+    """Argument checks of lqcd_p2p_export / lqcd_comm_init_p2p; and the solve over peer memory is bit-identical to the
+    solve over NCCL on one rank (same launches, same order of every sum), launched plainly (no graph replays)."""
+    whole = lq.lqcd_create(4, 4, 4, 4)
+    rc, _ = lq.lqcd_p2p_export(whole)
+    assert rc == lq.LQCD_EINVAL                                    # not a slab context
+    lq.lqcd_destroy(whole)
+    ctx = lq.lqcd_create_slab(4, 4, 4, 8, 0, 2)
+    assert lq.lqcd_comm_init_p2p(ctx, bytes(2 * lq.LQCD_P2P_HANDLE_BYTES)) == lq.LQCD_ECOMM      # nothing exported yet
+    rc, h = lq.lqcd_p2p_export(ctx)
+    assert rc == 0 and len(h) == lq.LQCD_P2P_HANDLE_BYTES
+    assert lq.lqcd_p2p_export(ctx)[0] == lq.LQCD_ECOMM             # one window per context
+    assert lq.lqcd_comm_init_p2p(ctx, h + h) == lq.LQCD_ECOMM      # second entry is not rank 1's
+    assert "rank order" in lq.lqcd_last_error(ctx)
+    lq.lqcd_destroy(ctx)
+
+    L = (4, 6, 4, 8)
+    U, f = make_inputs(L)
+    b_soa, _ = oracle_parity_vector(L, f.numpy(), 0)
+    b = torch.as_tensor(b_soa).cuda()
+    out = {}
+    for comm in ("nccl", "p2p"):
+        lat = lq.Lattice(L, mass=0.05, slab=(0, 1), comm=comm)
+        lat.set_gauge(U.cuda())
+        with torch.cuda.stream(torch.cuda.Stream()):
+            t = lat.doe(b)
+            x, info = lat.mshift_cg(b, SHIFTS, 1e-10)
+        torch.cuda.synchronize()
+        out[comm] = (t, x, info)
+        lat.close()
+    assert torch.equal(out["nccl"][0], out["p2p"][0])
+    assert out["nccl"][2]["iters"] == out["p2p"][2]["iters"] and out["nccl"][2]["freeze_iter"] == out["p2p"][2]["freeze_iter"]
+    for xa, xb in zip(out["nccl"][1], out["p2p"][1]):
+        assert torch.equal(xa, xb)
+    assert out["nccl"][2]["graph_replays"] > 0 and out["p2p"][2]["graph_replays"] == 0
+
+
 def _free_port():
     with socket.socket() as s:
         s.bind(("127.0.0.1", 0))
