@@ -117,10 +117,11 @@ def load_peaks():
 class ClockSampler:
     """Samples SM clock and throttle reasons of one GPU while the timed region runs (pynvml thread)."""
 
-    def __init__(self, index: int, period: float = 0.005):
+    def __init__(self, index: int, period: float = 0.002):
         self.index, self.period = index, period
         self.samples, self.reasons, self.max_mhz = [], set(), None
         self._stop = threading.Event()
+        self._warm = threading.Event()      # set once the first (discarded) poll is through: NVML's first call is slow
         self._thread = None
         try:
             import pynvml
@@ -146,6 +147,12 @@ class ClockSampler:
             getattr(nv, "nvmlClocksEventReasonSwThermalSlowdown", 0x20): "sw_thermal_slowdown",
             getattr(nv, "nvmlClocksEventReasonSwPowerCap", 0x4): "sw_power_cap",
         }
+        try:
+            nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM)
+        except Exception:
+            pass
+        self._warm.set()
+        self._armed.wait()
         while not self._stop.is_set():
             try:
                 self.samples.append(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM))
@@ -161,13 +168,20 @@ class ClockSampler:
             time.sleep(self.period)
 
     def __enter__(self):
+        """Starts the polling thread and returns once it is ready; samples are taken from arm() on."""
+        self._armed = threading.Event()
         if self.nv is not None:
             self._thread = threading.Thread(target=self._run, daemon=True)
             self._thread.start()
+            self._warm.wait(2.0)
         return self
+
+    def arm(self):
+        self._armed.set()
 
     def __exit__(self, *exc):
         self._stop.set()
+        self._armed.set()
         if self._thread is not None:
             self._thread.join()
 
@@ -496,6 +510,7 @@ def run_ours(args, world, rank, local):
         n0 = lat.launches
         e0, e1 = ev(), ev()
         with ClockSampler(local) as clocks:
+            clocks.arm()
             e0.record()
             _, info = lat.mshift_cg(b, shifts, tol, x=x, raise_on_noconv=False)
             e1.record()
