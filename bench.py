@@ -1009,8 +1009,10 @@ def main():
             line[key] = res[key]
     phase("GPU part done")
     if world > 1 or args.with_slab:
-        line["slab"] = guarded_slab_run(args, world, "nccl")
-        line["slab_p2p"] = guarded_slab_run(args, world, "p2p")
+        # a sub-run takes ~30 s including start-up; the limits keep a hang from eating the time the driver allows the
+        # whole bench (the headline line is printed after them)
+        line["slab"] = guarded_slab_run(args, world, "nccl", timeout_s=300.0)
+        line["slab_p2p"] = guarded_slab_run(args, world, "p2p", timeout_s=180.0)
         phase("slab sub-runs done")
     if not args.quick and world == 1:
         s_iter, cores, sample, _ = run_oracle(args.workload, budget_s=args.cpu_budget, steps=None)
