@@ -25,6 +25,9 @@
 //          one or two ranges of sites, so that the interior (t = 1..Lt-2, no halo needed) runs while the faces
 //          are in flight and the two border slices afterwards (Alg. 1).
 //
+// SLAB = 2 : the interior launch of a slab: the same site range and global time coordinate as SLAB = 1, but no hop
+//          crosses a face, so the hops are those of the whole-lattice kernel (no halo pointers, no runtime strides).
+//
 // EPI = 0 : out = D in
 // EPI = 2 : out = coef*pv - D in  (the paper's separate zaxpy kernel, fused into the D_eo epilogue)
 //
@@ -377,7 +380,8 @@ __device__ __forceinline__ void dslash_hops(const DslashArgs<T>& A, const int pa
     HOP_B(1, kyb, my);
     HOP_F(2, kzf, mz);
     HOP_B(2, kzb, mz);
-    if (!SLAB) {
+    if (SLAB != 1) {
+        // whole lattice, or the interior launch of a slab (SLAB == 2: t = 1 .. Lt-2, no hop leaves the slab)
         HOP_F(3, ktf, mtf);
         HOP_B(3, ktb, mtb);
     } else {

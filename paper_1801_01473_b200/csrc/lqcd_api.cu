@@ -398,18 +398,24 @@ int ensure_halo(lqcd_ctx* c) {
     return LQCD_OK;
 }
 
-template <typename T, int EPI, int U1>
+// SLAB = 2: the interior launch (no hop leaves the slab); SLAB = 1: the border slices (halo buffers on the t-hops)
+template <typename T, int EPI, int U1, int SLAB>
 void launch_dslash_slab_u(lqcd_ctx* c, const DslashArgs<T>& a, int grid, cudaStream_t stream) {
     if (bufs<T>(c).recon_stored == 12)
-        dslash_kernel<T, 12, EPI, U1, 1><<<grid, DS_BLOCK, 0, stream>>>(a);
+        dslash_kernel<T, 12, EPI, U1, SLAB><<<grid, DS_BLOCK, 0, stream>>>(a);
     else
-        dslash_kernel<T, 18, EPI, U1, 1><<<grid, DS_BLOCK, 0, stream>>>(a);
+        dslash_kernel<T, 18, EPI, U1, SLAB><<<grid, DS_BLOCK, 0, stream>>>(a);
     ++c->launches;
 }
 template <typename T, int EPI>
-void launch_dslash_slab_k(lqcd_ctx* c, const DslashArgs<T>& a, int grid, cudaStream_t stream) {
-    if (c->u1_on) launch_dslash_slab_u<T, EPI, 1>(c, a, grid, stream);
-    else launch_dslash_slab_u<T, EPI, 0>(c, a, grid, stream);
+void launch_dslash_slab_k(lqcd_ctx* c, const DslashArgs<T>& a, int grid, cudaStream_t stream, bool interior) {
+    if (interior) {
+        if (c->u1_on) launch_dslash_slab_u<T, EPI, 1, 2>(c, a, grid, stream);
+        else launch_dslash_slab_u<T, EPI, 0, 2>(c, a, grid, stream);
+    } else {
+        if (c->u1_on) launch_dslash_slab_u<T, EPI, 1, 1>(c, a, grid, stream);
+        else launch_dslash_slab_u<T, EPI, 0, 1>(c, a, grid, stream);
+    }
 }
 
 // One operator sweep on a slab (Alg. 1 of the paper): the two faces of the input are packed and
@@ -463,17 +469,18 @@ int slab_apply(lqcd_ctx* c, DslashArgs<T>& a, int kepi, const V2<T>* face_v, con
     a.in_lo = recv_lo;
     a.in_hi = recv_hi;
     a.Wt_lo = B.Wt_lo;
+    a.clear0 = a.clear1 = nullptr;      // set for the border launch only (peer-memory transport)
     // interior: t = 1 .. Lt-2; borders: t = 0 and t = Lt-1
     const int n_int = (int)(vh - 2 * face);
     const int grid_int = n_int > 0 ? (n_int + DS_BLOCK - 1) / DS_BLOCK : 0;
     const int grid_bor = (int)((2 * face + DS_BLOCK - 1) / DS_BLOCK);
     int part = 0;
-    auto launch = [&](int grid, cudaStream_t stream) {
+    auto launch = [&](int grid, cudaStream_t stream, bool interior) {
         a.part_off = part;
-        if (kepi == 0) launch_dslash_slab_k<T, 0>(c, a, grid, stream);
-        else if (kepi == 2) launch_dslash_slab_k<T, 2>(c, a, grid, stream);
-        else if (kepi == 4) launch_dslash_slab_k<T, 4>(c, a, grid, stream);
-        else launch_dslash_slab_k<T, 5>(c, a, grid, stream);
+        if (kepi == 0) launch_dslash_slab_k<T, 0>(c, a, grid, stream, interior);
+        else if (kepi == 2) launch_dslash_slab_k<T, 2>(c, a, grid, stream, interior);
+        else if (kepi == 4) launch_dslash_slab_k<T, 4>(c, a, grid, stream, interior);
+        else launch_dslash_slab_k<T, 5>(c, a, grid, stream, interior);
         part += grid;
     };
     if (n_int > 0) {
@@ -481,7 +488,7 @@ int slab_apply(lqcd_ctx* c, DslashArgs<T>& a, int kepi, const V2<T>* face_v, con
         a.na = n_int;
         a.k0b = 0;
         a.nsites = n_int;
-        launch(grid_int, c->stream);
+        launch(grid_int, c->stream, true);
     }
     // faces in flight on the communication stream; the two border slices (t = 0 and t = Lt-1) follow them on
     // that stream, so they run beside the interior (disjoint outputs and partial slots) instead of after it
@@ -495,7 +502,7 @@ int slab_apply(lqcd_ctx* c, DslashArgs<T>& a, int kepi, const V2<T>* face_v, con
     a.na = (int)face;
     a.k0b = (int)(vh - face);
     a.nsites = (int)(2 * face);
-    launch(grid_bor, c->comm_stream);
+    launch(grid_bor, c->comm_stream, false);
     CU(cudaEventRecord(c->ev_halo, c->comm_stream));
     CU(cudaStreamWaitEvent(c->stream, c->ev_halo, 0));
     CU(cudaGetLastError());
