@@ -6,8 +6,9 @@ test_gpu_u1.py, test_gpu_f32.py, test_gpu_parity.py (rational sum), test_gpu_sla
   * NEXT-2  single precision: 20 iterations of the multi-shift CG at a fixed count against the fp64 oracle fed the
             float-rounded links and source (PAPER.md:L147, L282); tolerance as in test_gpu_f32.py;
   * NEXT-1  rational sum accumulated in the solve, 20 iterations at a fixed count (PAPER.md:L82, L86-L89);
-  * NEXT-3  the slab operator on one rank (ring closed on itself over NCCL): bit-identical to the whole-lattice
-            kernel, and within 1e-12 of the oracle (PAPER.md:L108-L118);
+  * NEXT-3  one rank of the slab path (ring closed on itself, over NCCL and over peer memory): the operator
+            bit-identical to the whole-lattice kernel and within 1e-12 of the oracle, 20 CG iterations at a fixed
+            count against the oracle (PAPER.md:L108-L118);
   * NEXT-2  mixed precision, one system at 32^4 to tol 1e-10: the TRUE residual recomputed by the oracle's operator.
 
 The inputs are drawn once on the GPU (module fixture); the same bytes go to the oracle."""
@@ -92,22 +93,44 @@ def test_rational_apply_fixed_count_48(lq, big):
     lat.close()
 
 
-def test_slab_one_rank_48(lq, big):
-    L = big.L
+@pytest.mark.parametrize("comm", ["nccl", "p2p"])
+def test_slab_one_rank_48(lq, big, comm):
+    """One rank of the slab path at the size bench.py times it, over either transport: the operator bit-identical to
+    the whole-lattice kernel and within 1e-12 of the oracle; 20 iterations of the fused CG iteration on the slab (p
+    faces formed by their owner, interior + border launches, reductions through the transport) at a fixed count
+    against the oracle, <= 1e-11 as on the whole lattice."""
+    L, cfg, n_it = big.L, big.cfg, 20
     whole = lq.Lattice(L)
     whole.set_gauge(big.U)
-    slab = lq.Lattice(L, slab=(0, 1), comm="nccl")
+    slab = lq.Lattice(L, mass=cfg["mass"], slab=(0, 1), comm=comm)
     slab.set_gauge(big.U)
+    slab.set_option(lq.LQCD_OPT_MAX_ITER, n_it)
     with torch.cuda.stream(torch.cuda.Stream()):
         t0, t1 = whole.doe(big.b), slab.doe(big.b)
         u0, u1 = whole.deo(t0), slab.deo(t1)
+        x, info = slab.mshift_cg(big.b, cfg["shifts"], 1e-30, raise_on_noconv=False)
     torch.cuda.synchronize()
     assert torch.equal(t0, t1) and torch.equal(u0, u1)
+    whole.close()
     t_ref = oracle.doe(L, big.Uh, big.b_aos)
     assert rel_l2(soa_gpu_to_aos(t1), t_ref) <= TOL_D
     assert rel_l2(soa_gpu_to_aos(u1), oracle.deo(L, big.Uh, t_ref)) <= TOL_D
-    whole.close()
+    del t0, t1, u0, u1
+    x_ref, info_ref = _oracle_cg20(big)
+    assert info["iters"] == n_it == info_ref["iters"]
+    assert max(rel_l2(soa_gpu_to_aos(x[i]), x_ref[i]) for i in range(len(cfg["shifts"]))) <= 1e-11
     slab.close()
+
+
+_CG20 = {}
+
+
+def _oracle_cg20(big):
+    """20 iterations of the oracle's multi-shift CG on config 4 at a fixed count (computed once per module)"""
+    if "r" not in _CG20:
+        cfg = big.cfg
+        _CG20["r"] = oracle.mshift_cg(big.L, big.Uh, cfg["mass"], big.b_aos, cfg["shifts"], 1e-30, max_iter=20)
+    return _CG20["r"]
 
 
 def test_f32_cg_fixed_count_48(lq, big):
