@@ -355,8 +355,9 @@ def read_stream_gbs(nbytes: int, reps: int = 10):
 
 def time_small(lq, peak):
     """The small-lattice regime (SURVEY.md §7 "Small lattices are launch-bound", BASELINE config 2): the whole 16^4
-    solve, and the same 8 shifts at 32^4 (400 iterations, then the whole solve).  At 16^4 links (37.7 MB) and
-    vectors live in L2, so the rate is quoted against an L2 read stream measured here, not against HBM."""
+    solve, and the same 8 shifts at 32^4 (400 iterations, then the whole solve).  At 16^4 the links (37.7 MB) and
+    part of the vectors are served by L2, so the rate is quoted against an L2 read stream measured here, not against
+    HBM.  `driver` says which of the two drivers of the iteration the library chose."""
     cfg = gen.CONFIGS["config2_16^4"]
     out = {"l2_read_stream_gbs_40MB": read_stream_gbs(40 << 20, reps=20)}
     for name, L in (("16x16x16x16", cfg["L"]), ("32x32x32x32", (32, 32, 32, 32))):
@@ -371,7 +372,9 @@ def time_small(lq, peak):
         lat.set_option(lq.LQCD_OPT_MAX_ITER, 400)
         _, first = lat.mshift_cg(b, cfg["shifts"], cfg["tol"], x=x, raise_on_noconv=False)
         lat.set_option(lq.LQCD_OPT_MAX_ITER, 100000)
+        n0 = lat.launches
         _, full = lat.mshift_cg(b, cfg["shifts"], cfg["tol"], x=x, raise_on_noconv=False)
+        n_launch = lat.launches - n0
         moved = cg_dram_bytes(full["freeze_iter"], full["iters"], m, 18) * lat.Vh
         gbs = moved / (full["solve_ms"] * 1e6)
         out[name] = {"iters": full["iters"], "status": full["status"], "rel_res": full["rel_res"],
@@ -380,7 +383,9 @@ def time_small(lq, peak):
                      "solve_s": full["solve_ms"] * 1e-3, "freeze_iter": full["freeze_iter"],
                      "gbs_moved": gbs, "frac_of_hbm_peak": gbs / peak,
                      "frac_of_l2_read_stream": gbs / out["l2_read_stream_gbs_40MB"],
-                     "launches_per_iter": 2 + 1.0 / m}
+                     "launches_per_iter": n_launch / max(full["iters"], 1),
+                     "driver": ("CUDA graph of 4 launches per iteration" if full.get("graph_replays") else
+                                "one persistent cooperative kernel" if n_launch < 8 else "plain launches")}
         lat.close()
         del U, f, x, b
     out["note"] = ("config 2 (16^4, m=0.01, 8 shifts, tol 1e-10) whole solve, and the same at 32^4; gbs_moved = bytes the "

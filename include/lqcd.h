@@ -88,10 +88,12 @@ typedef struct lqcd_ctx lqcd_ctx;
                                        iteration counts, x_i equal up to rounding.  m = 1: every iteration.
                                        CHECK_EVERY is rounded up to a multiple of m.  lqcd_get_option returns the
                                        value in force.                                                         */
-#define LQCD_OPT_PERSISTENT      8  /* -1 (default): lattices whose stored links stay in L2 (e.g. 16^4) are solved by ONE
+#define LQCD_OPT_PERSISTENT      8  /* -1 (default): lattices whose stored links and solver vectors stay in L2 (links
+                                       up to 32 MB: e.g. 16^4 with two-row links, 12^4) are solved by ONE
                                        cooperative kernel that runs all iterations with grid-wide barriers between the
-                                       sweeps (no launch gaps, no host polling); larger ones by two launches per
-                                       iteration replayed as a CUDA graph.  0: never, 1: always the persistent kernel.
+                                       sweeps (no launch gaps, no host polling); larger ones by two operator launches
+                                       (+ two one-block kernels) per iteration replayed as a CUDA graph.
+                                       0: never, 1: always the persistent kernel.
                                        Same arithmetic per site; the scalar products are added over a different grid,
                                        so results agree to rounding.  Whole-lattice contexts only.            */
 #define LQCD_PREC_F64 1

@@ -709,12 +709,18 @@ int launch_persistent(lqcd_ctx* c) {
 }
 
 // The persistent solver pays when the iteration is bound by launch gaps and kernel tails rather than by bandwidth:
-// lattices whose links stay in L2 (links_resident).  LQCD_OPT_PERSISTENT overrides.
+// lattices whose links AND solver vectors stay in L2.  Measured at 16^4, whole config-2 solve, us per iteration,
+// persistent / launch path (four launches per iteration in a graph): two-row links (25 MB) 14.3 / 18.6, 18-real links
+// (38 MB: with the residual ring and the x_i, p_i the working set no longer fits) 20.0 / 19.5.  Hence the bound on the
+// stored links below.  LQCD_OPT_PERSISTENT overrides.
+#ifndef PERSIST_LINKS_MAX
+#define PERSIST_LINKS_MAX (32u << 20)
+#endif
 template <typename T>
 bool use_persistent(const lqcd_ctx* c) {
     if (c->slab || c->persistent_opt == 0) return false;
     if (!c->coop_launch || block_len(c) > PS_MAX_BLOCK) return false;
-    return c->persistent_opt == 1 || links_resident<T>(c);
+    return c->persistent_opt == 1 || links_bytes<T>(c, bufs_c<T>(c).recon_stored) <= PERSIST_LINKS_MAX;
 }
 
 // the host looks at the stop flag every this many iterations: a whole number of blocks
