@@ -34,6 +34,7 @@
 #include <cuda.h>
 #include <cuda_runtime.h>
 #include <stdint.h>
+#include <stdlib.h>
 #include <string.h>
 #include <unistd.h>
 
@@ -75,6 +76,7 @@ struct Transport {
     size_t cap = 0;                        // bytes of one face buffer
     unsigned int seq = 0, rseq = 0;        // exchanges / all-reduces issued so far (only their parity matters)
     mem_op32_fn wait32 = nullptr, write32 = nullptr;
+    bool kernel_signal = false;            // remote arrival words are set by a one-thread kernel, not by cuStreamWriteValue32
     const char* error = "";
 
     Header* hdr(int r) const { return (Header*)win[r]; }
@@ -107,6 +109,8 @@ inline int create_window(Transport* t, int rank, int nranks, size_t cap, Blob* o
     t->write32 = (mem_op32_fn)fn;
     t->rank = rank;
     t->nranks = nranks;
+    const char* ks = getenv("LQCD_P2P_KERNEL_SIGNAL");       // tests: take the fall-back of signal_wait from the start
+    t->kernel_signal = ks && ks[0] == '1';
     t->cap = (cap + 255) / 256 * 256;
     if (cudaGetDevice(&t->device) != cudaSuccess) return fail(t, "cudaGetDevice");
     void* w = nullptr;
@@ -198,13 +202,29 @@ inline void clear_words(Transport* t, unsigned int** w0, unsigned int** w1) {
     *w0 = &t->mine()->arrived[0][t->seq & 1];
     *w1 = &t->mine()->arrived[1][t->seq & 1];
 }
+// the two arrival words of a face exchange, set from a kernel: the fall-back when the driver refuses a stream memory
+// operation on a peer-mapped address (stores from kernels are what peer access is for)
+__global__ void p2p_signal_kernel(unsigned int* a, unsigned int* b) {
+    __threadfence_system();
+    *(volatile unsigned int*)a = 1u;
+    *(volatile unsigned int*)b = 1u;
+}
 inline int signal_wait(Transport* t, cudaStream_t stream, bool clear = true) {
     const unsigned int g = t->seq & 1;
     CUstream cs = (CUstream)stream;
     unsigned int* mine[2] = {&t->mine()->arrived[0][g], &t->mine()->arrived[1][g]};
-    if (t->write32(cs, dptr(&t->hdr(t->dn())->arrived[1][g]), 1u, CU_STREAM_WRITE_VALUE_DEFAULT) != CUDA_SUCCESS ||
-        t->write32(cs, dptr(&t->hdr(t->up())->arrived[0][g]), 1u, CU_STREAM_WRITE_VALUE_DEFAULT) != CUDA_SUCCESS)
+    unsigned int* dn = &t->hdr(t->dn())->arrived[1][g];
+    unsigned int* up = &t->hdr(t->up())->arrived[0][g];
+    if (!t->kernel_signal && t->write32(cs, dptr(dn), 1u, CU_STREAM_WRITE_VALUE_DEFAULT) != CUDA_SUCCESS) {
+        cudaGetLastError();
+        t->kernel_signal = true;               // nothing has been signalled yet: both words go by kernel from now on
+    }
+    if (t->kernel_signal) {
+        p2p_signal_kernel<<<1, 1, 0, stream>>>(dn, up);
+        if (cudaGetLastError() != cudaSuccess) return fail(t, "signalling a neighbour's window failed");
+    } else if (t->write32(cs, dptr(up), 1u, CU_STREAM_WRITE_VALUE_DEFAULT) != CUDA_SUCCESS) {
         return fail(t, "cuStreamWriteValue32 on a neighbour's window failed");
+    }
     for (int side = 0; side < 2; ++side)
         if (t->wait32(cs, dptr(mine[side]), 1u, CU_STREAM_WAIT_VALUE_GEQ) != CUDA_SUCCESS) return fail(t, "cuStreamWaitValue32 failed");
     for (int side = 0; clear && side < 2; ++side)

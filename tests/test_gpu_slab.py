@@ -153,6 +153,28 @@ def test_slab_errors():
     lq.lqcd_destroy(whole)
 
 
+def test_peer_memory_kernel_signal_fallback(monkeypatch):
+    """The arrival words of a face set by a one-thread kernel instead of cuStreamWriteValue32 (what the transport falls
+    back to when the driver refuses a stream memory operation on a peer-mapped address): same results, bit for bit."""
+    L = (4, 4, 6, 8)
+    U, f = make_inputs(L)
+    b_soa, _ = oracle_parity_vector(L, f.numpy(), 0)
+    b = torch.as_tensor(b_soa).cuda()
+    out = []
+    for flag in ("0", "1"):
+        monkeypatch.setenv("LQCD_P2P_KERNEL_SIGNAL", flag)
+        lat = lq.Lattice(L, mass=0.05, slab=(0, 1), comm="p2p")
+        lat.set_gauge(U.cuda())
+        with torch.cuda.stream(torch.cuda.Stream()):
+            t = lat.doe(b)
+            x, info = lat.mshift_cg(b, SHIFTS, 1e-10)
+        torch.cuda.synchronize()
+        out.append((t, x, info["iters"]))
+        lat.close()
+    assert torch.equal(out[0][0], out[1][0]) and out[0][2] == out[1][2]
+    assert all(torch.equal(a, c) for a, c in zip(out[0][1], out[1][1]))
+
+
 def test_peer_memory_transport_errors_and_determinism():
     """Argument checks of lqcd_p2p_export / lqcd_comm_init_p2p; and the solve over peer memory is bit-identical to the
     solve over NCCL on one rank (same launches, same order of every sum), launched plainly (no graph replays)."""
