@@ -16,8 +16,8 @@
 //
 // Every block carries the few scalars the sweeps need (rr, a, beta, iteration count, stop) redundantly in registers
 // -- same operands, same operations, hence the same bits in every block.  The recurrences of the shifted systems,
-// the block coefficients, freeze flags and statistics are advanced on the device state exactly as the last block of
-// a launch does on the multi-launch path (same functions), by ONE EXTRA BLOCK that owns no sites: its scalar step
+// the block coefficients, freeze flags and statistics are advanced on the device state exactly as the one-block
+// kernels do on the multi-launch path (same functions), by ONE EXTRA BLOCK that owns no sites: its scalar step
 // (a few dependent round trips to L2, ~2.5 us) runs while the other blocks are in the next sweep, so it is off the
 // critical path (measured at 16^4: with block 0 doing it on top of its sites every barrier waited for it and the
 // iteration took 22 us, no better than two launches).  No host round trip until the solve is over.
