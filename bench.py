@@ -384,7 +384,7 @@ def time_small(lq, peak):
                      "gbs_moved": gbs, "frac_of_hbm_peak": gbs / peak,
                      "frac_of_l2_read_stream": gbs / out["l2_read_stream_gbs_40MB"],
                      "launches_per_iter": n_launch / max(full["iters"], 1),
-                     "driver": ("CUDA graph of 4 launches per iteration" if full.get("graph_replays") else
+                     "driver": ("CUDA graph of the iteration's launches" if full.get("graph_replays") else
                                 "one persistent cooperative kernel" if n_launch < 8 else "plain launches")}
         lat.close()
         del U, f, x, b

@@ -89,10 +89,12 @@ typedef struct lqcd_ctx lqcd_ctx;
                                        CHECK_EVERY is rounded up to a multiple of m.  lqcd_get_option returns the
                                        value in force.                                                         */
 #define LQCD_OPT_PERSISTENT      8  /* -1 (default): lattices whose stored links and solver vectors stay in L2 (links
-                                       up to 32 MB: e.g. 16^4 with two-row links, 12^4) are solved by ONE
-                                       cooperative kernel that runs all iterations with grid-wide barriers between the
-                                       sweeps (no launch gaps, no host polling); larger ones by two operator launches
-                                       (+ two one-block kernels) per iteration replayed as a CUDA graph.
+                                       up to 32 MB) and that give most SMs a block of one site per thread (e.g. 16^4
+                                       with two-row links) are solved by ONE cooperative kernel that runs all
+                                       iterations with grid-wide barriers between the sweeps (no launch gaps, no
+                                       host polling); all others by two operator launches per iteration (+ two
+                                       one-block kernels, which small lattices fold into the launches) replayed as
+                                       a CUDA graph.
                                        0: never, 1: always the persistent kernel.
                                        Same arithmetic per site; the scalar products are added over a different grid,
                                        so results agree to rounding.  Whole-lattice contexts only.            */

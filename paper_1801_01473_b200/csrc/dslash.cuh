@@ -303,6 +303,10 @@ struct DslashArgs {
     const T* Th_lo;          // halo (U1): their U(1) angles, [parity of origin][face]
     int k0a, na, k0b, nsites;    // thread idx < na: site k0a+idx; else site k0b+(idx-na); nsites in all
     int part_off;            // EPI 4,5: first slot of this launch in `partials`
+    // FS == 1 only (small lattices: the scalar step rides in the next sweep instead of a launch of its own)
+    const double* red_in;    // block partials of the PREVIOUS sweep (K1: those of K2, K2: those of K1), red_n of them
+    int red_n;
+    int pending;             // K1: 1 = the scalar step after K2 of the previous iteration has not been run yet
     unsigned int *clear0, *clear1;   // not NULL (border launch, peer-memory transport): the arrival words of the halos
                              // this launch consumes, cleared for their next use (p2p.cuh)
 };
@@ -472,14 +476,14 @@ __device__ __forceinline__ double k2_finish(const K2Coef<T>& C, const size_t vh,
 }
 
 template <typename T>
-__device__ __forceinline__ K2Coef<T> k2_coef_from_state(const CgState* st, V2<T>* p_out, V2<T>* r_out, V2<T>* p_keep,
-                                                        int defer_base) {
+__device__ __forceinline__ K2Coef<T> k2_coef_from_state(const CgState* st, const double a, V2<T>* p_out, V2<T>* r_out,
+                                                        V2<T>* p_keep, int defer_base) {
     K2Coef<T> C;
     const int rational = st->rational, i0 = st->i0;
     C.beta = (T)st->b_prev;
-    C.a = (T)st->a;
+    C.a = (T)a;
     C.c0 = (T)st->c0;
-    C.ax = (T)(rational ? st->alpha[i0] * st->a : st->a);
+    C.ax = (T)(rational ? st->alpha[i0] * a : a);
     C.xp = (V2<T>*)(rational ? st->y : st->x[i0]);
     C.p_out = p_out;
     C.r_out = r_out;
@@ -488,15 +492,47 @@ __device__ __forceinline__ K2Coef<T> k2_coef_from_state(const CgState* st, V2<T>
     return C;
 }
 
-template <typename T, int RECON, int EPI, int U1, int SLAB = 0>
+// FS = 1 (EPI 4, 5 on small whole lattices, where a one-block kernel per scalar step is a third of the iteration): the
+// launch has one block more than the sites need.  EVERY block first adds the block partials of the previous sweep in
+// the same fixed order (a few hundred numbers from L2; the same bits in every block) and takes from the sum the one
+// scalar it needs -- K2: a = |r|^2 / <p,Ap>;  K1: beta = |r_new|^2 / |r|^2 and the stop decision -- while the extra block
+// runs the scalar step proper on the device state (zeta_i, block coefficients, freeze flags) for everybody else's
+// later use.  The fields the sweeping blocks read (rr, b_prev in K2; rr_keep, iter_keep in K1) are not written by the
+// scalar step that runs beside them.  The step after K2 of the last iteration of a block (and of a batch) is run by
+// cg_reduce_scalar_kernel before the block sweep; K1 of the next iteration is then launched with pending = 0.
+template <typename T, int RECON, int EPI, int U1, int SLAB = 0, int FS = 0>
 __global__ void __launch_bounds__(DS_BLOCK, (DsOcc<T, EPI>::minb)) dslash_kernel(const DslashArgs<T> A) {
     constexpr bool FLY = (EPI == 4);
     static_assert(EPI == 0 || EPI == 2 || EPI == 4 || EPI == 5, "EPI");
+    static_assert(!FS || (!SLAB && (EPI == 4 || EPI == 5)), "FS");
     if (SLAB && A.clear0 && blockIdx.x == 0 && threadIdx.x == 0) {
         *A.clear0 = 0u;
         *A.clear1 = 0u;
     }
     if (A.check_stop && A.st->stop) return;      // iterations launched beyond the one that converged
+    double a_fs = 0.0, beta_fs = 0.0;
+    if (FS) {
+        __shared__ double redf[32];
+        const bool have = (EPI == 5) || A.pending;
+        double sum_in = 0.0;
+        if (have) sum_in = broadcast0(final_sum<DS_BLOCK>(A.red_in, A.red_n, redf), redf);
+        if (blockIdx.x == gridDim.x - 1) {       // the block that owns no sites
+            if (have) {
+                if (EPI == 5) cg_scalars_after_pAp(A.st, sum_in);
+                else cg_scalars_after_rr(A.st, sum_in);
+            }
+            return;
+        }
+        if (EPI == 5) {
+            if (!(sum_in > 0.0) || !isfinite(sum_in)) return;            // breakdown: the scalar step records it
+            a_fs = A.st->rr / sum_in;
+        } else if (have) {
+            if (sum_in <= A.st->tol2bb || A.st->iter_keep + 1 >= A.st->max_iter) return;   // the solve is over
+            beta_fs = sum_in / A.st->rr_keep;
+        } else {
+            beta_fs = A.st->b_prev;
+        }
+    }
     const Geom& g = A.g;
     const int kraw = blockIdx.x * DS_BLOCK + threadIdx.x;
     bool valid;
@@ -517,7 +553,7 @@ __global__ void __launch_bounds__(DS_BLOCK, (DsOcc<T, EPI>::minb)) dslash_kernel
     if (EPI != 0) {
         // CG: m^2 + sigma0 from the device state (graph-invariant)
         coef = (T)((EPI == 2) ? A.coef : A.st->c0);
-        if (EPI == 4) beta = (T)A.st->b_prev;
+        if (EPI == 4) beta = (T)(FS ? beta_fs : A.st->b_prev);
         if (EPI != 4) {
 #pragma unroll
             for (int c = 0; c < 3; ++c) pv[c] = A.pv[c * vh + k];
@@ -544,7 +580,7 @@ __global__ void __launch_bounds__(DS_BLOCK, (DsOcc<T, EPI>::minb)) dslash_kernel
     if (EPI == 4) {
         dot = k1_finish<T>(A.out, vh, k, valid, ar, ai, pp, A.st->c0);
     } else if (EPI == 5) {
-        const K2Coef<T> C = k2_coef_from_state<T>(A.st, A.p_out, A.r_out, A.p_keep, A.defer_base);
+        K2Coef<T> C = k2_coef_from_state<T>(A.st, FS ? a_fs : A.st->a, A.p_out, A.r_out, A.p_keep, A.defer_base);
         dot = k2_finish<T>(C, vh, k, valid, pv, rv, ar, ai);
     } else {
         // out = coef*pv - D in

@@ -565,17 +565,42 @@ void launch_dslash(lqcd_ctx* c, int epi, V2<T>* out, const V2<T>* in, int par, c
 }
 
 // after K1 (which = 1) / K2 (which = 2) of the whole-lattice path: block partials -> sum -> scalar step, one block
-void launch_reduce_scalar(lqcd_ctx* c, int which) {
-    cg_reduce_scalar_kernel<<<1, CG_BLOCK, 0, c->stream>>>(c->st_dev, c->partials, ds_grid(c), which);
+void launch_reduce_scalar(lqcd_ctx* c, int which, const double* partials) {
+    cg_reduce_scalar_kernel<<<1, CG_BLOCK, 0, c->stream>>>(c->st_dev, partials, ds_grid(c), which);
     ++c->launches;
+}
+
+// Small whole lattices: the scalar step after a sweep rides in the NEXT sweep (dslash_kernel, FS = 1) instead of a
+// one-block launch of its own, which is a third of the iteration there (16^4: 7.3 + 3.8 + 6.7 + 3.8 us).  Every block of
+// the next sweep adds the partials itself, so their number must stay small.
+#ifndef FS_MAX_BLOCKS
+#define FS_MAX_BLOCKS 1024
+#endif
+bool fused_scalar(const lqcd_ctx* c) { return !c->slab && ds_grid(c) <= FS_MAX_BLOCKS; }
+// K1 writes its partials to the first half of c->partials, K2 to the second (each is read while the other is written)
+double* partials_k2(const lqcd_ctx* c) { return c->partials + (c->n_partials - 8) / 2; }
+
+template <typename T, int EPI, int U1>
+void launch_dslash_fs_u(lqcd_ctx* c, const DslashArgs<T>& a) {
+    if (bufs<T>(c).recon_stored == 12)
+        dslash_kernel<T, 12, EPI, U1, 0, 1><<<ds_grid(c) + 1, DS_BLOCK, 0, c->stream>>>(a);
+    else
+        dslash_kernel<T, 18, EPI, U1, 0, 1><<<ds_grid(c) + 1, DS_BLOCK, 0, c->stream>>>(a);
+    ++c->launches;
+}
+template <typename T, int EPI>
+void launch_dslash_fs(lqcd_ctx* c, const DslashArgs<T>& a) {
+    if (c->u1_on) launch_dslash_fs_u<T, EPI, 1>(c, a);
+    else launch_dslash_fs_u<T, EPI, 0>(c, a);
 }
 
 // The two launches of a fused CG iteration (dslash.cuh, EPI = 4 and 5; cg.cuh has the whole picture).
 //   K1: t = D_oe p with p = r + beta p_old formed at the neighbours; <p,Ap>; a, zeta_i
 //   K2: p, s = c0 p - D_eo t, r_new = r - a s, x_0 += a p at the thread's own site; |r_new|^2; beta, b_i, flags
 template <typename T>
-void launch_cg_fused(lqcd_ctx* c, const V2<T>* r_in, V2<T>* r_out, V2<T>* p_keep, int defer_base) {
+void launch_cg_fused(lqcd_ctx* c, const V2<T>* r_in, V2<T>* r_out, V2<T>* p_keep, int defer_base, int pos, int m) {
     PrecBufs<T>& B = bufs<T>(c);
+    const bool fs = fused_scalar(c);
     DslashArgs<T> a{};
     a.g = c->g;
     a.W = B.W;
@@ -588,8 +613,16 @@ void launch_cg_fused(lqcd_ctx* c, const V2<T>* r_in, V2<T>* r_out, V2<T>* p_keep
     a.in2 = B.p;
     a.out = B.t;
     a.par = 1;
-    launch_dslash_t<T, 4>(c, a);
-    launch_reduce_scalar(c, 1);
+    if (fs) {
+        // pos == 0: the step after K2 of the previous iteration was run by the launch that precedes the block sweep
+        a.red_in = partials_k2(c);
+        a.red_n = ds_grid(c);
+        a.pending = (pos != 0);
+        launch_dslash_fs<T, 4>(c, a);
+    } else {
+        launch_dslash_t<T, 4>(c, a);
+        launch_reduce_scalar(c, 1, c->partials);
+    }
     a.in = B.t;
     a.in2 = nullptr;
     a.out = nullptr;
@@ -600,8 +633,16 @@ void launch_cg_fused(lqcd_ctx* c, const V2<T>* r_in, V2<T>* r_out, V2<T>* p_keep
     a.p_out = B.p;
     a.p_keep = p_keep;
     a.defer_base = defer_base;
-    launch_dslash_t<T, 5>(c, a);
-    launch_reduce_scalar(c, 2);
+    if (fs) {
+        a.red_in = c->partials;
+        a.partials = partials_k2(c);
+        a.pending = 1;
+        launch_dslash_fs<T, 5>(c, a);
+        if (pos == m - 1) launch_reduce_scalar(c, 2, partials_k2(c));      // the block sweep needs the step done
+    } else {
+        launch_dslash_t<T, 5>(c, a);
+        launch_reduce_scalar(c, 2, c->partials);
+    }
 }
 
 // m >= 2: x_0 of the base system is updated by the block sweep too (CgState::defer_base)
@@ -656,7 +697,7 @@ int launch_cg_iteration(lqcd_ctx* c, int pos) {
         if (pos == m - 1) launch_flush<T>(c);
         return LQCD_OK;
     }
-    launch_cg_fused<T>(c, r_in, r_out, p_keep, defer);
+    launch_cg_fused<T>(c, r_in, r_out, p_keep, defer, pos, m);
     if (pos == m - 1) launch_flush<T>(c);
     return LQCD_OK;
 }
@@ -712,7 +753,8 @@ int launch_persistent(lqcd_ctx* c) {
 // lattices whose links AND solver vectors stay in L2.  Measured at 16^4, whole config-2 solve, us per iteration,
 // persistent / launch path (four launches per iteration in a graph): two-row links (25 MB) 14.3 / 18.6, 18-real links
 // (38 MB: with the residual ring and the x_i, p_i the working set no longer fits) 20.0 / 19.5.  Hence the bound on the
-// stored links below.  LQCD_OPT_PERSISTENT overrides.
+// stored links below.  Since the scalar steps ride in the sweeps on small lattices (dslash_kernel, FS = 1) the launch
+// path takes 16.1 us with 18-real and 15.1 with two-row links there.  LQCD_OPT_PERSISTENT overrides.
 #ifndef PERSIST_LINKS_MAX
 #define PERSIST_LINKS_MAX (32u << 20)
 #endif
@@ -720,7 +762,10 @@ template <typename T>
 bool use_persistent(const lqcd_ctx* c) {
     if (c->slab || c->persistent_opt == 0) return false;
     if (!c->coop_launch || block_len(c) > PS_MAX_BLOCK) return false;
-    return c->persistent_opt == 1 || links_bytes<T>(c, bufs_c<T>(c).recon_stored) <= PERSIST_LINKS_MAX;
+    // ... and enough sites to give most SMs a block of one site per thread (12^4: 41 blocks; 21 us per iteration against
+    // 11.8 on the launch path)
+    const bool fills = (long)((c->Vh + PS_BLOCK - 1) / PS_BLOCK) * 4 >= (long)c->num_sms * 3;
+    return c->persistent_opt == 1 || (fills && links_bytes<T>(c, bufs_c<T>(c).recon_stored) <= PERSIST_LINKS_MAX);
 }
 
 // the host looks at the stop flag every this many iterations: a whole number of blocks
@@ -1435,7 +1480,10 @@ int solve(lqcd_ctx* c, const T* b_even, const double* shifts, int nshift, double
         } else {
             for (int i = 0; i < nit; ++i)
                 if ((rc = launch_cg_iteration<T>(c, i % m))) return rc;
-            if (nit % m != 0) launch_flush<T>(c);            // the stop falls inside a block: close it
+            if (nit % m != 0) {                              // the stop falls inside a block: close it
+                if (fused_scalar(c)) launch_reduce_scalar(c, 2, partials_k2(c));
+                launch_flush<T>(c);
+            }
             CU(cudaGetLastError());
         }
         const int slot = (int)(batch & 1);

@@ -93,6 +93,10 @@ struct CgState {
     // nshift vectors; the first sweep reads P from the source b_src (one vector, shared) and X as zero, and writes them.
     int first_block;
     const void* b_src;
+    // small lattices (dslash_kernel, FS = 1): |r|^2 and the iteration count as they were BEFORE the scalar step after K2,
+    // which runs beside the blocks of the next K1 that still need them
+    double rr_keep;
+    int iter_keep;
 };
 
 #endif

@@ -160,6 +160,8 @@ __device__ __noinline__ void cg_scalars_after_pAp(CgState* st, double pAp) {
     if (tid == 0) {
         st->pAp = pAp;
         st->a = a;
+        st->rr_keep = rr;
+        st->iter_keep = st->iter;
     }
 }
 
