@@ -210,6 +210,21 @@ def test_mshift_cg_fixed_iteration_count(lq, solver_path):
     assert abs(info["rel_res"] - info_ref["rel_res"]) <= 1e-9 * info_ref["rel_res"]
 
 
+@pytest.mark.parametrize("L,n_it", [((20, 20, 20, 20), 40), ((24, 24, 24, 24), 20)])
+@pytest.mark.parametrize("solver_path", ["launches"], indirect=True)
+def test_mshift_cg_fixed_count_around_the_small_lattice_bound(lq, L, n_it, solver_path):
+    """20^4 (625 blocks, more than one wave of them): the scalar steps ride in the sweeps (dslash_kernel FS = 1);
+    24^4 (1296 blocks): the one-block kernels.  Both sides run exactly n iterations, across a block boundary of the
+    deferred updates at 20^4 (m = 32 there, 40 iterations)."""
+    mass = 0.01
+    shifts = gen.shifts_geometric(1e-4, 1.0, 6)
+    x, info, x_ref, info_ref, _ = run_cg_both(lq, L, mass, shifts, 1e-30, max_iter=n_it, stream=torch.cuda.Stream())
+    assert info["iters"] == n_it == info_ref["iters"]
+    for i in range(len(shifts)):
+        assert rel_l2(soa_gpu_to_aos(x[i]), x_ref[i]) <= 1e-11
+    assert abs(info["rel_res"] - info_ref["rel_res"]) <= 1e-9 * info_ref["rel_res"]
+
+
 @pytest.mark.parametrize("check_every", [1, 3, 64])
 @pytest.mark.parametrize("solver_path", ["launches"], indirect=True)      # the host polls only on the launch path
 def test_mshift_cg_check_every_does_not_change_the_result(lq, check_every, solver_path):
