@@ -79,7 +79,8 @@ def cg_dram_bytes(freeze_iter, iters: int, m: int, recon: int) -> int:
       K1  8 links + r + p_old in, t out;   K2  8 links + t + r + p_old in, p + r_new out;
       m >= 2: per block of m iterations p_keep out (48), and one sweep: the block's residuals in (48 each), x_i, p_i
               in and out (192) of every shifted system active when the block began, p_keep in + x_0 in/out (144);
-      m == 1: x_0 in/out in K2 (96); per iteration the residual (48) + 192 per active shifted system."""
+      m == 1: x_0 in/out in K2 (96); per iteration the residual (48) + 192 per active shifted system;
+      the last sweep of a solve does not write the p_i (48 per shifted system less)."""
     links = 8 * LINK_BYTES[recon]
     base = max(range(len(freeze_iter)), key=lambda i: freeze_iter[i])
     total = iters * (2 * links + 3 * 48 + 5 * 48)
@@ -93,6 +94,8 @@ def cg_dram_bytes(freeze_iter, iters: int, m: int, recon: int) -> int:
             total += 48 + 48 * nres + 192 * n_in + 144
         else:
             total += 96 + (48 + 192 * n_in if n_in else 0)
+        if n0 + m >= iters:
+            total -= 48 * n_in      # the sweep that ends the solve does not store the p_i (nothing reads them any more)
     return total
 
 

@@ -138,7 +138,7 @@ __global__ void __launch_bounds__(64) cg_scalar_slots_kernel(CgState* st, const 
 #define FLUSH_UNR_LONG 4     // MM = 32: the 32 residuals of a site already take 128 registers
 #endif
 template <typename T, int MM, bool RATIONAL, bool FULL, int U>
-__device__ __forceinline__ void cg_flush_body(const int nres, const int nl, const int e_base, const bool first,
+__device__ __forceinline__ void cg_flush_body(const int nres, const int nl, const int e_base, const bool first, const bool last,
                                               V2<T>* const* sx, V2<T>* const* sp, const V2<T>* const* sq,
                                               const V2<T>* const* sr, const T* sCP, const T* sB, const V2<T>* sDE,
                                               const T* sY, V2<T>* __restrict__ y, const size_t n) {
@@ -193,7 +193,8 @@ __device__ __forceinline__ void cg_flush_body(const int nres, const int nl, cons
                         yv.x += dx;
                         yv.y += dy;
                     }
-                    if (e != e_base) sp[e][j] = make_v2(px, py);      // the base system's p is kept by K2
+                    if (e != e_base && !last) sp[e][j] = make_v2(px, py);   // the base system's p is kept by K2; after the last
+                                                                            // iteration of a solve no p_i is needed any more
                 }
             }
         }
@@ -204,7 +205,7 @@ __device__ __forceinline__ void cg_flush_body(const int nres, const int nl, cons
 // The sweep as a block-level function (every thread of every block of the grid calls it; blockDim.x >=
 // LQCD_MAX_SHIFTS + MM): used by cg_flush_kernel and, between grid-wide barriers, by the persistent solver.
 template <typename T, int MM, int U = ((MM <= 16) ? FLUSH_UNR : FLUSH_UNR_LONG)>
-__device__ __forceinline__ void cg_flush_block(const CgState* st, const size_t n, const int nres) {
+__device__ __forceinline__ void cg_flush_block(const CgState* st, const size_t n, const int nres, const bool last) {
     __shared__ V2<T>* sx[LQCD_MAX_SHIFTS];
     __shared__ V2<T>* sp[LQCD_MAX_SHIFTS];           // p_i as written
     __shared__ const V2<T>* sq[LQCD_MAX_SHIFTS];     // P as read: p_i, p_keep (base system), or b in the first block
@@ -258,11 +259,11 @@ __device__ __forceinline__ void cg_flush_block(const CgState* st, const size_t n
     V2<T>* __restrict__ y = (V2<T>*)st->y;
     if (nl > 0) {
         if (rational) {
-            if (nres == MM) cg_flush_body<T, MM, true, true, U>(nres, nl, s_ebase, first, sx, sp, sq, sr, sCP, sB, sDE, sY, y, n);
-            else cg_flush_body<T, MM, true, false, U>(nres, nl, s_ebase, first, sx, sp, sq, sr, sCP, sB, sDE, sY, y, n);
+            if (nres == MM) cg_flush_body<T, MM, true, true, U>(nres, nl, s_ebase, first, last, sx, sp, sq, sr, sCP, sB, sDE, sY, y, n);
+            else cg_flush_body<T, MM, true, false, U>(nres, nl, s_ebase, first, last, sx, sp, sq, sr, sCP, sB, sDE, sY, y, n);
         } else {
-            if (nres == MM) cg_flush_body<T, MM, false, true, U>(nres, nl, s_ebase, first, sx, sp, sq, sr, sCP, sB, sDE, sY, y, n);
-            else cg_flush_body<T, MM, false, false, U>(nres, nl, s_ebase, first, sx, sp, sq, sr, sCP, sB, sDE, sY, y, n);
+            if (nres == MM) cg_flush_body<T, MM, false, true, U>(nres, nl, s_ebase, first, last, sx, sp, sq, sr, sCP, sB, sDE, sY, y, n);
+            else cg_flush_body<T, MM, false, false, U>(nres, nl, s_ebase, first, last, sx, sp, sq, sr, sCP, sB, sDE, sY, y, n);
         }
     }
 }
@@ -271,7 +272,7 @@ template <typename T, int MM>
 __global__ void __launch_bounds__(CG_BLOCK, (MM <= 8 ? 2 : 1)) cg_flush_kernel(CgState* st, size_t n) {
     const int nres = st->blk_j;
     if (nres == 0) return;                       // nothing accumulated (solve already over); same in every block
-    cg_flush_block<T, MM>(st, n, nres);
+    cg_flush_block<T, MM>(st, n, nres, st->stop != 0);      // stop is set: this is the sweep that ends the solve
     // the last block to finish closes the block of iterations; every block has read the state by then
     __syncthreads();
     if (threadIdx.x == 0) {

@@ -159,7 +159,7 @@ __global__ void __launch_bounds__(PS_BLOCK, 1) cg_persistent_kernel(const Persis
         const int nres = breakdown ? pos : pos + 1;          // iterations accumulated in the current block
         if ((pos == m - 1 || stop) && nres > 0) {
             grid.sync();                                     // the scalar block's coefficients are visible
-            cg_flush_block<T, PS_MAX_BLOCK, 4>(st, 3 * vh, nres);     // 4 systems in flight: the registers this kernel has
+            cg_flush_block<T, PS_MAX_BLOCK, 4>(st, 3 * vh, nres, stop);     // 4 systems in flight: the registers this kernel has
             close_block = true;
         }
         if (stop) break;
