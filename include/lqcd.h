@@ -295,7 +295,9 @@ int lqcd_comm_init_nccl(lqcd_ctx* ctx, const void* id /*HOST, 128 bytes*/);
  * the handles of all ranks by any means (e.g. torch.distributed.all_gather_object) and hands every rank the table of
  * all of them, in rank order, through lqcd_comm_init_p2p (not collective: it only maps the windows).  At most 16
  * ranks.  The window is allocated with cudaMalloc (CUDA IPC exports whole allocations): it is not part of a caller
- * workspace and is released by lqcd_destroy.  LQCD_ECOMM if a window cannot be mapped (no peer access, other node) or stream memory operations are
+ * workspace and is released by lqcd_destroy.  Environment: LQCD_P2P_KERNEL_SIGNAL=1 makes the arrival words of a face be
+ * set by a one-thread kernel instead of cuStreamWriteValue32 (the transport switches to that by itself if the driver
+ * refuses the stream memory operation on a peer-mapped address).  LQCD_ECOMM if a window cannot be mapped (no peer access, other node) or stream memory operations are
  * unavailable.  STATUS: verified on one GPU (one rank; two and four ranks as processes sharing the GPU over CUDA IPC);
  * not run between two or more GPUs. */
 #define LQCD_P2P_HANDLE_BYTES 96
