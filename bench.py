@@ -62,7 +62,7 @@ DSLASH_FLOPS = {18: 570, 12: 570 + 8 * 42}
 # dram__bytes_write.sum), keyed by (workload, recon): (read GB, write GB, file under profiles/ that holds them).
 # tests/test_host_logic.py checks these constants against that file.
 NCU_DRAM_GB_PER_LAUNCH = {
-    ("config4_48^4", 18): (3.190561, 0.104241, "profiles/ncu_full_r02.md"),
+    ("config4_48^4", 18): (3.190677, 0.104111, "profiles/ncu_full_r02.md"),
     ("config4_48^4", 12): (2.171204, 0.101689, "profiles/ncu_full_r01.md"),
 }
 

@@ -90,7 +90,7 @@ def test_ncu_traffic_constants_of_bench_match_the_profile_they_cite():
     assert bench.NCU_DRAM_GB_PER_LAUNCH
     for (workload, recon), (rd, wr, path) in bench.NCU_DRAM_GB_PER_LAUNCH.items():
         text = open(os.path.join(ROOT, path)).read()
-        m = re.search(r"dslash_kernel<double, %d, 0, 0, 0>.*?dram__bytes_read\.sum\s+([0-9.]+) (\w+).*?"
+        m = re.search(r"dslash_kernel<double, %d(?:, 0)+>.*?dram__bytes_read\.sum\s+([0-9.]+) (\w+).*?"
                       r"dram__bytes_write\.sum\s+([0-9.]+) (\w+)" % recon, text, flags=re.S)
         assert m, (workload, recon, path)
         assert abs(float(m.group(1)) * unit[m.group(2)] - rd) <= 1e-5 * rd
