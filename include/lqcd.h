@@ -161,6 +161,37 @@ int lqcd_deo_host(lqcd_ctx* ctx, double* out_even /*HOST*/, const double* in_odd
  * paper's D_oe, D_eo, zaxpy sequence in two launches. */
 int lqcd_mdagm(lqcd_ctx* ctx, double* out_even, const double* in_even, double sigma);
 
+/* lqcd_mdagm for callers that are not in a position to allocate device memory.
+ *
+ * Who that is: code that runs inside an application which has handed all of the GPU's memory to its own pool (an RHMC
+ * code that sized its fields for the whole 180 GB, a framework with a caching allocator), where a cudaMalloc from a
+ * library fails or fragments the pool; and code on a path that must not stall, since cudaMalloc and cudaFree
+ * synchronise the whole device and so stop every other stream of the process.  lqcd_mdagm needs one odd-parity
+ * temporary, t = D_oe in (D_oe, D_eo, zaxpy), which it allocates on first use -- from the workspace of
+ * lqcd_set_workspace if there is one, else with cudaMalloc -- together with the solver's small state.  This entry
+ * point makes the same two launches, with the same kernels and therefore the same bits in out_even, but keeps t in a
+ * buffer that is compiled into the library: it calls no cudaMalloc, cudaFree, cudaMallocHost or any other allocating
+ * routine, at any call.  (The stored links still have to exist: do lqcd_create and lqcd_set_gauge at start-up, where
+ * allocation is allowed, or give the context an arena with lqcd_set_workspace beforehand.)
+ *
+ * Limit: lattices of at most LQCD_STATIC_MAX_VH = 65536 sites per parity (16^4, 16^3 x 32, 8^3 x 256 ...); larger ones
+ * get LQCD_EINVAL with the two numbers in lqcd_last_error.  Double precision, whole-lattice contexts (a slab context
+ * gets LQCD_EINVAL).  The buffer is 3 MiB and is held by every GPU on which this library is used, from the moment its
+ * code is loaded there until the process ends, also by programs that never call lqcd_mdagm_static.
+ *
+ * First call on a device: the library asks the runtime where the buffer lives on that device (cudaGetSymbolAddress;
+ * the answer is kept per device).  The context's device must be the current one (else LQCD_EINVAL).  Make that first
+ * call ahead of any stream capture.  Later calls only check arguments and enqueue the two launches on the context's
+ * stream; like lqcd_mdagm the function returns without waiting for them.
+ *
+ * One buffer per device, shared by all contexts, streams and threads: two calls whose kernels may run on the same GPU
+ * at the same time (different streams, or different contexts) overwrite each other's t and both results are garbage.
+ * Keep such calls on one stream or order them with events.  The buffer holds whatever the last call left there;
+ * nothing needs clearing, because every call rewrites all of t before reading it.
+ *   out_even, in_even : parity vectors (even sites), DEVICE, must not alias;  sigma as lqcd_mdagm. */
+#define LQCD_STATIC_MAX_VH 65536
+int lqcd_mdagm_static(lqcd_ctx* ctx, double* out_even, const double* in_even, double sigma);
+
 /* Single precision: the same operators on float parity vectors (3*Vh complex floats,
  * same index order) with the links stored as floats (LQCD_OPT_LINK_PRECISIONS must include LQCD_PREC_F32 at
  * lqcd_set_gauge time, otherwise LQCD_ENOGAUGE).  Arithmetic is float; only the CG's scalar products and

@@ -12,6 +12,7 @@ LQCD_OK, LQCD_EINVAL, LQCD_ENOGAUGE, LQCD_ENOMEM, LQCD_ECUDA = 0, -1, -2, -3, -4
 LQCD_ENOCONV, LQCD_EBREAKDOWN, LQCD_ENOTSU3, LQCD_ECOMM = -5, -6, -7, -8
 LQCD_NCCL_ID_BYTES = 128
 LQCD_P2P_HANDLE_BYTES = 96
+LQCD_STATIC_MAX_VH = 65536       # lqcd_mdagm_static: sites per parity its built-in buffer holds
 LQCD_OPT_MASS, LQCD_OPT_ANTIPERIODIC_T, LQCD_OPT_RECON, LQCD_OPT_MAX_ITER = 0, 1, 2, 3
 LQCD_OPT_CHECK_EVERY, LQCD_OPT_USE_GRAPH, LQCD_OPT_LINK_PRECISIONS, LQCD_OPT_SHIFT_BLOCK = 4, 5, 6, 7
 LQCD_OPT_PERSISTENT = 8
@@ -54,6 +55,7 @@ EXPORTS = {
     "lqcd_doe_host": (_i, [_vp, _dp, _dp]),
     "lqcd_deo_host": (_i, [_vp, _dp, _dp]),
     "lqcd_mdagm": (_i, [_vp, _dp, _dp, _d]),
+    "lqcd_mdagm_static": (_i, [_vp, _dp, _dp, _d]),
     "lqcd_mshift_cg": (_i, [_vp, _dp, _pd, _i, _d, ctypes.POINTER(ctypes.c_void_p)]),
     "lqcd_mshift_cg_host": (_i, [_vp, _dp, _pd, _i, _d, ctypes.POINTER(ctypes.c_void_p)]),
     "lqcd_mshift_cg_mixed": (_i, [_vp, _dp, _pd, _i, _d, ctypes.POINTER(ctypes.c_void_p)]),
@@ -194,6 +196,10 @@ def lqcd_doe_f32_host(ctx, out_odd, in_even):
 
 def lqcd_deo_f32_host(ctx, out_even, in_odd):
     return load_library().lqcd_deo_f32_host(ctx, out_even, in_odd)
+
+
+def lqcd_mdagm_static(ctx, out_even, in_even, sigma):
+    return load_library().lqcd_mdagm_static(ctx, out_even, in_even, float(sigma))
 
 
 def lqcd_mdagm_f32(ctx, out_even, in_even, sigma):
@@ -601,6 +607,18 @@ class Lattice:
         pout = self._t(out, (3, self.Vh, 2), "cuda", v_even.dtype)
         self._sync_stream()
         self._check((lqcd_mdagm_f32 if f32 else lqcd_mdagm)(self.ctx, pout, pin, sigma))
+        return out
+
+    def mdagm_static(self, v_even, out, sigma: float = 0.0):
+        """``mdagm`` through ``lqcd_mdagm_static``: for callers that cannot allocate device memory (their application
+        owns all of it, or they must not trigger the device-wide synchronisation of cudaMalloc).  ``out`` is
+        therefore required, double precision only, at most ``LQCD_STATIC_MAX_VH`` sites per parity; the temporary
+        sits in a 3 MiB buffer built into the library and shared by every caller on the device, so calls must not
+        overlap on the GPU (include/lqcd.h)."""
+        pin = self._t(v_even, (3, self.Vh, 2), "cuda", self._torch.float64)
+        pout = self._t(out, (3, self.Vh, 2), "cuda", self._torch.float64)
+        self._sync_stream()
+        self._check(lqcd_mdagm_static(self.ctx, pout, pin, sigma))
         return out
 
     def mshift_cg(self, b_even, shifts: Sequence[float], tol: float, x=None, raise_on_noconv: bool = True):

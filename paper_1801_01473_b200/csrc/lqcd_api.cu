@@ -11,6 +11,7 @@
 #include <cstdint>
 #include <cstdio>
 #include <cstring>
+#include <mutex>
 #include <new>
 #include <vector>
 
@@ -1749,7 +1750,64 @@ int pack_unpack(lqcd_ctx* c, int parity, const T* in, T* out, bool pack) {
 
 }  // namespace
 
+// ---- lqcd_mdagm_static: the Eq. 2 operator for callers that must not allocate device memory (include/lqcd.h) -----
+// lqcd_mdagm keeps the odd-parity intermediate t = D_oe v in a buffer it allocates on first use.  Here that
+// intermediate lives in the array below, which is part of the library's image: the CUDA runtime places one copy of it
+// on every device that loads this module and keeps it until the process exits, whether or not the entry point is
+// ever called.  LQCD_STATIC_MAX_VH sites per parity x 3 colours x 16 bytes = 3 MiB.
+static __device__ __align__(256) double2 g_static_t[3 * (size_t)LQCD_STATIC_MAX_VH];
+
+namespace {
+
+// In host code `g_static_t` is only the handle under which the runtime knows the array -- it is not something a
+// kernel can dereference.  The address that kernels can use differs from device to device and is asked for once
+// per device, with that device current.
+constexpr int STATIC_MAX_DEVICES = 64;
+std::mutex g_static_mu;
+double2* g_static_addr[STATIC_MAX_DEVICES] = {};
+
+int static_scratch(lqcd_ctx* c, double2** out) {
+    int dev = -1;
+    CU(cudaGetDevice(&dev));
+    if (dev != c->device)
+        return fail(c, LQCD_EINVAL, "lqcd_mdagm_static: the context belongs to device %d but device %d is current", c->device,
+                    dev);
+    if (dev < 0 || dev >= STATIC_MAX_DEVICES)
+        return fail(c, LQCD_EINVAL, "lqcd_mdagm_static: device ordinal %d not supported (< %d)", dev, STATIC_MAX_DEVICES);
+    std::lock_guard<std::mutex> lock(g_static_mu);
+    if (!g_static_addr[dev]) {
+        void* p = nullptr;
+        CU(cudaGetSymbolAddress(&p, g_static_t));
+        if (!p) return fail(c, LQCD_ECUDA, "lqcd_mdagm_static: cudaGetSymbolAddress gave a NULL address");
+        g_static_addr[dev] = (double2*)p;
+    }
+    *out = g_static_addr[dev];
+    return LQCD_OK;
+}
+
+}  // namespace
+
 extern "C" {
+
+int lqcd_mdagm_static(lqcd_ctx* c, double* out_even, const double* in_even, double sigma) {
+    if (!c) return LQCD_EINVAL;
+    if (!out_even || !in_even) return fail(c, LQCD_EINVAL, "NULL vector");
+    if (out_even == in_even) return fail(c, LQCD_EINVAL, "in and out must not alias");
+    if (c->slab) return fail(c, LQCD_EINVAL, "lqcd_mdagm_static: whole-lattice contexts only (a slab needs halo buffers)");
+    if (c->Vh > (size_t)LQCD_STATIC_MAX_VH)
+        return fail(c, LQCD_EINVAL, "lqcd_mdagm_static: the lattice has %zu sites per parity, the built-in buffer holds at "
+                    "most %d (LQCD_STATIC_MAX_VH); use lqcd_mdagm", c->Vh, (int)LQCD_STATIC_MAX_VH);
+    int rc;
+    if ((rc = check_ctx_gauge<double>(c))) return rc;
+    double2* t = nullptr;
+    if ((rc = static_scratch(c, &t))) return rc;
+    // the same two launches as lqcd_mdagm; the first one writes every odd site of t, so nothing of an earlier call
+    // is read and nothing has to be cleared
+    launch_dslash<double>(c, 0, t, (const double2*)in_even, 1, nullptr, 0.0, 0);
+    launch_dslash<double>(c, 2, (double2*)out_even, t, 0, (const double2*)in_even, c->mass * c->mass + sigma, 0);
+    CU(cudaGetLastError());
+    return LQCD_OK;
+}
 
 int lqcd_doe(lqcd_ctx* c, double* out_odd, const double* in_even) { return apply_d<double>(c, out_odd, in_even, 1); }
 int lqcd_deo(lqcd_ctx* c, double* out_even, const double* in_odd) { return apply_d<double>(c, out_even, in_odd, 0); }
