@@ -95,9 +95,17 @@ typedef struct lqcd_ctx lqcd_ctx;
                                        host polling); all others by two operator launches per iteration (+ two
                                        one-block kernels, which small lattices fold into the launches) replayed as
                                        a CUDA graph.
-                                       0: never, 1: always the persistent kernel.
+                                       0: never, 1: always the persistent kernel -- a solve it cannot run (slab
+                                       context, LQCD_OPT_SHIFT_BLOCK above 16, a device without cooperative launches,
+                                       a refused launch) then returns LQCD_EINVAL / LQCD_ECUDA instead of silently
+                                       taking the other driver.  With -1 a refused cooperative launch (fewer blocks
+                                       resident than expected: another context or MPS client on the GPU) falls back
+                                       to the launches.  LQCD_STAT_SOLVER_PATH tells which driver ran.
                                        Same arithmetic per site; the scalar products are added over a different grid,
                                        so results agree to rounding.  Whole-lattice contexts only.            */
+#define LQCD_OPT_COMM_TIMEOUT    9  /* seconds (default 120; 0 = for ever) a solve on a slab context over the
+                                       peer-memory transport waits for a batch of iterations before it concludes
+                                       that a peer rank is gone and returns LQCD_ECOMM (see lqcd_comm_abort)    */
 #define LQCD_PREC_F64 1
 #define LQCD_PREC_F32 2
 
@@ -334,6 +342,22 @@ int lqcd_comm_init_nccl(lqcd_ctx* ctx, const void* id /*HOST, 128 bytes*/);
 #define LQCD_P2P_HANDLE_BYTES 96
 int lqcd_p2p_export(lqcd_ctx* ctx, void* handle /*HOST, LQCD_P2P_HANDLE_BYTES*/);
 int lqcd_comm_init_p2p(lqcd_ctx* ctx, const void* handles /*HOST, nranks * LQCD_P2P_HANDLE_BYTES, rank order*/);
+
+/* When a rank cannot go on.  Over the peer-memory transport the ranks wait for each other's faces and partial sums with
+ * stream operations on flag words; a rank that stops making the same calls as the others would leave them waiting.
+ *   - A rank whose solve fails (transport or CUDA error) marks the flag words of its peers before it returns; the
+ *     peers' waits complete, their kernels see the mark, and their lqcd_mshift_cg / lqcd_rational_apply return
+ *     LQCD_ECOMM (and pass the mark on, so ranks that were waiting for somebody else are released too).
+ *   - A rank that has to leave for a reason of its own (an exception in the caller) calls lqcd_comm_abort first.
+ *   - A rank whose process was killed marks nothing: the others give up after LQCD_OPT_COMM_TIMEOUT seconds without
+ *     progress and return LQCD_ECOMM.
+ * After LQCD_ECOMM (or lqcd_comm_abort) the context's transport is dead: every further solve or operator call on it
+ * returns LQCD_ECOMM at once.  The caller must lqcd_destroy the context on EVERY rank (the x[] of the failed solve are
+ * undefined), and to continue create new contexts, export new windows and exchange the handles again.  Operator calls
+ * (lqcd_doe ...) return after enqueueing and cannot report a peer's mark themselves; the next solve does.
+ * The NCCL transport has its own failure handling (NCCL's); a caller-supplied transport reports through its return
+ * codes.  lqcd_comm_abort on a slab context without the peer-memory transport does nothing. */
+int lqcd_comm_abort(lqcd_ctx* ctx);
 
 /* rank, nranks, first global time slice and global Lt of a context (0, 1, 0, Lt for a whole-lattice one) */
 int lqcd_slab_info(const lqcd_ctx* ctx, int* rank, int* nranks, int* t_offset, int* Lt_global /*HOST, may be NULL*/);

@@ -22,5 +22,5 @@ from .binding import (  # noqa: F401
     lqcd_doe_f32, lqcd_deo_f32, lqcd_doe_f32_host, lqcd_deo_f32_host, lqcd_mdagm_f32, lqcd_mshift_cg_f32,
     lqcd_mshift_cg_f32_host, lqcd_rational_apply_f32, lqcd_pack_vector_f32, lqcd_unpack_vector_f32,
     lqcd_create_slab, lqcd_set_comm, lqcd_nccl_unique_id, lqcd_comm_init_nccl, lqcd_p2p_export, lqcd_comm_init_p2p, lqcd_slab_info, lqcd_comm_ops,
-    TorchTransport, lqcd_mshift_cg_mixed, lqcd_mdagm_static, LQCD_STATIC_MAX_VH,
+    TorchTransport, lqcd_mshift_cg_mixed, lqcd_mdagm_static, LQCD_STATIC_MAX_VH, lqcd_comm_abort, LQCD_OPT_COMM_TIMEOUT,
 )

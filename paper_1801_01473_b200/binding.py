@@ -19,6 +19,8 @@ LQCD_OPT_PERSISTENT = 8
 LQCD_PREC_F64, LQCD_PREC_F32 = 1, 2
 LQCD_STAT_ITERS, LQCD_STAT_REL_RES, LQCD_STAT_FREEZE_ITER, LQCD_STAT_BASE_SHIFT = 0, 1, 2, 3
 LQCD_STAT_GPU_LAUNCHES, LQCD_STAT_SOLVE_MS, LQCD_STAT_RELIABLE_UPDATES, LQCD_STAT_GRAPH_REPLAYS = 4, 5, 6, 7
+LQCD_OPT_COMM_TIMEOUT = 9          # seconds a solve over the peer-memory transport waits for its peers (0: for ever)
+LQCD_STAT_SOLVER_PATH = 8          # 0 = plain launches, 1 = CUDA-graph replays, 2 = persistent kernel
 
 _ERRNAMES = {0: "LQCD_OK", -1: "LQCD_EINVAL", -2: "LQCD_ENOGAUGE", -3: "LQCD_ENOMEM", -4: "LQCD_ECUDA",
              -5: "LQCD_ENOCONV", -6: "LQCD_EBREAKDOWN", -7: "LQCD_ENOTSU3", -8: "LQCD_ECOMM"}
@@ -82,6 +84,7 @@ EXPORTS = {
     "lqcd_p2p_export": (_i, [_vp, _vp]),
     "lqcd_comm_init_p2p": (_i, [_vp, _vp]),
     "lqcd_slab_info": (_i, [_vp, _pi, _pi, _pi, _pi]),
+    "lqcd_comm_abort": (_i, [_vp]),
 }
 
 _lib = None
@@ -196,6 +199,10 @@ def lqcd_doe_f32_host(ctx, out_odd, in_even):
 
 def lqcd_deo_f32_host(ctx, out_even, in_odd):
     return load_library().lqcd_deo_f32_host(ctx, out_even, in_odd)
+
+
+def lqcd_comm_abort(ctx):
+    return load_library().lqcd_comm_abort(ctx)
 
 
 def lqcd_mdagm_static(ctx, out_even, in_even, sigma):
@@ -608,6 +615,10 @@ class Lattice:
         self._sync_stream()
         self._check((lqcd_mdagm_f32 if f32 else lqcd_mdagm)(self.ctx, pout, pin, sigma))
         return out
+
+    def comm_abort(self):
+        """This rank cannot go on: release the ranks that wait for it (include/lqcd.h, lqcd_comm_abort)."""
+        self._check(lqcd_comm_abort(self.ctx))
 
     def mdagm_static(self, v_even, out, sigma: float = 0.0):
         """``mdagm`` through ``lqcd_mdagm_static``: for callers that cannot allocate device memory (their application

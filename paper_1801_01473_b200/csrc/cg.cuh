@@ -110,13 +110,27 @@ __global__ void __launch_bounds__(64) cg_scalar_kernel(CgState* st, const double
 __global__ void __launch_bounds__(64) cg_scalar_slots_kernel(CgState* st, const double* slots, unsigned int* flags,
                                                              int nranks, int stride, int which) {
     __shared__ double sv;
+    __shared__ int poisoned;
     if (threadIdx.x == 0) {
         double acc = 0.0;
         for (int r = 0; r < nranks; ++r) acc += __ldcv(slots + r * stride);
         sv = acc;
+        poisoned = 0;
     }
-    if (threadIdx.x < nranks) flags[threadIdx.x] = 0u;
     __syncthreads();
+    // a rank that gave up left LQCD_P2P_POISON instead of 1 (p2p.cuh): its slot holds nothing; the mark stays
+    if (threadIdx.x < nranks) {
+        if (*(volatile unsigned int*)(flags + threadIdx.x) == LQCD_P2P_POISON) poisoned = 1;
+        else flags[threadIdx.x] = 0u;
+    }
+    __syncthreads();
+    if (poisoned) {
+        if (threadIdx.x == 0) {
+            st->status = LQCD_ECOMM_DEV;
+            st->stop = 1;
+        }
+        return;
+    }
     if (st->stop) return;
     if (which == 1) cg_scalars_after_pAp(st, sv);
     else cg_scalars_after_rr(st, sv);

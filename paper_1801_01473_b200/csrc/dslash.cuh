@@ -506,10 +506,18 @@ __global__ void __launch_bounds__(DS_BLOCK, (DsOcc<T, EPI>::minb)) dslash_kernel
     static_assert(EPI == 0 || EPI == 2 || EPI == 4 || EPI == 5, "EPI");
     static_assert(!FS || (!SLAB && (EPI == 4 || EPI == 5)), "FS");
     if (SLAB && A.clear0 && blockIdx.x == 0 && threadIdx.x == 0) {
-        *A.clear0 = 0u;
-        *A.clear1 = 0u;
+        // peer-memory transport: the two arrival words of the halos this launch reads are cleared for their next use --
+        // unless a neighbour that gave up wrote LQCD_P2P_POISON there (the halo is then not a halo): that stays, and
+        // the solve ends with LQCD_ECOMM
+        const unsigned int w0 = *(volatile unsigned int*)A.clear0, w1 = *(volatile unsigned int*)A.clear1;
+        if (w0 != LQCD_P2P_POISON) *A.clear0 = 0u;
+        if (w1 != LQCD_P2P_POISON) *A.clear1 = 0u;
+        if (w0 == LQCD_P2P_POISON || w1 == LQCD_P2P_POISON) {
+            A.st->status = LQCD_ECOMM_DEV;
+            A.st->stop = 1;
+        }
     }
-    if (A.check_stop && A.st->stop) return;      // iterations launched beyond the one that converged
+    if (!FS && A.check_stop && A.st->stop) return;      // iterations launched beyond the one that converged
     double a_fs = 0.0, beta_fs = 0.0;
     if (FS) {
         __shared__ double redf[32];

@@ -10,9 +10,11 @@
 #include <cstdarg>
 #include <cstdint>
 #include <cstdio>
+#include <chrono>
 #include <cstring>
 #include <mutex>
 #include <new>
+#include <thread>
 #include <vector>
 
 #include "cg.cuh"
@@ -81,6 +83,7 @@ struct lqcd_ctx {
     int recon_opt, max_iter, check_every, use_graph;
     int shift_block_opt;     // LQCD_OPT_SHIFT_BLOCK: 0 = chosen from the lattice size (block_len())
     int persistent_opt;      // LQCD_OPT_PERSISTENT: -1 = the library decides (lattices that live in L2), 0 = never, 1 = always
+    double comm_timeout;     // LQCD_OPT_COMM_TIMEOUT, seconds; <= 0: wait for ever
 
     // memory
     char* arena;             // caller workspace (not owned) or NULL
@@ -440,6 +443,7 @@ int slab_apply(lqcd_ctx* c, DslashArgs<T>& a, int kepi, const V2<T>* face_v, con
     // peer-memory transport: the faces are written straight into the neighbours' halo buffers (no send buffer, no
     // transport kernel), and the border launch reads my halos where the neighbours wrote them (p2p.cuh)
     const bool p2p = c->p2p.active && c->comm.user == (void*)&c->p2p;
+    if (p2p && c->p2p.dead) return fail(c, LQCD_ECOMM, "peer-memory transport has failed: %s", c->p2p.error);
     if (p2p) {
         const lqcd_p2p::Slots o = lqcd_p2p::begin(&c->p2p);
         send_lo = (V2<T>*)o.dst_dn;
@@ -769,11 +773,17 @@ bool use_persistent(const lqcd_ctx* c) {
     return c->persistent_opt == 1 || (fills && links_bytes<T>(c, bufs_c<T>(c).recon_stored) <= PERSIST_LINKS_MAX);
 }
 
+bool over_p2p(const lqcd_ctx* c);
+
 // the host looks at the stop flag every this many iterations: a whole number of blocks
 int check_every(const lqcd_ctx* c) {
     long v = c->check_every ? (long)c->check_every : (long)(4000000 / (long)c->Vh);
     if (v < 1) v = 1;
     if (!c->check_every && v > 64) v = 64;
+    // peer-memory transport with a time limit on the peers: the host runs two batches ahead of the device, and when a
+    // peer is gone everything it has enqueued sits behind one stream wait.  Keep that well below the depth at which a
+    // launch call itself blocks (there the time limit could not act): ~14 operations per iteration.
+    if (!c->check_every && over_p2p(c) && c->comm_timeout > 0.0 && v > 16) v = 16;
     const long m = block_len(c);
     return (int)((v + m - 1) / m * m);
 }
@@ -996,6 +1006,7 @@ lqcd_ctx* lqcd_create(int Lx, int Ly, int Lz, int Lt) {
     c->use_graph = 1;
     c->shift_block_opt = 0;
     c->persistent_opt = -1;
+    c->comm_timeout = 120.0;
     c->err[0] = 0;
     return c;
 }
@@ -1185,6 +1196,10 @@ int lqcd_set_option(lqcd_ctx* c, int key, double v) {
             if (v != -1.0 && v != 0.0 && v != 1.0) return fail(c, LQCD_EINVAL, "PERSISTENT must be -1 (auto), 0 or 1");
             c->persistent_opt = (int)v;
             break;
+        case LQCD_OPT_COMM_TIMEOUT:
+            if (!(v >= 0.0)) return fail(c, LQCD_EINVAL, "COMM_TIMEOUT must be >= 0 seconds (0: wait for ever)");
+            c->comm_timeout = v;
+            break;
         case LQCD_OPT_LINK_PRECISIONS:
             if (v != 1.0 && v != 2.0 && v != 3.0)
                 return fail(c, LQCD_EINVAL, "LINK_PRECISIONS must be LQCD_PREC_F64 (1), LQCD_PREC_F32 (2) or both (3)");
@@ -1208,6 +1223,7 @@ int lqcd_get_option(const lqcd_ctx* c, int key, double* v) {
         case LQCD_OPT_USE_GRAPH: *v = c->use_graph; break;
         case LQCD_OPT_LINK_PRECISIONS: *v = c->prec_opt; break;
         case LQCD_OPT_PERSISTENT: *v = c->persistent_opt; break;
+        case LQCD_OPT_COMM_TIMEOUT: *v = c->comm_timeout; break;
         default: return LQCD_EINVAL;
     }
     return LQCD_OK;
@@ -1380,9 +1396,64 @@ int apply_mdagm(lqcd_ctx* c, T* out_even, const T* in_even, double sigma) {
 
 // The solver behind lqcd_mshift_cg (x != NULL: every x[i] is stored) and lqcd_rational_apply (y != NULL:
 // only y = alpha0 b + sum_i alpha[i] x_i is accumulated), in precision T.
+// ---- a solve over the peer-memory transport must not wait for ever --------------------------------------------------
+// Over that transport a rank waits for its peers with stream memory operations on its own window (p2p.cuh).  A peer
+// that has failed releases the others by marking their words (lqcd_p2p::poison) -- but a peer whose process was killed
+// marks nothing.  So on such a context the host does not block in cudaEventSynchronize: it polls, and after
+// LQCD_OPT_COMM_TIMEOUT seconds without the awaited batch completing it gives up: it releases its own streams and its
+// peers and the solve returns LQCD_ECOMM.
+bool over_p2p(const lqcd_ctx* c) { return c->slab && c->p2p.active && c->comm.user == (const void*)&c->p2p; }
+
+int wait_event_watched(lqcd_ctx* c, cudaEvent_t ev, bool* timed_out) {
+    *timed_out = false;
+    if (!over_p2p(c) || !(c->comm_timeout > 0.0)) {
+        CU(cudaEventSynchronize(ev));
+        return LQCD_OK;
+    }
+    const auto t0 = std::chrono::steady_clock::now();
+    for (;;) {
+        const cudaError_t e = cudaEventQuery(ev);
+        if (e == cudaSuccess) return LQCD_OK;
+        if (e != cudaErrorNotReady) CU(e);
+        const double waited = std::chrono::duration<double>(std::chrono::steady_clock::now() - t0).count();
+        if (waited > c->comm_timeout) {
+            *timed_out = true;
+            return LQCD_OK;
+        }
+        if (waited > 2e-4) std::this_thread::sleep_for(std::chrono::microseconds(50));     // spin first: batches are short
+    }
+}
+
+// the awaited work did not complete in time: release everybody (this rank included), let this rank's streams drain
+int give_up_waiting(lqcd_ctx* c) {
+    lqcd_p2p::poison(&c->p2p, true);
+    bool again = false;
+    cudaEvent_t ev = c->ev[0];
+    if (cudaEventRecord(ev, c->stream) == cudaSuccess) wait_event_watched(c, ev, &again);
+    cudaGetLastError();
+    return fail(c, LQCD_ECOMM, "peer-memory transport: no sign of a peer rank for %.1f s (LQCD_OPT_COMM_TIMEOUT)%s; the "
+                "context can only be destroyed", c->comm_timeout, again ? ", and this rank's stream did not drain" : "");
+}
+
+template <typename T>
+int solve_impl(lqcd_ctx* c, const T* b_even, const double* shifts, int nshift, double tol, T* const* x, T* y, double alpha0,
+               const double* alpha);
+
 template <typename T>
 int solve(lqcd_ctx* c, const T* b_even, const double* shifts, int nshift, double tol, T* const* x, T* y, double alpha0,
           const double* alpha) {
+    if (c && c->p2p.dead)
+        return fail(c, LQCD_ECOMM, "the peer-memory transport of this context has failed (%s): destroy the context on every "
+                    "rank and set the ranks up again", c->p2p.error);
+    const int rc = solve_impl<T>(c, b_even, shifts, nshift, tol, x, y, alpha0, alpha);
+    // a rank that leaves a solve early takes its peers with it instead of leaving them waiting for its faces and sums
+    if (c && over_p2p(c) && (rc == LQCD_ECOMM || rc == LQCD_ECUDA)) lqcd_p2p::poison(&c->p2p, false);
+    return rc;
+}
+
+template <typename T>
+int solve_impl(lqcd_ctx* c, const T* b_even, const double* shifts, int nshift, double tol, T* const* x, T* y, double alpha0,
+               const double* alpha) {
     if (!c) return LQCD_EINVAL;
     if (!b_even || !shifts || (!x && !y) || (y && !alpha)) return fail(c, LQCD_EINVAL, "NULL argument");
     if (nshift < 1 || nshift > LQCD_MAX_SHIFTS) return fail(c, LQCD_EINVAL, "nshift must be in [1, %d]", LQCD_MAX_SHIFTS);
@@ -1491,12 +1562,20 @@ int solve(lqcd_ctx* c, const T* b_even, const double* shifts, int nshift, double
         CU(cudaMemcpyAsync(&c->flag_host[slot], &c->st_dev->stop, sizeof(int), cudaMemcpyDeviceToHost, c->stream));
         CU(cudaEventRecord(c->ev[slot], c->stream));
         if (batch >= 1) {
-            CU(cudaEventSynchronize(c->ev[slot ^ 1]));
+            bool late = false;
+            if ((rc = wait_event_watched(c, c->ev[slot ^ 1], &late))) return rc;
+            if (late) return give_up_waiting(c);
             if (c->flag_host[slot ^ 1]) done = true;
         }
     }
     CU(cudaEventRecord(c->ev_t1, c->stream));
     CU(cudaMemcpyAsync(h, c->st_dev, sizeof(CgState), cudaMemcpyDeviceToHost, c->stream));
+    {
+        bool late = false;
+        CU(cudaEventRecord(c->ev[0], c->stream));
+        if ((rc = wait_event_watched(c, c->ev[0], &late))) return rc;
+        if (late) return give_up_waiting(c);
+    }
     CU(cudaStreamSynchronize(c->stream));
     CU(cudaEventElapsedTime(&c->last_ms, c->ev_t0, c->ev_t1));
 
@@ -1788,6 +1867,13 @@ int static_scratch(lqcd_ctx* c, double2** out) {
 }  // namespace
 
 extern "C" {
+
+int lqcd_comm_abort(lqcd_ctx* c) {
+    if (!c) return LQCD_EINVAL;
+    if (!c->slab) return fail(c, LQCD_EINVAL, "not a slab context");
+    if (c->p2p.active) lqcd_p2p::poison(&c->p2p, true);
+    return LQCD_OK;
+}
 
 int lqcd_mdagm_static(lqcd_ctx* c, double* out_even, const double* in_even, double sigma) {
     if (!c) return LQCD_EINVAL;

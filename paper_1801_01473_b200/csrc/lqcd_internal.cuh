@@ -34,6 +34,11 @@ struct Geom {
 // every rank's window (its own included).  Lives in device memory, one per generation of the all-reduce.
 #define LQCD_P2P_MAX_RANKS 16
 #define LQCD_P2P_RED_MAX 4          // doubles per all-reduce slot
+// Written into the arrival words of its peers by a rank that gives up (p2p.cuh, poison): it satisfies every
+// ">= 1" stream wait (the comparison is a signed difference), is never written otherwise, and the kernels that consume
+// a halo or the slots of an all-reduce leave it in place and record LQCD_ECOMM in the CG state instead of clearing it.
+#define LQCD_P2P_POISON 0x40000000u
+#define LQCD_ECOMM_DEV (-8)         // LQCD_ECOMM of include/lqcd.h
 struct PeerPush {
     double* slot[LQCD_P2P_MAX_RANKS];
     unsigned int* flag[LQCD_P2P_MAX_RANKS];

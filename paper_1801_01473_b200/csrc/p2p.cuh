@@ -34,8 +34,10 @@
 #include <cuda.h>
 #include <cuda_runtime.h>
 #include <stdint.h>
+#include <stdio.h>
 #include <stdlib.h>
 #include <string.h>
+#include <time.h>
 #include <unistd.h>
 
 #include "lqcd_internal.cuh"
@@ -58,7 +60,7 @@ static_assert(sizeof(Header) <= HDR_BYTES, "window header");
 // what travels between the ranks (LQCD_P2P_HANDLE_BYTES of include/lqcd.h)
 struct Blob {
     cudaIpcMemHandle_t ipc;                // 64 bytes
-    long long pid;
+    long long pid;                         // process_tag() of the exporter: its pid and a number drawn once per process
     unsigned long long ptr;                // the window in the exporting process (used when it is this process)
     unsigned long long cap;
     int device;
@@ -77,6 +79,7 @@ struct Transport {
     unsigned int seq = 0, rseq = 0;        // exchanges / all-reduces issued so far (only their parity matters)
     mem_op32_fn wait32 = nullptr, write32 = nullptr;
     bool kernel_signal = false;            // remote arrival words are set by a one-thread kernel, not by cuStreamWriteValue32
+    bool dead = false;                     // an operation failed after connect: every later one is refused at once
     const char* error = "";
 
     Header* hdr(int r) const { return (Header*)win[r]; }
@@ -89,10 +92,32 @@ struct Transport {
 
 inline size_t window_bytes(size_t cap) { return HDR_BYTES + 4 * cap; }
 
+// A failure after connect() leaves this rank's exchange counters (seq, rseq) out of step with its peers', and
+// possibly half an exchange enqueued: nothing further can be matched, so the transport is dead from then on and
+// keeps the text of the first failure.
 inline int fail(Transport* t, const char* why) {
-    t->error = why;
+    if (!t->dead) t->error = why;
+    if (t->active) t->dead = true;
     cudaGetLastError();
     return -1;
+}
+inline bool usable(const Transport* t) { return t->active && !t->dead; }
+
+// Two ranks are "the same process" (and may use each other's device pointers as they are) only if pid AND a number
+// drawn once per process agree: ranks in different PID namespaces of one node (a container each) can have equal pids.
+inline long long process_tag() {
+    static long long tag = 0;
+    if (!tag) {
+        unsigned int nonce = 0;
+        FILE* f = fopen("/dev/urandom", "rb");
+        if (f) {
+            if (fread(&nonce, sizeof(nonce), 1, f) != 1) nonce = 0;
+            fclose(f);
+        }
+        if (!nonce) nonce = (unsigned int)((uintptr_t)&tag & 0xffffffffu) ^ (unsigned int)time(nullptr);
+        tag = ((long long)(unsigned int)getpid() << 32) | (long long)(nonce | 1u);
+    }
+    return tag;
 }
 
 // allocate this rank's window and describe it
@@ -122,7 +147,7 @@ inline int create_window(Transport* t, int rank, int nranks, size_t cap, Blob* o
     t->win[rank] = (char*)w;
     memset(out, 0, sizeof(Blob));
     if (cudaIpcGetMemHandle(&out->ipc, w) != cudaSuccess) cudaGetLastError();   // ranks of one process need no handle
-    out->pid = (long long)getpid();
+    out->pid = process_tag();
     out->ptr = (unsigned long long)(uintptr_t)w;
     out->cap = t->cap;
     out->device = t->device;
@@ -137,8 +162,13 @@ inline int connect(Transport* t, const Blob* blobs) {
         const Blob& b = blobs[r];
         if (b.rank != r || b.cap != t->cap) return fail(t, "handle table does not match this lattice / rank order");
         if (r == t->rank) continue;
-        if (b.pid == (long long)getpid()) {
-            // another context of this process: its pointer is valid here; peer access if it sits on another device
+        if (b.pid == process_tag()) {
+            // another context of this process: its pointer is valid here (checked); peer access if it sits on another
+            // device
+            cudaPointerAttributes at;
+            if (cudaPointerGetAttributes(&at, (const void*)(uintptr_t)b.ptr) != cudaSuccess ||
+                at.type != cudaMemoryTypeDevice || at.device != b.device)
+                return fail(t, "a handle claims to come from this process but its window is not device memory here");
             if (b.device != t->device) {
                 const cudaError_t e = cudaDeviceEnablePeerAccess(b.device, 0);
                 if (e != cudaSuccess && e != cudaErrorPeerAccessAlreadyEnabled) return fail(t, "no peer access to a rank of this process");
@@ -166,6 +196,40 @@ inline int connect(Transport* t, const Blob* blobs) {
         return fail(t, "writing the push targets");
     t->active = true;
     return 0;
+}
+
+// Release every rank that waits, or will wait, for something from this rank: LQCD_P2P_POISON into the arrival words this
+// rank is the writer of -- the face words of its two neighbours and its own entry of every rank's all-reduce words, both
+// generations.  Their stream waits complete, the kernels behind them find the mark and end the solve with LQCD_ECOMM
+// (cg.cuh, dslash.cuh), and every rank that returns LQCD_ECOMM does the same for ITS peers, so the release spreads to
+// ranks that were waiting for somebody else.  self = true (a rank that waited too long for a peer that may be gone
+// without a word): also all of this rank's own words, so that its own streams drain.
+// Plain 4-byte copies on a stream of their own: the rank's other streams may be the ones that are stuck.
+inline void poison(Transport* t, bool self) {
+    if (!t->win[t->rank]) return;
+    t->dead = true;
+    if (!*t->error) t->error = "aborted";
+    cudaStream_t s = nullptr;
+    if (cudaStreamCreateWithFlags(&s, cudaStreamNonBlocking) != cudaSuccess) {
+        cudaGetLastError();
+        return;
+    }
+    static const unsigned int mark = LQCD_P2P_POISON;
+    auto put = [&](unsigned int* w) { cudaMemcpyAsync(w, &mark, sizeof(mark), cudaMemcpyDefault, s); };
+    for (int g = 0; g < 2; ++g) {
+        if (t->win[t->dn()]) put(&t->hdr(t->dn())->arrived[1][g]);
+        if (t->win[t->up()]) put(&t->hdr(t->up())->arrived[0][g]);
+        for (int r = 0; r < t->nranks; ++r)
+            if (t->win[r]) put(&t->hdr(r)->red_arrived[g][t->rank]);
+        if (self) {
+            put(&t->mine()->arrived[0][g]);
+            put(&t->mine()->arrived[1][g]);
+            for (int r = 0; r < t->nranks; ++r) put(&t->mine()->red_arrived[g][r]);
+        }
+    }
+    cudaStreamSynchronize(s);
+    cudaStreamDestroy(s);
+    cudaGetLastError();
 }
 
 inline void destroy(Transport* t) {
@@ -209,6 +273,11 @@ __global__ void p2p_signal_kernel(unsigned int* a, unsigned int* b) {
     *(volatile unsigned int*)a = 1u;
     *(volatile unsigned int*)b = 1u;
 }
+// the two arrival words back to 0 for their next use, except a word that holds the mark of a rank that gave up
+__global__ void p2p_clear_kernel(unsigned int* a, unsigned int* b) {
+    unsigned int* w = threadIdx.x ? b : a;
+    if (*(volatile unsigned int*)w != LQCD_P2P_POISON) *w = 0u;
+}
 inline int signal_wait(Transport* t, cudaStream_t stream, bool clear = true) {
     const unsigned int g = t->seq & 1;
     CUstream cs = (CUstream)stream;
@@ -227,8 +296,10 @@ inline int signal_wait(Transport* t, cudaStream_t stream, bool clear = true) {
     }
     for (int side = 0; side < 2; ++side)
         if (t->wait32(cs, dptr(mine[side]), 1u, CU_STREAM_WAIT_VALUE_GEQ) != CUDA_SUCCESS) return fail(t, "cuStreamWaitValue32 failed");
-    for (int side = 0; clear && side < 2; ++side)
-        if (t->write32(cs, dptr(mine[side]), 0u, CU_STREAM_WRITE_VALUE_DEFAULT) != CUDA_SUCCESS) return fail(t, "cuStreamWriteValue32 failed");
+    if (clear) {
+        p2p_clear_kernel<<<1, 2, 0, stream>>>(mine[0], mine[1]);
+        if (cudaGetLastError() != cudaSuccess) return fail(t, "clearing the arrival words failed");
+    }
     return 0;
 }
 
@@ -236,6 +307,7 @@ inline int signal_wait(Transport* t, cudaStream_t stream, bool clear = true) {
 inline int exchange(void* user, const void* send_lo, const void* send_hi, void* recv_lo, void* recv_hi, size_t bytes,
                     void* stream) {
     Transport* t = (Transport*)user;
+    if (t->dead) return -1;
     if (!t->active) return fail(t, "transport not connected");
     if (bytes > t->cap) return fail(t, "message larger than a face buffer of the window");
     cudaStream_t s = (cudaStream_t)stream;
@@ -279,11 +351,12 @@ __global__ void __launch_bounds__(32) p2p_sum_kernel(const double* slots, unsign
         for (int r = 0; r < nranks; ++r) acc += __ldcv(slots + r * RED_MAX + j);
         out[j] = acc;
     }
-    if (j < nranks) flags[j] = 0u;
+    if (j < nranks && *(volatile unsigned int*)(flags + j) != LQCD_P2P_POISON) flags[j] = 0u;   // the mark of a rank that gave up stays
 }
 
 inline int allreduce_sum(void* user, double* dev_buf, int n, void* stream) {
     Transport* t = (Transport*)user;
+    if (t->dead) return -1;
     if (!t->active) return fail(t, "transport not connected");
     if (n < 1 || n > RED_MAX) return fail(t, "all-reduce of more values than a slot holds");
     cudaStream_t s = (cudaStream_t)stream;

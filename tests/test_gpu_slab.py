@@ -266,6 +266,38 @@ def test_four_ranks_share_the_gpu_over_peer_memory():
     _run_ranks(4, (4, 4, 4, 8), "p2p", timeout=300)     # two time slices per rank: no interior, four-way all-reduce
 
 
+@pytest.mark.parametrize("mode,world", [("abort", 2), ("abort", 3), ("late", 2)])
+def test_a_rank_that_stops_does_not_hang_the_others(mode, world):
+    """Peer-memory transport: the ranks wait for each other with stream operations on flag words, so a rank that stops
+    calling would leave the others waiting for ever.  The last rank sets up, takes part in one solve, then either calls
+    lqcd_comm_abort or just stays away (tests/_slab_abort_worker.py).  Every other rank -- with three ranks also the
+    one that is not the quitter's... every rank is a neighbour on a ring of three, but rank 0 and 1 also wait for each
+    other -- must return LQCD_ECOMM from its solve in bounded time (at once after an abort, after
+    LQCD_OPT_COMM_TIMEOUT = 3 s for a silent peer), must get LQCD_ECOMM again at once from the next call, and its
+    streams must drain."""
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", str(world),
+           "--master-addr", "127.0.0.1", "--master-port", str(_free_port()),
+           os.path.join("tests", "_slab_abort_worker.py"), mode]
+    proc = subprocess.Popen(cmd, cwd=ROOT, env=dict(os.environ, OMP_NUM_THREADS="4"), stdout=subprocess.PIPE,
+                            stderr=subprocess.PIPE, text=True, start_new_session=True)
+    try:
+        stdout, stderr = proc.communicate(timeout=240)
+    except subprocess.TimeoutExpired:
+        os.killpg(proc.pid, signal.SIGKILL)
+        stdout, stderr = proc.communicate()
+        raise AssertionError(f"{mode}: the ranks hung\n" + stdout[-2000:] + stderr[-3000:])
+    assert proc.returncode == 0, stdout[-2000:] + stderr[-3000:]
+    line = [l for l in stdout.splitlines() if l.startswith("RESULT ")]
+    assert len(line) == 1, stdout[-2000:]
+    res = json.loads(line[0][7:])
+    assert len(res) == world
+    for r in res[:-1]:
+        assert r["codes"] == [-8, -8], res                        # LQCD_ECOMM, twice
+        assert r["seconds"] < (30.0 if mode == "late" else 20.0), res
+        if mode == "late":
+            assert r["seconds"] >= 2.5 and "LQCD_OPT_COMM_TIMEOUT" in r["text"], res
+
+
 @pytest.mark.parametrize("comm", ["nccl", "p2p"])
 @pytest.mark.parametrize("world,L", [(2, (8, 8, 8, 8)), (4, (4, 6, 8, 16))])
 def test_ranks_on_their_own_gpus_over_nccl(world, L, comm):
