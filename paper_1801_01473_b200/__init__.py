@@ -13,7 +13,7 @@ from .binding import (  # noqa: F401
     LQCD_OPT_MASS, LQCD_OPT_ANTIPERIODIC_T, LQCD_OPT_RECON, LQCD_OPT_MAX_ITER, LQCD_OPT_CHECK_EVERY,
     LQCD_OPT_USE_GRAPH, LQCD_OPT_LINK_PRECISIONS, LQCD_OPT_SHIFT_BLOCK, LQCD_OPT_PERSISTENT, LQCD_PREC_F64, LQCD_PREC_F32,
     LQCD_STAT_ITERS, LQCD_STAT_REL_RES, LQCD_STAT_FREEZE_ITER, LQCD_STAT_BASE_SHIFT, LQCD_STAT_GPU_LAUNCHES,
-    LQCD_STAT_SOLVE_MS, LQCD_STAT_RELIABLE_UPDATES, LQCD_STAT_GRAPH_REPLAYS,
+    LQCD_STAT_SOLVE_MS, LQCD_STAT_RELIABLE_UPDATES, LQCD_STAT_GRAPH_REPLAYS, LQCD_STAT_SOLVER_PATH,
     LqcdError, Lattice, load_library, library_path, EXPORTS,
     lqcd_create, lqcd_destroy, lqcd_set_stream, lqcd_set_option, lqcd_get_option, lqcd_workspace_bytes,
     lqcd_set_workspace, lqcd_set_gauge, lqcd_set_gauge_host, lqcd_set_u1_phases, lqcd_set_u1_phases_host, lqcd_doe, lqcd_deo, lqcd_doe_host, lqcd_deo_host,

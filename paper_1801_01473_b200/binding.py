@@ -675,6 +675,7 @@ class Lattice:
             base_shift=int(self.stat(LQCD_STAT_BASE_SHIFT)),
             solve_ms=self.stat(LQCD_STAT_SOLVE_MS),
             graph_replays=int(self.stat(LQCD_STAT_GRAPH_REPLAYS)),
+            solver_path=int(self.stat(LQCD_STAT_SOLVER_PATH)),
         )
 
     def rational_apply(self, b_even, alpha0: float, alpha: Sequence[float], shifts: Sequence[float], tol: float,

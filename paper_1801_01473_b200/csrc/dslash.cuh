@@ -498,8 +498,12 @@ __device__ __forceinline__ K2Coef<T> k2_coef_from_state(const CgState* st, const
 // scalar it needs -- K2: a = |r|^2 / <p,Ap>;  K1: beta = |r_new|^2 / |r|^2 and the stop decision -- while the extra block
 // runs the scalar step proper on the device state (zeta_i, block coefficients, freeze flags) for everybody else's
 // later use.  The fields the sweeping blocks read (rr, b_prev in K2; rr_keep, iter_keep in K1) are not written by the
-// scalar step that runs beside them.  The step after K2 of the last iteration of a block (and of a batch) is run by
-// cg_reduce_scalar_kernel before the block sweep; K1 of the next iteration is then launched with pending = 0.
+// scalar step that runs beside them.  `stop` IS written beside them (after K2's sum: when the solve is over; after
+// K1's: on a breakdown), so a block does not let each thread read it: thread 0 reads it once and the block decides as
+// one (threads that disagreed would leave some of them out of the sum below).  Blocks may still read different values;
+// those that read 0 reach, from the sum, the decision the scalar step reached (the returns below).  The step after K2
+// of the last iteration of a block (and of a batch) is run by cg_reduce_scalar_kernel before the block sweep; K1 of the
+// next iteration is then launched with pending = 0.
 template <typename T, int RECON, int EPI, int U1, int SLAB = 0, int FS = 0>
 __global__ void __launch_bounds__(DS_BLOCK, (DsOcc<T, EPI>::minb)) dslash_kernel(const DslashArgs<T> A) {
     constexpr bool FLY = (EPI == 4);
@@ -521,9 +525,13 @@ __global__ void __launch_bounds__(DS_BLOCK, (DsOcc<T, EPI>::minb)) dslash_kernel
     double a_fs = 0.0, beta_fs = 0.0;
     if (FS) {
         __shared__ double redf[32];
+        __shared__ int stop_sh;
+        if (threadIdx.x == 0) stop_sh = A.check_stop ? A.st->stop : 0;
         const bool have = (EPI == 5) || A.pending;
         double sum_in = 0.0;
-        if (have) sum_in = broadcast0(final_sum<DS_BLOCK>(A.red_in, A.red_n, redf), redf);
+        if (have) sum_in = broadcast0(final_sum<DS_BLOCK>(A.red_in, A.red_n, redf), redf);   // barriers inside
+        else __syncthreads();
+        if (stop_sh) return;                     // iterations launched beyond the one that converged
         if (blockIdx.x == gridDim.x - 1) {       // the block that owns no sites
             if (have) {
                 if (EPI == 5) cg_scalars_after_pAp(A.st, sum_in);

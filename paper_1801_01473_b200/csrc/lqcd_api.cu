@@ -126,6 +126,7 @@ struct lqcd_ctx {
     float last_ms;
     int last_updates;        // reliable updates of the last mixed-precision solve
     int last_replays;        // CUDA-graph replays of the last solve (0: launched plainly, or the persistent kernel)
+    int last_path;           // LQCD_STAT_SOLVER_PATH of the last solve
     long long launches;
 
     char err[256];
@@ -534,6 +535,7 @@ int slab_reduce_step(lqcd_ctx* c, int n, int which, double tol, int check_stop) 
     int rc;
     if (which != 0 && c->p2p.active && c->comm.user == (void*)&c->p2p) {
         lqcd_p2p::Transport* t = &c->p2p;
+        if (t->dead) return fail(c, LQCD_ECOMM, "peer-memory transport has failed: %s", t->error);
         sum_partials_kernel<<<1, CG_BLOCK, 0, c->stream>>>(c->partials, n, c->red, c->st_dev, check_stop, lqcd_p2p::reduce_begin(t));
         if (lqcd_p2p::reduce_wait(t, c->stream)) return fail(c, LQCD_ECOMM, "peer-memory transport: %s", t->error);
         cg_scalar_slots_kernel<<<1, 64, 0, c->stream>>>(c->st_dev, lqcd_p2p::reduce_slots(t), lqcd_p2p::reduce_flags(t),
@@ -1519,7 +1521,28 @@ int solve_impl(lqcd_ctx* c, const T* b_even, const double* shifts, int nshift, d
     CU(cudaGetLastError());
 
     const int ce = check_every(c);
-    const bool persistent = use_persistent<T>(c);
+    bool persistent = use_persistent<T>(c);
+    if (c->persistent_opt == 1 && !persistent)
+        return fail(c, LQCD_EINVAL, "LQCD_OPT_PERSISTENT = 1, but the persistent kernel cannot run this solve (%s)",
+                    c->slab ? "slab context" : !c->coop_launch ? "no cooperative launches on this device"
+                                                               : "LQCD_OPT_SHIFT_BLOCK above 16");
+    c->flag_host[0] = c->flag_host[1] = 0;
+    c->last_replays = 0;
+    bool done = false;
+    if (persistent) {
+        // one cooperative kernel runs the iterations until the device-side stop (persist.cuh)
+        rc = launch_persistent<T>(c);
+        if (rc == LQCD_OK) {
+            done = true;
+        } else if (c->persistent_opt == 1) {
+            return rc;
+        } else {
+            // the library chose this driver and the launch was refused (fewer blocks can be resident than the occupancy
+            // query said: another context or MPS client on the device): nothing has run, take the other driver
+            cudaGetLastError();
+            persistent = false;
+        }
+    }
     // the legacy default stream cannot be captured: plain launches there
     // Slabs: a replayed graph does not keep the priority of the communication stream, so the border launches queue
     // behind the interior again; measured on one rank over NCCL, graph against plain launches, us per iteration:
@@ -1529,14 +1552,7 @@ int solve_impl(lqcd_ctx* c, const T* b_even, const double* shifts, int nshift, d
     if (use_graph && (B.graph_iters != ce || B.graph_block != m)) {
         if ((rc = build_graph<T>(c, ce, rational))) return rc;
     }
-    c->flag_host[0] = c->flag_host[1] = 0;
-    c->last_replays = 0;
-    bool done = false;
-    if (persistent) {
-        // one cooperative kernel runs the iterations until the device-side stop (persist.cuh)
-        if ((rc = launch_persistent<T>(c))) return rc;
-        done = true;
-    }
+    c->last_path = persistent ? 2 : use_graph ? 1 : 0;
     // MAX_ITER is reached inside batch number ceil(MAX_ITER / ce) at the latest: nothing is launched beyond it (the
     // kernels of a launch whose solve is over return at once, but 2 x 20,000 empty blocks per iteration are not free)
     const long max_batches = ((long)c->max_iter + ce - 1) / ce;
@@ -1589,6 +1605,9 @@ int solve_impl(lqcd_ctx* c, const T* b_even, const double* shifts, int nshift, d
     c->last_nshift = nshift;
     c->last_rel = (h->bb > 0.0) ? std::sqrt(h->rr / h->bb) : 0.0;
     for (int i = 0; i < nshift; ++i) c->last_freeze[i] = h->active[i] ? h->iter : h->freeze_iter[i];
+    if (h->status == LQCD_ECOMM)
+        return fail(c, LQCD_ECOMM, "peer-memory transport: a peer rank gave up during the solve (iteration %d); the context "
+                    "can only be destroyed", h->iter);
     if (!h->stop) return fail(c, LQCD_ECUDA, "solver loop ended without the device raising its stop flag");
     if (h->status == LQCD_EBREAKDOWN) return fail(c, LQCD_EBREAKDOWN, "<p,Ap> = %g at iteration %d", h->pAp, h->iter);
     if (h->status == LQCD_ENOCONV)
@@ -1962,6 +1981,7 @@ int lqcd_get_stat(const lqcd_ctx* c, int key, int idx, double* out) {
         case LQCD_STAT_SOLVE_MS: *out = c->last_ms; break;
         case LQCD_STAT_RELIABLE_UPDATES: *out = c->last_updates; break;
         case LQCD_STAT_GRAPH_REPLAYS: *out = c->last_replays; break;
+        case LQCD_STAT_SOLVER_PATH: *out = c->last_path; break;
         default: return LQCD_EINVAL;
     }
     return LQCD_OK;

@@ -76,7 +76,7 @@ def test_u1_dslash_48(lq, big, recon):
 
 
 def test_rational_apply_fixed_count_48(lq, big):
-    L, cfg, n_it = big.L, big.cfg, 20
+    L, cfg, n_it = big.L, big.cfg, 40        # a whole shift block of 32, then a short one
     rng = np.random.default_rng(7)
     n = len(cfg["shifts"])
     alpha = list(rng.uniform(0.05, 1.5, n) * rng.choice([-1.0, 1.0], n))
@@ -96,10 +96,10 @@ def test_rational_apply_fixed_count_48(lq, big):
 @pytest.mark.parametrize("comm", ["nccl", "p2p"])
 def test_slab_one_rank_48(lq, big, comm):
     """One rank of the slab path at the size bench.py times it, over either transport: the operator bit-identical to
-    the whole-lattice kernel and within 1e-12 of the oracle; 20 iterations of the fused CG iteration on the slab (p
+    the whole-lattice kernel and within 1e-12 of the oracle; 40 iterations of the fused CG iteration on the slab (p
     faces formed by their owner, interior + border launches, reductions through the transport) at a fixed count
     against the oracle, <= 1e-11 as on the whole lattice."""
-    L, cfg, n_it = big.L, big.cfg, 20
+    L, cfg, n_it = big.L, big.cfg, 40        # a whole shift block of 32, then a short one
     whole = lq.Lattice(L)
     whole.set_gauge(big.U)
     slab = lq.Lattice(L, mass=cfg["mass"], slab=(0, 1), comm=comm)
@@ -126,17 +126,17 @@ _CG20 = {}
 
 
 def _oracle_cg20(big):
-    """20 iterations of the oracle's multi-shift CG on config 4 at a fixed count (computed once per module)"""
+    """40 iterations of the oracle's multi-shift CG on config 4 at a fixed count (computed once per module)"""
     if "r" not in _CG20:
         cfg = big.cfg
-        _CG20["r"] = oracle.mshift_cg(big.L, big.Uh, cfg["mass"], big.b_aos, cfg["shifts"], 1e-30, max_iter=20)
+        _CG20["r"] = oracle.mshift_cg(big.L, big.Uh, cfg["mass"], big.b_aos, cfg["shifts"], 1e-30, max_iter=40)
     return _CG20["r"]
 
 
 def test_f32_cg_fixed_count_48(lq, big):
     """The oracle (fp64) sees the float-rounded links and source, so every difference is float arithmetic in the
-    kernels: 20 iterations x (24 + few) eps32 per iteration, bound 2e-5 as at 8^4 (test_gpu_f32.py)."""
-    L, cfg, n_it = big.L, big.cfg, 20
+    kernels: 40 iterations x (24 + few) eps32 per iteration, bound 2e-5 as at 8^4 (test_gpu_f32.py)."""
+    L, cfg, n_it = big.L, big.cfg, 40        # a whole shift block of 32, then a short one
     lat = lq.Lattice(L, mass=cfg["mass"], precisions=lq.LQCD_PREC_F32)
     lat.set_gauge(big.U)
     b32 = big.b.float()

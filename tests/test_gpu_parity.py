@@ -105,16 +105,25 @@ def oracle_iteration_band(L, U, mass, b_aos, shifts, tol, n_ref, trials):
     return min(counts), max(counts)
 
 
+_ORACLE_SOLVES = {}      # run_cg_both(keep_oracle=True): the oracle's solve of a long case, shared by its parametrizations
+
+
 def run_cg_both(lq, L, mass, shifts, tol, recon=18, use_graph=True, stream=None, max_iter=None, host=False,
-                check_every=None, band_trials=3):
+                check_every=None, band_trials=3, keep_oracle=False):
     U, f = make_inputs(L)
     b_soa, b_aos = oracle_parity_vector(L, f.numpy(), 0)
     kw = {} if max_iter is None else dict(max_iter=max_iter)
-    x_ref, info_ref = oracle.mshift_cg(L, U.numpy(), mass, b_aos, shifts, tol, **kw)
-    if max_iter is None and info_ref["iters"] > 300:
-        info_ref["band"] = oracle_iteration_band(L, U.numpy(), mass, b_aos, shifts, tol, info_ref["iters"], band_trials)
+    key = (tuple(L), mass, tuple(shifts), tol, max_iter, band_trials)
+    if keep_oracle and key in _ORACLE_SOLVES:
+        x_ref, info_ref = _ORACLE_SOLVES[key]
     else:
-        info_ref["band"] = (info_ref["iters"], info_ref["iters"])
+        x_ref, info_ref = oracle.mshift_cg(L, U.numpy(), mass, b_aos, shifts, tol, **kw)
+        if max_iter is None and info_ref["iters"] > 300:
+            info_ref["band"] = oracle_iteration_band(L, U.numpy(), mass, b_aos, shifts, tol, info_ref["iters"], band_trials)
+        else:
+            info_ref["band"] = (info_ref["iters"], info_ref["iters"])
+        if keep_oracle:
+            _ORACLE_SOLVES[key] = (x_ref, info_ref)
     lat = lq.Lattice(L, mass=mass, recon=recon)
     lat.set_option(lq.LQCD_OPT_USE_GRAPH, 1 if use_graph else 0)
     if max_iter is not None:
@@ -172,17 +181,22 @@ def test_mshift_cg_small(lq, L, mass, shifts, mode, solver_path):
     check_cg(x, info, x_ref, info_ref, shifts)
     if solver_path == "launches":
         assert launches >= 2 * info["iters"] + 2      # two launches per iteration (K1, K2 of cg.cuh) + init + sweeps
+        assert info["solver_path"] == (1 if mode in ("graph", "recon12", "host") else 0)
     else:
         assert launches <= 8                          # links, pack, |b|^2 + ONE kernel for all iterations
+        assert info["solver_path"] == 2
 
 
 @both_solvers
-def test_mshift_cg_config2_16x4(lq, solver_path):
-    """BASELINE config 2: 16^4, m = 0.01, 8 shifts 1e-4*10^(i/2), tol 1e-10 -- full solve on both sides."""
+@pytest.mark.parametrize("recon", [18, 12])
+def test_mshift_cg_config2_16x4(lq, solver_path, recon):
+    """BASELINE config 2: 16^4, m = 0.01, 8 shifts 1e-4*10^(i/2), tol 1e-10 -- full solve on both sides, with full
+    and with two-row links (16^4 with two-row links is the case the library itself gives to the persistent kernel)."""
     cfg = gen.CONFIGS["config2_16^4"]
-    x, info, x_ref, info_ref, _ = run_cg_both(lq, cfg["L"], cfg["mass"], cfg["shifts"], cfg["tol"],
-                                              stream=torch.cuda.Stream(), band_trials=1)
+    x, info, x_ref, info_ref, _ = run_cg_both(lq, cfg["L"], cfg["mass"], cfg["shifts"], cfg["tol"], recon=recon,
+                                              stream=torch.cuda.Stream(), band_trials=1, keep_oracle=True)
     assert info["status"] == 0 and info_ref["status"] == 0
+    assert info["solver_path"] == (2 if solver_path == "persistent" else 1)      # the driver asked for is the one that ran
     print("config 2: GPU iterations", info["iters"], "oracle", info_ref["iters"], "oracle band", info_ref["band"],
           "freeze", info["freeze_iter"], info_ref["freeze_iter"])
     check_cg(x, info, x_ref, info_ref, cfg["shifts"])
@@ -474,9 +488,11 @@ def large_config_protocol(lq, name, n_it, residual_shifts):
 
 def test_mshift_cg_config4_48x4(lq):
     """BASELINE config 4: 48^4, 16 shifts 1e-5..1, m = 0.0075, tol 1e-10."""
-    large_config_protocol(lq, "config4_48^4", n_it=20, residual_shifts=(0, 7, 15))      # one whole shift block + 4
+    # shift blocks are 32 iterations long here: 68 = the first sweep (iteration 32), a middle one (64: all residuals of
+    # the block, p_i read and stored -- the sweep a real solve runs a hundred times) and a short closing one (68)
+    large_config_protocol(lq, "config4_48^4", n_it=68, residual_shifts=(0, 7, 15))
 
 
 def test_mshift_cg_config5_64x4(lq):
     """BASELINE config 5: 64^4 (16.8M sites, 9.7 GB of links), 16 shifts, m = 0.005, tol 1e-10."""
-    large_config_protocol(lq, "config5_64^4", n_it=8, residual_shifts=(0, 15))
+    large_config_protocol(lq, "config5_64^4", n_it=34, residual_shifts=(0, 15))         # one whole block of 32 + 2

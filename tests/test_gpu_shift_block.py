@@ -109,7 +109,7 @@ def test_stop_in_the_middle_of_a_block(lq, n_iter, solver_path):
     lat = lq.Lattice(L, mass=mass)
     lat.set_gauge(U.cuda())
     b = cuda(b_soa)
-    for m in (1, 5, 8, 16, 32):
+    for m in ((1, 5, 8, 16) if solver_path == "persistent" else (1, 5, 8, 16, 32)):     # the persistent kernel: m <= 16
         x, info = solve(lq, lat, b, shifts, 1e-30, m, max_iter=n_iter)
         assert info["status"] == lq.LQCD_ENOCONV and info["iters"] == n_iter == info_ref["iters"]
         for i in range(16):
@@ -146,6 +146,8 @@ def test_freeze_in_the_middle_of_a_block(lq, solver_path):
 @both_solvers
 @pytest.mark.parametrize("m", [1, 4, 7, 16, 32])
 def test_rational_sum_with_blocks(lq, m, solver_path):
+    if solver_path == "persistent" and m > 16:
+        pytest.skip("the persistent kernel handles blocks of up to 16 iterations (test_persistent_option_is_strict)")
     L, mass = (8, 8, 8, 8), 0.01
     shifts = [1e-4 * 10 ** (i / 2) for i in range(8)]
     a0, al = rational_coefficients(len(shifts))
@@ -199,4 +201,35 @@ def test_single_precision_with_blocks(lq, solver_path):
             # 20 iterations x (24 + few) eps32 per iteration, as in test_gpu_f32.py
             assert rel_l2(oracle.soa_to_aos(x[i].double().cpu().numpy()), x_ref[i]) <= 2e-5, (m, i)
     assert len({res[m]["rel_res"] for m in blocks}) == 1
+    lat.close()
+
+
+def test_persistent_option_is_strict(lq):
+    """LQCD_OPT_PERSISTENT = 1 means the persistent kernel or an error, never a silent change of driver; -1 and 0 say
+    through LQCD_STAT_SOLVER_PATH which driver ran."""
+    L, mass, shifts = (8, 8, 8, 8), 0.05, [0.01, 0.1]
+    U, f = make_inputs(L)
+    b = cuda(oracle_parity_vector(L, f.numpy(), 0)[0])
+    lat = lq.Lattice(L, mass=mass)
+    lat.set_gauge(U.cuda())
+    with torch.cuda.stream(torch.cuda.Stream()):
+        lat.set_option(lq.LQCD_OPT_PERSISTENT, 1)
+        lat.set_option(lq.LQCD_OPT_SHIFT_BLOCK, 32)
+        with pytest.raises(lq.LqcdError) as e:
+            lat.mshift_cg(b, shifts, 1e-10)
+        assert e.value.code == lq.LQCD_EINVAL and "SHIFT_BLOCK" in str(e.value)
+        lat.set_option(lq.LQCD_OPT_SHIFT_BLOCK, 16)
+        x2, info2 = lat.mshift_cg(b, shifts, 1e-10)
+        assert info2["solver_path"] == 2
+        lat.set_option(lq.LQCD_OPT_PERSISTENT, 0)
+        x1, info1 = lat.mshift_cg(b, shifts, 1e-10)
+        assert info1["solver_path"] == 1 and info1["graph_replays"] >= 1
+        lat.set_option(lq.LQCD_OPT_USE_GRAPH, 0)
+        x0, info0 = lat.mshift_cg(b, shifts, 1e-10)
+        assert info0["solver_path"] == 0 and info0["graph_replays"] == 0
+    torch.cuda.synchronize()
+    assert info0["iters"] == info1["iters"] and abs(info2["iters"] - info1["iters"]) <= 1
+    for i in range(len(shifts)):
+        assert rel_l2(x0[i].cpu().numpy(), x1[i].cpu().numpy()) <= 1e-12
+        assert rel_l2(x2[i].cpu().numpy(), x1[i].cpu().numpy()) <= 1e-10
     lat.close()
